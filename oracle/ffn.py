@@ -1,0 +1,71 @@
+"""MoE FFN computed from each layout, for the equivalence the paper states.  TEST INFRASTRUCTURE.
+
+PAPER.md:46: the transformation produces "outputs equivalent to those the destination layout
+would produce"; SwiGLU MLP with gate and up projections and a down projection;
+PAPER.md:17: TP "synchronizes partial results with ... All-Reduce" (a sum of rank partials), EP
+routes each token to the rank owning its expert.
+
+y[t] = sum_k p[t,k] * ( silu(x[t] @ gate[e]) * (x[t] @ up[e]) ) @ down[e],  e = topk[t,k]
+gate, up: [E, H, I]; down: [E, I, H].  Arithmetic in the dtype of the inputs (fp32 in the test;
+fp64 for the dense reference).
+"""
+from __future__ import annotations
+
+import numpy as np
+
+
+def silu(a):
+    return a / (1.0 + np.exp(-a))
+
+
+def route_top2(logits: np.ndarray):
+    """Reading of SURVEY.md §8(c): softmax -> top-2 -> renormalise.  Both layouts share it."""
+    z = logits - logits.max(axis=1, keepdims=True)
+    p = np.exp(z)
+    p /= p.sum(axis=1, keepdims=True)
+    idx = np.argsort(-p, axis=1, kind="stable")[:, :2]
+    w = np.take_along_axis(p, idx, axis=1)
+    w = w / w.sum(axis=1, keepdims=True)
+    return idx, w
+
+
+def moe_ffn_dense(x, gate, up, down, idx, w):
+    y = np.zeros((x.shape[0], down.shape[2]), dtype=x.dtype)
+    for t in range(x.shape[0]):
+        for k in range(idx.shape[1]):
+            e = idx[t, k]
+            a = silu(x[t] @ gate[e]) * (x[t] @ up[e])
+            y[t] += w[t, k] * (a @ down[e])
+    return y
+
+
+def moe_ffn_tp(x, gate_tp, up_tp, down_tp, idx, w):
+    """gate_tp[r]: [E,H,I/R], up_tp[r] likewise, down_tp[r]: [E,I/R,H]; y = sum over ranks of the
+    partial each rank computes from its shards alone (the All-Reduce)."""
+    R = len(gate_tp)
+    y = np.zeros((x.shape[0], down_tp[0].shape[2]), dtype=x.dtype)
+    for r in range(R):
+        part = np.zeros_like(y)
+        for t in range(x.shape[0]):
+            for k in range(idx.shape[1]):
+                e = idx[t, k]
+                a = silu(x[t] @ gate_tp[r][e]) * (x[t] @ up_tp[r][e])
+                part[t] += w[t, k] * (a @ down_tp[r][e])
+        y += part
+    return y
+
+
+def moe_ffn_ep(x, gate_ep, up_ep, down_ep, idx, w):
+    """gate_ep[r]: [E/R,H,I] etc.; the token goes to the rank owning expert e = idx, which holds
+    it whole at local index e mod (E/R)."""
+    R = len(gate_ep)
+    n_loc = gate_ep[0].shape[0]
+    y = np.zeros((x.shape[0], down_ep[0].shape[2]), dtype=x.dtype)
+    for t in range(x.shape[0]):
+        for k in range(idx.shape[1]):
+            e = int(idx[t, k])
+            r, el = e // n_loc, e % n_loc
+            assert r < R
+            a = silu(x[t] @ gate_ep[r][el]) * (x[t] @ up_ep[r][el])
+            y[t] += w[t, k] * (a @ down_ep[r][el])
+    return y

@@ -1,0 +1,116 @@
+"""Seeded random draws.  No layout / partition / allocation arithmetic lives here."""
+from __future__ import annotations
+
+import numpy as np
+
+from .configs import Config
+
+
+def bf16_bits_from_f32(x: np.ndarray) -> np.ndarray:
+    """Round-to-nearest-even fp32 -> bf16, returned as uint16 bit patterns (numpy has no bf16)."""
+    u = np.ascontiguousarray(x, dtype=np.float32).view(np.uint32)
+    rounded = u + (np.uint32(0x7FFF) + ((u >> np.uint32(16)) & np.uint32(1)))
+    return (rounded >> np.uint32(16)).astype(np.uint16)
+
+
+def _np_dtype(w_dtype: str):
+    return {"bf16": np.uint16, "fp32": np.float32, "fp8_e4m3_b128": np.uint8}[w_dtype]
+
+
+def tag_fill_u16(shape, salt: int) -> np.ndarray:
+    """Coordinate-tag fill: element value = 16-bit hash of (salt, flat logical index).
+
+    Random bf16 values repeat; a tag makes a misplaced element visible."""
+    n = int(np.prod(shape))
+    idx = np.arange(n, dtype=np.uint64)
+    off = np.uint64((int(salt) * 0x9E3779B97F4A7C15) & 0xFFFFFFFFFFFFFFFF)
+    with np.errstate(over="ignore"):
+        h = idx + off
+        h ^= h >> np.uint64(33)
+        h = h * np.uint64(0xFF51AFD7ED558CCD)
+        h ^= h >> np.uint64(29)
+    return (h & np.uint64(0xFFFF)).astype(np.uint16).reshape(shape)
+
+
+def gen_logical_weight(cfg: Config, layer: int, kind: str, fill: str = "normal") -> np.ndarray:
+    """Logical expert tensor of one layer: gate/up [E,H,I], down [E,I,H] (BASELINE.json orientation).
+
+    bf16 -> uint16 bit patterns of N(0, 0.02); fp32 -> float32 N(0, 0.02); fp8 -> uint8 bytes
+    (opaque e4m3 codes, uniform over 0..255 minus the two NaN codes)."""
+    m = {"gate": 0, "up": 1, "down": 2}[kind]
+    shape = (cfg.E, cfg.H, cfg.I) if m < 2 else (cfg.E, cfg.I, cfg.H)
+    seed = (cfg.seed, 2000 + layer, m)
+    if fill == "tag":
+        t = tag_fill_u16(shape, salt=cfg.seed * 1000 + layer * 3 + m)
+        if cfg.w_dtype == "bf16":
+            return t
+        if cfg.w_dtype == "fp8_e4m3_b128":
+            return (t & 0xFF).astype(np.uint8)
+        return t.astype(np.float32)
+    rng = np.random.default_rng(seed)
+    if cfg.w_dtype == "fp8_e4m3_b128":
+        b = rng.integers(0, 256, size=shape, dtype=np.uint8)
+        b[(b & 0x7F) == 0x7F] = 0x38  # avoid NaN codes; bytes are opaque to the reshard anyway
+        return b
+    x = rng.normal(0.0, 0.02, size=shape).astype(np.float32)
+    return x if cfg.w_dtype == "fp32" else bf16_bits_from_f32(x)
+
+
+def gen_logical_scale(cfg: Config, layer: int, kind: str) -> np.ndarray:
+    """fp32 per-128x128-block scales: gate/up [E, H/128, I/128], down [E, I/128, H/128]."""
+    m = {"gate": 0, "up": 1, "down": 2}[kind]
+    shape = ((cfg.E, cfg.H // 128, cfg.I // 128) if m < 2 else (cfg.E, cfg.I // 128, cfg.H // 128))
+    rng = np.random.default_rng((cfg.seed, 2500 + layer, m))
+    return rng.uniform(0.5, 2.0, size=shape).astype(np.float32)
+
+
+def draw_seq_lens(cfg: Config, n_req: int | None = None) -> np.ndarray:
+    """Request lengths in tokens (int32), numpy.random.default_rng(cfg.seed)."""
+    n = cfg.n_req if n_req is None else n_req
+    rng = np.random.default_rng(cfg.seed)
+    d = cfg.len_dist
+    if d[0] == "uniform":
+        x = rng.integers(d[1], d[2] + 1, size=n)
+    elif d[0] == "lognormal":
+        x = np.rint(rng.lognormal(np.log(d[1]), d[2], size=n))
+        x = np.clip(x, 1, d[3])
+    elif d[0] == "geometric":
+        x = np.clip(rng.geometric(1.0 / d[1], size=n), 1, d[2])
+    else:
+        raise ValueError(d)
+    return x.astype(np.int32)
+
+
+def gen_kv_request(cfg: Config, layer: int, kv: int, req: int, length: int,
+                   fill: str = "normal") -> np.ndarray:
+    """K (kv=0) or V (kv=1) of one request in one layer: [len, kv_heads, head_dim] bf16 bits."""
+    shape = (int(length), cfg.kv_heads, cfg.head_dim)
+    if fill == "tag":
+        return tag_fill_u16(shape, salt=cfg.seed * 7919 + (layer * 2 + kv) * 100003 + req)
+    rng = np.random.default_rng((cfg.seed, 3000 + layer, kv, req))
+    return bf16_bits_from_f32(rng.normal(0.0, 1.0, size=shape).astype(np.float32))
+
+
+def random_page_tables(seq_lens, owner, n_ranks: int, n_pages: int, page: int, max_pages: int,
+                       seed: int) -> np.ndarray:
+    """Seeded random injective page assignment (reading A8: pages 'interleave arbitrarily',
+    PAPER.md:122).  `owner[i] < 0` means every rank uses the same table (one shared draw);
+    otherwise pages are drawn per owning rank.  Returns int32 [n, max_pages], -1 padded."""
+    rng = np.random.default_rng(seed)
+    seq_lens = np.asarray(seq_lens)
+    n = len(seq_lens)
+    bt = np.full((n, max_pages), -1, dtype=np.int32)
+    need = (seq_lens + page - 1) // page
+    groups = {}
+    for i in range(n):
+        groups.setdefault(int(owner[i]) if owner is not None else -1, []).append(i)
+    for g, members in sorted(groups.items()):
+        total = int(sum(need[i] for i in members))
+        if total > n_pages:
+            raise ValueError("pool too small for the random source tables")
+        perm = rng.permutation(n_pages)[:total]
+        k = 0
+        for i in members:
+            bt[i, :need[i]] = perm[k:k + need[i]]
+            k += need[i]
+    return bt
