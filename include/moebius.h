@@ -1,0 +1,201 @@
+/*
+ * moebius.h -- C ABI of the B200-native Moebius TP<->EP reshard (arXiv 2606.26607).
+ *
+ * The hot path of the paper on ONE GPU: the single resident copy of the MoE expert weights
+ * (gate/up/down) and of the paged KV cache is moved between the tensor-parallel layout and the
+ * expert-parallel layout at FIXED ADDRESSES (PAPER.md:35, :148-158 §4.2, :160-191 §4.3).  The R
+ * logical ranks are R fixed-address regions of one caller-owned device allocation.
+ *
+ * Conventions
+ *   - extern "C", plain pointers and sizes.  Every pointer is marked HOST or DEVICE below.
+ *   - Every function returns an int status: 0 = MOEBIUS_OK, negative = error.  No exceptions, no
+ *     aborts, no global state.  A failed call leaves the context and all device bytes untouched.
+ *   - The caller owns every device byte and the stream.  The library owns only host objects
+ *     (context, plans).  `moebius_reshard` allocates nothing on host or device (PAPER.md:158:
+ *     "a switch does not allocate dynamic buffers").
+ *   - POD structs carry `struct_size` (set it to sizeof(the struct) before the call).
+ *   - There is no CPU fallback: `moebius_reshard` needs a CUDA device and returns MOEBIUS_E_CUDA
+ *     without one.  The planner entry points are host-only and run anywhere.
+ *
+ * Layouts (PAPER.md:100 §3.1, :116 §3.2; orientation per BASELINE.json, reading A1)
+ *   TP  rank r: gate,up [E, H, I/R] = columns [r*I/R,(r+1)*I/R) of every expert; down [E, I/R, H] =
+ *       the matching rows; K/V pool [pages_tp, page_tokens, hpr, D] with r's KV-head shard of every
+ *       request, one block table shared by all ranks.  Fewer KV heads than ranks: head h is
+ *       replicated on ranks [h*rep, (h+1)*rep), rep = R/kv_heads.
+ *   EP  rank r: gate,up [E/R, H, I], down [E/R, I, H] = experts [r*E/R,(r+1)*E/R) whole; K/V pool
+ *       [pages_ep, page_tokens, kv_heads, D] with all heads of r's own requests.
+ *   Both views of a tensor live in the same rank region.  Weights: a chain of 3L+1 slots per rank,
+ *   object k = 3*layer + {gate:0, up:1, down:2}; the TP view of object k is slot k, the EP view is
+ *   slot k+1 (Fig. 7, at (layer,matrix) grain).  KV: the TP pool and the EP pool of
+ *   a (rank, layer, K|V) alias the same bytes with different page sizes.
+ */
+#ifndef MOEBIUS_H_
+#define MOEBIUS_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define MOEBIUS_API __attribute__((visibility("default")))
+
+typedef enum { MOEBIUS_TP = 0, MOEBIUS_EP = 1 } moebius_mode_t;
+typedef enum { MOEBIUS_BF16 = 0, MOEBIUS_FP32 = 1, MOEBIUS_FP8_E4M3_B128 = 2 } moebius_dtype_t;
+
+/* tensor ids for moebius_view */
+typedef enum {
+  MOEBIUS_T_GATE = 0, MOEBIUS_T_UP = 1, MOEBIUS_T_DOWN = 2,
+  MOEBIUS_T_KPOOL = 3, MOEBIUS_T_VPOOL = 4,
+  MOEBIUS_T_GATE_SCALE = 5, MOEBIUS_T_UP_SCALE = 6, MOEBIUS_T_DOWN_SCALE = 7 /* fp8 only */
+} moebius_tensor_t;
+
+typedef enum {
+  MOEBIUS_OK = 0,
+  MOEBIUS_E_INVAL = -1,    /* bad argument / unsupported shape (reading A3)            */
+  MOEBIUS_E_CAPACITY = -2, /* target mode cannot hold the live requests: cancel the switch
+                                                                               */
+  MOEBIUS_E_STAGING = -3,  /* staging buffer too small for the schedule this request set needs   */
+  MOEBIUS_E_STATE = -4,    /* plan.from != active mode, context not bound, ...                   */
+  MOEBIUS_E_CUDA = -5      /* CUDA runtime error or no device                                    */
+} moebius_status_t;
+
+typedef struct moebius_ctx moebius_ctx_t;   /* opaque, host */
+typedef struct moebius_plan moebius_plan_t; /* opaque, host */
+
+/* All caller-filled.  Symbols as in PAPER.md:100 (P there is R here). */
+typedef struct {
+  uint32_t struct_size;
+  int32_t R, L, E, H, I;      /* E%R==0, I%R==0, (I/R)*elem_bytes % 16 == 0, else MOEBIUS_E_INVAL */
+  int32_t w_dtype;            /* moebius_dtype_t; FP8_E4M3_B128 adds fp32 128x128-block scales    */
+  int32_t w_orient;           /* 0: gate,up [E,H,I], down [E,I,H] (BASELINE.json).  1 (paper's
+                                 W13 [E,2I,H], W2 [E,H,I]) is not implemented: MOEBIUS_E_INVAL    */
+  int32_t kv_heads, head_dim, page_tokens;
+  int32_t kv_dtype;           /* MOEBIUS_BF16 or MOEBIUS_FP32; kv_heads%R==0 or R%kv_heads==0     */
+  int64_t kv_pool_bytes_per_rank_layer; /* capacity of ONE K (or V) pool of one rank and layer; a
+                                 multiple of the EP page size page_tokens*kv_heads*head_dim*b    */
+  int32_t max_requests, max_pages_per_request;
+  int64_t staging_cap_bytes;  /* upper bound for spare weight slot (all ranks) + KV staging, e.g.
+                                 0.024 * resident (reading A12).  0 = no bound.     */
+} moebius_config_t;
+
+/* Sizes the caller must allocate, and where things are.  All byte counts. */
+typedef struct {
+  uint32_t struct_size;
+  int32_t pages_tp, pages_ep;           /* pages per pool in each mode                            */
+  int32_t tp_page_bytes, ep_page_bytes;
+  int64_t base_bytes;                   /* the unified allocation: R rank regions                 */
+  int64_t rank_stride_bytes;            /* rank r's region is [r*stride, (r+1)*stride)            */
+  int64_t weight_slot_bytes;            /* one (layer,matrix) object of one rank                  */
+  int64_t weight_spare_bytes;           /* the spare slot, all ranks                              */
+  int64_t staging_bytes;                /* KV staging buffer to allocate (may be 0)               */
+  int64_t desc_bytes;                   /* device descriptor/work-list buffer                     */
+  int64_t table_bytes;                  /* device block-table buffer                              */
+  int64_t resident_bytes;               /* expert bytes + KV pool capacity, all ranks (cap denominator) */
+  /* block-table buffer layout (int32 units from its start): header[16] = {active mode, n_req,
+     max_requests, max_pages_per_request, 0...}, then owner[max_requests] (-1 = all
+     ranks, TP), seq_lens[max_requests], block_tables[max_requests][max_pages_per_request] (-1 pad) */
+  int32_t tbl_owner_off, tbl_lens_off, tbl_bt_off, tbl_reserved;
+} moebius_layout_t;
+
+/* One dense row-major view; offset in bytes from dev_base; shape/stride in elements. */
+typedef struct {
+  uint32_t struct_size;
+  int32_t ndim, elem_bytes;
+  int64_t offset;
+  int64_t shape[4];
+  int64_t stride[4];
+} moebius_view_t;
+
+/* What one plan moves (reading A15). */
+typedef struct {
+  uint32_t struct_size;
+  int32_t n_segments, n_kv_moves, n_kv_rounds, n_kv_staged, n_pool_groups;
+  int64_t n_units;                       /* work units the kernel executes                        */
+  int64_t w_moved, w_relocated, w_read;  /* expert weights (+ scales): owner-changed / written / read */
+  int64_t kv_moved, kv_relocated, kv_read;
+  int64_t staging_used_bytes;            /* KV staging this plan uses                             */
+  int64_t desc_upload_bytes, table_upload_bytes;
+} moebius_stats_t;
+
+/* ---- context (host only) ------------------------------------------------------------------ */
+
+/* Validates the config and builds the region map ("one large contiguous unified
+ * buffer", views at fixed regions).  cfg: HOST.  out: HOST, receives a new context. */
+MOEBIUS_API int moebius_create(const moebius_config_t* cfg, moebius_ctx_t** out);
+MOEBIUS_API void moebius_destroy(moebius_ctx_t* ctx);
+
+/* Sizes of the four caller-owned device buffers.  out: HOST. */
+MOEBIUS_API int moebius_layout(const moebius_ctx_t* ctx, moebius_layout_t* out);
+
+/* The fixed view of one tensor ("two sets of tensor views ... alias the same
+ * rank-local backing buffer"; :158 "each mode-specific tensor keeps a fixed device-side memory
+ * address").  out: HOST.  Scale tensors: MOEBIUS_E_INVAL unless w_dtype is FP8_E4M3_B128. */
+MOEBIUS_API int moebius_view(const moebius_ctx_t* ctx, moebius_mode_t mode, int rank, int layer,
+                             int tensor_id, moebius_view_t* out);
+
+/* Binds the caller-owned DEVICE buffers (sizes from moebius_layout; all 256-byte aligned); they
+ * stay fixed for the life of the context.  dev_staging may be NULL when staging_bytes == 0.
+ * `initial_mode` says which layout the bytes under dev_base currently hold. */
+MOEBIUS_API int moebius_bind(moebius_ctx_t* ctx, void* dev_base, void* dev_staging, void* dev_desc,
+                             int32_t* dev_tables, moebius_mode_t initial_mode);
+
+MOEBIUS_API int moebius_active_mode(const moebius_ctx_t* ctx); /* moebius_mode_t or negative */
+
+/* ---- planner (host only) ------------------------------------------------------------------ */
+
+/* Emits the work list for one switch (§3): the owner-changed weight slices, the
+ * request ownership under `to` (TP->EP: sort by decreasing length, greedy least-loaded rank,
+ * PAPER.md:124), the target block tables (canonical allocation, reading A7), the KV page
+ * moves with their dependency rounds / staging, and the byte accounting.
+ *   seq_lens          HOST int32[n_req]            tokens per live request (0 = waiting, no KV)
+ *   src_owner         HOST int32[n_req]            EP source only (owner rank), else NULL
+ *   src_block_tables  HOST int32[n_req][max_pages_per_request], -1 padded; pages of the SOURCE
+ *                     mode (TP: shared table; EP: page ids within the owner's pool)
+ *   out               HOST, receives a new plan
+ * MOEBIUS_E_CAPACITY: the target mode cannot hold the requests -- the caller cancels the switch
+ * (PAPER.md:213).  n_req == 0 is the weight-only warm-up switch. */
+MOEBIUS_API int moebius_plan(moebius_ctx_t* ctx, moebius_mode_t from, moebius_mode_t to, int32_t n_req,
+                             const int32_t* seq_lens, const int32_t* src_owner,
+                             const int32_t* src_block_tables, moebius_plan_t** out);
+MOEBIUS_API void moebius_plan_destroy(moebius_plan_t* plan);
+
+/* The request state under the target mode.  dst_owner: HOST int32[n_req] (-1 = all ranks, TP).
+ * dst_block_tables: HOST int32[n_req][max_pages_per_request].  Either may be NULL. */
+MOEBIUS_API int moebius_block_tables(const moebius_plan_t* plan, int32_t* dst_owner,
+                                     int32_t* dst_block_tables);
+
+MOEBIUS_API int moebius_plan_stats(const moebius_plan_t* plan, moebius_stats_t* out);
+
+/* Diagnostic dump of the work list for host-side hazard checking (tests).  what: 0 = segments
+ * (moebius_segment_t-sized records), 1 = KV move descriptors (16 B each), 2 = 2-D
+ * copy descriptors (32 B each).  buf: HOST, cap bytes; *needed receives the full size. */
+MOEBIUS_API int moebius_plan_export(const moebius_plan_t* plan, int what, void* buf, int64_t cap,
+                                    int64_t* needed);
+
+/* ---- execution (needs a CUDA device) ------------------------------------------------------ */
+
+/* Enqueues one switch on `cuda_stream` (a cudaStream_t; NULL = default stream) and returns after
+ * the launch: work-list upload into dev_desc, ONE persistent sm_100a kernel that executes it
+ * ("reads from the source-mode alias and writes ... the target-mode slot", one HBM read
+ * and one write per element, Table 1 :185), then the new tables + active-mode flag into dev_tables.
+ * MOEBIUS_E_STATE if plan.from is not the active mode.  On success the active mode becomes plan.to.
+ * Work on the stream is ordered after everything enqueued before it; no other stream may touch
+ * the bound buffers while it runs. */
+MOEBIUS_API int moebius_reshard(moebius_ctx_t* ctx, const moebius_plan_t* plan, void* cuda_stream);
+
+/* Kernel-only device time of the last moebius_reshard, in ms (CUDA events on its stream; the call
+ * synchronises on the end event).  Enabled with moebius_set_timing(ctx, 1). */
+MOEBIUS_API int moebius_set_timing(moebius_ctx_t* ctx, int enable);
+MOEBIUS_API int moebius_last_kernel_ms(moebius_ctx_t* ctx, float* ms);
+
+/* Launch shape override for tuning: ctas_per_sm <= 0 and threads <= 0 restore the defaults. */
+MOEBIUS_API int moebius_set_launch(moebius_ctx_t* ctx, int ctas_per_sm, int threads, int unit_kb);
+
+MOEBIUS_API const char* moebius_status_str(int status);
+MOEBIUS_API int moebius_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* MOEBIUS_H_ */

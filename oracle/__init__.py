@@ -20,3 +20,4 @@ from .kv import (  # noqa: F401
 )
 from .accounting import kv_bytes, weight_bytes  # noqa: F401
 from .ffn import moe_ffn_dense, moe_ffn_ep, moe_ffn_tp, route_top2  # noqa: F401
+from .image import OracleLayout, State, np_view, target_request_state  # noqa: F401,E402

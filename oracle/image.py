@@ -1,0 +1,130 @@
+"""Placing oracle layouts into a byte image of the unified buffer, and comparing.  TEST INFRASTRUCTURE.
+
+The oracle does not know the address map: the caller passes `view_fn(mode, rank, layer, tensor_id)
+-> (byte_offset, shape, elem_bytes)` (the fixed views the library reports) and the
+pool page counts.  Nothing here imports the CUDA path.  mode: 0 = TP, 1 = EP; tensor ids: 0 gate,
+1 up, 2 down, 3 K pool, 4 V pool, 5/6/7 fp8 scales of gate/up/down.
+"""
+from __future__ import annotations
+
+import numpy as np
+
+import workloads as wl
+
+from . import kv as okv
+from . import weights as ow
+
+KINDS = ("gate", "up", "down")
+TP, EP = 0, 1
+
+
+class State:
+    """Logical state of one workload: expert tensors per layer, K/V per request, lengths."""
+
+    def __init__(self, cfg: wl.Config, seq_lens=None, fill="tag"):
+        self.cfg = cfg
+        self.lens = np.asarray(wl.draw_seq_lens(cfg) if seq_lens is None else seq_lens, dtype=np.int32)
+        self.fill = fill
+        self._w = {}
+        self._kv = {}
+
+    def weight(self, layer, kind):
+        key = (layer, kind)
+        if key not in self._w:
+            self._w[key] = wl.gen_logical_weight(self.cfg, layer, kind, fill=self.fill)
+        return self._w[key]
+
+    def scale(self, layer, kind):
+        return wl.gen_logical_scale(self.cfg, layer, kind)
+
+    def kv(self, layer, kvi):
+        key = (layer, kvi)
+        if key not in self._kv:
+            self._kv[key] = {i: wl.gen_kv_request(self.cfg, layer, kvi, i, int(n), fill=self.fill)
+                             for i, n in enumerate(self.lens)}
+        return self._kv[key]
+
+    def drop_cache(self):
+        self._w.clear()
+        self._kv.clear()
+
+
+def np_view(image: np.ndarray, desc):
+    off, shape, eb = desc
+    dt = {1: np.uint8, 2: np.uint16, 4: np.float32}[eb]
+    n = int(np.prod(shape)) * eb
+    return image[off:off + n].view(dt).reshape(shape)
+
+
+class OracleLayout:
+    """The oracle's views of one mode for a State and a request state (owner, bt)."""
+
+    def __init__(self, st: State, view_fn, pages_tp: int, pages_ep: int, mode: int, owner, bt):
+        self.st, self.view_fn, self.mode, self.owner, self.bt = st, view_fn, mode, owner, bt
+        self.pages_tp, self.pages_ep = pages_tp, pages_ep
+
+    def weight_view(self, r, layer, kind):
+        X = self.st.weight(layer, kind)
+        R = self.st.cfg.R
+        return ow.tp_weight_view(X, kind, r, R) if self.mode == TP else ow.ep_weight_view(X, r, R)
+
+    def scale_view(self, r, layer, kind):
+        S = self.st.scale(layer, kind)
+        c = self.st.cfg
+        return ow.tp_scale_view(S, kind, r, c.R, c.I) if self.mode == TP else ow.ep_scale_view(S, r, c.R)
+
+    def pool(self, r, layer, kvi):
+        c = self.st.cfg
+        KV = self.st.kv(layer, kvi)
+        if self.mode == TP:
+            return okv.tp_pool_image(KV, self.st.lens, self.bt, r, c.R, c.kv_heads, c.head_dim, c.page, self.pages_tp)
+        return okv.ep_pool_image(KV, self.st.lens, self.owner, self.bt, r, c.kv_heads, c.head_dim, c.page,
+                                 self.pages_ep)
+
+    def place(self, image: np.ndarray):
+        c = self.st.cfg
+        fp8 = c.w_dtype == "fp8_e4m3_b128"
+        for r in range(c.R):
+            for l in range(c.L):
+                for m, kind in enumerate(KINDS):
+                    np_view(image, self.view_fn(self.mode, r, l, m))[...] = self.weight_view(r, l, kind)
+                    if fp8:
+                        np_view(image, self.view_fn(self.mode, r, l, 5 + m))[...] = self.scale_view(r, l, kind)
+                for kvi in range(2):
+                    pool, mask = self.pool(r, l, kvi)
+                    np_view(image, self.view_fn(self.mode, r, l, 3 + kvi))[mask] = pool[mask]
+
+    def compare(self, image: np.ndarray):
+        """Bytewise comparison of every view of this mode; returns a list of mismatch strings.
+        KV bytes outside the validity mask are unspecified (reading A10) and not compared."""
+        c = self.st.cfg
+        fp8 = c.w_dtype == "fp8_e4m3_b128"
+        bad = []
+        for r in range(c.R):
+            for l in range(c.L):
+                for m, kind in enumerate(KINDS):
+                    got = np_view(image, self.view_fn(self.mode, r, l, m))
+                    want = self.weight_view(r, l, kind)
+                    if not np.array_equal(got.view(np.uint8), want.view(np.uint8)):
+                        bad.append("weight r%d l%d %s: %d elems differ" % (r, l, kind, int((got != want).sum())))
+                    if fp8:
+                        got = np_view(image, self.view_fn(self.mode, r, l, 5 + m))
+                        want = self.scale_view(r, l, kind)
+                        if not np.array_equal(got.view(np.uint32), want.view(np.uint32)):
+                            bad.append("scale r%d l%d %s" % (r, l, kind))
+                for kvi in range(2):
+                    pool, mask = self.pool(r, l, kvi)
+                    got = np_view(image, self.view_fn(self.mode, r, l, 3 + kvi))
+                    if not np.array_equal(got[mask], pool[mask]):
+                        bad.append("kv r%d l%d kv%d: %d slots differ" % (
+                            r, l, kvi, int((got[mask] != pool[mask]).any(axis=(1, 2)).sum())))
+        return bad
+
+
+def target_request_state(st: State, to_mode: int, pages_tp: int, pages_ep: int, max_pages: int):
+    """Oracle request state after a switch: owner and canonical tables (reading A7)."""
+    c = st.cfg
+    owner = okv.partition_requests(st.lens, c.R) if to_mode == EP else None
+    bt = okv.canonical_block_tables(st.lens, owner, "ep" if to_mode == EP else "tp",
+                                    pages_ep if to_mode == EP else pages_tp, c.page, max_pages)
+    return owner, bt

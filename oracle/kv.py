@@ -40,6 +40,11 @@ def tp_source_rank(head: int, new_owner: int, R: int, Hkv: int) -> int:
     raise AssertionError
 
 
+def _kv_dtype(KV):
+    vals = list(KV.values()) if isinstance(KV, dict) else list(KV)
+    return vals[0].dtype if vals else np.uint16   # no live request: an empty bf16 pool
+
+
 def pages_needed(length: int, pg: int) -> int:
     return (int(length) + pg - 1) // pg
 
@@ -106,32 +111,34 @@ def tp_pool_image(KV, seq_lens, bt, r: int, R: int, Hkv: int, D: int, pg: int, n
     rank r's heads only; every rank uses the same table.  KV[i] is the logical [len_i, Hkv, D].
     Bytes outside the mask are unspecified (reading A10)."""
     heads = kv_heads_of_rank(r, R, Hkv)
-    any_kv = next(iter(KV.values())) if isinstance(KV, dict) else KV[0]
-    pool = np.zeros((n_pages, pg, len(heads), D), dtype=any_kv.dtype)
+    pool = np.zeros((n_pages, pg, len(heads), D), dtype=_kv_dtype(KV))
     mask = np.zeros((n_pages, pg), dtype=bool)
     for i in range(len(seq_lens)):
-        for t in range(int(seq_lens[i])):
-            p = int(bt[i][t // pg])
-            assert 0 <= p < n_pages and not mask[p, t % pg]
-            pool[p, t % pg] = KV[i][t, heads, :]
-            mask[p, t % pg] = True
+        n = int(seq_lens[i])
+        for b in range(pages_needed(n, pg)):          # block b holds tokens [b*pg, min(n, (b+1)*pg))
+            p = int(bt[i][b])
+            k = min(pg, n - b * pg)
+            assert 0 <= p < n_pages and not mask[p].any()
+            pool[p, :k] = KV[i][b * pg:b * pg + k][:, heads, :]
+            mask[p, :k] = True
     return pool, mask
 
 
 def ep_pool_image(KV, seq_lens, owner, bt, r: int, Hkv: int, D: int, pg: int, n_pages: int):
     """K (or V) pool of rank r under EP for one layer: [n_pages, pg, Hkv, D] + mask; holds all
     heads of the requests rank r owns and nothing else."""
-    any_kv = next(iter(KV.values())) if isinstance(KV, dict) else KV[0]
-    pool = np.zeros((n_pages, pg, Hkv, D), dtype=any_kv.dtype)
+    pool = np.zeros((n_pages, pg, Hkv, D), dtype=_kv_dtype(KV))
     mask = np.zeros((n_pages, pg), dtype=bool)
     for i in range(len(seq_lens)):
         if int(owner[i]) != r:
             continue
-        for t in range(int(seq_lens[i])):
-            p = int(bt[i][t // pg])
-            assert 0 <= p < n_pages and not mask[p, t % pg]
-            pool[p, t % pg] = KV[i][t]
-            mask[p, t % pg] = True
+        n = int(seq_lens[i])
+        for b in range(pages_needed(n, pg)):
+            p = int(bt[i][b])
+            k = min(pg, n - b * pg)
+            assert 0 <= p < n_pages and not mask[p].any()
+            pool[p, :k] = KV[i][b * pg:b * pg + k]
+            mask[p, :k] = True
     return pool, mask
 
 

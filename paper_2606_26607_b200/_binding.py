@@ -1,0 +1,228 @@
+"""ctypes marshalling for include/moebius.h.  Same names, same semantics; errors raise."""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_LIB = os.path.join(_HERE, "libmoebius.so")
+
+MOEBIUS_TP, MOEBIUS_EP = 0, 1
+MOEBIUS_BF16, MOEBIUS_FP32, MOEBIUS_FP8_E4M3_B128 = 0, 1, 2
+T_GATE, T_UP, T_DOWN, T_KPOOL, T_VPOOL, T_GATE_SCALE, T_UP_SCALE, T_DOWN_SCALE = range(8)
+
+EXPORTED_SYMBOLS = [
+    "moebius_create", "moebius_destroy", "moebius_layout", "moebius_view", "moebius_bind",
+    "moebius_active_mode", "moebius_plan", "moebius_plan_destroy", "moebius_block_tables",
+    "moebius_plan_stats", "moebius_plan_export", "moebius_reshard", "moebius_set_timing",
+    "moebius_last_kernel_ms", "moebius_set_launch", "moebius_status_str", "moebius_version",
+]
+
+
+class MoebiusError(RuntimeError):
+    def __init__(self, status: int, where: str):
+        self.status = status
+        super().__init__("%s: %s (%d)" % (where, moebius_status_str(status), status))
+
+
+class moebius_config_t(C.Structure):
+    _fields_ = [("struct_size", C.c_uint32), ("R", C.c_int32), ("L", C.c_int32), ("E", C.c_int32),
+                ("H", C.c_int32), ("I", C.c_int32), ("w_dtype", C.c_int32), ("w_orient", C.c_int32),
+                ("kv_heads", C.c_int32), ("head_dim", C.c_int32), ("page_tokens", C.c_int32),
+                ("kv_dtype", C.c_int32), ("kv_pool_bytes_per_rank_layer", C.c_int64),
+                ("max_requests", C.c_int32), ("max_pages_per_request", C.c_int32),
+                ("staging_cap_bytes", C.c_int64)]
+
+
+class moebius_layout_t(C.Structure):
+    _fields_ = [("struct_size", C.c_uint32), ("pages_tp", C.c_int32), ("pages_ep", C.c_int32),
+                ("tp_page_bytes", C.c_int32), ("ep_page_bytes", C.c_int32), ("base_bytes", C.c_int64),
+                ("rank_stride_bytes", C.c_int64), ("weight_slot_bytes", C.c_int64),
+                ("weight_spare_bytes", C.c_int64), ("staging_bytes", C.c_int64), ("desc_bytes", C.c_int64),
+                ("table_bytes", C.c_int64), ("resident_bytes", C.c_int64), ("tbl_owner_off", C.c_int32),
+                ("tbl_lens_off", C.c_int32), ("tbl_bt_off", C.c_int32), ("tbl_reserved", C.c_int32)]
+
+
+class moebius_view_t(C.Structure):
+    _fields_ = [("struct_size", C.c_uint32), ("ndim", C.c_int32), ("elem_bytes", C.c_int32),
+                ("offset", C.c_int64), ("shape", C.c_int64 * 4), ("stride", C.c_int64 * 4)]
+
+
+class moebius_stats_t(C.Structure):
+    _fields_ = [("struct_size", C.c_uint32), ("n_segments", C.c_int32), ("n_kv_moves", C.c_int32),
+                ("n_kv_rounds", C.c_int32), ("n_kv_staged", C.c_int32), ("n_pool_groups", C.c_int32),
+                ("n_units", C.c_int64), ("w_moved", C.c_int64), ("w_relocated", C.c_int64),
+                ("w_read", C.c_int64), ("kv_moved", C.c_int64), ("kv_relocated", C.c_int64),
+                ("kv_read", C.c_int64), ("staging_used_bytes", C.c_int64),
+                ("desc_upload_bytes", C.c_int64), ("table_upload_bytes", C.c_int64)]
+
+    def as_dict(self):
+        return {k: getattr(self, k) for k, _ in self._fields_ if k != "struct_size"}
+
+
+# numpy mirrors of the exported work-list records (diagnostics / hazard tests)
+SEG_DTYPE = np.dtype([
+    ("kind", "<u4"), ("ep_is_src", "<u4"), ("wait_ctr", "<i4"), ("wait_target", "<u4"),
+    ("signal_ctr", "<i4"), ("unit_begin", "<u4"), ("n_units", "<u4"), ("run_bytes", "<u4"),
+    ("n_groups", "<u4"), ("rep", "<u4"), ("rows_per_unit", "<u4"), ("groups_per_unit", "<u4"),
+    ("chunk_bytes", "<u4"), ("chunks_per_run", "<u4"), ("rows_total", "<u4"), ("row_blocks", "<u4"),
+    ("ep_off", "<i8"), ("tp_off", "<i8"), ("kv_mode", "<u4"), ("desc_begin", "<u4"), ("n_desc", "<u4"),
+    ("pool_begin", "<u4"), ("n_pools", "<u4"), ("pools_per_unit", "<u4"), ("ep_page_bytes", "<u4"),
+    ("tp_page_bytes", "<u4"), ("pool_bytes", "<i8"), ("stg_pool_begin", "<u4"), ("stg_pools", "<u4")])
+KV_DTYPE = np.dtype([("ep_rank", "<i4"), ("ep_page", "<i4"), ("tp_page", "<i4"), ("ntok_slot", "<u4")])
+C2D_DTYPE = np.dtype([("src_off", "<i8"), ("dst_off", "<i8"), ("rows", "<u4"), ("run_bytes", "<u4"),
+                      ("src_stride", "<u4"), ("dst_stride", "<u4")])
+assert SEG_DTYPE.itemsize == 128 and KV_DTYPE.itemsize == 16 and C2D_DTYPE.itemsize == 32
+
+
+def lib_path() -> str:
+    return _LIB
+
+
+if not os.path.exists(_LIB):
+    raise ImportError(
+        "libmoebius.so is not built (%s). Build it with `python -m paper_2606_26607_b200.build` "
+        "(nvcc, sm_100a). There is no CPU fallback." % _LIB)
+_lib = C.CDLL(_LIB)
+
+_vp = C.c_void_p
+_i32p = C.POINTER(C.c_int32)
+_lib.moebius_create.argtypes = [C.POINTER(moebius_config_t), C.POINTER(_vp)]
+_lib.moebius_destroy.argtypes = [_vp]
+_lib.moebius_destroy.restype = None
+_lib.moebius_layout.argtypes = [_vp, C.POINTER(moebius_layout_t)]
+_lib.moebius_view.argtypes = [_vp, C.c_int, C.c_int, C.c_int, C.c_int, C.POINTER(moebius_view_t)]
+_lib.moebius_bind.argtypes = [_vp, _vp, _vp, _vp, _vp, C.c_int]
+_lib.moebius_active_mode.argtypes = [_vp]
+_lib.moebius_plan.argtypes = [_vp, C.c_int, C.c_int, C.c_int32, _vp, _vp, _vp, C.POINTER(_vp)]
+_lib.moebius_plan_destroy.argtypes = [_vp]
+_lib.moebius_plan_destroy.restype = None
+_lib.moebius_block_tables.argtypes = [_vp, _vp, _vp]
+_lib.moebius_plan_stats.argtypes = [_vp, C.POINTER(moebius_stats_t)]
+_lib.moebius_plan_export.argtypes = [_vp, C.c_int, _vp, C.c_int64, C.POINTER(C.c_int64)]
+_lib.moebius_reshard.argtypes = [_vp, _vp, _vp]
+_lib.moebius_set_timing.argtypes = [_vp, C.c_int]
+_lib.moebius_last_kernel_ms.argtypes = [_vp, C.POINTER(C.c_float)]
+_lib.moebius_set_launch.argtypes = [_vp, C.c_int, C.c_int, C.c_int]
+_lib.moebius_status_str.argtypes = [C.c_int]
+_lib.moebius_status_str.restype = C.c_char_p
+_lib.moebius_version.restype = C.c_int
+
+
+def moebius_status_str(status: int) -> str:
+    return _lib.moebius_status_str(int(status)).decode()
+
+
+def moebius_version() -> int:
+    return _lib.moebius_version()
+
+
+def _chk(status: int, where: str):
+    if status != 0:
+        raise MoebiusError(status, where)
+
+
+def moebius_create(cfg: moebius_config_t):
+    cfg.struct_size = C.sizeof(moebius_config_t)
+    out = _vp()
+    _chk(_lib.moebius_create(C.byref(cfg), C.byref(out)), "moebius_create")
+    return out
+
+
+def moebius_destroy(ctx):
+    _lib.moebius_destroy(ctx)
+
+
+def moebius_layout(ctx) -> moebius_layout_t:
+    out = moebius_layout_t()
+    out.struct_size = C.sizeof(moebius_layout_t)
+    _chk(_lib.moebius_layout(ctx, C.byref(out)), "moebius_layout")
+    return out
+
+
+def moebius_view(ctx, mode: int, rank: int, layer: int, tensor_id: int) -> moebius_view_t:
+    out = moebius_view_t()
+    out.struct_size = C.sizeof(moebius_view_t)
+    _chk(_lib.moebius_view(ctx, mode, rank, layer, tensor_id, C.byref(out)), "moebius_view")
+    return out
+
+
+def moebius_bind(ctx, dev_base: int, dev_staging: int, dev_desc: int, dev_tables: int, initial_mode: int):
+    _chk(_lib.moebius_bind(ctx, _vp(dev_base), _vp(dev_staging or None), _vp(dev_desc), _vp(dev_tables),
+                           initial_mode), "moebius_bind")
+
+
+def moebius_active_mode(ctx) -> int:
+    return _lib.moebius_active_mode(ctx)
+
+
+def _i32(a, shape=None):
+    a = np.ascontiguousarray(a, dtype=np.int32)
+    if shape is not None and a.shape != shape:
+        raise ValueError("expected shape %r, got %r" % (shape, a.shape))
+    return a
+
+
+def moebius_plan(ctx, from_mode: int, to_mode: int, seq_lens, src_owner, src_block_tables):
+    """seq_lens int32[n]; src_owner int32[n] or None; src_block_tables int32[n, max_pages]."""
+    n = 0 if seq_lens is None else len(seq_lens)
+    lens = _i32(seq_lens if n else np.zeros(0, np.int32))
+    own = None if src_owner is None else _i32(src_owner, (n,))
+    bt = _i32(src_block_tables if n else np.zeros((0, 1), np.int32))
+    out = _vp()
+    st = _lib.moebius_plan(ctx, from_mode, to_mode, n,
+                           lens.ctypes.data_as(_vp) if n else None,
+                           own.ctypes.data_as(_vp) if own is not None and n else None,
+                           bt.ctypes.data_as(_vp) if n else None, C.byref(out))
+    _chk(st, "moebius_plan")
+    return out
+
+
+def moebius_plan_destroy(plan):
+    _lib.moebius_plan_destroy(plan)
+
+
+def moebius_block_tables(plan, n_req: int, max_pages: int):
+    owner = np.empty(n_req, np.int32)
+    bt = np.empty((n_req, max_pages), np.int32)
+    _chk(_lib.moebius_block_tables(plan, owner.ctypes.data_as(_vp), bt.ctypes.data_as(_vp)),
+         "moebius_block_tables")
+    return owner, bt
+
+
+def moebius_plan_stats(plan) -> moebius_stats_t:
+    out = moebius_stats_t()
+    out.struct_size = C.sizeof(moebius_stats_t)
+    _chk(_lib.moebius_plan_stats(plan, C.byref(out)), "moebius_plan_stats")
+    return out
+
+
+def moebius_plan_export(plan, what: int) -> np.ndarray:
+    dt = (SEG_DTYPE, KV_DTYPE, C2D_DTYPE)[what]
+    need = C.c_int64(0)
+    _chk(_lib.moebius_plan_export(plan, what, None, 0, C.byref(need)), "moebius_plan_export")
+    buf = np.zeros(need.value // dt.itemsize, dtype=dt)
+    if need.value:
+        _chk(_lib.moebius_plan_export(plan, what, buf.ctypes.data_as(_vp), need.value, C.byref(need)),
+             "moebius_plan_export")
+    return buf
+
+
+def moebius_reshard(ctx, plan, cuda_stream: int = 0):
+    _chk(_lib.moebius_reshard(ctx, plan, _vp(cuda_stream or None)), "moebius_reshard")
+
+
+def moebius_set_timing(ctx, enable: bool):
+    _chk(_lib.moebius_set_timing(ctx, int(enable)), "moebius_set_timing")
+
+
+def moebius_last_kernel_ms(ctx) -> float:
+    ms = C.c_float(0)
+    _chk(_lib.moebius_last_kernel_ms(ctx, C.byref(ms)), "moebius_last_kernel_ms")
+    return ms.value
+
+
+def moebius_set_launch(ctx, ctas_per_sm: int = 0, threads: int = 0, unit_kb: int = 0):
+    _chk(_lib.moebius_set_launch(ctx, ctas_per_sm, threads, unit_kb), "moebius_set_launch")

@@ -1,0 +1,82 @@
+// moebius_host.h -- host-side objects behind the opaque C handles (product code, not the oracle).
+#ifndef MOEBIUS_HOST_H_
+#define MOEBIUS_HOST_H_
+
+#include <cstdint>
+#include <vector>
+
+#include "../../include/moebius.h"
+#include "moebius_units.h"
+
+namespace moebius {
+
+constexpr int kMaxCounters = 4096;
+constexpr int kMaxSegs = 8192;
+constexpr int64_t kHdrBytes = 256;                         // ticket lives at byte 0
+constexpr int64_t kCtrOff = kHdrBytes;                     // uint32 counters[kMaxCounters]
+constexpr int64_t kSegOff = kCtrOff + 4 * kMaxCounters;    // Seg[...]
+constexpr int kTblHdrInts = 16;
+
+struct ScaleGeom {           // fp8 block scales of one matrix kind (reading A13)
+  int64_t tp_bytes;          // per rank, allocated with the largest nb over ranks
+  int64_t ep_bytes;          // per rank
+};
+
+}  // namespace moebius
+
+struct moebius_ctx {
+  moebius_config_t cfg;
+  int wb, kvb;                    // element bytes
+  int ep_shift;                   // EP view of object k is slot k + ep_shift (0 when R == 1)
+  int64_t S;                      // weight slot bytes per rank
+  int64_t w_off, scale_tp_off, scale_ep_off, kv_off, rank_stride;
+  moebius::ScaleGeom sg[3];
+  int64_t scale_tp_layer, scale_ep_layer;  // bytes per layer per rank
+  int G, rep, hpr;
+  int64_t run_kv, ep_page_bytes, tp_page_bytes, pool_bytes;
+  int32_t pages_ep, pages_tp;
+  int64_t staging_bytes, desc_bytes, table_bytes, resident_bytes, spare_bytes;
+  int64_t max_kv_desc, max_c2d;
+  // bound buffers
+  bool bound;
+  char* base;
+  char* stg;
+  char* desc;
+  int32_t* tables;
+  int active_mode;
+  int64_t switch_count;
+  // launch shape
+  int ctas_per_sm, threads, unit_kb;
+  // device facts + timing (filled lazily by the CUDA side)
+  int n_sm;
+  int timing;
+  void* ev0;
+  void* ev1;
+  bool ev_valid;
+};
+
+struct moebius_plan {
+  const moebius_ctx* ctx;
+  int from, to, n_req;
+  std::vector<moebius::Seg> segs;
+  std::vector<moebius::KvDesc> kv;
+  std::vector<moebius::C2dDesc> c2d;
+  std::vector<int32_t> lens, owner, bt;   // target-mode request state
+  moebius_stats_t stats;
+  uint32_t n_counters, total_units;
+  // one contiguous upload image: [segs][kv][c2d], and the table image; pinned when CUDA allows
+  char* image;
+  int64_t image_bytes, kv_img_off, c2d_img_off;
+  int32_t* tbl_image;
+  int64_t tbl_bytes;
+  bool pinned;
+};
+
+namespace moebius {
+// CUDA side (moebius_cuda.cu)
+void* host_alloc(int64_t bytes, bool* pinned);
+void host_free(void* p, bool pinned);
+void cuda_ctx_destroy(moebius_ctx* ctx);
+}  // namespace moebius
+
+#endif

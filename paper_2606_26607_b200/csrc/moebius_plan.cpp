@@ -1,0 +1,757 @@
+// moebius_plan.cpp -- host side of the C ABI: region map (§4.2), the weight plan
+// (§3.1), request ownership and target block tables (§3.2), the KV
+// page-move list with its dependency rounds and bounded staging, and the byte accounting.
+// Product code: it shares nothing with oracle/.
+#include <algorithm>
+#include <cstdlib>
+#include <cstring>
+#include <new>
+#include <numeric>
+
+#include "moebius_host.h"
+
+using namespace moebius;
+
+namespace {
+
+int64_t align_up(int64_t x, int64_t a) { return (x + a - 1) / a * a; }
+int dtype_bytes(int d) { return d == MOEBIUS_BF16 ? 2 : d == MOEBIUS_FP32 ? 4 : d == MOEBIUS_FP8_E4M3_B128 ? 1 : 0; }
+
+// 128-wide blocks of the intermediate axis that TP shard r touches (reading A13)
+void scale_blocks(int r, int R, int I, int* lo, int* hi) {
+  int w = I / R;
+  *lo = (r * w) / 128;
+  *hi = ((r + 1) * w - 1) / 128 + 1;
+}
+
+struct Move {
+  int32_t req, blk, ep_rank, ep_page, tp_page, ntok;
+  int32_t level;
+  int32_t slot;
+  uint8_t staged;
+};
+
+constexpr int kMaxLevel = 24;
+
+}  // namespace
+
+extern "C" {
+
+const char* moebius_status_str(int s) {
+  switch (s) {
+    case MOEBIUS_OK: return "ok";
+    case MOEBIUS_E_INVAL: return "invalid argument";
+    case MOEBIUS_E_CAPACITY: return "target mode cannot hold the live requests";
+    case MOEBIUS_E_STAGING: return "staging buffer too small";
+    case MOEBIUS_E_STATE: return "wrong state";
+    case MOEBIUS_E_CUDA: return "CUDA error or no device";
+  }
+  return "unknown";
+}
+
+int moebius_version(void) { return 1; }
+
+int moebius_create(const moebius_config_t* c, moebius_ctx_t** out) {
+  if (!c || !out || c->struct_size != sizeof(moebius_config_t)) return MOEBIUS_E_INVAL;
+  *out = nullptr;
+  const int R = c->R, L = c->L, E = c->E, H = c->H, I = c->I;
+  if (R < 1 || L < 1 || E < 1 || H < 1 || I < 1 || R > 64) return MOEBIUS_E_INVAL;
+  if (E % R || I % R) return MOEBIUS_E_INVAL;
+  if (c->w_orient != 0) return MOEBIUS_E_INVAL;
+  const int wb = dtype_bytes(c->w_dtype);
+  const int kvb = (c->kv_dtype == MOEBIUS_BF16 || c->kv_dtype == MOEBIUS_FP32) ? dtype_bytes(c->kv_dtype) : 0;
+  if (!wb || !kvb) return MOEBIUS_E_INVAL;
+  if (((int64_t)(I / R) * wb) % 16) return MOEBIUS_E_INVAL;  // reading A3
+  if (c->w_dtype == MOEBIUS_FP8_E4M3_B128 && (H % 128 || I % 128)) return MOEBIUS_E_INVAL;
+  const int Hkv = c->kv_heads, D = c->head_dim, pg = c->page_tokens;
+  if (Hkv < 1 || D < 1 || pg < 1 || pg > 255) return MOEBIUS_E_INVAL;
+  if (!(Hkv % R == 0 || R % Hkv == 0)) return MOEBIUS_E_INVAL;
+  if (c->max_requests < 0 || c->max_pages_per_request < 0) return MOEBIUS_E_INVAL;
+  if (c->staging_cap_bytes < 0 || c->kv_pool_bytes_per_rank_layer < 0) return MOEBIUS_E_INVAL;
+
+  moebius_ctx* x = new (std::nothrow) moebius_ctx();
+  if (!x) return MOEBIUS_E_INVAL;
+  x->cfg = *c;
+  x->wb = wb;
+  x->kvb = kvb;
+  x->ep_shift = R == 1 ? 0 : 1;
+  x->hpr = Hkv >= R ? Hkv / R : 1;
+  x->rep = Hkv >= R ? 1 : R / Hkv;
+  x->G = Hkv >= R ? R : Hkv;
+  x->run_kv = (int64_t)x->hpr * D * kvb;
+  if (x->run_kv % 16) { delete x; return MOEBIUS_E_INVAL; }
+  x->tp_page_bytes = (int64_t)pg * x->run_kv;
+  x->ep_page_bytes = x->tp_page_bytes * x->G;
+  x->pool_bytes = c->kv_pool_bytes_per_rank_layer;
+  if (x->pool_bytes % x->ep_page_bytes || x->ep_page_bytes > (1 << 30)) { delete x; return MOEBIUS_E_INVAL; }
+  int64_t pe = x->pool_bytes / x->ep_page_bytes;
+  if (pe * x->G > INT32_MAX) { delete x; return MOEBIUS_E_INVAL; }
+  x->pages_ep = (int32_t)pe;
+  x->pages_tp = (int32_t)(pe * x->G);
+
+  // rank region: [weight chain: 3L+ep_shift slots][TP scales][EP scales][2L KV pools]
+  x->S = align_up((int64_t)(E / R) * H * I * wb, 256);
+  x->w_off = 0;
+  int64_t off = (int64_t)(3 * L + x->ep_shift) * x->S;
+  x->scale_tp_layer = x->scale_ep_layer = 0;
+  memset(x->sg, 0, sizeof(x->sg));
+  if (c->w_dtype == MOEBIUS_FP8_E4M3_B128) {
+    int nb_max = 0;
+    for (int r = 0; r < R; ++r) { int lo, hi; scale_blocks(r, R, I, &lo, &hi); nb_max = std::max(nb_max, hi - lo); }
+    for (int m = 0; m < 3; ++m) {
+      x->sg[m].tp_bytes = align_up((int64_t)E * (H / 128) * nb_max * 4, 256);
+      x->sg[m].ep_bytes = align_up((int64_t)(E / R) * (H / 128) * (I / 128) * 4, 256);
+      x->scale_tp_layer += x->sg[m].tp_bytes;
+      x->scale_ep_layer += x->sg[m].ep_bytes;
+    }
+  }
+  x->scale_tp_off = off;  off += x->scale_tp_layer * L;
+  x->scale_ep_off = off;  off += x->scale_ep_layer * L;
+  off = align_up(off, 4096);
+  x->kv_off = off;        off += 2 * (int64_t)L * x->pool_bytes;
+  x->rank_stride = align_up(off, 4096);
+
+  x->spare_bytes = (int64_t)x->ep_shift * x->S * R;
+  x->resident_bytes = (int64_t)3 * L * x->S * R + 2 * (int64_t)L * x->pool_bytes * R;
+  const int64_t kv_total = 2 * (int64_t)L * x->pool_bytes * R;
+  if (c->staging_cap_bytes == 0) {
+    x->staging_bytes = kv_total / 50;   // no bound given: 2% of the KV capacity
+  } else {
+    if (c->staging_cap_bytes < x->spare_bytes) { delete x; return MOEBIUS_E_STAGING; }
+    x->staging_bytes = std::min(c->staging_cap_bytes - x->spare_bytes, kv_total);
+  }
+  x->staging_bytes = x->staging_bytes / x->ep_page_bytes * x->ep_page_bytes;
+
+  // descriptor buffer: header, counters, segments, KV moves (each live page at most twice), scale copies
+  int64_t live_max = std::max<int64_t>((int64_t)x->pages_tp, (int64_t)x->pages_ep * R);
+  live_max = std::min<int64_t>(live_max, (int64_t)c->max_requests * c->max_pages_per_request);
+  x->max_kv_desc = live_max;
+  x->max_c2d = c->w_dtype == MOEBIUS_FP8_E4M3_B128 ? (int64_t)3 * L * R * R : 0;
+  x->desc_bytes = align_up(kSegOff + (int64_t)kMaxSegs * sizeof(Seg) + x->max_kv_desc * sizeof(KvDesc) +
+                               x->max_c2d * sizeof(C2dDesc) + 1024, 4096);
+  x->table_bytes = align_up(4 * ((int64_t)kTblHdrInts + 2 * (int64_t)c->max_requests +
+                                 (int64_t)c->max_requests * c->max_pages_per_request), 256);
+  x->bound = false;
+  x->base = x->stg = x->desc = nullptr;
+  x->tables = nullptr;
+  x->active_mode = -1;
+  x->switch_count = 0;
+  x->ctas_per_sm = 0;
+  x->threads = 0;
+  x->unit_kb = 0;
+  x->n_sm = 0;
+  x->timing = 0;
+  x->ev0 = x->ev1 = nullptr;
+  x->ev_valid = false;
+  *out = x;
+  return MOEBIUS_OK;
+}
+
+void moebius_destroy(moebius_ctx_t* ctx) {
+  if (!ctx) return;
+  cuda_ctx_destroy(ctx);
+  delete ctx;
+}
+
+int moebius_layout(const moebius_ctx_t* x, moebius_layout_t* o) {
+  if (!x || !o || o->struct_size != sizeof(moebius_layout_t)) return MOEBIUS_E_INVAL;
+  o->pages_tp = x->pages_tp;
+  o->pages_ep = x->pages_ep;
+  o->tp_page_bytes = (int32_t)x->tp_page_bytes;
+  o->ep_page_bytes = (int32_t)x->ep_page_bytes;
+  o->base_bytes = x->rank_stride * x->cfg.R;
+  o->rank_stride_bytes = x->rank_stride;
+  o->weight_slot_bytes = x->S;
+  o->weight_spare_bytes = x->spare_bytes;
+  o->staging_bytes = x->staging_bytes;
+  o->desc_bytes = x->desc_bytes;
+  o->table_bytes = x->table_bytes;
+  o->resident_bytes = x->resident_bytes;
+  o->tbl_owner_off = kTblHdrInts;
+  o->tbl_lens_off = kTblHdrInts + x->cfg.max_requests;
+  o->tbl_bt_off = kTblHdrInts + 2 * x->cfg.max_requests;
+  o->tbl_reserved = 0;
+  return MOEBIUS_OK;
+}
+
+int moebius_view(const moebius_ctx_t* x, moebius_mode_t mode, int rank, int layer, int t, moebius_view_t* o) {
+  if (!x || !o || o->struct_size != sizeof(moebius_view_t)) return MOEBIUS_E_INVAL;
+  const moebius_config_t& c = x->cfg;
+  if (rank < 0 || rank >= c.R || layer < 0 || layer >= c.L) return MOEBIUS_E_INVAL;
+  if (mode != MOEBIUS_TP && mode != MOEBIUS_EP) return MOEBIUS_E_INVAL;
+  const bool tp = mode == MOEBIUS_TP;
+  const int64_t rbase = (int64_t)rank * x->rank_stride;
+  const int R = c.R, E = c.E, H = c.H, I = c.I;
+  for (int i = 0; i < 4; ++i) o->shape[i] = 1;
+  if (t >= MOEBIUS_T_GATE && t <= MOEBIUS_T_DOWN) {
+    int k = 3 * layer + t;
+    o->offset = rbase + x->w_off + (int64_t)(k + (tp ? 0 : x->ep_shift)) * x->S;
+    o->elem_bytes = x->wb;
+    o->ndim = 3;
+    if (t != MOEBIUS_T_DOWN) { o->shape[0] = tp ? E : E / R; o->shape[1] = H; o->shape[2] = tp ? I / R : I; }
+    else                     { o->shape[0] = tp ? E : E / R; o->shape[1] = tp ? I / R : I; o->shape[2] = H; }
+  } else if (t == MOEBIUS_T_KPOOL || t == MOEBIUS_T_VPOOL) {
+    int z = 2 * layer + (t - MOEBIUS_T_KPOOL);
+    o->offset = rbase + x->kv_off + (int64_t)z * x->pool_bytes;
+    o->elem_bytes = x->kvb;
+    o->ndim = 4;
+    o->shape[0] = tp ? x->pages_tp : x->pages_ep;
+    o->shape[1] = c.page_tokens;
+    o->shape[2] = tp ? x->hpr : c.kv_heads;
+    o->shape[3] = c.head_dim;
+  } else if (t >= MOEBIUS_T_GATE_SCALE && t <= MOEBIUS_T_DOWN_SCALE) {
+    if (c.w_dtype != MOEBIUS_FP8_E4M3_B128) return MOEBIUS_E_INVAL;
+    int m = t - MOEBIUS_T_GATE_SCALE;
+    int64_t within = 0;
+    for (int mm = 0; mm < m; ++mm) within += tp ? x->sg[mm].tp_bytes : x->sg[mm].ep_bytes;
+    o->offset = rbase + (tp ? x->scale_tp_off + layer * x->scale_tp_layer
+                            : x->scale_ep_off + layer * x->scale_ep_layer) + within;
+    o->elem_bytes = 4;
+    o->ndim = 3;
+    int lo, hi;
+    scale_blocks(rank, R, I, &lo, &hi);
+    int nb = hi - lo;
+    if (m < 2) { o->shape[0] = tp ? E : E / R; o->shape[1] = H / 128; o->shape[2] = tp ? nb : I / 128; }
+    else       { o->shape[0] = tp ? E : E / R; o->shape[1] = tp ? nb : I / 128; o->shape[2] = H / 128; }
+  } else {
+    return MOEBIUS_E_INVAL;
+  }
+  int64_t st = 1;
+  for (int i = 3; i >= 0; --i) {
+    if (i >= o->ndim) { o->stride[i] = 0; continue; }
+    o->stride[i] = st;
+    st *= o->shape[i];
+  }
+  return MOEBIUS_OK;
+}
+
+int moebius_active_mode(const moebius_ctx_t* x) { return x ? x->active_mode : MOEBIUS_E_INVAL; }
+
+int moebius_set_launch(moebius_ctx_t* x, int ctas_per_sm, int threads, int unit_kb) {
+  if (!x) return MOEBIUS_E_INVAL;
+  if (threads > 0 && (threads % 32 || threads > 1024)) return MOEBIUS_E_INVAL;
+  x->ctas_per_sm = ctas_per_sm > 0 ? ctas_per_sm : 0;
+  x->threads = threads > 0 ? threads : 0;
+  x->unit_kb = unit_kb > 0 ? unit_kb : 0;
+  return MOEBIUS_OK;
+}
+
+void moebius_plan_destroy(moebius_plan_t* p) {
+  if (!p) return;
+  if (p->image) host_free(p->image, p->pinned);
+  delete p;
+}
+
+}  // extern "C"
+
+// ------------------------------------------------------------------------------------------------
+namespace {
+
+// Split `run` into equal chunks of at most `limit` bytes, each a multiple of 16.
+uint32_t pick_chunk(int64_t run, int64_t limit) {
+  if (run <= limit) return (uint32_t)run;
+  for (int64_t n = (run + limit - 1) / limit; n <= run / 16; ++n)
+    if (run % n == 0 && (run / n) % 16 == 0) return (uint32_t)(run / n);
+  return 16;
+}
+
+struct Chain {
+  std::vector<Seg> segs;
+  int64_t units = 0;
+};
+
+void push_seg(Chain& ch, const Seg& s) {
+  if (s.n_units == 0) return;
+  ch.segs.push_back(s);
+  ch.units += s.n_units;
+}
+
+Seg blank_seg() {
+  Seg s;
+  memset(&s, 0, sizeof(s));
+  s.wait_ctr = -1;
+  s.signal_ctr = -1;
+  s.rep = 1;
+  s.chunks_per_run = 1;
+  s.rows_per_unit = 1;
+  s.groups_per_unit = 1;
+  s.pools_per_unit = 1;
+  s.row_blocks = 1;
+  return s;
+}
+
+}  // namespace
+
+extern "C" int moebius_plan(moebius_ctx_t* x, moebius_mode_t from, moebius_mode_t to, int32_t n_req,
+                            const int32_t* seq_lens, const int32_t* src_owner, const int32_t* src_bt,
+                            moebius_plan_t** out) {
+  if (!x || !out) return MOEBIUS_E_INVAL;
+  *out = nullptr;
+  const moebius_config_t& c = x->cfg;
+  if (!((from == MOEBIUS_TP && to == MOEBIUS_EP) || (from == MOEBIUS_EP && to == MOEBIUS_TP))) return MOEBIUS_E_INVAL;
+  if (n_req < 0 || n_req > c.max_requests) return MOEBIUS_E_INVAL;
+  if (n_req > 0 && (!seq_lens || !src_bt)) return MOEBIUS_E_INVAL;
+  if (n_req > 0 && from == MOEBIUS_EP && !src_owner) return MOEBIUS_E_INVAL;
+  const int R = c.R, L = c.L, pg = c.page_tokens, MP = c.max_pages_per_request;
+  const bool e2t = from == MOEBIUS_EP;
+  const int n_pools_all = 2 * L;
+  const int64_t unit_bytes = (int64_t)(x->unit_kb > 0 ? x->unit_kb : 32) * 1024;
+
+  // ---- request state under the target mode ----------------------------------------------------
+  std::vector<int32_t> npages(n_req);
+  int64_t total_pages = 0;
+  for (int i = 0; i < n_req; ++i) {
+    if (seq_lens[i] < 0) return MOEBIUS_E_INVAL;
+    npages[i] = (seq_lens[i] + pg - 1) / pg;
+    if (npages[i] > MP) return MOEBIUS_E_INVAL;
+    total_pages += npages[i];
+    if (e2t && (src_owner[i] < 0 || src_owner[i] >= R)) return MOEBIUS_E_INVAL;
+  }
+  std::vector<int32_t> owner(n_req, -1);
+  if (!e2t) {
+    // decreasing length, greedy least-loaded rank, deterministic.  Reading A9: ties by
+    // request id; least loaded = smallest (tokens, requests, rank).
+    std::vector<int32_t> order(n_req);
+    std::iota(order.begin(), order.end(), 0);
+    std::stable_sort(order.begin(), order.end(), [&](int a, int b) { return seq_lens[a] > seq_lens[b]; });
+    std::vector<int64_t> tok(R, 0), cnt(R, 0);
+    for (int i : order) {
+      int best = 0;
+      for (int r = 1; r < R; ++r)
+        if (tok[r] < tok[best] || (tok[r] == tok[best] && cnt[r] < cnt[best])) best = r;
+      owner[i] = best;
+      tok[best] += seq_lens[i];
+      cnt[best] += 1;
+    }
+  }
+  // reading A7: ascending request id, consecutive pages; TP bumps up from 0, EP down from the top
+  std::vector<int32_t> bt((size_t)n_req * MP, -1);
+  if (e2t) {
+    if (total_pages > x->pages_tp) return MOEBIUS_E_CAPACITY;
+    int32_t nxt = 0;
+    for (int i = 0; i < n_req; ++i)
+      for (int b = 0; b < npages[i]; ++b) bt[(size_t)i * MP + b] = nxt++;
+  } else {
+    std::vector<int64_t> used(R, 0);
+    for (int i = 0; i < n_req; ++i) {
+      int r = owner[i];
+      if (used[r] + npages[i] > x->pages_ep) return MOEBIUS_E_CAPACITY;
+      for (int b = 0; b < npages[i]; ++b) bt[(size_t)i * MP + b] = (int32_t)(x->pages_ep - 1 - (used[r] + b));
+      used[r] += npages[i];
+    }
+  }
+
+  // ---- KV page moves (one per live (request, block); layer- and K/V-agnostic) ----
+  const int kappa = x->G;  // TP-page granules per EP page
+  std::vector<Move> mv;
+  mv.reserve((size_t)total_pages);
+  for (int i = 0; i < n_req; ++i) {
+    for (int b = 0; b < npages[i]; ++b) {
+      Move m;
+      m.req = i; m.blk = b;
+      int32_t sp = src_bt[(size_t)i * MP + b];
+      int32_t dp = bt[(size_t)i * MP + b];
+      if (sp < 0 || sp >= (e2t ? x->pages_ep : x->pages_tp)) return MOEBIUS_E_INVAL;
+      m.ep_rank = e2t ? src_owner[i] : owner[i];
+      m.ep_page = e2t ? sp : dp;
+      m.tp_page = e2t ? dp : sp;
+      m.ntok = std::min(pg, seq_lens[i] - b * pg);
+      m.level = 0; m.slot = -1; m.staged = 0;
+      mv.push_back(m);
+    }
+  }
+  const int nm = (int)mv.size();
+  {  // source pages must be unique (per owner under EP, globally under TP)
+    std::vector<uint8_t> seen((size_t)(e2t ? R : 1) * (e2t ? x->pages_ep : x->pages_tp), 0);
+    for (const Move& m : mv) {
+      size_t id = e2t ? (size_t)m.ep_rank * x->pages_ep + m.ep_page : (size_t)m.tp_page;
+      if (seen[id]) return MOEBIUS_E_INVAL;
+      seen[id] = 1;
+    }
+  }
+  // reader[rank*pages_tp + granule] = move that reads it (TP-page-sized granules of a pool)
+  std::vector<int32_t> reader;
+  std::vector<std::vector<int32_t>> dependents;  // edge b -> m: m writes what b reads
+  std::vector<std::vector<int32_t>> blockers;
+  int n_staged = 0, K = 0;
+  if (nm > 0) {
+    reader.assign((size_t)R * x->pages_tp, -1);
+    auto gid = [&](int rank, int64_t gran) { return (size_t)rank * x->pages_tp + (size_t)gran; };
+    for (int m = 0; m < nm; ++m) {
+      if (e2t) {
+        for (int g = 0; g < kappa; ++g) {
+          int32_t& rd = reader[gid(mv[m].ep_rank, (int64_t)mv[m].ep_page * kappa + g)];
+          if (rd >= 0) return MOEBIUS_E_INVAL;  // source page listed twice
+          rd = m;
+        }
+      } else {
+        for (int g = 0; g < x->G; ++g) {
+          int32_t& rd = reader[gid((int)tp_src_rank((uint32_t)g, (uint32_t)x->rep, mv[m].ep_rank), mv[m].tp_page)];
+          if (rd >= 0) return MOEBIUS_E_INVAL;
+          rd = m;
+        }
+      }
+    }
+    blockers.assign(nm, {});
+    dependents.assign(nm, {});
+    for (int m = 0; m < nm; ++m) {
+      auto& bl = blockers[m];
+      auto note = [&](int32_t b) {
+        if (b < 0) return;
+        if (b == m) { mv[m].staged = 1; return; }  // a move whose target overlaps its own source
+        bl.push_back(b);
+      };
+      if (e2t) for (int j = 0; j < R; ++j) note(reader[gid(j, mv[m].tp_page)]);
+      else     for (int g = 0; g < kappa; ++g) note(reader[gid(mv[m].ep_rank, (int64_t)mv[m].ep_page * kappa + g)]);
+      std::sort(bl.begin(), bl.end());
+      bl.erase(std::unique(bl.begin(), bl.end()), bl.end());
+      for (int32_t b : bl) dependents[b].push_back(m);
+    }
+    // Level the DAG of direct moves; a staged move is read in round 0 and written in the last round.
+    for (int pass = 0; pass < 8; ++pass) {
+      std::vector<int32_t> indeg(nm, 0), queue;
+      std::vector<uint8_t> done(nm, 0);
+      for (int m = 0; m < nm; ++m) {
+        mv[m].level = 0;
+        if (mv[m].staged) { done[m] = 1; continue; }
+        for (int32_t b : blockers[m]) {
+          if (mv[b].staged) mv[m].level = 1; else indeg[m]++;
+        }
+      }
+      for (int m = 0; m < nm; ++m) if (!done[m] && indeg[m] == 0) queue.push_back(m);
+      size_t qh = 0;
+      int scan = 0, resolved = 0, n_direct = 0;
+      for (int m = 0; m < nm; ++m) n_direct += !mv[m].staged;
+      std::vector<int32_t> stamp(nm, -1);
+      int32_t walk_id = 0;
+      auto release = [&](int m, int lvl) {
+        for (int32_t d : dependents[m]) {
+          if (done[d] || mv[d].staged) continue;
+          mv[d].level = std::max(mv[d].level, lvl);
+          if (--indeg[d] == 0) queue.push_back(d);
+        }
+      };
+      while (resolved < n_direct) {
+        if (qh < queue.size()) {
+          int m = queue[qh++];
+          done[m] = 1; ++resolved;
+          release(m, mv[m].level + 1);
+          continue;
+        }
+        // only cycles (and what sits behind them) are left: walk blockers to find a node ON a cycle
+        while (scan < nm && done[scan]) ++scan;
+        int v = scan;
+        ++walk_id;
+        for (;;) {
+          if (stamp[v] == walk_id) break;
+          stamp[v] = walk_id;
+          int nxt = -1;
+          for (int32_t b : blockers[v]) if (!done[b] && !mv[b].staged) { nxt = b; break; }
+          v = nxt;  // exists: indeg[v] > 0
+        }
+        mv[v].staged = 1; done[v] = 1; --n_direct;
+        release(v, 1);
+      }
+      int maxlvl = 0;
+      for (int m = 0; m < nm; ++m) if (!mv[m].staged) maxlvl = std::max(maxlvl, mv[m].level);
+      if (maxlvl <= kMaxLevel) { K = maxlvl; break; }
+      for (int m = 0; m < nm; ++m) if (!mv[m].staged && mv[m].level > kMaxLevel) mv[m].staged = 1;
+      K = kMaxLevel;
+    }
+    for (int m = 0; m < nm; ++m) if (!mv[m].staged && mv[m].level > K) mv[m].staged = 1;  // pass limit hit
+    for (int m = 0; m < nm; ++m) if (mv[m].staged) mv[m].slot = n_staged++;
+  }
+  int pools_per_group = n_pools_all;
+  if (n_staged > 0) {
+    int64_t per_pool = (int64_t)n_staged * x->ep_page_bytes;
+    int64_t fit = x->staging_bytes / per_pool;
+    if (fit < 1) return MOEBIUS_E_STAGING;
+    pools_per_group = (int)std::min<int64_t>(fit, n_pools_all);
+    if (n_staged >= (1 << 24)) return MOEBIUS_E_STAGING;
+  }
+  const int n_pool_groups = nm > 0 ? (n_pools_all + pools_per_group - 1) / pools_per_group : 0;
+
+  // ---- build the plan ---------------------------------------------------------------------------
+  moebius_plan_t* P = new (std::nothrow) moebius_plan_t();
+  if (!P) return MOEBIUS_E_INVAL;
+  P->ctx = x; P->from = from; P->to = to; P->n_req = n_req;
+  P->image = nullptr; P->tbl_image = nullptr; P->pinned = false;
+  memset(&P->stats, 0, sizeof(P->stats));
+  P->stats.struct_size = sizeof(moebius_stats_t);
+  uint32_t next_ctr = 0;
+  auto fail = [&](int code) { moebius_plan_destroy(P); return code; };
+
+  // weights: one segment per (layer, matrix) object, chained in the direction-specific order
+  // ("EP->TP adopts the sequential order while TP->EP adopts the reverse order")
+  Chain cw, ck, cs;
+  if (R > 1) {
+    int prev_ctr = -1; uint32_t prev_units = 0;
+    for (int step = 0; step < 3 * L; ++step) {
+      int k = e2t ? step : 3 * L - 1 - step;
+      int m = k % 3;
+      Seg s = blank_seg();
+      s.kind = SEG_XPOSE;
+      s.ep_is_src = e2t;
+      s.n_groups = R;
+      s.rep = 1;
+      int64_t run = (m < 2) ? (int64_t)(c.I / R) * x->wb : (int64_t)(c.I / R) * c.H * x->wb;
+      s.rows_total = (m < 2) ? (uint32_t)(c.E / R) * c.H : (uint32_t)(c.E / R);
+      if (run > (1ll << 31)) return fail(MOEBIUS_E_INVAL);
+      s.run_bytes = (uint32_t)run;
+      if (run * R <= unit_bytes || run <= 4096) {
+        s.groups_per_unit = R;
+        s.chunk_bytes = (uint32_t)run;
+        s.chunks_per_run = 1;
+        s.rows_per_unit = (uint32_t)std::max<int64_t>(1, unit_bytes / (run * R));
+      } else {
+        s.groups_per_unit = 1;
+        s.chunk_bytes = pick_chunk(run, unit_bytes);
+        s.chunks_per_run = (uint32_t)(run / s.chunk_bytes);
+        s.rows_per_unit = s.chunks_per_run == 1 ? (uint32_t)std::max<int64_t>(1, unit_bytes / run) : 1;
+      }
+      s.row_blocks = (s.rows_total + s.rows_per_unit - 1) / s.rows_per_unit;
+      s.tp_off = x->w_off + (int64_t)k * x->S;
+      s.ep_off = x->w_off + (int64_t)(k + x->ep_shift) * x->S;
+      int64_t nu = (int64_t)R * s.row_blocks * (s.n_groups / s.groups_per_unit) * s.chunks_per_run;
+      if (nu > (1ll << 30)) return fail(MOEBIUS_E_INVAL);
+      s.n_units = (uint32_t)nu;
+      s.wait_ctr = prev_ctr; s.wait_target = prev_units;
+      s.signal_ctr = (int32_t)next_ctr++;
+      prev_ctr = s.signal_ctr; prev_units = s.n_units;
+      push_seg(cw, s);
+    }
+    int64_t all = (int64_t)3 * L * c.E * c.H * c.I * x->wb;
+    P->stats.w_relocated = P->stats.w_read = all;
+    P->stats.w_moved = all / R * (R - 1);
+  }
+
+  // fp8 block scales: TP and EP scale views live in disjoint fixed regions, so these are plain
+  // out-of-place 2-D copies with no hazard (reading A13)
+  if (c.w_dtype == MOEBIUS_FP8_E4M3_B128 && R > 1) {
+    const int HB = c.H / 128, IB = c.I / 128, EL = c.E / R;
+    for (int l = 0; l < L; ++l) for (int m = 0; m < 3; ++m) {
+      int64_t tp_within = 0, ep_within = 0;
+      for (int mm = 0; mm < m; ++mm) { tp_within += x->sg[mm].tp_bytes; ep_within += x->sg[mm].ep_bytes; }
+      int prev_hi = 0;
+      for (int j = 0; j < R; ++j) {
+        int lo, hi; scale_blocks(j, R, c.I, &lo, &hi);
+        int nb = hi - lo;
+        int a = e2t ? lo : std::max(lo, prev_hi);   // TP->EP: each EP block is read from its lowest holder
+        prev_hi = std::max(prev_hi, hi);
+        int take = hi - a;
+        if (take <= 0) continue;
+        for (int q = 0; q < R; ++q) {
+          C2dDesc d;
+          int64_t tp_base = (int64_t)j * x->rank_stride + x->scale_tp_off + l * x->scale_tp_layer + tp_within;
+          int64_t ep_base = (int64_t)q * x->rank_stride + x->scale_ep_off + l * x->scale_ep_layer + ep_within;
+          int64_t tp_o, ep_o; uint32_t rows, run, tp_st, ep_st;
+          if (m < 2) {   // TP [E, HB, nb] ; EP [EL, HB, IB]; rows = (e', hb)
+            rows = (uint32_t)EL * HB; run = (uint32_t)take * 4;
+            tp_st = (uint32_t)nb * 4; ep_st = (uint32_t)IB * 4;
+            tp_o = tp_base + ((int64_t)q * EL * HB * nb + (a - lo)) * 4;
+            ep_o = ep_base + (int64_t)a * 4;
+          } else {       // TP [E, nb, HB] ; EP [EL, IB, HB]; rows = e'
+            rows = (uint32_t)EL; run = (uint32_t)take * HB * 4;
+            tp_st = (uint32_t)nb * HB * 4; ep_st = (uint32_t)IB * HB * 4;
+            tp_o = tp_base + ((int64_t)q * EL * nb + (a - lo)) * HB * 4;
+            ep_o = ep_base + (int64_t)a * HB * 4;
+          }
+          d.rows = rows; d.run_bytes = run;
+          if (e2t) { d.src_off = ep_o; d.dst_off = tp_o; d.src_stride = ep_st; d.dst_stride = tp_st; }
+          else     { d.src_off = tp_o; d.dst_off = ep_o; d.src_stride = tp_st; d.dst_stride = ep_st; }
+          P->c2d.push_back(d);
+          int64_t bytes = (int64_t)rows * run;
+          P->stats.w_relocated += bytes; P->stats.w_read += bytes;
+          if (q != j) P->stats.w_moved += bytes;
+        }
+      }
+    }
+    Seg s = blank_seg();
+    s.kind = SEG_COPY2D;
+    s.desc_begin = 0;
+    s.n_desc = (uint32_t)P->c2d.size();
+    s.n_units = s.n_desc;
+    push_seg(cs, s);
+  }
+
+  // KV: descriptors ordered [level 0][level 1]...[level K][staged]
+  if (nm > 0) {
+    std::vector<uint32_t> lvl_begin(K + 2, 0);
+    for (int m = 0; m < nm; ++m) if (!mv[m].staged) lvl_begin[mv[m].level + 1]++;
+    for (int l = 0; l <= K; ++l) lvl_begin[l + 1] += lvl_begin[l];
+    const uint32_t n_direct = lvl_begin[K + 1];
+    P->kv.resize(nm);
+    std::vector<uint32_t> cur(lvl_begin.begin(), lvl_begin.end() - 1);
+    uint32_t scur = n_direct;
+    for (int m = 0; m < nm; ++m) {
+      KvDesc d;
+      d.ep_rank = mv[m].ep_rank; d.ep_page = mv[m].ep_page; d.tp_page = mv[m].tp_page;
+      d.ntok_slot = (uint32_t)mv[m].ntok | (mv[m].staged ? ((uint32_t)mv[m].slot << 8) : 0u);
+      if (mv[m].staged) P->kv[scur++] = d; else P->kv[cur[mv[m].level]++] = d;
+    }
+    uint32_t ppu = (uint32_t)std::max<int64_t>(1, std::min<int64_t>(unit_bytes / x->ep_page_bytes, 2));
+    auto kv_seg = [&](uint32_t mode, uint32_t ep_src, uint32_t d0, uint32_t nd, int pool0, int npool) {
+      Seg s = blank_seg();
+      s.kind = SEG_KV;
+      s.kv_mode = mode;
+      s.ep_is_src = ep_src;
+      s.run_bytes = (uint32_t)x->run_kv;
+      s.n_groups = (uint32_t)x->G;
+      s.rep = (uint32_t)x->rep;
+      s.ep_off = s.tp_off = x->kv_off;
+      s.desc_begin = d0; s.n_desc = nd;
+      s.pool_begin = (uint32_t)pool0; s.n_pools = (uint32_t)npool;
+      s.pools_per_unit = std::min<uint32_t>(ppu, (uint32_t)npool);
+      s.ep_page_bytes = (uint32_t)x->ep_page_bytes;
+      s.tp_page_bytes = (uint32_t)x->tp_page_bytes;
+      s.pool_bytes = x->pool_bytes;
+      s.stg_pool_begin = (uint32_t)pool0;
+      s.stg_pools = (uint32_t)npool;
+      uint32_t pool_blocks = (s.n_pools + s.pools_per_unit - 1) / s.pools_per_unit;
+      s.n_units = nd * pool_blocks;
+      return s;
+    };
+    // a round = every segment that signals the same counter; the next round waits for all of them
+    const int64_t kv_units_est = (int64_t)nm * ((n_pools_all + ppu - 1) / ppu);
+    const int64_t slice_units = std::max<int64_t>(8192, kv_units_est / std::max(1, 3 * L));
+    int prev_ctr = -1; uint32_t prev_total = 0;
+    for (int g = 0; g < n_pool_groups; ++g) {
+      int pool0 = g * pools_per_group;
+      int npool = std::min(pools_per_group, n_pools_all - pool0);
+      for (int round = 0; round <= K + 1; ++round) {
+        std::vector<Seg> parts;
+        if (round == 0 && n_staged)      // save staged sources: EP->TP copies the EP page, TP->EP gathers into the slot
+          parts.push_back(kv_seg(e2t ? KV_STG_COPY : KV_MOVE_STG, e2t ? 1u : 0u, n_direct, (uint32_t)n_staged, pool0, npool));
+        if (round <= K && lvl_begin[round + 1] > lvl_begin[round])
+          parts.push_back(kv_seg(KV_MOVE, e2t ? 1u : 0u, lvl_begin[round], lvl_begin[round + 1] - lvl_begin[round], pool0, npool));
+        if (round == K + 1 && n_staged)  // every source has been read by now
+          parts.push_back(kv_seg(e2t ? KV_MOVE_STG : KV_STG_COPY, e2t ? 1u : 0u, n_direct, (uint32_t)n_staged, pool0, npool));
+        uint32_t total = 0;
+        for (auto& s : parts) total += s.n_units;
+        if (!total) continue;
+        if (next_ctr >= (uint32_t)kMaxCounters) return fail(MOEBIUS_E_STAGING);
+        int ctr = (int)next_ctr++;
+        for (auto& s : parts) {
+          // slice long segments so they interleave with the weight chain (drains of one hide behind the other)
+          uint32_t pool_blocks = (s.n_pools + s.pools_per_unit - 1) / s.pools_per_unit;
+          uint32_t desc_per_slice = (uint32_t)std::max<int64_t>(1, slice_units / pool_blocks);
+          for (uint32_t d0 = 0; d0 < s.n_desc; d0 += desc_per_slice) {
+            Seg t = s;
+            t.desc_begin = s.desc_begin + d0;
+            t.n_desc = std::min(desc_per_slice, s.n_desc - d0);
+            t.n_units = t.n_desc * pool_blocks;
+            t.wait_ctr = prev_ctr; t.wait_target = prev_total;
+            t.signal_ctr = ctr;
+            push_seg(ck, t);
+          }
+        }
+        prev_ctr = ctr; prev_total = total;
+      }
+    }
+    // accounting (reading A15): per pool, per move
+    for (int m = 0; m < nm; ++m) {
+      int64_t row = (int64_t)mv[m].ntok * x->run_kv;     // one group's bytes of this page
+      if (e2t) {
+        P->stats.kv_read += row * x->G;
+        P->stats.kv_relocated += row * x->G * x->rep;
+        P->stats.kv_moved += row * (x->G * x->rep - 1);  // the owner's own shard stays on its rank
+      } else {
+        P->stats.kv_read += row * x->G;
+        P->stats.kv_relocated += row * x->G;
+        P->stats.kv_moved += row * (x->G - 1);           // the new owner always holds one group itself
+      }
+    }
+    P->stats.kv_read *= n_pools_all; P->stats.kv_relocated *= n_pools_all; P->stats.kv_moved *= n_pools_all;
+  }
+
+  // merge the chains by fractional position (each keeps its own order)
+  struct Item { double pos; int chain; size_t idx; };
+  std::vector<Item> items;
+  auto add_chain = [&](Chain& ch, int id) {
+    int64_t acc = 0;
+    for (size_t i = 0; i < ch.segs.size(); ++i) {
+      items.push_back({ch.units ? (acc + 0.5 * ch.segs[i].n_units) / (double)ch.units : 0.0, id, i});
+      acc += ch.segs[i].n_units;
+    }
+  };
+  add_chain(cs, 0); add_chain(cw, 1); add_chain(ck, 2);
+  std::stable_sort(items.begin(), items.end(), [](const Item& a, const Item& b) {
+    if (a.chain == 0 || b.chain == 0) return a.chain == 0 && b.chain != 0;
+    return a.pos < b.pos;
+  });
+  uint64_t ub = 0;
+  for (auto& it : items) {
+    Seg s = (it.chain == 0 ? cs : it.chain == 1 ? cw : ck).segs[it.idx];
+    s.unit_begin = (uint32_t)ub;
+    ub += s.n_units;
+    P->segs.push_back(s);
+  }
+  if (ub >= (1ull << 32) || P->segs.size() > (size_t)kMaxSegs || P->kv.size() > (size_t)x->max_kv_desc + 0 ||
+      P->c2d.size() > (size_t)x->max_c2d)
+    return fail(MOEBIUS_E_INVAL);
+  P->total_units = (uint32_t)ub;
+  P->n_counters = next_ctr;
+
+  // ---- target request state + upload images -----------------------------------------------------
+  P->lens.assign(seq_lens, seq_lens + n_req);
+  P->owner = owner;
+  P->bt = bt;
+  int64_t seg_b = align_up((int64_t)P->segs.size() * sizeof(Seg), 256);
+  int64_t kv_b = align_up((int64_t)P->kv.size() * sizeof(KvDesc), 256);
+  int64_t c2d_b = align_up((int64_t)P->c2d.size() * sizeof(C2dDesc), 256);
+  P->kv_img_off = seg_b;
+  P->c2d_img_off = seg_b + kv_b;
+  P->image_bytes = seg_b + kv_b + c2d_b;
+  P->tbl_bytes = 4 * ((int64_t)kTblHdrInts + 2 * (int64_t)c.max_requests + (int64_t)n_req * MP);
+  P->image = (char*)host_alloc(P->image_bytes + P->tbl_bytes + 256, &P->pinned);
+  if (!P->image) return fail(MOEBIUS_E_INVAL);
+  memset(P->image, 0, (size_t)(P->image_bytes + P->tbl_bytes + 256));
+  if (!P->segs.empty()) memcpy(P->image, P->segs.data(), P->segs.size() * sizeof(Seg));
+  if (!P->kv.empty()) memcpy(P->image + P->kv_img_off, P->kv.data(), P->kv.size() * sizeof(KvDesc));
+  if (!P->c2d.empty()) memcpy(P->image + P->c2d_img_off, P->c2d.data(), P->c2d.size() * sizeof(C2dDesc));
+  P->tbl_image = (int32_t*)(P->image + align_up(P->image_bytes, 256));
+  int32_t* T = P->tbl_image;
+  T[0] = to; T[1] = n_req; T[2] = c.max_requests; T[3] = MP;
+  for (int i = 0; i < c.max_requests; ++i) { T[kTblHdrInts + i] = -1; T[kTblHdrInts + c.max_requests + i] = 0; }
+  for (int i = 0; i < n_req; ++i) { T[kTblHdrInts + i] = owner[i]; T[kTblHdrInts + c.max_requests + i] = seq_lens[i]; }
+  if (n_req) memcpy(T + kTblHdrInts + 2 * c.max_requests, bt.data(), (size_t)n_req * MP * 4);
+
+  P->stats.n_segments = (int32_t)P->segs.size();
+  P->stats.n_kv_moves = nm;
+  P->stats.n_kv_rounds = nm ? K + 1 + (n_staged ? 1 : 0) : 0;
+  P->stats.n_kv_staged = n_staged;
+  P->stats.n_pool_groups = n_pool_groups;
+  P->stats.n_units = (int64_t)ub;
+  P->stats.staging_used_bytes = (int64_t)n_staged * x->ep_page_bytes * (n_staged ? pools_per_group : 0);
+  P->stats.desc_upload_bytes = P->image_bytes;
+  P->stats.table_upload_bytes = P->tbl_bytes;
+  *out = P;
+  return MOEBIUS_OK;
+}
+
+extern "C" int moebius_block_tables(const moebius_plan_t* p, int32_t* dst_owner, int32_t* dst_bt) {
+  if (!p) return MOEBIUS_E_INVAL;
+  if (dst_owner && p->n_req) memcpy(dst_owner, p->owner.data(), (size_t)p->n_req * 4);
+  if (dst_bt && p->n_req) memcpy(dst_bt, p->bt.data(), p->bt.size() * 4);
+  return MOEBIUS_OK;
+}
+
+extern "C" int moebius_plan_stats(const moebius_plan_t* p, moebius_stats_t* o) {
+  if (!p || !o || o->struct_size != sizeof(moebius_stats_t)) return MOEBIUS_E_INVAL;
+  *o = p->stats;
+  return MOEBIUS_OK;
+}
+
+extern "C" int moebius_plan_export(const moebius_plan_t* p, int what, void* buf, int64_t cap, int64_t* needed) {
+  if (!p || !needed) return MOEBIUS_E_INVAL;
+  const void* src; int64_t n;
+  switch (what) {
+    case 0: src = p->segs.data(); n = (int64_t)p->segs.size() * sizeof(Seg); break;
+    case 1: src = p->kv.data();   n = (int64_t)p->kv.size() * sizeof(KvDesc); break;
+    case 2: src = p->c2d.data();  n = (int64_t)p->c2d.size() * sizeof(C2dDesc); break;
+    default: return MOEBIUS_E_INVAL;
+  }
+  *needed = n;
+  if (buf && cap >= n && n) memcpy(buf, src, (size_t)n);
+  return MOEBIUS_OK;
+}

@@ -1,0 +1,195 @@
+// moebius_units.h -- work-list format and unit decode, shared by the host planner and the sm_100a
+// kernel (both are the product; the CPU oracle under oracle/ shares nothing with this file).
+//
+// A plan is an ordered list of SEGMENTS; a segment is n_units independent work UNITS of one kind;
+// a unit is what one warp executes.  Units are handed out in list order by one global ticket.
+// A segment may WAIT on a completion counter (all units that signal that counter have finished)
+// and may SIGNAL one.  Dependencies always point backwards in list order, so in-order hand-out is
+// deadlock-free whatever the number of resident warps.
+//
+// Every data move is one of three shapes:
+//   XBOX  "run transposition": an EP-side block [rows][J runs][cc*16 B] that is contiguous per row,
+//         against J TP-side blocks [rows][cc*16 B], one per group (each on `rep` ranks).  This is
+//         the paper's owner-changed slice: expert weights (rank q's EP row holds
+//         the R TP shards of that row side by side) and KV pages (an EP page row
+//         = one token's G head groups side by side; a TP page row = one group).
+//   LIN   contiguous copy (KV page <-> staging slot).
+//   C2D   small 2-D strided copy in 4-byte elements (fp8 block scales).
+#ifndef MOEBIUS_UNITS_H_
+#define MOEBIUS_UNITS_H_
+
+#include <stdint.h>
+
+#if defined(__CUDACC__)
+#define MB_HD __host__ __device__ __forceinline__
+#else
+#define MB_HD inline
+#endif
+
+namespace moebius {
+
+enum : uint32_t { SEG_XPOSE = 0, SEG_KV = 1, SEG_COPY2D = 2 };
+enum : uint32_t { KV_MOVE = 0, KV_MOVE_STG = 1, KV_STG_COPY = 2 };
+
+struct Seg {              // 128 bytes, uploaded verbatim
+  uint32_t kind;
+  uint32_t ep_is_src;     // 1: EP side is read, TP side written (EP->TP); 0: the reverse
+  int32_t  wait_ctr;      // -1: none
+  uint32_t wait_target;
+  int32_t  signal_ctr;    // -1: none
+  uint32_t unit_begin;    // global id of this segment's first unit
+  uint32_t n_units;
+  uint32_t run_bytes;     // one group's contiguous piece of an EP row (= TP row)
+  uint32_t n_groups;      // runs per EP row: R (weights) or G = min(kv_heads, R) (KV)
+  uint32_t rep;           // TP ranks per group: 1 (weights) or max(1, R/kv_heads) (KV)
+  uint32_t rows_per_unit;
+  uint32_t groups_per_unit;  // n_groups, or 1 when a run is split into chunks
+  uint32_t chunk_bytes;      // bytes of a run one unit handles (== run_bytes unless chunked)
+  uint32_t chunks_per_run;
+  uint32_t rows_total;       // XPOSE: rows per EP rank (E/R*H for gate/up, E/R for down)
+  uint32_t row_blocks;       // XPOSE: ceil(rows_total / rows_per_unit)
+  int64_t  ep_off;           // XPOSE: EP view offset in the rank region; KV: pool 0 offset
+  int64_t  tp_off;           // XPOSE: TP view offset in the rank region; KV: == ep_off
+  uint32_t kv_mode;
+  uint32_t desc_begin;       // first descriptor (KV move or C2D) of this segment
+  uint32_t n_desc;
+  uint32_t pool_begin;       // KV: first pool (z = 2*layer + {K:0,V:1}) of this segment
+  uint32_t n_pools;
+  uint32_t pools_per_unit;
+  uint32_t ep_page_bytes;
+  uint32_t tp_page_bytes;
+  int64_t  pool_bytes;
+  uint32_t stg_pool_begin;   // KV staging: slot s, pool z lives at ((s*stg_pools)+(z-stg_pool_begin))*ep_page_bytes
+  uint32_t stg_pools;
+};
+static_assert(sizeof(Seg) == 128, "Seg must be 128 bytes");
+
+struct KvDesc {           // 16 bytes: one (request, block) page move, layer- and K/V-agnostic
+  int32_t  ep_rank;       // EP-side owner of the request (one index vector for all layers)
+  int32_t  ep_page;       // EP page id in that rank's pool
+  int32_t  tp_page;       // TP page id (same on every rank)
+  uint32_t ntok_slot;     // bits 0..7: valid tokens in the page (1..page_tokens <= 255);
+                          // bits 8..31: staging slot (KV_MOVE_STG / KV_STG_COPY segments only)
+};
+static_assert(sizeof(KvDesc) == 16, "KvDesc must be 16 bytes");
+
+struct C2dDesc {          // 32 bytes: rows x run_bytes, 4-byte elements, offsets from dev_base
+  int64_t  src_off, dst_off;
+  uint32_t rows, run_bytes, src_stride, dst_stride;
+};
+static_assert(sizeof(C2dDesc) == 32, "C2dDesc must be 32 bytes");
+
+struct DevParams {        // kernel arguments
+  char*            base;
+  char*            stg;
+  const Seg*       segs;
+  const KvDesc* kv;
+  const C2dDesc*   c2d;
+  uint32_t*        ticket;
+  uint32_t*        counters;
+  int64_t          rank_stride;
+  uint32_t         n_segs;
+  uint32_t         total_units;
+};
+
+// One executable shape.  lin != 0: contiguous copy of lin_bytes from src to dst.
+struct Box {
+  char*    ep;            // EP-side row 0 (first group / chunk of this unit)
+  char*    tp;            // TP-side row 0 at rank 0; add rank*rank_stride
+  uint32_t ep_row_stride, tp_row_stride;
+  uint32_t nrows, J, g0, cc;   // cc = 16-byte chunks per (row, group)
+  uint32_t run_bytes, rep;
+  int32_t  owner;         // TP->EP source rule: group g is read from `owner` if it holds g, else
+                          // from the lowest-rank holder g*rep (reading A5); -1: rank g
+  uint32_t lin;
+  char    *lin_src, *lin_dst;
+  uint64_t lin_bytes;
+};
+
+MB_HD uint32_t seg_boxes(const Seg& s, uint32_t u) {
+  if (s.kind != SEG_KV) return 1;
+  uint32_t pool_blocks = (s.n_pools + s.pools_per_unit - 1) / s.pools_per_unit;
+  uint32_t pb = u % pool_blocks;
+  uint32_t z0 = pb * s.pools_per_unit;
+  uint32_t n = s.n_pools - z0;
+  return n < s.pools_per_unit ? n : s.pools_per_unit;
+}
+
+// TP rank that holds the copy of group g that is READ in a TP->EP move.
+MB_HD uint32_t tp_src_rank(uint32_t g, uint32_t rep, int32_t owner) {
+  if (owner >= 0 && (uint32_t)owner / rep == g) return (uint32_t)owner;
+  return g * rep;
+}
+
+// Decode box k of unit u (u is LOCAL to the segment).
+MB_HD void decode_box(const Seg& s, const DevParams& p, uint32_t u, uint32_t k, Box& b) {
+  b.lin = 0;
+  b.run_bytes = s.run_bytes;
+  b.rep = s.rep;
+  b.tp_row_stride = s.run_bytes;
+  if (s.kind == SEG_XPOSE) {
+    uint32_t ch = u % s.chunks_per_run;  u /= s.chunks_per_run;
+    uint32_t jgroups = s.n_groups / s.groups_per_unit;
+    uint32_t jg = u % jgroups;           u /= jgroups;
+    uint32_t rb = u % s.row_blocks;      uint32_t q = u / s.row_blocks;
+    uint32_t row0 = rb * s.rows_per_unit;
+    uint32_t nrows = s.rows_total - row0;
+    if (nrows > s.rows_per_unit) nrows = s.rows_per_unit;
+    b.nrows = nrows;
+    b.J = s.groups_per_unit;
+    b.g0 = jg * s.groups_per_unit;
+    b.cc = s.chunk_bytes >> 4;
+    b.owner = -1;
+    b.ep_row_stride = s.n_groups * s.run_bytes;
+    int64_t ep = (int64_t)q * p.rank_stride + s.ep_off +
+                 ((int64_t)row0 * s.n_groups + b.g0) * s.run_bytes + (int64_t)ch * s.chunk_bytes;
+    int64_t tp = s.tp_off + ((int64_t)q * s.rows_total + row0) * s.run_bytes + (int64_t)ch * s.chunk_bytes;
+    b.ep = p.base + ep;
+    b.tp = p.base + tp;
+    return;
+  }
+  // SEG_KV
+  uint32_t pool_blocks = (s.n_pools + s.pools_per_unit - 1) / s.pools_per_unit;
+  uint32_t pb = u % pool_blocks;
+  uint32_t di = u / pool_blocks;
+  uint32_t z = s.pool_begin + pb * s.pools_per_unit + k;
+  KvDesc d = p.kv[s.desc_begin + di];
+  uint32_t ntok = d.ntok_slot & 0xFFu;
+  uint32_t slot = d.ntok_slot >> 8;
+  int64_t pool = s.ep_off + (int64_t)z * s.pool_bytes;
+  char* ep_pool = p.base + (int64_t)d.ep_rank * p.rank_stride + pool + (int64_t)d.ep_page * s.ep_page_bytes;
+  char* ep_stg = p.stg + ((int64_t)slot * s.stg_pools + (z - s.stg_pool_begin)) * (int64_t)s.ep_page_bytes;
+  uint32_t row_bytes = s.n_groups * s.run_bytes;
+  if (s.kv_mode == KV_STG_COPY) {
+    b.lin = 1;
+    b.lin_bytes = (uint64_t)ntok * row_bytes;
+    // ep_is_src: the pool page is saved into its staging slot; else the slot is written back
+    b.lin_src = s.ep_is_src ? ep_pool : ep_stg;
+    b.lin_dst = s.ep_is_src ? ep_stg : ep_pool;
+    return;
+  }
+  b.ep = (s.kv_mode == KV_MOVE_STG) ? ep_stg : ep_pool;
+  b.tp = p.base + pool + (int64_t)d.tp_page * s.tp_page_bytes;
+  b.ep_row_stride = row_bytes;
+  b.nrows = ntok;
+  b.J = s.n_groups;
+  b.g0 = 0;
+  b.cc = s.run_bytes >> 4;
+  b.owner = d.ep_rank;
+}
+
+// Addresses of 16-byte chunk idx of a box (idx < nrows*J*cc, EP-side linear order).
+// tp_rel excludes the rank term; the caller adds rank*rank_stride.
+MB_HD void box_chunk(const Box& b, uint32_t idx, char*& ep, char*& tp_rel, uint32_t& group) {
+  uint32_t per_row = b.J * b.cc;
+  uint32_t t = idx / per_row;
+  uint32_t rem = idx - t * per_row;
+  uint32_t jj = rem / b.cc;
+  uint32_t c = rem - jj * b.cc;
+  ep = b.ep + (int64_t)t * b.ep_row_stride + (int64_t)jj * b.run_bytes + ((int64_t)c << 4);
+  tp_rel = b.tp + (int64_t)t * b.tp_row_stride + ((int64_t)c << 4);
+  group = b.g0 + jj;
+}
+
+}  // namespace moebius
+#endif  // MOEBIUS_UNITS_H_

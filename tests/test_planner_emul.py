@@ -1,0 +1,204 @@
+"""CPU tests of the product's host planner + unit decode through the test-only host emulator.
+The emulator executes the exported work list with the product's own decode code on host memory and
+checks every access against the ordering the device counters enforce; the result is compared with
+the oracle bytewise.  (Device execution itself is covered by the -m gpu tests.)"""
+import numpy as np
+import pytest
+
+import workloads as wl
+from harness import (EP, TP, OracleLayout, State, emulate, expected_bytes, expected_target, mb, mb_config,
+                     source_tables)
+
+
+def run_switch(st, sess, image, staging, from_mode, src_owner, src_bt):
+    to_mode = EP if from_mode == TP else TP
+    plan = sess.plan(to_mode, st.lens, src_owner, src_bt, from_mode=from_mode)
+    stats = mb.moebius_plan_stats(plan).as_dict()
+    owner, bt = sess.block_tables(plan, len(st.lens))
+    want_owner, want_bt = expected_target(st, sess, to_mode)
+    if to_mode == EP:
+        assert np.array_equal(owner, want_owner)
+    else:
+        assert np.all(owner == -1)
+    assert np.array_equal(bt, want_bt)
+    res = emulate(sess, plan, image, staging)
+    assert res["violations"] == 0 and res["oob"] == 0 and res["bad_wait"] == 0 and res["bad_begin"] == 0, res
+    assert res["units"] == stats["n_units"]
+    # byte accounting == oracle enumeration ("moves only the owner-changed bytes")
+    ep_owner = src_owner if from_mode == EP else owner
+    w, k = expected_bytes(st, from_mode, ep_owner)
+    if st.cfg.w_dtype != "fp8_e4m3_b128":
+        assert (stats["w_moved"], stats["w_relocated"], stats["w_read"]) == (w["moved"], w["relocated"], w["read"])
+    assert (stats["kv_moved"], stats["kv_relocated"], stats["kv_read"]) == (k["moved"], k["relocated"], k["read"])
+    direct_bytes = stats["w_relocated"] + stats["kv_relocated"]
+    staged_extra = res["bytes_written"] - direct_bytes
+    assert staged_extra >= 0
+    if stats["n_kv_staged"] == 0:
+        assert res["bytes_written"] == direct_bytes and res["bytes_read"] == stats["w_read"] + stats["kv_read"]
+    tgt = OracleLayout(st, sess, to_mode, want_owner, want_bt)
+    bad = tgt.compare(image)
+    assert not bad, bad[:5]
+    sess.free_plan(plan)
+    return to_mode, (want_owner if to_mode == EP else None), want_bt, stats
+
+
+def make(cfg, lens=None, policy=None, cap_frac=0.0, pool_bytes=None):
+    st = State(cfg, lens)
+    sess = mb.Session(mb_config(cfg, st.lens, policy, cap_frac, pool_bytes))
+    image = np.zeros(sess.layout.base_bytes, np.uint8)
+    image[:] = 0xA5
+    staging = np.full(max(sess.layout.staging_bytes, 16), 0x5A, np.uint8)
+    return st, sess, image, staging
+
+
+@pytest.mark.parametrize("src", ["canonical", "random"])
+def test_tiny_round_trip(src):
+    """TP -> EP -> TP on the tiny config: every view bit-exact after each switch, and the final TP
+    bytes equal the initial ones on every valid byte."""
+    st, sess, image, staging = make(wl.get_config("tiny"))
+    owner, bt = source_tables(st, sess, TP, src)
+    OracleLayout(st, sess, TP, owner, bt).place(image)
+    mode, owner, bt, s1 = run_switch(st, sess, image, staging, TP, owner, bt)
+    assert mode == EP
+    mode, owner, bt, s2 = run_switch(st, sess, image, staging, EP, owner, bt)
+    assert mode == TP
+    assert s1["w_moved"] == s2["w_moved"] == 49152  # (1 - 1/2) * 3 * 8*64*32*2 bytes
+
+
+SMALLISH = wl.get_config("small").with_(L=2, H=128, I=256, n_req=24, len_dist=("uniform", 1, 200), seed=77)
+
+
+@pytest.mark.parametrize("first", [TP, EP])
+@pytest.mark.parametrize("src", ["canonical", "random"])
+def test_smallish_alternating(first, src):
+    st, sess, image, staging = make(SMALLISH)
+    mode = first
+    owner, bt = source_tables(st, sess, mode, src)
+    OracleLayout(st, sess, mode, owner, bt).place(image)
+    for _ in range(3):
+        mode, owner, bt, stats = run_switch(st, sess, image, staging, mode, owner, bt)
+
+
+@pytest.mark.parametrize("R,Hkv", [(8, 4), (4, 4), (2, 8), (4, 1), (1, 2)])
+def test_head_geometries(R, Hkv):
+    """Replicated heads (Qwen3 4 heads on 8 ranks), Hkv == R (Fig. 8(b)), several
+    heads per rank, a single head, and R = 1 (empty weight plan)."""
+    cfg = wl.get_config("tiny").with_(R=R, E=8, I=64, kv_heads=Hkv, n_req=7, len_dist=("uniform", 1, 70), seed=5 + R)
+    st, sess, image, staging = make(cfg)
+    owner, bt = source_tables(st, sess, TP, "random")
+    OracleLayout(st, sess, TP, owner, bt).place(image)
+    mode, owner, bt, s1 = run_switch(st, sess, image, staging, TP, owner, bt)
+    mode, owner, bt, s2 = run_switch(st, sess, image, staging, EP, owner, bt)
+    if R == 1:
+        assert s1["w_moved"] == 0 and s1["w_relocated"] == 0
+
+
+def test_weight_only_warmup_switch():
+    """n_req = 0: PAPER.md:199 'a weight-only warmup switch ... while no request is active'."""
+    st, sess, image, staging = make(wl.get_config("tiny"), lens=[])
+    OracleLayout(st, sess, TP, None, np.zeros((0, 1), np.int32)).place(image)
+    mode, owner, bt, s = run_switch(st, sess, image, staging, TP, None, np.zeros((0, 1), np.int32))
+    assert s["n_kv_moves"] == 0 and s["kv_moved"] == 0
+    run_switch(st, sess, image, staging, EP, np.zeros(0, np.int32), np.zeros((0, 1), np.int32))
+
+
+@pytest.mark.parametrize("first", [TP, EP])
+def test_tight_pool_rounds_and_staging(first):
+    """Tight pool: target pages overlap live source pages, so the plan needs dependency rounds and
+    staging (BASELINE.json: 'in-place permutation cycles through a bounded staging buffer')."""
+    cfg = SMALLISH.with_(L=1, n_req=40, seed=99)
+    lens = wl.draw_seq_lens(cfg)
+    seen_rounds = seen_staged = 0
+    for seed in range(3):
+        st, sess, image, staging = make(cfg, lens, "tight", cap_frac=0.5)
+        mode = first
+        owner, bt = source_tables(st, sess, mode, "random", seed=seed)
+        OracleLayout(st, sess, mode, owner, bt).place(image)
+        for _ in range(2):
+            mode, owner, bt, stats = run_switch(st, sess, image, staging, mode, owner, bt)
+            seen_rounds = max(seen_rounds, stats["n_kv_rounds"])
+            seen_staged = max(seen_staged, stats["n_kv_staged"])
+            assert stats["staging_used_bytes"] <= sess.layout.staging_bytes
+    assert seen_rounds > 2 and seen_staged > 0
+
+
+def test_staging_reused_across_pool_groups_and_too_small():
+    """When the staged pages of all 2L pools do not fit the staging buffer, the pools are processed
+    in groups that reuse it; when not even one pool fits, the plan fails with E_STAGING and the
+    caller cancels the switch (like a capacity failure)."""
+    cfg = SMALLISH.with_(L=2, n_req=40, seed=99)
+    lens = wl.draw_seq_lens(cfg)
+    st, sess, image, staging = make(cfg, lens, "tight", cap_frac=0.5)
+    owner, bt = source_tables(st, sess, TP, "random", seed=1)
+    plan = sess.plan(EP, st.lens, owner, bt, from_mode=TP)
+    s = mb.moebius_plan_stats(plan).as_dict()
+    assert s["n_kv_staged"] > 0 and s["n_pool_groups"] == 1
+    per_pool = s["n_kv_staged"] * sess.layout.ep_page_bytes
+    spare = sess.layout.weight_spare_bytes
+    # room for one pool's staged pages only -> 2L = 4 groups
+    c = mb_config(cfg, lens, "tight")
+    c.staging_cap_bytes = spare + per_pool + sess.layout.ep_page_bytes
+    sess2 = mb.Session(c)
+    image = np.full(sess2.layout.base_bytes, 0xA5, np.uint8)
+    staging = np.full(sess2.layout.staging_bytes, 0x5A, np.uint8)
+    OracleLayout(st, sess2, TP, owner, bt).place(image)
+    mode, o2, bt2, stats = run_switch(st, sess2, image, staging, TP, owner, bt)
+    assert stats["n_pool_groups"] == 4 and stats["staging_used_bytes"] <= sess2.layout.staging_bytes
+    run_switch(st, sess2, image, staging, EP, o2, bt2)
+    # not even one pool fits
+    c.staging_cap_bytes = spare + per_pool - sess.layout.ep_page_bytes
+    sess3 = mb.Session(c)
+    with pytest.raises(mb.MoebiusError) as e:
+        sess3.plan(EP, st.lens, owner, bt, from_mode=TP)
+    assert e.value.status == -3
+    # cap below the spare weight slot itself
+    c.staging_cap_bytes = spare - 1
+    with pytest.raises(mb.MoebiusError) as e:
+        mb.Session(c)
+    assert e.value.status == -3
+
+
+def test_capacity_error_cancels_switch():
+    """TP replication halves capacity; a switch that does not fit is cancelled."""
+    cfg = wl.get_config("tiny").with_(R=4, I=64, kv_heads=2, n_req=6, len_dist=("uniform", 30, 64), seed=11)
+    lens = wl.draw_seq_lens(cfg)
+    pages = int(((lens + 15) // 16).sum())
+    ep_page = 16 * 2 * 16 * 2
+    # EP pools can hold every request of a rank, but the TP pool (same bytes, 2 heads on 4 ranks ->
+    # each rank stores a replicated head) cannot hold all requests
+    pool = ep_page * (pages // 2)
+    st = State(cfg, lens)
+    sess = mb.Session(mb_config(cfg, lens, pool_bytes=pool))
+    assert sess.layout.pages_tp == 2 * sess.layout.pages_ep and sess.layout.pages_tp < pages
+    owner, bt = source_tables(st, sess, EP, "canonical")
+    with pytest.raises(mb.MoebiusError) as e:
+        sess.plan(TP, st.lens, owner, bt, from_mode=EP)
+    assert e.value.status == -2
+
+
+def test_invalid_inputs():
+    cfg = wl.get_config("tiny")
+    lens = np.array([5, 20], np.int32)
+    sess = mb.Session(mb_config(cfg, lens))
+    bt = np.array([[0, -1], [1, 1]], np.int32)       # page 1 listed twice
+    with pytest.raises(mb.MoebiusError) as e:
+        sess.plan(EP, lens, None, bt, from_mode=TP)
+    assert e.value.status == -1
+    bt = np.array([[0, -1], [1, 9999]], np.int32)    # out of range
+    with pytest.raises(mb.MoebiusError):
+        sess.plan(EP, lens, None, bt, from_mode=TP)
+    with pytest.raises(mb.MoebiusError):             # from == to
+        sess.plan(TP, lens, None, bt, from_mode=TP)
+    for bad in (dict(I=30), dict(E=7), dict(kv_heads=3, R=2)):
+        with pytest.raises(mb.MoebiusError):
+            mb.Session(mb_config(cfg.with_(**bad), lens))
+
+
+def test_fp8_scales():
+    cfg = wl.get_config("fp8_graph").with_(L=1, E=8, H=256, I=1536, n_req=6, len_dist=("uniform", 1, 60), seed=3)
+    st, sess, image, staging = make(cfg)
+    st.fill = "normal"
+    owner, bt = source_tables(st, sess, TP, "random")
+    OracleLayout(st, sess, TP, owner, bt).place(image)
+    mode, owner, bt, s = run_switch(st, sess, image, staging, TP, owner, bt)
+    mode, owner, bt, s = run_switch(st, sess, image, staging, EP, owner, bt)

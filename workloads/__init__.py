@@ -13,5 +13,6 @@ from .gen import (  # noqa: F401
     gen_logical_weight,
     gen_logical_scale,
     random_page_tables,
+    kv_pool_bytes,
     tag_fill_u16,
 )

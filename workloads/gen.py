@@ -114,3 +114,29 @@ def random_page_tables(seq_lens, owner, n_ranks: int, n_pages: int, page: int, m
             bt[i, :need[i]] = perm[k:k + need[i]]
             k += need[i]
     return bt
+
+
+def kv_pool_bytes(cfg: Config, seq_lens, policy: str | None = None) -> int:
+    """Capacity of one K (or V) pool of one rank and layer (a workload parameter BASELINE.json
+    leaves open).  "roomy": 1.1 x (TP need + an upper bound of the largest EP
+    share), so source and target pages never have to overlap; "tight": 1.05 x TP need, which
+    forces dependency rounds and staging.  Rounded up to whole EP pages."""
+    policy = policy or cfg.pool_policy
+    seq_lens = np.asarray(seq_lens, dtype=np.int64)
+    b = cfg.kv_elem_bytes
+    hpr = max(1, cfg.kv_heads // cfg.R)
+    tp_page = cfg.page * hpr * cfg.head_dim * b
+    ep_page = cfg.page * cfg.kv_heads * cfg.head_dim * b
+    pages = (seq_lens + cfg.page - 1) // cfg.page
+    total = int(pages.sum())
+    biggest = int(pages.max()) if len(pages) else 0
+    tp_need = total * tp_page
+    ep_share = (-(-total // cfg.R) + biggest) * ep_page   # LPT bound on the fullest rank
+    if policy == "roomy":
+        need = 1.1 * (tp_need + ep_share)
+    elif policy == "tight":
+        need = max(1.05 * tp_need, ep_share)
+    else:
+        raise ValueError(policy)
+    n_pages = max(1, int(-(-need // ep_page)))
+    return n_pages * ep_page
