@@ -188,6 +188,9 @@ MOEBIUS_API int moebius_reshard(moebius_ctx_t* ctx, const moebius_plan_t* plan, 
  * synchronises on the end event).  Enabled with moebius_set_timing(ctx, 1). */
 MOEBIUS_API int moebius_set_timing(moebius_ctx_t* ctx, int enable);
 MOEBIUS_API int moebius_last_kernel_ms(moebius_ctx_t* ctx, float* ms);
+/* The same for the most recent calls (a ring of 64), oldest first.  out_ms: HOST float[cap];
+ * *n_out receives how many were written.  Synchronises on each end event. */
+MOEBIUS_API int moebius_kernel_ms_history(moebius_ctx_t* ctx, float* out_ms, int cap, int* n_out);
 
 /* Launch shape override for tuning: ctas_per_sm <= 0 and threads <= 0 restore the defaults. */
 MOEBIUS_API int moebius_set_launch(moebius_ctx_t* ctx, int ctas_per_sm, int threads, int unit_kb);

@@ -17,7 +17,7 @@ EXPORTED_SYMBOLS = [
     "moebius_create", "moebius_destroy", "moebius_layout", "moebius_view", "moebius_bind",
     "moebius_active_mode", "moebius_plan", "moebius_plan_destroy", "moebius_block_tables",
     "moebius_plan_stats", "moebius_plan_export", "moebius_reshard", "moebius_set_timing",
-    "moebius_last_kernel_ms", "moebius_set_launch", "moebius_status_str", "moebius_version",
+    "moebius_last_kernel_ms", "moebius_kernel_ms_history", "moebius_set_launch", "moebius_status_str", "moebius_version",
 ]
 
 
@@ -83,7 +83,7 @@ def lib_path() -> str:
 
 if not os.path.exists(_LIB):
     raise ImportError(
-        "libmoebius.so is not built (%s). Build it with `python -m paper_2606_26607_b200.build` "
+        "libmoebius.so is not built (%s). Build it with `python paper_2606_26607_b200/build.py` "
         "(nvcc, sm_100a). There is no CPU fallback." % _LIB)
 _lib = C.CDLL(_LIB)
 
@@ -105,6 +105,7 @@ _lib.moebius_plan_export.argtypes = [_vp, C.c_int, _vp, C.c_int64, C.POINTER(C.c
 _lib.moebius_reshard.argtypes = [_vp, _vp, _vp]
 _lib.moebius_set_timing.argtypes = [_vp, C.c_int]
 _lib.moebius_last_kernel_ms.argtypes = [_vp, C.POINTER(C.c_float)]
+_lib.moebius_kernel_ms_history.argtypes = [_vp, C.POINTER(C.c_float), C.c_int, C.POINTER(C.c_int)]
 _lib.moebius_set_launch.argtypes = [_vp, C.c_int, C.c_int, C.c_int]
 _lib.moebius_status_str.argtypes = [C.c_int]
 _lib.moebius_status_str.restype = C.c_char_p
@@ -222,6 +223,13 @@ def moebius_last_kernel_ms(ctx) -> float:
     ms = C.c_float(0)
     _chk(_lib.moebius_last_kernel_ms(ctx, C.byref(ms)), "moebius_last_kernel_ms")
     return ms.value
+
+
+def moebius_kernel_ms_history(ctx, cap: int = 64):
+    buf = (C.c_float * cap)()
+    n = C.c_int(0)
+    _chk(_lib.moebius_kernel_ms_history(ctx, buf, cap, C.byref(n)), "moebius_kernel_ms_history")
+    return [buf[i] for i in range(n.value)]
 
 
 def moebius_set_launch(ctx, ctas_per_sm: int = 0, threads: int = 0, unit_kb: int = 0):

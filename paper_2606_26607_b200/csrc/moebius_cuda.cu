@@ -188,8 +188,7 @@ void host_free(void* p, bool pinned) {
 
 void cuda_ctx_destroy(moebius_ctx* x) {
   if (x->ev_valid) {
-    cudaEventDestroy((cudaEvent_t)x->ev0);
-    cudaEventDestroy((cudaEvent_t)x->ev1);
+    for (int i = 0; i < 2 * kTimingRing; ++i) cudaEventDestroy((cudaEvent_t)x->ev[i]);
     x->ev_valid = false;
   }
 }
@@ -220,11 +219,26 @@ extern "C" int moebius_set_timing(moebius_ctx_t* x, int enable) {
   return MOEBIUS_OK;
 }
 
-extern "C" int moebius_last_kernel_ms(moebius_ctx_t* x, float* ms) {
-  if (!x || !ms || !x->ev_valid) return MOEBIUS_E_STATE;
-  if (cudaEventSynchronize((cudaEvent_t)x->ev1) != cudaSuccess) return MOEBIUS_E_CUDA;
-  if (cudaEventElapsedTime(ms, (cudaEvent_t)x->ev0, (cudaEvent_t)x->ev1) != cudaSuccess) return MOEBIUS_E_CUDA;
+extern "C" int moebius_kernel_ms_history(moebius_ctx_t* x, float* out_ms, int cap, int* n_out) {
+  if (!x || !out_ms || !n_out || cap < 0) return MOEBIUS_E_INVAL;
+  *n_out = 0;
+  if (!x->ev_valid || x->ev_count == 0) return MOEBIUS_E_STATE;
+  int64_t n = x->ev_count < kTimingRing ? x->ev_count : kTimingRing;
+  if (n > cap) n = cap;
+  for (int64_t i = 0; i < n; ++i) {
+    int64_t k = (x->ev_count - n + i) % kTimingRing;
+    cudaEvent_t a = (cudaEvent_t)x->ev[2 * k], b = (cudaEvent_t)x->ev[2 * k + 1];
+    if (cudaEventSynchronize(b) != cudaSuccess) return MOEBIUS_E_CUDA;
+    if (cudaEventElapsedTime(out_ms + i, a, b) != cudaSuccess) return MOEBIUS_E_CUDA;
+  }
+  *n_out = (int)n;
   return MOEBIUS_OK;
+}
+
+extern "C" int moebius_last_kernel_ms(moebius_ctx_t* x, float* ms) {
+  if (!x || !ms) return MOEBIUS_E_INVAL;
+  int n = 0;
+  return moebius_kernel_ms_history(x, ms, 1, &n);
 }
 
 extern "C" int moebius_reshard(moebius_ctx_t* x, const moebius_plan_t* P, void* cuda_stream) {
@@ -238,9 +252,17 @@ extern "C" int moebius_reshard(moebius_ctx_t* x, const moebius_plan_t* P, void* 
     x->n_sm = n;
   }
   if (x->timing && !x->ev_valid) {
-    cudaEvent_t a, b;
-    if (cudaEventCreate(&a) != cudaSuccess || cudaEventCreate(&b) != cudaSuccess) return MOEBIUS_E_CUDA;
-    x->ev0 = a; x->ev1 = b; x->ev_valid = true;
+    for (int i = 0; i < 2 * kTimingRing; ++i) {
+      cudaEvent_t e;
+      if (cudaEventCreate(&e) != cudaSuccess) return MOEBIUS_E_CUDA;
+      x->ev[i] = e;
+    }
+    x->ev_valid = true;
+  }
+  cudaEvent_t ev_a = nullptr, ev_b = nullptr;
+  if (x->timing) {
+    int64_t k = x->ev_count % kTimingRing;
+    ev_a = (cudaEvent_t)x->ev[2 * k]; ev_b = (cudaEvent_t)x->ev[2 * k + 1];
   }
   // 1. work list -> device; ticket and the counters this plan uses -> 0
   if (cudaMemsetAsync(x->desc, 0, (size_t)(kCtrOff + 4 * (int64_t)(P->n_counters ? P->n_counters : 1)), st) != cudaSuccess)
@@ -267,14 +289,15 @@ extern "C" int moebius_reshard(moebius_ctx_t* x, const moebius_plan_t* P, void* 
     int64_t grid = (int64_t)x->n_sm * per_sm;
     int64_t grid_cap = (warps_needed + threads / 32 - 1) / (threads / 32);
     if (grid > grid_cap) grid = grid_cap;
-    if (x->timing) cudaEventRecord((cudaEvent_t)x->ev0, st);
+    if (x->timing) cudaEventRecord(ev_a, st);
     moebius_reshard_kernel<<<(unsigned)grid, threads, 0, st>>>(p);
     if (cudaGetLastError() != cudaSuccess) return MOEBIUS_E_CUDA;
-    if (x->timing) cudaEventRecord((cudaEvent_t)x->ev1, st);
+    if (x->timing) cudaEventRecord(ev_b, st);
   } else if (x->timing) {
-    cudaEventRecord((cudaEvent_t)x->ev0, st);
-    cudaEventRecord((cudaEvent_t)x->ev1, st);
+    cudaEventRecord(ev_a, st);
+    cudaEventRecord(ev_b, st);
   }
+  if (x->timing) x->ev_count++;
   // 3. publish: new tables, owner vector and the active-mode flag at their fixed address
   if (cudaMemcpyAsync(x->tables, P->tbl_image, (size_t)P->tbl_bytes, cudaMemcpyHostToDevice, st) != cudaSuccess)
     return MOEBIUS_E_CUDA;

@@ -16,6 +16,7 @@ constexpr int64_t kHdrBytes = 256;                         // ticket lives at by
 constexpr int64_t kCtrOff = kHdrBytes;                     // uint32 counters[kMaxCounters]
 constexpr int64_t kSegOff = kCtrOff + 4 * kMaxCounters;    // Seg[...]
 constexpr int kTblHdrInts = 16;
+constexpr int kTimingRing = 64;
 
 struct ScaleGeom {           // fp8 block scales of one matrix kind (reading A13)
   int64_t tp_bytes;          // per rank, allocated with the largest nb over ranks
@@ -50,8 +51,8 @@ struct moebius_ctx {
   // device facts + timing (filled lazily by the CUDA side)
   int n_sm;
   int timing;
-  void* ev0;
-  void* ev1;
+  void* ev[2 * moebius::kTimingRing];   // event pairs (begin, end) round the kernel, a ring
+  int64_t ev_count;                     // pairs recorded so far
   bool ev_valid;
 };
 

@@ -141,7 +141,8 @@ int moebius_create(const moebius_config_t* c, moebius_ctx_t** out) {
   x->unit_kb = 0;
   x->n_sm = 0;
   x->timing = 0;
-  x->ev0 = x->ev1 = nullptr;
+  memset(x->ev, 0, sizeof(x->ev));
+  x->ev_count = 0;
   x->ev_valid = false;
   *out = x;
   return MOEBIUS_OK;
@@ -229,7 +230,7 @@ int moebius_active_mode(const moebius_ctx_t* x) { return x ? x->active_mode : MO
 
 int moebius_set_launch(moebius_ctx_t* x, int ctas_per_sm, int threads, int unit_kb) {
   if (!x) return MOEBIUS_E_INVAL;
-  if (threads > 0 && (threads % 32 || threads > 1024)) return MOEBIUS_E_INVAL;
+  if (threads > 0 && (threads % 32 || threads > 512)) return MOEBIUS_E_INVAL;
   x->ctas_per_sm = ctas_per_sm > 0 ? ctas_per_sm : 0;
   x->threads = threads > 0 ? threads : 0;
   x->unit_kb = unit_kb > 0 ? unit_kb : 0;

@@ -1,0 +1,212 @@
+"""GPU parity: the sm_100a reshard kernel, called through the C ABI, against the CPU oracle.
+
+Every case places the oracle's SOURCE layout at the library's fixed view offsets, uploads it, runs
+`moebius_plan` + `moebius_reshard` on the device, downloads the unified buffer and compares the
+TARGET layout bytewise with what the oracle builds from the logical tensors (bit-exact: it is byte
+movement), plus the block tables and the owner vector.  Guard strips round
+every caller-owned buffer must come back untouched.
+"""
+import numpy as np
+import pytest
+
+import workloads as wl
+from harness import (EP, TP, OracleLayout, State, expected_bytes, expected_target, mb, mb_config,
+                     source_tables)
+
+torch = pytest.importorskip("torch")
+pytestmark = pytest.mark.gpu
+
+GUARD = 4096
+CANARY = 0xC3
+
+
+def gpu_session(cfg, lens=None, policy=None, cap_frac=0.0, pool_bytes=None, fill="tag", initial_mode=TP):
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device (there is no CPU fallback)"
+    st = State(cfg, lens, fill=fill)
+    sess = mb.Session(mb_config(cfg, st.lens, policy, cap_frac, pool_bytes), device="cuda:0", guard_bytes=GUARD,
+                      initial_mode=initial_mode)
+    sess.arena.fill_(CANARY)
+    return st, sess
+
+
+def upload(sess, image):
+    sess.base[:image.size].copy_(torch.from_numpy(image))
+
+
+def download(sess):
+    torch.cuda.synchronize()
+    return sess.base.cpu().numpy()
+
+
+def check_guards(sess):
+    for i, g in enumerate(sess.guards()):
+        assert bool((g == CANARY).all()), "guard strip %d was written" % i
+
+
+def device_tables(sess, n_req):
+    """What the captured graphs read: header, owner, lens and block tables at their fixed address."""
+    lay = sess.layout
+    t = sess.tables.cpu().numpy()
+    mr, mp = sess.cfg.max_requests, sess.cfg.max_pages_per_request
+    hdr = t[:16]
+    owner = t[lay.tbl_owner_off:lay.tbl_owner_off + mr]
+    lens = t[lay.tbl_lens_off:lay.tbl_lens_off + mr]
+    bt = t[lay.tbl_bt_off:lay.tbl_bt_off + n_req * mp].reshape(n_req, mp)
+    return hdr, owner, lens, bt
+
+
+def gpu_switch(st, sess, from_mode, src_owner, src_bt):
+    to_mode = EP if from_mode == TP else TP
+    plan = sess.plan(to_mode, st.lens, src_owner, src_bt, from_mode=from_mode)
+    stats = mb.moebius_plan_stats(plan).as_dict()
+    owner, bt = sess.block_tables(plan, len(st.lens))
+    want_owner, want_bt = expected_target(st, sess, to_mode)
+    sess.reshard(plan)
+    got = download(sess)
+    assert mb.moebius_active_mode(sess.ctx) == to_mode
+    # tables: host copy and the published device copy, bit-exact with the oracle
+    if to_mode == EP:
+        assert np.array_equal(owner, want_owner)
+    else:
+        assert np.all(owner == -1)
+    assert np.array_equal(bt, want_bt)
+    n = len(st.lens)
+    hdr, d_owner, d_lens, d_bt = device_tables(sess, n)
+    assert hdr[0] == to_mode and hdr[1] == n
+    assert np.array_equal(d_bt, want_bt)
+    assert np.array_equal(d_lens[:n], st.lens)
+    assert np.array_equal(d_owner[:n], want_owner if to_mode == EP else np.full(n, -1, np.int32))
+    # every view of the target mode, bytewise
+    bad = OracleLayout(st, sess, to_mode, want_owner, want_bt).compare(got)
+    assert not bad, bad[:5]
+    check_guards(sess)
+    # accounting
+    ep_owner = src_owner if from_mode == EP else owner
+    w, k = expected_bytes(st, from_mode, ep_owner)
+    if st.cfg.w_dtype != "fp8_e4m3_b128":
+        assert (stats["w_moved"], stats["w_relocated"]) == (w["moved"], w["relocated"])
+    assert (stats["kv_moved"], stats["kv_relocated"], stats["kv_read"]) == (k["moved"], k["relocated"], k["read"])
+    sess.free_plan(plan)
+    return to_mode, (want_owner if to_mode == EP else None), want_bt, stats
+
+
+def start(st, sess, mode, how, seed=7):
+    owner, bt = source_tables(st, sess, mode, how, seed=seed)
+    image = np.full(sess.layout.base_bytes, 0xA5, np.uint8)
+    OracleLayout(st, sess, mode, owner, bt).place(image)
+    upload(sess, image)
+    return owner, bt, image
+
+
+@pytest.mark.parametrize("src", ["canonical", "random"])
+def test_tiny_round_trip(src):
+    """BASELINE.json config 1: TP -> EP -> TP; the final TP views equal the initial ones."""
+    st, sess = gpu_session(wl.get_config("tiny"))
+    owner, bt, image0 = start(st, sess, TP, src)
+    mode, owner, bt, _ = gpu_switch(st, sess, TP, owner, bt)
+    mode, owner, bt, _ = gpu_switch(st, sess, mode, owner, bt)
+    assert mode == TP
+    # the weights' TP views sit at the same fixed addresses as before: bytes identical
+    got = download(sess)
+    c = st.cfg
+    for r in range(c.R):
+        for m in range(3):
+            v = sess.view_desc(TP, r, 0, m)
+            n = int(np.prod([v.shape[i] for i in range(v.ndim)])) * v.elem_bytes
+            assert np.array_equal(got[v.offset:v.offset + n], image0[v.offset:v.offset + n])
+    sess.close()
+
+
+SMALLISH = wl.get_config("small").with_(L=2, H=128, I=256, n_req=24, len_dist=("uniform", 1, 200), seed=77)
+
+
+@pytest.mark.parametrize("first", [TP, EP])
+def test_smallish_alternating(first):
+    st, sess = gpu_session(SMALLISH, initial_mode=first)
+    mode = first
+    owner, bt, _ = start(st, sess, mode, "random")
+    for _ in range(4):
+        mode, owner, bt, _ = gpu_switch(st, sess, mode, owner, bt)
+    sess.close()
+
+
+@pytest.mark.parametrize("R,Hkv", [(8, 4), (4, 4), (2, 8), (4, 1), (1, 2)])
+def test_head_geometries(R, Hkv):
+    cfg = wl.get_config("tiny").with_(R=R, E=8, I=64, kv_heads=Hkv, n_req=7, len_dist=("uniform", 1, 70), seed=5 + R)
+    st, sess = gpu_session(cfg)
+    owner, bt, _ = start(st, sess, TP, "random")
+    mode, owner, bt, _ = gpu_switch(st, sess, TP, owner, bt)
+    mode, owner, bt, _ = gpu_switch(st, sess, mode, owner, bt)
+    sess.close()
+
+
+def test_weight_only_warmup_switch():
+    """n_req = 0."""
+    st, sess = gpu_session(wl.get_config("tiny"), lens=[])
+    empty = np.zeros((0, 1), np.int32)
+    image = np.full(sess.layout.base_bytes, 0xA5, np.uint8)
+    OracleLayout(st, sess, TP, None, empty).place(image)
+    upload(sess, image)
+    mode, owner, bt, s = gpu_switch(st, sess, TP, None, empty)
+    assert s["n_kv_moves"] == 0
+    gpu_switch(st, sess, mode, np.zeros(0, np.int32), empty)
+    sess.close()
+
+
+@pytest.mark.parametrize("first", [TP, EP])
+def test_tight_pool_rounds_and_staging(first):
+    """Target pages overlap live source pages: dependency rounds + bounded staging on the device."""
+    cfg = SMALLISH.with_(L=1, n_req=40, seed=99)
+    lens = wl.draw_seq_lens(cfg)
+    rounds = staged = 0
+    for seed in range(3):
+        st, sess = gpu_session(cfg, lens, "tight", cap_frac=0.5, initial_mode=first)
+        mode = first
+        owner, bt, _ = start(st, sess, mode, "random", seed=seed)
+        for _ in range(2):
+            mode, owner, bt, stats = gpu_switch(st, sess, mode, owner, bt)
+            rounds, staged = max(rounds, stats["n_kv_rounds"]), max(staged, stats["n_kv_staged"])
+        sess.close()
+    assert rounds > 2 and staged > 0
+
+
+def test_fp8_scales():
+    cfg = wl.get_config("fp8_graph").with_(L=1, E=8, H=256, I=1536, n_req=6, len_dist=("uniform", 1, 60), seed=3)
+    st, sess = gpu_session(cfg, fill="normal")
+    owner, bt, _ = start(st, sess, TP, "random")
+    mode, owner, bt, _ = gpu_switch(st, sess, TP, owner, bt)
+    mode, owner, bt, _ = gpu_switch(st, sess, mode, owner, bt)
+    sess.close()
+
+
+def test_small_config_alternating():
+    """BASELINE.json config 2 (R=4, 4 layers, E=16, H=1024, I=512; 64 requests of 128-2048 tokens):
+    alternating TP->EP and EP->TP switches; spans many tiles of every segment kind and ragged tails."""
+    cfg = wl.get_config("small")
+    st, sess = gpu_session(cfg)
+    mode = TP
+    owner, bt, _ = start(st, sess, mode, "random")
+    for _ in range(2):
+        mode, owner, bt, _ = gpu_switch(st, sess, mode, owner, bt)
+    sess.close()
+
+
+@pytest.mark.parametrize("threads,ctas,unit_kb", [(128, 1, 4), (512, 2, 64), (256, 8, 16)])
+def test_launch_shapes(threads, ctas, unit_kb):
+    """The result does not depend on the launch shape or the unit size."""
+    st, sess = gpu_session(SMALLISH, initial_mode=EP)
+    mb.moebius_set_launch(sess.ctx, ctas, threads, unit_kb)
+    owner, bt, _ = start(st, sess, EP, "random")
+    mode, owner, bt, _ = gpu_switch(st, sess, EP, owner, bt)
+    gpu_switch(st, sess, mode, owner, bt)
+    sess.close()
+
+
+def test_state_errors():
+    st, sess = gpu_session(wl.get_config("tiny"))
+    owner, bt, _ = start(st, sess, TP, "canonical")
+    plan = sess.plan(TP, st.lens, *source_tables(st, sess, EP, "canonical"), from_mode=EP)
+    with pytest.raises(mb.MoebiusError) as e:     # active mode is TP, plan.from is EP
+        sess.reshard(plan)
+    assert e.value.status == -4
+    sess.close()
