@@ -49,6 +49,8 @@ def parse():
     ap.add_argument("--staging-cap-frac", type=float, default=0.024,
                     help="cap on spare slot + staging as a fraction of resident bytes (0 = library default)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--profile-region", action="store_true",
+                    help="cudaProfilerStart/Stop round warm-up + timed steps (ncu --profile-from-start off skips the fill)")
     ap.add_argument("--cpu-sample-requests", type=int, default=48)
     return ap.parse_args()
 
@@ -273,6 +275,9 @@ def run_moebius(args):
         return plan, (new_owner if to == EP else None), new_bt, (t1 - t0) * 1e3
 
     mb.moebius_set_timing(sess.ctx, True)
+    if args.profile_region:
+        torch.cuda.synchronize()
+        torch.cuda.cudart().cudaProfilerStart()
     # warm-up: W round trips (the first one starts from the random tables)
     owner, bt, mode = None, bt0, TP
     first_ms = {}
@@ -307,6 +312,8 @@ def run_moebius(args):
     if world > 1:
         dist.barrier()
     dev_ms = e0.elapsed_time(e1)
+    if args.profile_region:
+        torch.cuda.cudart().cudaProfilerStop()
     hist = mb.moebius_kernel_ms_history(sess.ctx, 64)[-2 * args.steps:]
     k_t2e, k_e2t = hist[0::2], hist[1::2]
 
