@@ -48,6 +48,8 @@ def parse():
     ap.add_argument("--layers", type=int, default=0, help="override L (profiling captures only; named in config.workload)")
     ap.add_argument("--staging-cap-frac", type=float, default=0.024,
                     help="cap on spare slot + staging as a fraction of resident bytes (0 = library default)")
+    ap.add_argument("--n-req", type=int, default=-1, help="override the number of live requests (experiments; named in config.workload)")
+    ap.add_argument("--tma", default="", help="enable,pipes,stage_kb (tuning; default: library defaults)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--profile-region", action="store_true",
                     help="cudaProfilerStart/Stop round warm-up + timed steps (ncu --profile-from-start off skips the fill)")
@@ -245,10 +247,13 @@ def run_moebius(args):
         cfg = cfg.with_(L=args.layers, name="%s[L=%d]" % (cfg.name, args.layers))
     lens = wl.draw_seq_lens(cfg)
     pool = wl.kv_pool_bytes(cfg, lens, args.pool)
-    mp = int(max((int(x) + cfg.page - 1) // cfg.page for x in lens))
+    if args.n_req >= 0:
+        lens = lens[:args.n_req]
+        cfg = cfg.with_(n_req=args.n_req, name="%s[n_req=%d]" % (cfg.name, args.n_req))
+    mp = int(max([1] + [(int(x) + cfg.page - 1) // cfg.page for x in lens]))
     c = mb.make_config(R=cfg.R, L=cfg.L, E=cfg.E, H=cfg.H, I=cfg.I, w_dtype=cfg.w_dtype, kv_heads=cfg.kv_heads,
                        head_dim=cfg.head_dim, page_tokens=cfg.page, kv_pool_bytes_per_rank_layer=pool,
-                       max_requests=len(lens), max_pages_per_request=mp, staging_cap_bytes=0)
+                       max_requests=max(len(lens), 1), max_pages_per_request=mp, staging_cap_bytes=0)
     probe = mb.Session(c)
     resident = probe.layout.resident_bytes
     probe.close()
@@ -258,6 +263,9 @@ def run_moebius(args):
     if args.launch:
         a, b, u = (int(x) for x in args.launch.split(","))
         mb.moebius_set_launch(sess.ctx, a, b, u)
+    if args.tma:
+        a, b, u = (int(x) for x in args.tma.split(","))
+        mb.moebius_set_tma(sess.ctx, a, b, u)
     fill_device(sess, cfg, mb, torch)
     TP, EP = mb.MOEBIUS_TP, mb.MOEBIUS_EP
     n = len(lens)

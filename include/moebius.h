@@ -192,7 +192,15 @@ MOEBIUS_API int moebius_last_kernel_ms(moebius_ctx_t* ctx, float* ms);
  * *n_out receives how many were written.  Synchronises on each end event. */
 MOEBIUS_API int moebius_kernel_ms_history(moebius_ctx_t* ctx, float* out_ms, int cap, int* n_out);
 
-/* Launch shape override for tuning: ctas_per_sm <= 0 and threads <= 0 restore the defaults. */
+/* Data-path selection, before the first moebius_plan of a context.  enable != 0 (the default):
+ * segments whose shapes allow it run on the TMA path (tensor-map loads/stores through shared memory,
+ * `pipes` warps per SM with two `stage_kb` KB stages each; 0 = defaults 2 and 48).  enable == 0:
+ * everything runs on the ld.global/st.global path.  Results are identical either way.  A plan built
+ * before the call cannot be executed after it (MOEBIUS_E_STATE).  2*pipes*stage_kb <= 208. */
+MOEBIUS_API int moebius_set_tma(moebius_ctx_t* ctx, int enable, int pipes, int stage_kb);
+
+/* Launch shape override for the ld/st path (tuning): values <= 0 restore the defaults; threads is a
+ * multiple of 32, at most 256. */
 MOEBIUS_API int moebius_set_launch(moebius_ctx_t* ctx, int ctas_per_sm, int threads, int unit_kb);
 
 MOEBIUS_API const char* moebius_status_str(int status);

@@ -10,6 +10,7 @@
 // Data path: 16-byte ld.global / st.global with L1 no-allocate, 8 loads in flight per lane, lanes
 // mapped to consecutive 16-byte chunks of the EP-side row so that both sides are accessed in whole
 // contiguous runs (>= one 32-byte sector, usually whole 128-byte lines).
+#include <cuda.h>
 #include <cuda_runtime.h>
 
 #include <cstdio>
@@ -120,13 +121,247 @@ __device__ __forceinline__ void c2d_copy(const C2dDesc& d, char* base, uint32_t 
   }
 }
 
-__global__ void __launch_bounds__(512, 1) moebius_reshard_kernel(const DevParams p) {
-  const uint32_t lane = threadIdx.x & 31;
+// ---- TMA path (PATH_TMA segments) ---------------------------------------------------------------
+// PTX wrappers.  SASS: UTMALDG / UTMASTG (tensor), UBLKCP (bulk), SYNCS (mbarrier).
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint64_t* b, uint32_t n) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" :: "r"(smem_u32(b)), "r"(n));
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t* b, uint32_t bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" :: "r"(smem_u32(b)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ bool mbar_try_wait(uint64_t* b, uint32_t parity) {
+  uint32_t ok;
+  asm volatile("{\n .reg .pred p;\n mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n selp.u32 %0, 1, 0, p;\n}\n"
+               : "=r"(ok) : "r"(smem_u32(b)), "r"(parity) : "memory");
+  return ok != 0;
+}
+// A lost transaction would hang the GPU box; trap instead (about 10 s of polling)
+__device__ __forceinline__ void mbar_wait(uint64_t* b, uint32_t parity) {
+  for (uint32_t spins = 0; !mbar_try_wait(b, parity); ++spins)
+    if (spins > (1u << 28)) __trap();
+}
+__device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t bytes, uint64_t* bar) {
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+               :: "r"(smem_u32(dst)), "l"(src), "r"(bytes), "r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void bulk_s2g(void* dst, const void* src, uint32_t bytes) {
+  asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;"
+               :: "l"(dst), "r"(smem_u32(src)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void tma_load_5d(void* dst, const CUtensorMap* tm, int c0, int c1, int c2, int c3, int c4, uint64_t* bar) {
+  asm volatile("cp.async.bulk.tensor.5d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2,%3,%4,%5,%6}], [%7];"
+               :: "r"(smem_u32(dst)), "l"(tm), "r"(c0), "r"(c1), "r"(c2), "r"(c3), "r"(c4), "r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void tma_store_5d(const CUtensorMap* tm, int c0, int c1, int c2, int c3, int c4, const void* src) {
+  asm volatile("cp.async.bulk.tensor.5d.global.shared::cta.tile.bulk_group [%0, {%1,%2,%3,%4,%5}], [%6];"
+               :: "l"(tm), "r"(c0), "r"(c1), "r"(c2), "r"(c3), "r"(c4), "r"(smem_u32(src)) : "memory");
+}
+__device__ __forceinline__ void bulk_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
+template <int N> __device__ __forceinline__ void bulk_wait_read() { asm volatile("cp.async.bulk.wait_group.read %0;" :: "n"(N) : "memory"); }
+template <int N> __device__ __forceinline__ void bulk_wait() { asm volatile("cp.async.bulk.wait_group %0;" :: "n"(N) : "memory"); }
+__device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async;" ::: "memory"); }
+
+// One unit through one stage.  Geometry comes from decode_box / the segment, exactly as on the LSU
+// path; smem layout of a stage: XT [group][xt_rows][run], LT [row][chunk], KT [pool][group][page][run].
+struct TmaCtx {
+  const DevParams* p;
+  const CUtensorMap* tm_w;
+  const CUtensorMap* tm_kv;
+};
+
+__device__ __forceinline__ void tma_issue_load(const TmaCtx& c, const Seg& s, uint32_t ul, char* stage, uint64_t* bar) {
+  const DevParams& p = *c.p;
+  if (seg_kind(s) == SEG_XPOSE) {
+    Box b;
+    decode_box(s, p, ul, 0, b);
+    if (s.groups_per_unit == s.n_groups) {          // XT
+      const uint32_t q = ul / s.row_blocks, row0 = (ul % s.row_blocks) * s.rows_per_unit;
+      const uint32_t piece = p.xt_rows * s.run_bytes;
+      if (s.ep_is_src) {
+        mbar_expect_tx(bar, piece * s.n_groups);     // the box is always delivered whole (rows past the end are zero-filled)
+        tma_load_5d(stage, c.tm_w, 0, (int)row0, 0, (int)q, (int)s.desc_begin, bar);
+      } else {
+        const uint32_t bytes = b.nrows * s.run_bytes;
+        mbar_expect_tx(bar, bytes * s.n_groups);
+        for (uint32_t g = 0; g < s.n_groups; ++g)
+          bulk_g2s(stage + (size_t)g * piece, b.tp + (int64_t)g * p.rank_stride, bytes, bar);
+      }
+    } else {                                          // LT: one group, nrows pieces of chunk bytes
+      const uint32_t chunk = s.chunk_bytes;
+      mbar_expect_tx(bar, b.nrows * chunk);
+      if (s.ep_is_src) {
+        for (uint32_t t = 0; t < b.nrows; ++t) bulk_g2s(stage + (size_t)t * chunk, b.ep + (int64_t)t * b.ep_row_stride, chunk, bar);
+      } else {
+        bulk_g2s(stage, b.tp + (int64_t)b.g0 * p.rank_stride, b.nrows * chunk, bar);
+      }
+    }
+    return;
+  }
+  // KT
+  uint32_t pb, di;
+  kv_unit(s, ul, pb, di);
+  const uint32_t nb = seg_boxes(s, ul);
+  const uint32_t z0 = s.pool_begin + pb * s.pools_per_unit;
+  const KvDesc d = p.kv[s.desc_begin + di];
+  const uint32_t ntok = d.ntok_slot & 0xFFu;
+  if (s.ep_is_src) {
+    mbar_expect_tx(bar, nb * s.ep_page_bytes);
+    for (uint32_t k = 0; k < nb; ++k)
+      tma_load_5d(stage + (size_t)k * s.ep_page_bytes, c.tm_kv, 0, (int)(d.ep_page * p.page_tokens), 0, (int)(z0 + k), d.ep_rank, bar);
+  } else {
+    const uint32_t bytes = ntok * s.run_bytes;
+    mbar_expect_tx(bar, nb * s.n_groups * bytes);
+    for (uint32_t k = 0; k < nb; ++k) {
+      const char* pool = p.base + s.ep_off + (int64_t)(z0 + k) * s.pool_bytes + (int64_t)d.tp_page * s.tp_page_bytes;
+      for (uint32_t g = 0; g < s.n_groups; ++g)
+        bulk_g2s(stage + (size_t)k * s.ep_page_bytes + (size_t)g * s.tp_page_bytes,
+                 pool + (int64_t)tp_src_rank(g, s.rep, d.ep_rank) * p.rank_stride, bytes, bar);
+    }
+  }
+}
+
+__device__ __forceinline__ void tma_issue_store(const TmaCtx& c, const Seg& s, uint32_t ul, char* stage) {
+  const DevParams& p = *c.p;
+  if (seg_kind(s) == SEG_XPOSE) {
+    Box b;
+    decode_box(s, p, ul, 0, b);
+    if (s.groups_per_unit == s.n_groups) {          // XT
+      const uint32_t q = ul / s.row_blocks, row0 = (ul % s.row_blocks) * s.rows_per_unit;
+      const uint32_t piece = p.xt_rows * s.run_bytes;
+      if (s.ep_is_src) {
+        const uint32_t bytes = b.nrows * s.run_bytes;
+        for (uint32_t g = 0; g < s.n_groups; ++g)
+          bulk_s2g(b.tp + (int64_t)g * p.rank_stride, stage + (size_t)g * piece, bytes);
+      } else {
+        tma_store_5d(c.tm_w, 0, (int)row0, 0, (int)q, (int)s.desc_begin, stage);   // rows past the end are clipped
+      }
+    } else {                                          // LT
+      const uint32_t chunk = s.chunk_bytes;
+      if (s.ep_is_src) {
+        bulk_s2g(b.tp + (int64_t)b.g0 * p.rank_stride, stage, b.nrows * chunk);
+      } else {
+        for (uint32_t t = 0; t < b.nrows; ++t) bulk_s2g(b.ep + (int64_t)t * b.ep_row_stride, stage + (size_t)t * chunk, chunk);
+      }
+    }
+    bulk_commit();
+    return;
+  }
+  uint32_t pb, di;
+  kv_unit(s, ul, pb, di);
+  const uint32_t nb = seg_boxes(s, ul);
+  const uint32_t z0 = s.pool_begin + pb * s.pools_per_unit;
+  const KvDesc d = p.kv[s.desc_begin + di];
+  const uint32_t ntok = d.ntok_slot & 0xFFu;
+  if (s.ep_is_src) {
+    const uint32_t bytes = ntok * s.run_bytes;
+    for (uint32_t k = 0; k < nb; ++k) {
+      char* pool = p.base + s.ep_off + (int64_t)(z0 + k) * s.pool_bytes + (int64_t)d.tp_page * s.tp_page_bytes;
+      for (uint32_t g = 0; g < s.n_groups; ++g)
+        for (uint32_t r = 0; r < s.rep; ++r)
+          bulk_s2g(pool + (int64_t)(g * s.rep + r) * p.rank_stride,
+                   stage + (size_t)k * s.ep_page_bytes + (size_t)g * s.tp_page_bytes, bytes);
+    }
+  } else {
+    // the whole page box is written: slots past the valid tokens get unspecified bytes (reading A10)
+    for (uint32_t k = 0; k < nb; ++k)
+      tma_store_5d(c.tm_kv, 0, (int)(d.ep_page * p.page_tokens), 0, (int)(z0 + k), d.ep_rank, stage + (size_t)k * s.ep_page_bytes);
+  }
+  bulk_commit();
+}
+
+__device__ __forceinline__ void lsu_unit(const Seg& s, const DevParams& p, uint32_t ul, uint32_t lane) {
+  if (seg_kind(s) == SEG_COPY2D) {
+    c2d_copy(p.c2d[s.desc_begin + ul], p.base, lane);
+    return;
+  }
+  const uint32_t nb = seg_boxes(s, ul);
+  for (uint32_t k = 0; k < nb; ++k) {
+    Box b;
+    decode_box(s, p, ul, k, b);
+    if (b.lin) lin_copy(b.lin_src, b.lin_dst, b.lin_bytes, lane);
+    else if (s.ep_is_src) xbox_ep_to_tp(b, p.rank_stride, lane);
+    else xbox_tp_to_ep(b, p.rank_stride, lane);
+  }
+}
+
+// Every warp is a PIPE: it takes unit tickets in list order and, for PATH_TMA units, keeps a
+// two-stage software pipeline in its private slice of shared memory -- the loads of unit i+1 fly
+// while the stores of unit i drain (lane 0 issues everything; measured best among 1-6 pipes x 2-4
+// stages).  PATH_LSU units are copied by the whole warp.  Before a pipe blocks on a
+// dependency counter it drains its own pipeline, so waits can never be circular.
+__global__ void __launch_bounds__(256, 2)
+moebius_reshard_kernel(const __grid_constant__ DevParams p, const __grid_constant__ CUtensorMap tm_w,
+                       const __grid_constant__ CUtensorMap tm_kv) {
+  extern __shared__ __align__(1024) char smem[];
+  const uint32_t lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  uint64_t* bar = (uint64_t*)smem + 2 * warp;                       // 2 barriers per pipe
+  char* ring = smem + 1024 + (size_t)warp * 2 * p.stage_bytes;     // 2 stages per pipe
+  if (lane == 0 && p.stage_bytes) {
+    mbar_init(bar, 1);
+    mbar_init(bar + 1, 1);
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  __syncwarp();
+  TmaCtx tc{&p, &tm_w, &tm_kv};
+
+  // pipe state; identical in every lane (it depends on uniform values only)
+  bool loading = false;           // a unit's loads are in flight
+  uint32_t ld_si = 0, ld_ul = 0, ld_stage = 0;
+  uint32_t phase0 = 0, phase1 = 0;
+  uint32_t next_stage = 0;
+  // completion signals are batched: units whose store groups are committed but not yet signalled all
+  // belong to counter pend_ctr; one fence + one atomicAdd publishes them when the counter changes or
+  // the pipe drains (a per-unit fence + atomic costs a third of the pipe's time)
+  int32_t pend_ctr = -1;
+  uint32_t pend_n = 0;
+
+  auto publish = [&]() {                // lane 0, after the pending units' writes have completed
+    if (pend_ctr >= 0 && pend_n) { fence_proxy_async(); __threadfence(); atomicAdd(p.counters + pend_ctr, pend_n); }
+  };
+  auto retire = [&]() {                  // loads landed -> issue the stores of the loading unit
+    if (!loading) return;
+    const Seg& s = p.segs[ld_si];
+    const int32_t ctr = s.signal_ctr;
+    if (lane == 0) {
+      mbar_wait(bar + ld_stage, ld_stage ? phase1 : phase0);
+      tma_issue_store(tc, s, ld_ul, ring + (size_t)ld_stage * p.stage_bytes);
+      if (ctr != pend_ctr && pend_ctr >= 0 && pend_n) { bulk_wait<1>(); publish(); }   // all but the group just committed
+    }
+    if (ld_stage) phase1 ^= 1; else phase0 ^= 1;
+    if (ctr != pend_ctr) { pend_ctr = ctr; pend_n = 0; }
+    ++pend_n;
+    loading = false;
+  };
+  auto drain = [&]() {                   // everything this pipe has in flight completes and is signalled
+    retire();
+    if (lane == 0) { bulk_wait<0>(); publish(); }
+    pend_n = 0;
+    __syncwarp();
+  };
+  auto wait_for = [&](const Seg& s) {    // dependency of a segment (rare: chain links, KV rounds)
+    if (s.wait_ctr < 0) return;
+    uint32_t ok = 0;
+    if (lane == 0) ok = ld_acquire(p.counters + s.wait_ctr) >= s.wait_target;
+    ok = __shfl_sync(0xffffffffu, ok, 0);
+    if (!ok) {
+      drain();
+      if (lane == 0) {
+        for (uint32_t spins = 0; ld_acquire(p.counters + s.wait_ctr) < s.wait_target; ++spins) {
+          __nanosleep(200);
+          if (spins > (1u << 26)) __trap();
+        }
+      }
+    }
+    if (lane == 0) fence_proxy_async();
+    __syncwarp();
+  };
+  auto fetch = [&]() -> uint32_t { return lane == 0 ? atomicAdd(p.ticket, 1u) : 0u; };
+
   uint32_t si = 0;
+  uint32_t t_next = fetch();
   for (;;) {
-    uint32_t u = 0;
-    if (lane == 0) u = atomicAdd(p.ticket, 1u);
-    u = __shfl_sync(0xffffffffu, u, 0);
+    const uint32_t u = __shfl_sync(0xffffffffu, t_next, 0);
     if (u >= p.total_units) break;
     // units are handed out in increasing order: search forward from the last segment
     while (si + 1 < p.n_segs && u >= __ldg(&p.segs[si + 1].unit_begin)) {
@@ -137,35 +372,29 @@ __global__ void __launch_bounds__(512, 1) moebius_reshard_kernel(const DevParams
       }
       si = lo;
     }
-    const Seg s = p.segs[si];
+    const Seg& s = p.segs[si];
     const uint32_t ul = u - s.unit_begin;
-    if (s.wait_ctr >= 0) {
+    if (seg_path(s) == PATH_TMA) {
+      retire();
+      wait_for(s);
       if (lane == 0) {
-        const uint32_t* c = p.counters + s.wait_ctr;
-        while (ld_acquire(c) < s.wait_target) __nanosleep(200);
+        bulk_wait_read<1>();   // the stage about to be refilled was read by the store group before the last one
+        tma_issue_load(tc, s, ul, ring + (size_t)next_stage * p.stage_bytes, bar + next_stage);
       }
-      __syncwarp();
-    }
-    if (s.kind == SEG_COPY2D) {
-      c2d_copy(p.c2d[s.desc_begin + ul], p.base, lane);
+      loading = true; ld_si = si; ld_ul = ul; ld_stage = next_stage;
+      next_stage ^= 1;
+      t_next = fetch();        // its latency hides behind the loads just issued
     } else {
-      const uint32_t nb = seg_boxes(s, ul);
-      for (uint32_t k = 0; k < nb; ++k) {
-        Box b;
-        decode_box(s, p, ul, k, b);
-        if (b.lin) lin_copy(b.lin_src, b.lin_dst, b.lin_bytes, lane);
-        else if (s.ep_is_src) xbox_ep_to_tp(b, p.rank_stride, lane);
-        else xbox_tp_to_ep(b, p.rank_stride, lane);
-      }
-    }
-    if (s.signal_ctr >= 0) {
-      __syncwarp();
-      if (lane == 0) {
-        __threadfence();
-        atomicAdd(p.counters + s.signal_ctr, 1u);
+      t_next = fetch();
+      wait_for(s);
+      lsu_unit(s, p, ul, lane);
+      if (s.signal_ctr >= 0) {
+        __syncwarp();
+        if (lane == 0) { __threadfence(); atomicAdd(p.counters + s.signal_ctr, 1u); }
       }
     }
   }
+  drain();
 }
 
 void* host_alloc(int64_t bytes, bool* pinned) {
@@ -184,6 +413,55 @@ void* host_alloc(int64_t bytes, bool* pinned) {
 void host_free(void* p, bool pinned) {
   if (!p) return;
   if (pinned) cudaFreeHost(p); else free(p);
+}
+
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                  const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
+                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+// The two tensor maps of the TMA path, over the caller's bound allocation (uint32 elements):
+//   weights (gate/up slots):  [run/4][rows = E/R*H][group R][rank R][slot 3L+1], box [run/4][xt_rows][R][1][1]
+//   KV (EP pools):            [run/4][rows = pages_ep*pg][group G][pool 2L][rank R], box [run/4][pg][G][1][1]
+// Dimension 1 (rows) has the LARGER stride and dimension 2 (group) the smaller one, so a box lands
+// in shared memory as [group][row][run]: the run transposition is done by the TMA engine.
+static int encode_tmaps(moebius_ctx* x) {
+  static_assert(sizeof(CUtensorMap) <= sizeof(x->tmap_w), "CUtensorMap storage");
+  memset(x->tmap_w, 0, sizeof(x->tmap_w));
+  memset(x->tmap_kv, 0, sizeof(x->tmap_kv));
+  x->tmaps_valid = true;
+  if (!x->use_tma || (!x->xt_ok && !x->kt_ok)) return MOEBIUS_OK;
+  void* fn = nullptr;
+  cudaDriverEntryPointQueryResult qres;
+  if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres) != cudaSuccess || !fn) {
+    cudaGetLastError();
+    x->tmaps_valid = false;
+    return MOEBIUS_E_CUDA;
+  }
+  EncodeTiledFn enc = (EncodeTiledFn)fn;
+  const moebius_config_t& c = x->cfg;
+  const cuuint32_t ones[5] = {1, 1, 1, 1, 1};
+  if (x->xt_ok) {
+    const cuuint64_t run = (cuuint64_t)(c.I / c.R) * x->wb;
+    cuuint64_t dims[5] = {run / 4, (cuuint64_t)(c.E / c.R) * c.H, (cuuint64_t)c.R, (cuuint64_t)c.R,
+                          (cuuint64_t)(3 * c.L + x->ep_shift)};
+    cuuint64_t strides[4] = {run * c.R, run, (cuuint64_t)x->rank_stride, (cuuint64_t)x->S};
+    cuuint32_t box[5] = {(cuuint32_t)(run / 4), (cuuint32_t)x->xt_rows, (cuuint32_t)c.R, 1, 1};
+    if (enc((CUtensorMap*)x->tmap_w, CU_TENSOR_MAP_DATA_TYPE_UINT32, 5, x->base + x->w_off, dims, strides, box, ones,
+            CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_NONE,
+            CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS) { x->tmaps_valid = false; return MOEBIUS_E_CUDA; }
+  }
+  if (x->kt_ok) {
+    const cuuint64_t run = (cuuint64_t)x->run_kv;
+    cuuint64_t dims[5] = {run / 4, (cuuint64_t)x->pages_ep * c.page_tokens, (cuuint64_t)x->G, (cuuint64_t)(2 * c.L),
+                          (cuuint64_t)c.R};
+    cuuint64_t strides[4] = {run * x->G, run, (cuuint64_t)x->pool_bytes, (cuuint64_t)x->rank_stride};
+    cuuint32_t box[5] = {(cuuint32_t)(run / 4), (cuuint32_t)c.page_tokens, (cuuint32_t)x->G, 1, 1};
+    if (x->pages_ep < 1 ||
+        enc((CUtensorMap*)x->tmap_kv, CU_TENSOR_MAP_DATA_TYPE_UINT32, 5, x->base + x->kv_off, dims, strides, box, ones,
+            CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_NONE,
+            CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS) { x->tmaps_valid = false; return MOEBIUS_E_CUDA; }
+  }
+  return MOEBIUS_OK;
 }
 
 void cuda_ctx_destroy(moebius_ctx* x) {
@@ -210,6 +488,7 @@ extern "C" int moebius_bind(moebius_ctx_t* x, void* dev_base, void* dev_staging,
   x->tables = dev_tables;
   x->active_mode = initial_mode;
   x->bound = true;
+  x->tmaps_valid = false;   // encoded on the first reshard (needs a device)
   return MOEBIUS_OK;
 }
 
@@ -273,6 +552,7 @@ extern "C" int moebius_reshard(moebius_ctx_t* x, const moebius_plan_t* P, void* 
   // 2. the kernel
   if (P->total_units) {
     DevParams p;
+    memset(&p, 0, sizeof(p));
     p.base = x->base;
     p.stg = x->stg;
     p.segs = (const Seg*)(x->desc + kSegOff);
@@ -283,14 +563,32 @@ extern "C" int moebius_reshard(moebius_ctx_t* x, const moebius_plan_t* P, void* 
     p.rank_stride = x->rank_stride;
     p.n_segs = (uint32_t)P->segs.size();
     p.total_units = P->total_units;
-    int threads = x->threads > 0 ? x->threads : 512;
-    int per_sm = x->ctas_per_sm > 0 ? x->ctas_per_sm : 2;
-    int64_t warps_needed = P->total_units;
+    p.page_tokens = (uint32_t)x->cfg.page_tokens;
+    int threads, per_sm;
+    size_t smem = 0;
+    if (P->uses_tma) {
+      // one CTA per SM, n_pipes warps, each with two private stages
+      if (P->stage_bytes != x->stage_bytes || P->xt_rows != x->xt_rows) return MOEBIUS_E_STATE;  // set_tma after plan
+      if (!x->tmaps_valid) { int rc = encode_tmaps(x); if (rc != MOEBIUS_OK) return rc; }
+      p.stage_bytes = (uint32_t)x->stage_bytes;
+      p.xt_rows = (uint32_t)x->xt_rows;
+      threads = 32 * x->n_pipes;
+      per_sm = 1;
+      smem = 1024 + (size_t)x->n_pipes * 2 * (size_t)x->stage_bytes;
+      if (smem != x->smem_set) {
+        if (cudaFuncSetAttribute(moebius_reshard_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess)
+          return MOEBIUS_E_CUDA;
+        x->smem_set = smem;
+      }
+    } else {
+      threads = x->threads > 0 ? x->threads : 256;
+      per_sm = x->ctas_per_sm > 0 ? x->ctas_per_sm : 2;
+    }
     int64_t grid = (int64_t)x->n_sm * per_sm;
-    int64_t grid_cap = (warps_needed + threads / 32 - 1) / (threads / 32);
+    int64_t grid_cap = ((int64_t)P->total_units + threads / 32 - 1) / (threads / 32);
     if (grid > grid_cap) grid = grid_cap;
     if (x->timing) cudaEventRecord(ev_a, st);
-    moebius_reshard_kernel<<<(unsigned)grid, threads, 0, st>>>(p);
+    moebius_reshard_kernel<<<(unsigned)grid, threads, smem, st>>>(p, *(const CUtensorMap*)x->tmap_w, *(const CUtensorMap*)x->tmap_kv);
     if (cudaGetLastError() != cudaSuccess) return MOEBIUS_E_CUDA;
     if (x->timing) cudaEventRecord(ev_b, st);
   } else if (x->timing) {

@@ -46,8 +46,18 @@ struct moebius_ctx {
   int32_t* tables;
   int active_mode;
   int64_t switch_count;
-  // launch shape
+  // launch shape (PATH_LSU tuning) and the TMA path's geometry (fixed before the first plan)
   int ctas_per_sm, threads, unit_kb;
+  int use_tma;                    // planner emits PATH_TMA segments where the shapes allow
+  int n_pipes;                    // TMA pipes (warps) per CTA, one CTA per SM
+  int64_t stage_bytes;            // bytes of one shared-memory stage; 2 stages per pipe
+  int xt_ok, kt_ok;               // weight / KV tensor maps exist for this config
+  int xt_rows;                    // rows of the weight tensor-map box
+  int kt_pools;                   // pools per KV unit
+  alignas(64) unsigned char tmap_w[128];   // CUtensorMap storage (encoded at bind time)
+  alignas(64) unsigned char tmap_kv[128];
+  bool tmaps_valid;
+  size_t smem_set;                // dynamic shared memory the kernel attribute is currently set to
   // device facts + timing (filled lazily by the CUDA side)
   int n_sm;
   int timing;
@@ -65,6 +75,8 @@ struct moebius_plan {
   std::vector<int32_t> lens, owner, bt;   // target-mode request state
   moebius_stats_t stats;
   uint32_t n_counters, total_units;
+  bool uses_tma;                  // some segment is PATH_TMA: needs the pipes' shared-memory rings
+  int64_t stage_bytes; int xt_rows;   // geometry the plan was built for
   // one contiguous upload image: [segs][kv][c2d], and the table image; pinned when CUDA allows
   char* image;
   int64_t image_bytes, kv_img_off, c2d_img_off;
@@ -78,6 +90,7 @@ namespace moebius {
 void* host_alloc(int64_t bytes, bool* pinned);
 void host_free(void* p, bool pinned);
 void cuda_ctx_destroy(moebius_ctx* ctx);
+void tma_geometry(moebius_ctx* ctx);   // derives xt_ok/kt_ok/xt_rows/kt_pools from cfg + stage_bytes (host only)
 }  // namespace moebius
 
 #endif

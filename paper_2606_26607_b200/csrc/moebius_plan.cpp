@@ -35,6 +35,18 @@ constexpr int kMaxLevel = 24;
 
 }  // namespace
 
+// Shapes the TMA path can take (see moebius_units.h PATH_TMA).  Box dimensions are limited to 256
+// elements (uint32 elements here, so a run of at most 1024 bytes) and a unit must fit one stage.
+void moebius::tma_geometry(moebius_ctx* x) {
+  const moebius_config_t& c = x->cfg;
+  const int64_t run_gu = (int64_t)(c.I / c.R) * x->wb;
+  x->xt_ok = c.R > 1 && run_gu <= 1024 && run_gu * c.R <= x->stage_bytes && c.R <= 256;
+  x->xt_rows = x->xt_ok ? (int)std::min<int64_t>(256, x->stage_bytes / (run_gu * c.R)) : 0;
+  x->kt_ok = x->run_kv <= 1024 && c.page_tokens <= 256 && x->G <= 256 && x->ep_page_bytes <= x->stage_bytes &&
+             x->ep_page_bytes % 128 == 0;
+  x->kt_pools = x->kt_ok ? (int)std::min<int64_t>(x->stage_bytes / x->ep_page_bytes, 2 * (int64_t)c.L) : 0;
+}
+
 extern "C" {
 
 const char* moebius_status_str(int s) {
@@ -139,6 +151,12 @@ int moebius_create(const moebius_config_t* c, moebius_ctx_t** out) {
   x->ctas_per_sm = 0;
   x->threads = 0;
   x->unit_kb = 0;
+  x->use_tma = 1;
+  x->n_pipes = 2;
+  x->stage_bytes = 48 * 1024;
+  x->tmaps_valid = false;
+  x->smem_set = 0;
+  tma_geometry(x);
   x->n_sm = 0;
   x->timing = 0;
   memset(x->ev, 0, sizeof(x->ev));
@@ -228,9 +246,23 @@ int moebius_view(const moebius_ctx_t* x, moebius_mode_t mode, int rank, int laye
 
 int moebius_active_mode(const moebius_ctx_t* x) { return x ? x->active_mode : MOEBIUS_E_INVAL; }
 
+int moebius_set_tma(moebius_ctx_t* x, int enable, int pipes, int stage_kb) {
+  if (!x) return MOEBIUS_E_INVAL;
+  if (pipes < 0 || pipes > 8 || stage_kb < 0) return MOEBIUS_E_INVAL;
+  int np = pipes > 0 ? pipes : 2;
+  int64_t sb = stage_kb > 0 ? (int64_t)stage_kb * 1024 : 48 * 1024;
+  if ((int64_t)np * 2 * sb > 208 * 1024) return MOEBIUS_E_INVAL;   // 227 KB per CTA minus barriers and slack
+  x->use_tma = enable ? 1 : 0;
+  x->n_pipes = np;
+  x->stage_bytes = sb;
+  x->tmaps_valid = false;
+  tma_geometry(x);
+  return MOEBIUS_OK;
+}
+
 int moebius_set_launch(moebius_ctx_t* x, int ctas_per_sm, int threads, int unit_kb) {
   if (!x) return MOEBIUS_E_INVAL;
-  if (threads > 0 && (threads % 32 || threads > 512)) return MOEBIUS_E_INVAL;
+  if (threads > 0 && (threads % 32 || threads > 256)) return MOEBIUS_E_INVAL;
   x->ctas_per_sm = ctas_per_sm > 0 ? ctas_per_sm : 0;
   x->threads = threads > 0 ? threads : 0;
   x->unit_kb = unit_kb > 0 ? unit_kb : 0;
@@ -499,7 +531,24 @@ extern "C" int moebius_plan(moebius_ctx_t* x, moebius_mode_t from, moebius_mode_
       s.rows_total = (m < 2) ? (uint32_t)(c.E / R) * c.H : (uint32_t)(c.E / R);
       if (run > (1ll << 31)) return fail(MOEBIUS_E_INVAL);
       s.run_bytes = (uint32_t)run;
-      if (run * R <= unit_bytes || run <= 4096) {
+      s.desc_begin = (uint32_t)(k + x->ep_shift);   // EP slot index (tensor-map coordinate)
+      const int64_t stage = x->stage_bytes;
+      const uint32_t lt_chunk = pick_chunk(run, stage);
+      if (x->use_tma && m < 2 && x->xt_ok) {
+        // one tensor-map box per unit: xt_rows rows x all R groups
+        s.kind = SEG_XPOSE | (PATH_TMA << 8);
+        s.groups_per_unit = R;
+        s.chunk_bytes = (uint32_t)run;
+        s.chunks_per_run = 1;
+        s.rows_per_unit = (uint32_t)x->xt_rows;
+      } else if (x->use_tma && (run > 1024 || run * R > stage) && (lt_chunk == run || lt_chunk >= 4096)) {
+        // one group per unit: plain bulk copies (long runs: the down projection)
+        s.kind = SEG_XPOSE | (PATH_TMA << 8);
+        s.groups_per_unit = 1;
+        s.chunk_bytes = lt_chunk;
+        s.chunks_per_run = (uint32_t)(run / s.chunk_bytes);
+        s.rows_per_unit = s.chunks_per_run == 1 ? (uint32_t)std::min<int64_t>(32, std::max<int64_t>(1, stage / run)) : 1;
+      } else if (run * R <= unit_bytes || run <= 4096) {
         s.groups_per_unit = R;
         s.chunk_bytes = (uint32_t)run;
         s.chunks_per_run = 1;
@@ -519,6 +568,8 @@ extern "C" int moebius_plan(moebius_ctx_t* x, moebius_mode_t from, moebius_mode_
       s.wait_ctr = prev_ctr; s.wait_target = prev_units;
       s.signal_ctr = (int32_t)next_ctr++;
       prev_ctr = s.signal_ctr; prev_units = s.n_units;
+      if (getenv("MOEBIUS_DEBUG_NOWAIT")) { s.wait_ctr = -1; s.signal_ctr = -1; }        // DEBUG timing experiments only
+      if (getenv("MOEBIUS_DEBUG_ONLY") && atoi(getenv("MOEBIUS_DEBUG_ONLY")) != (m < 2 ? 1 : 2)) continue;  // DEBUG
       push_seg(cw, s);
     }
     int64_t all = (int64_t)3 * L * c.E * c.H * c.I * x->wb;
@@ -590,10 +641,14 @@ extern "C" int moebius_plan(moebius_ctx_t* x, moebius_mode_t from, moebius_mode_
       d.ntok_slot = (uint32_t)mv[m].ntok | (mv[m].staged ? ((uint32_t)mv[m].slot << 8) : 0u);
       if (mv[m].staged) P->kv[scur++] = d; else P->kv[cur[mv[m].level]++] = d;
     }
-    uint32_t ppu = (uint32_t)std::max<int64_t>(1, std::min<int64_t>(unit_bytes / x->ep_page_bytes, 2));
+    const uint32_t ppu_lsu = (uint32_t)std::max<int64_t>(1, std::min<int64_t>(unit_bytes / x->ep_page_bytes, 2));
+    const bool kv_tma = x->use_tma && x->kt_ok;
+    uint32_t ppu = kv_tma ? (uint32_t)x->kt_pools : ppu_lsu;
     auto kv_seg = [&](uint32_t mode, uint32_t ep_src, uint32_t d0, uint32_t nd, int pool0, int npool) {
       Seg s = blank_seg();
-      s.kind = SEG_KV;
+      const bool tma = kv_tma && mode == KV_MOVE;
+      const uint32_t ppu = tma ? (uint32_t)x->kt_pools : ppu_lsu;
+      s.kind = SEG_KV | ((tma ? PATH_TMA : PATH_LSU) << 8);
       s.kv_mode = mode;
       s.ep_is_src = ep_src;
       s.run_bytes = (uint32_t)x->run_kv;
@@ -692,6 +747,10 @@ extern "C" int moebius_plan(moebius_ctx_t* x, moebius_mode_t from, moebius_mode_
     return fail(MOEBIUS_E_INVAL);
   P->total_units = (uint32_t)ub;
   P->n_counters = next_ctr;
+  P->uses_tma = false;
+  for (const Seg& s : P->segs) if (seg_path(s) == PATH_TMA) P->uses_tma = true;
+  P->stage_bytes = x->stage_bytes;
+  P->xt_rows = x->xt_rows;
 
   // ---- target request state + upload images -----------------------------------------------------
   P->lens.assign(seq_lens, seq_lens + n_req);

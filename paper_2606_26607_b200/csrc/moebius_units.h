@@ -30,9 +30,18 @@ namespace moebius {
 
 enum : uint32_t { SEG_XPOSE = 0, SEG_KV = 1, SEG_COPY2D = 2 };
 enum : uint32_t { KV_MOVE = 0, KV_MOVE_STG = 1, KV_STG_COPY = 2 };
+// How the kernel executes a segment's units (bits 8..15 of Seg::kind).  The unit geometry is the
+// same for both paths (decode_box below is the single definition); only the data path differs:
+//   PATH_LSU  one warp copies the unit with 16-byte ld.global / st.global
+//   PATH_TMA  one elected lane moves it through a shared-memory stage with TMA: the EP side is ONE
+//             cp.async.bulk.tensor over a 5-D tensor map whose box is the whole unit (the run
+//             transposition happens in the box: smem holds [group][row][run]), the TP side is one
+//             contiguous cp.async.bulk per (group, replica).  Units with a single group (chunks of
+//             long runs, e.g. the down projection) use plain 1-D bulk copies on both sides.
+enum : uint32_t { PATH_LSU = 0, PATH_TMA = 1 };
 
 struct Seg {              // 128 bytes, uploaded verbatim
-  uint32_t kind;
+  uint32_t kind;          // bits 0..7: SEG_*; bits 8..15: PATH_*
   uint32_t ep_is_src;     // 1: EP side is read, TP side written (EP->TP); 0: the reverse
   int32_t  wait_ctr;      // -1: none
   uint32_t wait_target;
@@ -51,7 +60,7 @@ struct Seg {              // 128 bytes, uploaded verbatim
   int64_t  ep_off;           // XPOSE: EP view offset in the rank region; KV: pool 0 offset
   int64_t  tp_off;           // XPOSE: TP view offset in the rank region; KV: == ep_off
   uint32_t kv_mode;
-  uint32_t desc_begin;       // first descriptor (KV move or C2D) of this segment
+  uint32_t desc_begin;       // first descriptor (KV move or C2D) of this segment; XPOSE: EP slot index
   uint32_t n_desc;
   uint32_t pool_begin;       // KV: first pool (z = 2*layer + {K:0,V:1}) of this segment
   uint32_t n_pools;
@@ -90,7 +99,14 @@ struct DevParams {        // kernel arguments
   int64_t          rank_stride;
   uint32_t         n_segs;
   uint32_t         total_units;
+  uint32_t         stage_bytes;   // PATH_TMA: bytes of one shared-memory stage (2 per pipe)
+  uint32_t         xt_rows;       // PATH_TMA: rows of the weight tensor-map box (= rows_per_unit)
+  uint32_t         page_tokens;
+  uint32_t         pad_;
 };
+
+MB_HD uint32_t seg_kind(const Seg& s) { return s.kind & 0xFFu; }
+MB_HD uint32_t seg_path(const Seg& s) { return (s.kind >> 8) & 0xFFu; }
 
 // One executable shape.  lin != 0: contiguous copy of lin_bytes from src to dst.
 struct Box {
@@ -106,10 +122,18 @@ struct Box {
   uint64_t lin_bytes;
 };
 
+// KV unit u of a segment = (pool block pb, descriptor di), pool-block-major: consecutive units are
+// consecutive page descriptors of the SAME pools, so concurrently running pipes touch neighbouring
+// pages (canonical tables hand out consecutive pages) instead of 2L pools x R ranks far apart.
+MB_HD void kv_unit(const Seg& s, uint32_t u, uint32_t& pb, uint32_t& di) {
+  pb = u / s.n_desc;
+  di = u - pb * s.n_desc;
+}
+
 MB_HD uint32_t seg_boxes(const Seg& s, uint32_t u) {
-  if (s.kind != SEG_KV) return 1;
-  uint32_t pool_blocks = (s.n_pools + s.pools_per_unit - 1) / s.pools_per_unit;
-  uint32_t pb = u % pool_blocks;
+  if (seg_kind(s) != SEG_KV) return 1;
+  uint32_t pb, di;
+  kv_unit(s, u, pb, di);
   uint32_t z0 = pb * s.pools_per_unit;
   uint32_t n = s.n_pools - z0;
   return n < s.pools_per_unit ? n : s.pools_per_unit;
@@ -127,7 +151,7 @@ MB_HD void decode_box(const Seg& s, const DevParams& p, uint32_t u, uint32_t k, 
   b.run_bytes = s.run_bytes;
   b.rep = s.rep;
   b.tp_row_stride = s.run_bytes;
-  if (s.kind == SEG_XPOSE) {
+  if (seg_kind(s) == SEG_XPOSE) {
     uint32_t ch = u % s.chunks_per_run;  u /= s.chunks_per_run;
     uint32_t jgroups = s.n_groups / s.groups_per_unit;
     uint32_t jg = u % jgroups;           u /= jgroups;
@@ -149,9 +173,8 @@ MB_HD void decode_box(const Seg& s, const DevParams& p, uint32_t u, uint32_t k, 
     return;
   }
   // SEG_KV
-  uint32_t pool_blocks = (s.n_pools + s.pools_per_unit - 1) / s.pools_per_unit;
-  uint32_t pb = u % pool_blocks;
-  uint32_t di = u / pool_blocks;
+  uint32_t pb, di;
+  kv_unit(s, u, pb, di);
   uint32_t z = s.pool_begin + pb * s.pools_per_unit + k;
   KvDesc d = p.kv[s.desc_begin + di];
   uint32_t ntok = d.ntok_slot & 0xFFu;

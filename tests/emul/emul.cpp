@@ -88,7 +88,7 @@ int emul_run(char* base, int64_t base_bytes, char* stg, int64_t stg_bytes, const
     if (s.unit_begin != expect_begin) ++bad_begin;
     expect_begin += s.n_units;
     for (uint32_t u = 0; u < s.n_units; ++u) {
-      if (s.kind == SEG_COPY2D) {
+      if (seg_kind(s) == SEG_COPY2D) {
         const C2dDesc& d = c2d[s.desc_begin + u];
         for (uint32_t r = 0; r < d.rows; ++r) {
           // scales are 4-byte granular: account at 16-byte chunk level only for bounds, copy bytes
@@ -130,6 +130,18 @@ int emul_run(char* base, int64_t base_bytes, char* stg, int64_t stg_bytes, const
             ck.on_read(src, si, 16);
             ck.on_write(ep, si, 16);
             if (ck.chunk_of(ep) >= 0 && ck.chunk_of(src) >= 0) memcpy(ep, src, 16);
+          }
+        }
+        // PATH_TMA, TP->EP page move: the tensor-map store writes the WHOLE EP page box, so the
+        // slots past the valid tokens receive unspecified bytes (reading A10)
+        if (seg_path(s) == PATH_TMA && seg_kind(s) == SEG_KV && !s.ep_is_src) {
+          uint32_t row_bytes = s.n_groups * s.run_bytes;
+          uint32_t pg = s.ep_page_bytes / row_bytes;
+          for (uint32_t t = b.nrows; t < pg; ++t) {
+            char* row = b.ep + (int64_t)t * row_bytes;
+            ck.on_write(row, si, (int)row_bytes);
+            if (ck.chunk_of(row) >= 0 && ck.chunk_of(row + row_bytes - 16) >= 0) memset(row, 0xEE, row_bytes);
+            ck.bytes_written -= row_bytes;   // not part of the accounted (valid-token) bytes
           }
         }
       }

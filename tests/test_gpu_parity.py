@@ -20,11 +20,13 @@ GUARD = 4096
 CANARY = 0xC3
 
 
-def gpu_session(cfg, lens=None, policy=None, cap_frac=0.0, pool_bytes=None, fill="tag", initial_mode=TP):
+def gpu_session(cfg, lens=None, policy=None, cap_frac=0.0, pool_bytes=None, fill="tag", initial_mode=TP, tma=None):
     assert torch.cuda.is_available(), "GPU tests need a CUDA device (there is no CPU fallback)"
     st = State(cfg, lens, fill=fill)
     sess = mb.Session(mb_config(cfg, st.lens, policy, cap_frac, pool_bytes), device="cuda:0", guard_bytes=GUARD,
                       initial_mode=initial_mode)
+    if tma is not None:
+        mb.moebius_set_tma(sess.ctx, *tma)
     sess.arena.fill_(CANARY)
     return st, sess
 
@@ -191,13 +193,36 @@ def test_small_config_alternating():
     sess.close()
 
 
-@pytest.mark.parametrize("threads,ctas,unit_kb", [(128, 1, 4), (512, 2, 64), (256, 8, 16)])
+@pytest.mark.parametrize("threads,ctas,unit_kb", [(128, 1, 4), (256, 2, 64), (64, 8, 16)])
 def test_launch_shapes(threads, ctas, unit_kb):
-    """The result does not depend on the launch shape or the unit size."""
-    st, sess = gpu_session(SMALLISH, initial_mode=EP)
+    """ld/st path only (TMA off): the result does not depend on the launch shape or the unit size."""
+    st, sess = gpu_session(SMALLISH, initial_mode=EP, tma=(0, 0, 0))
     mb.moebius_set_launch(sess.ctx, ctas, threads, unit_kb)
     owner, bt, _ = start(st, sess, EP, "random")
     mode, owner, bt, _ = gpu_switch(st, sess, EP, owner, bt)
+    gpu_switch(st, sess, mode, owner, bt)
+    sess.close()
+
+
+@pytest.mark.parametrize("pipes,stage_kb", [(1, 96), (2, 48), (4, 24), (8, 8), (2, 16)])
+@pytest.mark.parametrize("first", [TP, EP])
+def test_tma_shapes(first, pipes, stage_kb):
+    """TMA path: the result does not depend on the number of pipes or the stage size (which sets the
+    rows per tensor-map box and the pools per KV unit); ragged last row blocks and partial pages."""
+    st, sess = gpu_session(SMALLISH, initial_mode=first, tma=(1, pipes, stage_kb))
+    owner, bt, _ = start(st, sess, first, "random")
+    mode, owner, bt, _ = gpu_switch(st, sess, first, owner, bt)
+    gpu_switch(st, sess, mode, owner, bt)
+    sess.close()
+
+
+@pytest.mark.parametrize("tma", [0, 1])
+def test_small_config_both_paths(tma):
+    """BASELINE.json config 2 on the ld/st path and on the TMA path: identical results."""
+    cfg = wl.get_config("small")
+    st, sess = gpu_session(cfg, tma=(tma, 0, 0))
+    owner, bt, _ = start(st, sess, TP, "random")
+    mode, owner, bt, _ = gpu_switch(st, sess, TP, owner, bt)
     gpu_switch(st, sess, mode, owner, bt)
     sess.close()
 
