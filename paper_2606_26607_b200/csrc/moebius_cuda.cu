@@ -164,13 +164,28 @@ __device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.
 
 // One unit through one stage.  Geometry comes from decode_box / the segment, exactly as on the LSU
 // path; smem layout of a stage: XT [group][xt_rows][run], LT [row][chunk], KT [pool][group][page][run].
+// The whole warp calls these: lane l issues operations l, l+32, ... of the unit (a unit is up to
+// pools x groups x replicas bulk copies), so address arithmetic and issue run in parallel.  Bulk
+// async-groups are per thread, hence every lane commits and waits on its own groups in lockstep.
 struct TmaCtx {
   const DevParams* p;
   const CUtensorMap* tm_w;
   const CUtensorMap* tm_kv;
 };
 
-__device__ __forceinline__ void tma_issue_load(const TmaCtx& c, const Seg& s, uint32_t ul, char* stage, uint64_t* bar) {
+__device__ __forceinline__ KvDesc tma_prefetch_desc(const DevParams& p, const Seg& s, uint32_t ul) {
+  KvDesc d = {0, 0, 0, 0};
+  if (seg_kind(s) == SEG_KV) {
+    uint32_t pb, di;
+    kv_unit(s, ul, pb, di);
+    const int4 v = __ldg((const int4*)(p.kv + s.desc_begin + di));
+    d.ep_rank = v.x; d.ep_page = v.y; d.tp_page = v.z; d.ntok_slot = (uint32_t)v.w;
+  }
+  return d;
+}
+
+__device__ __forceinline__ void tma_issue_load(const TmaCtx& c, const Seg& s, uint32_t ul, const KvDesc& d, char* stage,
+                                               uint64_t* bar, uint32_t lane) {
   const DevParams& p = *c.p;
   if (seg_kind(s) == SEG_XPOSE) {
     Box b;
@@ -179,20 +194,24 @@ __device__ __forceinline__ void tma_issue_load(const TmaCtx& c, const Seg& s, ui
       const uint32_t q = ul / s.row_blocks, row0 = (ul % s.row_blocks) * s.rows_per_unit;
       const uint32_t piece = p.xt_rows * s.run_bytes;
       if (s.ep_is_src) {
-        mbar_expect_tx(bar, piece * s.n_groups);     // the box is always delivered whole (rows past the end are zero-filled)
-        tma_load_5d(stage, c.tm_w, 0, (int)row0, 0, (int)q, (int)s.desc_begin, bar);
+        if (lane == 0) {
+          mbar_expect_tx(bar, piece * s.n_groups);   // the box is always delivered whole (rows past the end are zero-filled)
+          tma_load_5d(stage, c.tm_w, 0, (int)row0, 0, (int)q, (int)s.desc_begin, bar);
+        }
       } else {
         const uint32_t bytes = b.nrows * s.run_bytes;
-        mbar_expect_tx(bar, bytes * s.n_groups);
-        for (uint32_t g = 0; g < s.n_groups; ++g)
+        if (lane == 0) mbar_expect_tx(bar, bytes * s.n_groups);
+        __syncwarp();
+        for (uint32_t g = lane; g < s.n_groups; g += 32)
           bulk_g2s(stage + (size_t)g * piece, b.tp + (int64_t)g * p.rank_stride, bytes, bar);
       }
     } else {                                          // LT: one group, nrows pieces of chunk bytes
       const uint32_t chunk = s.chunk_bytes;
-      mbar_expect_tx(bar, b.nrows * chunk);
+      if (lane == 0) mbar_expect_tx(bar, b.nrows * chunk);
+      __syncwarp();
       if (s.ep_is_src) {
-        for (uint32_t t = 0; t < b.nrows; ++t) bulk_g2s(stage + (size_t)t * chunk, b.ep + (int64_t)t * b.ep_row_stride, chunk, bar);
-      } else {
+        for (uint32_t t = lane; t < b.nrows; t += 32) bulk_g2s(stage + (size_t)t * chunk, b.ep + (int64_t)t * b.ep_row_stride, chunk, bar);
+      } else if (lane == 0) {
         bulk_g2s(stage, b.tp + (int64_t)b.g0 * p.rank_stride, b.nrows * chunk, bar);
       }
     }
@@ -203,25 +222,27 @@ __device__ __forceinline__ void tma_issue_load(const TmaCtx& c, const Seg& s, ui
   kv_unit(s, ul, pb, di);
   const uint32_t nb = seg_boxes(s, ul);
   const uint32_t z0 = s.pool_begin + pb * s.pools_per_unit;
-  const KvDesc d = p.kv[s.desc_begin + di];
   const uint32_t ntok = d.ntok_slot & 0xFFu;
   if (s.ep_is_src) {
-    mbar_expect_tx(bar, nb * s.ep_page_bytes);
-    for (uint32_t k = 0; k < nb; ++k)
+    if (lane == 0) mbar_expect_tx(bar, nb * s.ep_page_bytes);
+    __syncwarp();
+    for (uint32_t k = lane; k < nb; k += 32)
       tma_load_5d(stage + (size_t)k * s.ep_page_bytes, c.tm_kv, 0, (int)(d.ep_page * p.page_tokens), 0, (int)(z0 + k), d.ep_rank, bar);
   } else {
     const uint32_t bytes = ntok * s.run_bytes;
-    mbar_expect_tx(bar, nb * s.n_groups * bytes);
-    for (uint32_t k = 0; k < nb; ++k) {
-      const char* pool = p.base + s.ep_off + (int64_t)(z0 + k) * s.pool_bytes + (int64_t)d.tp_page * s.tp_page_bytes;
-      for (uint32_t g = 0; g < s.n_groups; ++g)
-        bulk_g2s(stage + (size_t)k * s.ep_page_bytes + (size_t)g * s.tp_page_bytes,
-                 pool + (int64_t)tp_src_rank(g, s.rep, d.ep_rank) * p.rank_stride, bytes, bar);
+    if (lane == 0) mbar_expect_tx(bar, nb * s.n_groups * bytes);
+    __syncwarp();
+    for (uint32_t o = lane; o < nb * s.n_groups; o += 32) {
+      const uint32_t k = o / s.n_groups, g = o - k * s.n_groups;
+      const char* src = p.base + s.ep_off + (int64_t)(z0 + k) * s.pool_bytes + (int64_t)d.tp_page * s.tp_page_bytes +
+                        (int64_t)tp_src_rank(g, s.rep, d.ep_rank) * p.rank_stride;
+      bulk_g2s(stage + (size_t)k * s.ep_page_bytes + (size_t)g * s.tp_page_bytes, src, bytes, bar);
     }
   }
 }
 
-__device__ __forceinline__ void tma_issue_store(const TmaCtx& c, const Seg& s, uint32_t ul, char* stage) {
+__device__ __forceinline__ void tma_issue_store(const TmaCtx& c, const Seg& s, uint32_t ul, const KvDesc& d, char* stage,
+                                                uint32_t lane) {
   const DevParams& p = *c.p;
   if (seg_kind(s) == SEG_XPOSE) {
     Box b;
@@ -231,17 +252,17 @@ __device__ __forceinline__ void tma_issue_store(const TmaCtx& c, const Seg& s, u
       const uint32_t piece = p.xt_rows * s.run_bytes;
       if (s.ep_is_src) {
         const uint32_t bytes = b.nrows * s.run_bytes;
-        for (uint32_t g = 0; g < s.n_groups; ++g)
+        for (uint32_t g = lane; g < s.n_groups; g += 32)
           bulk_s2g(b.tp + (int64_t)g * p.rank_stride, stage + (size_t)g * piece, bytes);
-      } else {
+      } else if (lane == 0) {
         tma_store_5d(c.tm_w, 0, (int)row0, 0, (int)q, (int)s.desc_begin, stage);   // rows past the end are clipped
       }
     } else {                                          // LT
       const uint32_t chunk = s.chunk_bytes;
       if (s.ep_is_src) {
-        bulk_s2g(b.tp + (int64_t)b.g0 * p.rank_stride, stage, b.nrows * chunk);
+        if (lane == 0) bulk_s2g(b.tp + (int64_t)b.g0 * p.rank_stride, stage, b.nrows * chunk);
       } else {
-        for (uint32_t t = 0; t < b.nrows; ++t) bulk_s2g(b.ep + (int64_t)t * b.ep_row_stride, stage + (size_t)t * chunk, chunk);
+        for (uint32_t t = lane; t < b.nrows; t += 32) bulk_s2g(b.ep + (int64_t)t * b.ep_row_stride, stage + (size_t)t * chunk, chunk);
       }
     }
     bulk_commit();
@@ -251,20 +272,19 @@ __device__ __forceinline__ void tma_issue_store(const TmaCtx& c, const Seg& s, u
   kv_unit(s, ul, pb, di);
   const uint32_t nb = seg_boxes(s, ul);
   const uint32_t z0 = s.pool_begin + pb * s.pools_per_unit;
-  const KvDesc d = p.kv[s.desc_begin + di];
   const uint32_t ntok = d.ntok_slot & 0xFFu;
   if (s.ep_is_src) {
     const uint32_t bytes = ntok * s.run_bytes;
-    for (uint32_t k = 0; k < nb; ++k) {
-      char* pool = p.base + s.ep_off + (int64_t)(z0 + k) * s.pool_bytes + (int64_t)d.tp_page * s.tp_page_bytes;
-      for (uint32_t g = 0; g < s.n_groups; ++g)
-        for (uint32_t r = 0; r < s.rep; ++r)
-          bulk_s2g(pool + (int64_t)(g * s.rep + r) * p.rank_stride,
-                   stage + (size_t)k * s.ep_page_bytes + (size_t)g * s.tp_page_bytes, bytes);
+    const uint32_t per_pool = s.n_groups * s.rep;
+    for (uint32_t o = lane; o < nb * per_pool; o += 32) {
+      const uint32_t k = o / per_pool, gr = o - k * per_pool, g = gr / s.rep;   // gr = g*rep + r = destination rank
+      char* dst = p.base + s.ep_off + (int64_t)(z0 + k) * s.pool_bytes + (int64_t)d.tp_page * s.tp_page_bytes +
+                  (int64_t)gr * p.rank_stride;
+      bulk_s2g(dst, stage + (size_t)k * s.ep_page_bytes + (size_t)g * s.tp_page_bytes, bytes);
     }
   } else {
     // the whole page box is written: slots past the valid tokens get unspecified bytes (reading A10)
-    for (uint32_t k = 0; k < nb; ++k)
+    for (uint32_t k = lane; k < nb; k += 32)
       tma_store_5d(c.tm_kv, 0, (int)(d.ep_page * p.page_tokens), 0, (int)(z0 + k), d.ep_rank, stage + (size_t)k * s.ep_page_bytes);
   }
   bulk_commit();
@@ -290,7 +310,8 @@ __device__ __forceinline__ void lsu_unit(const Seg& s, const DevParams& p, uint3
 // while the stores of unit i drain (lane 0 issues everything; measured best among 1-6 pipes x 2-4
 // stages).  PATH_LSU units are copied by the whole warp.  Before a pipe blocks on a
 // dependency counter it drains its own pipeline, so waits can never be circular.
-__global__ void __launch_bounds__(256, 2)
+template <int kMinCtasPerSm>   // 1: plans with PATH_TMA segments (shared-memory bound); 2: ld/st-only plans
+__global__ void __launch_bounds__(256, kMinCtasPerSm)
 moebius_reshard_kernel(const __grid_constant__ DevParams p, const __grid_constant__ CUtensorMap tm_w,
                        const __grid_constant__ CUtensorMap tm_kv) {
   extern __shared__ __align__(1024) char smem[];
@@ -308,6 +329,7 @@ moebius_reshard_kernel(const __grid_constant__ DevParams p, const __grid_constan
   // pipe state; identical in every lane (it depends on uniform values only)
   bool loading = false;           // a unit's loads are in flight
   uint32_t ld_si = 0, ld_ul = 0, ld_stage = 0;
+  KvDesc ld_d = {0, 0, 0, 0};
   uint32_t phase0 = 0, phase1 = 0;
   uint32_t next_stage = 0;
   // completion signals are batched: units whose store groups are committed but not yet signalled all
@@ -316,18 +338,19 @@ moebius_reshard_kernel(const __grid_constant__ DevParams p, const __grid_constan
   int32_t pend_ctr = -1;
   uint32_t pend_n = 0;
 
-  auto publish = [&]() {                // lane 0, after the pending units' writes have completed
-    if (pend_ctr >= 0 && pend_n) { fence_proxy_async(); __threadfence(); atomicAdd(p.counters + pend_ctr, pend_n); }
+  auto publish = [&]() {                // after every lane's pending writes have completed
+    fence_proxy_async();
+    __syncwarp();
+    if (lane == 0 && pend_ctr >= 0 && pend_n) { __threadfence(); atomicAdd(p.counters + pend_ctr, pend_n); }
   };
   auto retire = [&]() {                  // loads landed -> issue the stores of the loading unit
     if (!loading) return;
     const Seg& s = p.segs[ld_si];
     const int32_t ctr = s.signal_ctr;
-    if (lane == 0) {
-      mbar_wait(bar + ld_stage, ld_stage ? phase1 : phase0);
-      tma_issue_store(tc, s, ld_ul, ring + (size_t)ld_stage * p.stage_bytes);
-      if (ctr != pend_ctr && pend_ctr >= 0 && pend_n) { bulk_wait<1>(); publish(); }   // all but the group just committed
-    }
+    if (lane == 0) mbar_wait(bar + ld_stage, ld_stage ? phase1 : phase0);
+    __syncwarp();
+    tma_issue_store(tc, s, ld_ul, ld_d, ring + (size_t)ld_stage * p.stage_bytes, lane);
+    if (ctr != pend_ctr && pend_ctr >= 0 && pend_n) { bulk_wait<1>(); publish(); }   // all but the group just committed
     if (ld_stage) phase1 ^= 1; else phase0 ^= 1;
     if (ctr != pend_ctr) { pend_ctr = ctr; pend_n = 0; }
     ++pend_n;
@@ -335,12 +358,15 @@ moebius_reshard_kernel(const __grid_constant__ DevParams p, const __grid_constan
   };
   auto drain = [&]() {                   // everything this pipe has in flight completes and is signalled
     retire();
-    if (lane == 0) { bulk_wait<0>(); publish(); }
+    bulk_wait<0>();
+    publish();
     pend_n = 0;
     __syncwarp();
   };
-  auto wait_for = [&](const Seg& s) {    // dependency of a segment (rare: chain links, KV rounds)
-    if (s.wait_ctr < 0) return;
+  uint32_t ok_si = 0xffffffffu;          // segment whose dependency this pipe has already seen satisfied
+  auto wait_for = [&](const Seg& s, uint32_t si) {   // dependency of a segment (chain links, KV rounds)
+    if (s.wait_ctr < 0 || si == ok_si) return;       // one acquire-load per segment, not per unit
+    ok_si = si;
     uint32_t ok = 0;
     if (lane == 0) ok = ld_acquire(p.counters + s.wait_ctr) >= s.wait_target;
     ok = __shfl_sync(0xffffffffu, ok, 0);
@@ -353,8 +379,8 @@ moebius_reshard_kernel(const __grid_constant__ DevParams p, const __grid_constan
         }
       }
     }
-    if (lane == 0) fence_proxy_async();
     __syncwarp();
+    fence_proxy_async();     // every lane issues TMA reads of what the signalling units wrote
   };
   auto fetch = [&]() -> uint32_t { return lane == 0 ? atomicAdd(p.ticket, 1u) : 0u; };
 
@@ -375,18 +401,17 @@ moebius_reshard_kernel(const __grid_constant__ DevParams p, const __grid_constan
     const Seg& s = p.segs[si];
     const uint32_t ul = u - s.unit_begin;
     if (seg_path(s) == PATH_TMA) {
+      const KvDesc d = tma_prefetch_desc(p, s, ul);   // its latency hides behind the wait in retire()
       retire();
-      wait_for(s);
-      if (lane == 0) {
-        bulk_wait_read<1>();   // the stage about to be refilled was read by the store group before the last one
-        tma_issue_load(tc, s, ul, ring + (size_t)next_stage * p.stage_bytes, bar + next_stage);
-      }
-      loading = true; ld_si = si; ld_ul = ul; ld_stage = next_stage;
+      wait_for(s, si);
+      bulk_wait_read<1>();     // the stage about to be refilled was read by the store group before the last one
+      tma_issue_load(tc, s, ul, d, ring + (size_t)next_stage * p.stage_bytes, bar + next_stage, lane);
+      loading = true; ld_si = si; ld_ul = ul; ld_stage = next_stage; ld_d = d;
       next_stage ^= 1;
       t_next = fetch();        // its latency hides behind the loads just issued
     } else {
       t_next = fetch();
-      wait_for(s);
+      wait_for(s, si);
       lsu_unit(s, p, ul, lane);
       if (s.signal_ctr >= 0) {
         __syncwarp();
@@ -576,7 +601,7 @@ extern "C" int moebius_reshard(moebius_ctx_t* x, const moebius_plan_t* P, void* 
       per_sm = 1;
       smem = 1024 + (size_t)x->n_pipes * 2 * (size_t)x->stage_bytes;
       if (smem != x->smem_set) {
-        if (cudaFuncSetAttribute(moebius_reshard_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess)
+        if (cudaFuncSetAttribute(moebius_reshard_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess)
           return MOEBIUS_E_CUDA;
         x->smem_set = smem;
       }
@@ -588,7 +613,10 @@ extern "C" int moebius_reshard(moebius_ctx_t* x, const moebius_plan_t* P, void* 
     int64_t grid_cap = ((int64_t)P->total_units + threads / 32 - 1) / (threads / 32);
     if (grid > grid_cap) grid = grid_cap;
     if (x->timing) cudaEventRecord(ev_a, st);
-    moebius_reshard_kernel<<<(unsigned)grid, threads, smem, st>>>(p, *(const CUtensorMap*)x->tmap_w, *(const CUtensorMap*)x->tmap_kv);
+    if (P->uses_tma)
+      moebius_reshard_kernel<1><<<(unsigned)grid, threads, smem, st>>>(p, *(const CUtensorMap*)x->tmap_w, *(const CUtensorMap*)x->tmap_kv);
+    else
+      moebius_reshard_kernel<2><<<(unsigned)grid, threads, 0, st>>>(p, *(const CUtensorMap*)x->tmap_w, *(const CUtensorMap*)x->tmap_kv);
     if (cudaGetLastError() != cudaSuccess) return MOEBIUS_E_CUDA;
     if (x->timing) cudaEventRecord(ev_b, st);
   } else if (x->timing) {
