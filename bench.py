@@ -350,6 +350,20 @@ def run_moebius(args):
     return locals()
 
 
+def reduce_over_ranks(times_ms, amounts, world, device):
+    """Replicas only: every rank runs the same independent job on its own GPU, so the
+    whole-job figure is (sum over ranks of the bytes) / (max over ranks of the time).  No data-path
+    collective exists; these two all-reduces of a few scalars happen after the timed region."""
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor(list(times_ms), dtype=torch.float64, device=device)
+    b = torch.tensor(list(amounts), dtype=torch.float64, device=device)
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        dist.all_reduce(b, op=dist.ReduceOp.SUM)
+    return [float(x) for x in t], [float(x) for x in b]
+
+
 def main():
     args = parse()
     if args.impl == "reference":
@@ -360,14 +374,7 @@ def main():
     world, rank, cfg, steps = r["world"], r["rank"], r["cfg"], args.steps
     st_t2e, st_e2t = r["st_t2e"], r["st_e2t"]
     moved_step = st_t2e["w_moved"] + st_t2e["kv_moved"] + st_e2t["w_moved"] + st_e2t["kv_moved"]
-    # max over ranks of the device time and of the e2e host time; sum over ranks of the bytes
-    t = torch.tensor([r["dev_ms"], r["e2e_s"] * 1e3], dtype=torch.float64, device=r["dev"])
-    b = torch.tensor([float(moved_step)], dtype=torch.float64, device=r["dev"])
-    if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        dist.all_reduce(b, op=dist.ReduceOp.SUM)
-    dev_ms, e2e_ms = float(t[0]), float(t[1])
-    moved_all = float(b[0])
+    (dev_ms, e2e_ms), (moved_all,) = reduce_over_ranks([r["dev_ms"], r["e2e_s"] * 1e3], [float(moved_step)], world, r["dev"])
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()

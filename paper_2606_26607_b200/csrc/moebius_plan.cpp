@@ -568,8 +568,6 @@ extern "C" int moebius_plan(moebius_ctx_t* x, moebius_mode_t from, moebius_mode_
       s.wait_ctr = prev_ctr; s.wait_target = prev_units;
       s.signal_ctr = (int32_t)next_ctr++;
       prev_ctr = s.signal_ctr; prev_units = s.n_units;
-      if (getenv("MOEBIUS_DEBUG_NOWAIT")) { s.wait_ctr = -1; s.signal_ctr = -1; }        // DEBUG timing experiments only
-      if (getenv("MOEBIUS_DEBUG_ONLY") && atoi(getenv("MOEBIUS_DEBUG_ONLY")) != (m < 2 ? 1 : 2)) continue;  // DEBUG
       push_seg(cw, s);
     }
     int64_t all = (int64_t)3 * L * c.E * c.H * c.I * x->wb;

@@ -1,0 +1,237 @@
+"""Full-size parity in the launch configuration bench.py times (library defaults, roomy pools, spare +
+staging capped at 2.4 % of resident bytes), at BASELINE.json's own sizes.
+
+The ~143 GB state of config 4 cannot be built on the host.  The device is filled through
+tests/devfill.py: every element of the sampled objects = tag of its LOGICAL coordinate (the same
+counter-based generator as workloads.tag_fill_u16), everything else random bytes.  After each switch
+  * sampled objects -- whole (layer, matrix) expert tensors and whole (layer, K|V) pools, on every
+    rank -- are downloaded and compared bytewise with the views the oracle builds from the logical
+    tensors regenerated on the host with numpy;
+  * the block tables / owner vector (host copy and published device copy) are compared with the oracle;
+  * properties that hold at any size are checked on EVERY expert object: the multiset of a
+    (layer, matrix) object's elements over all ranks is unchanged by a switch (permutation-invariant
+    checksum), and TP -> EP -> TP restores every TP view exactly (position-weighted checksum).
+"""
+import numpy as np
+import pytest
+
+import devfill
+import oracle
+import workloads as wl
+from harness import EP, TP, mb
+
+torch = pytest.importorskip("torch")
+pytestmark = pytest.mark.gpu
+
+KINDS = ("gate", "up", "down")
+
+
+def bench_session(cfg, lens, cap_frac=0.024):
+    """The session bench.py builds: roomy pools, staging cap as a fraction of resident bytes."""
+    pool = wl.kv_pool_bytes(cfg, lens, "roomy")
+    mp = int(max([1] + [(int(x) + cfg.page - 1) // cfg.page for x in lens]))
+    c = mb.make_config(R=cfg.R, L=cfg.L, E=cfg.E, H=cfg.H, I=cfg.I, w_dtype=cfg.w_dtype, kv_heads=cfg.kv_heads,
+                       head_dim=cfg.head_dim, page_tokens=cfg.page, kv_pool_bytes_per_rank_layer=pool,
+                       max_requests=max(len(lens), 1), max_pages_per_request=mp, staging_cap_bytes=0)
+    probe = mb.Session(c)
+    c.staging_cap_bytes = int(cap_frac * probe.layout.resident_bytes)
+    probe.close()
+    return mb.Session(c, device="cuda:0"), mp
+
+
+def host_view(sess, mode, r, layer, tid):
+    return sess.view(mode, r, layer, tid).cpu().numpy()
+
+
+def check_weight_object(sess, cfg, mode, layer, kind, X):
+    for r in range(cfg.R):
+        want = oracle.tp_weight_view(X, kind, r, cfg.R) if mode == TP else oracle.ep_weight_view(X, r, cfg.R)
+        got = host_view(sess, mode, r, layer, KINDS.index(kind))
+        assert got.shape == want.shape
+        assert np.array_equal(got.view(np.uint8), np.ascontiguousarray(want).view(np.uint8)), (mode, layer, kind, r)
+
+
+def check_pool(sess, cfg, mode, layer, kvi, KV, lens, owner, bt, lay):
+    for r in range(cfg.R):
+        if mode == TP:
+            pool, mask = oracle.tp_pool_image(KV, lens, bt, r, cfg.R, cfg.kv_heads, cfg.head_dim, cfg.page, lay.pages_tp)
+        else:
+            pool, mask = oracle.ep_pool_image(KV, lens, owner, bt, r, cfg.kv_heads, cfg.head_dim, cfg.page, lay.pages_ep)
+        got = host_view(sess, mode, r, layer, 3 + kvi).view(np.uint16)
+        assert np.array_equal(got[mask], pool[mask]), (mode, layer, kvi, r)
+
+
+def object_sums(sess, cfg, mode):
+    """Permutation-invariant checksum of every (layer, matrix) object over all ranks."""
+    out = {}
+    for l in range(cfg.L):
+        for t in range(3):
+            out[(l, t)] = sum(int(sess.view(mode, r, l, t).sum(dtype=torch.int64)) for r in range(cfg.R))
+    return out
+
+
+def view_checksums(sess, cfg, mode):
+    return {(r, l, t): devfill.weighted_checksum(sess.view(mode, r, l, t))
+            for r in range(cfg.R) for l in range(cfg.L) for t in range(3)}
+
+
+def device_tables(sess, n, mp):
+    lay = sess.layout
+    t = sess.tables.cpu().numpy()
+    return (t[:16], t[lay.tbl_owner_off:lay.tbl_owner_off + n], t[lay.tbl_lens_off:lay.tbl_lens_off + n],
+            t[lay.tbl_bt_off:lay.tbl_bt_off + n * mp].reshape(n, mp))
+
+
+def switch_and_check_tables(sess, st_lens, to, owner, bt, frm, mp, cfg):
+    plan = sess.plan(to, st_lens, owner, bt, from_mode=frm)
+    sess.reshard(plan)
+    torch.cuda.synchronize()
+    got_owner, got_bt = sess.block_tables(plan, len(st_lens))
+    lay = sess.layout
+    want_owner = oracle.partition_requests(st_lens, cfg.R) if to == EP else None
+    want_bt = oracle.canonical_block_tables(st_lens, want_owner, "ep" if to == EP else "tp",
+                                            lay.pages_ep if to == EP else lay.pages_tp, cfg.page, mp)
+    assert np.array_equal(got_bt, want_bt)
+    if to == EP:
+        assert np.array_equal(got_owner, want_owner)
+    hdr, d_owner, d_lens, d_bt = device_tables(sess, len(st_lens), mp)
+    assert hdr[0] == to and hdr[1] == len(st_lens)
+    assert np.array_equal(d_bt, want_bt) and np.array_equal(d_lens, st_lens)
+    assert np.array_equal(d_owner, want_owner if to == EP else np.full(len(st_lens), -1, np.int32))
+    stats = mb.moebius_plan_stats(plan).as_dict()
+    sess.free_plan(plan)
+    return want_owner, want_bt, stats
+
+
+def test_qwen3_235b_sampled_parity():
+    """BASELINE.json config 4 (R=8, L=12, E=128, H=4096, I=1536 bf16, ~58 GB of experts; 512 requests,
+    lognormal lengths, 4 KV heads on 8 ranks), from seeded random source tables."""
+    assert torch.cuda.is_available()
+    cfg = wl.get_config("qwen3_235b")
+    lens = wl.draw_seq_lens(cfg)
+    sess, mp = bench_session(cfg, lens)
+    lay = sess.layout
+    assert (lay.weight_spare_bytes + lay.staging_bytes) <= 0.024 * lay.resident_bytes + 1
+    w_samples = [(0, "gate"), (5, "up"), (11, "down")]
+    kv_samples = [(0, 0), (11, 1)]
+    bt0 = wl.random_page_tables(lens, None, cfg.R, lay.pages_tp, cfg.page, mp, seed=cfg.seed)
+    devfill.fill_random(sess)
+    for l, kind in w_samples:
+        devfill.fill_tp_weight(sess, cfg, l, kind)
+    for l, kvi in kv_samples:
+        devfill.fill_tp_pool(sess, cfg, l, kvi, lens, bt0)
+    torch.cuda.synchronize()
+    sums0 = object_sums(sess, cfg, TP)
+    chk0 = view_checksums(sess, cfg, TP)
+
+    # the logical tensors of the samples, regenerated on the host (numpy)
+    X = {(l, kind): wl.gen_logical_weight(cfg, l, kind, fill="tag") for l, kind in w_samples}
+    KV = {(l, kvi): {i: wl.gen_kv_request(cfg, l, kvi, i, int(n), fill="tag") for i, n in enumerate(lens)}
+          for l, kvi in kv_samples}
+
+    owner, bt, stats = switch_and_check_tables(sess, lens, EP, None, bt0, TP, mp, cfg)
+    w = oracle.weight_bytes(cfg.R, cfg.L, cfg.E, cfg.H, cfg.I, 2, "tp2ep")
+    k = oracle.kv_bytes(lens, owner, cfg.R, cfg.L, cfg.kv_heads, cfg.head_dim, 2, "tp2ep")
+    assert (stats["w_moved"], stats["w_relocated"]) == (w["moved"], w["relocated"])
+    assert (stats["kv_moved"], stats["kv_relocated"], stats["kv_read"]) == (k["moved"], k["relocated"], k["read"])
+    for l, kind in w_samples:
+        check_weight_object(sess, cfg, EP, l, kind, X[(l, kind)])
+    for l, kvi in kv_samples:
+        check_pool(sess, cfg, EP, l, kvi, KV[(l, kvi)], lens, owner, bt, lay)
+    assert object_sums(sess, cfg, EP) == sums0
+
+    owner_ep = owner
+    _, bt_tp, stats = switch_and_check_tables(sess, lens, TP, owner_ep, bt, EP, mp, cfg)
+    k = oracle.kv_bytes(lens, owner_ep, cfg.R, cfg.L, cfg.kv_heads, cfg.head_dim, 2, "ep2tp")
+    assert (stats["kv_moved"], stats["kv_relocated"], stats["kv_read"]) == (k["moved"], k["relocated"], k["read"])
+    for l, kind in w_samples:
+        check_weight_object(sess, cfg, TP, l, kind, X[(l, kind)])
+    for l, kvi in kv_samples:
+        check_pool(sess, cfg, TP, l, kvi, KV[(l, kvi)], lens, None, bt_tp, lay)
+    assert object_sums(sess, cfg, TP) == sums0
+    assert view_checksums(sess, cfg, TP) == chk0        # the same before and after
+    sess.close()
+
+
+def test_fp8_graph_stress_fullsize():
+    """BASELINE.json config 5 at its own size: Qwen3-235B-shaped, R=8, 4 layers, fp8 e4m3 experts with
+    fp32 128x128 block scales, 2048 requests with a geometric tail; 8 back-to-back alternating switches
+    with the captured graph of the active mode replayed after each.  The graphs read whole sampled
+    expert objects, every scale tensor, and the sampled pools of the first requests through the
+    published tables, all via baked-in pointers."""
+    assert torch.cuda.is_available()
+    cfg = wl.get_config("fp8_graph")
+    lens = wl.draw_seq_lens(cfg)
+    n = len(lens)
+    sess, mp = bench_session(cfg, lens)
+    lay = sess.layout
+    w_samples = [(0, "up"), (3, "down")]
+    kv_samples = [(0, 1), (3, 0)]
+    n_kv_req = 24
+    bt0 = wl.random_page_tables(lens, None, cfg.R, lay.pages_tp, cfg.page, mp, seed=cfg.seed)
+    devfill.fill_random(sess)
+    for l, kind in w_samples:
+        devfill.fill_tp_weight(sess, cfg, l, kind)
+    for l, kvi in kv_samples:
+        devfill.fill_tp_pool(sess, cfg, l, kvi, lens, bt0)
+    S = {(l, kind): wl.gen_logical_scale(cfg, l, kind) for l in range(cfg.L) for kind in KINDS}
+    for (l, kind), s in S.items():           # scales are small: the oracle's TP views are uploaded
+        for r in range(cfg.R):
+            v = sess.view(TP, r, l, 5 + KINDS.index(kind))
+            v.copy_(torch.from_numpy(np.ascontiguousarray(oracle.tp_scale_view(s, kind, r, cfg.R, cfg.I))))
+    torch.cuda.synchronize()
+
+    graphs = {}
+    for mode in (TP, EP):                    # captured ONCE, before the first switch
+        g = {"w": {}, "s": {}, "kv": {}}
+        wv = {(r, l, kind): sess.view(mode, r, l, KINDS.index(kind)) for r in range(cfg.R) for l, kind in w_samples}
+        sv = {(r, l, kind): sess.view(mode, r, l, 5 + KINDS.index(kind)) for r in range(cfg.R) for (l, kind) in S}
+        kvv = {(r, l, kvi): sess.view(mode, r, l, 3 + kvi) for r in range(cfg.R) for l, kvi in kv_samples}
+        torch.cuda.synchronize()
+        graph = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(graph):
+            g["hdr"] = sess.tables[:16].clone()
+            g["owner"] = sess.tables[lay.tbl_owner_off:lay.tbl_owner_off + n].clone()
+            idx = sess.tables[lay.tbl_bt_off:lay.tbl_bt_off + n_kv_req * mp].clamp(min=0).long()
+            for key, v in wv.items():
+                g["w"][key] = v.clone()
+            for key, v in sv.items():
+                g["s"][key] = v.clone()
+            for key, v in kvv.items():
+                g["kv"][key] = v.index_select(0, idx)
+        g["graph"] = graph
+        graphs[mode] = g
+
+    X = {(l, kind): wl.gen_logical_weight(cfg, l, kind, fill="tag") for l, kind in w_samples}
+    KV = {(l, kvi): {i: wl.gen_kv_request(cfg, l, kvi, i, int(lens[i]), fill="tag") for i in range(n_kv_req)}
+          for l, kvi in kv_samples}
+    want_w = {}
+    for mode in (TP, EP):                    # the weights' views are the same after every switch into a mode
+        for l, kind in w_samples:
+            for r in range(cfg.R):
+                v = oracle.tp_weight_view(X[(l, kind)], kind, r, cfg.R) if mode == TP else oracle.ep_weight_view(X[(l, kind)], r, cfg.R)
+                want_w[(mode, r, l, kind)] = np.ascontiguousarray(v)
+    owner, bt, mode = None, bt0, TP
+    pg = cfg.page
+    for _ in range(8):
+        to = EP if mode == TP else TP
+        owner, bt, _ = switch_and_check_tables(sess, lens, to, owner, bt, mode, mp, cfg)
+        g = graphs[to]
+        g["graph"].replay()
+        torch.cuda.synchronize()
+        assert int(g["hdr"][0]) == to
+        for (r, l, kind), out in g["w"].items():
+            assert np.array_equal(out.cpu().numpy(), want_w[(to, r, l, kind)]), (to, r, l, kind)
+        for (r, l, kind), out in g["s"].items():
+            want = oracle.tp_scale_view(S[(l, kind)], kind, r, cfg.R, cfg.I) if to == TP else oracle.ep_scale_view(S[(l, kind)], r, cfg.R)
+            assert np.array_equal(out.cpu().numpy().view(np.uint32), np.ascontiguousarray(want).view(np.uint32)), (to, r, l, kind)
+        g_owner = g["owner"].cpu().numpy()
+        for (r, l, kvi), out in g["kv"].items():
+            got = out.cpu().numpy().view(np.uint16).reshape(n_kv_req, mp * pg, -1, cfg.head_dim)
+            heads = list(range(cfg.kv_heads)) if to == EP else oracle.kv_heads_of_rank(r, cfg.R, cfg.kv_heads)
+            for i in range(n_kv_req):
+                if to == EP and g_owner[i] != r:
+                    continue
+                assert np.array_equal(got[i, :int(lens[i])], KV[(l, kvi)][i][:, heads, :]), (to, r, l, kvi, i)
+        mode = to
+    sess.close()

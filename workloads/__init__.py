@@ -15,4 +15,8 @@ from .gen import (  # noqa: F401
     random_page_tables,
     kv_pool_bytes,
     tag_fill_u16,
+    tag_fill_u16_torch,
+    tag_salt_offset,
+    weight_tag_salt,
+    kv_tag_salt,
 )

@@ -20,16 +20,46 @@ def _np_dtype(w_dtype: str):
 def tag_fill_u16(shape, salt: int) -> np.ndarray:
     """Coordinate-tag fill: element value = 16-bit hash of (salt, flat logical index).
 
-    Random bf16 values repeat; a tag makes a misplaced element visible."""
+    Random bf16 values repeat; a tag makes a misplaced element visible.
+    Generated in blocks so that a full-size tensor (8e8 elements) needs no multi-GB temporaries."""
     n = int(np.prod(shape))
-    idx = np.arange(n, dtype=np.uint64)
+    out = np.empty(n, dtype=np.uint16)
     off = np.uint64((int(salt) * 0x9E3779B97F4A7C15) & 0xFFFFFFFFFFFFFFFF)
+    step = 1 << 24
     with np.errstate(over="ignore"):
-        h = idx + off
-        h ^= h >> np.uint64(33)
-        h = h * np.uint64(0xFF51AFD7ED558CCD)
-        h ^= h >> np.uint64(29)
-    return (h & np.uint64(0xFFFF)).astype(np.uint16).reshape(shape)
+        for a in range(0, n, step):
+            h = np.arange(a, min(n, a + step), dtype=np.uint64) + off
+            h ^= h >> np.uint64(33)
+            h *= np.uint64(0xFF51AFD7ED558CCD)
+            h ^= h >> np.uint64(29)
+            out[a:a + step] = (h & np.uint64(0xFFFF)).astype(np.uint16)
+    return out.reshape(shape)
+
+
+def tag_salt_offset(salt: int) -> int:
+    """The additive offset tag_fill_u16 derives from a salt, as a signed 64-bit integer."""
+    off = (int(salt) * 0x9E3779B97F4A7C15) & 0xFFFFFFFFFFFFFFFF
+    return off - (1 << 64) if off >= (1 << 63) else off
+
+
+def tag_fill_u16_torch(flat_index, offset):
+    """The same counter-based generator as tag_fill_u16, on torch int64 tensors (any device):
+    `flat_index` = flat logical index of each element, `offset` = tag_salt_offset(salt) (a Python
+    int or a broadcastable int64 tensor).  Returns int64 values in [0, 65535].  int64 arithmetic
+    wraps like uint64; logical right shifts are arithmetic shifts with the sign bits masked off."""
+    h = flat_index + offset
+    h = h ^ ((h >> 33) & 0x7FFFFFFF)
+    h = h * (0xFF51AFD7ED558CCD - (1 << 64))
+    h = h ^ ((h >> 29) & ((1 << 35) - 1))
+    return h & 0xFFFF
+
+
+def weight_tag_salt(cfg: Config, layer: int, kind: str) -> int:
+    return cfg.seed * 1000 + layer * 3 + {"gate": 0, "up": 1, "down": 2}[kind]
+
+
+def kv_tag_salt(cfg: Config, layer: int, kv: int, req: int) -> int:
+    return cfg.seed * 7919 + (layer * 2 + kv) * 100003 + req
 
 
 def gen_logical_weight(cfg: Config, layer: int, kind: str, fill: str = "normal") -> np.ndarray:
@@ -41,7 +71,7 @@ def gen_logical_weight(cfg: Config, layer: int, kind: str, fill: str = "normal")
     shape = (cfg.E, cfg.H, cfg.I) if m < 2 else (cfg.E, cfg.I, cfg.H)
     seed = (cfg.seed, 2000 + layer, m)
     if fill == "tag":
-        t = tag_fill_u16(shape, salt=cfg.seed * 1000 + layer * 3 + m)
+        t = tag_fill_u16(shape, salt=weight_tag_salt(cfg, layer, kind))
         if cfg.w_dtype == "bf16":
             return t
         if cfg.w_dtype == "fp8_e4m3_b128":
@@ -86,7 +116,7 @@ def gen_kv_request(cfg: Config, layer: int, kv: int, req: int, length: int,
     """K (kv=0) or V (kv=1) of one request in one layer: [len, kv_heads, head_dim] bf16 bits."""
     shape = (int(length), cfg.kv_heads, cfg.head_dim)
     if fill == "tag":
-        return tag_fill_u16(shape, salt=cfg.seed * 7919 + (layer * 2 + kv) * 100003 + req)
+        return tag_fill_u16(shape, salt=kv_tag_salt(cfg, layer, kv, req))
     rng = np.random.default_rng((cfg.seed, 3000 + layer, kv, req))
     return bf16_bits_from_f32(rng.normal(0.0, 1.0, size=shape).astype(np.float32))
 
