@@ -293,7 +293,10 @@ def run_moebius(args):
         for to in (EP, TP):
             plan, owner, bt, _ = switch(to, owner, bt, mode)
             if w == 0:
-                first_ms["tp2ep" if to == EP else "ep2tp"] = mb.moebius_last_kernel_ms(sess.ctx)
+                fs = mb.moebius_plan_stats(plan).as_dict()
+                first_ms["tp2ep" if to == EP else "ep2tp"] = {
+                    "kernel_ms": mb.moebius_last_kernel_ms(sess.ctx), "kv_rounds": fs["n_kv_rounds"],
+                    "kv_staged": fs["n_kv_staged"], "pool_groups": fs["n_pool_groups"], "segments": fs["n_segments"]}
             sess.free_plan(plan)
             mode = to
     torch.cuda.synchronize()
@@ -324,6 +327,27 @@ def run_moebius(args):
         torch.cuda.cudart().cudaProfilerStop()
     hist = mb.moebius_kernel_ms_history(sess.ctx, 64)[-2 * args.steps:]
     k_t2e, k_e2t = hist[0::2], hist[1::2]
+    # context: a plain device-to-device copy of a weight slot on this box, now (read + write bytes)
+    d2d = None
+    if cfg.R > 1:
+        n_copy = int(min(lay.weight_slot_bytes * (3 * cfg.L), 8 << 30)) // 256 * 256
+        a0 = sess.view_desc(TP, 0, 0, mb.T_GATE).offset
+        a1 = sess.view_desc(TP, cfg.R - 1, 0, mb.T_GATE).offset
+        src, dst = sess.base[a0:a0 + n_copy], sess.base[a1:a1 + n_copy]
+        keep = dst.clone()
+        best = None
+        for _ in range(5):
+            c0, c1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            c0.record(stream)
+            dst.copy_(src)
+            c1.record(stream)
+            torch.cuda.synchronize()
+            ms = c0.elapsed_time(c1)
+            best = ms if best is None else min(best, ms)
+        dst.copy_(keep)
+        del keep
+        torch.cuda.synchronize()
+        d2d = {"bytes": n_copy, "ms_best_of_5": best, "GBps_read_plus_write": 2 * n_copy / best / 1e6}
 
     # e2e: host inputs -> plan -> reshard (uploads) -> device->host read-back of the published tables
     host_tables = torch.empty(lay.table_bytes // 4, dtype=torch.int32, pin_memory=True)
@@ -418,7 +442,8 @@ def main():
                    "step": "one TP->EP + one EP->TP switch", "l2": "working set >> L2 (126 MB); no flush needed",
                    "parallelism": "replicas only" if world > 1 else "1 GPU, R logical ranks as regions"},
         "tp2ep": d_t2e, "ep2tp": d_e2t,
-        "first_switch_from_random_tables_kernel_ms": r["first_ms"],
+        "first_switch_from_random_tables": r["first_ms"],
+        "d2d_copy_same_box": r["d2d"],
         "plan_ms": {"tp2ep": r["plan_ms_t2e"], "ep2tp": r["plan_ms_e2t"], "e2e_avg": avg(r["plan_ms"])},
         "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
                      "traffic": committed_traffic(cfg.name), "peak_source": peak_src,
