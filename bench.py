@@ -50,6 +50,7 @@ def parse():
                     help="cap on spare slot + staging as a fraction of resident bytes (0 = library default)")
     ap.add_argument("--n-req", type=int, default=-1, help="override the number of live requests (experiments; named in config.workload)")
     ap.add_argument("--tma", default="", help="enable,pipes,stage_kb (tuning; default: library defaults)")
+    ap.add_argument("--kv-rounds", type=int, default=0, help="max dependent KV rounds before chains are cut by staging (tuning)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--profile-region", action="store_true",
                     help="cudaProfilerStart/Stop round warm-up + timed steps (ncu --profile-from-start off skips the fill)")
@@ -266,6 +267,8 @@ def run_moebius(args):
     if args.tma:
         a, b, u = (int(x) for x in args.tma.split(","))
         mb.moebius_set_tma(sess.ctx, a, b, u)
+    if args.kv_rounds:
+        mb.moebius_set_kv_rounds(sess.ctx, args.kv_rounds)
     fill_device(sess, cfg, mb, torch)
     TP, EP = mb.MOEBIUS_TP, mb.MOEBIUS_EP
     n = len(lens)

@@ -199,6 +199,14 @@ MOEBIUS_API int moebius_kernel_ms_history(moebius_ctx_t* ctx, float* out_ms, int
  * before the call cannot be executed after it (MOEBIUS_E_STATE).  2*pipes*stage_kb <= 208. */
 MOEBIUS_API int moebius_set_tma(moebius_ctx_t* ctx, int enable, int pipes, int stage_kb);
 
+/* KV schedule (tuning; before moebius_plan).  When target pages overlap live source pages the page
+ * moves form dependency chains; the planner runs them in at most `max_level` + 2 device-wide rounds
+ * and cuts longer chains by staging the page at the cut (bounded staging buffer; if the cut pages
+ * of one pool do not fit it, longer chains are allowed).  0 restores the default (64: a round costs
+ * ~10 us on B200, a staged page an extra copy of it in all 2L pools); at most 1024.  Results are
+ * identical for every value. */
+MOEBIUS_API int moebius_set_kv_rounds(moebius_ctx_t* ctx, int max_level);
+
 /* Launch shape override for the ld/st path (tuning): values <= 0 restore the defaults; threads is a
  * multiple of 32, at most 256. */
 MOEBIUS_API int moebius_set_launch(moebius_ctx_t* ctx, int ctas_per_sm, int threads, int unit_kb);

@@ -17,7 +17,7 @@ EXPORTED_SYMBOLS = [
     "moebius_create", "moebius_destroy", "moebius_layout", "moebius_view", "moebius_bind",
     "moebius_active_mode", "moebius_plan", "moebius_plan_destroy", "moebius_block_tables",
     "moebius_plan_stats", "moebius_plan_export", "moebius_reshard", "moebius_set_timing",
-    "moebius_last_kernel_ms", "moebius_kernel_ms_history", "moebius_set_launch", "moebius_set_tma", "moebius_status_str", "moebius_version",
+    "moebius_last_kernel_ms", "moebius_kernel_ms_history", "moebius_set_launch", "moebius_set_tma", "moebius_set_kv_rounds", "moebius_status_str", "moebius_version",
 ]
 
 
@@ -108,6 +108,7 @@ _lib.moebius_last_kernel_ms.argtypes = [_vp, C.POINTER(C.c_float)]
 _lib.moebius_kernel_ms_history.argtypes = [_vp, C.POINTER(C.c_float), C.c_int, C.POINTER(C.c_int)]
 _lib.moebius_set_launch.argtypes = [_vp, C.c_int, C.c_int, C.c_int]
 _lib.moebius_set_tma.argtypes = [_vp, C.c_int, C.c_int, C.c_int]
+_lib.moebius_set_kv_rounds.argtypes = [_vp, C.c_int]
 _lib.moebius_status_str.argtypes = [C.c_int]
 _lib.moebius_status_str.restype = C.c_char_p
 _lib.moebius_version.restype = C.c_int
@@ -239,3 +240,7 @@ def moebius_set_launch(ctx, ctas_per_sm: int = 0, threads: int = 0, unit_kb: int
 
 def moebius_set_tma(ctx, enable: bool = True, pipes: int = 0, stage_kb: int = 0):
     _chk(_lib.moebius_set_tma(ctx, int(enable), pipes, stage_kb), "moebius_set_tma")
+
+
+def moebius_set_kv_rounds(ctx, max_level: int = 0):
+    _chk(_lib.moebius_set_kv_rounds(ctx, max_level), "moebius_set_kv_rounds")

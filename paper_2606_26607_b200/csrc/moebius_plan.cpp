@@ -31,7 +31,7 @@ struct Move {
   uint8_t staged;
 };
 
-constexpr int kMaxLevel = 24;
+constexpr int kMaxLevelCap = 1024;   // hard bound on dependency rounds (counters: kMaxCounters)
 
 }  // namespace
 
@@ -151,6 +151,7 @@ int moebius_create(const moebius_config_t* c, moebius_ctx_t** out) {
   x->ctas_per_sm = 0;
   x->threads = 0;
   x->unit_kb = 0;
+  x->kv_max_level = 64;
   x->use_tma = 1;
   x->n_pipes = 2;
   x->stage_bytes = 48 * 1024;
@@ -257,6 +258,12 @@ int moebius_set_tma(moebius_ctx_t* x, int enable, int pipes, int stage_kb) {
   x->stage_bytes = sb;
   x->tmaps_valid = false;
   tma_geometry(x);
+  return MOEBIUS_OK;
+}
+
+int moebius_set_kv_rounds(moebius_ctx_t* x, int max_level) {
+  if (!x || max_level < 0 || max_level > kMaxLevelCap) return MOEBIUS_E_INVAL;
+  x->kv_max_level = max_level > 0 ? max_level : 64;
   return MOEBIUS_OK;
 }
 
@@ -440,21 +447,32 @@ extern "C" int moebius_plan(moebius_ctx_t* x, moebius_mode_t from, moebius_mode_
       bl.erase(std::unique(bl.begin(), bl.end()), bl.end());
       for (int32_t b : bl) dependents[b].push_back(m);
     }
-    // Level the DAG of direct moves; a staged move is read in round 0 and written in the last round.
-    for (int pass = 0; pass < 8; ++pass) {
+    // Level the DAG of direct moves (Kahn order); a staged move is read in round 0 and written in the
+    // last round.  Cycles are broken by staging one move on the cycle.  Chains longer than
+    // kv_max_level rounds are CUT rather than staged whole: a move whose level would exceed the
+    // limit is staged, so its source is saved in round 0 and everything behind it restarts at
+    // level 1.  A round costs a device-wide drain, a staged page one extra copy: short schedules
+    // with a few percent of staged pages are the cheapest.
+    std::vector<uint8_t> self_staged(nm);
+    for (int m = 0; m < nm; ++m) self_staged[m] = mv[m].staged;
+    // If the staged pages of one pool do not fit the staging buffer, allow longer chains (fewer cuts).
+    for (int max_level = x->kv_max_level;; max_level = std::min(kMaxLevelCap, max_level * 4)) {
+      for (int m = 0; m < nm; ++m) mv[m].staged = self_staged[m];
       std::vector<int32_t> indeg(nm, 0), queue;
       std::vector<uint8_t> done(nm, 0);
+      queue.reserve(nm);
+      int n_direct = 0;
       for (int m = 0; m < nm; ++m) {
         mv[m].level = 0;
         if (mv[m].staged) { done[m] = 1; continue; }
+        ++n_direct;
         for (int32_t b : blockers[m]) {
           if (mv[b].staged) mv[m].level = 1; else indeg[m]++;
         }
       }
       for (int m = 0; m < nm; ++m) if (!done[m] && indeg[m] == 0) queue.push_back(m);
       size_t qh = 0;
-      int scan = 0, resolved = 0, n_direct = 0;
-      for (int m = 0; m < nm; ++m) n_direct += !mv[m].staged;
+      int scan = 0, resolved = 0;
       std::vector<int32_t> stamp(nm, -1);
       int32_t walk_id = 0;
       auto release = [&](int m, int lvl) {
@@ -467,8 +485,14 @@ extern "C" int moebius_plan(moebius_ctx_t* x, moebius_mode_t from, moebius_mode_
       while (resolved < n_direct) {
         if (qh < queue.size()) {
           int m = queue[qh++];
-          done[m] = 1; ++resolved;
-          release(m, mv[m].level + 1);
+          done[m] = 1;
+          if (mv[m].level > max_level) {        // cut the chain here
+            mv[m].staged = 1; --n_direct;
+            release(m, 1);
+          } else {
+            ++resolved;
+            release(m, mv[m].level + 1);
+          }
           continue;
         }
         // only cycles (and what sits behind them) are left: walk blockers to find a node ON a cycle
@@ -485,13 +509,11 @@ extern "C" int moebius_plan(moebius_ctx_t* x, moebius_mode_t from, moebius_mode_
         mv[v].staged = 1; done[v] = 1; --n_direct;
         release(v, 1);
       }
-      int maxlvl = 0;
-      for (int m = 0; m < nm; ++m) if (!mv[m].staged) maxlvl = std::max(maxlvl, mv[m].level);
-      if (maxlvl <= kMaxLevel) { K = maxlvl; break; }
-      for (int m = 0; m < nm; ++m) if (!mv[m].staged && mv[m].level > kMaxLevel) mv[m].staged = 1;
-      K = kMaxLevel;
+      K = 0;
+      int64_t ns = 0;
+      for (int m = 0; m < nm; ++m) { if (!mv[m].staged) K = std::max(K, (int)mv[m].level); else ++ns; }
+      if (ns * x->ep_page_bytes <= x->staging_bytes || max_level >= kMaxLevelCap) break;
     }
-    for (int m = 0; m < nm; ++m) if (!mv[m].staged && mv[m].level > K) mv[m].staged = 1;  // pass limit hit
     for (int m = 0; m < nm; ++m) if (mv[m].staged) mv[m].slot = n_staged++;
   }
   int pools_per_group = n_pools_all;

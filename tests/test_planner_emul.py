@@ -124,8 +124,9 @@ def test_tight_pool_rounds_and_staging(first):
 
 def test_staging_reused_across_pool_groups_and_too_small():
     """When the staged pages of all 2L pools do not fit the staging buffer, the pools are processed
-    in groups that reuse it; when not even one pool fits, the plan fails with E_STAGING and the
-    caller cancels the switch (like a capacity failure)."""
+    in groups that reuse it; when not even one pool fits, chains are cut less often; when the
+    cycle-breaking pages alone do not fit, the plan fails with E_STAGING and the caller cancels
+    the switch (like a capacity failure)."""
     cfg = SMALLISH.with_(L=2, n_req=40, seed=99)
     lens = wl.draw_seq_lens(cfg)
     st, sess, image, staging = make(cfg, lens, "tight", cap_frac=0.5)
@@ -145,11 +146,21 @@ def test_staging_reused_across_pool_groups_and_too_small():
     mode, o2, bt2, stats = run_switch(st, sess2, image, staging, TP, owner, bt)
     assert stats["n_pool_groups"] == 4 and stats["staging_used_bytes"] <= sess2.layout.staging_bytes
     run_switch(st, sess2, image, staging, EP, o2, bt2)
-    # not even one pool fits
+    # not even one pool's cut pages fit: the planner allows longer chains (fewer cuts, more rounds)
     c.staging_cap_bytes = spare + per_pool - sess.layout.ep_page_bytes
     sess3 = mb.Session(c)
+    image = np.full(sess3.layout.base_bytes, 0xA5, np.uint8)
+    staging = np.full(sess3.layout.staging_bytes, 0x5A, np.uint8)
+    OracleLayout(st, sess3, TP, owner, bt).place(image)
+    _, _, _, stats3 = run_switch(st, sess3, image, staging, TP, owner, bt)
+    assert stats3["n_kv_staged"] < s["n_kv_staged"] and stats3["n_kv_rounds"] >= s["n_kv_rounds"]
+    assert stats3["staging_used_bytes"] <= sess3.layout.staging_bytes
+    # no staging at all, but cycles need it: E_STAGING, the caller cancels the switch
+    c.staging_cap_bytes = spare
+    sess4 = mb.Session(c)
+    assert sess4.layout.staging_bytes == 0
     with pytest.raises(mb.MoebiusError) as e:
-        sess3.plan(EP, st.lens, owner, bt, from_mode=TP)
+        sess4.plan(EP, st.lens, owner, bt, from_mode=TP)
     assert e.value.status == -3
     # cap below the spare weight slot itself
     c.staging_cap_bytes = spare - 1
@@ -202,3 +213,22 @@ def test_fp8_scales():
     OracleLayout(st, sess, TP, owner, bt).place(image)
     mode, owner, bt, s = run_switch(st, sess, image, staging, TP, owner, bt)
     mode, owner, bt, s = run_switch(st, sess, image, staging, EP, owner, bt)
+
+
+@pytest.mark.parametrize("max_level", [1, 2, 6, 1024])
+@pytest.mark.parametrize("first", [TP, EP])
+def test_chain_cut_levels(first, max_level):
+    """Dependency chains are cut by staging after `max_level` rounds (moebius_set_kv_rounds): the
+    result and the hazard ordering are the same for every setting; only rounds vs staged pages trade."""
+    cfg = SMALLISH.with_(L=1, n_req=40, seed=99)
+    lens = wl.draw_seq_lens(cfg)
+    st, sess, image, staging = make(cfg, lens, "tight", cap_frac=0.5)
+    mb.moebius_set_kv_rounds(sess.ctx, max_level)
+    owner, bt = source_tables(st, sess, first, "random", seed=2)
+    OracleLayout(st, sess, first, owner, bt).place(image)
+    mode, owner, bt, stats = run_switch(st, sess, image, staging, first, owner, bt)
+    assert stats["n_kv_rounds"] <= max_level + 2
+    if max_level == 1024:
+        assert stats["n_kv_rounds"] > 8          # the uncut chains are long here
+    run_switch(st, sess, image, staging, mode, owner, bt)
+    sess.close()
