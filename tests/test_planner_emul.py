@@ -130,6 +130,7 @@ def test_staging_reused_across_pool_groups_and_too_small():
     cfg = SMALLISH.with_(L=2, n_req=40, seed=99)
     lens = wl.draw_seq_lens(cfg)
     st, sess, image, staging = make(cfg, lens, "tight", cap_frac=0.5)
+    mb.moebius_set_kv_rounds(sess.ctx, 2)       # short schedules: chains are cut often, many staged pages
     owner, bt = source_tables(st, sess, TP, "random", seed=1)
     plan = sess.plan(EP, st.lens, owner, bt, from_mode=TP)
     s = mb.moebius_plan_stats(plan).as_dict()
@@ -140,6 +141,7 @@ def test_staging_reused_across_pool_groups_and_too_small():
     c = mb_config(cfg, lens, "tight")
     c.staging_cap_bytes = spare + per_pool + sess.layout.ep_page_bytes
     sess2 = mb.Session(c)
+    mb.moebius_set_kv_rounds(sess2.ctx, 2)
     image = np.full(sess2.layout.base_bytes, 0xA5, np.uint8)
     staging = np.full(sess2.layout.staging_bytes, 0x5A, np.uint8)
     OracleLayout(st, sess2, TP, owner, bt).place(image)
@@ -149,6 +151,7 @@ def test_staging_reused_across_pool_groups_and_too_small():
     # not even one pool's cut pages fit: the planner allows longer chains (fewer cuts, more rounds)
     c.staging_cap_bytes = spare + per_pool - sess.layout.ep_page_bytes
     sess3 = mb.Session(c)
+    mb.moebius_set_kv_rounds(sess3.ctx, 2)
     image = np.full(sess3.layout.base_bytes, 0xA5, np.uint8)
     staging = np.full(sess3.layout.staging_bytes, 0x5A, np.uint8)
     OracleLayout(st, sess3, TP, owner, bt).place(image)
