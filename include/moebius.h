@@ -123,6 +123,8 @@ typedef struct {
 /* Validates the config and builds the region map ("one large contiguous unified
  * buffer", views at fixed regions).  cfg: HOST.  out: HOST, receives a new context. */
 MOEBIUS_API int moebius_create(const moebius_config_t* cfg, moebius_ctx_t** out);
+/* Destroy every plan of a context before the context itself (a destroyed plan hands its pinned
+ * upload image back to its context for the next moebius_plan to reuse). */
 MOEBIUS_API void moebius_destroy(moebius_ctx_t* ctx);
 
 /* Sizes of the four caller-owned device buffers.  out: HOST. */

@@ -422,22 +422,51 @@ moebius_reshard_kernel(const __grid_constant__ DevParams p, const __grid_constan
   drain();
 }
 
-void* host_alloc(int64_t bytes, bool* pinned) {
-  void* p = nullptr;
-  *pinned = false;
-  int ndev = 0;
-  if (cudaGetDeviceCount(&ndev) == cudaSuccess && ndev > 0 &&
-      cudaHostAlloc(&p, (size_t)bytes, cudaHostAllocDefault) == cudaSuccess) {
-    *pinned = true;
-    return p;
+// Upload images.  A plan's image is read by the async H2D copies of moebius_reshard, so a buffer that
+// goes back to the pool keeps the event recorded after its last upload; the next plan that takes the
+// buffer waits on that event before overwriting it.
+bool image_acquire(moebius_ctx* x, int64_t bytes, ImageBuf* out) {
+  size_t best = x->image_pool.size();
+  for (size_t i = 0; i < x->image_pool.size(); ++i)
+    if (x->image_pool[i].bytes >= bytes && (best == x->image_pool.size() || x->image_pool[i].bytes < x->image_pool[best].bytes))
+      best = i;
+  if (best < x->image_pool.size()) {
+    *out = x->image_pool[best];
+    x->image_pool.erase(x->image_pool.begin() + (long)best);
+    if (out->ev && cudaEventSynchronize((cudaEvent_t)out->ev) != cudaSuccess) cudaGetLastError();
+    return true;
   }
-  cudaGetLastError();
-  return malloc((size_t)bytes);
+  if (x->has_device < 0) {
+    int ndev = 0;
+    x->has_device = (cudaGetDeviceCount(&ndev) == cudaSuccess && ndev > 0) ? 1 : 0;
+    cudaGetLastError();
+  }
+  // round up so that plans of slightly different sizes share buffers
+  int64_t cap = (bytes + (1 << 20) - 1) >> 20 << 20;
+  out->p = nullptr; out->bytes = cap; out->pinned = false; out->ev = nullptr;
+  if (x->has_device) {
+    void* p = nullptr;
+    if (cudaHostAlloc(&p, (size_t)cap, cudaHostAllocDefault) == cudaSuccess) {
+      out->p = (char*)p; out->pinned = true;
+      cudaEvent_t e;
+      if (cudaEventCreateWithFlags(&e, cudaEventDisableTiming) == cudaSuccess) out->ev = e; else cudaGetLastError();
+      return true;
+    }
+    cudaGetLastError();
+  }
+  out->p = (char*)malloc((size_t)cap);
+  return out->p != nullptr;
 }
 
-void host_free(void* p, bool pinned) {
-  if (!p) return;
-  if (pinned) cudaFreeHost(p); else free(p);
+void image_free(const ImageBuf& b) {
+  if (!b.p) return;
+  if (b.ev) { cudaEventSynchronize((cudaEvent_t)b.ev); cudaEventDestroy((cudaEvent_t)b.ev); }
+  if (b.pinned) cudaFreeHost(b.p); else free(b.p);
+}
+
+void image_release(moebius_ctx* x, const ImageBuf& b) {
+  if (!b.p) return;
+  if (x->image_pool.size() < 4) x->image_pool.push_back(b); else image_free(b);
 }
 
 typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
@@ -490,6 +519,8 @@ static int encode_tmaps(moebius_ctx* x) {
 }
 
 void cuda_ctx_destroy(moebius_ctx* x) {
+  for (const ImageBuf& b : x->image_pool) image_free(b);
+  x->image_pool.clear();
   if (x->ev_valid) {
     for (int i = 0; i < 2 * kTimingRing; ++i) cudaEventDestroy((cudaEvent_t)x->ev[i]);
     x->ev_valid = false;
@@ -627,6 +658,7 @@ extern "C" int moebius_reshard(moebius_ctx_t* x, const moebius_plan_t* P, void* 
   // 3. publish: new tables, owner vector and the active-mode flag at their fixed address
   if (cudaMemcpyAsync(x->tables, P->tbl_image, (size_t)P->tbl_bytes, cudaMemcpyHostToDevice, st) != cudaSuccess)
     return MOEBIUS_E_CUDA;
+  if (P->buf.ev && cudaEventRecord((cudaEvent_t)P->buf.ev, st) != cudaSuccess) return MOEBIUS_E_CUDA;
   x->active_mode = P->to;
   x->switch_count++;
   return MOEBIUS_OK;

@@ -18,6 +18,31 @@ constexpr int64_t kSegOff = kCtrOff + 4 * kMaxCounters;    // Seg[...]
 constexpr int kTblHdrInts = 16;
 constexpr int kTimingRing = 64;
 
+struct ImageBuf {            // host upload image of a plan; pinned when a CUDA device is present
+  char* p;
+  int64_t bytes;
+  bool pinned;
+  void* ev;                  // cudaEvent_t recorded after the last upload that reads this buffer (or null)
+};
+
+struct Move {                // one live (request, block) page under both modes
+  int32_t req, blk, ep_rank, ep_page, tp_page, ntok;
+  int32_t level;
+  int32_t slot;
+  uint8_t staged;
+};
+
+// Planner workspace, kept by the context so that a steady stream of switches re-uses warm memory
+// (a fresh multi-megabyte vector per plan costs more in page faults than the planning itself).
+struct PlanScratch {
+  std::vector<int32_t> npages, order, owner, bt, reader, indeg, queue, stamp;
+  std::vector<int32_t> blk_off, blk, dep_off, dep, dep_cur;   // CSR: blockers of m, dependents of b
+  std::vector<int64_t> tok, cnt, used;
+  std::vector<uint8_t> seen, done, self_staged;
+  std::vector<uint32_t> lvl_begin, cur;
+  std::vector<Move> mv;
+};
+
 struct ScaleGeom {           // fp8 block scales of one matrix kind (reading A13)
   int64_t tp_bytes;          // per rank, allocated with the largest nb over ranks
   int64_t ep_bytes;          // per rank
@@ -65,15 +90,22 @@ struct moebius_ctx {
   void* ev[2 * moebius::kTimingRing];   // event pairs (begin, end) round the kernel, a ring
   int64_t ev_count;                     // pairs recorded so far
   bool ev_valid;
+  // upload images released by destroyed plans, reused by the next moebius_plan (pinning a fresh
+  // buffer costs milliseconds; a switch must not pay it every time)
+  std::vector<moebius::ImageBuf> image_pool;
+  moebius::PlanScratch scratch;
+  int has_device;                       // -1 unknown, 0 no CUDA device (host-only planner), 1 yes
 };
 
 struct moebius_plan {
-  const moebius_ctx* ctx;
+  moebius_ctx* ctx;
   int from, to, n_req;
   std::vector<moebius::Seg> segs;
-  std::vector<moebius::KvDesc> kv;
   std::vector<moebius::C2dDesc> c2d;
-  std::vector<int32_t> lens, owner, bt;   // target-mode request state
+  const moebius::KvDesc* kv;      // n_kv descriptors, inside `image`
+  int64_t n_kv;
+  std::vector<int32_t> lens, owner;   // target-mode request state
+  const int32_t* bt;              // [n_req][max_pages_per_request], inside `tbl_image`
   moebius_stats_t stats;
   uint32_t n_counters, total_units;
   bool uses_tma;                  // some segment is PATH_TMA: needs the pipes' shared-memory rings
@@ -83,13 +115,14 @@ struct moebius_plan {
   int64_t image_bytes, kv_img_off, c2d_img_off;
   int32_t* tbl_image;
   int64_t tbl_bytes;
-  bool pinned;
+  moebius::ImageBuf buf;          // backing storage of image + tbl_image
 };
 
 namespace moebius {
 // CUDA side (moebius_cuda.cu)
-void* host_alloc(int64_t bytes, bool* pinned);
-void host_free(void* p, bool pinned);
+bool image_acquire(moebius_ctx* ctx, int64_t bytes, ImageBuf* out);   // from the pool, else fresh
+void image_release(moebius_ctx* ctx, const ImageBuf& buf);             // back to the pool (bounded)
+void image_free(const ImageBuf& buf);
 void cuda_ctx_destroy(moebius_ctx* ctx);
 void tma_geometry(moebius_ctx* ctx);   // derives xt_ok/kt_ok/xt_rows/kt_pools from cfg + stage_bytes (host only)
 }  // namespace moebius

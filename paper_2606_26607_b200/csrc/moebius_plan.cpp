@@ -24,13 +24,6 @@ void scale_blocks(int r, int R, int I, int* lo, int* hi) {
   *hi = ((r + 1) * w - 1) / 128 + 1;
 }
 
-struct Move {
-  int32_t req, blk, ep_rank, ep_page, tp_page, ntok;
-  int32_t level;
-  int32_t slot;
-  uint8_t staged;
-};
-
 constexpr int kMaxLevelCap = 1024;   // hard bound on dependency rounds (counters: kMaxCounters)
 
 }  // namespace
@@ -163,6 +156,7 @@ int moebius_create(const moebius_config_t* c, moebius_ctx_t** out) {
   memset(x->ev, 0, sizeof(x->ev));
   x->ev_count = 0;
   x->ev_valid = false;
+  x->has_device = -1;
   *out = x;
   return MOEBIUS_OK;
 }
@@ -278,7 +272,7 @@ int moebius_set_launch(moebius_ctx_t* x, int ctas_per_sm, int threads, int unit_
 
 void moebius_plan_destroy(moebius_plan_t* p) {
   if (!p) return;
-  if (p->image) host_free(p->image, p->pinned);
+  image_release(p->ctx, p->buf);
   delete p;
 }
 
@@ -338,7 +332,9 @@ extern "C" int moebius_plan(moebius_ctx_t* x, moebius_mode_t from, moebius_mode_
   const int64_t unit_bytes = (int64_t)(x->unit_kb > 0 ? x->unit_kb : 32) * 1024;
 
   // ---- request state under the target mode ----------------------------------------------------
-  std::vector<int32_t> npages(n_req);
+  PlanScratch& W = x->scratch;   // warm workspace: no fresh multi-megabyte allocation per switch
+  std::vector<int32_t>& npages = W.npages;
+  npages.assign(n_req, 0);
   int64_t total_pages = 0;
   for (int i = 0; i < n_req; ++i) {
     if (seq_lens[i] < 0) return MOEBIUS_E_INVAL;
@@ -347,14 +343,17 @@ extern "C" int moebius_plan(moebius_ctx_t* x, moebius_mode_t from, moebius_mode_
     total_pages += npages[i];
     if (e2t && (src_owner[i] < 0 || src_owner[i] >= R)) return MOEBIUS_E_INVAL;
   }
-  std::vector<int32_t> owner(n_req, -1);
+  std::vector<int32_t>& owner = W.owner;
+  owner.assign(n_req, -1);
   if (!e2t) {
     // decreasing length, greedy least-loaded rank, deterministic.  Reading A9: ties by
     // request id; least loaded = smallest (tokens, requests, rank).
-    std::vector<int32_t> order(n_req);
+    std::vector<int32_t>& order = W.order;
+    order.resize(n_req);
     std::iota(order.begin(), order.end(), 0);
     std::stable_sort(order.begin(), order.end(), [&](int a, int b) { return seq_lens[a] > seq_lens[b]; });
-    std::vector<int64_t> tok(R, 0), cnt(R, 0);
+    W.tok.assign(R, 0); W.cnt.assign(R, 0);
+    std::vector<int64_t>&tok = W.tok, &cnt = W.cnt;
     for (int i : order) {
       int best = 0;
       for (int r = 1; r < R; ++r)
@@ -364,15 +363,19 @@ extern "C" int moebius_plan(moebius_ctx_t* x, moebius_mode_t from, moebius_mode_
       cnt[best] += 1;
     }
   }
-  // reading A7: ascending request id, consecutive pages; TP bumps up from 0, EP down from the top
-  std::vector<int32_t> bt((size_t)n_req * MP, -1);
+  // reading A7: ascending request id, consecutive pages; TP bumps up from 0, EP down from the top.
+  // Only the first npages[i] entries of a row are written here; the -1 padding is laid down when
+  // the table image is built.
+  std::vector<int32_t>& bt = W.bt;
+  if (bt.size() < (size_t)n_req * MP) bt.resize((size_t)n_req * MP);
   if (e2t) {
     if (total_pages > x->pages_tp) return MOEBIUS_E_CAPACITY;
     int32_t nxt = 0;
     for (int i = 0; i < n_req; ++i)
       for (int b = 0; b < npages[i]; ++b) bt[(size_t)i * MP + b] = nxt++;
   } else {
-    std::vector<int64_t> used(R, 0);
+    W.used.assign(R, 0);
+    std::vector<int64_t>& used = W.used;
     for (int i = 0; i < n_req; ++i) {
       int r = owner[i];
       if (used[r] + npages[i] > x->pages_ep) return MOEBIUS_E_CAPACITY;
@@ -383,7 +386,8 @@ extern "C" int moebius_plan(moebius_ctx_t* x, moebius_mode_t from, moebius_mode_
 
   // ---- KV page moves (one per live (request, block); layer- and K/V-agnostic) ----
   const int kappa = x->G;  // TP-page granules per EP page
-  std::vector<Move> mv;
+  std::vector<Move>& mv = W.mv;
+  mv.clear();
   mv.reserve((size_t)total_pages);
   for (int i = 0; i < n_req; ++i) {
     for (int b = 0; b < npages[i]; ++b) {
@@ -402,19 +406,36 @@ extern "C" int moebius_plan(moebius_ctx_t* x, moebius_mode_t from, moebius_mode_
   }
   const int nm = (int)mv.size();
   {  // source pages must be unique (per owner under EP, globally under TP)
-    std::vector<uint8_t> seen((size_t)(e2t ? R : 1) * (e2t ? x->pages_ep : x->pages_tp), 0);
+    std::vector<uint8_t>& seen = W.seen;
+    seen.assign((size_t)(e2t ? R : 1) * (e2t ? x->pages_ep : x->pages_tp), 0);
     for (const Move& m : mv) {
       size_t id = e2t ? (size_t)m.ep_rank * x->pages_ep + m.ep_page : (size_t)m.tp_page;
       if (seen[id]) return MOEBIUS_E_INVAL;
       seen[id] = 1;
     }
   }
-  // reader[rank*pages_tp + granule] = move that reads it (TP-page-sized granules of a pool)
-  std::vector<int32_t> reader;
-  std::vector<std::vector<int32_t>> dependents;  // edge b -> m: m writes what b reads
-  std::vector<std::vector<int32_t>> blockers;
+  // reader[rank*pages_tp + granule] = move that reads it (TP-page-sized granules of a pool).
+  // Hazard graph in CSR form: blk[blk_off[m] .. blk_off[m+1]) = moves that READ what m overwrites
+  // (m must run after them); dep[...] is the transpose (who waits for b).
   int n_staged = 0, K = 0;
+  // Fast path: with the two-ended allocation (reading A7) the targets are TP pages [0, total_pages)
+  // on every rank resp. the top used[r] EP pages of rank r.  If every source page lies outside those
+  // ranges nothing overwrites a live source: one round, no graph needed.
+  bool disjoint = nm > 0;
   if (nm > 0) {
+    if (e2t) {
+      int64_t min_src = INT64_MAX;
+      for (const Move& m : mv) min_src = std::min<int64_t>(min_src, (int64_t)m.ep_page * kappa);
+      disjoint = min_src >= total_pages;
+    } else {
+      int64_t max_src = -1, min_dst = INT64_MAX;
+      for (const Move& m : mv) max_src = std::max<int64_t>(max_src, m.tp_page);
+      for (int r = 0; r < R; ++r) min_dst = std::min<int64_t>(min_dst, ((int64_t)x->pages_ep - W.used[r]) * kappa);
+      disjoint = max_src < min_dst;
+    }
+  }
+  if (nm > 0 && !disjoint) {
+    std::vector<int32_t>& reader = W.reader;
     reader.assign((size_t)R * x->pages_tp, -1);
     auto gid = [&](int rank, int64_t gran) { return (size_t)rank * x->pages_tp + (size_t)gran; };
     for (int m = 0; m < nm; ++m) {
@@ -432,20 +453,36 @@ extern "C" int moebius_plan(moebius_ctx_t* x, moebius_mode_t from, moebius_mode_
         }
       }
     }
-    blockers.assign(nm, {});
-    dependents.assign(nm, {});
+    std::vector<int32_t>&blk_off = W.blk_off, &blk = W.blk, &dep_off = W.dep_off, &dep = W.dep;
+    blk_off.assign(nm + 1, 0);
+    blk.clear();
+    dep_off.assign(nm + 1, 0);
     for (int m = 0; m < nm; ++m) {
-      auto& bl = blockers[m];
+      int32_t bl[64];            // R <= 64, kappa <= R
+      int nb = 0;
       auto note = [&](int32_t b) {
         if (b < 0) return;
         if (b == m) { mv[m].staged = 1; return; }  // a move whose target overlaps its own source
-        bl.push_back(b);
+        bl[nb++] = b;
       };
       if (e2t) for (int j = 0; j < R; ++j) note(reader[gid(j, mv[m].tp_page)]);
       else     for (int g = 0; g < kappa; ++g) note(reader[gid(mv[m].ep_rank, (int64_t)mv[m].ep_page * kappa + g)]);
-      std::sort(bl.begin(), bl.end());
-      bl.erase(std::unique(bl.begin(), bl.end()), bl.end());
-      for (int32_t b : bl) dependents[b].push_back(m);
+      if (nb > 1) {
+        std::sort(bl, bl + nb);
+        nb = (int)(std::unique(bl, bl + nb) - bl);
+      }
+      for (int i = 0; i < nb; ++i) { blk.push_back(bl[i]); dep_off[bl[i] + 1]++; }
+      blk_off[m + 1] = (int32_t)blk.size();
+    }
+    const bool any_edge = !blk.empty();
+    bool any_self = false;
+    for (int m = 0; m < nm; ++m) any_self |= mv[m].staged != 0;
+    if (any_edge) {
+      for (int m = 0; m < nm; ++m) dep_off[m + 1] += dep_off[m];
+      dep.resize(blk.size());
+      W.dep_cur.assign(dep_off.begin(), dep_off.end() - 1);
+      for (int m = 0; m < nm; ++m)
+        for (int32_t e = blk_off[m]; e < blk_off[m + 1]; ++e) dep[W.dep_cur[blk[e]]++] = m;
     }
     // Level the DAG of direct moves (Kahn order); a staged move is read in round 0 and written in the
     // last round.  Cycles are broken by staging one move on the cycle.  Chains longer than
@@ -453,66 +490,77 @@ extern "C" int moebius_plan(moebius_ctx_t* x, moebius_mode_t from, moebius_mode_
     // limit is staged, so its source is saved in round 0 and everything behind it restarts at
     // level 1.  A round costs a device-wide drain, a staged page one extra copy: short schedules
     // with a few percent of staged pages are the cheapest.
-    std::vector<uint8_t> self_staged(nm);
-    for (int m = 0; m < nm; ++m) self_staged[m] = mv[m].staged;
-    // If the staged pages of one pool do not fit the staging buffer, allow longer chains (fewer cuts).
-    for (int max_level = x->kv_max_level;; max_level = std::min(kMaxLevelCap, max_level * 4)) {
-      for (int m = 0; m < nm; ++m) mv[m].staged = self_staged[m];
-      std::vector<int32_t> indeg(nm, 0), queue;
-      std::vector<uint8_t> done(nm, 0);
-      queue.reserve(nm);
-      int n_direct = 0;
-      for (int m = 0; m < nm; ++m) {
-        mv[m].level = 0;
-        if (mv[m].staged) { done[m] = 1; continue; }
-        ++n_direct;
-        for (int32_t b : blockers[m]) {
-          if (mv[b].staged) mv[m].level = 1; else indeg[m]++;
-        }
-      }
-      for (int m = 0; m < nm; ++m) if (!done[m] && indeg[m] == 0) queue.push_back(m);
-      size_t qh = 0;
-      int scan = 0, resolved = 0;
-      std::vector<int32_t> stamp(nm, -1);
-      int32_t walk_id = 0;
-      auto release = [&](int m, int lvl) {
-        for (int32_t d : dependents[m]) {
-          if (done[d] || mv[d].staged) continue;
-          mv[d].level = std::max(mv[d].level, lvl);
-          if (--indeg[d] == 0) queue.push_back(d);
-        }
-      };
-      while (resolved < n_direct) {
-        if (qh < queue.size()) {
-          int m = queue[qh++];
-          done[m] = 1;
-          if (mv[m].level > max_level) {        // cut the chain here
-            mv[m].staged = 1; --n_direct;
-            release(m, 1);
-          } else {
-            ++resolved;
-            release(m, mv[m].level + 1);
+    // No edge at all (the common case: two-ended allocation in a roomy pool) => one round, done.
+    if (any_edge) {
+      std::vector<uint8_t>&self_staged = W.self_staged, &done = W.done;
+      std::vector<int32_t>&indeg = W.indeg, &queue = W.queue, &stamp = W.stamp;
+      self_staged.resize(nm);
+      for (int m = 0; m < nm; ++m) self_staged[m] = mv[m].staged;
+      // If the staged pages of one pool do not fit the staging buffer, allow longer chains (fewer cuts).
+      for (int max_level = x->kv_max_level;; max_level = std::min(kMaxLevelCap, max_level * 4)) {
+        for (int m = 0; m < nm; ++m) mv[m].staged = self_staged[m];
+        indeg.assign(nm, 0);
+        done.assign(nm, 0);
+        queue.clear();
+        queue.reserve(nm);
+        int n_direct = 0;
+        for (int m = 0; m < nm; ++m) {
+          mv[m].level = 0;
+          if (mv[m].staged) { done[m] = 1; continue; }
+          ++n_direct;
+          for (int32_t e = blk_off[m]; e < blk_off[m + 1]; ++e) {
+            if (mv[blk[e]].staged) mv[m].level = 1; else indeg[m]++;
           }
-          continue;
         }
-        // only cycles (and what sits behind them) are left: walk blockers to find a node ON a cycle
-        while (scan < nm && done[scan]) ++scan;
-        int v = scan;
-        ++walk_id;
-        for (;;) {
-          if (stamp[v] == walk_id) break;
-          stamp[v] = walk_id;
-          int nxt = -1;
-          for (int32_t b : blockers[v]) if (!done[b] && !mv[b].staged) { nxt = b; break; }
-          v = nxt;  // exists: indeg[v] > 0
+        for (int m = 0; m < nm; ++m) if (!done[m] && indeg[m] == 0) queue.push_back(m);
+        size_t qh = 0;
+        int scan = 0, resolved = 0;
+        stamp.assign(nm, -1);
+        int32_t walk_id = 0;
+        auto release = [&](int m, int lvl) {
+          for (int32_t e = dep_off[m]; e < dep_off[m + 1]; ++e) {
+            const int32_t d = dep[e];
+            if (done[d] || mv[d].staged) continue;
+            mv[d].level = std::max(mv[d].level, lvl);
+            if (--indeg[d] == 0) queue.push_back(d);
+          }
+        };
+        while (resolved < n_direct) {
+          if (qh < queue.size()) {
+            int m = queue[qh++];
+            done[m] = 1;
+            if (mv[m].level > max_level) {        // cut the chain here
+              mv[m].staged = 1; --n_direct;
+              release(m, 1);
+            } else {
+              ++resolved;
+              release(m, mv[m].level + 1);
+            }
+            continue;
+          }
+          // only cycles (and what sits behind them) are left: walk blockers to find a node ON a cycle
+          while (scan < nm && done[scan]) ++scan;
+          int v = scan;
+          ++walk_id;
+          for (;;) {
+            if (stamp[v] == walk_id) break;
+            stamp[v] = walk_id;
+            int nxt = -1;
+            for (int32_t e = blk_off[v]; e < blk_off[v + 1]; ++e)
+              if (!done[blk[e]] && !mv[blk[e]].staged) { nxt = blk[e]; break; }
+            v = nxt;  // exists: indeg[v] > 0
+          }
+          mv[v].staged = 1; done[v] = 1; --n_direct;
+          release(v, 1);
         }
-        mv[v].staged = 1; done[v] = 1; --n_direct;
-        release(v, 1);
+        K = 0;
+        int64_t ns = 0;
+        for (int m = 0; m < nm; ++m) { if (!mv[m].staged) K = std::max(K, (int)mv[m].level); else ++ns; }
+        if (ns * x->ep_page_bytes <= x->staging_bytes || max_level >= kMaxLevelCap) break;
       }
+    } else if (any_self) {
+      // self-overlapping moves only: they are staged; nobody else depends on anything
       K = 0;
-      int64_t ns = 0;
-      for (int m = 0; m < nm; ++m) { if (!mv[m].staged) K = std::max(K, (int)mv[m].level); else ++ns; }
-      if (ns * x->ep_page_bytes <= x->staging_bytes || max_level >= kMaxLevelCap) break;
     }
     for (int m = 0; m < nm; ++m) if (mv[m].staged) mv[m].slot = n_staged++;
   }
@@ -530,7 +578,8 @@ extern "C" int moebius_plan(moebius_ctx_t* x, moebius_mode_t from, moebius_mode_
   moebius_plan_t* P = new (std::nothrow) moebius_plan_t();
   if (!P) return MOEBIUS_E_INVAL;
   P->ctx = x; P->from = from; P->to = to; P->n_req = n_req;
-  P->image = nullptr; P->tbl_image = nullptr; P->pinned = false;
+  P->image = nullptr; P->tbl_image = nullptr; P->kv = nullptr; P->n_kv = 0; P->bt = nullptr;
+  P->buf.p = nullptr; P->buf.bytes = 0; P->buf.pinned = false; P->buf.ev = nullptr;
   memset(&P->stats, 0, sizeof(P->stats));
   P->stats.struct_size = sizeof(moebius_stats_t);
   uint32_t next_ctr = 0;
@@ -648,19 +697,11 @@ extern "C" int moebius_plan(moebius_ctx_t* x, moebius_mode_t from, moebius_mode_
 
   // KV: descriptors ordered [level 0][level 1]...[level K][staged]
   if (nm > 0) {
-    std::vector<uint32_t> lvl_begin(K + 2, 0);
+    std::vector<uint32_t>& lvl_begin = W.lvl_begin;
+    lvl_begin.assign(K + 2, 0);
     for (int m = 0; m < nm; ++m) if (!mv[m].staged) lvl_begin[mv[m].level + 1]++;
     for (int l = 0; l <= K; ++l) lvl_begin[l + 1] += lvl_begin[l];
-    const uint32_t n_direct = lvl_begin[K + 1];
-    P->kv.resize(nm);
-    std::vector<uint32_t> cur(lvl_begin.begin(), lvl_begin.end() - 1);
-    uint32_t scur = n_direct;
-    for (int m = 0; m < nm; ++m) {
-      KvDesc d;
-      d.ep_rank = mv[m].ep_rank; d.ep_page = mv[m].ep_page; d.tp_page = mv[m].tp_page;
-      d.ntok_slot = (uint32_t)mv[m].ntok | (mv[m].staged ? ((uint32_t)mv[m].slot << 8) : 0u);
-      if (mv[m].staged) P->kv[scur++] = d; else P->kv[cur[mv[m].level]++] = d;
-    }
+    const uint32_t n_direct = lvl_begin[K + 1];   // the descriptors themselves are written into the image below
     const uint32_t ppu_lsu = (uint32_t)std::max<int64_t>(1, std::min<int64_t>(unit_bytes / x->ep_page_bytes, 2));
     const bool kv_tma = x->use_tma && x->kt_ok;
     uint32_t ppu = kv_tma ? (uint32_t)x->kt_pools : ppu_lsu;
@@ -762,7 +803,7 @@ extern "C" int moebius_plan(moebius_ctx_t* x, moebius_mode_t from, moebius_mode_
     ub += s.n_units;
     P->segs.push_back(s);
   }
-  if (ub >= (1ull << 32) || P->segs.size() > (size_t)kMaxSegs || P->kv.size() > (size_t)x->max_kv_desc + 0 ||
+  if (ub >= (1ull << 32) || P->segs.size() > (size_t)kMaxSegs || (int64_t)nm > x->max_kv_desc ||
       P->c2d.size() > (size_t)x->max_c2d)
     return fail(MOEBIUS_E_INVAL);
   P->total_units = (uint32_t)ub;
@@ -772,29 +813,58 @@ extern "C" int moebius_plan(moebius_ctx_t* x, moebius_mode_t from, moebius_mode_
   P->stage_bytes = x->stage_bytes;
   P->xt_rows = x->xt_rows;
 
-  // ---- target request state + upload images -----------------------------------------------------
+  // ---- target request state + upload images (written in place: [segs][kv][c2d] | tables) ---------
   P->lens.assign(seq_lens, seq_lens + n_req);
   P->owner = owner;
-  P->bt = bt;
   int64_t seg_b = align_up((int64_t)P->segs.size() * sizeof(Seg), 256);
-  int64_t kv_b = align_up((int64_t)P->kv.size() * sizeof(KvDesc), 256);
+  int64_t kv_b = align_up((int64_t)nm * sizeof(KvDesc), 256);
   int64_t c2d_b = align_up((int64_t)P->c2d.size() * sizeof(C2dDesc), 256);
   P->kv_img_off = seg_b;
   P->c2d_img_off = seg_b + kv_b;
   P->image_bytes = seg_b + kv_b + c2d_b;
   P->tbl_bytes = 4 * ((int64_t)kTblHdrInts + 2 * (int64_t)c.max_requests + (int64_t)n_req * MP);
-  P->image = (char*)host_alloc(P->image_bytes + P->tbl_bytes + 256, &P->pinned);
-  if (!P->image) return fail(MOEBIUS_E_INVAL);
-  memset(P->image, 0, (size_t)(P->image_bytes + P->tbl_bytes + 256));
-  if (!P->segs.empty()) memcpy(P->image, P->segs.data(), P->segs.size() * sizeof(Seg));
-  if (!P->kv.empty()) memcpy(P->image + P->kv_img_off, P->kv.data(), P->kv.size() * sizeof(KvDesc));
-  if (!P->c2d.empty()) memcpy(P->image + P->c2d_img_off, P->c2d.data(), P->c2d.size() * sizeof(C2dDesc));
+  if (!image_acquire(x, P->image_bytes + P->tbl_bytes + 256, &P->buf)) return fail(MOEBIUS_E_INVAL);
+  P->image = P->buf.p;
+  if (!P->segs.empty()) {
+    memcpy(P->image, P->segs.data(), P->segs.size() * sizeof(Seg));
+    memset(P->image + P->segs.size() * sizeof(Seg), 0, (size_t)(seg_b - (int64_t)(P->segs.size() * sizeof(Seg))));
+  }
+  {  // KV descriptors ordered [level 0][level 1]...[level K][staged]
+    KvDesc* kvd = (KvDesc*)(P->image + P->kv_img_off);
+    P->kv = kvd;
+    P->n_kv = nm;
+    if (nm > 0) {
+      std::vector<uint32_t>& cur = W.cur;
+      cur.assign(W.lvl_begin.begin(), W.lvl_begin.end() - 1);
+      uint32_t scur = W.lvl_begin[K + 1];
+      for (int m = 0; m < nm; ++m) {
+        KvDesc d;
+        d.ep_rank = mv[m].ep_rank; d.ep_page = mv[m].ep_page; d.tp_page = mv[m].tp_page;
+        d.ntok_slot = (uint32_t)mv[m].ntok | (mv[m].staged ? ((uint32_t)mv[m].slot << 8) : 0u);
+        if (mv[m].staged) kvd[scur++] = d; else kvd[cur[mv[m].level]++] = d;
+      }
+    }
+    memset(P->image + P->kv_img_off + (int64_t)nm * sizeof(KvDesc), 0, (size_t)(kv_b - (int64_t)nm * (int64_t)sizeof(KvDesc)));
+  }
+  if (c2d_b) {
+    memcpy(P->image + P->c2d_img_off, P->c2d.data(), P->c2d.size() * sizeof(C2dDesc));
+    memset(P->image + P->c2d_img_off + P->c2d.size() * sizeof(C2dDesc), 0, (size_t)(c2d_b - (int64_t)(P->c2d.size() * sizeof(C2dDesc))));
+  }
   P->tbl_image = (int32_t*)(P->image + align_up(P->image_bytes, 256));
   int32_t* T = P->tbl_image;
+  memset(T, 0, kTblHdrInts * 4);
   T[0] = to; T[1] = n_req; T[2] = c.max_requests; T[3] = MP;
   for (int i = 0; i < c.max_requests; ++i) { T[kTblHdrInts + i] = -1; T[kTblHdrInts + c.max_requests + i] = 0; }
   for (int i = 0; i < n_req; ++i) { T[kTblHdrInts + i] = owner[i]; T[kTblHdrInts + c.max_requests + i] = seq_lens[i]; }
-  if (n_req) memcpy(T + kTblHdrInts + 2 * c.max_requests, bt.data(), (size_t)n_req * MP * 4);
+  {
+    int32_t* tb = T + kTblHdrInts + 2 * c.max_requests;
+    for (int i = 0; i < n_req; ++i) {
+      int32_t* row = tb + (size_t)i * MP;
+      memcpy(row, bt.data() + (size_t)i * MP, (size_t)npages[i] * 4);
+      for (int b = npages[i]; b < MP; ++b) row[b] = -1;
+    }
+    P->bt = tb;
+  }
 
   P->stats.n_segments = (int32_t)P->segs.size();
   P->stats.n_kv_moves = nm;
@@ -812,7 +882,8 @@ extern "C" int moebius_plan(moebius_ctx_t* x, moebius_mode_t from, moebius_mode_
 extern "C" int moebius_block_tables(const moebius_plan_t* p, int32_t* dst_owner, int32_t* dst_bt) {
   if (!p) return MOEBIUS_E_INVAL;
   if (dst_owner && p->n_req) memcpy(dst_owner, p->owner.data(), (size_t)p->n_req * 4);
-  if (dst_bt && p->n_req) memcpy(dst_bt, p->bt.data(), p->bt.size() * 4);
+  if (dst_bt && p->n_req)
+    memcpy(dst_bt, p->bt, (size_t)p->n_req * (size_t)p->ctx->cfg.max_pages_per_request * 4);
   return MOEBIUS_OK;
 }
 
@@ -827,7 +898,7 @@ extern "C" int moebius_plan_export(const moebius_plan_t* p, int what, void* buf,
   const void* src; int64_t n;
   switch (what) {
     case 0: src = p->segs.data(); n = (int64_t)p->segs.size() * sizeof(Seg); break;
-    case 1: src = p->kv.data();   n = (int64_t)p->kv.size() * sizeof(KvDesc); break;
+    case 1: src = p->kv;          n = p->n_kv * (int64_t)sizeof(KvDesc); break;
     case 2: src = p->c2d.data();  n = (int64_t)p->c2d.size() * sizeof(C2dDesc); break;
     default: return MOEBIUS_E_INVAL;
   }
