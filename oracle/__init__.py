@@ -12,7 +12,7 @@ brute force, closed forms, invariants, the FFN equivalence the paper states (PAP
 hand-worked fixtures under `tests/golden/`.  No function is "parity unpinned".
 """
 from .weights import (  # noqa: F401
-    ep_weight_view, tp_weight_view, tp_scale_blocks, tp_scale_view, ep_scale_view,
+    ep_weight_view, tp_weight_view, tp_scale_blocks, tp_scale_view, ep_scale_view, tp_w13_view, tp_w2_view,
 )
 from .kv import (  # noqa: F401
     CapacityError, canonical_block_tables, ep_pool_image, kv_heads_of_rank, pages_needed,
@@ -20,4 +20,5 @@ from .kv import (  # noqa: F401
 )
 from .accounting import kv_bytes, weight_bytes  # noqa: F401
 from .ffn import moe_ffn_dense, moe_ffn_ep, moe_ffn_tp, route_top2  # noqa: F401
+from .ffn import moe_ffn_dense_w13, moe_ffn_ep_w13, moe_ffn_tp_w13  # noqa: F401
 from .image import OracleLayout, State, np_view, target_request_state  # noqa: F401,E402

@@ -69,3 +69,48 @@ def moe_ffn_ep(x, gate_ep, up_ep, down_ep, idx, w):
             a = silu(x[t] @ gate_ep[r][el]) * (x[t] @ up_ep[r][el])
             y[t] += w[t, k] * (a @ down_ep[r][el])
     return y
+
+
+# ---- the same FFN from the paper's orientation (W13 [E,2I,H], W2 [E,H,I]) ----------
+# Row i of W13[e] is output channel i of the gate projection (i < I) or of the up projection
+# (i >= I); W2[e] maps the I intermediate channels back to H:  a = silu(W13g x) * (W13u x), y = W2 a.
+
+def moe_ffn_dense_w13(x, W13, W2, idx, w):
+    I = W13.shape[1] // 2
+    y = np.zeros((x.shape[0], W2.shape[1]), dtype=x.dtype)
+    for t in range(x.shape[0]):
+        for k in range(idx.shape[1]):
+            e = idx[t, k]
+            h = W13[e] @ x[t]
+            y[t] += w[t, k] * (W2[e] @ (silu(h[:I]) * h[I:]))
+    return y
+
+
+def moe_ffn_tp_w13(x, W13_tp, W2_tp, idx, w):
+    """W13_tp[r]: [E, 2I/R, H] (gate block then up block, reading A2), W2_tp[r]: [E, H, I/R]; each
+    rank computes a partial from its shards alone, the All-Reduce sums them."""
+    y = np.zeros((x.shape[0], W2_tp[0].shape[1]), dtype=x.dtype)
+    for r in range(len(W13_tp)):
+        wloc = W13_tp[r].shape[1] // 2
+        part = np.zeros_like(y)
+        for t in range(x.shape[0]):
+            for k in range(idx.shape[1]):
+                e = idx[t, k]
+                h = W13_tp[r][e] @ x[t]
+                part[t] += w[t, k] * (W2_tp[r][e] @ (silu(h[:wloc]) * h[wloc:]))
+        y += part
+    return y
+
+
+def moe_ffn_ep_w13(x, W13_ep, W2_ep, idx, w):
+    """W13_ep[r]: [E/R, 2I, H], W2_ep[r]: [E/R, H, I]; the owner of expert e computes it whole."""
+    n_loc = W13_ep[0].shape[0]
+    I = W13_ep[0].shape[1] // 2
+    y = np.zeros((x.shape[0], W2_ep[0].shape[1]), dtype=x.dtype)
+    for t in range(x.shape[0]):
+        for k in range(idx.shape[1]):
+            e = int(idx[t, k])
+            r, el = e // n_loc, e % n_loc
+            h = W13_ep[r][el] @ x[t]
+            y[t] += w[t, k] * (W2_ep[r][el] @ (silu(h[:I]) * h[I:]))
+    return y

@@ -3,7 +3,8 @@
 The oracle does not know the address map: the caller passes `view_fn(mode, rank, layer, tensor_id)
 -> (byte_offset, shape, elem_bytes)` (the fixed views the library reports) and the
 pool page counts.  Nothing here imports the CUDA path.  mode: 0 = TP, 1 = EP; tensor ids: 0 gate,
-1 up, 2 down, 3 K pool, 4 V pool, 5/6/7 fp8 scales of gate/up/down.
+1 up, 2 down, 3 K pool, 4 V pool, 5/6/7 fp8 scales of gate/up/down; paper orientation (w_orient = 1,
+PAPER.md:100): 8 W13, 9 W2, 10/11 their fp8 scales.
 """
 from __future__ import annotations
 
@@ -16,6 +17,13 @@ from . import weights as ow
 
 KINDS = ("gate", "up", "down")
 TP, EP = 0, 1
+
+
+def weight_tensors(cfg):
+    """[(kind, tensor id, scale tensor id)] of the orientation the config names."""
+    if getattr(cfg, "w_orient", 0) == 1:
+        return [("w13", 8, 10), ("w2", 9, 11)]
+    return [("gate", 0, 5), ("up", 1, 6), ("down", 2, 7)]
 
 
 class State:
@@ -86,10 +94,10 @@ class OracleLayout:
         fp8 = c.w_dtype == "fp8_e4m3_b128"
         for r in range(c.R):
             for l in range(c.L):
-                for m, kind in enumerate(KINDS):
-                    np_view(image, self.view_fn(self.mode, r, l, m))[...] = self.weight_view(r, l, kind)
+                for kind, tid, sid in weight_tensors(c):
+                    np_view(image, self.view_fn(self.mode, r, l, tid))[...] = self.weight_view(r, l, kind)
                     if fp8:
-                        np_view(image, self.view_fn(self.mode, r, l, 5 + m))[...] = self.scale_view(r, l, kind)
+                        np_view(image, self.view_fn(self.mode, r, l, sid))[...] = self.scale_view(r, l, kind)
                 for kvi in range(2):
                     pool, mask = self.pool(r, l, kvi)
                     np_view(image, self.view_fn(self.mode, r, l, 3 + kvi))[mask] = pool[mask]
@@ -102,13 +110,13 @@ class OracleLayout:
         bad = []
         for r in range(c.R):
             for l in range(c.L):
-                for m, kind in enumerate(KINDS):
-                    got = np_view(image, self.view_fn(self.mode, r, l, m))
+                for kind, tid, sid in weight_tensors(c):
+                    got = np_view(image, self.view_fn(self.mode, r, l, tid))
                     want = self.weight_view(r, l, kind)
                     if not np.array_equal(got.view(np.uint8), want.view(np.uint8)):
                         bad.append("weight r%d l%d %s: %d elems differ" % (r, l, kind, int((got != want).sum())))
                     if fp8:
-                        got = np_view(image, self.view_fn(self.mode, r, l, 5 + m))
+                        got = np_view(image, self.view_fn(self.mode, r, l, sid))
                         want = self.scale_view(r, l, kind)
                         if not np.array_equal(got.view(np.uint32), want.view(np.uint32)):
                             bad.append("scale r%d l%d %s" % (r, l, kind))

@@ -33,7 +33,41 @@ def tp_weight_view(X: np.ndarray, kind: str, r: int, R: int) -> np.ndarray:
         _check(E, I, R)
         w = I // R
         return np.ascontiguousarray(X[:, r * w:(r + 1) * w, :])
+    if kind == "w13":
+        return tp_w13_view(X, r, R)
+    if kind == "w2":
+        return tp_w2_view(X, r, R)
     raise ValueError(kind)
+
+
+# ---- the paper's own orientation (PAPER.md:100; readings A1/A2; w_orient = 1) --------------------
+# "stores the full gate-up projection W13 with shape (E_local, 2I, H), where the leading factor of
+# two stacks the gate and up projections of the SwiGLU MLP, and the full down projection W2 with
+# shape (E_local, H, I).  Under TP ... W13 has shape (E, 2I/P, H), and W2 has shape (E, H, I/P)."
+# PAPER.md:110: gate-up reshards along the OUTPUT intermediate dimension (rows of W13), down along
+# the INPUT intermediate dimension (columns of W2).
+
+def tp_w13_view(W13: np.ndarray, r: int, R: int) -> np.ndarray:
+    """[E, 2I, H] -> [E, 2I/R, H].  Reading A2 (per projection): rank r takes rows
+    [r*I/R, (r+1)*I/R) of the gate half (rows 0..I-1) and the same rows of the up half
+    (rows I..2I-1), gate block first -- so every rank can run SwiGLU on its own shard."""
+    E, I2, H = W13.shape
+    if I2 % 2:
+        raise ValueError("W13 stacks gate and up: its middle axis must be even")
+    I = I2 // 2
+    _check(E, I, R)
+    w = I // R
+    gate_rows = W13[:, r * w:(r + 1) * w, :]
+    up_rows = W13[:, I + r * w:I + (r + 1) * w, :]
+    return np.ascontiguousarray(np.concatenate([gate_rows, up_rows], axis=1))
+
+
+def tp_w2_view(W2: np.ndarray, r: int, R: int) -> np.ndarray:
+    """[E, H, I] -> [E, H, I/R]: columns [r*I/R, (r+1)*I/R) (the input-intermediate dimension)."""
+    E, H, I = W2.shape
+    _check(E, I, R)
+    w = I // R
+    return np.ascontiguousarray(W2[:, :, r * w:(r + 1) * w])
 
 
 def ep_weight_view(X: np.ndarray, r: int, R: int) -> np.ndarray:
@@ -61,10 +95,15 @@ def tp_scale_view(S: np.ndarray, kind: str, r: int, R: int, I: int) -> np.ndarra
     """gate/up scales [E, H/128, I/128] -> [E, H/128, nb_r]; down scales [E, I/128, H/128] ->
     [E, nb_r, H/128], nb_r = number of blocks shard r touches."""
     lo, hi = tp_scale_blocks(r, R, I)
-    if kind in ("gate", "up"):
+    if kind in ("gate", "up", "w2"):      # w2 scales [E, H/128, I/128]: intermediate blocks last
         return np.ascontiguousarray(S[:, :, lo:hi])
     if kind == "down":
         return np.ascontiguousarray(S[:, lo:hi, :])
+    if kind == "w13":
+        # scales [E, 2I/128, H/128]: the shard carries the blocks its gate rows touch, then the
+        # blocks its up rows touch (the same block indices, offset by I/128) -> [E, 2*nb_r, H/128]
+        ib = I // 128
+        return np.ascontiguousarray(np.concatenate([S[:, lo:hi, :], S[:, ib + lo:ib + hi, :]], axis=1))
     raise ValueError(kind)
 
 

@@ -18,5 +18,6 @@ from .gen import (  # noqa: F401
     tag_fill_u16_torch,
     tag_salt_offset,
     weight_tag_salt,
+    weight_shape,
     kv_tag_salt,
 )

@@ -25,6 +25,7 @@ class Config:
     len_dist: tuple   # ("uniform", lo, hi) | ("lognormal", median, sigma, cap) | ("geometric", mean, cap)
     seed: int
     pool_policy: str = "roomy"   # roomy = 1.1 x (TP need + max EP live)
+    w_orient: int = 0            # 0: gate,up [E,H,I], down [E,I,H] (BASELINE.json); 1: W13 [E,2I,H], W2 [E,H,I]
     extra: dict = field(default_factory=dict)
 
     @property
@@ -34,6 +35,10 @@ class Config:
     @property
     def kv_elem_bytes(self) -> int:
         return 2  # bf16 in every config (reading A14)
+
+    @property
+    def w_kinds(self) -> tuple:
+        return ("gate", "up", "down") if self.w_orient == 0 else ("w13", "w2")
 
     def with_(self, **kw) -> "Config":
         return replace(self, **kw)

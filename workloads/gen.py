@@ -54,8 +54,21 @@ def tag_fill_u16_torch(flat_index, offset):
     return h & 0xFFFF
 
 
+_KIND_ID = {"gate": 0, "up": 1, "down": 2, "w13": 3, "w2": 4}
+
+
+def weight_shape(cfg: Config, kind: str) -> tuple:
+    """Logical shape of one layer's expert tensor: gate/up [E,H,I], down [E,I,H] (BASELINE.json);
+    w13 [E,2I,H], w2 [E,H,I] (the paper's own orientation)."""
+    return {"gate": (cfg.E, cfg.H, cfg.I), "up": (cfg.E, cfg.H, cfg.I), "down": (cfg.E, cfg.I, cfg.H),
+            "w13": (cfg.E, 2 * cfg.I, cfg.H), "w2": (cfg.E, cfg.H, cfg.I)}[kind]
+
+
 def weight_tag_salt(cfg: Config, layer: int, kind: str) -> int:
-    return cfg.seed * 1000 + layer * 3 + {"gate": 0, "up": 1, "down": 2}[kind]
+    m = _KIND_ID[kind]
+    if m < 3:
+        return cfg.seed * 1000 + layer * 3 + m
+    return cfg.seed * 1000 + 500 + layer * 2 + (m - 3)
 
 
 def kv_tag_salt(cfg: Config, layer: int, kv: int, req: int) -> int:
@@ -67,8 +80,8 @@ def gen_logical_weight(cfg: Config, layer: int, kind: str, fill: str = "normal")
 
     bf16 -> uint16 bit patterns of N(0, 0.02); fp32 -> float32 N(0, 0.02); fp8 -> uint8 bytes
     (opaque e4m3 codes, uniform over 0..255 minus the two NaN codes)."""
-    m = {"gate": 0, "up": 1, "down": 2}[kind]
-    shape = (cfg.E, cfg.H, cfg.I) if m < 2 else (cfg.E, cfg.I, cfg.H)
+    m = _KIND_ID[kind]
+    shape = weight_shape(cfg, kind)
     seed = (cfg.seed, 2000 + layer, m)
     if fill == "tag":
         t = tag_fill_u16(shape, salt=weight_tag_salt(cfg, layer, kind))
@@ -87,9 +100,10 @@ def gen_logical_weight(cfg: Config, layer: int, kind: str, fill: str = "normal")
 
 
 def gen_logical_scale(cfg: Config, layer: int, kind: str) -> np.ndarray:
-    """fp32 per-128x128-block scales: gate/up [E, H/128, I/128], down [E, I/128, H/128]."""
-    m = {"gate": 0, "up": 1, "down": 2}[kind]
-    shape = ((cfg.E, cfg.H // 128, cfg.I // 128) if m < 2 else (cfg.E, cfg.I // 128, cfg.H // 128))
+    """fp32 per-128x128-block scales: gate/up [E, H/128, I/128], down [E, I/128, H/128];
+    w13 [E, 2I/128, H/128], w2 [E, H/128, I/128]."""
+    m = _KIND_ID[kind]
+    shape = tuple([cfg.E] + [d // 128 for d in weight_shape(cfg, kind)[1:]])
     rng = np.random.default_rng((cfg.seed, 2500 + layer, m))
     return rng.uniform(0.5, 2.0, size=shape).astype(np.float32)
 
