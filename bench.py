@@ -51,6 +51,8 @@ def parse():
     ap.add_argument("--n-req", type=int, default=-1, help="override the number of live requests (experiments; named in config.workload)")
     ap.add_argument("--tma", default="", help="enable,pipes,stage_kb (tuning; default: library defaults)")
     ap.add_argument("--kv-rounds", type=int, default=0, help="max dependent KV rounds before chains are cut by staging (tuning)")
+    ap.add_argument("--w-orient", type=int, default=0, choices=[0, 1],
+                    help="0: gate,up [E,H,I], down [E,I,H] (BASELINE.json, the headline); 1: the paper's W13 [E,2I,H], W2 [E,H,I] (named in config.workload)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--profile-region", action="store_true",
                     help="cudaProfilerStart/Stop round warm-up + timed steps (ncu --profile-from-start off skips the fill)")
@@ -121,8 +123,8 @@ def oracle_sample(cfg, n_sample_req, seed=0):
     rng = np.random.default_rng(seed)
     dt = {"bf16": np.uint16, "fp32": np.float32, "fp8_e4m3_b128": np.uint8}[cfg.w_dtype]
     W = {}
-    for kind in ("gate", "up", "down"):
-        shape = (cfg.E, cfg.H, cfg.I) if kind != "down" else (cfg.E, cfg.I, cfg.H)
+    for kind in cfg.w_kinds:
+        shape = wl.weight_shape(cfg, kind)
         if dt == np.float32:
             W[kind] = rng.standard_normal(shape, dtype=np.float32)
         else:   # opaque bit patterns: generation cost is excluded from the timing anyway
@@ -147,14 +149,14 @@ def oracle_round_trip(cfg, W, lens, KV, pool_bytes):
     owner = oracle.partition_requests(lens, R)
     bt_ep = oracle.canonical_block_tables(lens, owner, "ep", pages_ep, pg, mp)
     for r in range(R):
-        for kind in ("gate", "up", "down"):
+        for kind in cfg.w_kinds:
             oracle.ep_weight_view(W[kind], r, R)
         for kvi in range(2):
             oracle.ep_pool_image(KV[kvi], lens, owner, bt_ep, r, Hkv, D, pg, pages_ep)
     # EP -> TP
     bt_tp = oracle.canonical_block_tables(lens, None, "tp", pages_tp, pg, mp)
     for r in range(R):
-        for kind in ("gate", "up", "down"):
+        for kind in cfg.w_kinds:
             oracle.tp_weight_view(W[kind], kind, r, R)
         for kvi in range(2):
             oracle.tp_pool_image(KV[kvi], lens, bt_tp, r, R, Hkv, D, pg, pages_tp)
@@ -180,8 +182,8 @@ def time_oracle(cfg, n_sample_req, steps, warmup, pool_bytes):
         owner = oracle_round_trip(cfg, W, lens, KV, pool_bytes)
     dt = time.perf_counter() - t0
     moved = steps * oracle_sample_moved(cfg, lens, owner)
-    sample = ("layer 0 of %d: gate/up/down of all %d experts + K and V pools of the first %d of %d requests; "
-              "one TP->EP->TP round trip per step" % (cfg.L, cfg.E, len(lens), cfg.n_req))
+    sample = ("layer 0 of %d: %s of all %d experts + K and V pools of the first %d of %d requests; "
+              "one TP->EP->TP round trip per step" % (cfg.L, "/".join(cfg.w_kinds), cfg.E, len(lens), cfg.n_req))
     return {"value": moved / dt / 1e9, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample,
             "seconds": dt, "ms_per_step": dt / steps * 1e3}
 
@@ -215,7 +217,7 @@ def fill_device(sess, cfg, mb, torch):
     g.manual_seed(cfg.seed)
     for r in range(cfg.R):
         for l in range(cfg.L):
-            for t in (mb.T_GATE, mb.T_UP, mb.T_DOWN):
+            for t in ((mb.T_GATE, mb.T_UP, mb.T_DOWN) if cfg.w_orient == 0 else (mb.T_W13, mb.T_W2)):
                 v = sess.view(mb.MOEBIUS_TP, r, l, t)
                 if v.dtype == torch.int16:
                     v.view(torch.bfloat16).normal_(0.0, 0.02, generator=g)
@@ -246,6 +248,8 @@ def run_moebius(args):
     cfg = wl.get_config(args.config)
     if args.layers:
         cfg = cfg.with_(L=args.layers, name="%s[L=%d]" % (cfg.name, args.layers))
+    if args.w_orient:
+        cfg = cfg.with_(w_orient=1, name="%s[w_orient=1]" % cfg.name)
     lens = wl.draw_seq_lens(cfg)
     pool = wl.kv_pool_bytes(cfg, lens, args.pool)
     if args.n_req >= 0:
@@ -254,7 +258,8 @@ def run_moebius(args):
     mp = int(max([1] + [(int(x) + cfg.page - 1) // cfg.page for x in lens]))
     c = mb.make_config(R=cfg.R, L=cfg.L, E=cfg.E, H=cfg.H, I=cfg.I, w_dtype=cfg.w_dtype, kv_heads=cfg.kv_heads,
                        head_dim=cfg.head_dim, page_tokens=cfg.page, kv_pool_bytes_per_rank_layer=pool,
-                       max_requests=max(len(lens), 1), max_pages_per_request=mp, staging_cap_bytes=0)
+                       max_requests=max(len(lens), 1), max_pages_per_request=mp, staging_cap_bytes=0,
+                       w_orient=cfg.w_orient)
     probe = mb.Session(c)
     resident = probe.layout.resident_bytes
     probe.close()
@@ -334,8 +339,9 @@ def run_moebius(args):
     d2d = None
     if cfg.R > 1:
         n_copy = int(min(lay.weight_slot_bytes * (3 * cfg.L), 8 << 30)) // 256 * 256
-        a0 = sess.view_desc(TP, 0, 0, mb.T_GATE).offset
-        a1 = sess.view_desc(TP, cfg.R - 1, 0, mb.T_GATE).offset
+        t0_id = mb.T_GATE if cfg.w_orient == 0 else mb.T_W13
+        a0 = sess.view_desc(TP, 0, 0, t0_id).offset
+        a1 = sess.view_desc(TP, cfg.R - 1, 0, t0_id).offset
         src, dst = sess.base[a0:a0 + n_copy], sess.base[a1:a1 + n_copy]
         keep = dst.clone()
         best = None

@@ -28,6 +28,9 @@
  *   object k = 3*layer + {gate:0, up:1, down:2}; the TP view of object k is slot k, the EP view is
  *   slot k+1 (Fig. 7, at (layer,matrix) grain).  KV: the TP pool and the EP pool of
  *   a (rank, layer, K|V) alias the same bytes with different page sizes.
+ *   w_orient = 1 (the paper's own shapes): two objects per layer, W13 (2 slots) at slot 3*layer and
+ *   W2 (1 slot) at slot 3*layer+2; every EP view starts 2 slots (the largest object) after its TP
+ *   view, so the chain has 3L+2 slots.
  */
 #ifndef MOEBIUS_H_
 #define MOEBIUS_H_
@@ -47,7 +50,10 @@ typedef enum { MOEBIUS_BF16 = 0, MOEBIUS_FP32 = 1, MOEBIUS_FP8_E4M3_B128 = 2 } m
 typedef enum {
   MOEBIUS_T_GATE = 0, MOEBIUS_T_UP = 1, MOEBIUS_T_DOWN = 2,
   MOEBIUS_T_KPOOL = 3, MOEBIUS_T_VPOOL = 4,
-  MOEBIUS_T_GATE_SCALE = 5, MOEBIUS_T_UP_SCALE = 6, MOEBIUS_T_DOWN_SCALE = 7 /* fp8 only */
+  MOEBIUS_T_GATE_SCALE = 5, MOEBIUS_T_UP_SCALE = 6, MOEBIUS_T_DOWN_SCALE = 7, /* fp8 only */
+  /* w_orient = 1 (the paper's own shapes): ids 0..2 and 5..7 are invalid, these are valid */
+  MOEBIUS_T_W13 = 8, MOEBIUS_T_W2 = 9,
+  MOEBIUS_T_W13_SCALE = 10, MOEBIUS_T_W2_SCALE = 11 /* fp8 only */
 } moebius_tensor_t;
 
 typedef enum {
@@ -68,8 +74,10 @@ typedef struct {
   uint32_t struct_size;
   int32_t R, L, E, H, I;      /* E%R==0, I%R==0, (I/R)*elem_bytes % 16 == 0, else MOEBIUS_E_INVAL */
   int32_t w_dtype;            /* moebius_dtype_t; FP8_E4M3_B128 adds fp32 128x128-block scales    */
-  int32_t w_orient;           /* 0: gate,up [E,H,I], down [E,I,H] (BASELINE.json).  1 (paper's
-                                 W13 [E,2I,H], W2 [E,H,I]) is not implemented: MOEBIUS_E_INVAL    */
+  int32_t w_orient;           /* 0: gate,up [E,H,I], down [E,I,H] (BASELINE.json, the default).
+                                 1: the paper's W13 [E,2I,H] (gate rows, then up rows) and W2
+                                 [E,H,I]; TP shards: W13 [E,2I/R,H] = rank r's gate
+                                 rows then its up rows (reading A2), W2 [E,H,I/R]                */
   int32_t kv_heads, head_dim, page_tokens;
   int32_t kv_dtype;           /* MOEBIUS_BF16 or MOEBIUS_FP32; kv_heads%R==0 or R%kv_heads==0     */
   int64_t kv_pool_bytes_per_rank_layer; /* capacity of ONE K (or V) pool of one rank and layer; a

@@ -8,6 +8,7 @@ Importing this package fails loudly if the library has not been built
 from ._binding import (  # noqa: F401
     MOEBIUS_TP, MOEBIUS_EP, MOEBIUS_BF16, MOEBIUS_FP32, MOEBIUS_FP8_E4M3_B128,
     T_GATE, T_UP, T_DOWN, T_KPOOL, T_VPOOL, T_GATE_SCALE, T_UP_SCALE, T_DOWN_SCALE,
+    T_W13, T_W2, T_W13_SCALE, T_W2_SCALE,
     MoebiusError, moebius_config_t, moebius_layout_t, moebius_view_t, moebius_stats_t,
     moebius_create, moebius_destroy, moebius_layout, moebius_view, moebius_bind, moebius_active_mode,
     moebius_plan, moebius_plan_destroy, moebius_block_tables, moebius_plan_stats, moebius_plan_export,

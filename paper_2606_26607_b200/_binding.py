@@ -12,6 +12,7 @@ _LIB = os.path.join(_HERE, "libmoebius.so")
 MOEBIUS_TP, MOEBIUS_EP = 0, 1
 MOEBIUS_BF16, MOEBIUS_FP32, MOEBIUS_FP8_E4M3_B128 = 0, 1, 2
 T_GATE, T_UP, T_DOWN, T_KPOOL, T_VPOOL, T_GATE_SCALE, T_UP_SCALE, T_DOWN_SCALE = range(8)
+T_W13, T_W2, T_W13_SCALE, T_W2_SCALE = range(8, 12)   # w_orient = 1
 
 EXPORTED_SYMBOLS = [
     "moebius_create", "moebius_destroy", "moebius_layout", "moebius_view", "moebius_bind",

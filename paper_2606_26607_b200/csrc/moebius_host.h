@@ -43,6 +43,18 @@ struct PlanScratch {
   std::vector<Move> mv;
 };
 
+// One expert-weight object of a layer = one link of the slot chain (PAPER.md:150-156 at (layer,
+// matrix) grain).  Its EP view of rank q is [rows][R runs][run bytes], its TP view of rank j is
+// [q][rows][run bytes].  Offsets in units of the slot size S.
+struct WObj {
+  int tensor_id;             // moebius_tensor_t of the weight; scale tensor id in scale_id
+  int scale_id;
+  int slot, n_slots;         // TP view starts at slot `slot` of the layer's 3 slots; size n_slots * S
+  int long_run;              // 0: run = (I/R)*b, rows = (E/R)*H (the intermediate axis is last)
+                             // 1: run = (I/R)*H*b, rows = (E/R)*row_mult (the intermediate axis is in the middle)
+  int row_mult;              // 2 for the stacked W13 (gate block, up block), else 1
+};
+
 struct ScaleGeom {           // fp8 block scales of one matrix kind (reading A13)
   int64_t tp_bytes;          // per rank, allocated with the largest nb over ranks
   int64_t ep_bytes;          // per rank
@@ -53,7 +65,10 @@ struct ScaleGeom {           // fp8 block scales of one matrix kind (DESIGN.md r
 struct moebius_ctx {
   moebius_config_t cfg;
   int wb, kvb;                    // element bytes
-  int ep_shift;                   // EP view of object k is slot k + ep_shift (0 when R == 1)
+  int ep_shift;                   // the EP view of an object starts ep_shift slots after its TP view
+                                  // (= the largest object, in slots; 0 when R == 1)
+  int n_obj;                      // objects per layer: 3 (gate, up, down) or 2 (W13, W2)
+  moebius::WObj obj[3];
   int64_t S;                      // weight slot bytes per rank
   int64_t w_off, scale_tp_off, scale_ep_off, kv_off, rank_stride;
   moebius::ScaleGeom sg[3];

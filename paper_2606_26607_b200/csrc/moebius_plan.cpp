@@ -62,7 +62,7 @@ int moebius_create(const moebius_config_t* c, moebius_ctx_t** out) {
   const int R = c->R, L = c->L, E = c->E, H = c->H, I = c->I;
   if (R < 1 || L < 1 || E < 1 || H < 1 || I < 1 || R > 64) return MOEBIUS_E_INVAL;
   if (E % R || I % R) return MOEBIUS_E_INVAL;
-  if (c->w_orient != 0) return MOEBIUS_E_INVAL;
+  if (c->w_orient != 0 && c->w_orient != 1) return MOEBIUS_E_INVAL;
   const int wb = dtype_bytes(c->w_dtype);
   const int kvb = (c->kv_dtype == MOEBIUS_BF16 || c->kv_dtype == MOEBIUS_FP32) ? dtype_bytes(c->kv_dtype) : 0;
   if (!wb || !kvb) return MOEBIUS_E_INVAL;
@@ -79,7 +79,19 @@ int moebius_create(const moebius_config_t* c, moebius_ctx_t** out) {
   x->cfg = *c;
   x->wb = wb;
   x->kvb = kvb;
-  x->ep_shift = R == 1 ? 0 : 1;
+  if (c->w_orient == 0) {   // BASELINE.json: gate, up [E,H,I], down [E,I,H]
+    x->n_obj = 3;
+    x->obj[0] = {MOEBIUS_T_GATE, MOEBIUS_T_GATE_SCALE, 0, 1, 0, 1};
+    x->obj[1] = {MOEBIUS_T_UP, MOEBIUS_T_UP_SCALE, 1, 1, 0, 1};
+    x->obj[2] = {MOEBIUS_T_DOWN, MOEBIUS_T_DOWN_SCALE, 2, 1, 1, 1};
+  } else {                  // W13 [E,2I,H] (gate rows then up rows), W2 [E,H,I]
+    x->n_obj = 2;
+    x->obj[0] = {MOEBIUS_T_W13, MOEBIUS_T_W13_SCALE, 0, 2, 1, 2};
+    x->obj[1] = {MOEBIUS_T_W2, MOEBIUS_T_W2_SCALE, 2, 1, 0, 1};
+    x->obj[2] = {-1, -1, 0, 0, 0, 0};
+  }
+  x->ep_shift = 0;
+  if (R > 1) for (int o = 0; o < x->n_obj; ++o) x->ep_shift = std::max(x->ep_shift, x->obj[o].n_slots);
   x->hpr = Hkv >= R ? Hkv / R : 1;
   x->rep = Hkv >= R ? 1 : R / Hkv;
   x->G = Hkv >= R ? R : Hkv;
@@ -103,9 +115,10 @@ int moebius_create(const moebius_config_t* c, moebius_ctx_t** out) {
   if (c->w_dtype == MOEBIUS_FP8_E4M3_B128) {
     int nb_max = 0;
     for (int r = 0; r < R; ++r) { int lo, hi; scale_blocks(r, R, I, &lo, &hi); nb_max = std::max(nb_max, hi - lo); }
-    for (int m = 0; m < 3; ++m) {
-      x->sg[m].tp_bytes = align_up((int64_t)E * (H / 128) * nb_max * 4, 256);
-      x->sg[m].ep_bytes = align_up((int64_t)(E / R) * (H / 128) * (I / 128) * 4, 256);
+    for (int m = 0; m < x->n_obj; ++m) {
+      const int mult = x->obj[m].row_mult;
+      x->sg[m].tp_bytes = align_up((int64_t)E * (H / 128) * nb_max * mult * 4, 256);
+      x->sg[m].ep_bytes = align_up((int64_t)(E / R) * (H / 128) * (I / 128) * mult * 4, 256);
       x->scale_tp_layer += x->sg[m].tp_bytes;
       x->scale_ep_layer += x->sg[m].ep_bytes;
     }
@@ -131,7 +144,7 @@ int moebius_create(const moebius_config_t* c, moebius_ctx_t** out) {
   int64_t live_max = std::max<int64_t>((int64_t)x->pages_tp, (int64_t)x->pages_ep * R);
   live_max = std::min<int64_t>(live_max, (int64_t)c->max_requests * c->max_pages_per_request);
   x->max_kv_desc = live_max;
-  x->max_c2d = c->w_dtype == MOEBIUS_FP8_E4M3_B128 ? (int64_t)3 * L * R * R : 0;
+  x->max_c2d = c->w_dtype == MOEBIUS_FP8_E4M3_B128 ? (int64_t)x->n_obj * L * R * R : 0;
   x->desc_bytes = align_up(kSegOff + (int64_t)kMaxSegs * sizeof(Seg) + x->max_kv_desc * sizeof(KvDesc) +
                                x->max_c2d * sizeof(C2dDesc) + 1024, 4096);
   x->table_bytes = align_up(4 * ((int64_t)kTblHdrInts + 2 * (int64_t)c->max_requests +
@@ -197,13 +210,20 @@ int moebius_view(const moebius_ctx_t* x, moebius_mode_t mode, int rank, int laye
   const int64_t rbase = (int64_t)rank * x->rank_stride;
   const int R = c.R, E = c.E, H = c.H, I = c.I;
   for (int i = 0; i < 4; ++i) o->shape[i] = 1;
-  if (t >= MOEBIUS_T_GATE && t <= MOEBIUS_T_DOWN) {
-    int k = 3 * layer + t;
-    o->offset = rbase + x->w_off + (int64_t)(k + (tp ? 0 : x->ep_shift)) * x->S;
+  int wo = -1, so = -1;   // object whose weight / scale tensor this id names
+  for (int o = 0; o < x->n_obj; ++o) {
+    if (x->obj[o].tensor_id == t) wo = o;
+    if (x->obj[o].scale_id == t) so = o;
+  }
+  if (wo >= 0) {
+    const WObj& ob = x->obj[wo];
+    o->offset = rbase + x->w_off + (int64_t)(3 * layer + ob.slot + (tp ? 0 : x->ep_shift)) * x->S;
     o->elem_bytes = x->wb;
     o->ndim = 3;
-    if (t != MOEBIUS_T_DOWN) { o->shape[0] = tp ? E : E / R; o->shape[1] = H; o->shape[2] = tp ? I / R : I; }
-    else                     { o->shape[0] = tp ? E : E / R; o->shape[1] = tp ? I / R : I; o->shape[2] = H; }
+    o->shape[0] = tp ? E : E / R;
+    const int64_t i_dim = (int64_t)(tp ? I / R : I) * ob.row_mult;
+    if (!ob.long_run) { o->shape[1] = H; o->shape[2] = i_dim; }   // gate, up, W2: [., H, I]
+    else              { o->shape[1] = i_dim; o->shape[2] = H; }   // down, W13:    [., I or 2I, H]
   } else if (t == MOEBIUS_T_KPOOL || t == MOEBIUS_T_VPOOL) {
     int z = 2 * layer + (t - MOEBIUS_T_KPOOL);
     o->offset = rbase + x->kv_off + (int64_t)z * x->pool_bytes;
@@ -213,20 +233,21 @@ int moebius_view(const moebius_ctx_t* x, moebius_mode_t mode, int rank, int laye
     o->shape[1] = c.page_tokens;
     o->shape[2] = tp ? x->hpr : c.kv_heads;
     o->shape[3] = c.head_dim;
-  } else if (t >= MOEBIUS_T_GATE_SCALE && t <= MOEBIUS_T_DOWN_SCALE) {
+  } else if (so >= 0) {
     if (c.w_dtype != MOEBIUS_FP8_E4M3_B128) return MOEBIUS_E_INVAL;
-    int m = t - MOEBIUS_T_GATE_SCALE;
+    const WObj& ob = x->obj[so];
     int64_t within = 0;
-    for (int mm = 0; mm < m; ++mm) within += tp ? x->sg[mm].tp_bytes : x->sg[mm].ep_bytes;
+    for (int mm = 0; mm < so; ++mm) within += tp ? x->sg[mm].tp_bytes : x->sg[mm].ep_bytes;
     o->offset = rbase + (tp ? x->scale_tp_off + layer * x->scale_tp_layer
                             : x->scale_ep_off + layer * x->scale_ep_layer) + within;
     o->elem_bytes = 4;
     o->ndim = 3;
     int lo, hi;
     scale_blocks(rank, R, I, &lo, &hi);
-    int nb = hi - lo;
-    if (m < 2) { o->shape[0] = tp ? E : E / R; o->shape[1] = H / 128; o->shape[2] = tp ? nb : I / 128; }
-    else       { o->shape[0] = tp ? E : E / R; o->shape[1] = tp ? nb : I / 128; o->shape[2] = H / 128; }
+    const int64_t i_dim = (int64_t)(tp ? hi - lo : I / 128) * ob.row_mult;
+    o->shape[0] = tp ? E : E / R;
+    if (!ob.long_run) { o->shape[1] = H / 128; o->shape[2] = i_dim; }
+    else              { o->shape[1] = i_dim; o->shape[2] = H / 128; }
   } else {
     return MOEBIUS_E_INVAL;
   }
@@ -586,26 +607,33 @@ extern "C" int moebius_plan(moebius_ctx_t* x, moebius_mode_t from, moebius_mode_
   auto fail = [&](int code) { moebius_plan_destroy(P); return code; };
 
   // weights: one segment per (layer, matrix) object, chained in the direction-specific order
-  // ("EP->TP adopts the sequential order while TP->EP adopts the reverse order")
+  // ("EP->TP adopts the sequential order while TP->EP adopts the reverse order").
+  // Every EP view starts ep_shift slots (= the largest object) behind its TP view, so an object's
+  // write never lands on its own source nor on the source of an object still to come, and the
+  // regions it does overwrite belong to objects earlier in the chain, which have completed
+  // (each link waits for the previous one, transitively for all of them).
   Chain cw, ck, cs;
   if (R > 1) {
     int prev_ctr = -1; uint32_t prev_units = 0;
-    for (int step = 0; step < 3 * L; ++step) {
-      int k = e2t ? step : 3 * L - 1 - step;
-      int m = k % 3;
+    const int n_links = L * x->n_obj;
+    for (int step = 0; step < n_links; ++step) {
+      const int k = e2t ? step : n_links - 1 - step;
+      const int layer = k / x->n_obj;
+      const WObj& ob = x->obj[k % x->n_obj];
+      const int tp_slot = 3 * layer + ob.slot;
       Seg s = blank_seg();
       s.kind = SEG_XPOSE;
       s.ep_is_src = e2t;
       s.n_groups = R;
       s.rep = 1;
-      int64_t run = (m < 2) ? (int64_t)(c.I / R) * x->wb : (int64_t)(c.I / R) * c.H * x->wb;
-      s.rows_total = (m < 2) ? (uint32_t)(c.E / R) * c.H : (uint32_t)(c.E / R);
+      int64_t run = !ob.long_run ? (int64_t)(c.I / R) * x->wb : (int64_t)(c.I / R) * c.H * x->wb;
+      s.rows_total = !ob.long_run ? (uint32_t)(c.E / R) * c.H : (uint32_t)(c.E / R) * ob.row_mult;
       if (run > (1ll << 31)) return fail(MOEBIUS_E_INVAL);
       s.run_bytes = (uint32_t)run;
-      s.desc_begin = (uint32_t)(k + x->ep_shift);   // EP slot index (tensor-map coordinate)
+      s.desc_begin = (uint32_t)(tp_slot + x->ep_shift);   // EP slot index (tensor-map coordinate)
       const int64_t stage = x->stage_bytes;
       const uint32_t lt_chunk = pick_chunk(run, stage);
-      if (x->use_tma && m < 2 && x->xt_ok) {
+      if (x->use_tma && !ob.long_run && x->xt_ok) {
         // one tensor-map box per unit: xt_rows rows x all R groups
         s.kind = SEG_XPOSE | (PATH_TMA << 8);
         s.groups_per_unit = R;
@@ -613,7 +641,7 @@ extern "C" int moebius_plan(moebius_ctx_t* x, moebius_mode_t from, moebius_mode_
         s.chunks_per_run = 1;
         s.rows_per_unit = (uint32_t)x->xt_rows;
       } else if (x->use_tma && (run > 1024 || run * R > stage) && (lt_chunk == run || lt_chunk >= 4096)) {
-        // one group per unit: plain bulk copies (long runs: the down projection)
+        // one group per unit: plain bulk copies (long runs: the down projection, the W13 stack)
         s.kind = SEG_XPOSE | (PATH_TMA << 8);
         s.groups_per_unit = 1;
         s.chunk_bytes = lt_chunk;
@@ -631,8 +659,8 @@ extern "C" int moebius_plan(moebius_ctx_t* x, moebius_mode_t from, moebius_mode_
         s.rows_per_unit = s.chunks_per_run == 1 ? (uint32_t)std::max<int64_t>(1, unit_bytes / run) : 1;
       }
       s.row_blocks = (s.rows_total + s.rows_per_unit - 1) / s.rows_per_unit;
-      s.tp_off = x->w_off + (int64_t)k * x->S;
-      s.ep_off = x->w_off + (int64_t)(k + x->ep_shift) * x->S;
+      s.tp_off = x->w_off + (int64_t)tp_slot * x->S;
+      s.ep_off = x->w_off + (int64_t)(tp_slot + x->ep_shift) * x->S;
       int64_t nu = (int64_t)R * s.row_blocks * (s.n_groups / s.groups_per_unit) * s.chunks_per_run;
       if (nu > (1ll << 30)) return fail(MOEBIUS_E_INVAL);
       s.n_units = (uint32_t)nu;
@@ -650,7 +678,8 @@ extern "C" int moebius_plan(moebius_ctx_t* x, moebius_mode_t from, moebius_mode_
   // out-of-place 2-D copies with no hazard (reading A13)
   if (c.w_dtype == MOEBIUS_FP8_E4M3_B128 && R > 1) {
     const int HB = c.H / 128, IB = c.I / 128, EL = c.E / R;
-    for (int l = 0; l < L; ++l) for (int m = 0; m < 3; ++m) {
+    for (int l = 0; l < L; ++l) for (int m = 0; m < x->n_obj; ++m) {
+      const WObj& ob = x->obj[m];
       int64_t tp_within = 0, ep_within = 0;
       for (int mm = 0; mm < m; ++mm) { tp_within += x->sg[mm].tp_bytes; ep_within += x->sg[mm].ep_bytes; }
       int prev_hi = 0;
@@ -666,15 +695,16 @@ extern "C" int moebius_plan(moebius_ctx_t* x, moebius_mode_t from, moebius_mode_
           int64_t tp_base = (int64_t)j * x->rank_stride + x->scale_tp_off + l * x->scale_tp_layer + tp_within;
           int64_t ep_base = (int64_t)q * x->rank_stride + x->scale_ep_off + l * x->scale_ep_layer + ep_within;
           int64_t tp_o, ep_o; uint32_t rows, run, tp_st, ep_st;
-          if (m < 2) {   // TP [E, HB, nb] ; EP [EL, HB, IB]; rows = (e', hb)
+          if (!ob.long_run) {   // TP [E, HB, nb] ; EP [EL, HB, IB]; rows = (e', hb)
             rows = (uint32_t)EL * HB; run = (uint32_t)take * 4;
             tp_st = (uint32_t)nb * 4; ep_st = (uint32_t)IB * 4;
             tp_o = tp_base + ((int64_t)q * EL * HB * nb + (a - lo)) * 4;
             ep_o = ep_base + (int64_t)a * 4;
-          } else {       // TP [E, nb, HB] ; EP [EL, IB, HB]; rows = e'
-            rows = (uint32_t)EL; run = (uint32_t)take * HB * 4;
+          } else {       // TP [E, mult*nb, HB] ; EP [EL, mult*IB, HB]; rows = (e', gate|up block)
+            const int mult = ob.row_mult;
+            rows = (uint32_t)EL * mult; run = (uint32_t)take * HB * 4;
             tp_st = (uint32_t)nb * HB * 4; ep_st = (uint32_t)IB * HB * 4;
-            tp_o = tp_base + ((int64_t)q * EL * nb + (a - lo)) * HB * 4;
+            tp_o = tp_base + ((int64_t)q * EL * mult * nb + (a - lo)) * HB * 4;
             ep_o = ep_base + (int64_t)a * HB * 4;
           }
           d.rows = rows; d.run_bytes = run;

@@ -15,11 +15,11 @@ _W_DT = {"bf16": B.MOEBIUS_BF16, "fp32": B.MOEBIUS_FP32, "fp8_e4m3_b128": B.MOEB
 
 def make_config(*, R, L, E, H, I, w_dtype="bf16", kv_heads, head_dim, page_tokens,
                 kv_pool_bytes_per_rank_layer, max_requests, max_pages_per_request,
-                staging_cap_bytes=0, kv_dtype="bf16") -> B.moebius_config_t:
+                staging_cap_bytes=0, kv_dtype="bf16", w_orient=0) -> B.moebius_config_t:
     c = B.moebius_config_t()
     c.R, c.L, c.E, c.H, c.I = R, L, E, H, I
     c.w_dtype = _W_DT[w_dtype]
-    c.w_orient = 0
+    c.w_orient = w_orient
     c.kv_heads, c.head_dim, c.page_tokens = kv_heads, head_dim, page_tokens
     c.kv_dtype = _W_DT[kv_dtype]
     c.kv_pool_bytes_per_rank_layer = int(kv_pool_bytes_per_rank_layer)

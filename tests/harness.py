@@ -28,7 +28,7 @@ def mb_config(cfg: wl.Config, seq_lens, pool_policy=None, staging_cap_frac=0.0, 
     c = mb.make_config(R=cfg.R, L=cfg.L, E=cfg.E, H=cfg.H, I=cfg.I, w_dtype=cfg.w_dtype,
                        kv_heads=cfg.kv_heads, head_dim=cfg.head_dim, page_tokens=cfg.page,
                        kv_pool_bytes_per_rank_layer=pool, max_requests=max_requests or max(n, 1),
-                       max_pages_per_request=mp, staging_cap_bytes=0)
+                       max_pages_per_request=mp, staging_cap_bytes=0, w_orient=cfg.w_orient)
     if staging_cap_frac:
         s = mb.Session(c)
         c.staging_cap_bytes = int(staging_cap_frac * s.layout.resident_bytes)

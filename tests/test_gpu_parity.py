@@ -235,3 +235,47 @@ def test_state_errors():
         sess.reshard(plan)
     assert e.value.status == -4
     sess.close()
+
+
+# ---- the paper's own weight orientation (w_orient = 1) and odd shapes ----------------
+
+@pytest.mark.parametrize("tma", [0, 1])
+def test_paper_orientation_small_config(tma):
+    """Config 2 shapes with W13 [E,2I,H] / W2 [E,H,I]: chain objects of 2 slots + 1 slot per layer."""
+    cfg = wl.get_config("small").with_(w_orient=1)
+    st, sess = gpu_session(cfg, tma=(tma, 0, 0))
+    owner, bt, _ = start(st, sess, TP, "random")
+    mode, owner, bt, _ = gpu_switch(st, sess, TP, owner, bt)
+    gpu_switch(st, sess, mode, owner, bt)
+    sess.close()
+
+
+@pytest.mark.parametrize("first", [TP, EP])
+def test_paper_orientation_tiny_and_fp8(first):
+    st, sess = gpu_session(wl.get_config("tiny").with_(w_orient=1), initial_mode=first)
+    owner, bt, _ = start(st, sess, first, "random")
+    mode, owner, bt, _ = gpu_switch(st, sess, first, owner, bt)
+    gpu_switch(st, sess, mode, owner, bt)
+    sess.close()
+    cfg = wl.get_config("fp8_graph").with_(L=2, E=8, H=256, I=1536, n_req=6, len_dist=("uniform", 1, 60), seed=3,
+                                           w_orient=1)
+    st, sess = gpu_session(cfg, fill="normal", initial_mode=first)
+    owner, bt, _ = start(st, sess, first, "random")
+    mode, owner, bt, _ = gpu_switch(st, sess, first, owner, bt)
+    gpu_switch(st, sess, mode, owner, bt)
+    sess.close()
+
+
+@pytest.mark.parametrize("orient", [0, 1])
+@pytest.mark.parametrize("R,E,H,I,Hkv", [(3, 6, 40, 72, 3), (6, 12, 24, 48, 2), (5, 10, 56, 40, 5)])
+def test_non_power_of_two_shapes(orient, R, E, H, I, Hkv):
+    """Shifted slots move every object out of place: odd rank counts and shapes need nothing special
+    (as an in-place transposition they would give very long cycles)."""
+    cfg = wl.get_config("tiny").with_(R=R, L=2, E=E, H=H, I=I, kv_heads=Hkv, head_dim=24, n_req=9,
+                                      len_dist=("uniform", 1, 90), seed=31 + R, w_orient=orient)
+    st, sess = gpu_session(cfg)
+    owner, bt, _ = start(st, sess, TP, "random")
+    mode, owner, bt, _ = gpu_switch(st, sess, TP, owner, bt)
+    mode, owner, bt, _ = gpu_switch(st, sess, mode, owner, bt)
+    assert mode == TP
+    sess.close()

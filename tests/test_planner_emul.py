@@ -235,3 +235,73 @@ def test_chain_cut_levels(first, max_level):
         assert stats["n_kv_rounds"] > 8          # the uncut chains are long here
     run_switch(st, sess, image, staging, mode, owner, bt)
     sess.close()
+
+
+# ---- the paper's own weight orientation (w_orient = 1) and odd shapes ----------------
+
+@pytest.mark.parametrize("src", ["canonical", "random"])
+def test_paper_orientation_tiny_round_trip(src):
+    """W13 [E,2I,H] / W2 [E,H,I]: two chain objects of different size per layer (2 slots + 1 slot),
+    EP views shifted by the larger one.  TP -> EP -> TP, every view bit-exact after each switch."""
+    st, sess, image, staging = make(wl.get_config("tiny").with_(w_orient=1))
+    assert sess.layout.weight_spare_bytes == 2 * sess.layout.weight_slot_bytes * st.cfg.R
+    owner, bt = source_tables(st, sess, TP, src)
+    OracleLayout(st, sess, TP, owner, bt).place(image)
+    mode, owner, bt, s1 = run_switch(st, sess, image, staging, TP, owner, bt)
+    mode, owner, bt, s2 = run_switch(st, sess, image, staging, EP, owner, bt)
+    assert mode == TP and s1["w_moved"] == s2["w_moved"] == 49152
+
+
+@pytest.mark.parametrize("first", [TP, EP])
+def test_paper_orientation_smallish_alternating(first):
+    st, sess, image, staging = make(SMALLISH.with_(w_orient=1))
+    mode = first
+    owner, bt = source_tables(st, sess, mode, "random")
+    OracleLayout(st, sess, mode, owner, bt).place(image)
+    for _ in range(3):
+        mode, owner, bt, stats = run_switch(st, sess, image, staging, mode, owner, bt)
+
+
+def test_paper_orientation_fp8_scales():
+    cfg = wl.get_config("fp8_graph").with_(L=2, E=8, H=256, I=1536, n_req=6, len_dist=("uniform", 1, 60), seed=3,
+                                           w_orient=1)
+    st, sess, image, staging = make(cfg)
+    st.fill = "normal"
+    owner, bt = source_tables(st, sess, TP, "random")
+    OracleLayout(st, sess, TP, owner, bt).place(image)
+    mode, owner, bt, s = run_switch(st, sess, image, staging, TP, owner, bt)
+    mode, owner, bt, s = run_switch(st, sess, image, staging, EP, owner, bt)
+
+
+def test_paper_orientation_view_ids():
+    """Tensor ids are per orientation: gate/up/down ids are invalid under w_orient = 1 and vice versa."""
+    cfg = wl.get_config("tiny")
+    lens = np.array([5], np.int32)
+    s0 = mb.Session(mb_config(cfg, lens))
+    s1 = mb.Session(mb_config(cfg.with_(w_orient=1), lens))
+    for t in (mb.T_W13, mb.T_W2):
+        with pytest.raises(mb.MoebiusError):
+            s0.view_desc(TP, 0, 0, t)
+    for t in (mb.T_GATE, mb.T_UP, mb.T_DOWN):
+        with pytest.raises(mb.MoebiusError):
+            s1.view_desc(TP, 0, 0, t)
+    v = s1.view_desc(TP, 1, 0, mb.T_W13)
+    assert tuple(v.shape[:3]) == (cfg.E, 2 * cfg.I // cfg.R, cfg.H)
+    v = s1.view_desc(EP, 1, 0, mb.T_W2)
+    assert tuple(v.shape[:3]) == (cfg.E // cfg.R, cfg.H, cfg.I)
+
+
+@pytest.mark.parametrize("orient", [0, 1])
+@pytest.mark.parametrize("R,E,H,I,Hkv", [(3, 6, 40, 72, 3), (6, 12, 24, 48, 2), (5, 10, 56, 40, 5)])
+def test_non_power_of_two_shapes(orient, R, E, H, I, Hkv):
+    """as an in-place transposition, non-power-of-two shapes give very long cycles; with
+    shifted slots every object moves out of place, so nothing about the shape matters beyond reading
+    A3 (E % R == 0, I % R == 0, 16-byte runs)."""
+    cfg = wl.get_config("tiny").with_(R=R, L=2, E=E, H=H, I=I, kv_heads=Hkv, head_dim=24, n_req=9,
+                                      len_dist=("uniform", 1, 90), seed=31 + R, w_orient=orient)
+    st, sess, image, staging = make(cfg)
+    owner, bt = source_tables(st, sess, TP, "random")
+    OracleLayout(st, sess, TP, owner, bt).place(image)
+    mode, owner, bt, _ = run_switch(st, sess, image, staging, TP, owner, bt)
+    mode, owner, bt, _ = run_switch(st, sess, image, staging, EP, owner, bt)
+    assert mode == TP
