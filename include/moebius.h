@@ -194,6 +194,21 @@ MOEBIUS_API int moebius_plan_export(const moebius_plan_t* plan, int what, void* 
  * the bound buffers while it runs. */
 MOEBIUS_API int moebius_reshard(moebius_ctx_t* ctx, const moebius_plan_t* plan, void* cuda_stream);
 
+/* The same switch as a PLAN-INDEPENDENT sequence, for callers that keep the switch itself inside a
+ * captured CUDA graph (PAPER.md:197-201 keeps everything round the switch in
+ * graphs).  moebius_stage_plan (host only, plus one pinned allocation on its first call) copies the
+ * plan's work list and tables into a pinned mailbox at a fixed host address, checks plan.from against
+ * the active mode and makes plan.to the active mode.  moebius_reshard_staged enqueues: counters := 0,
+ * mailbox -> dev_desc (fixed size: the whole descriptor capacity), the kernel with a fixed full grid
+ * and arguments that do not depend on the plan (the kernel reads segment/unit counts from the
+ * uploaded header), mailbox tables -> dev_tables (fixed size).  It may be called under stream
+ * capture; each replay of the captured graph executes whatever plan was staged last.  Exactly one
+ * execution must follow each moebius_stage_plan, and the next plan may be staged only after that
+ * execution's uploads have completed (synchronise the stream or an event recorded after it).
+ * MOEBIUS_E_STATE: nothing staged yet / wrong active mode. */
+MOEBIUS_API int moebius_stage_plan(moebius_ctx_t* ctx, const moebius_plan_t* plan);
+MOEBIUS_API int moebius_reshard_staged(moebius_ctx_t* ctx, void* cuda_stream);
+
 /* Kernel-only device time of the last moebius_reshard, in ms (CUDA events on its stream; the call
  * synchronises on the end event).  Enabled with moebius_set_timing(ctx, 1). */
 MOEBIUS_API int moebius_set_timing(moebius_ctx_t* ctx, int enable);

@@ -12,7 +12,7 @@ from ._binding import (  # noqa: F401
     MoebiusError, moebius_config_t, moebius_layout_t, moebius_view_t, moebius_stats_t,
     moebius_create, moebius_destroy, moebius_layout, moebius_view, moebius_bind, moebius_active_mode,
     moebius_plan, moebius_plan_destroy, moebius_block_tables, moebius_plan_stats, moebius_plan_export,
-    moebius_reshard, moebius_set_timing, moebius_last_kernel_ms, moebius_kernel_ms_history, moebius_set_launch, moebius_set_tma, moebius_set_kv_rounds,
+    moebius_reshard, moebius_stage_plan, moebius_reshard_staged, moebius_set_timing, moebius_last_kernel_ms, moebius_kernel_ms_history, moebius_set_launch, moebius_set_tma, moebius_set_kv_rounds,
     moebius_status_str, moebius_version, lib_path, EXPORTED_SYMBOLS, SEG_DTYPE, KV_DTYPE, C2D_DTYPE,
 )
 from .session import Session, make_config  # noqa: F401

@@ -17,7 +17,8 @@ T_W13, T_W2, T_W13_SCALE, T_W2_SCALE = range(8, 12)   # w_orient = 1 (PAPER.md:1
 EXPORTED_SYMBOLS = [
     "moebius_create", "moebius_destroy", "moebius_layout", "moebius_view", "moebius_bind",
     "moebius_active_mode", "moebius_plan", "moebius_plan_destroy", "moebius_block_tables",
-    "moebius_plan_stats", "moebius_plan_export", "moebius_reshard", "moebius_set_timing",
+    "moebius_plan_stats", "moebius_plan_export", "moebius_reshard", "moebius_stage_plan", "moebius_reshard_staged",
+    "moebius_set_timing",
     "moebius_last_kernel_ms", "moebius_kernel_ms_history", "moebius_set_launch", "moebius_set_tma", "moebius_set_kv_rounds", "moebius_status_str", "moebius_version",
 ]
 
@@ -104,6 +105,8 @@ _lib.moebius_block_tables.argtypes = [_vp, _vp, _vp]
 _lib.moebius_plan_stats.argtypes = [_vp, C.POINTER(moebius_stats_t)]
 _lib.moebius_plan_export.argtypes = [_vp, C.c_int, _vp, C.c_int64, C.POINTER(C.c_int64)]
 _lib.moebius_reshard.argtypes = [_vp, _vp, _vp]
+_lib.moebius_stage_plan.argtypes = [_vp, _vp]
+_lib.moebius_reshard_staged.argtypes = [_vp, _vp]
 _lib.moebius_set_timing.argtypes = [_vp, C.c_int]
 _lib.moebius_last_kernel_ms.argtypes = [_vp, C.POINTER(C.c_float)]
 _lib.moebius_kernel_ms_history.argtypes = [_vp, C.POINTER(C.c_float), C.c_int, C.POINTER(C.c_int)]
@@ -216,6 +219,14 @@ def moebius_plan_export(plan, what: int) -> np.ndarray:
 
 def moebius_reshard(ctx, plan, cuda_stream: int = 0):
     _chk(_lib.moebius_reshard(ctx, plan, _vp(cuda_stream or None)), "moebius_reshard")
+
+
+def moebius_stage_plan(ctx, plan):
+    _chk(_lib.moebius_stage_plan(ctx, plan), "moebius_stage_plan")
+
+
+def moebius_reshard_staged(ctx, cuda_stream: int = 0):
+    _chk(_lib.moebius_reshard_staged(ctx, _vp(cuda_stream or None)), "moebius_reshard_staged")
 
 
 def moebius_set_timing(ctx, enable: bool):

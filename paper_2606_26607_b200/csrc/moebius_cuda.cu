@@ -312,9 +312,20 @@ __device__ __forceinline__ void lsu_unit(const Seg& s, const DevParams& p, uint3
 // dependency counter it drains its own pipeline, so waits can never be circular.
 template <int kMinCtasPerSm>   // 1: plans with PATH_TMA segments (shared-memory bound); 2: ld/st-only plans
 __global__ void __launch_bounds__(256, kMinCtasPerSm)
-moebius_reshard_kernel(const __grid_constant__ DevParams p, const __grid_constant__ CUtensorMap tm_w,
+moebius_reshard_kernel(const __grid_constant__ DevParams p_in, const __grid_constant__ CUtensorMap tm_w,
                        const __grid_constant__ CUtensorMap tm_kv) {
   extern __shared__ __align__(1024) char smem[];
+  // The arguments are the same for every switch of a context (so that the launch can be replayed
+  // from a captured graph); what differs per plan is read from the uploaded image's header.
+  DevParams p = p_in;
+  {
+    const uint4 h = __ldg((const uint4*)p_in.hdr);
+    p.n_segs = h.x;
+    p.total_units = h.y;
+    p.segs = (const Seg*)((const char*)p_in.hdr + sizeof(PlanHdr));
+    p.kv = (const KvDesc*)((const char*)p_in.hdr + h.z);
+    p.c2d = (const C2dDesc*)((const char*)p_in.hdr + h.w);
+  }
   const uint32_t lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   uint64_t* bar = (uint64_t*)smem + 2 * warp;                       // 2 barriers per pipe
   char* ring = smem + 1024 + (size_t)warp * 2 * p.stage_bytes;     // 2 stages per pipe
@@ -521,6 +532,7 @@ static int encode_tmaps(moebius_ctx* x) {
 void cuda_ctx_destroy(moebius_ctx* x) {
   for (const ImageBuf& b : x->image_pool) image_free(b);
   x->image_pool.clear();
+  if (x->mailbox) { cudaFreeHost(x->mailbox); x->mailbox = nullptr; }
   if (x->ev_valid) {
     for (int i = 0; i < 2 * kTimingRing; ++i) cudaEventDestroy((cudaEvent_t)x->ev[i]);
     x->ev_valid = false;
@@ -576,16 +588,69 @@ extern "C" int moebius_last_kernel_ms(moebius_ctx_t* x, float* ms) {
   return moebius_kernel_ms_history(x, ms, 1, &n);
 }
 
-extern "C" int moebius_reshard(moebius_ctx_t* x, const moebius_plan_t* P, void* cuda_stream) {
-  if (!x || !P || P->ctx != x) return MOEBIUS_E_INVAL;
-  if (!x->bound || x->active_mode != P->from) return MOEBIUS_E_STATE;
-  cudaStream_t st = (cudaStream_t)cuda_stream;
+namespace {
+
+int ensure_device_facts(moebius_ctx* x) {
   if (x->n_sm == 0) {
     int dev = 0, n = 0;
     if (cudaGetDevice(&dev) != cudaSuccess) return MOEBIUS_E_CUDA;
     if (cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || n <= 0) return MOEBIUS_E_CUDA;
     x->n_sm = n;
   }
+  return MOEBIUS_OK;
+}
+
+// Launches the reshard kernel over the image that sits at dev_desc + kSegOff.  `tma`: the variant with
+// the pipes' shared-memory rings (it also executes PATH_LSU segments).  `unit_hint` > 0 caps the grid
+// for small plans; 0 = the full persistent grid (plan-independent: what a captured graph needs).
+int launch_reshard_kernel(moebius_ctx* x, bool tma, int64_t unit_hint, cudaStream_t st) {
+  DevParams p;
+  memset(&p, 0, sizeof(p));
+  p.base = x->base;
+  p.stg = x->stg;
+  p.hdr = (const PlanHdr*)(x->desc + kSegOff);
+  p.ticket = (uint32_t*)x->desc;
+  p.counters = (uint32_t*)(x->desc + kCtrOff);
+  p.rank_stride = x->rank_stride;
+  p.page_tokens = (uint32_t)x->cfg.page_tokens;
+  int threads, per_sm;
+  size_t smem = 0;
+  if (tma) {
+    // one CTA per SM, n_pipes warps, each with two private stages
+    if (!x->tmaps_valid) { int rc = encode_tmaps(x); if (rc != MOEBIUS_OK) return rc; }
+    p.stage_bytes = (uint32_t)x->stage_bytes;
+    p.xt_rows = (uint32_t)x->xt_rows;
+    threads = 32 * x->n_pipes;
+    per_sm = 1;
+    smem = 1024 + (size_t)x->n_pipes * 2 * (size_t)x->stage_bytes;
+    if (smem != x->smem_set) {
+      if (cudaFuncSetAttribute(moebius_reshard_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess)
+        return MOEBIUS_E_CUDA;
+      x->smem_set = smem;
+    }
+  } else {
+    threads = x->threads > 0 ? x->threads : 256;
+    per_sm = x->ctas_per_sm > 0 ? x->ctas_per_sm : 2;
+  }
+  int64_t grid = (int64_t)x->n_sm * per_sm;
+  if (unit_hint > 0) {
+    int64_t grid_cap = (unit_hint + threads / 32 - 1) / (threads / 32);
+    if (grid > grid_cap) grid = grid_cap;
+  }
+  if (tma)
+    moebius_reshard_kernel<1><<<(unsigned)grid, threads, smem, st>>>(p, *(const CUtensorMap*)x->tmap_w, *(const CUtensorMap*)x->tmap_kv);
+  else
+    moebius_reshard_kernel<2><<<(unsigned)grid, threads, 0, st>>>(p, *(const CUtensorMap*)x->tmap_w, *(const CUtensorMap*)x->tmap_kv);
+  return cudaGetLastError() == cudaSuccess ? MOEBIUS_OK : MOEBIUS_E_CUDA;
+}
+
+}  // namespace
+
+extern "C" int moebius_reshard(moebius_ctx_t* x, const moebius_plan_t* P, void* cuda_stream) {
+  if (!x || !P || P->ctx != x) return MOEBIUS_E_INVAL;
+  if (!x->bound || x->active_mode != P->from) return MOEBIUS_E_STATE;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  if (int rc = ensure_device_facts(x)) return rc;
   if (x->timing && !x->ev_valid) {
     for (int i = 0; i < 2 * kTimingRing; ++i) {
       cudaEvent_t e;
@@ -599,67 +664,63 @@ extern "C" int moebius_reshard(moebius_ctx_t* x, const moebius_plan_t* P, void* 
     int64_t k = x->ev_count % kTimingRing;
     ev_a = (cudaEvent_t)x->ev[2 * k]; ev_b = (cudaEvent_t)x->ev[2 * k + 1];
   }
+  if (P->uses_tma && (P->stage_bytes != x->stage_bytes || P->xt_rows != x->xt_rows)) return MOEBIUS_E_STATE;  // set_tma after plan
   // 1. work list -> device; ticket and the counters this plan uses -> 0
   if (cudaMemsetAsync(x->desc, 0, (size_t)(kCtrOff + 4 * (int64_t)(P->n_counters ? P->n_counters : 1)), st) != cudaSuccess)
     return MOEBIUS_E_CUDA;
-  if (P->image_bytes &&
-      cudaMemcpyAsync(x->desc + kSegOff, P->image, (size_t)P->image_bytes, cudaMemcpyHostToDevice, st) != cudaSuccess)
+  if (cudaMemcpyAsync(x->desc + kSegOff, P->image, (size_t)P->image_bytes, cudaMemcpyHostToDevice, st) != cudaSuccess)
     return MOEBIUS_E_CUDA;
   // 2. the kernel
+  if (x->timing) cudaEventRecord(ev_a, st);
   if (P->total_units) {
-    DevParams p;
-    memset(&p, 0, sizeof(p));
-    p.base = x->base;
-    p.stg = x->stg;
-    p.segs = (const Seg*)(x->desc + kSegOff);
-    p.kv = (const KvDesc*)(x->desc + kSegOff + P->kv_img_off);
-    p.c2d = (const C2dDesc*)(x->desc + kSegOff + P->c2d_img_off);
-    p.ticket = (uint32_t*)x->desc;
-    p.counters = (uint32_t*)(x->desc + kCtrOff);
-    p.rank_stride = x->rank_stride;
-    p.n_segs = (uint32_t)P->segs.size();
-    p.total_units = P->total_units;
-    p.page_tokens = (uint32_t)x->cfg.page_tokens;
-    int threads, per_sm;
-    size_t smem = 0;
-    if (P->uses_tma) {
-      // one CTA per SM, n_pipes warps, each with two private stages
-      if (P->stage_bytes != x->stage_bytes || P->xt_rows != x->xt_rows) return MOEBIUS_E_STATE;  // set_tma after plan
-      if (!x->tmaps_valid) { int rc = encode_tmaps(x); if (rc != MOEBIUS_OK) return rc; }
-      p.stage_bytes = (uint32_t)x->stage_bytes;
-      p.xt_rows = (uint32_t)x->xt_rows;
-      threads = 32 * x->n_pipes;
-      per_sm = 1;
-      smem = 1024 + (size_t)x->n_pipes * 2 * (size_t)x->stage_bytes;
-      if (smem != x->smem_set) {
-        if (cudaFuncSetAttribute(moebius_reshard_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess)
-          return MOEBIUS_E_CUDA;
-        x->smem_set = smem;
-      }
-    } else {
-      threads = x->threads > 0 ? x->threads : 256;
-      per_sm = x->ctas_per_sm > 0 ? x->ctas_per_sm : 2;
-    }
-    int64_t grid = (int64_t)x->n_sm * per_sm;
-    int64_t grid_cap = ((int64_t)P->total_units + threads / 32 - 1) / (threads / 32);
-    if (grid > grid_cap) grid = grid_cap;
-    if (x->timing) cudaEventRecord(ev_a, st);
-    if (P->uses_tma)
-      moebius_reshard_kernel<1><<<(unsigned)grid, threads, smem, st>>>(p, *(const CUtensorMap*)x->tmap_w, *(const CUtensorMap*)x->tmap_kv);
-    else
-      moebius_reshard_kernel<2><<<(unsigned)grid, threads, 0, st>>>(p, *(const CUtensorMap*)x->tmap_w, *(const CUtensorMap*)x->tmap_kv);
-    if (cudaGetLastError() != cudaSuccess) return MOEBIUS_E_CUDA;
-    if (x->timing) cudaEventRecord(ev_b, st);
-  } else if (x->timing) {
-    cudaEventRecord(ev_a, st);
-    cudaEventRecord(ev_b, st);
+    if (int rc = launch_reshard_kernel(x, P->uses_tma, (int64_t)P->total_units, st)) return rc;
   }
-  if (x->timing) x->ev_count++;
+  if (x->timing) { cudaEventRecord(ev_b, st); x->ev_count++; }
   // 3. publish: new tables, owner vector and the active-mode flag at their fixed address
   if (cudaMemcpyAsync(x->tables, P->tbl_image, (size_t)P->tbl_bytes, cudaMemcpyHostToDevice, st) != cudaSuccess)
     return MOEBIUS_E_CUDA;
   if (P->buf.ev && cudaEventRecord((cudaEvent_t)P->buf.ev, st) != cudaSuccess) return MOEBIUS_E_CUDA;
   x->active_mode = P->to;
   x->switch_count++;
+  return MOEBIUS_OK;
+}
+
+// ---- the switch as a graph-capturable, plan-independent sequence ------------------------------------
+extern "C" int moebius_stage_plan(moebius_ctx_t* x, const moebius_plan_t* P) {
+  if (!x || !P || P->ctx != x) return MOEBIUS_E_INVAL;
+  if (!x->bound || x->active_mode != P->from) return MOEBIUS_E_STATE;
+  if (P->uses_tma && (P->stage_bytes != x->stage_bytes || P->xt_rows != x->xt_rows)) return MOEBIUS_E_STATE;
+  const int64_t img_cap = x->desc_bytes - kSegOff;
+  if (P->image_bytes > img_cap || P->tbl_bytes > x->table_bytes) return MOEBIUS_E_INVAL;
+  if (!x->mailbox) {
+    void* m = nullptr;
+    if (cudaHostAlloc(&m, (size_t)(img_cap + x->table_bytes), cudaHostAllocDefault) != cudaSuccess) {
+      cudaGetLastError();
+      return MOEBIUS_E_CUDA;
+    }
+    memset(m, 0, (size_t)(img_cap + x->table_bytes));
+    x->mailbox = (char*)m;
+  }
+  memcpy(x->mailbox, P->image, (size_t)P->image_bytes);
+  memcpy(x->mailbox + img_cap, P->tbl_image, (size_t)P->tbl_bytes);
+  x->active_mode = P->to;
+  x->switch_count++;
+  return MOEBIUS_OK;
+}
+
+extern "C" int moebius_reshard_staged(moebius_ctx_t* x, void* cuda_stream) {
+  if (!x) return MOEBIUS_E_INVAL;
+  if (!x->bound || !x->mailbox) return MOEBIUS_E_STATE;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  if (int rc = ensure_device_facts(x)) return rc;
+  const int64_t img_cap = x->desc_bytes - kSegOff;
+  // every size, address and launch dimension below is the same for every plan of this context
+  if (cudaMemsetAsync(x->desc, 0, (size_t)kSegOff, st) != cudaSuccess) return MOEBIUS_E_CUDA;
+  if (cudaMemcpyAsync(x->desc + kSegOff, x->mailbox, (size_t)img_cap, cudaMemcpyHostToDevice, st) != cudaSuccess)
+    return MOEBIUS_E_CUDA;
+  const bool tma = x->use_tma && (x->xt_ok || x->kt_ok);
+  if (int rc = launch_reshard_kernel(x, tma, 0, st)) return rc;
+  if (cudaMemcpyAsync(x->tables, x->mailbox + img_cap, (size_t)x->table_bytes, cudaMemcpyHostToDevice, st) != cudaSuccess)
+    return MOEBIUS_E_CUDA;
   return MOEBIUS_OK;
 }

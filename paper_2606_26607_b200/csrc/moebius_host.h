@@ -110,6 +110,8 @@ struct moebius_ctx {
   std::vector<moebius::ImageBuf> image_pool;
   moebius::PlanScratch scratch;
   int has_device;                       // -1 unknown, 0 no CUDA device (host-only planner), 1 yes
+  char* mailbox;                        // pinned, fixed address: [work-list image capacity][tables]; what
+                                        // moebius_reshard_staged uploads (allocated by the first moebius_stage_plan)
 };
 
 struct moebius_plan {

@@ -145,7 +145,7 @@ int moebius_create(const moebius_config_t* c, moebius_ctx_t** out) {
   live_max = std::min<int64_t>(live_max, (int64_t)c->max_requests * c->max_pages_per_request);
   x->max_kv_desc = live_max;
   x->max_c2d = c->w_dtype == MOEBIUS_FP8_E4M3_B128 ? (int64_t)x->n_obj * L * R * R : 0;
-  x->desc_bytes = align_up(kSegOff + (int64_t)kMaxSegs * sizeof(Seg) + x->max_kv_desc * sizeof(KvDesc) +
+  x->desc_bytes = align_up(kSegOff + (int64_t)sizeof(PlanHdr) + (int64_t)kMaxSegs * sizeof(Seg) + x->max_kv_desc * sizeof(KvDesc) +
                                x->max_c2d * sizeof(C2dDesc) + 1024, 4096);
   x->table_bytes = align_up(4 * ((int64_t)kTblHdrInts + 2 * (int64_t)c->max_requests +
                                  (int64_t)c->max_requests * c->max_pages_per_request), 256);
@@ -170,6 +170,7 @@ int moebius_create(const moebius_config_t* c, moebius_ctx_t** out) {
   x->ev_count = 0;
   x->ev_valid = false;
   x->has_device = -1;
+  x->mailbox = nullptr;
   *out = x;
   return MOEBIUS_OK;
 }
@@ -849,15 +850,24 @@ extern "C" int moebius_plan(moebius_ctx_t* x, moebius_mode_t from, moebius_mode_
   int64_t seg_b = align_up((int64_t)P->segs.size() * sizeof(Seg), 256);
   int64_t kv_b = align_up((int64_t)nm * sizeof(KvDesc), 256);
   int64_t c2d_b = align_up((int64_t)P->c2d.size() * sizeof(C2dDesc), 256);
-  P->kv_img_off = seg_b;
-  P->c2d_img_off = seg_b + kv_b;
-  P->image_bytes = seg_b + kv_b + c2d_b;
+  const int64_t hdr_b = sizeof(PlanHdr);
+  P->kv_img_off = hdr_b + seg_b;
+  P->c2d_img_off = hdr_b + seg_b + kv_b;
+  P->image_bytes = hdr_b + seg_b + kv_b + c2d_b;
   P->tbl_bytes = 4 * ((int64_t)kTblHdrInts + 2 * (int64_t)c.max_requests + (int64_t)n_req * MP);
   if (!image_acquire(x, P->image_bytes + P->tbl_bytes + 256, &P->buf)) return fail(MOEBIUS_E_INVAL);
   P->image = P->buf.p;
+  {
+    PlanHdr* h = (PlanHdr*)P->image;
+    memset(h, 0, sizeof(PlanHdr));
+    h->n_segs = (uint32_t)P->segs.size();
+    h->total_units = P->total_units;
+    h->kv_off = (uint32_t)P->kv_img_off;
+    h->c2d_off = (uint32_t)P->c2d_img_off;
+  }
   if (!P->segs.empty()) {
-    memcpy(P->image, P->segs.data(), P->segs.size() * sizeof(Seg));
-    memset(P->image + P->segs.size() * sizeof(Seg), 0, (size_t)(seg_b - (int64_t)(P->segs.size() * sizeof(Seg))));
+    memcpy(P->image + hdr_b, P->segs.data(), P->segs.size() * sizeof(Seg));
+    memset(P->image + hdr_b + P->segs.size() * sizeof(Seg), 0, (size_t)(seg_b - (int64_t)(P->segs.size() * sizeof(Seg))));
   }
   {  // KV descriptors ordered [level 0][level 1]...[level K][staged]
     KvDesc* kvd = (KvDesc*)(P->image + P->kv_img_off);

@@ -88,9 +88,22 @@ struct C2dDesc {          // 32 bytes: rows x run_bytes, 4-byte elements, offset
 };
 static_assert(sizeof(C2dDesc) == 32, "C2dDesc must be 32 bytes");
 
-struct DevParams {        // kernel arguments
+// First 256 bytes of the uploaded work-list image.  Everything that differs from plan to plan is
+// read by the kernel from here, so the kernel's ARGUMENTS are the same for every switch of a
+// context and the launch can sit in a captured CUDA graph (moebius_reshard_staged).
+struct PlanHdr {
+  uint32_t n_segs;
+  uint32_t total_units;
+  uint32_t kv_off;        // byte offsets from the start of the image
+  uint32_t c2d_off;
+  uint32_t pad_[60];
+};
+static_assert(sizeof(PlanHdr) == 256, "PlanHdr must be 256 bytes");
+
+struct DevParams {        // decoded launch state (the kernel fills the plan-dependent fields from PlanHdr)
   char*            base;
   char*            stg;
+  const PlanHdr*   hdr;           // the uploaded image; segs/kv/c2d/n_segs/total_units below come from it
   const Seg*       segs;
   const KvDesc* kv;
   const C2dDesc*   c2d;

@@ -101,6 +101,16 @@ class Session:
         s = torch.cuda.current_stream(self.device) if stream is None else stream
         B.moebius_reshard(self.ctx, plan, s.cuda_stream)
 
+    def stage(self, plan):
+        """Copies the plan into the fixed pinned mailbox (host side of a graph-captured switch)."""
+        B.moebius_stage_plan(self.ctx, plan)
+
+    def reshard_staged(self, stream=None):
+        """Plan-independent enqueue of the staged switch; legal under CUDA-graph capture."""
+        import torch
+        s = torch.cuda.current_stream(self.device) if stream is None else stream
+        B.moebius_reshard_staged(self.ctx, s.cuda_stream)
+
     def free_plan(self, plan):
         self._plans = [p for p in self._plans if p.value != plan.value]
         B.moebius_plan_destroy(plan)

@@ -122,3 +122,49 @@ def test_fp8_graph_stress_reduced():
 def test_bf16_graph_replay_from_ep():
     cfg = wl.get_config("small").with_(L=2, H=128, I=256, n_req=12, len_dist=("uniform", 1, 150), seed=21)
     run_graph_stress(cfg, 4, first=EP)
+
+
+def test_switch_itself_inside_a_captured_graph():
+    """the switch launch captured ONCE in a CUDA graph (moebius_reshard_staged:
+    fixed grid, fixed copy sizes, plan-dependent counts read from the uploaded header) and replayed
+    for six plans -- both directions, the first from random tables in a tight pool (dependency rounds +
+    staging): the plans differ in segment count, unit count and descriptor offsets.  The reader graph of the new mode is
+    replayed after each and compared with the oracle."""
+    cfg = wl.get_config("small").with_(L=2, H=128, I=256, n_req=30, len_dist=("uniform", 1, 200), seed=23)
+    st = State(cfg, fill="tag")
+    sess = mb.Session(mb_config(cfg, st.lens, "tight", 0.5), device="cuda:0", initial_mode=TP)
+    n = len(st.lens)
+    readers = {m: ModeGraph(sess, cfg, m, n, False) for m in (TP, EP)}
+    owner, bt = source_tables(st, sess, TP, "random")
+    image = np.full(sess.layout.base_bytes, 0xA5, np.uint8)
+    OracleLayout(st, sess, TP, owner, bt).place(image)
+    sess.base[:image.size].copy_(torch.from_numpy(image))
+    # stage the first plan, warm the launch up once outside capture, then capture
+    mode = TP
+    plan = sess.plan(EP, st.lens, owner, bt, from_mode=mode)
+    first_stats = mb.moebius_plan_stats(plan).as_dict()
+    sess.stage(plan)
+    with pytest.raises(mb.MoebiusError):          # staging made EP the active mode: the same plan no longer applies
+        sess.stage(plan)
+    switch_graph = torch.cuda.CUDAGraph()
+    torch.cuda.synchronize()
+    with torch.cuda.graph(switch_graph):
+        sess.reshard_staged(torch.cuda.current_stream())
+    seen = set()
+    for k in range(6):
+        to = EP if mode == TP else TP
+        if k > 0:
+            plan = sess.plan(to, st.lens, owner, bt, from_mode=mode)
+            sess.stage(plan)
+        s = mb.moebius_plan_stats(plan).as_dict()
+        seen.add((s["n_segments"], s["n_units"]))
+        switch_graph.replay()
+        readers[to].replay()
+        want_owner, want_bt = expected_target(st, sess, to)
+        readers[to].check(st, want_owner, want_bt)
+        torch.cuda.synchronize()                  # uploads of this replay are done: the next plan may be staged
+        sess.free_plan(plan)
+        owner, bt, mode = (want_owner if to == EP else None), want_bt, to
+    assert first_stats["n_kv_rounds"] > 1         # the first plan really needed rounds
+    assert len(seen) >= 2                          # the replays executed plans of different size
+    sess.close()
