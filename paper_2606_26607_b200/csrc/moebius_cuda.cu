@@ -436,24 +436,7 @@ moebius_reshard_kernel(const __grid_constant__ DevParams p_in, const __grid_cons
 // Upload images.  A plan's image is read by the async H2D copies of moebius_reshard, so a buffer that
 // goes back to the pool keeps the event recorded after its last upload; the next plan that takes the
 // buffer waits on that event before overwriting it.
-bool image_acquire(moebius_ctx* x, int64_t bytes, ImageBuf* out) {
-  size_t best = x->image_pool.size();
-  for (size_t i = 0; i < x->image_pool.size(); ++i)
-    if (x->image_pool[i].bytes >= bytes && (best == x->image_pool.size() || x->image_pool[i].bytes < x->image_pool[best].bytes))
-      best = i;
-  if (best < x->image_pool.size()) {
-    *out = x->image_pool[best];
-    x->image_pool.erase(x->image_pool.begin() + (long)best);
-    if (out->ev && cudaEventSynchronize((cudaEvent_t)out->ev) != cudaSuccess) cudaGetLastError();
-    return true;
-  }
-  if (x->has_device < 0) {
-    int ndev = 0;
-    x->has_device = (cudaGetDeviceCount(&ndev) == cudaSuccess && ndev > 0) ? 1 : 0;
-    cudaGetLastError();
-  }
-  // round up so that plans of slightly different sizes share buffers
-  int64_t cap = (bytes + (1 << 20) - 1) >> 20 << 20;
+static bool image_fresh(moebius_ctx* x, int64_t cap, ImageBuf* out) {
   out->p = nullptr; out->bytes = cap; out->pinned = false; out->ev = nullptr;
   if (x->has_device) {
     void* p = nullptr;
@@ -467,6 +450,44 @@ bool image_acquire(moebius_ctx* x, int64_t bytes, ImageBuf* out) {
   }
   out->p = (char*)malloc((size_t)cap);
   return out->p != nullptr;
+}
+
+bool image_acquire(moebius_ctx* x, int64_t bytes, ImageBuf* out) {
+  // smallest pooled buffer that fits, preferring one whose last upload has already completed (so that
+  // planning the next switch while the current one runs does not wait for the device)
+  const size_t none = x->image_pool.size();
+  size_t best = none;
+  bool best_ready = false;
+  for (size_t i = 0; i < x->image_pool.size(); ++i) {
+    const ImageBuf& b = x->image_pool[i];
+    if (b.bytes < bytes) continue;
+    bool ready = !b.ev || cudaEventQuery((cudaEvent_t)b.ev) == cudaSuccess;
+    if (!ready) cudaGetLastError();
+    if (best == none || (ready && !best_ready) || (ready == best_ready && b.bytes < x->image_pool[best].bytes)) {
+      best = i; best_ready = ready;
+    }
+  }
+  if (best != none) {
+    *out = x->image_pool[best];
+    x->image_pool.erase(x->image_pool.begin() + (long)best);
+    if (out->ev && !best_ready && cudaEventSynchronize((cudaEvent_t)out->ev) != cudaSuccess) cudaGetLastError();
+    return true;
+  }
+  if (x->has_device < 0) {
+    int ndev = 0;
+    x->has_device = (cudaGetDeviceCount(&ndev) == cudaSuccess && ndev > 0) ? 1 : 0;
+    cudaGetLastError();
+  }
+  // round up so that plans of slightly different sizes share buffers
+  const int64_t cap = (bytes + (1 << 20) - 1) >> 20 << 20;
+  if (!image_fresh(x, cap, out)) return false;
+  // pinning memory can wait for the device: allocate a twin now, so that two plans can be alive
+  // (one executing, one being built) without another allocation later
+  if (out->pinned && x->image_pool.empty()) {
+    ImageBuf twin;
+    if (image_fresh(x, cap, &twin)) x->image_pool.push_back(twin);
+  }
+  return true;
 }
 
 void image_free(const ImageBuf& b) {
