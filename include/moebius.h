@@ -236,6 +236,51 @@ MOEBIUS_API int moebius_set_kv_rounds(moebius_ctx_t* ctx, int max_level);
  * multiple of 32, at most 256. */
 MOEBIUS_API int moebius_set_launch(moebius_ctx_t* ctx, int ctas_per_sm, int threads, int unit_kb);
 
+/* ---- switch coordinator (host only; §4.5) ----------------------------------- */
+
+typedef struct moebius_policy moebius_policy_t; /* opaque, host */
+typedef enum { MOEBIUS_POLICY_INTERACTIVE = 0, MOEBIUS_POLICY_ROLLOUT = 1 } moebius_policy_kind_t;
+typedef enum {
+  MOEBIUS_DECISION_STAY = 0,
+  MOEBIUS_DECISION_SWITCH = 1,    /* the caller now plans + reshards to the other mode */
+  MOEBIUS_DECISION_CANCELLED = 2  /* the policy wanted to switch but the target mode cannot hold the
+                                     live requests: cancelled, retried after the cooldown (:213) */
+} moebius_decision_t;
+typedef struct {
+  uint32_t struct_size;
+  int32_t W;                  /* averaging window in iterations (EP->TP), >= 1                    */
+  double T_h, T_l;            /* TP->EP when the latest count > T_h; EP->TP when the mean of the
+                                 last W counts < T_l; T_l <= T_h (hysteresis band)   */
+  double cooldown_s;          /* no decision for this long after a switch or a cancelled attempt   */
+} moebius_policy_config_t;
+
+/* The paper's two settings: interactive T_l = 0.8 T_h, W = 8; rollout T_l = T_h,
+ * W = 1.  The paper runs T_h = 256, cooldown 5 s.  out: HOST (struct_size set by the caller). */
+MOEBIUS_API int moebius_policy_preset(int kind, double T_h, double cooldown_s, moebius_policy_config_t* out);
+MOEBIUS_API int moebius_policy_create(const moebius_policy_config_t* cfg, moebius_mode_t initial_mode,
+                                      moebius_policy_t** out);
+MOEBIUS_API void moebius_policy_destroy(moebius_policy_t* policy);
+MOEBIUS_API int moebius_policy_mode(const moebius_policy_t* policy);
+
+/* One sample of the control signal -- the global in-flight request count n_req -- taken after a
+ * decode iteration at time now_s (seconds, any monotonic origin).  seq_lens: HOST
+ * int32[n_req], used only for the capacity check of the target mode, which runs through `ctx`
+ * (NULL = no check).  *decision receives a moebius_decision_t, *mode_after (may be NULL) the mode
+ * the policy is in after the call.  The policy only decides; the caller executes the switch. */
+MOEBIUS_API int moebius_policy_step(moebius_policy_t* policy, moebius_ctx_t* ctx, double now_s, int32_t n_req,
+                                    const int32_t* seq_lens, int32_t* decision, int32_t* mode_after);
+
+/* MOEBIUS_OK if mode `to` can hold these requests (TP: all pages in one pool of pages_tp; EP: the
+ * greedy partition of PAPER.md:124, each rank's share in pages_ep), else MOEBIUS_E_CAPACITY
+ * (TP replication reduces capacity when there are fewer KV heads than ranks). */
+MOEBIUS_API int moebius_capacity_check(moebius_ctx_t* ctx, moebius_mode_t to, int32_t n_req, const int32_t* seq_lens);
+
+/* Startup calibration: from decode costs probed at ascending batch sizes under both
+ * modes, the batch size where they cross (linear interpolation between probes; EP never cheaper ->
+ * the largest probe, always cheaper -> the smallest).  All arrays HOST, length n. */
+MOEBIUS_API int moebius_policy_calibrate(int32_t n, const int32_t* batch_sizes, const double* tp_cost,
+                                         const double* ep_cost, int32_t* T_h_out);
+
 MOEBIUS_API const char* moebius_status_str(int status);
 MOEBIUS_API int moebius_version(void);
 

@@ -18,7 +18,8 @@ EXPORTED_SYMBOLS = [
     "moebius_create", "moebius_destroy", "moebius_layout", "moebius_view", "moebius_bind",
     "moebius_active_mode", "moebius_plan", "moebius_plan_destroy", "moebius_block_tables",
     "moebius_plan_stats", "moebius_plan_export", "moebius_reshard", "moebius_stage_plan", "moebius_reshard_staged",
-    "moebius_set_timing",
+    "moebius_set_timing", "moebius_policy_preset", "moebius_policy_create", "moebius_policy_destroy",
+    "moebius_policy_mode", "moebius_policy_step", "moebius_capacity_check", "moebius_policy_calibrate",
     "moebius_last_kernel_ms", "moebius_kernel_ms_history", "moebius_set_launch", "moebius_set_tma", "moebius_set_kv_rounds", "moebius_status_str", "moebius_version",
 ]
 
@@ -36,6 +37,15 @@ class moebius_config_t(C.Structure):
                 ("kv_dtype", C.c_int32), ("kv_pool_bytes_per_rank_layer", C.c_int64),
                 ("max_requests", C.c_int32), ("max_pages_per_request", C.c_int32),
                 ("staging_cap_bytes", C.c_int64)]
+
+
+class moebius_policy_config_t(C.Structure):
+    _fields_ = [("struct_size", C.c_uint32), ("W", C.c_int32), ("T_h", C.c_double), ("T_l", C.c_double),
+                ("cooldown_s", C.c_double)]
+
+
+POLICY_INTERACTIVE, POLICY_ROLLOUT = 0, 1
+DECISION_STAY, DECISION_SWITCH, DECISION_CANCELLED = 0, 1, 2
 
 
 class moebius_layout_t(C.Structure):
@@ -105,6 +115,14 @@ _lib.moebius_block_tables.argtypes = [_vp, _vp, _vp]
 _lib.moebius_plan_stats.argtypes = [_vp, C.POINTER(moebius_stats_t)]
 _lib.moebius_plan_export.argtypes = [_vp, C.c_int, _vp, C.c_int64, C.POINTER(C.c_int64)]
 _lib.moebius_reshard.argtypes = [_vp, _vp, _vp]
+_lib.moebius_policy_preset.argtypes = [C.c_int, C.c_double, C.c_double, C.POINTER(moebius_policy_config_t)]
+_lib.moebius_policy_create.argtypes = [C.POINTER(moebius_policy_config_t), C.c_int, C.POINTER(_vp)]
+_lib.moebius_policy_destroy.argtypes = [_vp]
+_lib.moebius_policy_destroy.restype = None
+_lib.moebius_policy_mode.argtypes = [_vp]
+_lib.moebius_policy_step.argtypes = [_vp, _vp, C.c_double, C.c_int32, _vp, _i32p, _i32p]
+_lib.moebius_capacity_check.argtypes = [_vp, C.c_int, C.c_int32, _vp]
+_lib.moebius_policy_calibrate.argtypes = [C.c_int32, _vp, _vp, _vp, _i32p]
 _lib.moebius_stage_plan.argtypes = [_vp, _vp]
 _lib.moebius_reshard_staged.argtypes = [_vp, _vp]
 _lib.moebius_set_timing.argtypes = [_vp, C.c_int]
@@ -219,6 +237,63 @@ def moebius_plan_export(plan, what: int) -> np.ndarray:
 
 def moebius_reshard(ctx, plan, cuda_stream: int = 0):
     _chk(_lib.moebius_reshard(ctx, plan, _vp(cuda_stream or None)), "moebius_reshard")
+
+
+def moebius_policy_preset(kind: int, T_h: float = 256.0, cooldown_s: float = 5.0) -> moebius_policy_config_t:
+    out = moebius_policy_config_t()
+    out.struct_size = C.sizeof(moebius_policy_config_t)
+    _chk(_lib.moebius_policy_preset(kind, T_h, cooldown_s, C.byref(out)), "moebius_policy_preset")
+    return out
+
+
+def moebius_policy_config(T_h: float, T_l: float, W: int, cooldown_s: float) -> moebius_policy_config_t:
+    out = moebius_policy_config_t()
+    out.struct_size = C.sizeof(moebius_policy_config_t)
+    out.T_h, out.T_l, out.W, out.cooldown_s = T_h, T_l, W, cooldown_s
+    return out
+
+
+def moebius_policy_create(cfg: moebius_policy_config_t, initial_mode: int):
+    cfg.struct_size = C.sizeof(moebius_policy_config_t)
+    out = _vp()
+    _chk(_lib.moebius_policy_create(C.byref(cfg), initial_mode, C.byref(out)), "moebius_policy_create")
+    return out
+
+
+def moebius_policy_destroy(policy):
+    _lib.moebius_policy_destroy(policy)
+
+
+def moebius_policy_mode(policy) -> int:
+    return _lib.moebius_policy_mode(policy)
+
+
+def moebius_policy_step(policy, ctx, now_s: float, seq_lens):
+    """Returns (decision, mode_after).  ctx may be None (no capacity check)."""
+    lens = _i32(seq_lens if len(seq_lens) else np.zeros(0, np.int32))
+    dec, mode = C.c_int32(0), C.c_int32(0)
+    _chk(_lib.moebius_policy_step(policy, ctx, now_s, len(lens), lens.ctypes.data_as(_vp) if len(lens) else None,
+                                  C.byref(dec), C.byref(mode)), "moebius_policy_step")
+    return dec.value, mode.value
+
+
+def moebius_capacity_check(ctx, to_mode: int, seq_lens) -> bool:
+    lens = _i32(seq_lens if len(seq_lens) else np.zeros(0, np.int32))
+    st = _lib.moebius_capacity_check(ctx, to_mode, len(lens), lens.ctypes.data_as(_vp) if len(lens) else None)
+    if st == -2:
+        return False
+    _chk(st, "moebius_capacity_check")
+    return True
+
+
+def moebius_policy_calibrate(batch_sizes, tp_cost, ep_cost) -> int:
+    b = _i32(batch_sizes)
+    t = np.ascontiguousarray(tp_cost, np.float64)
+    e = np.ascontiguousarray(ep_cost, np.float64)
+    out = C.c_int32(0)
+    _chk(_lib.moebius_policy_calibrate(len(b), b.ctypes.data_as(_vp), t.ctypes.data_as(_vp), e.ctypes.data_as(_vp),
+                                       C.byref(out)), "moebius_policy_calibrate")
+    return out.value
 
 
 def moebius_stage_plan(ctx, plan):

@@ -141,6 +141,7 @@ bool image_acquire(moebius_ctx* ctx, int64_t bytes, ImageBuf* out);   // from th
 void image_release(moebius_ctx* ctx, const ImageBuf& buf);             // back to the pool (bounded)
 void image_free(const ImageBuf& buf);
 void cuda_ctx_destroy(moebius_ctx* ctx);
+void lpt_partition(int n_req, const int32_t* seq_lens, int R, PlanScratch& scratch, int32_t* owner);
 void tma_geometry(moebius_ctx* ctx);   // derives xt_ok/kt_ok/xt_rows/kt_pools from cfg + stage_bytes (host only)
 }  // namespace moebius
 

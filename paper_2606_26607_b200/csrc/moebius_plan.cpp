@@ -338,6 +338,25 @@ Seg blank_seg() {
 
 }  // namespace
 
+// decreasing length, greedy least-loaded rank, deterministic.  Reading A9: ties by
+// request id; least loaded = smallest (tokens, requests, rank).
+void moebius::lpt_partition(int n_req, const int32_t* seq_lens, int R, PlanScratch& W, int32_t* owner) {
+  std::vector<int32_t>& order = W.order;
+  order.resize(n_req);
+  std::iota(order.begin(), order.end(), 0);
+  std::stable_sort(order.begin(), order.end(), [&](int a, int b) { return seq_lens[a] > seq_lens[b]; });
+  W.tok.assign(R, 0); W.cnt.assign(R, 0);
+  std::vector<int64_t>&tok = W.tok, &cnt = W.cnt;
+  for (int i : order) {
+    int best = 0;
+    for (int r = 1; r < R; ++r)
+      if (tok[r] < tok[best] || (tok[r] == tok[best] && cnt[r] < cnt[best])) best = r;
+    owner[i] = best;
+    tok[best] += seq_lens[i];
+    cnt[best] += 1;
+  }
+}
+
 extern "C" int moebius_plan(moebius_ctx_t* x, moebius_mode_t from, moebius_mode_t to, int32_t n_req,
                             const int32_t* seq_lens, const int32_t* src_owner, const int32_t* src_bt,
                             moebius_plan_t** out) {
@@ -368,22 +387,7 @@ extern "C" int moebius_plan(moebius_ctx_t* x, moebius_mode_t from, moebius_mode_
   std::vector<int32_t>& owner = W.owner;
   owner.assign(n_req, -1);
   if (!e2t) {
-    // decreasing length, greedy least-loaded rank, deterministic.  Reading A9: ties by
-    // request id; least loaded = smallest (tokens, requests, rank).
-    std::vector<int32_t>& order = W.order;
-    order.resize(n_req);
-    std::iota(order.begin(), order.end(), 0);
-    std::stable_sort(order.begin(), order.end(), [&](int a, int b) { return seq_lens[a] > seq_lens[b]; });
-    W.tok.assign(R, 0); W.cnt.assign(R, 0);
-    std::vector<int64_t>&tok = W.tok, &cnt = W.cnt;
-    for (int i : order) {
-      int best = 0;
-      for (int r = 1; r < R; ++r)
-        if (tok[r] < tok[best] || (tok[r] == tok[best] && cnt[r] < cnt[best])) best = r;
-      owner[i] = best;
-      tok[best] += seq_lens[i];
-      cnt[best] += 1;
-    }
+    lpt_partition(n_req, seq_lens, R, W, owner.data());
   }
   // reading A7: ascending request id, consecutive pages; TP bumps up from 0, EP down from the top.
   // Only the first npages[i] entries of a row are written here; the -1 padding is laid down when
