@@ -1,6 +1,6 @@
 // moebius_policy.cpp -- the switch coordinator's policy (§4.5) and the KV-capacity
-// check that precedes every switch.  Host only.  Product code: shares nothing
-// with oracle/.
+// check that precedes every switch.  Host only.
+// Product code: shares nothing with oracle/.
 #include <algorithm>
 #include <cstring>
 #include <new>
