@@ -179,7 +179,8 @@ MOEBIUS_API int moebius_plan_stats(const moebius_plan_t* plan, moebius_stats_t* 
 
 /* Diagnostic dump of the work list for host-side hazard checking (tests).  what: 0 = segments
  * (moebius_segment_t-sized records), 1 = KV move descriptors (16 B each), 2 = 2-D
- * copy descriptors (32 B each).  buf: HOST, cap bytes; *needed receives the full size. */
+ * copy descriptors (32 B each), 3 = the dependency wave of every segment (int32 each).  buf: HOST, cap
+ * bytes; *needed receives the full size. */
 MOEBIUS_API int moebius_plan_export(const moebius_plan_t* plan, int what, void* buf, int64_t cap,
                                     int64_t* needed);
 
@@ -209,6 +210,25 @@ MOEBIUS_API int moebius_reshard(moebius_ctx_t* ctx, const moebius_plan_t* plan, 
 MOEBIUS_API int moebius_stage_plan(moebius_ctx_t* ctx, const moebius_plan_t* plan);
 MOEBIUS_API int moebius_reshard_staged(moebius_ctx_t* ctx, void* cuda_stream);
 
+/* Rank-share execution, the multi-GPU form of a switch.
+ * A plan's segments fall into dependency WAVES (moebius_plan_waves); within a wave nothing depends on
+ * anything.  Every process builds the same plan (the planner is deterministic), binds a
+ * moebius_arena in which it owns ranks [rank_lo, rank_hi), and for wave = 0 .. n_waves-1 calls
+ * moebius_reshard_share, which enqueues one launch executing only the units whose EP-side rank it
+ * owns -- EP->TP: read the own EP view, store into every TP owner's region (push); TP->EP: load from
+ * the TP holders, write the own EP view (pull) -- followed by a barrier across the processes (one per
+ * dependency round).  After the last wave each process calls moebius_reshard_publish (tables + the
+ * active-mode flip).  Wave 0 also uploads the work list.  On one GPU the shares of a wave may simply
+ * be enqueued one after another; the result is identical to moebius_reshard. */
+MOEBIUS_API int moebius_plan_waves(const moebius_plan_t* plan, int32_t* n_waves);
+MOEBIUS_API int moebius_reshard_share(moebius_ctx_t* ctx, const moebius_plan_t* plan, int rank_lo, int rank_hi,
+                                      int wave, void* cuda_stream);
+/* What ranks [rank_lo, rank_hi) execute of a plan in `wave` (-1: all waves).  out4: HOST int64[4] =
+ * {units, bytes read, bytes written, bytes crossing between ranks}; the crossing bytes of all ranks
+ * sum to the plan's owner-changed bytes (moebius_stats_t w_moved + kv_moved). */
+MOEBIUS_API int moebius_share_stats(const moebius_plan_t* plan, int rank_lo, int rank_hi, int wave, int64_t* out4);
+MOEBIUS_API int moebius_reshard_publish(moebius_ctx_t* ctx, const moebius_plan_t* plan, void* cuda_stream);
+
 /* Kernel-only device time of the last moebius_reshard, in ms (CUDA events on its stream; the call
  * synchronises on the end event).  Enabled with moebius_set_timing(ctx, 1). */
 MOEBIUS_API int moebius_set_timing(moebius_ctx_t* ctx, int enable);
@@ -235,6 +255,25 @@ MOEBIUS_API int moebius_set_kv_rounds(moebius_ctx_t* ctx, int max_level);
 /* Launch shape override for the ld/st path (tuning): values <= 0 restore the defaults; threads is a
  * multiple of 32, at most 256. */
 MOEBIUS_API int moebius_set_launch(moebius_ctx_t* ctx, int ctas_per_sm, int threads, int unit_kb);
+
+/* ---- peer-mappable unified buffer (needs a CUDA device) ------------- */
+
+/* each rank's buffer is exported once and mapped by its peers, whose kernels
+ * store into it.  Here: ONE virtual range of R * rank_stride bytes (rank_stride is a multiple of
+ * 2 MiB for this), rank r's region backed by its OWN physical allocation mapped at
+ * base + r * rank_stride.  Ranks [rank_lo, rank_hi) are created on `device` by this call; the others
+ * are imported from the processes that own them (POSIX file descriptors of their allocations, sent
+ * over a unix socket by the caller).  All addresses the planner and kernel use, tensor maps
+ * included, are the same whether the ranks share a GPU or have one each.  The resulting base is a
+ * valid `dev_base` for moebius_bind once every rank is mapped (moebius_arena_ready == MOEBIUS_OK). */
+typedef struct moebius_arena moebius_arena_t; /* opaque, host */
+MOEBIUS_API int moebius_arena_create(const moebius_ctx_t* ctx, int device, int rank_lo, int rank_hi,
+                                     moebius_arena_t** out);
+MOEBIUS_API void moebius_arena_destroy(moebius_arena_t* arena);
+MOEBIUS_API void* moebius_arena_base(const moebius_arena_t* arena);        /* DEVICE pointer */
+MOEBIUS_API int moebius_arena_ready(const moebius_arena_t* arena);
+MOEBIUS_API int moebius_arena_export(const moebius_arena_t* arena, int rank, int* fd_out); /* a local rank */
+MOEBIUS_API int moebius_arena_import(moebius_arena_t* arena, int rank, int fd);            /* a peer's rank */
 
 /* ---- switch coordinator (host only; §4.5) ----------------------------------- */
 

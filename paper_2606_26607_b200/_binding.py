@@ -18,6 +18,9 @@ EXPORTED_SYMBOLS = [
     "moebius_create", "moebius_destroy", "moebius_layout", "moebius_view", "moebius_bind",
     "moebius_active_mode", "moebius_plan", "moebius_plan_destroy", "moebius_block_tables",
     "moebius_plan_stats", "moebius_plan_export", "moebius_reshard", "moebius_stage_plan", "moebius_reshard_staged",
+    "moebius_share_stats", "moebius_plan_waves", "moebius_reshard_share", "moebius_reshard_publish",
+    "moebius_arena_create", "moebius_arena_destroy", "moebius_arena_base", "moebius_arena_ready",
+    "moebius_arena_export", "moebius_arena_import",
     "moebius_set_timing", "moebius_policy_preset", "moebius_policy_create", "moebius_policy_destroy",
     "moebius_policy_mode", "moebius_policy_step", "moebius_capacity_check", "moebius_policy_calibrate",
     "moebius_last_kernel_ms", "moebius_kernel_ms_history", "moebius_set_launch", "moebius_set_tma", "moebius_set_kv_rounds", "moebius_status_str", "moebius_version",
@@ -123,6 +126,18 @@ _lib.moebius_policy_mode.argtypes = [_vp]
 _lib.moebius_policy_step.argtypes = [_vp, _vp, C.c_double, C.c_int32, _vp, _i32p, _i32p]
 _lib.moebius_capacity_check.argtypes = [_vp, C.c_int, C.c_int32, _vp]
 _lib.moebius_policy_calibrate.argtypes = [C.c_int32, _vp, _vp, _vp, _i32p]
+_lib.moebius_plan_waves.argtypes = [_vp, _i32p]
+_lib.moebius_share_stats.argtypes = [_vp, C.c_int, C.c_int, C.c_int, _vp]
+_lib.moebius_reshard_share.argtypes = [_vp, _vp, C.c_int, C.c_int, C.c_int, _vp]
+_lib.moebius_reshard_publish.argtypes = [_vp, _vp, _vp]
+_lib.moebius_arena_create.argtypes = [_vp, C.c_int, C.c_int, C.c_int, C.POINTER(_vp)]
+_lib.moebius_arena_destroy.argtypes = [_vp]
+_lib.moebius_arena_destroy.restype = None
+_lib.moebius_arena_base.argtypes = [_vp]
+_lib.moebius_arena_base.restype = _vp
+_lib.moebius_arena_ready.argtypes = [_vp]
+_lib.moebius_arena_export.argtypes = [_vp, C.c_int, _i32p]
+_lib.moebius_arena_import.argtypes = [_vp, C.c_int, C.c_int]
 _lib.moebius_stage_plan.argtypes = [_vp, _vp]
 _lib.moebius_reshard_staged.argtypes = [_vp, _vp]
 _lib.moebius_set_timing.argtypes = [_vp, C.c_int]
@@ -225,7 +240,7 @@ def moebius_plan_stats(plan) -> moebius_stats_t:
 
 
 def moebius_plan_export(plan, what: int) -> np.ndarray:
-    dt = (SEG_DTYPE, KV_DTYPE, C2D_DTYPE)[what]
+    dt = (SEG_DTYPE, KV_DTYPE, C2D_DTYPE, np.dtype("<i4"))[what]
     need = C.c_int64(0)
     _chk(_lib.moebius_plan_export(plan, what, None, 0, C.byref(need)), "moebius_plan_export")
     buf = np.zeros(need.value // dt.itemsize, dtype=dt)
@@ -294,6 +309,54 @@ def moebius_policy_calibrate(batch_sizes, tp_cost, ep_cost) -> int:
     _chk(_lib.moebius_policy_calibrate(len(b), b.ctypes.data_as(_vp), t.ctypes.data_as(_vp), e.ctypes.data_as(_vp),
                                        C.byref(out)), "moebius_policy_calibrate")
     return out.value
+
+
+def moebius_plan_waves(plan) -> int:
+    n = C.c_int32(0)
+    _chk(_lib.moebius_plan_waves(plan, C.byref(n)), "moebius_plan_waves")
+    return n.value
+
+
+def moebius_share_stats(plan, rank_lo: int, rank_hi: int, wave: int = -1) -> dict:
+    out = np.zeros(4, np.int64)
+    _chk(_lib.moebius_share_stats(plan, rank_lo, rank_hi, wave, out.ctypes.data_as(_vp)), "moebius_share_stats")
+    return {"units": int(out[0]), "read": int(out[1]), "written": int(out[2]), "cross": int(out[3])}
+
+
+def moebius_reshard_share(ctx, plan, rank_lo: int, rank_hi: int, wave: int, cuda_stream: int = 0):
+    _chk(_lib.moebius_reshard_share(ctx, plan, rank_lo, rank_hi, wave, _vp(cuda_stream or None)), "moebius_reshard_share")
+
+
+def moebius_reshard_publish(ctx, plan, cuda_stream: int = 0):
+    _chk(_lib.moebius_reshard_publish(ctx, plan, _vp(cuda_stream or None)), "moebius_reshard_publish")
+
+
+def moebius_arena_create(ctx, device: int, rank_lo: int, rank_hi: int):
+    out = _vp()
+    _chk(_lib.moebius_arena_create(ctx, device, rank_lo, rank_hi, C.byref(out)), "moebius_arena_create")
+    return out
+
+
+def moebius_arena_destroy(arena):
+    _lib.moebius_arena_destroy(arena)
+
+
+def moebius_arena_base(arena) -> int:
+    return int(_lib.moebius_arena_base(arena) or 0)
+
+
+def moebius_arena_ready(arena) -> bool:
+    return _lib.moebius_arena_ready(arena) == 0
+
+
+def moebius_arena_export(arena, rank: int) -> int:
+    fd = C.c_int32(-1)
+    _chk(_lib.moebius_arena_export(arena, rank, C.byref(fd)), "moebius_arena_export")
+    return fd.value
+
+
+def moebius_arena_import(arena, rank: int, fd: int):
+    _chk(_lib.moebius_arena_import(arena, rank, fd), "moebius_arena_import")
 
 
 def moebius_stage_plan(ctx, plan):

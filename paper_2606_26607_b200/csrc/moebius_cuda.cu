@@ -323,8 +323,8 @@ moebius_reshard_kernel(const __grid_constant__ DevParams p_in, const __grid_cons
     p.n_segs = h.x;
     p.total_units = h.y;
     p.segs = (const Seg*)((const char*)p_in.hdr + sizeof(PlanHdr));
-    p.kv = (const KvDesc*)((const char*)p_in.hdr + h.z);
-    p.c2d = (const C2dDesc*)((const char*)p_in.hdr + h.w);
+    p.kv = (const KvDesc*)((const char*)p_in.hdr + (int64_t)(int32_t)h.z);     // signed: a wave header sits
+    p.c2d = (const C2dDesc*)((const char*)p_in.hdr + (int64_t)(int32_t)h.w);   // behind the arrays it uses
   }
   const uint32_t lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   uint64_t* bar = (uint64_t*)smem + 2 * warp;                       // 2 barriers per pipe
@@ -395,6 +395,7 @@ moebius_reshard_kernel(const __grid_constant__ DevParams p_in, const __grid_cons
   };
   auto fetch = [&]() -> uint32_t { return lane == 0 ? atomicAdd(p.ticket, 1u) : 0u; };
 
+  const bool share = p.rank_hi - p.rank_lo < p.n_ranks;
   uint32_t si = 0;
   uint32_t t_next = fetch();
   for (;;) {
@@ -411,6 +412,10 @@ moebius_reshard_kernel(const __grid_constant__ DevParams p_in, const __grid_cons
     }
     const Seg& s = p.segs[si];
     const uint32_t ul = u - s.unit_begin;
+    if (share) {   // rank share: this launch executes only the units of the ranks it owns
+      const uint32_t q = unit_ep_rank(s, p, ul);
+      if (q < p.rank_lo || q >= p.rank_hi) { t_next = fetch(); continue; }
+    }
     if (seg_path(s) == PATH_TMA) {
       const KvDesc d = tma_prefetch_desc(p, s, ul);   // its latency hides behind the wait in retire()
       retire();
@@ -624,12 +629,16 @@ int ensure_device_facts(moebius_ctx* x) {
 // Launches the reshard kernel over the image that sits at dev_desc + kSegOff.  `tma`: the variant with
 // the pipes' shared-memory rings (it also executes PATH_LSU segments).  `unit_hint` > 0 caps the grid
 // for small plans; 0 = the full persistent grid (plan-independent: what a captured graph needs).
-int launch_reshard_kernel(moebius_ctx* x, bool tma, int64_t unit_hint, cudaStream_t st) {
+int launch_reshard_kernel(moebius_ctx* x, bool tma, int64_t unit_hint, cudaStream_t st, int64_t hdr_off = 0,
+                          int rank_lo = 0, int rank_hi = -1) {
   DevParams p;
   memset(&p, 0, sizeof(p));
   p.base = x->base;
   p.stg = x->stg;
-  p.hdr = (const PlanHdr*)(x->desc + kSegOff);
+  p.hdr = (const PlanHdr*)(x->desc + kSegOff + hdr_off);
+  p.n_ranks = (uint32_t)x->cfg.R;
+  p.rank_lo = (uint32_t)rank_lo;
+  p.rank_hi = (uint32_t)(rank_hi < 0 ? x->cfg.R : rank_hi);
   p.ticket = (uint32_t*)x->desc;
   p.counters = (uint32_t*)(x->desc + kCtrOff);
   p.rank_stride = x->rank_stride;
@@ -743,5 +752,43 @@ extern "C" int moebius_reshard_staged(moebius_ctx_t* x, void* cuda_stream) {
   if (int rc = launch_reshard_kernel(x, tma, 0, st)) return rc;
   if (cudaMemcpyAsync(x->tables, x->mailbox + img_cap, (size_t)x->table_bytes, cudaMemcpyHostToDevice, st) != cudaSuccess)
     return MOEBIUS_E_CUDA;
+  return MOEBIUS_OK;
+}
+
+// ---- rank-share execution: the plan wave by wave, each launch restricted to a range of ranks -------
+extern "C" int moebius_plan_waves(const moebius_plan_t* P, int32_t* n_waves) {
+  if (!P || !n_waves) return MOEBIUS_E_INVAL;
+  *n_waves = P->n_waves;
+  return MOEBIUS_OK;
+}
+
+extern "C" int moebius_reshard_share(moebius_ctx_t* x, const moebius_plan_t* P, int rank_lo, int rank_hi, int wave,
+                                     void* cuda_stream) {
+  if (!x || !P || P->ctx != x) return MOEBIUS_E_INVAL;
+  if (rank_lo < 0 || rank_hi > x->cfg.R || rank_lo >= rank_hi || wave < 0 || wave >= P->n_waves) return MOEBIUS_E_INVAL;
+  if (!x->bound || x->active_mode != P->from) return MOEBIUS_E_STATE;
+  if (P->uses_tma && (P->stage_bytes != x->stage_bytes || P->xt_rows != x->xt_rows)) return MOEBIUS_E_STATE;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  if (int rc = ensure_device_facts(x)) return rc;
+  if (wave == 0) {   // the work list (all waves) goes up once, with the first wave
+    if (cudaMemcpyAsync(x->desc + kSegOff, P->image, (size_t)P->image_bytes, cudaMemcpyHostToDevice, st) != cudaSuccess)
+      return MOEBIUS_E_CUDA;
+    if (P->buf.ev && cudaEventRecord((cudaEvent_t)P->buf.ev, st) != cudaSuccess) return MOEBIUS_E_CUDA;
+  }
+  if (cudaMemsetAsync(x->desc, 0, (size_t)kHdrBytes, st) != cudaSuccess) return MOEBIUS_E_CUDA;   // the ticket
+  if (P->wave_units[(size_t)wave] == 0) return MOEBIUS_OK;
+  return launch_reshard_kernel(x, P->uses_tma, (int64_t)P->wave_units[(size_t)wave], st, P->wave_hdr_off[(size_t)wave],
+                               rank_lo, rank_hi);
+}
+
+extern "C" int moebius_reshard_publish(moebius_ctx_t* x, const moebius_plan_t* P, void* cuda_stream) {
+  if (!x || !P || P->ctx != x) return MOEBIUS_E_INVAL;
+  if (!x->bound || x->active_mode != P->from) return MOEBIUS_E_STATE;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  if (cudaMemcpyAsync(x->tables, P->tbl_image, (size_t)P->tbl_bytes, cudaMemcpyHostToDevice, st) != cudaSuccess)
+    return MOEBIUS_E_CUDA;
+  if (P->buf.ev && cudaEventRecord((cudaEvent_t)P->buf.ev, st) != cudaSuccess) return MOEBIUS_E_CUDA;
+  x->active_mode = P->to;
+  x->switch_count++;
   return MOEBIUS_OK;
 }

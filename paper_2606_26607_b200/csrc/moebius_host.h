@@ -130,6 +130,12 @@ struct moebius_plan {
   // one contiguous upload image: [segs][kv][c2d], and the table image; pinned when CUDA allows
   char* image;
   int64_t image_bytes, kv_img_off, c2d_img_off;
+  // rank-share execution (multi-GPU): per dependency wave a header + segment list inside the image
+  int32_t n_waves;
+  int64_t wave_img_off;
+  std::vector<int32_t> seg_wave;       // dependency wave of every segment
+  std::vector<int64_t> wave_hdr_off;
+  std::vector<uint32_t> wave_units;
   int32_t* tbl_image;
   int64_t tbl_bytes;
   moebius::ImageBuf buf;          // backing storage of image + tbl_image

@@ -127,7 +127,7 @@ int moebius_create(const moebius_config_t* c, moebius_ctx_t** out) {
   x->scale_ep_off = off;  off += x->scale_ep_layer * L;
   off = align_up(off, 4096);
   x->kv_off = off;        off += 2 * (int64_t)L * x->pool_bytes;
-  x->rank_stride = align_up(off, 4096);
+  x->rank_stride = align_up(off, 2 << 20);   // 2 MiB: a rank region can be its own physical allocation (moebius_arena_*)
 
   x->spare_bytes = (int64_t)x->ep_shift * x->S * R;
   x->resident_bytes = (int64_t)3 * L * x->S * R + 2 * (int64_t)L * x->pool_bytes * R;
@@ -145,7 +145,7 @@ int moebius_create(const moebius_config_t* c, moebius_ctx_t** out) {
   live_max = std::min<int64_t>(live_max, (int64_t)c->max_requests * c->max_pages_per_request);
   x->max_kv_desc = live_max;
   x->max_c2d = c->w_dtype == MOEBIUS_FP8_E4M3_B128 ? (int64_t)x->n_obj * L * R * R : 0;
-  x->desc_bytes = align_up(kSegOff + (int64_t)sizeof(PlanHdr) + (int64_t)kMaxSegs * sizeof(Seg) + x->max_kv_desc * sizeof(KvDesc) +
+  x->desc_bytes = align_up(kSegOff + (int64_t)(1 + kMaxCounters) * sizeof(PlanHdr) + 2 * (int64_t)kMaxSegs * sizeof(Seg) + x->max_kv_desc * sizeof(KvDesc) +
                                x->max_c2d * sizeof(C2dDesc) + 1024, 4096);
   x->table_bytes = align_up(4 * ((int64_t)kTblHdrInts + 2 * (int64_t)c->max_requests +
                                  (int64_t)c->max_requests * c->max_pages_per_request), 256);
@@ -724,6 +724,7 @@ extern "C" int moebius_plan(moebius_ctx_t* x, moebius_mode_t from, moebius_mode_
     }
     Seg s = blank_seg();
     s.kind = SEG_COPY2D;
+    s.ep_is_src = e2t;          // which side of a descriptor is the EP side (rank-share filter)
     s.desc_begin = 0;
     s.n_desc = (uint32_t)P->c2d.size();
     s.n_units = s.n_desc;
@@ -848,7 +849,25 @@ extern "C" int moebius_plan(moebius_ctx_t* x, moebius_mode_t from, moebius_mode_
   P->stage_bytes = x->stage_bytes;
   P->xt_rows = x->xt_rows;
 
-  // ---- target request state + upload images (written in place: [segs][kv][c2d] | tables) ---------
+  // Waves: wave(s) = 0 without a dependency, else 1 + the latest wave among the segments that signal
+  // the counter s waits on.  A multi-GPU run executes wave by wave with a barrier across GPUs in
+  // between (one barrier per dependency round); the fused launch ignores them.
+  std::vector<int32_t>& seg_wave = P->seg_wave;
+  seg_wave.assign(P->segs.size(), 0);
+  {
+    std::vector<int32_t> ctr_wave(next_ctr ? next_ctr : 1, -1);
+    int32_t n_waves = P->segs.empty() ? 0 : 1;
+    for (size_t i = 0; i < P->segs.size(); ++i) {
+      const Seg& sg = P->segs[i];
+      int32_t w = sg.wait_ctr >= 0 ? ctr_wave[(size_t)sg.wait_ctr] + 1 : 0;
+      seg_wave[i] = w;
+      if (sg.signal_ctr >= 0) ctr_wave[(size_t)sg.signal_ctr] = std::max(ctr_wave[(size_t)sg.signal_ctr], w);
+      n_waves = std::max(n_waves, w + 1);
+    }
+    P->n_waves = n_waves;
+  }
+
+  // ---- target request state + upload images (written in place: [segs][kv][c2d][waves] | tables) ---
   P->lens.assign(seq_lens, seq_lens + n_req);
   P->owner = owner;
   int64_t seg_b = align_up((int64_t)P->segs.size() * sizeof(Seg), 256);
@@ -857,7 +876,10 @@ extern "C" int moebius_plan(moebius_ctx_t* x, moebius_mode_t from, moebius_mode_
   const int64_t hdr_b = sizeof(PlanHdr);
   P->kv_img_off = hdr_b + seg_b;
   P->c2d_img_off = hdr_b + seg_b + kv_b;
-  P->image_bytes = hdr_b + seg_b + kv_b + c2d_b;
+  P->wave_img_off = hdr_b + seg_b + kv_b + c2d_b;
+  const int64_t wave_b = (int64_t)P->n_waves * hdr_b + (int64_t)P->segs.size() * (int64_t)sizeof(Seg);
+  P->image_bytes = P->wave_img_off + wave_b;
+  if (kSegOff + P->image_bytes > x->desc_bytes) return fail(MOEBIUS_E_INVAL);
   P->tbl_bytes = 4 * ((int64_t)kTblHdrInts + 2 * (int64_t)c.max_requests + (int64_t)n_req * MP);
   if (!image_acquire(x, P->image_bytes + P->tbl_bytes + 256, &P->buf)) return fail(MOEBIUS_E_INVAL);
   P->image = P->buf.p;
@@ -893,6 +915,35 @@ extern "C" int moebius_plan(moebius_ctx_t* x, moebius_mode_t from, moebius_mode_
   if (c2d_b) {
     memcpy(P->image + P->c2d_img_off, P->c2d.data(), P->c2d.size() * sizeof(C2dDesc));
     memset(P->image + P->c2d_img_off + P->c2d.size() * sizeof(C2dDesc), 0, (size_t)(c2d_b - (int64_t)(P->c2d.size() * sizeof(C2dDesc))));
+  }
+  {  // per wave: a header + that wave's segments with their own unit numbering and no dependencies;
+     // descriptor offsets are relative to the wave's header (negative: the arrays sit before it)
+    P->wave_hdr_off.assign((size_t)P->n_waves, 0);
+    P->wave_units.assign((size_t)P->n_waves, 0);
+    int64_t at = P->wave_img_off;
+    for (int32_t w = 0; w < P->n_waves; ++w) {
+      PlanHdr* h = (PlanHdr*)(P->image + at);
+      memset(h, 0, sizeof(PlanHdr));
+      P->wave_hdr_off[(size_t)w] = at;
+      Seg* out_segs = (Seg*)(P->image + at + hdr_b);
+      uint32_t n = 0, units = 0;
+      bool tma = false;
+      for (size_t i = 0; i < P->segs.size(); ++i) {
+        if (seg_wave[i] != w) continue;
+        Seg t = P->segs[i];
+        t.wait_ctr = -1; t.signal_ctr = -1;
+        t.unit_begin = units;
+        units += t.n_units;
+        tma |= seg_path(t) == PATH_TMA;
+        out_segs[n++] = t;
+      }
+      h->n_segs = n;
+      h->total_units = units;
+      h->kv_off = (uint32_t)(int32_t)(P->kv_img_off - at);
+      h->c2d_off = (uint32_t)(int32_t)(P->c2d_img_off - at);
+      P->wave_units[(size_t)w] = units;
+      at += hdr_b + (int64_t)n * (int64_t)sizeof(Seg);
+    }
   }
   P->tbl_image = (int32_t*)(P->image + align_up(P->image_bytes, 256));
   int32_t* T = P->tbl_image;
@@ -944,9 +995,69 @@ extern "C" int moebius_plan_export(const moebius_plan_t* p, int what, void* buf,
     case 0: src = p->segs.data(); n = (int64_t)p->segs.size() * sizeof(Seg); break;
     case 1: src = p->kv;          n = p->n_kv * (int64_t)sizeof(KvDesc); break;
     case 2: src = p->c2d.data();  n = (int64_t)p->c2d.size() * sizeof(C2dDesc); break;
+    case 3: src = p->seg_wave.data(); n = (int64_t)p->seg_wave.size() * 4; break;
     default: return MOEBIUS_E_INVAL;
   }
   *needed = n;
   if (buf && cap >= n && n) memcpy(buf, src, (size_t)n);
+  return MOEBIUS_OK;
+}
+
+// What the ranks [rank_lo, rank_hi) execute of a plan (wave < 0: all waves): units, bytes read, bytes
+// written, and the bytes that cross between ranks (EP->TP: stored into another rank's region;
+// TP->EP: loaded from another rank's region) -- the per-GPU interconnect volume of PAPER.md:189.
+extern "C" int moebius_share_stats(const moebius_plan_t* P, int rank_lo, int rank_hi, int wave, int64_t* out4) {
+  if (!P || !out4) return MOEBIUS_E_INVAL;
+  const moebius_ctx* x = P->ctx;
+  if (rank_lo < 0 || rank_hi > x->cfg.R || rank_lo >= rank_hi || wave >= P->n_waves) return MOEBIUS_E_INVAL;
+  DevParams p;
+  memset(&p, 0, sizeof(p));
+  p.kv = P->kv;
+  p.c2d = P->c2d.data();
+  p.rank_stride = x->rank_stride;
+  int64_t units = 0, rd = 0, wr = 0, cross = 0;
+  for (size_t si = 0; si < P->segs.size(); ++si) {
+    if (wave >= 0 && P->seg_wave[si] != wave) continue;
+    const Seg& s = P->segs[si];
+    for (uint32_t u = 0; u < s.n_units; ++u) {
+      const int q = (int)unit_ep_rank(s, p, u);
+      if (q < rank_lo || q >= rank_hi) continue;
+      ++units;
+      if (seg_kind(s) == SEG_COPY2D) {
+        const C2dDesc& d = p.c2d[s.desc_begin + u];
+        const int64_t b = (int64_t)d.rows * d.run_bytes;
+        rd += b; wr += b;
+        if (d.src_off / x->rank_stride != d.dst_off / x->rank_stride) cross += b;
+        continue;
+      }
+      if (seg_kind(s) == SEG_XPOSE) {
+        uint32_t v = u / s.chunks_per_run;
+        const uint32_t jgroups = s.n_groups / s.groups_per_unit;
+        const uint32_t jg = v % jgroups;
+        const uint32_t rb = (v / jgroups) % s.row_blocks;
+        const int64_t nrows = std::min<int64_t>(s.rows_per_unit, (int64_t)s.rows_total - (int64_t)rb * s.rows_per_unit);
+        const int64_t per_group = nrows * s.chunk_bytes;
+        rd += per_group * s.groups_per_unit; wr += per_group * s.groups_per_unit;
+        for (uint32_t g = jg * s.groups_per_unit; g < (jg + 1) * s.groups_per_unit; ++g)
+          if ((int)g != q) cross += per_group;
+        continue;
+      }
+      uint32_t pb, di;
+      kv_unit(s, u, pb, di);
+      const KvDesc& d = p.kv[s.desc_begin + di];
+      const int64_t row = (int64_t)(d.ntok_slot & 0xFFu) * s.run_bytes * seg_boxes(s, u);   // one group, all pools of the unit
+      if (s.kv_mode == KV_STG_COPY) { rd += row * s.n_groups; wr += row * s.n_groups; continue; }
+      rd += row * s.n_groups;
+      if (s.ep_is_src) {
+        wr += row * s.n_groups * s.rep;
+        cross += row * ((int64_t)s.n_groups * s.rep - 1);
+      } else {
+        wr += row * s.n_groups;
+        for (uint32_t g = 0; g < s.n_groups; ++g)
+          if ((int)tp_src_rank(g, s.rep, d.ep_rank) != d.ep_rank) cross += row;
+      }
+    }
+  }
+  out4[0] = units; out4[1] = rd; out4[2] = wr; out4[3] = cross;
   return MOEBIUS_OK;
 }

@@ -115,7 +115,9 @@ struct DevParams {        // decoded launch state (the kernel fills the plan-dep
   uint32_t         stage_bytes;   // PATH_TMA: bytes of one shared-memory stage (2 per pipe)
   uint32_t         xt_rows;       // PATH_TMA: rows of the weight tensor-map box (= rows_per_unit)
   uint32_t         page_tokens;
-  uint32_t         pad_;
+  uint32_t         n_ranks;       // R
+  uint32_t         rank_lo, rank_hi;   // rank share: only units whose EP-side rank is in [lo, hi) are
+                                       // executed (multi-GPU: the ranks this GPU owns); [0, R) = all
 };
 
 MB_HD uint32_t seg_kind(const Seg& s) { return s.kind & 0xFFu; }
@@ -156,6 +158,25 @@ MB_HD uint32_t seg_boxes(const Seg& s, uint32_t u) {
 MB_HD uint32_t tp_src_rank(uint32_t g, uint32_t rep, int32_t owner) {
   if (owner >= 0 && (uint32_t)owner / rep == g) return (uint32_t)owner;
   return g * rep;
+}
+
+// EP-side rank of a unit: the rank whose EP view it reads (EP->TP: pushed to the TP owners) or writes
+// (TP->EP: pulled from the TP holders).  PAPER.md:172: "each kernel reads from the source-mode alias
+// and writes the slice into the peer's target-mode slot" -- on several GPUs a unit runs on the GPU
+// that owns this rank.
+MB_HD uint32_t unit_ep_rank(const Seg& s, const DevParams& p, uint32_t u) {
+  if (seg_kind(s) == SEG_XPOSE) {
+    u /= s.chunks_per_run;
+    u /= s.n_groups / s.groups_per_unit;
+    return u / s.row_blocks;
+  }
+  if (seg_kind(s) == SEG_KV) {
+    uint32_t pb, di;
+    kv_unit(s, u, pb, di);
+    return (uint32_t)p.kv[s.desc_begin + di].ep_rank;
+  }
+  const C2dDesc& d = p.c2d[s.desc_begin + u];
+  return (uint32_t)((s.ep_is_src ? d.src_off : d.dst_off) / p.rank_stride);
 }
 
 // Decode box k of unit u (u is LOCAL to the segment).

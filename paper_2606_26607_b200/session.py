@@ -28,17 +28,27 @@ def make_config(*, R, L, E, H, I, w_dtype="bf16", kv_heads, head_dim, page_token
     return c
 
 
+class _RawCuda:
+    """A device byte range that torch did not allocate, exposed through __cuda_array_interface__."""
+
+    def __init__(self, ptr: int, nbytes: int):
+        self.__cuda_array_interface__ = {"shape": (nbytes,), "typestr": "|u1", "data": (ptr, False), "version": 2}
+
+
 class Session:
     """One context + its torch-owned device buffers.  `device=None` keeps it host-only (planner)."""
 
     def __init__(self, cfg: B.moebius_config_t, device=None, initial_mode: int = B.MOEBIUS_TP,
-                 guard_bytes: int = 0):
+                 guard_bytes: int = 0, vmm: bool = False):
+        """vmm=True: the unified buffer is a moebius_arena -- one virtual range, one physical allocation
+        per rank (the address layout of a multi-GPU deployment, here with every rank on `device`)."""
         self.cfg = cfg
         self.ctx = B.moebius_create(cfg)
         self.layout = B.moebius_layout(self.ctx)
         self.device = device
         self.guard_bytes = guard_bytes
         self._plans = []
+        self.vmm_arena = None
         if device is not None:
             import torch
             if not torch.cuda.is_available():
@@ -46,7 +56,8 @@ class Session:
             lay = self.layout
             g = guard_bytes
             al = lambda n: (int(n) + 255) // 256 * 256  # noqa: E731
-            sizes = [al(lay.base_bytes), al(max(lay.staging_bytes, 256)), al(lay.desc_bytes), al(lay.table_bytes)]
+            sizes = [0 if vmm else al(lay.base_bytes), al(max(lay.staging_bytes, 256)), al(lay.desc_bytes),
+                     al(lay.table_bytes)]
             total = sum(s + g for s in sizes) + g
             self.arena = torch.empty(total, dtype=torch.uint8, device=device)
             assert self.arena.data_ptr() % 256 == 0
@@ -55,7 +66,14 @@ class Session:
                 offs.append(o)
                 o += s + g
             self._offs, self._sizes = offs, sizes
-            self.base = self.arena[offs[0]:offs[0] + sizes[0]]
+            if vmm:
+                dev_index = torch.device(device).index or 0
+                self.vmm_arena = B.moebius_arena_create(self.ctx, dev_index, 0, cfg.R)
+                assert B.moebius_arena_ready(self.vmm_arena)
+                self.base = torch.as_tensor(_RawCuda(B.moebius_arena_base(self.vmm_arena), int(lay.base_bytes)),
+                                            device=device)
+            else:
+                self.base = self.arena[offs[0]:offs[0] + sizes[0]]
             self.staging = self.arena[offs[1]:offs[1] + sizes[1]]
             self.desc = self.arena[offs[2]:offs[2] + sizes[2]]
             self.tables = self.arena[offs[3]:offs[3] + sizes[3]].view(torch.int32)
@@ -119,6 +137,12 @@ class Session:
         for p in self._plans:
             B.moebius_plan_destroy(p)
         self._plans = []
+        if self.vmm_arena is not None:
+            import torch
+            torch.cuda.synchronize()
+            self.base = None
+            B.moebius_arena_destroy(self.vmm_arena)
+            self.vmm_arena = None
         if self.ctx:
             B.moebius_destroy(self.ctx)
             self.ctx = None

@@ -20,11 +20,12 @@ GUARD = 4096
 CANARY = 0xC3
 
 
-def gpu_session(cfg, lens=None, policy=None, cap_frac=0.0, pool_bytes=None, fill="tag", initial_mode=TP, tma=None):
+def gpu_session(cfg, lens=None, policy=None, cap_frac=0.0, pool_bytes=None, fill="tag", initial_mode=TP, tma=None,
+                vmm=False):
     assert torch.cuda.is_available(), "GPU tests need a CUDA device (there is no CPU fallback)"
     st = State(cfg, lens, fill=fill)
     sess = mb.Session(mb_config(cfg, st.lens, policy, cap_frac, pool_bytes), device="cuda:0", guard_bytes=GUARD,
-                      initial_mode=initial_mode)
+                      initial_mode=initial_mode, vmm=vmm)
     if tma is not None:
         mb.moebius_set_tma(sess.ctx, *tma)
     sess.arena.fill_(CANARY)
@@ -57,13 +58,16 @@ def device_tables(sess, n_req):
     return hdr, owner, lens, bt
 
 
-def gpu_switch(st, sess, from_mode, src_owner, src_bt):
+def gpu_switch(st, sess, from_mode, src_owner, src_bt, execute=None):
     to_mode = EP if from_mode == TP else TP
     plan = sess.plan(to_mode, st.lens, src_owner, src_bt, from_mode=from_mode)
     stats = mb.moebius_plan_stats(plan).as_dict()
     owner, bt = sess.block_tables(plan, len(st.lens))
     want_owner, want_bt = expected_target(st, sess, to_mode)
-    sess.reshard(plan)
+    if execute is None:
+        sess.reshard(plan)
+    else:
+        execute(sess, plan)
     got = download(sess)
     assert mb.moebius_active_mode(sess.ctx) == to_mode
     # tables: host copy and the published device copy, bit-exact with the oracle
@@ -278,4 +282,93 @@ def test_non_power_of_two_shapes(orient, R, E, H, I, Hkv):
     mode, owner, bt, _ = gpu_switch(st, sess, TP, owner, bt)
     mode, owner, bt, _ = gpu_switch(st, sess, mode, owner, bt)
     assert mode == TP
+    sess.close()
+
+
+# ---- peer-mappable unified buffer: one virtual range, one physical allocation per rank (NEXT-1) ----
+
+@pytest.mark.parametrize("name,orient", [("tiny", 0), ("small", 0), ("small", 1)])
+def test_vmm_arena_round_trip(name, orient):
+    """Every rank region is its own physical allocation mapped at base + r * rank_stride (PAPER.md:158,
+    :172: exported once, mapped by peers); planner, kernel and tensor maps run unchanged on it."""
+    cfg = wl.get_config(name).with_(w_orient=orient)
+    st, sess = gpu_session(cfg, vmm=True)
+    assert sess.layout.rank_stride_bytes % (2 << 20) == 0
+    owner, bt, _ = start(st, sess, TP, "random")
+    mode, owner, bt, _ = gpu_switch(st, sess, TP, owner, bt)
+    mode, owner, bt, _ = gpu_switch(st, sess, mode, owner, bt)
+    assert mode == TP
+    sess.close()
+
+
+def test_vmm_arena_export_import():
+    """Arena B creates ranks [0, R/2) itself and imports ranks [R/2, R) from arena A through POSIX file
+    descriptors (what a process does with its peers' regions).  A switch executed on B's range must be
+    visible through A's mapping of the shared ranks: same physical bytes, two virtual addresses."""
+    cfg = wl.get_config("small").with_(L=2, H=128, I=256, n_req=24, len_dist=("uniform", 1, 200), seed=77)
+    st, sess = gpu_session(cfg)            # plain session: used for its context and side buffers
+    R, half = cfg.R, cfg.R // 2
+    stride = sess.layout.rank_stride_bytes
+    A = mb.moebius_arena_create(sess.ctx, 0, half, R)
+    B = mb.moebius_arena_create(sess.ctx, 0, 0, half)
+    assert not mb.moebius_arena_ready(A) and not mb.moebius_arena_ready(B)
+    import os
+    for r in range(half, R):
+        fd = mb.moebius_arena_export(A, r)
+        mb.moebius_arena_import(B, r, fd)
+        os.close(fd)
+    assert mb.moebius_arena_ready(B)
+    with pytest.raises(mb.MoebiusError):
+        mb.moebius_arena_export(B, R - 1)   # not B's own allocation
+    from paper_2606_26607_b200.session import _RawCuda
+    baseB = torch.as_tensor(_RawCuda(mb.moebius_arena_base(B), int(sess.layout.base_bytes)), device="cuda:0")
+    upperA = torch.as_tensor(_RawCuda(mb.moebius_arena_base(A) + half * stride, int((R - half) * stride)), device="cuda:0")
+    mb.moebius_bind(sess.ctx, baseB.data_ptr(), sess.staging.data_ptr(), sess.desc.data_ptr(), sess.tables.data_ptr(), TP)
+    sess.base = baseB
+    owner, bt, _ = start(st, sess, TP, "random")
+    mode, owner, bt, _ = gpu_switch(st, sess, TP, owner, bt)
+    torch.cuda.synchronize()
+    assert torch.equal(upperA, baseB[half * stride:])
+    assert int((upperA != 0xA5).sum()) > 0
+    del baseB, upperA
+    sess.base = None
+    sess.close()
+    mb.moebius_arena_destroy(B)
+    mb.moebius_arena_destroy(A)
+
+
+def share_execute(ranks_per_share):
+    """The multi-GPU form on one GPU: wave by wave, the shares of a wave enqueued one after another (on
+    R GPUs they run concurrently, with a barrier across GPUs after each wave), then publish."""
+    def run(sess, plan):
+        R = sess.cfg.R
+        stream = torch.cuda.current_stream().cuda_stream
+        for wave in range(mb.moebius_plan_waves(plan)):
+            for lo in range(0, R, ranks_per_share):
+                mb.moebius_reshard_share(sess.ctx, plan, lo, min(R, lo + ranks_per_share), wave, stream)
+        mb.moebius_reshard_publish(sess.ctx, plan, stream)
+    return run
+
+
+@pytest.mark.parametrize("ranks_per_share", [1, 2])
+@pytest.mark.parametrize("first", [TP, EP])
+def test_rank_share_execution(first, ranks_per_share):
+    """NEXT-1: every GPU executes only the units of the ranks it owns, one launch per dependency wave.
+    Bit-identical to the fused launch: both must equal the oracle.  Runs on a VMM arena (one physical
+    allocation per rank), from random tables in a tight pool (rounds + staging) and back."""
+    cfg = wl.get_config("small").with_(L=2, H=128, I=256, n_req=30, len_dist=("uniform", 1, 200), seed=61)
+    st, sess = gpu_session(cfg, None, "tight", cap_frac=0.5, initial_mode=first, vmm=True)
+    owner, bt, _ = start(st, sess, first, "random")
+    mode, owner, bt, s1 = gpu_switch(st, sess, first, owner, bt, execute=share_execute(ranks_per_share))
+    mode, owner, bt, s2 = gpu_switch(st, sess, mode, owner, bt, execute=share_execute(ranks_per_share))
+    assert mode == first and max(s1["n_kv_rounds"], s2["n_kv_rounds"]) > 1
+    sess.close()
+
+
+def test_rank_share_execution_fp8_replicated_heads():
+    cfg = wl.get_config("fp8_graph").with_(L=2, E=8, H=256, I=1536, n_req=12, len_dist=("uniform", 1, 90), seed=3)
+    st, sess = gpu_session(cfg, fill="normal", vmm=True)
+    owner, bt, _ = start(st, sess, TP, "random")
+    mode, owner, bt, _ = gpu_switch(st, sess, TP, owner, bt, execute=share_execute(1))
+    mode, owner, bt, _ = gpu_switch(st, sess, mode, owner, bt, execute=share_execute(4))
     sess.close()

@@ -305,3 +305,83 @@ def test_non_power_of_two_shapes(orient, R, E, H, I, Hkv):
     mode, owner, bt, _ = run_switch(st, sess, image, staging, TP, owner, bt)
     mode, owner, bt, _ = run_switch(st, sess, image, staging, EP, owner, bt)
     assert mode == TP
+
+
+# ---- rank-share execution: the plan wave by wave (multi-GPU form) ----------
+
+def wave_barrier_list(plan):
+    """The exported work list re-ordered wave by wave, every wave waiting for ALL of the previous one
+    (a barrier across GPUs): counter w is signalled by every segment of wave w."""
+    segs = mb.moebius_plan_export(plan, 0).copy()
+    waves = mb.moebius_plan_export(plan, 3)
+    assert len(waves) == len(segs) and mb.moebius_plan_waves(plan) == (int(waves.max()) + 1 if len(waves) else 0)
+    order = np.argsort(waves, kind="stable")
+    out = segs[order]
+    w_sorted = waves[order]
+    units = np.array([int(out["n_units"][w_sorted == w].sum()) for w in range(int(w_sorted.max()) + 1)])
+    out["signal_ctr"] = w_sorted
+    out["wait_ctr"] = w_sorted - 1
+    out["wait_target"] = np.where(w_sorted > 0, units[np.maximum(w_sorted - 1, 0)], 0)
+    out["unit_begin"] = np.concatenate([[0], np.cumsum(out["n_units"])[:-1]])
+    return out, w_sorted
+
+
+@pytest.mark.parametrize("first", [TP, EP])
+@pytest.mark.parametrize("policy,orient", [(None, 0), ("tight", 0), (None, 1)])
+def test_waves_with_barriers_are_hazard_free(first, policy, orient):
+    """Executing the plan wave by wave, with nothing ordered inside a wave, is hazard-free and gives the
+    oracle's layout: this is what R GPUs do with one barrier per wave (moebius_reshard_share)."""
+    import ctypes as C
+    from harness import emul_lib
+    cfg = SMALLISH.with_(L=2, n_req=30, seed=41, w_orient=orient)
+    st, sess, image, staging = make(cfg, None, policy, cap_frac=0.5 if policy else 0.0)
+    owner, bt = source_tables(st, sess, first, "random")
+    OracleLayout(st, sess, first, owner, bt).place(image)
+    to = EP if first == TP else TP
+    plan = sess.plan(to, st.lens, owner, bt, from_mode=first)
+    segs, w_sorted = wave_barrier_list(plan)
+    # a dependent segment is always in a later wave than what it waits for
+    orig = mb.moebius_plan_export(plan, 0)
+    waves = mb.moebius_plan_export(plan, 3)
+    for i, s in enumerate(orig):
+        if s["wait_ctr"] >= 0:
+            assert all(waves[j] < waves[i] for j in range(len(orig)) if orig[j]["signal_ctr"] == s["wait_ctr"])
+    kv = mb.moebius_plan_export(plan, 1)
+    c2d = mb.moebius_plan_export(plan, 2)
+    out = np.zeros(8, np.int64)
+    vp = lambda a: a.ctypes.data_as(C.c_void_p) if a.size else None  # noqa: E731
+    emul_lib().emul_run(vp(image), image.size, vp(staging), staging.size, vp(segs), len(segs), vp(kv), vp(c2d),
+                        sess.layout.rank_stride_bytes, vp(out))
+    assert out[0] == 0 and out[1] == 0 and out[2] == 0 and out[3] == 0, out
+    want_owner, want_bt = expected_target(st, sess, to)
+    assert not OracleLayout(st, sess, to, want_owner, want_bt).compare(image)
+    sess.free_plan(plan)
+
+
+@pytest.mark.parametrize("first", [TP, EP])
+@pytest.mark.parametrize("R,Hkv", [(8, 4), (4, 8), (4, 4)])
+def test_share_stats_partition_the_plan(first, R, Hkv):
+    """The rank shares are a disjoint cover of the plan, wave by wave, and the bytes that cross between
+    ranks sum to the owner-changed bytes (oracle/accounting.py enumerates them)."""
+    cfg = SMALLISH.with_(R=R, E=16, kv_heads=Hkv, L=2, n_req=20, seed=51)
+    st, sess, image, staging = make(cfg)
+    owner, bt = source_tables(st, sess, first, "random")
+    to = EP if first == TP else TP
+    plan = sess.plan(to, st.lens, owner, bt, from_mode=first)
+    stats = mb.moebius_plan_stats(plan).as_dict()
+    new_owner, _ = sess.block_tables(plan, len(st.lens))
+    w, k = expected_bytes(st, first, owner if first == EP else new_owner)
+    per_rank = [mb.moebius_share_stats(plan, r, r + 1) for r in range(R)]
+    assert sum(s["units"] for s in per_rank) == stats["n_units"]
+    assert sum(s["cross"] for s in per_rank) == w["moved"] + k["moved"] == stats["w_moved"] + stats["kv_moved"]
+    if stats["n_kv_staged"] == 0:
+        assert sum(s["written"] for s in per_rank) == w["relocated"] + k["relocated"]
+        assert sum(s["read"] for s in per_rank) == w["read"] + k["read"]
+    whole = mb.moebius_share_stats(plan, 0, R)
+    assert whole == {key: sum(s[key] for s in per_rank) for key in whole}
+    n_waves = mb.moebius_plan_waves(plan)
+    by_wave = [mb.moebius_share_stats(plan, 0, R, wv) for wv in range(n_waves)]
+    assert sum(s["units"] for s in by_wave) == stats["n_units"] and all(s["units"] > 0 for s in by_wave)
+    # weights are balanced across ranks by construction; every rank has work in every weight wave
+    assert all(mb.moebius_share_stats(plan, r, r + 1, 0)["units"] > 0 for r in range(R))
+    sess.free_plan(plan)
