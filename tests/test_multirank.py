@@ -59,3 +59,70 @@ def test_product_arm_fails_loudly_without_a_gpu():
     r = subprocess.run([sys.executable, "bench.py", "--steps", "1", "--warmup", "1"], capture_output=True, text=True, cwd=ROOT,
                        timeout=600)
     assert r.returncode != 0 and "no CPU fallback" in (r.stderr + r.stdout)
+
+
+# ---- rank-share form of a switch, host side, world_size 2 on gloo -----------
+
+SHARE_WORKER = r"""
+import os, sys, json, hashlib
+sys.path.insert(0, %r); sys.path.insert(0, os.path.join(%r, "tests"))
+import numpy as np
+import torch, torch.distributed as dist
+import workloads as wl
+import paper_2606_26607_b200 as mb
+from paper_2606_26607_b200 import multiproc
+from harness import mb_config
+dist.init_process_group("gloo")
+rank, world = dist.get_rank(), dist.get_world_size()
+cfg = wl.get_config("small").with_(L=2, H=128, I=256, n_req=30, len_dist=("uniform", 1, 200), seed=61)
+lens = wl.draw_seq_lens(cfg)
+sess = mb.Session(mb_config(cfg, lens, "tight", 0.5))          # host only: the planner
+bt = wl.random_page_tables(lens, None, cfg.R, sess.layout.pages_tp, cfg.page, sess.cfg.max_pages_per_request, seed=7)
+plan = sess.plan(mb.MOEBIUS_EP, lens, None, bt, from_mode=mb.MOEBIUS_TP)
+# 1. every process builds the same plan
+digest = hashlib.sha256(mb.moebius_plan_export(plan, 0).tobytes() + mb.moebius_plan_export(plan, 1).tobytes()
+                        + mb.moebius_plan_export(plan, 3).tobytes()).digest()
+all_d = [None] * world
+dist.all_gather_object(all_d, digest)
+# 2. the shares partition the plan, wave by wave; crossing bytes sum to the owner-changed bytes
+lo, hi = multiproc.owned_ranks(cfg.R, world, rank)
+n_waves = mb.moebius_plan_waves(plan)
+mine = np.array([[mb.moebius_share_stats(plan, lo, hi, w)[k] for k in ("units", "read", "written", "cross")]
+                 for w in range(n_waves)], dtype=np.int64)
+tot = torch.from_numpy(mine.copy())
+dist.all_reduce(tot)
+stats = mb.moebius_plan_stats(plan).as_dict()
+# 3. the fd exchange the arena mapping uses, with ordinary files standing in for the allocations
+fds = {}
+for r in range(lo, hi):
+    f = os.open(os.path.join(sys.argv[1], "region%%d" %% r), os.O_CREAT | os.O_RDWR)
+    os.write(f, b"rank-%%d" %% r)
+    fds[r] = f
+peers = multiproc.exchange_fds(fds, cfg.R, world, rank, sys.argv[1], timeout_s=60)
+seen = {}
+for r, fd in peers.items():
+    os.lseek(fd, 0, os.SEEK_SET)
+    seen[r] = os.read(fd, 64).decode()
+    os.close(fd)
+json.dump({"rank": rank, "same_plan": all(d == digest for d in all_d), "n_waves": n_waves,
+           "units_total": int(tot[:, 0].sum()), "cross_total": int(tot[:, 3].sum()),
+           "n_units": stats["n_units"], "moved": stats["w_moved"] + stats["kv_moved"],
+           "every_wave_has_units": bool((tot[:, 0] > 0).all()), "seen": seen, "owned": [lo, hi]},
+          open(os.path.join(sys.argv[1], "share%%d.json" %% rank), "w"))
+dist.barrier()
+dist.destroy_process_group()
+""" % (ROOT, ROOT)
+
+
+def test_rank_share_host_logic_world2(tmp_path):
+    script = tmp_path / "share_worker.py"
+    script.write_text(SHARE_WORKER)
+    r = torchrun([str(script), str(tmp_path)], 29613)
+    assert r.returncode == 0, r.stderr[-3000:]
+    res = sorted((json.load(open(tmp_path / ("share%d.json" % k))) for k in range(2)), key=lambda x: x["rank"])
+    assert [x["owned"] for x in res] == [[0, 2], [2, 4]]
+    for x in res:
+        assert x["same_plan"] and x["n_waves"] > 2
+        assert x["units_total"] == x["n_units"] and x["cross_total"] == x["moved"]
+        assert x["every_wave_has_units"]
+    assert res[0]["seen"] == {"2": "rank-2", "3": "rank-3"} and res[1]["seen"] == {"0": "rank-0", "1": "rank-1"}
