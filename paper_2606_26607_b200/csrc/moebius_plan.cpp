@@ -681,7 +681,7 @@ extern "C" int moebius_plan(moebius_ctx_t* x, moebius_mode_t from, moebius_mode_
 
   // fp8 block scales: TP and EP scale views live in disjoint fixed regions, so these are plain
   // out-of-place 2-D copies with no hazard (reading A13)
-  if (c.w_dtype == MOEBIUS_FP8_E4M3_B128 && R > 1) {
+  if (c.w_dtype == MOEBIUS_FP8_E4M3_B128) {   // also for R == 1: the two scale views never alias
     const int HB = c.H / 128, IB = c.I / 128, EL = c.E / R;
     for (int l = 0; l < L; ++l) for (int m = 0; m < x->n_obj; ++m) {
       const WObj& ob = x->obj[m];

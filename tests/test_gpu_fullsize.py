@@ -103,17 +103,19 @@ def switch_and_check_tables(sess, st_lens, to, owner, bt, frm, mp, cfg):
     return want_owner, want_bt, stats
 
 
-def test_qwen3_235b_sampled_parity():
+@pytest.mark.parametrize("name", ["qwen3_235b", "qwen3_30b"])
+def test_full_size_sampled_parity(name):
     """BASELINE.json config 4 (R=8, L=12, E=128, H=4096, I=1536 bf16, ~58 GB of experts; 512 requests,
-    lognormal lengths, 4 KV heads on 8 ranks), from seeded random source tables."""
+    lognormal lengths, 4 KV heads on 8 ranks) and config 3 (L=24, H=2048, I=768: 192-byte runs; 256
+    requests; staging capped at 2.4 % of resident bytes), from seeded random source tables."""
     assert torch.cuda.is_available()
-    cfg = wl.get_config("qwen3_235b")
+    cfg = wl.get_config(name)
     lens = wl.draw_seq_lens(cfg)
     sess, mp = bench_session(cfg, lens)
     lay = sess.layout
     assert (lay.weight_spare_bytes + lay.staging_bytes) <= 0.024 * lay.resident_bytes + 1
-    w_samples = [(0, "gate"), (5, "up"), (11, "down")]
-    kv_samples = [(0, 0), (11, 1)]
+    w_samples = [(0, "gate"), (cfg.L // 2 - 1, "up"), (cfg.L - 1, "down")]
+    kv_samples = [(0, 0), (cfg.L - 1, 1)]
     bt0 = wl.random_page_tables(lens, None, cfg.R, lay.pages_tp, cfg.page, mp, seed=cfg.seed)
     devfill.fill_random(sess)
     for l, kind in w_samples:

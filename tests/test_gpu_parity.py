@@ -372,3 +372,31 @@ def test_rank_share_execution_fp8_replicated_heads():
     mode, owner, bt, _ = gpu_switch(st, sess, TP, owner, bt, execute=share_execute(1))
     mode, owner, bt, _ = gpu_switch(st, sess, mode, owner, bt, execute=share_execute(4))
     sess.close()
+
+
+# ---- seeded fuzz on the device: the same draws as tests/test_planner_fuzz.py -------------------------
+
+@pytest.mark.parametrize("seed", range(0, 160, 5))
+def test_fuzz_round_trip_on_device(seed):
+    from test_planner_fuzz import draw_case
+    cfg, policy, first, src, rounds = draw_case(seed)
+    st = State(cfg, fill="normal" if cfg.w_dtype == "fp8_e4m3_b128" else "tag")
+    try:
+        c = mb_config(cfg, st.lens, policy, 0.5 if policy == "tight" else 0.0)
+        sess = mb.Session(c, device="cuda:0", guard_bytes=GUARD, initial_mode=first, vmm=bool(seed % 2))
+    except mb.MoebiusError as e:
+        assert e.status == -3
+        return
+    if rounds:
+        mb.moebius_set_kv_rounds(sess.ctx, rounds)
+    sess.arena.fill_(CANARY)
+    owner, bt, _ = start(st, sess, first, src, seed=seed)
+    mode = first
+    for k in range(2):
+        try:
+            mode, owner, bt, _ = gpu_switch(st, sess, mode, owner, bt,
+                                            execute=share_execute(1) if seed % 3 == 0 else None)
+        except mb.MoebiusError as e:
+            assert e.status == -3 and policy == "tight"
+            break
+    sess.close()
