@@ -237,3 +237,26 @@ def test_status_strings():
     for s in (-1, -2, -3, -4, -5):
         assert mb.moebius_status_str(s) not in ("ok", "unknown")
     assert mb.moebius_version() >= 1
+
+
+def test_header_is_plain_c():
+    """The boundary is a C ABI: include/moebius.h must compile as C99 (and as C++) on its own."""
+    import subprocess
+    hdr = os.path.join(ROOT, "include", "moebius.h")
+    for args in (["gcc", "-std=c99", "-pedantic", "-Wall", "-Werror", "-fsyntax-only", "-x", "c"],
+                 ["g++", "-std=c++17", "-Wall", "-Werror", "-fsyntax-only", "-x", "c++"]):
+        r = subprocess.run(args + [hdr], capture_output=True, text=True)
+        assert r.returncode == 0, r.stderr
+
+
+def test_plain_c_client_links_and_runs(tmp_path):
+    """tests/abi_client.c: a C99 program against include/moebius.h + libmoebius.so, host-only calls."""
+    import subprocess
+    exe = str(tmp_path / "abi_client")
+    lib_dir = os.path.dirname(mb.lib_path())
+    r = subprocess.run(["gcc", "-std=c99", "-Wall", "-Werror", "-I", os.path.join(ROOT, "include"),
+                        os.path.join(ROOT, "tests", "abi_client.c"), "-o", exe, "-L", lib_dir, "-lmoebius",
+                        "-Wl,-rpath," + lib_dir], capture_output=True, text=True)
+    assert r.returncode == 0, r.stderr
+    r = subprocess.run([exe], capture_output=True, text=True, timeout=120)
+    assert r.returncode == 0 and r.stdout.startswith("OK"), r.stdout + r.stderr
