@@ -237,3 +237,62 @@ def test_fp8_graph_stress_fullsize():
                 assert np.array_equal(got[i, :int(lens[i])], KV[(l, kvi)][i][:, heads, :]), (to, r, l, kvi, i)
         mode = to
     sess.close()
+
+
+@pytest.mark.parametrize("name,trips", [("qwen3_30b", 10), ("qwen3_235b", 6)])
+def test_full_size_tight_pool_soak(name, trips):
+    """Full-size shapes with TIGHT pools (max(1.05 x TP need, EP share)): from random tables every switch
+    needs the full schedule -- 66 dependency rounds and hundreds to thousands of staged pages -- in both
+    directions.  After every switch sampled requests are gathered through the new tables (PAPER.md:126:
+    'each resumes decoding at the same position'); after the last the position-weighted checksum of
+    every TP weight view equals the initial one.  Properties that hold at any size."""
+    assert torch.cuda.is_available()
+    cfg = wl.get_config(name)
+    lens = wl.draw_seq_lens(cfg)
+    pool = wl.kv_pool_bytes(cfg, lens, "tight")
+    mp = int(max((int(x) + cfg.page - 1) // cfg.page for x in lens))
+    c = mb.make_config(R=cfg.R, L=cfg.L, E=cfg.E, H=cfg.H, I=cfg.I, w_dtype=cfg.w_dtype, kv_heads=cfg.kv_heads,
+                       head_dim=cfg.head_dim, page_tokens=cfg.page, kv_pool_bytes_per_rank_layer=pool,
+                       max_requests=len(lens), max_pages_per_request=mp, staging_cap_bytes=0)
+    probe = mb.Session(c)
+    c.staging_cap_bytes = int(0.05 * probe.layout.resident_bytes)
+    probe.close()
+    sess = mb.Session(c, device="cuda:0")
+    lay = sess.layout
+    devfill.fill_random(sess)
+    rep = max(1, cfg.R // cfg.kv_heads)
+    for l in range(cfg.L):              # the replicas of a head hold identical bytes under TP (PAPER.md:116)
+        for t in (mb.T_KPOOL, mb.T_VPOOL):
+            for r in range(cfg.R):
+                if r % rep:
+                    sess.view(TP, r, l, t).copy_(sess.view(TP, r - r % rep, l, t))
+    torch.cuda.synchronize()
+    chk0 = view_checksums(sess, cfg, TP)
+    bt = wl.random_page_tables(lens, None, cfg.R, lay.pages_tp, cfg.page, mp, seed=1)
+    samples = (0, len(lens) // 2, len(lens) - 1)
+    last_layer = cfg.L - 1
+
+    def gather(mode, owner, bt):        # head 0 of the sampled requests, K of layer 0 and V of the last layer
+        out = []
+        for i in samples:
+            r = 0 if mode == TP else int(owner[i])
+            pages = torch.from_numpy(bt[i][:(int(lens[i]) + cfg.page - 1) // cfg.page].astype(np.int64)).cuda()
+            for layer, t in ((0, mb.T_KPOOL), (last_layer, mb.T_VPOOL)):
+                v = sess.view(mode, r, layer, t)
+                g = v.index_select(0, pages).reshape(-1, v.shape[2], v.shape[3])[:int(lens[i]), 0, :]
+                out.append(devfill.weighted_checksum(g.contiguous()))
+        return out
+
+    want = gather(TP, None, bt)
+    seen_rounds = seen_staged = 0
+    for k in range(trips):
+        owner_ep, bt_ep, s1 = switch_and_check_tables(sess, lens, EP, None, bt, TP, mp, cfg)
+        assert gather(EP, owner_ep, bt_ep) == want, ("EP", k)
+        _, bt, s2 = switch_and_check_tables(sess, lens, TP, owner_ep, bt_ep, EP, mp, cfg)
+        assert gather(TP, None, bt) == want, ("TP", k)
+        seen_rounds = max(seen_rounds, s1["n_kv_rounds"], s2["n_kv_rounds"])
+        seen_staged = max(seen_staged, s1["n_kv_staged"], s2["n_kv_staged"])
+        assert max(s1["staging_used_bytes"], s2["staging_used_bytes"]) <= lay.staging_bytes
+    assert view_checksums(sess, cfg, TP) == chk0
+    assert seen_rounds > 8 and seen_staged > 100
+    sess.close()
