@@ -157,6 +157,14 @@ __device__ __forceinline__ void tma_store_5d(const CUtensorMap* tm, int c0, int 
   asm volatile("cp.async.bulk.tensor.5d.global.shared::cta.tile.bulk_group [%0, {%1,%2,%3,%4,%5}], [%6];"
                :: "l"(tm), "r"(c0), "r"(c1), "r"(c2), "r"(c3), "r"(c4), "r"(smem_u32(src)) : "memory");
 }
+__device__ __forceinline__ void tma_load_3d(void* dst, const CUtensorMap* tm, int c0, int c1, int c2, uint64_t* bar) {
+  asm volatile("cp.async.bulk.tensor.3d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2,%3,%4}], [%5];"
+               :: "r"(smem_u32(dst)), "l"(tm), "r"(c0), "r"(c1), "r"(c2), "r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void tma_store_3d(const CUtensorMap* tm, int c0, int c1, int c2, const void* src) {
+  asm volatile("cp.async.bulk.tensor.3d.global.shared::cta.tile.bulk_group [%0, {%1,%2,%3}], [%4];"
+               :: "l"(tm), "r"(c0), "r"(c1), "r"(c2), "r"(smem_u32(src)) : "memory");
+}
 __device__ __forceinline__ void bulk_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
 template <int N> __device__ __forceinline__ void bulk_wait_read() { asm volatile("cp.async.bulk.wait_group.read %0;" :: "n"(N) : "memory"); }
 template <int N> __device__ __forceinline__ void bulk_wait() { asm volatile("cp.async.bulk.wait_group %0;" :: "n"(N) : "memory"); }
@@ -171,7 +179,14 @@ struct TmaCtx {
   const DevParams* p;
   const CUtensorMap* tm_w;
   const CUtensorMap* tm_kv;
+  const CUtensorMap* tm_stg;
 };
+
+// Row coordinate (in the staging tensor map) of pool z's copy of staging slot `slot`: the staging
+// buffer is an array of EP-page images, slot-major then pool (moebius_units.h, Seg::stg_pools).
+__device__ __forceinline__ int stg_row(const Seg& s, const DevParams& p, uint32_t slot, uint32_t z) {
+  return (int)((slot * s.stg_pools + (z - s.stg_pool_begin)) * p.page_tokens);
+}
 
 __device__ __forceinline__ KvDesc tma_prefetch_desc(const DevParams& p, const Seg& s, uint32_t ul) {
   KvDesc d = {0, 0, 0, 0};
@@ -217,17 +232,23 @@ __device__ __forceinline__ void tma_issue_load(const TmaCtx& c, const Seg& s, ui
     }
     return;
   }
-  // KT
+  // KT.  The EP side of a unit is the pool page (KV_MOVE), the staging slot (KV_MOVE_STG), or both
+  // (KV_STG_COPY: page -> slot when ep_is_src, slot -> page otherwise); page and slot have the same
+  // image, so the same box through either tensor map.
   uint32_t pb, di;
   kv_unit(s, ul, pb, di);
   const uint32_t nb = seg_boxes(s, ul);
   const uint32_t z0 = s.pool_begin + pb * s.pools_per_unit;
   const uint32_t ntok = d.ntok_slot & 0xFFu;
-  if (s.ep_is_src) {
+  const uint32_t slot = d.ntok_slot >> 8;
+  const bool from_slot = s.kv_mode == KV_MOVE_STG || (s.kv_mode == KV_STG_COPY && !s.ep_is_src);
+  if (s.ep_is_src || s.kv_mode == KV_STG_COPY) {
     if (lane == 0) mbar_expect_tx(bar, nb * s.ep_page_bytes);
     __syncwarp();
-    for (uint32_t k = lane; k < nb; k += 32)
-      tma_load_5d(stage + (size_t)k * s.ep_page_bytes, c.tm_kv, 0, (int)(d.ep_page * p.page_tokens), 0, (int)(z0 + k), d.ep_rank, bar);
+    for (uint32_t k = lane; k < nb; k += 32) {
+      if (from_slot) tma_load_3d(stage + (size_t)k * s.ep_page_bytes, c.tm_stg, 0, stg_row(s, p, slot, z0 + k), 0, bar);
+      else tma_load_5d(stage + (size_t)k * s.ep_page_bytes, c.tm_kv, 0, (int)(d.ep_page * p.page_tokens), 0, (int)(z0 + k), d.ep_rank, bar);
+    }
   } else {
     const uint32_t bytes = ntok * s.run_bytes;
     if (lane == 0) mbar_expect_tx(bar, nb * s.n_groups * bytes);
@@ -273,7 +294,9 @@ __device__ __forceinline__ void tma_issue_store(const TmaCtx& c, const Seg& s, u
   const uint32_t nb = seg_boxes(s, ul);
   const uint32_t z0 = s.pool_begin + pb * s.pools_per_unit;
   const uint32_t ntok = d.ntok_slot & 0xFFu;
-  if (s.ep_is_src) {
+  const uint32_t slot = d.ntok_slot >> 8;
+  const bool to_slot = (s.kv_mode == KV_MOVE_STG && !s.ep_is_src) || (s.kv_mode == KV_STG_COPY && s.ep_is_src);
+  if (s.ep_is_src && s.kv_mode != KV_STG_COPY) {
     const uint32_t bytes = ntok * s.run_bytes;
     const uint32_t per_pool = s.n_groups * s.rep;
     for (uint32_t o = lane; o < nb * per_pool; o += 32) {
@@ -284,8 +307,10 @@ __device__ __forceinline__ void tma_issue_store(const TmaCtx& c, const Seg& s, u
     }
   } else {
     // the whole page box is written: slots past the valid tokens get unspecified bytes (reading A10)
-    for (uint32_t k = lane; k < nb; k += 32)
-      tma_store_5d(c.tm_kv, 0, (int)(d.ep_page * p.page_tokens), 0, (int)(z0 + k), d.ep_rank, stage + (size_t)k * s.ep_page_bytes);
+    for (uint32_t k = lane; k < nb; k += 32) {
+      if (to_slot) tma_store_3d(c.tm_stg, 0, stg_row(s, p, slot, z0 + k), 0, stage + (size_t)k * s.ep_page_bytes);
+      else tma_store_5d(c.tm_kv, 0, (int)(d.ep_page * p.page_tokens), 0, (int)(z0 + k), d.ep_rank, stage + (size_t)k * s.ep_page_bytes);
+    }
   }
   bulk_commit();
 }
@@ -313,7 +338,7 @@ __device__ __forceinline__ void lsu_unit(const Seg& s, const DevParams& p, uint3
 template <int kMinCtasPerSm>   // 1: plans with PATH_TMA segments (shared-memory bound); 2: ld/st-only plans
 __global__ void __launch_bounds__(256, kMinCtasPerSm)
 moebius_reshard_kernel(const __grid_constant__ DevParams p_in, const __grid_constant__ CUtensorMap tm_w,
-                       const __grid_constant__ CUtensorMap tm_kv) {
+                       const __grid_constant__ CUtensorMap tm_kv, const __grid_constant__ CUtensorMap tm_stg) {
   extern __shared__ __align__(1024) char smem[];
   // The arguments are the same for every switch of a context (so that the launch can be replayed
   // from a captured graph); what differs per plan is read from the uploaded image's header.
@@ -335,7 +360,7 @@ moebius_reshard_kernel(const __grid_constant__ DevParams p_in, const __grid_cons
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   __syncwarp();
-  TmaCtx tc{&p, &tm_w, &tm_kv};
+  TmaCtx tc{&p, &tm_w, &tm_kv, &tm_stg};
 
   // pipe state; identical in every lane (it depends on uniform values only)
   bool loading = false;           // a unit's loads are in flight
@@ -519,6 +544,7 @@ static int encode_tmaps(moebius_ctx* x) {
   static_assert(sizeof(CUtensorMap) <= sizeof(x->tmap_w), "CUtensorMap storage");
   memset(x->tmap_w, 0, sizeof(x->tmap_w));
   memset(x->tmap_kv, 0, sizeof(x->tmap_kv));
+  memset(x->tmap_stg, 0, sizeof(x->tmap_stg));
   x->tmaps_valid = true;
   if (!x->use_tma || (!x->xt_ok && !x->kt_ok)) return MOEBIUS_OK;
   void* fn = nullptr;
@@ -549,6 +575,17 @@ static int encode_tmaps(moebius_ctx* x) {
     cuuint32_t box[5] = {(cuuint32_t)(run / 4), (cuuint32_t)c.page_tokens, (cuuint32_t)x->G, 1, 1};
     if (x->pages_ep < 1 ||
         enc((CUtensorMap*)x->tmap_kv, CU_TENSOR_MAP_DATA_TYPE_UINT32, 5, x->base + x->kv_off, dims, strides, box, ones,
+            CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_NONE,
+            CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS) { x->tmaps_valid = false; return MOEBIUS_E_CUDA; }
+  }
+  // staging buffer = an array of EP-page images: [run/4][rows = slots*pg][group G], the same box
+  if (x->kt_ok && x->staging_bytes >= x->ep_page_bytes && x->stg) {
+    const cuuint64_t run = (cuuint64_t)x->run_kv;
+    cuuint64_t dims[3] = {run / 4, (cuuint64_t)(x->staging_bytes / x->ep_page_bytes) * c.page_tokens, (cuuint64_t)x->G};
+    cuuint64_t strides[2] = {run * x->G, run};
+    cuuint32_t box[3] = {(cuuint32_t)(run / 4), (cuuint32_t)c.page_tokens, (cuuint32_t)x->G};
+    if (dims[1] > (1ull << 31) ||
+        enc((CUtensorMap*)x->tmap_stg, CU_TENSOR_MAP_DATA_TYPE_UINT32, 3, x->stg, dims, strides, box, ones,
             CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_NONE,
             CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS) { x->tmaps_valid = false; return MOEBIUS_E_CUDA; }
   }
@@ -668,9 +705,11 @@ int launch_reshard_kernel(moebius_ctx* x, bool tma, int64_t unit_hint, cudaStrea
     if (grid > grid_cap) grid = grid_cap;
   }
   if (tma)
-    moebius_reshard_kernel<1><<<(unsigned)grid, threads, smem, st>>>(p, *(const CUtensorMap*)x->tmap_w, *(const CUtensorMap*)x->tmap_kv);
+    moebius_reshard_kernel<1><<<(unsigned)grid, threads, smem, st>>>(p, *(const CUtensorMap*)x->tmap_w, *(const CUtensorMap*)x->tmap_kv,
+                                                                     *(const CUtensorMap*)x->tmap_stg);
   else
-    moebius_reshard_kernel<2><<<(unsigned)grid, threads, 0, st>>>(p, *(const CUtensorMap*)x->tmap_w, *(const CUtensorMap*)x->tmap_kv);
+    moebius_reshard_kernel<2><<<(unsigned)grid, threads, 0, st>>>(p, *(const CUtensorMap*)x->tmap_w, *(const CUtensorMap*)x->tmap_kv,
+                                                                  *(const CUtensorMap*)x->tmap_stg);
   return cudaGetLastError() == cudaSuccess ? MOEBIUS_OK : MOEBIUS_E_CUDA;
 }
 

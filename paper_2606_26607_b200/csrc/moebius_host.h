@@ -97,6 +97,7 @@ struct moebius_ctx {
   int kt_pools;                   // pools per KV unit
   alignas(64) unsigned char tmap_w[128];   // CUtensorMap storage (encoded at bind time)
   alignas(64) unsigned char tmap_kv[128];
+  alignas(64) unsigned char tmap_stg[128];  // the staging buffer as an array of EP-page images
   bool tmaps_valid;
   size_t smem_set;                // dynamic shared memory the kernel attribute is currently set to
   // device facts + timing (filled lazily by the CUDA side)

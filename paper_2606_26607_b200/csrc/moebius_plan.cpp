@@ -743,7 +743,8 @@ extern "C" int moebius_plan(moebius_ctx_t* x, moebius_mode_t from, moebius_mode_
     uint32_t ppu = kv_tma ? (uint32_t)x->kt_pools : ppu_lsu;
     auto kv_seg = [&](uint32_t mode, uint32_t ep_src, uint32_t d0, uint32_t nd, int pool0, int npool) {
       Seg s = blank_seg();
-      const bool tma = kv_tma && mode == KV_MOVE;
+      const bool tma = kv_tma;   // staged pages too: the staging buffer has its own tensor map (page images)
+      (void)mode;
       const uint32_t ppu = tma ? (uint32_t)x->kt_pools : ppu_lsu;
       s.kind = SEG_KV | ((tma ? PATH_TMA : PATH_LSU) << 8);
       s.kv_mode = mode;

@@ -105,6 +105,18 @@ int emul_run(char* base, int64_t base_bytes, char* stg, int64_t stg_bytes, const
         Box b;
         decode_box(s, p, u, k, b);
         if (b.lin) {
+          if (seg_path(s) == PATH_TMA) {
+            // the device moves the WHOLE page image through the tensor maps: rows past the valid
+            // tokens are read and written too (unspecified bytes, reading A10)
+            ck.on_read(b.lin_src, si, (int)s.ep_page_bytes);
+            ck.on_write(b.lin_dst, si, (int)s.ep_page_bytes);
+            ck.bytes_read -= s.ep_page_bytes - b.lin_bytes;
+            ck.bytes_written -= s.ep_page_bytes - b.lin_bytes;
+            if (ck.chunk_of(b.lin_src) >= 0 && ck.chunk_of(b.lin_dst) >= 0 &&
+                ck.chunk_of(b.lin_src + s.ep_page_bytes - 16) >= 0 && ck.chunk_of(b.lin_dst + s.ep_page_bytes - 16) >= 0)
+              memmove(b.lin_dst, b.lin_src, s.ep_page_bytes);
+            continue;
+          }
           ck.on_read(b.lin_src, si, (int)b.lin_bytes);
           ck.on_write(b.lin_dst, si, (int)b.lin_bytes);
           if (ck.chunk_of(b.lin_src) >= 0 && ck.chunk_of(b.lin_dst) >= 0 &&
