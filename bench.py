@@ -8,8 +8,9 @@ A STEP is one round trip of the whole hot path, TP->EP then EP->TP, over one syn
 relayout, publish).  `value` = owner-changed bytes of both switches / device time (inputs resident
 in HBM, plans built before the timed region, CUDA events round K steps of `moebius_reshard`).
 `e2e` = the same metric through the C ABI starting from HOST inputs (seq_lens, owners and block
-tables in host memory): moebius_plan + moebius_reshard (work-list and table upload) + a device->host
-read-back of the published tables, every switch, timed on the host round a synchronize.  The
+tables in host memory): moebius_plan + moebius_reshard (work-list and table upload) for both switches
+of the step -- the second is planned while the first runs, moebius_reshard only enqueues -- + a
+device->host read-back of the published tables, every step, timed on the host round a synchronize.  The
 weights and the KV cache are resident by the definition of the method (one
 resident copy at fixed addresses), so they are not re-uploaded per step.
 N > 1: independent replicas, one per GPU, no collective; value is the
@@ -367,17 +368,22 @@ def run_moebius(args):
     h2d = d2h = 0
     plan_ms = []
     for _ in range(args.steps):
+        # moebius_reshard only enqueues: the second switch of the step is planned on the host while the
+        # first one runs on the device (its inputs are the first plan's tables, known on the host)
+        live = []
         for to in (EP, TP):
             plan, owner, bt_cur, pms = switch(to, owner, bt_cur, mode)
-            host_tables[:tbl_n].copy_(sess.tables[:tbl_n], non_blocking=True)
-            torch.cuda.synchronize()
-            assert int(host_tables[0]) == to and int(host_tables[1]) == n
             s = mb.moebius_plan_stats(plan)
             h2d += s.desc_upload_bytes + s.table_upload_bytes
-            d2h += tbl_n * 4
             plan_ms.append(pms)
-            sess.free_plan(plan)
+            live.append(plan)
             mode = to
+        host_tables[:tbl_n].copy_(sess.tables[:tbl_n], non_blocking=True)   # the step's result
+        torch.cuda.synchronize()
+        assert int(host_tables[0]) == TP and int(host_tables[1]) == n
+        d2h += tbl_n * 4
+        for plan in live:
+            sess.free_plan(plan)
     e2e_s = time.perf_counter() - t0
     clocks = sampler.summary()
     return locals()

@@ -76,8 +76,11 @@ dist.destroy_process_group()
 @pytest.mark.parametrize("orient", [0, 1])
 def test_two_processes_share_one_switch(tmp_path, orient):
     assert torch.cuda.is_available()
+    import shutil
+    import tempfile
     script = tmp_path / "mp_worker.py"
     script.write_text(WORKER)
+    tmp_path = type(tmp_path)(tempfile.mkdtemp(prefix="mb", dir="/tmp"))   # AF_UNIX paths are limited to 108 bytes
     env = dict(os.environ, MASTER_ADDR="127.0.0.1", OMP_NUM_THREADS="1")
     cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", "2",
            "--master-addr", "127.0.0.1", "--master-port", str(29621 + orient), str(script), str(tmp_path), str(orient)]
@@ -89,3 +92,4 @@ def test_two_processes_share_one_switch(tmp_path, orient):
         assert not x["bad"], x["bad"]
         assert x["waves"][0] > 2                 # tight pool from random tables: real dependency rounds
         assert all(c > 0 for c in x["cross"])    # each process really moved bytes into / out of its peer's regions
+    shutil.rmtree(str(tmp_path), ignore_errors=True)

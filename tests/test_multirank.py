@@ -115,8 +115,11 @@ dist.destroy_process_group()
 
 
 def test_rank_share_host_logic_world2(tmp_path):
+    import shutil
+    import tempfile
     script = tmp_path / "share_worker.py"
     script.write_text(SHARE_WORKER)
+    tmp_path = type(tmp_path)(tempfile.mkdtemp(prefix="mb", dir="/tmp"))   # AF_UNIX paths are limited to 108 bytes
     r = torchrun([str(script), str(tmp_path)], 29613)
     assert r.returncode == 0, r.stderr[-3000:]
     res = sorted((json.load(open(tmp_path / ("share%d.json" % k))) for k in range(2)), key=lambda x: x["rank"])
@@ -126,3 +129,4 @@ def test_rank_share_host_logic_world2(tmp_path):
         assert x["units_total"] == x["n_units"] and x["cross_total"] == x["moved"]
         assert x["every_wave_has_units"]
     assert res[0]["seen"] == {"2": "rank-2", "3": "rank-3"} and res[1]["seen"] == {"0": "rank-0", "1": "rank-1"}
+    shutil.rmtree(str(tmp_path), ignore_errors=True)
