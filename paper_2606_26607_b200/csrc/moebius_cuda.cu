@@ -6,10 +6,14 @@
 // The paper's H200 kernels push slices over NVLink to peers; here the R ranks are regions of one
 // allocation, so the same descriptors drive an on-device relayout bounded by HBM bandwidth.
 //
-// Scheduling: each warp takes unit ids from one global ticket, in list order; a unit is <= ~32 KB.
-// Data path: 16-byte ld.global / st.global with L1 no-allocate, 8 loads in flight per lane, lanes
-// mapped to consecutive 16-byte chunks of the EP-side row so that both sides are accessed in whole
-// contiguous runs (>= one 32-byte sector, usually whole 128-byte lines).
+// Scheduling: each warp takes unit ids from one global ticket, in list order; a unit is <= one
+// shared-memory stage (48 KB by default).  Dependencies (chain links, KV rounds) are device counters.
+// Data path (PATH_TMA, the default): the warps move no data; each is a pipe that issues TMA operations
+// through two shared-memory stages -- tensor-map boxes (cp.async.bulk.tensor) on the EP side, where the
+// box does the run transposition, and contiguous cp.async.bulk copies on the TP side; expert weights,
+// KV pages and staged KV pages alike.  Fallback (PATH_LSU: fp8 scale copies, shapes no box fits, or
+// moebius_set_tma(ctx, 0, ..)): 16-byte ld.global / st.global with L1 no-allocate, 8 loads in flight per
+// lane, lanes on consecutive 16-byte chunks of the EP-side row.
 #include <cuda.h>
 #include <cuda_runtime.h>
 

@@ -37,7 +37,8 @@ enum : uint32_t { KV_MOVE = 0, KV_MOVE_STG = 1, KV_STG_COPY = 2 };
 //             cp.async.bulk.tensor over a 5-D tensor map whose box is the whole unit (the run
 //             transposition happens in the box: smem holds [group][row][run]), the TP side is one
 //             contiguous cp.async.bulk per (group, replica).  Units with a single group (chunks of
-//             long runs, e.g. the down projection) use plain 1-D bulk copies on both sides.
+//             long runs, e.g. the down projection) use plain 1-D bulk copies on both sides.  Staged KV
+//             pages use a second tensor map over the staging buffer (an array of page images).
 enum : uint32_t { PATH_LSU = 0, PATH_TMA = 1 };
 
 struct Seg {              // 128 bytes, uploaded verbatim
