@@ -161,6 +161,17 @@ int moebius_create(const moebius_config_t* c, moebius_ctx_t** out) {
   x->use_tma = 1;
   x->n_pipes = 2;
   x->stage_bytes = 48 * 1024;
+  // A KV unit is a whole number of EP pages: size the stage to a multiple of the page so that no part of
+  // it stays empty, and use the shared memory that frees for more pipes (bytes in flight per SM are
+  // what sets the rate: 2 pipes x 2 stages x 48 KB at 16-KB pages; 3 x 2 x 32 KB at 32-KB pages).
+  if (x->ep_page_bytes % 128 == 0 && x->ep_page_bytes <= 96 * 1024) {
+    const int64_t k = std::max<int64_t>(1, (48 * 1024) / x->ep_page_bytes);
+    const int64_t sb = k * x->ep_page_bytes;
+    if (sb >= 24 * 1024) {
+      x->stage_bytes = sb;
+      x->n_pipes = (int)std::max<int64_t>(1, std::min<int64_t>(4, (208 * 1024) / (2 * sb)));
+    }
+  }
   x->tmaps_valid = false;
   x->smem_set = 0;
   tma_geometry(x);
