@@ -239,7 +239,8 @@ MOEBIUS_API int moebius_kernel_ms_history(moebius_ctx_t* ctx, float* out_ms, int
 
 /* Data-path selection, before the first moebius_plan of a context.  enable != 0 (the default):
  * segments whose shapes allow it run on the TMA path (tensor-map loads/stores through shared memory,
- * `pipes` warps per SM with two `stage_kb` KB stages each; 0 = defaults 2 and 48).  enable == 0:
+ * `pipes` warps per SM with two `stage_kb` KB stages each; 0 = the context's defaults: the stage is a whole
+ * number of EP pages near 48 KB and the pipes fill 208 KB -- 2 and 48 at 16-KB pages).  enable == 0:
  * everything runs on the ld.global/st.global path.  Results are identical either way.  A plan built
  * before the call cannot be executed after it (MOEBIUS_E_STATE).  2*pipes*stage_kb <= 208. */
 MOEBIUS_API int moebius_set_tma(moebius_ctx_t* ctx, int enable, int pipes, int stage_kb);

@@ -92,6 +92,8 @@ struct moebius_ctx {
   int use_tma;                    // planner emits PATH_TMA segments where the shapes allow
   int n_pipes;                    // TMA pipes (warps) per CTA, one CTA per SM
   int64_t stage_bytes;            // bytes of one shared-memory stage; 2 stages per pipe
+  int def_pipes;                  // the defaults moebius_create derived from the EP page size
+  int64_t def_stage_bytes;
   int xt_ok, kt_ok;               // weight / KV tensor maps exist for this config
   int xt_rows;                    // rows of the weight tensor-map box
   int kt_pools;                   // pools per KV unit

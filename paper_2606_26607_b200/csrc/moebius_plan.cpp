@@ -172,6 +172,8 @@ int moebius_create(const moebius_config_t* c, moebius_ctx_t** out) {
       x->n_pipes = (int)std::max<int64_t>(1, std::min<int64_t>(4, (208 * 1024) / (2 * sb)));
     }
   }
+  x->def_pipes = x->n_pipes;
+  x->def_stage_bytes = x->stage_bytes;
   x->tmaps_valid = false;
   x->smem_set = 0;
   tma_geometry(x);
@@ -277,8 +279,8 @@ int moebius_active_mode(const moebius_ctx_t* x) { return x ? x->active_mode : MO
 int moebius_set_tma(moebius_ctx_t* x, int enable, int pipes, int stage_kb) {
   if (!x) return MOEBIUS_E_INVAL;
   if (pipes < 0 || pipes > 8 || stage_kb < 0) return MOEBIUS_E_INVAL;
-  int np = pipes > 0 ? pipes : 2;
-  int64_t sb = stage_kb > 0 ? (int64_t)stage_kb * 1024 : 48 * 1024;
+  int np = pipes > 0 ? pipes : x->def_pipes;
+  int64_t sb = stage_kb > 0 ? (int64_t)stage_kb * 1024 : x->def_stage_bytes;
   if ((int64_t)np * 2 * sb > 208 * 1024) return MOEBIUS_E_INVAL;   // 227 KB per CTA minus barriers and slack
   x->use_tma = enable ? 1 : 0;
   x->n_pipes = np;
