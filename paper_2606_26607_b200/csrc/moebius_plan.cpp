@@ -370,6 +370,677 @@ void moebius::lpt_partition(int n_req, const int32_t* seq_lens, int R, PlanScrat
   }
 }
 
+namespace {
+
+// One moebius_plan call, stage by stage.  The members are what the stages share; every stage returns a
+// moebius_status_t and leaves the context untouched on failure (cancel and retry).
+struct PlanBuilder {
+  moebius_ctx* x;
+  const moebius_config_t& c;
+  const moebius_mode_t from, to;
+  const int32_t n_req;
+  const int32_t *seq_lens, *src_owner, *src_bt;
+  const int R, L, pg, MP;
+  const bool e2t;
+  const int n_pools_all;
+  const int64_t unit_bytes;
+  const int kappa;                       // TP-page granules per EP page
+  PlanScratch& W;                        // warm workspace: no fresh multi-megabyte allocation per switch
+  std::vector<int32_t>&npages, &owner, &bt;
+  std::vector<Move>& mv;
+  int64_t total_pages = 0;
+  int nm = 0, n_staged = 0, K = 0, pools_per_group = 0, n_pool_groups = 0;
+  moebius_plan_t* P = nullptr;
+  uint32_t next_ctr = 0;
+  uint64_t ub = 0;                       // units of the merged list
+  Chain cw, ck, cs;                      // weight chain, KV rounds, scale copies
+
+  PlanBuilder(moebius_ctx* x_, moebius_mode_t from_, moebius_mode_t to_, int32_t n, const int32_t* lens,
+              const int32_t* so, const int32_t* sbt)
+      : x(x_), c(x_->cfg), from(from_), to(to_), n_req(n), seq_lens(lens), src_owner(so), src_bt(sbt),
+        R(c.R), L(c.L), pg(c.page_tokens), MP(c.max_pages_per_request), e2t(from_ == MOEBIUS_EP),
+        n_pools_all(2 * c.L), unit_bytes((int64_t)(x_->unit_kb > 0 ? x_->unit_kb : 32) * 1024), kappa(x_->G),
+        W(x_->scratch), npages(W.npages), owner(W.owner), bt(W.bt), mv(W.mv) {}
+
+  int fail(int code) { moebius_plan_destroy(P); P = nullptr; return code; }
+
+  // ownership and block tables under the target mode
+  int request_state() {
+    // ---- request state under the target mode ----------------------------------------------------
+    npages.assign(n_req, 0);
+    total_pages = 0;
+    for (int i = 0; i < n_req; ++i) {
+      if (seq_lens[i] < 0) return MOEBIUS_E_INVAL;
+      npages[i] = (seq_lens[i] + pg - 1) / pg;
+      if (npages[i] > MP) return MOEBIUS_E_INVAL;
+      total_pages += npages[i];
+      if (e2t && (src_owner[i] < 0 || src_owner[i] >= R)) return MOEBIUS_E_INVAL;
+    }
+    owner.assign(n_req, -1);
+    if (!e2t) {
+      lpt_partition(n_req, seq_lens, R, W, owner.data());
+    }
+    // reading A7: ascending request id, consecutive pages; TP bumps up from 0, EP down from the top.
+    // Only the first npages[i] entries of a row are written here; the -1 padding is laid down when
+    // the table image is built.
+    if (bt.size() < (size_t)n_req * MP) bt.resize((size_t)n_req * MP);
+    if (e2t) {
+      if (total_pages > x->pages_tp) return MOEBIUS_E_CAPACITY;
+      int32_t nxt = 0;
+      for (int i = 0; i < n_req; ++i)
+        for (int b = 0; b < npages[i]; ++b) bt[(size_t)i * MP + b] = nxt++;
+    } else {
+      W.used.assign(R, 0);
+      std::vector<int64_t>& used = W.used;
+      for (int i = 0; i < n_req; ++i) {
+        int r = owner[i];
+        if (used[r] + npages[i] > x->pages_ep) return MOEBIUS_E_CAPACITY;
+        for (int b = 0; b < npages[i]; ++b) bt[(size_t)i * MP + b] = (int32_t)(x->pages_ep - 1 - (used[r] + b));
+        used[r] += npages[i];
+      }
+    }
+    return MOEBIUS_OK;
+  }
+
+  // one move per live (request, block)
+  int kv_moves() {
+    // ---- KV page moves (one per live (request, block); layer- and K/V-agnostic) ----
+    mv.clear();
+    mv.reserve((size_t)total_pages);
+    for (int i = 0; i < n_req; ++i) {
+      for (int b = 0; b < npages[i]; ++b) {
+        Move m;
+        m.req = i; m.blk = b;
+        int32_t sp = src_bt[(size_t)i * MP + b];
+        int32_t dp = bt[(size_t)i * MP + b];
+        if (sp < 0 || sp >= (e2t ? x->pages_ep : x->pages_tp)) return MOEBIUS_E_INVAL;
+        m.ep_rank = e2t ? src_owner[i] : owner[i];
+        m.ep_page = e2t ? sp : dp;
+        m.tp_page = e2t ? dp : sp;
+        m.ntok = std::min(pg, seq_lens[i] - b * pg);
+        m.level = 0; m.slot = -1; m.staged = 0;
+        mv.push_back(m);
+      }
+    }
+    nm = (int)mv.size();
+    {  // source pages must be unique (per owner under EP, globally under TP)
+      std::vector<uint8_t>& seen = W.seen;
+      seen.assign((size_t)(e2t ? R : 1) * (e2t ? x->pages_ep : x->pages_tp), 0);
+      for (const Move& m : mv) {
+        size_t id = e2t ? (size_t)m.ep_rank * x->pages_ep + m.ep_page : (size_t)m.tp_page;
+        if (seen[id]) return MOEBIUS_E_INVAL;
+        seen[id] = 1;
+      }
+    }
+    return MOEBIUS_OK;
+  }
+
+  // hazard graph over the page moves -> dependency rounds + staged pages (bounded staging)
+  int kv_schedule() {
+    // reader[rank*pages_tp + granule] = move that reads it (TP-page-sized granules of a pool).
+    // Hazard graph in CSR form: blk[blk_off[m] .. blk_off[m+1]) = moves that READ what m overwrites
+    // (m must run after them); dep[...] is the transpose (who waits for b).
+    n_staged = 0; K = 0;
+    // Fast path: with the two-ended allocation (reading A7) the targets are TP pages [0, total_pages)
+    // on every rank resp. the top used[r] EP pages of rank r.  If every source page lies outside those
+    // ranges nothing overwrites a live source: one round, no graph needed.
+    bool disjoint = nm > 0;
+    if (nm > 0) {
+      if (e2t) {
+        int64_t min_src = INT64_MAX;
+        for (const Move& m : mv) min_src = std::min<int64_t>(min_src, (int64_t)m.ep_page * kappa);
+        disjoint = min_src >= total_pages;
+      } else {
+        int64_t max_src = -1, min_dst = INT64_MAX;
+        for (const Move& m : mv) max_src = std::max<int64_t>(max_src, m.tp_page);
+        for (int r = 0; r < R; ++r) min_dst = std::min<int64_t>(min_dst, ((int64_t)x->pages_ep - W.used[r]) * kappa);
+        disjoint = max_src < min_dst;
+      }
+    }
+    if (nm > 0 && !disjoint) {
+      std::vector<int32_t>& reader = W.reader;
+      reader.assign((size_t)R * x->pages_tp, -1);
+      auto gid = [&](int rank, int64_t gran) { return (size_t)rank * x->pages_tp + (size_t)gran; };
+      for (int m = 0; m < nm; ++m) {
+        if (e2t) {
+          for (int g = 0; g < kappa; ++g) {
+            int32_t& rd = reader[gid(mv[m].ep_rank, (int64_t)mv[m].ep_page * kappa + g)];
+            if (rd >= 0) return MOEBIUS_E_INVAL;  // source page listed twice
+            rd = m;
+          }
+        } else {
+          for (int g = 0; g < x->G; ++g) {
+            int32_t& rd = reader[gid((int)tp_src_rank((uint32_t)g, (uint32_t)x->rep, mv[m].ep_rank), mv[m].tp_page)];
+            if (rd >= 0) return MOEBIUS_E_INVAL;
+            rd = m;
+          }
+        }
+      }
+      std::vector<int32_t>&blk_off = W.blk_off, &blk = W.blk, &dep_off = W.dep_off, &dep = W.dep;
+      blk_off.assign(nm + 1, 0);
+      blk.clear();
+      dep_off.assign(nm + 1, 0);
+      for (int m = 0; m < nm; ++m) {
+        int32_t bl[64];            // R <= 64, kappa <= R
+        int nb = 0;
+        auto note = [&](int32_t b) {
+          if (b < 0) return;
+          if (b == m) { mv[m].staged = 1; return; }  // a move whose target overlaps its own source
+          bl[nb++] = b;
+        };
+        if (e2t) for (int j = 0; j < R; ++j) note(reader[gid(j, mv[m].tp_page)]);
+        else     for (int g = 0; g < kappa; ++g) note(reader[gid(mv[m].ep_rank, (int64_t)mv[m].ep_page * kappa + g)]);
+        if (nb > 1) {
+          std::sort(bl, bl + nb);
+          nb = (int)(std::unique(bl, bl + nb) - bl);
+        }
+        for (int i = 0; i < nb; ++i) { blk.push_back(bl[i]); dep_off[bl[i] + 1]++; }
+        blk_off[m + 1] = (int32_t)blk.size();
+      }
+      const bool any_edge = !blk.empty();
+      bool any_self = false;
+      for (int m = 0; m < nm; ++m) any_self |= mv[m].staged != 0;
+      if (any_edge) {
+        for (int m = 0; m < nm; ++m) dep_off[m + 1] += dep_off[m];
+        dep.resize(blk.size());
+        W.dep_cur.assign(dep_off.begin(), dep_off.end() - 1);
+        for (int m = 0; m < nm; ++m)
+          for (int32_t e = blk_off[m]; e < blk_off[m + 1]; ++e) dep[W.dep_cur[blk[e]]++] = m;
+      }
+      // Level the DAG of direct moves (Kahn order); a staged move is read in round 0 and written in the
+      // last round.  Cycles are broken by staging one move on the cycle.  Chains longer than
+      // kv_max_level rounds are CUT rather than staged whole: a move whose level would exceed the
+      // limit is staged, so its source is saved in round 0 and everything behind it restarts at
+      // level 1.  A round costs a device-wide drain, a staged page one extra copy: short schedules
+      // with a few percent of staged pages are the cheapest.
+      // No edge at all (the common case: two-ended allocation in a roomy pool) => one round, done.
+      if (any_edge) {
+        std::vector<uint8_t>&self_staged = W.self_staged, &done = W.done;
+        std::vector<int32_t>&indeg = W.indeg, &queue = W.queue, &stamp = W.stamp;
+        self_staged.resize(nm);
+        for (int m = 0; m < nm; ++m) self_staged[m] = mv[m].staged;
+        // If the staged pages of one pool do not fit the staging buffer, allow longer chains (fewer cuts).
+        for (int max_level = x->kv_max_level;; max_level = std::min(kMaxLevelCap, max_level * 4)) {
+          for (int m = 0; m < nm; ++m) mv[m].staged = self_staged[m];
+          indeg.assign(nm, 0);
+          done.assign(nm, 0);
+          queue.clear();
+          queue.reserve(nm);
+          int n_direct = 0;
+          for (int m = 0; m < nm; ++m) {
+            mv[m].level = 0;
+            if (mv[m].staged) { done[m] = 1; continue; }
+            ++n_direct;
+            for (int32_t e = blk_off[m]; e < blk_off[m + 1]; ++e) {
+              if (mv[blk[e]].staged) mv[m].level = 1; else indeg[m]++;
+            }
+          }
+          for (int m = 0; m < nm; ++m) if (!done[m] && indeg[m] == 0) queue.push_back(m);
+          size_t qh = 0;
+          int scan = 0, resolved = 0;
+          stamp.assign(nm, -1);
+          int32_t walk_id = 0;
+          auto release = [&](int m, int lvl) {
+            for (int32_t e = dep_off[m]; e < dep_off[m + 1]; ++e) {
+              const int32_t d = dep[e];
+              if (done[d] || mv[d].staged) continue;
+              mv[d].level = std::max(mv[d].level, lvl);
+              if (--indeg[d] == 0) queue.push_back(d);
+            }
+          };
+          while (resolved < n_direct) {
+            if (qh < queue.size()) {
+              int m = queue[qh++];
+              done[m] = 1;
+              if (mv[m].level > max_level) {        // cut the chain here
+                mv[m].staged = 1; --n_direct;
+                release(m, 1);
+              } else {
+                ++resolved;
+                release(m, mv[m].level + 1);
+              }
+              continue;
+            }
+            // only cycles (and what sits behind them) are left: walk blockers to find a node ON a cycle
+            while (scan < nm && done[scan]) ++scan;
+            int v = scan;
+            ++walk_id;
+            for (;;) {
+              if (stamp[v] == walk_id) break;
+              stamp[v] = walk_id;
+              int nxt = -1;
+              for (int32_t e = blk_off[v]; e < blk_off[v + 1]; ++e)
+                if (!done[blk[e]] && !mv[blk[e]].staged) { nxt = blk[e]; break; }
+              v = nxt;  // exists: indeg[v] > 0
+            }
+            mv[v].staged = 1; done[v] = 1; --n_direct;
+            release(v, 1);
+          }
+          K = 0;
+          int64_t ns = 0;
+          for (int m = 0; m < nm; ++m) { if (!mv[m].staged) K = std::max(K, (int)mv[m].level); else ++ns; }
+          if (ns * x->ep_page_bytes <= x->staging_bytes || max_level >= kMaxLevelCap) break;
+        }
+      } else if (any_self) {
+        // self-overlapping moves only: they are staged; nobody else depends on anything
+        K = 0;
+      }
+      for (int m = 0; m < nm; ++m) if (mv[m].staged) mv[m].slot = n_staged++;
+    }
+    pools_per_group = n_pools_all;
+    if (n_staged > 0) {
+      int64_t per_pool = (int64_t)n_staged * x->ep_page_bytes;
+      int64_t fit = x->staging_bytes / per_pool;
+      if (fit < 1) return MOEBIUS_E_STAGING;
+      pools_per_group = (int)std::min<int64_t>(fit, n_pools_all);
+      if (n_staged >= (1 << 24)) return MOEBIUS_E_STAGING;
+    }
+    n_pool_groups = nm > 0 ? (n_pools_all + pools_per_group - 1) / pools_per_group : 0;
+    return MOEBIUS_OK;
+  }
+
+  // the plan object
+  int new_plan() {
+    // ---- build the plan ---------------------------------------------------------------------------
+    P = new (std::nothrow) moebius_plan_t();
+    if (!P) return MOEBIUS_E_INVAL;
+    P->ctx = x; P->from = from; P->to = to; P->n_req = n_req;
+    P->image = nullptr; P->tbl_image = nullptr; P->kv = nullptr; P->n_kv = 0; P->bt = nullptr;
+    P->buf.p = nullptr; P->buf.bytes = 0; P->buf.pinned = false; P->buf.ev = nullptr;
+    memset(&P->stats, 0, sizeof(P->stats));
+    P->stats.struct_size = sizeof(moebius_stats_t);
+    next_ctr = 0;
+    return MOEBIUS_OK;
+  }
+
+  // expert-weight objects
+  int weight_chain() {
+    // weights: one segment per (layer, matrix) object, chained in the direction-specific order
+    // ("EP->TP adopts the sequential order while TP->EP adopts the reverse order").
+    // Every EP view starts ep_shift slots (= the largest object) behind its TP view, so an object's
+    // write never lands on its own source nor on the source of an object still to come, and the
+    // regions it does overwrite belong to objects earlier in the chain, which have completed
+    // (each link waits for the previous one, transitively for all of them).
+    if (R > 1) {
+      int prev_ctr = -1; uint32_t prev_units = 0;
+      const int n_links = L * x->n_obj;
+      for (int step = 0; step < n_links; ++step) {
+        const int k = e2t ? step : n_links - 1 - step;
+        const int layer = k / x->n_obj;
+        const WObj& ob = x->obj[k % x->n_obj];
+        const int tp_slot = 3 * layer + ob.slot;
+        Seg s = blank_seg();
+        s.kind = SEG_XPOSE;
+        s.ep_is_src = e2t;
+        s.n_groups = R;
+        s.rep = 1;
+        int64_t run = !ob.long_run ? (int64_t)(c.I / R) * x->wb : (int64_t)(c.I / R) * c.H * x->wb;
+        s.rows_total = !ob.long_run ? (uint32_t)(c.E / R) * c.H : (uint32_t)(c.E / R) * ob.row_mult;
+        if (run > (1ll << 31)) return fail(MOEBIUS_E_INVAL);
+        s.run_bytes = (uint32_t)run;
+        s.desc_begin = (uint32_t)(tp_slot + x->ep_shift);   // EP slot index (tensor-map coordinate)
+        const int64_t stage = x->stage_bytes;
+        const uint32_t lt_chunk = pick_chunk(run, stage);
+        if (x->use_tma && !ob.long_run && x->xt_ok) {
+          // one tensor-map box per unit: xt_rows rows x all R groups
+          s.kind = SEG_XPOSE | (PATH_TMA << 8);
+          s.groups_per_unit = R;
+          s.chunk_bytes = (uint32_t)run;
+          s.chunks_per_run = 1;
+          s.rows_per_unit = (uint32_t)x->xt_rows;
+        } else if (x->use_tma && (run > 1024 || run * R > stage) && (lt_chunk == run || lt_chunk >= 4096)) {
+          // one group per unit: plain bulk copies (long runs: the down projection, the W13 stack)
+          s.kind = SEG_XPOSE | (PATH_TMA << 8);
+          s.groups_per_unit = 1;
+          s.chunk_bytes = lt_chunk;
+          s.chunks_per_run = (uint32_t)(run / s.chunk_bytes);
+          s.rows_per_unit = s.chunks_per_run == 1 ? (uint32_t)std::min<int64_t>(32, std::max<int64_t>(1, stage / run)) : 1;
+        } else if (run * R <= unit_bytes || run <= 4096) {
+          s.groups_per_unit = R;
+          s.chunk_bytes = (uint32_t)run;
+          s.chunks_per_run = 1;
+          s.rows_per_unit = (uint32_t)std::max<int64_t>(1, unit_bytes / (run * R));
+        } else {
+          s.groups_per_unit = 1;
+          s.chunk_bytes = pick_chunk(run, unit_bytes);
+          s.chunks_per_run = (uint32_t)(run / s.chunk_bytes);
+          s.rows_per_unit = s.chunks_per_run == 1 ? (uint32_t)std::max<int64_t>(1, unit_bytes / run) : 1;
+        }
+        s.row_blocks = (s.rows_total + s.rows_per_unit - 1) / s.rows_per_unit;
+        s.tp_off = x->w_off + (int64_t)tp_slot * x->S;
+        s.ep_off = x->w_off + (int64_t)(tp_slot + x->ep_shift) * x->S;
+        int64_t nu = (int64_t)R * s.row_blocks * (s.n_groups / s.groups_per_unit) * s.chunks_per_run;
+        if (nu > (1ll << 30)) return fail(MOEBIUS_E_INVAL);
+        s.n_units = (uint32_t)nu;
+        s.wait_ctr = prev_ctr; s.wait_target = prev_units;
+        s.signal_ctr = (int32_t)next_ctr++;
+        prev_ctr = s.signal_ctr; prev_units = s.n_units;
+        push_seg(cw, s);
+      }
+      int64_t all = (int64_t)3 * L * c.E * c.H * c.I * x->wb;
+      P->stats.w_relocated = P->stats.w_read = all;
+      P->stats.w_moved = all / R * (R - 1);
+    }
+    return MOEBIUS_OK;
+  }
+
+  // fp8 block scales
+  int scale_copies() {
+    // fp8 block scales: TP and EP scale views live in disjoint fixed regions, so these are plain
+    // out-of-place 2-D copies with no hazard (reading A13)
+    if (c.w_dtype == MOEBIUS_FP8_E4M3_B128) {   // also for R == 1: the two scale views never alias
+      const int HB = c.H / 128, IB = c.I / 128, EL = c.E / R;
+      for (int l = 0; l < L; ++l) for (int m = 0; m < x->n_obj; ++m) {
+        const WObj& ob = x->obj[m];
+        int64_t tp_within = 0, ep_within = 0;
+        for (int mm = 0; mm < m; ++mm) { tp_within += x->sg[mm].tp_bytes; ep_within += x->sg[mm].ep_bytes; }
+        int prev_hi = 0;
+        for (int j = 0; j < R; ++j) {
+          int lo, hi; scale_blocks(j, R, c.I, &lo, &hi);
+          int nb = hi - lo;
+          int a = e2t ? lo : std::max(lo, prev_hi);   // TP->EP: each EP block is read from its lowest holder
+          prev_hi = std::max(prev_hi, hi);
+          int take = hi - a;
+          if (take <= 0) continue;
+          for (int q = 0; q < R; ++q) {
+            C2dDesc d;
+            int64_t tp_base = (int64_t)j * x->rank_stride + x->scale_tp_off + l * x->scale_tp_layer + tp_within;
+            int64_t ep_base = (int64_t)q * x->rank_stride + x->scale_ep_off + l * x->scale_ep_layer + ep_within;
+            int64_t tp_o, ep_o; uint32_t rows, run, tp_st, ep_st;
+            if (!ob.long_run) {   // TP [E, HB, nb] ; EP [EL, HB, IB]; rows = (e', hb)
+              rows = (uint32_t)EL * HB; run = (uint32_t)take * 4;
+              tp_st = (uint32_t)nb * 4; ep_st = (uint32_t)IB * 4;
+              tp_o = tp_base + ((int64_t)q * EL * HB * nb + (a - lo)) * 4;
+              ep_o = ep_base + (int64_t)a * 4;
+            } else {       // TP [E, mult*nb, HB] ; EP [EL, mult*IB, HB]; rows = (e', gate|up block)
+              const int mult = ob.row_mult;
+              rows = (uint32_t)EL * mult; run = (uint32_t)take * HB * 4;
+              tp_st = (uint32_t)nb * HB * 4; ep_st = (uint32_t)IB * HB * 4;
+              tp_o = tp_base + ((int64_t)q * EL * mult * nb + (a - lo)) * HB * 4;
+              ep_o = ep_base + (int64_t)a * HB * 4;
+            }
+            d.rows = rows; d.run_bytes = run;
+            if (e2t) { d.src_off = ep_o; d.dst_off = tp_o; d.src_stride = ep_st; d.dst_stride = tp_st; }
+            else     { d.src_off = tp_o; d.dst_off = ep_o; d.src_stride = tp_st; d.dst_stride = ep_st; }
+            P->c2d.push_back(d);
+            int64_t bytes = (int64_t)rows * run;
+            P->stats.w_relocated += bytes; P->stats.w_read += bytes;
+            if (q != j) P->stats.w_moved += bytes;
+          }
+        }
+      }
+      Seg s = blank_seg();
+      s.kind = SEG_COPY2D;
+      s.ep_is_src = e2t;          // which side of a descriptor is the EP side (rank-share filter)
+      s.desc_begin = 0;
+      s.n_desc = (uint32_t)P->c2d.size();
+      s.n_units = s.n_desc;
+      push_seg(cs, s);
+    }
+    return MOEBIUS_OK;
+  }
+
+  // KV rounds as segments + byte accounting
+  int kv_segments() {
+    // KV: descriptors ordered [level 0][level 1]...[level K][staged]
+    if (nm > 0) {
+      std::vector<uint32_t>& lvl_begin = W.lvl_begin;
+      lvl_begin.assign(K + 2, 0);
+      for (int m = 0; m < nm; ++m) if (!mv[m].staged) lvl_begin[mv[m].level + 1]++;
+      for (int l = 0; l <= K; ++l) lvl_begin[l + 1] += lvl_begin[l];
+      const uint32_t n_direct = lvl_begin[K + 1];   // the descriptors themselves are written into the image below
+      const uint32_t ppu_lsu = (uint32_t)std::max<int64_t>(1, std::min<int64_t>(unit_bytes / x->ep_page_bytes, 2));
+      const bool kv_tma = x->use_tma && x->kt_ok;
+      uint32_t ppu = kv_tma ? (uint32_t)x->kt_pools : ppu_lsu;
+      auto kv_seg = [&](uint32_t mode, uint32_t ep_src, uint32_t d0, uint32_t nd, int pool0, int npool) {
+        Seg s = blank_seg();
+        const bool tma = kv_tma;   // staged pages too: the staging buffer has its own tensor map (page images)
+        (void)mode;
+        const uint32_t ppu = tma ? (uint32_t)x->kt_pools : ppu_lsu;
+        s.kind = SEG_KV | ((tma ? PATH_TMA : PATH_LSU) << 8);
+        s.kv_mode = mode;
+        s.ep_is_src = ep_src;
+        s.run_bytes = (uint32_t)x->run_kv;
+        s.n_groups = (uint32_t)x->G;
+        s.rep = (uint32_t)x->rep;
+        s.ep_off = s.tp_off = x->kv_off;
+        s.desc_begin = d0; s.n_desc = nd;
+        s.pool_begin = (uint32_t)pool0; s.n_pools = (uint32_t)npool;
+        s.pools_per_unit = std::min<uint32_t>(ppu, (uint32_t)npool);
+        s.ep_page_bytes = (uint32_t)x->ep_page_bytes;
+        s.tp_page_bytes = (uint32_t)x->tp_page_bytes;
+        s.pool_bytes = x->pool_bytes;
+        s.stg_pool_begin = (uint32_t)pool0;
+        s.stg_pools = (uint32_t)npool;
+        uint32_t pool_blocks = (s.n_pools + s.pools_per_unit - 1) / s.pools_per_unit;
+        s.n_units = nd * pool_blocks;
+        return s;
+      };
+      // a round = every segment that signals the same counter; the next round waits for all of them
+      const int64_t kv_units_est = (int64_t)nm * ((n_pools_all + ppu - 1) / ppu);
+      const int64_t slice_units = std::max<int64_t>(8192, kv_units_est / std::max(1, 3 * L));
+      int prev_ctr = -1; uint32_t prev_total = 0;
+      for (int g = 0; g < n_pool_groups; ++g) {
+        int pool0 = g * pools_per_group;
+        int npool = std::min(pools_per_group, n_pools_all - pool0);
+        for (int round = 0; round <= K + 1; ++round) {
+          std::vector<Seg> parts;
+          if (round == 0 && n_staged)      // save staged sources: EP->TP copies the EP page, TP->EP gathers into the slot
+            parts.push_back(kv_seg(e2t ? KV_STG_COPY : KV_MOVE_STG, e2t ? 1u : 0u, n_direct, (uint32_t)n_staged, pool0, npool));
+          if (round <= K && lvl_begin[round + 1] > lvl_begin[round])
+            parts.push_back(kv_seg(KV_MOVE, e2t ? 1u : 0u, lvl_begin[round], lvl_begin[round + 1] - lvl_begin[round], pool0, npool));
+          if (round == K + 1 && n_staged)  // every source has been read by now
+            parts.push_back(kv_seg(e2t ? KV_MOVE_STG : KV_STG_COPY, e2t ? 1u : 0u, n_direct, (uint32_t)n_staged, pool0, npool));
+          uint32_t total = 0;
+          for (auto& s : parts) total += s.n_units;
+          if (!total) continue;
+          if (next_ctr >= (uint32_t)kMaxCounters) return fail(MOEBIUS_E_STAGING);
+          int ctr = (int)next_ctr++;
+          for (auto& s : parts) {
+            // slice long segments so they interleave with the weight chain (drains of one hide behind the other)
+            uint32_t pool_blocks = (s.n_pools + s.pools_per_unit - 1) / s.pools_per_unit;
+            uint32_t desc_per_slice = (uint32_t)std::max<int64_t>(1, slice_units / pool_blocks);
+            for (uint32_t d0 = 0; d0 < s.n_desc; d0 += desc_per_slice) {
+              Seg t = s;
+              t.desc_begin = s.desc_begin + d0;
+              t.n_desc = std::min(desc_per_slice, s.n_desc - d0);
+              t.n_units = t.n_desc * pool_blocks;
+              t.wait_ctr = prev_ctr; t.wait_target = prev_total;
+              t.signal_ctr = ctr;
+              push_seg(ck, t);
+            }
+          }
+          prev_ctr = ctr; prev_total = total;
+        }
+      }
+      // accounting (reading A15): per pool, per move
+      for (int m = 0; m < nm; ++m) {
+        int64_t row = (int64_t)mv[m].ntok * x->run_kv;     // one group's bytes of this page
+        if (e2t) {
+          P->stats.kv_read += row * x->G;
+          P->stats.kv_relocated += row * x->G * x->rep;
+          P->stats.kv_moved += row * (x->G * x->rep - 1);  // the owner's own shard stays on its rank
+        } else {
+          P->stats.kv_read += row * x->G;
+          P->stats.kv_relocated += row * x->G;
+          P->stats.kv_moved += row * (x->G - 1);           // the new owner always holds one group itself
+        }
+      }
+      P->stats.kv_read *= n_pools_all; P->stats.kv_relocated *= n_pools_all; P->stats.kv_moved *= n_pools_all;
+    }
+    return MOEBIUS_OK;
+  }
+
+  // one ordered list; dependency waves
+  int merge_and_waves() {
+    // merge the chains by fractional position (each keeps its own order)
+    struct Item { double pos; int chain; size_t idx; };
+    std::vector<Item> items;
+    auto add_chain = [&](Chain& ch, int id) {
+      int64_t acc = 0;
+      for (size_t i = 0; i < ch.segs.size(); ++i) {
+        items.push_back({ch.units ? (acc + 0.5 * ch.segs[i].n_units) / (double)ch.units : 0.0, id, i});
+        acc += ch.segs[i].n_units;
+      }
+    };
+    add_chain(cs, 0); add_chain(cw, 1); add_chain(ck, 2);
+    std::stable_sort(items.begin(), items.end(), [](const Item& a, const Item& b) {
+      if (a.chain == 0 || b.chain == 0) return a.chain == 0 && b.chain != 0;
+      return a.pos < b.pos;
+    });
+    ub = 0;
+    for (auto& it : items) {
+      Seg s = (it.chain == 0 ? cs : it.chain == 1 ? cw : ck).segs[it.idx];
+      s.unit_begin = (uint32_t)ub;
+      ub += s.n_units;
+      P->segs.push_back(s);
+    }
+    if (ub >= (1ull << 32) || P->segs.size() > (size_t)kMaxSegs || (int64_t)nm > x->max_kv_desc ||
+        P->c2d.size() > (size_t)x->max_c2d)
+      return fail(MOEBIUS_E_INVAL);
+    P->total_units = (uint32_t)ub;
+    P->n_counters = next_ctr;
+    P->uses_tma = false;
+    for (const Seg& s : P->segs) if (seg_path(s) == PATH_TMA) P->uses_tma = true;
+    P->stage_bytes = x->stage_bytes;
+    P->xt_rows = x->xt_rows;
+
+    // Waves: wave(s) = 0 without a dependency, else 1 + the latest wave among the segments that signal
+    // the counter s waits on.  A multi-GPU run executes wave by wave with a barrier across GPUs in
+    // between (one barrier per dependency round); the fused launch ignores them.
+    std::vector<int32_t>& seg_wave = P->seg_wave;
+    seg_wave.assign(P->segs.size(), 0);
+    {
+      std::vector<int32_t> ctr_wave(next_ctr ? next_ctr : 1, -1);
+      int32_t n_waves = P->segs.empty() ? 0 : 1;
+      for (size_t i = 0; i < P->segs.size(); ++i) {
+        const Seg& sg = P->segs[i];
+        int32_t w = sg.wait_ctr >= 0 ? ctr_wave[(size_t)sg.wait_ctr] + 1 : 0;
+        seg_wave[i] = w;
+        if (sg.signal_ctr >= 0) ctr_wave[(size_t)sg.signal_ctr] = std::max(ctr_wave[(size_t)sg.signal_ctr], w);
+        n_waves = std::max(n_waves, w + 1);
+      }
+      P->n_waves = n_waves;
+    }
+    return MOEBIUS_OK;
+  }
+
+  // upload images
+  int build_images() {
+    const std::vector<int32_t>& seg_wave = P->seg_wave;
+    // ---- target request state + upload images (written in place: [segs][kv][c2d][waves] | tables) ---
+    P->lens.assign(seq_lens, seq_lens + n_req);
+    P->owner = owner;
+    int64_t seg_b = align_up((int64_t)P->segs.size() * sizeof(Seg), 256);
+    int64_t kv_b = align_up((int64_t)nm * sizeof(KvDesc), 256);
+    int64_t c2d_b = align_up((int64_t)P->c2d.size() * sizeof(C2dDesc), 256);
+    const int64_t hdr_b = sizeof(PlanHdr);
+    P->kv_img_off = hdr_b + seg_b;
+    P->c2d_img_off = hdr_b + seg_b + kv_b;
+    P->wave_img_off = hdr_b + seg_b + kv_b + c2d_b;
+    const int64_t wave_b = (int64_t)P->n_waves * hdr_b + (int64_t)P->segs.size() * (int64_t)sizeof(Seg);
+    P->image_bytes = P->wave_img_off + wave_b;
+    if (kSegOff + P->image_bytes > x->desc_bytes) return fail(MOEBIUS_E_INVAL);
+    P->tbl_bytes = 4 * ((int64_t)kTblHdrInts + 2 * (int64_t)c.max_requests + (int64_t)n_req * MP);
+    if (!image_acquire(x, P->image_bytes + P->tbl_bytes + 256, &P->buf)) return fail(MOEBIUS_E_INVAL);
+    P->image = P->buf.p;
+    {
+      PlanHdr* h = (PlanHdr*)P->image;
+      memset(h, 0, sizeof(PlanHdr));
+      h->n_segs = (uint32_t)P->segs.size();
+      h->total_units = P->total_units;
+      h->kv_off = (uint32_t)P->kv_img_off;
+      h->c2d_off = (uint32_t)P->c2d_img_off;
+    }
+    if (!P->segs.empty()) {
+      memcpy(P->image + hdr_b, P->segs.data(), P->segs.size() * sizeof(Seg));
+      memset(P->image + hdr_b + P->segs.size() * sizeof(Seg), 0, (size_t)(seg_b - (int64_t)(P->segs.size() * sizeof(Seg))));
+    }
+    {  // KV descriptors ordered [level 0][level 1]...[level K][staged]
+      KvDesc* kvd = (KvDesc*)(P->image + P->kv_img_off);
+      P->kv = kvd;
+      P->n_kv = nm;
+      if (nm > 0) {
+        std::vector<uint32_t>& cur = W.cur;
+        cur.assign(W.lvl_begin.begin(), W.lvl_begin.end() - 1);
+        uint32_t scur = W.lvl_begin[K + 1];
+        for (int m = 0; m < nm; ++m) {
+          KvDesc d;
+          d.ep_rank = mv[m].ep_rank; d.ep_page = mv[m].ep_page; d.tp_page = mv[m].tp_page;
+          d.ntok_slot = (uint32_t)mv[m].ntok | (mv[m].staged ? ((uint32_t)mv[m].slot << 8) : 0u);
+          if (mv[m].staged) kvd[scur++] = d; else kvd[cur[mv[m].level]++] = d;
+        }
+      }
+      memset(P->image + P->kv_img_off + (int64_t)nm * sizeof(KvDesc), 0, (size_t)(kv_b - (int64_t)nm * (int64_t)sizeof(KvDesc)));
+    }
+    if (c2d_b) {
+      memcpy(P->image + P->c2d_img_off, P->c2d.data(), P->c2d.size() * sizeof(C2dDesc));
+      memset(P->image + P->c2d_img_off + P->c2d.size() * sizeof(C2dDesc), 0, (size_t)(c2d_b - (int64_t)(P->c2d.size() * sizeof(C2dDesc))));
+    }
+    {  // per wave: a header + that wave's segments with their own unit numbering and no dependencies;
+       // descriptor offsets are relative to the wave's header (negative: the arrays sit before it)
+      P->wave_hdr_off.assign((size_t)P->n_waves, 0);
+      P->wave_units.assign((size_t)P->n_waves, 0);
+      int64_t at = P->wave_img_off;
+      for (int32_t w = 0; w < P->n_waves; ++w) {
+        PlanHdr* h = (PlanHdr*)(P->image + at);
+        memset(h, 0, sizeof(PlanHdr));
+        P->wave_hdr_off[(size_t)w] = at;
+        Seg* out_segs = (Seg*)(P->image + at + hdr_b);
+        uint32_t n = 0, units = 0;
+        bool tma = false;
+        for (size_t i = 0; i < P->segs.size(); ++i) {
+          if (seg_wave[i] != w) continue;
+          Seg t = P->segs[i];
+          t.wait_ctr = -1; t.signal_ctr = -1;
+          t.unit_begin = units;
+          units += t.n_units;
+          tma |= seg_path(t) == PATH_TMA;
+          out_segs[n++] = t;
+        }
+        h->n_segs = n;
+        h->total_units = units;
+        h->kv_off = (uint32_t)(int32_t)(P->kv_img_off - at);
+        h->c2d_off = (uint32_t)(int32_t)(P->c2d_img_off - at);
+        P->wave_units[(size_t)w] = units;
+        at += hdr_b + (int64_t)n * (int64_t)sizeof(Seg);
+      }
+    }
+    P->tbl_image = (int32_t*)(P->image + align_up(P->image_bytes, 256));
+    int32_t* T = P->tbl_image;
+    memset(T, 0, kTblHdrInts * 4);
+    T[0] = to; T[1] = n_req; T[2] = c.max_requests; T[3] = MP;
+    for (int i = 0; i < c.max_requests; ++i) { T[kTblHdrInts + i] = -1; T[kTblHdrInts + c.max_requests + i] = 0; }
+    for (int i = 0; i < n_req; ++i) { T[kTblHdrInts + i] = owner[i]; T[kTblHdrInts + c.max_requests + i] = seq_lens[i]; }
+    {
+      int32_t* tb = T + kTblHdrInts + 2 * c.max_requests;
+      for (int i = 0; i < n_req; ++i) {
+        int32_t* row = tb + (size_t)i * MP;
+        memcpy(row, bt.data() + (size_t)i * MP, (size_t)npages[i] * 4);
+        for (int b = npages[i]; b < MP; ++b) row[b] = -1;
+      }
+      P->bt = tb;
+    }
+    return MOEBIUS_OK;
+  }
+
+  // statistics
+  int finish_stats() {
+    P->stats.n_segments = (int32_t)P->segs.size();
+    P->stats.n_kv_moves = nm;
+    P->stats.n_kv_rounds = nm ? K + 1 + (n_staged ? 1 : 0) : 0;
+    P->stats.n_kv_staged = n_staged;
+    P->stats.n_pool_groups = n_pool_groups;
+    P->stats.n_units = (int64_t)ub;
+    P->stats.staging_used_bytes = (int64_t)n_staged * x->ep_page_bytes * (n_staged ? pools_per_group : 0);
+    P->stats.desc_upload_bytes = P->image_bytes;
+    P->stats.table_upload_bytes = P->tbl_bytes;
+    return MOEBIUS_OK;
+  }
+};
+
+}  // namespace
+
 extern "C" int moebius_plan(moebius_ctx_t* x, moebius_mode_t from, moebius_mode_t to, int32_t n_req,
                             const int32_t* seq_lens, const int32_t* src_owner, const int32_t* src_bt,
                             moebius_plan_t** out) {
@@ -380,611 +1051,14 @@ extern "C" int moebius_plan(moebius_ctx_t* x, moebius_mode_t from, moebius_mode_
   if (n_req < 0 || n_req > c.max_requests) return MOEBIUS_E_INVAL;
   if (n_req > 0 && (!seq_lens || !src_bt)) return MOEBIUS_E_INVAL;
   if (n_req > 0 && from == MOEBIUS_EP && !src_owner) return MOEBIUS_E_INVAL;
-  const int R = c.R, L = c.L, pg = c.page_tokens, MP = c.max_pages_per_request;
-  const bool e2t = from == MOEBIUS_EP;
-  const int n_pools_all = 2 * L;
-  const int64_t unit_bytes = (int64_t)(x->unit_kb > 0 ? x->unit_kb : 32) * 1024;
-
-  // ---- request state under the target mode ----------------------------------------------------
-  PlanScratch& W = x->scratch;   // warm workspace: no fresh multi-megabyte allocation per switch
-  std::vector<int32_t>& npages = W.npages;
-  npages.assign(n_req, 0);
-  int64_t total_pages = 0;
-  for (int i = 0; i < n_req; ++i) {
-    if (seq_lens[i] < 0) return MOEBIUS_E_INVAL;
-    npages[i] = (seq_lens[i] + pg - 1) / pg;
-    if (npages[i] > MP) return MOEBIUS_E_INVAL;
-    total_pages += npages[i];
-    if (e2t && (src_owner[i] < 0 || src_owner[i] >= R)) return MOEBIUS_E_INVAL;
-  }
-  std::vector<int32_t>& owner = W.owner;
-  owner.assign(n_req, -1);
-  if (!e2t) {
-    lpt_partition(n_req, seq_lens, R, W, owner.data());
-  }
-  // reading A7: ascending request id, consecutive pages; TP bumps up from 0, EP down from the top.
-  // Only the first npages[i] entries of a row are written here; the -1 padding is laid down when
-  // the table image is built.
-  std::vector<int32_t>& bt = W.bt;
-  if (bt.size() < (size_t)n_req * MP) bt.resize((size_t)n_req * MP);
-  if (e2t) {
-    if (total_pages > x->pages_tp) return MOEBIUS_E_CAPACITY;
-    int32_t nxt = 0;
-    for (int i = 0; i < n_req; ++i)
-      for (int b = 0; b < npages[i]; ++b) bt[(size_t)i * MP + b] = nxt++;
-  } else {
-    W.used.assign(R, 0);
-    std::vector<int64_t>& used = W.used;
-    for (int i = 0; i < n_req; ++i) {
-      int r = owner[i];
-      if (used[r] + npages[i] > x->pages_ep) return MOEBIUS_E_CAPACITY;
-      for (int b = 0; b < npages[i]; ++b) bt[(size_t)i * MP + b] = (int32_t)(x->pages_ep - 1 - (used[r] + b));
-      used[r] += npages[i];
-    }
-  }
-
-  // ---- KV page moves (one per live (request, block); layer- and K/V-agnostic) ----
-  const int kappa = x->G;  // TP-page granules per EP page
-  std::vector<Move>& mv = W.mv;
-  mv.clear();
-  mv.reserve((size_t)total_pages);
-  for (int i = 0; i < n_req; ++i) {
-    for (int b = 0; b < npages[i]; ++b) {
-      Move m;
-      m.req = i; m.blk = b;
-      int32_t sp = src_bt[(size_t)i * MP + b];
-      int32_t dp = bt[(size_t)i * MP + b];
-      if (sp < 0 || sp >= (e2t ? x->pages_ep : x->pages_tp)) return MOEBIUS_E_INVAL;
-      m.ep_rank = e2t ? src_owner[i] : owner[i];
-      m.ep_page = e2t ? sp : dp;
-      m.tp_page = e2t ? dp : sp;
-      m.ntok = std::min(pg, seq_lens[i] - b * pg);
-      m.level = 0; m.slot = -1; m.staged = 0;
-      mv.push_back(m);
-    }
-  }
-  const int nm = (int)mv.size();
-  {  // source pages must be unique (per owner under EP, globally under TP)
-    std::vector<uint8_t>& seen = W.seen;
-    seen.assign((size_t)(e2t ? R : 1) * (e2t ? x->pages_ep : x->pages_tp), 0);
-    for (const Move& m : mv) {
-      size_t id = e2t ? (size_t)m.ep_rank * x->pages_ep + m.ep_page : (size_t)m.tp_page;
-      if (seen[id]) return MOEBIUS_E_INVAL;
-      seen[id] = 1;
-    }
-  }
-  // reader[rank*pages_tp + granule] = move that reads it (TP-page-sized granules of a pool).
-  // Hazard graph in CSR form: blk[blk_off[m] .. blk_off[m+1]) = moves that READ what m overwrites
-  // (m must run after them); dep[...] is the transpose (who waits for b).
-  int n_staged = 0, K = 0;
-  // Fast path: with the two-ended allocation (reading A7) the targets are TP pages [0, total_pages)
-  // on every rank resp. the top used[r] EP pages of rank r.  If every source page lies outside those
-  // ranges nothing overwrites a live source: one round, no graph needed.
-  bool disjoint = nm > 0;
-  if (nm > 0) {
-    if (e2t) {
-      int64_t min_src = INT64_MAX;
-      for (const Move& m : mv) min_src = std::min<int64_t>(min_src, (int64_t)m.ep_page * kappa);
-      disjoint = min_src >= total_pages;
-    } else {
-      int64_t max_src = -1, min_dst = INT64_MAX;
-      for (const Move& m : mv) max_src = std::max<int64_t>(max_src, m.tp_page);
-      for (int r = 0; r < R; ++r) min_dst = std::min<int64_t>(min_dst, ((int64_t)x->pages_ep - W.used[r]) * kappa);
-      disjoint = max_src < min_dst;
-    }
-  }
-  if (nm > 0 && !disjoint) {
-    std::vector<int32_t>& reader = W.reader;
-    reader.assign((size_t)R * x->pages_tp, -1);
-    auto gid = [&](int rank, int64_t gran) { return (size_t)rank * x->pages_tp + (size_t)gran; };
-    for (int m = 0; m < nm; ++m) {
-      if (e2t) {
-        for (int g = 0; g < kappa; ++g) {
-          int32_t& rd = reader[gid(mv[m].ep_rank, (int64_t)mv[m].ep_page * kappa + g)];
-          if (rd >= 0) return MOEBIUS_E_INVAL;  // source page listed twice
-          rd = m;
-        }
-      } else {
-        for (int g = 0; g < x->G; ++g) {
-          int32_t& rd = reader[gid((int)tp_src_rank((uint32_t)g, (uint32_t)x->rep, mv[m].ep_rank), mv[m].tp_page)];
-          if (rd >= 0) return MOEBIUS_E_INVAL;
-          rd = m;
-        }
-      }
-    }
-    std::vector<int32_t>&blk_off = W.blk_off, &blk = W.blk, &dep_off = W.dep_off, &dep = W.dep;
-    blk_off.assign(nm + 1, 0);
-    blk.clear();
-    dep_off.assign(nm + 1, 0);
-    for (int m = 0; m < nm; ++m) {
-      int32_t bl[64];            // R <= 64, kappa <= R
-      int nb = 0;
-      auto note = [&](int32_t b) {
-        if (b < 0) return;
-        if (b == m) { mv[m].staged = 1; return; }  // a move whose target overlaps its own source
-        bl[nb++] = b;
-      };
-      if (e2t) for (int j = 0; j < R; ++j) note(reader[gid(j, mv[m].tp_page)]);
-      else     for (int g = 0; g < kappa; ++g) note(reader[gid(mv[m].ep_rank, (int64_t)mv[m].ep_page * kappa + g)]);
-      if (nb > 1) {
-        std::sort(bl, bl + nb);
-        nb = (int)(std::unique(bl, bl + nb) - bl);
-      }
-      for (int i = 0; i < nb; ++i) { blk.push_back(bl[i]); dep_off[bl[i] + 1]++; }
-      blk_off[m + 1] = (int32_t)blk.size();
-    }
-    const bool any_edge = !blk.empty();
-    bool any_self = false;
-    for (int m = 0; m < nm; ++m) any_self |= mv[m].staged != 0;
-    if (any_edge) {
-      for (int m = 0; m < nm; ++m) dep_off[m + 1] += dep_off[m];
-      dep.resize(blk.size());
-      W.dep_cur.assign(dep_off.begin(), dep_off.end() - 1);
-      for (int m = 0; m < nm; ++m)
-        for (int32_t e = blk_off[m]; e < blk_off[m + 1]; ++e) dep[W.dep_cur[blk[e]]++] = m;
-    }
-    // Level the DAG of direct moves (Kahn order); a staged move is read in round 0 and written in the
-    // last round.  Cycles are broken by staging one move on the cycle.  Chains longer than
-    // kv_max_level rounds are CUT rather than staged whole: a move whose level would exceed the
-    // limit is staged, so its source is saved in round 0 and everything behind it restarts at
-    // level 1.  A round costs a device-wide drain, a staged page one extra copy: short schedules
-    // with a few percent of staged pages are the cheapest.
-    // No edge at all (the common case: two-ended allocation in a roomy pool) => one round, done.
-    if (any_edge) {
-      std::vector<uint8_t>&self_staged = W.self_staged, &done = W.done;
-      std::vector<int32_t>&indeg = W.indeg, &queue = W.queue, &stamp = W.stamp;
-      self_staged.resize(nm);
-      for (int m = 0; m < nm; ++m) self_staged[m] = mv[m].staged;
-      // If the staged pages of one pool do not fit the staging buffer, allow longer chains (fewer cuts).
-      for (int max_level = x->kv_max_level;; max_level = std::min(kMaxLevelCap, max_level * 4)) {
-        for (int m = 0; m < nm; ++m) mv[m].staged = self_staged[m];
-        indeg.assign(nm, 0);
-        done.assign(nm, 0);
-        queue.clear();
-        queue.reserve(nm);
-        int n_direct = 0;
-        for (int m = 0; m < nm; ++m) {
-          mv[m].level = 0;
-          if (mv[m].staged) { done[m] = 1; continue; }
-          ++n_direct;
-          for (int32_t e = blk_off[m]; e < blk_off[m + 1]; ++e) {
-            if (mv[blk[e]].staged) mv[m].level = 1; else indeg[m]++;
-          }
-        }
-        for (int m = 0; m < nm; ++m) if (!done[m] && indeg[m] == 0) queue.push_back(m);
-        size_t qh = 0;
-        int scan = 0, resolved = 0;
-        stamp.assign(nm, -1);
-        int32_t walk_id = 0;
-        auto release = [&](int m, int lvl) {
-          for (int32_t e = dep_off[m]; e < dep_off[m + 1]; ++e) {
-            const int32_t d = dep[e];
-            if (done[d] || mv[d].staged) continue;
-            mv[d].level = std::max(mv[d].level, lvl);
-            if (--indeg[d] == 0) queue.push_back(d);
-          }
-        };
-        while (resolved < n_direct) {
-          if (qh < queue.size()) {
-            int m = queue[qh++];
-            done[m] = 1;
-            if (mv[m].level > max_level) {        // cut the chain here
-              mv[m].staged = 1; --n_direct;
-              release(m, 1);
-            } else {
-              ++resolved;
-              release(m, mv[m].level + 1);
-            }
-            continue;
-          }
-          // only cycles (and what sits behind them) are left: walk blockers to find a node ON a cycle
-          while (scan < nm && done[scan]) ++scan;
-          int v = scan;
-          ++walk_id;
-          for (;;) {
-            if (stamp[v] == walk_id) break;
-            stamp[v] = walk_id;
-            int nxt = -1;
-            for (int32_t e = blk_off[v]; e < blk_off[v + 1]; ++e)
-              if (!done[blk[e]] && !mv[blk[e]].staged) { nxt = blk[e]; break; }
-            v = nxt;  // exists: indeg[v] > 0
-          }
-          mv[v].staged = 1; done[v] = 1; --n_direct;
-          release(v, 1);
-        }
-        K = 0;
-        int64_t ns = 0;
-        for (int m = 0; m < nm; ++m) { if (!mv[m].staged) K = std::max(K, (int)mv[m].level); else ++ns; }
-        if (ns * x->ep_page_bytes <= x->staging_bytes || max_level >= kMaxLevelCap) break;
-      }
-    } else if (any_self) {
-      // self-overlapping moves only: they are staged; nobody else depends on anything
-      K = 0;
-    }
-    for (int m = 0; m < nm; ++m) if (mv[m].staged) mv[m].slot = n_staged++;
-  }
-  int pools_per_group = n_pools_all;
-  if (n_staged > 0) {
-    int64_t per_pool = (int64_t)n_staged * x->ep_page_bytes;
-    int64_t fit = x->staging_bytes / per_pool;
-    if (fit < 1) return MOEBIUS_E_STAGING;
-    pools_per_group = (int)std::min<int64_t>(fit, n_pools_all);
-    if (n_staged >= (1 << 24)) return MOEBIUS_E_STAGING;
-  }
-  const int n_pool_groups = nm > 0 ? (n_pools_all + pools_per_group - 1) / pools_per_group : 0;
-
-  // ---- build the plan ---------------------------------------------------------------------------
-  moebius_plan_t* P = new (std::nothrow) moebius_plan_t();
-  if (!P) return MOEBIUS_E_INVAL;
-  P->ctx = x; P->from = from; P->to = to; P->n_req = n_req;
-  P->image = nullptr; P->tbl_image = nullptr; P->kv = nullptr; P->n_kv = 0; P->bt = nullptr;
-  P->buf.p = nullptr; P->buf.bytes = 0; P->buf.pinned = false; P->buf.ev = nullptr;
-  memset(&P->stats, 0, sizeof(P->stats));
-  P->stats.struct_size = sizeof(moebius_stats_t);
-  uint32_t next_ctr = 0;
-  auto fail = [&](int code) { moebius_plan_destroy(P); return code; };
-
-  // weights: one segment per (layer, matrix) object, chained in the direction-specific order
-  // ("EP->TP adopts the sequential order while TP->EP adopts the reverse order").
-  // Every EP view starts ep_shift slots (= the largest object) behind its TP view, so an object's
-  // write never lands on its own source nor on the source of an object still to come, and the
-  // regions it does overwrite belong to objects earlier in the chain, which have completed
-  // (each link waits for the previous one, transitively for all of them).
-  Chain cw, ck, cs;
-  if (R > 1) {
-    int prev_ctr = -1; uint32_t prev_units = 0;
-    const int n_links = L * x->n_obj;
-    for (int step = 0; step < n_links; ++step) {
-      const int k = e2t ? step : n_links - 1 - step;
-      const int layer = k / x->n_obj;
-      const WObj& ob = x->obj[k % x->n_obj];
-      const int tp_slot = 3 * layer + ob.slot;
-      Seg s = blank_seg();
-      s.kind = SEG_XPOSE;
-      s.ep_is_src = e2t;
-      s.n_groups = R;
-      s.rep = 1;
-      int64_t run = !ob.long_run ? (int64_t)(c.I / R) * x->wb : (int64_t)(c.I / R) * c.H * x->wb;
-      s.rows_total = !ob.long_run ? (uint32_t)(c.E / R) * c.H : (uint32_t)(c.E / R) * ob.row_mult;
-      if (run > (1ll << 31)) return fail(MOEBIUS_E_INVAL);
-      s.run_bytes = (uint32_t)run;
-      s.desc_begin = (uint32_t)(tp_slot + x->ep_shift);   // EP slot index (tensor-map coordinate)
-      const int64_t stage = x->stage_bytes;
-      const uint32_t lt_chunk = pick_chunk(run, stage);
-      if (x->use_tma && !ob.long_run && x->xt_ok) {
-        // one tensor-map box per unit: xt_rows rows x all R groups
-        s.kind = SEG_XPOSE | (PATH_TMA << 8);
-        s.groups_per_unit = R;
-        s.chunk_bytes = (uint32_t)run;
-        s.chunks_per_run = 1;
-        s.rows_per_unit = (uint32_t)x->xt_rows;
-      } else if (x->use_tma && (run > 1024 || run * R > stage) && (lt_chunk == run || lt_chunk >= 4096)) {
-        // one group per unit: plain bulk copies (long runs: the down projection, the W13 stack)
-        s.kind = SEG_XPOSE | (PATH_TMA << 8);
-        s.groups_per_unit = 1;
-        s.chunk_bytes = lt_chunk;
-        s.chunks_per_run = (uint32_t)(run / s.chunk_bytes);
-        s.rows_per_unit = s.chunks_per_run == 1 ? (uint32_t)std::min<int64_t>(32, std::max<int64_t>(1, stage / run)) : 1;
-      } else if (run * R <= unit_bytes || run <= 4096) {
-        s.groups_per_unit = R;
-        s.chunk_bytes = (uint32_t)run;
-        s.chunks_per_run = 1;
-        s.rows_per_unit = (uint32_t)std::max<int64_t>(1, unit_bytes / (run * R));
-      } else {
-        s.groups_per_unit = 1;
-        s.chunk_bytes = pick_chunk(run, unit_bytes);
-        s.chunks_per_run = (uint32_t)(run / s.chunk_bytes);
-        s.rows_per_unit = s.chunks_per_run == 1 ? (uint32_t)std::max<int64_t>(1, unit_bytes / run) : 1;
-      }
-      s.row_blocks = (s.rows_total + s.rows_per_unit - 1) / s.rows_per_unit;
-      s.tp_off = x->w_off + (int64_t)tp_slot * x->S;
-      s.ep_off = x->w_off + (int64_t)(tp_slot + x->ep_shift) * x->S;
-      int64_t nu = (int64_t)R * s.row_blocks * (s.n_groups / s.groups_per_unit) * s.chunks_per_run;
-      if (nu > (1ll << 30)) return fail(MOEBIUS_E_INVAL);
-      s.n_units = (uint32_t)nu;
-      s.wait_ctr = prev_ctr; s.wait_target = prev_units;
-      s.signal_ctr = (int32_t)next_ctr++;
-      prev_ctr = s.signal_ctr; prev_units = s.n_units;
-      push_seg(cw, s);
-    }
-    int64_t all = (int64_t)3 * L * c.E * c.H * c.I * x->wb;
-    P->stats.w_relocated = P->stats.w_read = all;
-    P->stats.w_moved = all / R * (R - 1);
-  }
-
-  // fp8 block scales: TP and EP scale views live in disjoint fixed regions, so these are plain
-  // out-of-place 2-D copies with no hazard (reading A13)
-  if (c.w_dtype == MOEBIUS_FP8_E4M3_B128) {   // also for R == 1: the two scale views never alias
-    const int HB = c.H / 128, IB = c.I / 128, EL = c.E / R;
-    for (int l = 0; l < L; ++l) for (int m = 0; m < x->n_obj; ++m) {
-      const WObj& ob = x->obj[m];
-      int64_t tp_within = 0, ep_within = 0;
-      for (int mm = 0; mm < m; ++mm) { tp_within += x->sg[mm].tp_bytes; ep_within += x->sg[mm].ep_bytes; }
-      int prev_hi = 0;
-      for (int j = 0; j < R; ++j) {
-        int lo, hi; scale_blocks(j, R, c.I, &lo, &hi);
-        int nb = hi - lo;
-        int a = e2t ? lo : std::max(lo, prev_hi);   // TP->EP: each EP block is read from its lowest holder
-        prev_hi = std::max(prev_hi, hi);
-        int take = hi - a;
-        if (take <= 0) continue;
-        for (int q = 0; q < R; ++q) {
-          C2dDesc d;
-          int64_t tp_base = (int64_t)j * x->rank_stride + x->scale_tp_off + l * x->scale_tp_layer + tp_within;
-          int64_t ep_base = (int64_t)q * x->rank_stride + x->scale_ep_off + l * x->scale_ep_layer + ep_within;
-          int64_t tp_o, ep_o; uint32_t rows, run, tp_st, ep_st;
-          if (!ob.long_run) {   // TP [E, HB, nb] ; EP [EL, HB, IB]; rows = (e', hb)
-            rows = (uint32_t)EL * HB; run = (uint32_t)take * 4;
-            tp_st = (uint32_t)nb * 4; ep_st = (uint32_t)IB * 4;
-            tp_o = tp_base + ((int64_t)q * EL * HB * nb + (a - lo)) * 4;
-            ep_o = ep_base + (int64_t)a * 4;
-          } else {       // TP [E, mult*nb, HB] ; EP [EL, mult*IB, HB]; rows = (e', gate|up block)
-            const int mult = ob.row_mult;
-            rows = (uint32_t)EL * mult; run = (uint32_t)take * HB * 4;
-            tp_st = (uint32_t)nb * HB * 4; ep_st = (uint32_t)IB * HB * 4;
-            tp_o = tp_base + ((int64_t)q * EL * mult * nb + (a - lo)) * HB * 4;
-            ep_o = ep_base + (int64_t)a * HB * 4;
-          }
-          d.rows = rows; d.run_bytes = run;
-          if (e2t) { d.src_off = ep_o; d.dst_off = tp_o; d.src_stride = ep_st; d.dst_stride = tp_st; }
-          else     { d.src_off = tp_o; d.dst_off = ep_o; d.src_stride = tp_st; d.dst_stride = ep_st; }
-          P->c2d.push_back(d);
-          int64_t bytes = (int64_t)rows * run;
-          P->stats.w_relocated += bytes; P->stats.w_read += bytes;
-          if (q != j) P->stats.w_moved += bytes;
-        }
-      }
-    }
-    Seg s = blank_seg();
-    s.kind = SEG_COPY2D;
-    s.ep_is_src = e2t;          // which side of a descriptor is the EP side (rank-share filter)
-    s.desc_begin = 0;
-    s.n_desc = (uint32_t)P->c2d.size();
-    s.n_units = s.n_desc;
-    push_seg(cs, s);
-  }
-
-  // KV: descriptors ordered [level 0][level 1]...[level K][staged]
-  if (nm > 0) {
-    std::vector<uint32_t>& lvl_begin = W.lvl_begin;
-    lvl_begin.assign(K + 2, 0);
-    for (int m = 0; m < nm; ++m) if (!mv[m].staged) lvl_begin[mv[m].level + 1]++;
-    for (int l = 0; l <= K; ++l) lvl_begin[l + 1] += lvl_begin[l];
-    const uint32_t n_direct = lvl_begin[K + 1];   // the descriptors themselves are written into the image below
-    const uint32_t ppu_lsu = (uint32_t)std::max<int64_t>(1, std::min<int64_t>(unit_bytes / x->ep_page_bytes, 2));
-    const bool kv_tma = x->use_tma && x->kt_ok;
-    uint32_t ppu = kv_tma ? (uint32_t)x->kt_pools : ppu_lsu;
-    auto kv_seg = [&](uint32_t mode, uint32_t ep_src, uint32_t d0, uint32_t nd, int pool0, int npool) {
-      Seg s = blank_seg();
-      const bool tma = kv_tma;   // staged pages too: the staging buffer has its own tensor map (page images)
-      (void)mode;
-      const uint32_t ppu = tma ? (uint32_t)x->kt_pools : ppu_lsu;
-      s.kind = SEG_KV | ((tma ? PATH_TMA : PATH_LSU) << 8);
-      s.kv_mode = mode;
-      s.ep_is_src = ep_src;
-      s.run_bytes = (uint32_t)x->run_kv;
-      s.n_groups = (uint32_t)x->G;
-      s.rep = (uint32_t)x->rep;
-      s.ep_off = s.tp_off = x->kv_off;
-      s.desc_begin = d0; s.n_desc = nd;
-      s.pool_begin = (uint32_t)pool0; s.n_pools = (uint32_t)npool;
-      s.pools_per_unit = std::min<uint32_t>(ppu, (uint32_t)npool);
-      s.ep_page_bytes = (uint32_t)x->ep_page_bytes;
-      s.tp_page_bytes = (uint32_t)x->tp_page_bytes;
-      s.pool_bytes = x->pool_bytes;
-      s.stg_pool_begin = (uint32_t)pool0;
-      s.stg_pools = (uint32_t)npool;
-      uint32_t pool_blocks = (s.n_pools + s.pools_per_unit - 1) / s.pools_per_unit;
-      s.n_units = nd * pool_blocks;
-      return s;
-    };
-    // a round = every segment that signals the same counter; the next round waits for all of them
-    const int64_t kv_units_est = (int64_t)nm * ((n_pools_all + ppu - 1) / ppu);
-    const int64_t slice_units = std::max<int64_t>(8192, kv_units_est / std::max(1, 3 * L));
-    int prev_ctr = -1; uint32_t prev_total = 0;
-    for (int g = 0; g < n_pool_groups; ++g) {
-      int pool0 = g * pools_per_group;
-      int npool = std::min(pools_per_group, n_pools_all - pool0);
-      for (int round = 0; round <= K + 1; ++round) {
-        std::vector<Seg> parts;
-        if (round == 0 && n_staged)      // save staged sources: EP->TP copies the EP page, TP->EP gathers into the slot
-          parts.push_back(kv_seg(e2t ? KV_STG_COPY : KV_MOVE_STG, e2t ? 1u : 0u, n_direct, (uint32_t)n_staged, pool0, npool));
-        if (round <= K && lvl_begin[round + 1] > lvl_begin[round])
-          parts.push_back(kv_seg(KV_MOVE, e2t ? 1u : 0u, lvl_begin[round], lvl_begin[round + 1] - lvl_begin[round], pool0, npool));
-        if (round == K + 1 && n_staged)  // every source has been read by now
-          parts.push_back(kv_seg(e2t ? KV_MOVE_STG : KV_STG_COPY, e2t ? 1u : 0u, n_direct, (uint32_t)n_staged, pool0, npool));
-        uint32_t total = 0;
-        for (auto& s : parts) total += s.n_units;
-        if (!total) continue;
-        if (next_ctr >= (uint32_t)kMaxCounters) return fail(MOEBIUS_E_STAGING);
-        int ctr = (int)next_ctr++;
-        for (auto& s : parts) {
-          // slice long segments so they interleave with the weight chain (drains of one hide behind the other)
-          uint32_t pool_blocks = (s.n_pools + s.pools_per_unit - 1) / s.pools_per_unit;
-          uint32_t desc_per_slice = (uint32_t)std::max<int64_t>(1, slice_units / pool_blocks);
-          for (uint32_t d0 = 0; d0 < s.n_desc; d0 += desc_per_slice) {
-            Seg t = s;
-            t.desc_begin = s.desc_begin + d0;
-            t.n_desc = std::min(desc_per_slice, s.n_desc - d0);
-            t.n_units = t.n_desc * pool_blocks;
-            t.wait_ctr = prev_ctr; t.wait_target = prev_total;
-            t.signal_ctr = ctr;
-            push_seg(ck, t);
-          }
-        }
-        prev_ctr = ctr; prev_total = total;
-      }
-    }
-    // accounting (reading A15): per pool, per move
-    for (int m = 0; m < nm; ++m) {
-      int64_t row = (int64_t)mv[m].ntok * x->run_kv;     // one group's bytes of this page
-      if (e2t) {
-        P->stats.kv_read += row * x->G;
-        P->stats.kv_relocated += row * x->G * x->rep;
-        P->stats.kv_moved += row * (x->G * x->rep - 1);  // the owner's own shard stays on its rank
-      } else {
-        P->stats.kv_read += row * x->G;
-        P->stats.kv_relocated += row * x->G;
-        P->stats.kv_moved += row * (x->G - 1);           // the new owner always holds one group itself
-      }
-    }
-    P->stats.kv_read *= n_pools_all; P->stats.kv_relocated *= n_pools_all; P->stats.kv_moved *= n_pools_all;
-  }
-
-  // merge the chains by fractional position (each keeps its own order)
-  struct Item { double pos; int chain; size_t idx; };
-  std::vector<Item> items;
-  auto add_chain = [&](Chain& ch, int id) {
-    int64_t acc = 0;
-    for (size_t i = 0; i < ch.segs.size(); ++i) {
-      items.push_back({ch.units ? (acc + 0.5 * ch.segs[i].n_units) / (double)ch.units : 0.0, id, i});
-      acc += ch.segs[i].n_units;
-    }
-  };
-  add_chain(cs, 0); add_chain(cw, 1); add_chain(ck, 2);
-  std::stable_sort(items.begin(), items.end(), [](const Item& a, const Item& b) {
-    if (a.chain == 0 || b.chain == 0) return a.chain == 0 && b.chain != 0;
-    return a.pos < b.pos;
-  });
-  uint64_t ub = 0;
-  for (auto& it : items) {
-    Seg s = (it.chain == 0 ? cs : it.chain == 1 ? cw : ck).segs[it.idx];
-    s.unit_begin = (uint32_t)ub;
-    ub += s.n_units;
-    P->segs.push_back(s);
-  }
-  if (ub >= (1ull << 32) || P->segs.size() > (size_t)kMaxSegs || (int64_t)nm > x->max_kv_desc ||
-      P->c2d.size() > (size_t)x->max_c2d)
-    return fail(MOEBIUS_E_INVAL);
-  P->total_units = (uint32_t)ub;
-  P->n_counters = next_ctr;
-  P->uses_tma = false;
-  for (const Seg& s : P->segs) if (seg_path(s) == PATH_TMA) P->uses_tma = true;
-  P->stage_bytes = x->stage_bytes;
-  P->xt_rows = x->xt_rows;
-
-  // Waves: wave(s) = 0 without a dependency, else 1 + the latest wave among the segments that signal
-  // the counter s waits on.  A multi-GPU run executes wave by wave with a barrier across GPUs in
-  // between (one barrier per dependency round); the fused launch ignores them.
-  std::vector<int32_t>& seg_wave = P->seg_wave;
-  seg_wave.assign(P->segs.size(), 0);
-  {
-    std::vector<int32_t> ctr_wave(next_ctr ? next_ctr : 1, -1);
-    int32_t n_waves = P->segs.empty() ? 0 : 1;
-    for (size_t i = 0; i < P->segs.size(); ++i) {
-      const Seg& sg = P->segs[i];
-      int32_t w = sg.wait_ctr >= 0 ? ctr_wave[(size_t)sg.wait_ctr] + 1 : 0;
-      seg_wave[i] = w;
-      if (sg.signal_ctr >= 0) ctr_wave[(size_t)sg.signal_ctr] = std::max(ctr_wave[(size_t)sg.signal_ctr], w);
-      n_waves = std::max(n_waves, w + 1);
-    }
-    P->n_waves = n_waves;
-  }
-
-  // ---- target request state + upload images (written in place: [segs][kv][c2d][waves] | tables) ---
-  P->lens.assign(seq_lens, seq_lens + n_req);
-  P->owner = owner;
-  int64_t seg_b = align_up((int64_t)P->segs.size() * sizeof(Seg), 256);
-  int64_t kv_b = align_up((int64_t)nm * sizeof(KvDesc), 256);
-  int64_t c2d_b = align_up((int64_t)P->c2d.size() * sizeof(C2dDesc), 256);
-  const int64_t hdr_b = sizeof(PlanHdr);
-  P->kv_img_off = hdr_b + seg_b;
-  P->c2d_img_off = hdr_b + seg_b + kv_b;
-  P->wave_img_off = hdr_b + seg_b + kv_b + c2d_b;
-  const int64_t wave_b = (int64_t)P->n_waves * hdr_b + (int64_t)P->segs.size() * (int64_t)sizeof(Seg);
-  P->image_bytes = P->wave_img_off + wave_b;
-  if (kSegOff + P->image_bytes > x->desc_bytes) return fail(MOEBIUS_E_INVAL);
-  P->tbl_bytes = 4 * ((int64_t)kTblHdrInts + 2 * (int64_t)c.max_requests + (int64_t)n_req * MP);
-  if (!image_acquire(x, P->image_bytes + P->tbl_bytes + 256, &P->buf)) return fail(MOEBIUS_E_INVAL);
-  P->image = P->buf.p;
-  {
-    PlanHdr* h = (PlanHdr*)P->image;
-    memset(h, 0, sizeof(PlanHdr));
-    h->n_segs = (uint32_t)P->segs.size();
-    h->total_units = P->total_units;
-    h->kv_off = (uint32_t)P->kv_img_off;
-    h->c2d_off = (uint32_t)P->c2d_img_off;
-  }
-  if (!P->segs.empty()) {
-    memcpy(P->image + hdr_b, P->segs.data(), P->segs.size() * sizeof(Seg));
-    memset(P->image + hdr_b + P->segs.size() * sizeof(Seg), 0, (size_t)(seg_b - (int64_t)(P->segs.size() * sizeof(Seg))));
-  }
-  {  // KV descriptors ordered [level 0][level 1]...[level K][staged]
-    KvDesc* kvd = (KvDesc*)(P->image + P->kv_img_off);
-    P->kv = kvd;
-    P->n_kv = nm;
-    if (nm > 0) {
-      std::vector<uint32_t>& cur = W.cur;
-      cur.assign(W.lvl_begin.begin(), W.lvl_begin.end() - 1);
-      uint32_t scur = W.lvl_begin[K + 1];
-      for (int m = 0; m < nm; ++m) {
-        KvDesc d;
-        d.ep_rank = mv[m].ep_rank; d.ep_page = mv[m].ep_page; d.tp_page = mv[m].tp_page;
-        d.ntok_slot = (uint32_t)mv[m].ntok | (mv[m].staged ? ((uint32_t)mv[m].slot << 8) : 0u);
-        if (mv[m].staged) kvd[scur++] = d; else kvd[cur[mv[m].level]++] = d;
-      }
-    }
-    memset(P->image + P->kv_img_off + (int64_t)nm * sizeof(KvDesc), 0, (size_t)(kv_b - (int64_t)nm * (int64_t)sizeof(KvDesc)));
-  }
-  if (c2d_b) {
-    memcpy(P->image + P->c2d_img_off, P->c2d.data(), P->c2d.size() * sizeof(C2dDesc));
-    memset(P->image + P->c2d_img_off + P->c2d.size() * sizeof(C2dDesc), 0, (size_t)(c2d_b - (int64_t)(P->c2d.size() * sizeof(C2dDesc))));
-  }
-  {  // per wave: a header + that wave's segments with their own unit numbering and no dependencies;
-     // descriptor offsets are relative to the wave's header (negative: the arrays sit before it)
-    P->wave_hdr_off.assign((size_t)P->n_waves, 0);
-    P->wave_units.assign((size_t)P->n_waves, 0);
-    int64_t at = P->wave_img_off;
-    for (int32_t w = 0; w < P->n_waves; ++w) {
-      PlanHdr* h = (PlanHdr*)(P->image + at);
-      memset(h, 0, sizeof(PlanHdr));
-      P->wave_hdr_off[(size_t)w] = at;
-      Seg* out_segs = (Seg*)(P->image + at + hdr_b);
-      uint32_t n = 0, units = 0;
-      bool tma = false;
-      for (size_t i = 0; i < P->segs.size(); ++i) {
-        if (seg_wave[i] != w) continue;
-        Seg t = P->segs[i];
-        t.wait_ctr = -1; t.signal_ctr = -1;
-        t.unit_begin = units;
-        units += t.n_units;
-        tma |= seg_path(t) == PATH_TMA;
-        out_segs[n++] = t;
-      }
-      h->n_segs = n;
-      h->total_units = units;
-      h->kv_off = (uint32_t)(int32_t)(P->kv_img_off - at);
-      h->c2d_off = (uint32_t)(int32_t)(P->c2d_img_off - at);
-      P->wave_units[(size_t)w] = units;
-      at += hdr_b + (int64_t)n * (int64_t)sizeof(Seg);
-    }
-  }
-  P->tbl_image = (int32_t*)(P->image + align_up(P->image_bytes, 256));
-  int32_t* T = P->tbl_image;
-  memset(T, 0, kTblHdrInts * 4);
-  T[0] = to; T[1] = n_req; T[2] = c.max_requests; T[3] = MP;
-  for (int i = 0; i < c.max_requests; ++i) { T[kTblHdrInts + i] = -1; T[kTblHdrInts + c.max_requests + i] = 0; }
-  for (int i = 0; i < n_req; ++i) { T[kTblHdrInts + i] = owner[i]; T[kTblHdrInts + c.max_requests + i] = seq_lens[i]; }
-  {
-    int32_t* tb = T + kTblHdrInts + 2 * c.max_requests;
-    for (int i = 0; i < n_req; ++i) {
-      int32_t* row = tb + (size_t)i * MP;
-      memcpy(row, bt.data() + (size_t)i * MP, (size_t)npages[i] * 4);
-      for (int b = npages[i]; b < MP; ++b) row[b] = -1;
-    }
-    P->bt = tb;
-  }
-
-  P->stats.n_segments = (int32_t)P->segs.size();
-  P->stats.n_kv_moves = nm;
-  P->stats.n_kv_rounds = nm ? K + 1 + (n_staged ? 1 : 0) : 0;
-  P->stats.n_kv_staged = n_staged;
-  P->stats.n_pool_groups = n_pool_groups;
-  P->stats.n_units = (int64_t)ub;
-  P->stats.staging_used_bytes = (int64_t)n_staged * x->ep_page_bytes * (n_staged ? pools_per_group : 0);
-  P->stats.desc_upload_bytes = P->image_bytes;
-  P->stats.table_upload_bytes = P->tbl_bytes;
-  *out = P;
+  PlanBuilder b(x, from, to, n_req, seq_lens, src_owner, src_bt);
+  int rc;
+  if ((rc = b.request_state()) || (rc = b.kv_moves()) || (rc = b.kv_schedule())) return rc;   // nothing allocated yet
+  if ((rc = b.new_plan())) return rc;
+  if ((rc = b.weight_chain()) || (rc = b.scale_copies()) || (rc = b.kv_segments()) || (rc = b.merge_and_waves()) ||
+      (rc = b.build_images()) || (rc = b.finish_stats()))
+    return rc;                                          // the failing stage has destroyed the plan
+  *out = b.P;
   return MOEBIUS_OK;
 }
 
