@@ -359,6 +359,8 @@ def run_moebius(args):
         torch.cuda.synchronize()
         d2d = {"bytes": n_copy, "ms_best_of_5": best, "GBps_read_plus_write": 2 * n_copy / best / 1e6}
 
+    sess.free_plan(plan_t2e)     # their pinned upload images go back to the context's pool
+    sess.free_plan(plan_e2t)
     # e2e: host inputs -> plan -> reshard (uploads) -> device->host read-back of the published tables
     host_tables = torch.empty(lay.table_bytes // 4, dtype=torch.int32, pin_memory=True)
     tbl_n = lay.tbl_bt_off + n * mp
