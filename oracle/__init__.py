@@ -18,7 +18,7 @@ from .kv import (  # noqa: F401
     CapacityError, canonical_block_tables, ep_pool_image, kv_heads_of_rank, pages_needed,
     partition_requests, tp_pool_image, tp_source_rank, gather_request_from_tp, gather_request_from_ep,
 )
-from .accounting import kv_bytes, weight_bytes  # noqa: F401
+from .accounting import kv_bytes, scale_bytes, weight_bytes  # noqa: F401
 from .ffn import moe_ffn_dense, moe_ffn_ep, moe_ffn_tp, route_top2  # noqa: F401
 from .ffn import moe_ffn_dense_w13, moe_ffn_ep_w13, moe_ffn_tp_w13  # noqa: F401
 from .image import OracleLayout, State, np_view, target_request_state  # noqa: F401,E402

@@ -51,3 +51,45 @@ def kv_bytes(seq_lens, owner, R, L, Hkv, D, elem_bytes, direction: str):
                     moved += n * head_bytes
     f = 2 * L
     return {"moved": moved * f, "relocated": relocated * f, "read": read * f}
+
+
+def scale_bytes(R, L, E, H, I, direction: str, kinds=("gate", "up", "down")):
+    """fp8 block scales (BASELINE.json config 5; SURVEY.md §8(c) "bytes moved ... (+ scales)";
+    reading A13), by enumeration of (expert e, TP rank j, 128-block ib of the intermediate axis).
+
+    One fp32 scale per 128x128 block: an (e, ib) pair stands for the H/128 scales of that block
+    column (gate/up/w2: [E, H/128, I/128]) or block row (down: [E, I/128, H/128]); the stacked
+    `w13` ([E, 2I/128, H/128]) has every ib twice, once in the gate half and once in the up half.
+    TP shard j carries every block its I/R columns touch, so a block that straddles two shards is
+    held by both (like a replicated KV head):
+      ep2tp  every holder j of (e, ib) receives a copy from the EP owner q = e div (E/R): each copy
+             is `relocated`, and `moved` when j != q; the source is read once per (e, ib).
+      tp2ep  the EP owner q receives (e, ib) once, read from its LOWEST-rank holder (the rule of
+             reading A5 applied to scales): `moved` when that holder != q.
+    """
+    from .weights import tp_scale_blocks
+    per_block = (H // 128) * 4
+    holders = {}
+    for j in range(R):
+        lo, hi = tp_scale_blocks(j, R, I)
+        for ib in range(lo, hi):
+            holders.setdefault(ib, []).append(j)
+    assert sorted(holders) == list(range(I // 128))
+    moved = relocated = read = 0
+    for e in range(E):
+        q = e // (E // R)
+        for ib in range(I // 128):
+            if direction == "ep2tp":
+                read += per_block
+                for j in holders[ib]:
+                    relocated += per_block
+                    if j != q:
+                        moved += per_block
+            else:
+                src = min(holders[ib])
+                read += per_block
+                relocated += per_block
+                if src != q:
+                    moved += per_block
+    f = L * sum(2 if k == "w13" else 1 for k in kinds)
+    return {"moved": moved * f, "relocated": relocated * f, "read": read * f}

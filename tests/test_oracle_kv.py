@@ -183,3 +183,67 @@ def test_kv_bytes_closed_form():
             assert e2t["relocated"] == T * L * Hkv * 2 * D * b
         assert t2e["relocated"] == T * L * Hkv * 2 * D * b
         assert e2t["read"] == T * L * Hkv * 2 * D * b and t2e["read"] == T * L * Hkv * 2 * D * b
+
+
+def test_scale_bytes_closed_forms():
+    """oracle.scale_bytes (SURVEY.md §8(c) "(+ scales)", reading A13) against closed forms worked by hand.
+
+    I/R = 192 (I = 1536, R = 8; the Qwen3-235B shape): shard j covers columns [192j, 192j+191], i.e.
+    blocks {0,1} {1,2} {3,4} {4,5} {6,7} {7,8} {9,10} {10,11}: 2 blocks per shard, 16 holder slots for
+    the 12 blocks; blocks 1, 4, 7, 10 are straddled.  Lowest holders of blocks 0..11:
+    0 0 1 2 2 3 4 4 5 6 6 7 -- every block has ONE source rank, which owns E/R of the experts itself.
+      ep2tp: relocated = 16 slots, moved = 16 * (1 - 1/R), read = 12 (each source block once)
+      tp2ep: relocated = read = 12, moved = 12 * (1 - 1/R)          [per expert, x H/128 * 4 bytes]
+    Aligned shape (I/R a multiple of 128): no block is shared, both directions move (1 - 1/R) of
+    E * I/128 * H/128 * 4 bytes, exactly like the weights."""
+    R, L, E, H, I = 8, 4, 128, 4096, 1536
+    blk = (H // 128) * 4
+    for kinds, f in ((("gate", "up", "down"), 3), (("w13", "w2"), 3), (("down",), 1)):
+        e2t = oracle.scale_bytes(R, L, E, H, I, "ep2tp", kinds)
+        t2e = oracle.scale_bytes(R, L, E, H, I, "tp2ep", kinds)
+        assert e2t == {"relocated": L * f * E * 16 * blk, "moved": L * f * (E - E // R) * 16 * blk,
+                       "read": L * f * E * 12 * blk}
+        assert t2e == {"relocated": L * f * E * 12 * blk, "moved": L * f * (E - E // R) * 12 * blk,
+                       "read": L * f * E * 12 * blk}
+    # BASELINE.json config 5: 2.36 MB of scales in total (SURVEY.md §8(a) row a8)
+    assert oracle.scale_bytes(8, 4, 128, 4096, 1536, "tp2ep")["relocated"] == 2359296
+    for (R, L, E, H, I) in [(4, 2, 8, 256, 1024), (2, 1, 4, 128, 256), (8, 1, 8, 128, 1024)]:
+        assert (I // R) % 128 == 0
+        tot = L * 3 * E * (I // 128) * (H // 128) * 4
+        for d in ("ep2tp", "tp2ep"):
+            a = oracle.scale_bytes(R, L, E, H, I, d)
+            assert a["relocated"] == tot and a["read"] == tot and a["moved"] * R == tot * (R - 1)
+    # R = 1: one rank holds everything, nothing changes owner
+    a = oracle.scale_bytes(1, 1, 4, 128, 256, "ep2tp")
+    assert a["moved"] == 0 and a["relocated"] == 3 * 4 * 2 * 1 * 4
+
+
+@pytest.mark.parametrize("R,E,H,I", [(8, 16, 256, 1536), (4, 8, 128, 768), (8, 8, 128, 2048), (2, 4, 256, 384)])
+def test_scale_bytes_equal_the_scale_views(R, E, H, I):
+    """Reduction onto the separately pinned views (tp_scale_view is pinned by the dequantised-shard
+    equality in test_oracle_weights.py): EP->TP writes exactly the TP scale views, TP->EP exactly the
+    EP scale views; and the owner-changed part counted by brute force over explicit owner arrays."""
+    L = 1
+    for kinds in (("gate", "up", "down"), ("w13", "w2")):
+        tp_bytes = ep_bytes = moved_e2t = moved_t2e = 0
+        for kind in kinds:
+            mult = 2 if kind == "w13" else 1
+            shape = (E, H // 128, I // 128) if kind in ("gate", "up", "w2") else (E, mult * I // 128, H // 128)
+            S = np.arange(int(np.prod(shape)), dtype=np.float32).reshape(shape)
+            ids = np.arange(S.size).reshape(shape).astype(np.float32)        # identity of every scale
+            owner_of = np.repeat(np.arange(R), E // R)                       # EP owner of expert e
+            first_holder = {}
+            for j in range(R):
+                v = oracle.tp_scale_view(ids, kind, j, R, I)
+                tp_bytes += v.nbytes
+                q = np.broadcast_to(owner_of.reshape(-1, 1, 1), v.shape)
+                moved_e2t += int((q != j).sum()) * 4
+                for x, qq in zip(v.ravel().tolist(), q.ravel().tolist()):
+                    first_holder.setdefault(x, (j, qq))                      # lowest rank seen first
+                ep_bytes += oracle.ep_scale_view(S, j, R).nbytes
+            assert len(first_holder) == S.size
+            moved_t2e += sum(4 for (j, qq) in first_holder.values() if j != qq)
+        e2t = oracle.scale_bytes(R, L, E, H, I, "ep2tp", kinds)
+        t2e = oracle.scale_bytes(R, L, E, H, I, "tp2ep", kinds)
+        assert (e2t["relocated"], e2t["moved"], e2t["read"]) == (tp_bytes, moved_e2t, ep_bytes)
+        assert (t2e["relocated"], t2e["moved"], t2e["read"]) == (ep_bytes, moved_t2e, ep_bytes)
