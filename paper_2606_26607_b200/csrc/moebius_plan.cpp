@@ -739,6 +739,7 @@ struct PlanBuilder {
           int lo, hi; scale_blocks(j, R, c.I, &lo, &hi);
           int nb = hi - lo;
           int a = e2t ? lo : std::max(lo, prev_hi);   // TP->EP: each EP block is read from its lowest holder
+          const int fresh_hi = prev_hi;               // blocks below it were already counted as read
           prev_hi = std::max(prev_hi, hi);
           int take = hi - a;
           if (take <= 0) continue;
@@ -764,8 +765,11 @@ struct PlanBuilder {
             else     { d.src_off = tp_o; d.dst_off = ep_o; d.src_stride = tp_st; d.dst_stride = ep_st; }
             P->c2d.push_back(d);
             int64_t bytes = (int64_t)rows * run;
-            P->stats.w_relocated += bytes; P->stats.w_read += bytes;
+            P->stats.w_relocated += bytes;
             if (q != j) P->stats.w_moved += bytes;
+            // unique source bytes (reading A15): EP->TP reads a straddled block once for both holders
+            const int fresh = hi - std::max(lo, fresh_hi);
+            if (fresh > 0) P->stats.w_read += (int64_t)rows * fresh * (run / take);
           }
         }
       }

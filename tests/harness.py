@@ -75,6 +75,9 @@ def expected_bytes(st: State, from_mode: int, ep_owner):
     d = "ep2tp" if from_mode == EP else "tp2ep"
     w = oracle.weight_bytes(c.R, c.L, c.E, c.H, c.I, c.w_elem_bytes, d) if c.R > 1 else \
         {"moved": 0, "relocated": 0, "read": 0}
+    if c.w_dtype == "fp8_e4m3_b128":      # the block scales travel with their weights (reading A13)
+        s = oracle.scale_bytes(c.R, c.L, c.E, c.H, c.I, d, c.w_kinds)
+        w = {key: w[key] + s[key] for key in w}
     k = oracle.kv_bytes(st.lens, ep_owner if ep_owner is not None else np.zeros(len(st.lens), np.int32),
                         c.R, c.L, c.kv_heads, c.head_dim, c.kv_elem_bytes, d)
     return w, k

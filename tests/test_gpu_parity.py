@@ -89,8 +89,7 @@ def gpu_switch(st, sess, from_mode, src_owner, src_bt, execute=None):
     # accounting
     ep_owner = src_owner if from_mode == EP else owner
     w, k = expected_bytes(st, from_mode, ep_owner)
-    if st.cfg.w_dtype != "fp8_e4m3_b128":
-        assert (stats["w_moved"], stats["w_relocated"]) == (w["moved"], w["relocated"])
+    assert (stats["w_moved"], stats["w_relocated"], stats["w_read"]) == (w["moved"], w["relocated"], w["read"])
     assert (stats["kv_moved"], stats["kv_relocated"], stats["kv_read"]) == (k["moved"], k["relocated"], k["read"])
     sess.free_plan(plan)
     return to_mode, (want_owner if to_mode == EP else None), want_bt, stats
