@@ -103,13 +103,16 @@ int moebius_arena_create(const moebius_ctx_t* x, int device, int rank_lo, int ra
   for (int r = rank_lo; r < rank_hi; ++r) {
     CUdeviceptr at = a->va + (CUdeviceptr)((int64_t)r * a->rank_stride);
     if (a->drv.Create(&a->handle[(size_t)r], (size_t)a->rank_stride, &prop, 0) != CUDA_SUCCESS ||
-        a->drv.Map(at, (size_t)a->rank_stride, 0, a->handle[(size_t)r], 0) != CUDA_SUCCESS ||
-        a->drv.SetAccess(at, (size_t)a->rank_stride, &acc, 1) != CUDA_SUCCESS) {
+        a->drv.Map(at, (size_t)a->rank_stride, 0, a->handle[(size_t)r], 0) != CUDA_SUCCESS) {
       moebius_arena_destroy(a);
       return MOEBIUS_E_CUDA;
     }
-    a->mapped[(size_t)r] = 1;
+    a->mapped[(size_t)r] = 1;   // mapped from here on: destroy must unmap it even if SetAccess fails
     a->local[(size_t)r] = 1;
+    if (a->drv.SetAccess(at, (size_t)a->rank_stride, &acc, 1) != CUDA_SUCCESS) {
+      moebius_arena_destroy(a);
+      return MOEBIUS_E_CUDA;
+    }
   }
   *out = a;
   return MOEBIUS_OK;

@@ -450,6 +450,7 @@ moebius_reshard_kernel(const __grid_constant__ DevParams p_in, const __grid_cons
       retire();
       wait_for(s, si);
       bulk_wait_read<1>();     // the stage about to be refilled was read by the store group before the last one
+      __syncwarp();            // wait_group is per thread: every lane's stores have read the stage before lane 0 refills it
       tma_issue_load(tc, s, ul, d, ring + (size_t)next_stage * p.stage_bytes, bar + next_stage, lane);
       loading = true; ld_si = si; ld_ul = ul; ld_stage = next_stage; ld_d = d;
       next_stage ^= 1;
@@ -610,6 +611,60 @@ void cuda_ctx_destroy(moebius_ctx* x) {
 
 using namespace moebius;
 
+namespace moebius {
+
+// One-off device-side setup of a bound context: device facts, the timing-event ring, the driver entry
+// point + the three tensor maps, and the kernel's dynamic shared-memory attribute.  Called by
+// moebius_bind and again by moebius_set_tma (the stage geometry changes the maps and the attribute), so
+// that moebius_reshard / _staged / _share find everything in place: they create no event, resolve no
+// symbol, encode no descriptor and set no attribute.
+int device_prepare(moebius_ctx* x) {
+  x->prepared = false;
+  if (!x->bound) return MOEBIUS_OK;
+  if (x->has_device < 0) {
+    int ndev = 0;
+    x->has_device = (cudaGetDeviceCount(&ndev) == cudaSuccess && ndev > 0) ? 1 : 0;
+    cudaGetLastError();
+  }
+  if (!x->has_device) return MOEBIUS_OK;
+  if (x->n_sm == 0) {
+    int dev = 0, n = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) return MOEBIUS_E_CUDA;
+    if (cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || n <= 0) return MOEBIUS_E_CUDA;
+    x->n_sm = n;
+  }
+  if (!x->ev_valid) {
+    for (int i = 0; i < 2 * kTimingRing; ++i) {
+      cudaEvent_t e;
+      if (cudaEventCreate(&e) != cudaSuccess) {
+        for (int k = 0; k < i; ++k) cudaEventDestroy((cudaEvent_t)x->ev[k]);
+        return MOEBIUS_E_CUDA;
+      }
+      x->ev[i] = e;
+    }
+    x->ev_valid = true;
+  }
+  if (int rc = encode_tmaps(x)) return rc;
+  const bool tma = x->use_tma && (x->xt_ok || x->kt_ok);
+  if (tma) {
+    const size_t smem = 1024 + (size_t)x->n_pipes * 2 * (size_t)x->stage_bytes;
+    if (cudaFuncSetAttribute(moebius_reshard_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) {
+      cudaGetLastError();
+      return MOEBIUS_E_CUDA;
+    }
+    x->smem_set = smem;
+  }
+  {  // lazy module loading would otherwise hit the first switch: resolve both kernel variants now
+    cudaFuncAttributes fa;
+    if (cudaFuncGetAttributes(&fa, moebius_reshard_kernel<1>) != cudaSuccess ||
+        cudaFuncGetAttributes(&fa, moebius_reshard_kernel<2>) != cudaSuccess) { cudaGetLastError(); return MOEBIUS_E_CUDA; }
+  }
+  x->prepared = true;
+  return MOEBIUS_OK;
+}
+
+}  // namespace moebius
+
 extern "C" int moebius_bind(moebius_ctx_t* x, void* dev_base, void* dev_staging, void* dev_desc,
                             int32_t* dev_tables, moebius_mode_t initial_mode) {
   if (!x || !dev_base || !dev_desc || !dev_tables) return MOEBIUS_E_INVAL;
@@ -623,8 +678,12 @@ extern "C" int moebius_bind(moebius_ctx_t* x, void* dev_base, void* dev_staging,
   x->tables = dev_tables;
   x->active_mode = initial_mode;
   x->bound = true;
-  x->tmaps_valid = false;   // encoded on the first reshard (needs a device)
-  return MOEBIUS_OK;
+  x->tmaps_valid = false;
+  x->prepared = false;
+  // Everything a first switch would otherwise have to set up is done here (the switch
+  // path itself allocates nothing).  Without a CUDA device the context stays usable for the host-only
+  // planner calls; moebius_reshard then returns MOEBIUS_E_CUDA.
+  return device_prepare(x);
 }
 
 extern "C" int moebius_set_timing(moebius_ctx_t* x, int enable) {
@@ -657,13 +716,12 @@ extern "C" int moebius_last_kernel_ms(moebius_ctx_t* x, float* ms) {
 
 namespace {
 
-int ensure_device_facts(moebius_ctx* x) {
-  if (x->n_sm == 0) {
-    int dev = 0, n = 0;
-    if (cudaGetDevice(&dev) != cudaSuccess) return MOEBIUS_E_CUDA;
-    if (cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || n <= 0) return MOEBIUS_E_CUDA;
-    x->n_sm = n;
-  }
+// What must hold before anything is enqueued: a CUDA device, the one-off setup of device_prepare, and a
+// plan built for the current stage geometry (moebius_set_tma after moebius_plan invalidates the plan).
+int ready_to_launch(const moebius_ctx* x, const moebius_plan_t* P) {
+  if (!x->has_device || !x->prepared) return x->has_device ? MOEBIUS_E_STATE : MOEBIUS_E_CUDA;
+  if (P && P->uses_tma && (P->stage_bytes != x->stage_bytes || P->xt_rows != x->xt_rows)) return MOEBIUS_E_STATE;
+  if (P && (kSegOff + P->image_bytes > x->desc_bytes || P->tbl_bytes > x->table_bytes)) return MOEBIUS_E_INVAL;
   return MOEBIUS_OK;
 }
 
@@ -687,18 +745,14 @@ int launch_reshard_kernel(moebius_ctx* x, bool tma, int64_t unit_hint, cudaStrea
   int threads, per_sm;
   size_t smem = 0;
   if (tma) {
-    // one CTA per SM, n_pipes warps, each with two private stages
-    if (!x->tmaps_valid) { int rc = encode_tmaps(x); if (rc != MOEBIUS_OK) return rc; }
+    // one CTA per SM, n_pipes warps, each with two private stages (tensor maps and the shared-memory
+    // attribute were set up by device_prepare)
     p.stage_bytes = (uint32_t)x->stage_bytes;
     p.xt_rows = (uint32_t)x->xt_rows;
     threads = 32 * x->n_pipes;
     per_sm = 1;
     smem = 1024 + (size_t)x->n_pipes * 2 * (size_t)x->stage_bytes;
-    if (smem != x->smem_set) {
-      if (cudaFuncSetAttribute(moebius_reshard_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess)
-        return MOEBIUS_E_CUDA;
-      x->smem_set = smem;
-    }
+    if (smem != x->smem_set || !x->tmaps_valid) return MOEBIUS_E_STATE;
   } else {
     threads = x->threads > 0 ? x->threads : 256;
     per_sm = x->ctas_per_sm > 0 ? x->ctas_per_sm : 2;
@@ -723,21 +777,14 @@ extern "C" int moebius_reshard(moebius_ctx_t* x, const moebius_plan_t* P, void* 
   if (!x || !P || P->ctx != x) return MOEBIUS_E_INVAL;
   if (!x->bound || x->active_mode != P->from) return MOEBIUS_E_STATE;
   cudaStream_t st = (cudaStream_t)cuda_stream;
-  if (int rc = ensure_device_facts(x)) return rc;
-  if (x->timing && !x->ev_valid) {
-    for (int i = 0; i < 2 * kTimingRing; ++i) {
-      cudaEvent_t e;
-      if (cudaEventCreate(&e) != cudaSuccess) return MOEBIUS_E_CUDA;
-      x->ev[i] = e;
-    }
-    x->ev_valid = true;
-  }
+  // Every check comes before the first enqueue: a call that fails here has touched nothing.  (A CUDA
+  // error returned by one of the enqueues below is a sticky device fault, not a recoverable state.)
+  if (int rc = ready_to_launch(x, P)) return rc;
   cudaEvent_t ev_a = nullptr, ev_b = nullptr;
   if (x->timing) {
     int64_t k = x->ev_count % kTimingRing;
     ev_a = (cudaEvent_t)x->ev[2 * k]; ev_b = (cudaEvent_t)x->ev[2 * k + 1];
   }
-  if (P->uses_tma && (P->stage_bytes != x->stage_bytes || P->xt_rows != x->xt_rows)) return MOEBIUS_E_STATE;  // set_tma after plan
   // 1. work list -> device; ticket and the counters this plan uses -> 0
   if (cudaMemsetAsync(x->desc, 0, (size_t)(kCtrOff + 4 * (int64_t)(P->n_counters ? P->n_counters : 1)), st) != cudaSuccess)
     return MOEBIUS_E_CUDA;
@@ -762,7 +809,7 @@ extern "C" int moebius_reshard(moebius_ctx_t* x, const moebius_plan_t* P, void* 
 extern "C" int moebius_stage_plan(moebius_ctx_t* x, const moebius_plan_t* P) {
   if (!x || !P || P->ctx != x) return MOEBIUS_E_INVAL;
   if (!x->bound || x->active_mode != P->from) return MOEBIUS_E_STATE;
-  if (P->uses_tma && (P->stage_bytes != x->stage_bytes || P->xt_rows != x->xt_rows)) return MOEBIUS_E_STATE;
+  if (int rc = ready_to_launch(x, P)) return rc;
   const int64_t img_cap = x->desc_bytes - kSegOff;
   if (P->image_bytes > img_cap || P->tbl_bytes > x->table_bytes) return MOEBIUS_E_INVAL;
   if (!x->mailbox) {
@@ -785,7 +832,7 @@ extern "C" int moebius_reshard_staged(moebius_ctx_t* x, void* cuda_stream) {
   if (!x) return MOEBIUS_E_INVAL;
   if (!x->bound || !x->mailbox) return MOEBIUS_E_STATE;
   cudaStream_t st = (cudaStream_t)cuda_stream;
-  if (int rc = ensure_device_facts(x)) return rc;
+  if (int rc = ready_to_launch(x, nullptr)) return rc;
   const int64_t img_cap = x->desc_bytes - kSegOff;
   // every size, address and launch dimension below is the same for every plan of this context
   if (cudaMemsetAsync(x->desc, 0, (size_t)kSegOff, st) != cudaSuccess) return MOEBIUS_E_CUDA;
@@ -810,9 +857,8 @@ extern "C" int moebius_reshard_share(moebius_ctx_t* x, const moebius_plan_t* P, 
   if (!x || !P || P->ctx != x) return MOEBIUS_E_INVAL;
   if (rank_lo < 0 || rank_hi > x->cfg.R || rank_lo >= rank_hi || wave < 0 || wave >= P->n_waves) return MOEBIUS_E_INVAL;
   if (!x->bound || x->active_mode != P->from) return MOEBIUS_E_STATE;
-  if (P->uses_tma && (P->stage_bytes != x->stage_bytes || P->xt_rows != x->xt_rows)) return MOEBIUS_E_STATE;
   cudaStream_t st = (cudaStream_t)cuda_stream;
-  if (int rc = ensure_device_facts(x)) return rc;
+  if (int rc = ready_to_launch(x, P)) return rc;
   if (wave == 0) {   // the work list (all waves) goes up once, with the first wave
     if (cudaMemcpyAsync(x->desc + kSegOff, P->image, (size_t)P->image_bytes, cudaMemcpyHostToDevice, st) != cudaSuccess)
       return MOEBIUS_E_CUDA;
@@ -828,6 +874,7 @@ extern "C" int moebius_reshard_publish(moebius_ctx_t* x, const moebius_plan_t* P
   if (!x || !P || P->ctx != x) return MOEBIUS_E_INVAL;
   if (!x->bound || x->active_mode != P->from) return MOEBIUS_E_STATE;
   cudaStream_t st = (cudaStream_t)cuda_stream;
+  if (int rc = ready_to_launch(x, P)) return rc;
   if (cudaMemcpyAsync(x->tables, P->tbl_image, (size_t)P->tbl_bytes, cudaMemcpyHostToDevice, st) != cudaSuccess)
     return MOEBIUS_E_CUDA;
   if (P->buf.ev && cudaEventRecord((cudaEvent_t)P->buf.ev, st) != cudaSuccess) return MOEBIUS_E_CUDA;

@@ -101,6 +101,7 @@ struct moebius_ctx {
   alignas(64) unsigned char tmap_kv[128];
   alignas(64) unsigned char tmap_stg[128];  // the staging buffer as an array of EP-page images
   bool tmaps_valid;
+  bool prepared;                  // device_prepare has run for the current buffers and stage geometry
   size_t smem_set;                // dynamic shared memory the kernel attribute is currently set to
   // device facts + timing (filled lazily by the CUDA side)
   int n_sm;
@@ -151,6 +152,7 @@ void image_release(moebius_ctx* ctx, const ImageBuf& buf);             // back t
 void image_free(const ImageBuf& buf);
 void cuda_ctx_destroy(moebius_ctx* ctx);
 void lpt_partition(int n_req, const int32_t* seq_lens, int R, PlanScratch& scratch, int32_t* owner);
+int device_prepare(moebius_ctx* ctx);  // one-off device-side setup of a bound context (moebius_bind, moebius_set_tma)
 void tma_geometry(moebius_ctx* ctx);   // derives xt_ok/kt_ok/xt_rows/kt_pools from cfg + stage_bytes (host only)
 }  // namespace moebius
 

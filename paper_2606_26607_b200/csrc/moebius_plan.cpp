@@ -175,6 +175,7 @@ int moebius_create(const moebius_config_t* c, moebius_ctx_t** out) {
   x->def_pipes = x->n_pipes;
   x->def_stage_bytes = x->stage_bytes;
   x->tmaps_valid = false;
+  x->prepared = false;
   x->smem_set = 0;
   tma_geometry(x);
   x->n_sm = 0;
@@ -287,7 +288,7 @@ int moebius_set_tma(moebius_ctx_t* x, int enable, int pipes, int stage_kb) {
   x->stage_bytes = sb;
   x->tmaps_valid = false;
   tma_geometry(x);
-  return MOEBIUS_OK;
+  return device_prepare(x);   // a bound context re-encodes its tensor maps and shared-memory size here
 }
 
 int moebius_set_kv_rounds(moebius_ctx_t* x, int max_level) {
@@ -713,6 +714,7 @@ struct PlanBuilder {
         if (nu > (1ll << 30)) return fail(MOEBIUS_E_INVAL);
         s.n_units = (uint32_t)nu;
         s.wait_ctr = prev_ctr; s.wait_target = prev_units;
+        if (next_ctr >= (uint32_t)kMaxCounters) return fail(MOEBIUS_E_INVAL);   // the counters sit below the uploaded image
         s.signal_ctr = (int32_t)next_ctr++;
         prev_ctr = s.signal_ctr; prev_units = s.n_units;
         push_seg(cw, s);

@@ -93,6 +93,11 @@ int moebius_capacity_check(moebius_ctx_t* x, moebius_mode_t to, int32_t n_req, c
 int moebius_policy_step(moebius_policy_t* p, moebius_ctx_t* ctx, double now_s, int32_t n_req,
                         const int32_t* seq_lens, int32_t* decision, int32_t* mode_after) {
   if (!p || !decision || n_req < 0) return MOEBIUS_E_INVAL;
+  // everything that can be rejected is rejected before the window or the cooldown clock move
+  if (ctx && n_req > 0) {
+    if (!seq_lens) return MOEBIUS_E_INVAL;
+    for (int32_t i = 0; i < n_req; ++i) if (seq_lens[i] < 0) return MOEBIUS_E_INVAL;
+  }
   const moebius_policy_config_t& c = p->cfg;
   // the window always advances, cooling down or not (reading P2)
   const size_t slot = (size_t)(p->seen % c.W);
@@ -109,16 +114,18 @@ int moebius_policy_step(moebius_policy_t* p, moebius_ctx_t* ctx, double now_s, i
     if ((double)p->sum / (double)c.W < c.T_l) want = MOEBIUS_TP;       // mean of the last W below T_l
   }
   if (want < 0) return MOEBIUS_OK;
-  p->has_event = true;
-  p->t_last = now_s;
   if (ctx) {
     int rc = moebius_capacity_check(ctx, (moebius_mode_t)want, n_req, seq_lens);
+    if (rc != MOEBIUS_OK && rc != MOEBIUS_E_CAPACITY) return rc;         // a failed call starts no cooldown
     if (rc == MOEBIUS_E_CAPACITY) {                                      // cancel, retry after the cooldown
+      p->has_event = true;
+      p->t_last = now_s;
       *decision = MOEBIUS_DECISION_CANCELLED;
       return MOEBIUS_OK;
     }
-    if (rc != MOEBIUS_OK) return rc;
   }
+  p->has_event = true;
+  p->t_last = now_s;
   p->mode = want;
   *decision = MOEBIUS_DECISION_SWITCH;
   if (mode_after) *mode_after = p->mode;

@@ -16,6 +16,7 @@ import torch
 import workloads as wl
 
 KINDS = ("gate", "up", "down")
+TENSOR_ID = {"gate": 0, "up": 1, "down": 2, "w13": 8, "w2": 9}   # moebius_tensor_t
 
 
 def fill_random(sess):
@@ -39,19 +40,20 @@ def fill_tp_weight(sess, cfg, layer, kind, experts_per_chunk=16):
     R, E, H, I = cfg.R, cfg.E, cfg.H, cfg.I
     w = I // R
     off = wl.tag_salt_offset(wl.weight_tag_salt(cfg, layer, kind))
-    tid = KINDS.index(kind)
+    tid = TENSOR_ID[kind]
     for j in range(R):
         view = sess.view(0, j, layer, tid)
         for e0 in range(0, E, experts_per_chunk):
             e = torch.arange(e0, min(E, e0 + experts_per_chunk), device=dev, dtype=torch.int64)
-            if kind != "down":      # logical [E,H,I]; TP shard j = columns [j*w, (j+1)*w)
-                h = torch.arange(H, device=dev, dtype=torch.int64)
-                c = torch.arange(w, device=dev, dtype=torch.int64) + j * w
+            h = torch.arange(H, device=dev, dtype=torch.int64)
+            c = torch.arange(w, device=dev, dtype=torch.int64) + j * w
+            if kind in ("gate", "up", "w2"):   # logical [E,H,I]; TP shard j = columns [j*w, (j+1)*w)
                 flat = (e[:, None, None] * H + h[None, :, None]) * I + c[None, None, :]
-            else:                   # logical [E,I,H]; TP shard j = rows [j*w, (j+1)*w)
-                c = torch.arange(w, device=dev, dtype=torch.int64) + j * w
-                h = torch.arange(H, device=dev, dtype=torch.int64)
+            elif kind == "down":               # logical [E,I,H]; TP shard j = rows [j*w, (j+1)*w)
                 flat = (e[:, None, None] * I + c[None, :, None]) * H + h[None, None, :]
+            else:                              # w13: logical [E,2I,H]; TP shard j = gate rows [j*w, (j+1)*w) then
+                c2 = torch.cat([c, c + I])     # the same rows of the up half (reading A2)
+                flat = (e[:, None, None] * (2 * I) + c2[None, :, None]) * H + h[None, None, :]
             _store(view[e0:e0 + len(e)], wl.tag_fill_u16_torch(flat, off))
             del flat
 

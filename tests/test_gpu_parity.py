@@ -399,3 +399,69 @@ def test_fuzz_round_trip_on_device(seed):
             assert e.status == -3 and policy == "tight"
             break
     sess.close()
+
+
+def test_first_switch_after_bind_allocates_nothing():
+    """"a switch does not allocate dynamic buffers".  Everything one-off (timing events,
+    the driver entry point, the tensor maps, the kernel's shared-memory attribute, module loading) is
+    done by moebius_bind; the very FIRST moebius_reshard of a context -- and every later one -- leaves
+    the free device memory and the host heap (glibc mallinfo2: arena + mmapped bytes in use) exactly as
+    they were.  The plan (host object, pinned upload image) is built before the measured call."""
+    import ctypes as C
+
+    class Mallinfo2(C.Structure):
+        _fields_ = [(n, C.c_size_t) for n in ("arena", "ordblks", "smblks", "hblks", "hblkhd", "usmblks", "fsmblks",
+                                                "uordblks", "fordblks", "keepcost")]
+    libc = C.CDLL("libc.so.6")
+    libc.mallinfo2.restype = Mallinfo2
+
+    def heap():
+        m = libc.mallinfo2()
+        return m.uordblks + m.hblkhd
+
+    cfg = SMALLISH.with_(L=1)
+    st, sess = gpu_session(cfg)
+    mb.moebius_set_timing(sess.ctx, True)
+    owner, bt, _ = start(st, sess, TP, "random")
+    stream = torch.cuda.current_stream().cuda_stream
+    mode = TP
+    for k in range(3):
+        to = EP if mode == TP else TP
+        plan = sess.plan(to, st.lens, owner, bt, from_mode=mode)
+        torch.cuda.synchronize()
+        free0, _ = torch.cuda.mem_get_info()
+        h0 = heap()
+        mb.moebius_reshard(sess.ctx, plan, stream)          # the measured call: ctypes straight into the C ABI
+        h1 = heap()
+        torch.cuda.synchronize()
+        free1, _ = torch.cuda.mem_get_info()
+        assert free1 == free0, ("device memory changed during switch %d" % k, free0 - free1)
+        assert h1 == h0, ("host heap changed during switch %d" % k, h1 - h0)
+        want_owner, want_bt = expected_target(st, sess, to)
+        assert not OracleLayout(st, sess, to, want_owner, want_bt).compare(download(sess))
+        sess.free_plan(plan)
+        owner, bt, mode = (want_owner if to == EP else None), want_bt, to
+    assert mb.moebius_last_kernel_ms(sess.ctx) > 0
+    sess.close()
+
+
+def test_reshard_checks_come_before_the_first_enqueue():
+    """include/moebius.h: a failed call leaves the context and all device bytes untouched.  A plan built
+    for another stage geometry (moebius_set_tma after moebius_plan) is refused with E_STATE before
+    anything is enqueued: the descriptor buffer, the tables and the data keep their bytes."""
+    st, sess = gpu_session(SMALLISH.with_(L=1))
+    owner, bt, _ = start(st, sess, TP, "random")
+    plan = sess.plan(EP, st.lens, owner, bt, from_mode=TP)
+    mb.moebius_set_tma(sess.ctx, 1, 2, 32)
+    torch.cuda.synchronize()
+    before = sess.arena.clone()
+    with pytest.raises(mb.MoebiusError) as e:
+        sess.reshard(plan)
+    assert e.value.status == -4
+    torch.cuda.synchronize()
+    assert torch.equal(before, sess.arena)
+    assert mb.moebius_active_mode(sess.ctx) == TP
+    # a plan built for the new geometry runs
+    sess.free_plan(plan)
+    gpu_switch(st, sess, TP, owner, bt)
+    sess.close()

@@ -137,3 +137,20 @@ def test_calibration_and_argument_checks():
         mb.moebius_policy_create(mb.moebius_policy_config(10, 10, 0, 1.0), TP)     # W < 1
     with pytest.raises(mb.MoebiusError):
         mb.moebius_policy_calibrate([4, 4], [1, 1], [2, 2])                        # not ascending
+
+
+def test_a_rejected_sample_moves_neither_the_window_nor_the_cooldown():
+    """A call that fails argument validation (a negative length) must leave the policy as it was:
+    the next valid sample decides as if the bad one had never been sent (no cooldown started)."""
+    cfg = wl.get_config("tiny")
+    lens_ok = np.full(6, 10, np.int32)
+    sess = mb.Session(mb_config(cfg, lens_ok))
+    pol = mb.moebius_policy_create(mb.moebius_policy_config(5, 5, 1, 100.0), TP)   # T_h = T_l = 5, W = 1, C = 100 s
+    bad = lens_ok.copy()
+    bad[2] = -1
+    with pytest.raises(mb.MoebiusError):
+        mb.moebius_policy_step(pol, sess.ctx, 0.0, bad)
+    d, m = mb.moebius_policy_step(pol, sess.ctx, 1.0, lens_ok)       # 6 > T_h: switches right away
+    assert (d, m) == (mb.DECISION_SWITCH, EP)
+    mb.moebius_policy_destroy(pol)
+    sess.close()
