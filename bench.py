@@ -55,6 +55,8 @@ def parse():
     ap.add_argument("--w-orient", type=int, default=0, choices=[0, 1],
                     help="0: gate,up [E,H,I], down [E,I,H] (BASELINE.json, the headline); 1: the paper's W13 [E,2I,H], W2 [E,H,I] (named in config.workload)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-other-configs", action="store_true",
+                    help="default run only: skip timing configs 3, 5, 2 and the tight-pool variant after config 4")
     ap.add_argument("--profile-region", action="store_true",
                     help="cudaProfilerStart/Stop round warm-up + timed steps (ncu --profile-from-start off skips the fill)")
     ap.add_argument("--cpu-sample-requests", type=int, default=48)
@@ -71,16 +73,36 @@ def measured_peak():
     return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
 
 
+KERNEL_SOURCES = ("paper_2606_26607_b200/csrc/moebius_cuda.cu", "paper_2606_26607_b200/csrc/moebius_units.h")
+
+
+def kernel_sha16():
+    """First 16 hex digits of sha256 over the kernel's source files: ties a committed ncu figure to the
+    kernel it was measured on."""
+    import hashlib
+    h = hashlib.sha256()
+    for f in KERNEL_SOURCES:
+        h.update(open(os.path.join(ROOT, f), "rb").read())
+    return h.hexdigest()[:16]
+
+
 def committed_traffic(config_name):
-    """DRAM bytes per launch of the reshard kernel from the committed ncu --set full capture
-    (profiles/roofline_traffic.json-like text file written by hand from the capture), or None."""
+    """(traffic, source): DRAM bytes per launch of the reshard kernel (dram__bytes_read.sum +
+    dram__bytes_write.sum) from the committed ncu capture of this config, with where it came from.
+    None when there is no capture or when the kernel sources have changed since it was taken."""
     p = os.path.join(ROOT, "profiles", "traffic_%s.txt" % config_name)
     if not os.path.exists(p):
-        return None
+        return None, "no ncu capture committed for this config"
+    kv = {}
     for line in open(p):
-        if line.startswith("traffic_bytes_per_launch="):
-            return float(line.split("=", 1)[1])
-    return None
+        if "=" in line and not line.startswith("#"):
+            k, v = line.strip().split("=", 1)
+            kv[k] = v
+    if kv.get("kernel_sha16") != kernel_sha16():
+        return None, "stale: %s was captured on kernel %s, HEAD's kernel is %s" % (
+            os.path.relpath(p, ROOT), kv.get("kernel_sha16"), kernel_sha16())
+    return float(kv["traffic_bytes_per_launch"]), "%s (ncu, %s, commit %s)" % (
+        kv.get("capture", os.path.relpath(p, ROOT)), kv.get("command", "see profiles/README.md"), kv.get("commit", "?"))
 
 
 class ClockSampler(threading.Thread):
@@ -118,10 +140,10 @@ class ClockSampler(threading.Thread):
 
 # ---- the oracle, timed as it stands (cpu_baseline leg and --impl reference) ---------------------------
 
-def oracle_sample(cfg, n_sample_req, seed=0):
-    """Logical state of the bounded sample: layer 0 of the expert weights (gate, up, down, all E
-    experts) and layer 0's K and V of the first `n_sample_req` requests of the workload."""
-    rng = np.random.default_rng(seed)
+def oracle_sample(cfg, n_sample_req, layer=0, seed=0):
+    """Logical state of the bounded sample: ONE layer of the expert weights (gate, up, down, all E
+    experts) and that layer's K and V of the first `n_sample_req` requests of the workload."""
+    rng = np.random.default_rng((seed, layer))
     dt = {"bf16": np.uint16, "fp32": np.float32, "fp8_e4m3_b128": np.uint8}[cfg.w_dtype]
     W = {}
     for kind in cfg.w_kinds:
@@ -131,7 +153,7 @@ def oracle_sample(cfg, n_sample_req, seed=0):
         else:   # opaque bit patterns: generation cost is excluded from the timing anyway
             W[kind] = rng.integers(0, np.iinfo(dt).max, size=shape, dtype=dt, endpoint=True)
     lens = wl.draw_seq_lens(cfg)[:n_sample_req]
-    KV = [{i: wl.gen_kv_request(cfg, 0, kvi, i, int(n)) for i, n in enumerate(lens)} for kvi in range(2)]
+    KV = [{i: wl.gen_kv_request(cfg, layer, kvi, i, int(n)) for i, n in enumerate(lens)} for kvi in range(2)]
     return W, lens, KV
 
 
@@ -174,8 +196,15 @@ def oracle_sample_moved(cfg, lens, owner):
     return moved
 
 
-def time_oracle(cfg, n_sample_req, steps, warmup, pool_bytes):
-    W, lens, KV = oracle_sample(cfg, n_sample_req)
+def _sample_text(cfg, n_lens, layers):
+    return ("layer%s %s of %d: %s of all %d experts + K and V pools of the first %d of %d requests; "
+            "one TP->EP->TP round trip per step" % ("s" if len(layers) > 1 else "", ",".join(str(l) for l in layers), cfg.L,
+                                                    "/".join(cfg.w_kinds), cfg.E, n_lens, cfg.n_req))
+
+
+def time_oracle(cfg, n_sample_req, steps, warmup, pool_bytes, layer=0):
+    """Single-thread leg: the oracle as it stands on one layer's sample, in this process."""
+    W, lens, KV = oracle_sample(cfg, n_sample_req, layer)
     for _ in range(warmup):
         oracle_round_trip(cfg, W, lens, KV, pool_bytes)
     t0 = time.perf_counter()
@@ -183,10 +212,81 @@ def time_oracle(cfg, n_sample_req, steps, warmup, pool_bytes):
         owner = oracle_round_trip(cfg, W, lens, KV, pool_bytes)
     dt = time.perf_counter() - t0
     moved = steps * oracle_sample_moved(cfg, lens, owner)
-    sample = ("layer 0 of %d: %s of all %d experts + K and V pools of the first %d of %d requests; "
-              "one TP->EP->TP round trip per step" % (cfg.L, "/".join(cfg.w_kinds), cfg.E, len(lens), cfg.n_req))
-    return {"value": moved / dt / 1e9, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample,
-            "seconds": dt, "ms_per_step": dt / steps * 1e3}
+    return {"value": moved / dt / 1e9, "unit": UNIT, "cores": 1, "kind": "oracle",
+            "sample": _sample_text(cfg, len(lens), [layer]), "seconds": dt, "ms_per_step": dt / steps * 1e3,
+            "moved_bytes": moved}
+
+
+def _oracle_worker(cfg, n_sample_req, pool_bytes, layer, ready, go, out):
+    """One process of the per-core leg: layers are independent, so worker w
+    builds the views of its own layer.  Generation happens before the common start signal."""
+    W, lens, KV = oracle_sample(cfg, n_sample_req, layer)
+    ready.put(layer)
+    go.wait()
+    t0 = time.perf_counter()
+    owner = oracle_round_trip(cfg, W, lens, KV, pool_bytes)
+    t1 = time.perf_counter()
+    out.put((layer, t0, t1, oracle_sample_moved(cfg, lens, owner)))
+
+
+def time_oracle_per_core(cfg, n_sample_req, pool_bytes, host_cores):
+    """Per-core leg: one oracle process per host core, each on its own layer (at most L processes, and
+    no more than the host memory allows: one layer of logical state + its views per process)."""
+    import multiprocessing as mp
+    layer_bytes = sum(int(np.prod(wl.weight_shape(cfg, k))) for k in cfg.w_kinds) * cfg.w_elem_bytes
+    try:
+        import psutil
+        avail = psutil.virtual_memory().available
+    except Exception:
+        avail = 32 << 30
+    by_mem = max(1, int(avail * 0.6 // max(1, int(layer_bytes * 1.6))))
+    n = max(1, min(host_cores, cfg.L, by_mem, 16))
+    ctx = mp.get_context("spawn")     # this process holds a CUDA context: never fork it
+    ready, out, go = ctx.Queue(), ctx.Queue(), ctx.Event()
+    procs = [ctx.Process(target=_oracle_worker, args=(cfg, n_sample_req, pool_bytes, l, ready, go, out)) for l in range(n)]
+    for p in procs:
+        p.start()
+
+    def take(q, deadline_s=600):      # a worker that died must not leave the bench waiting
+        t_end = time.time() + deadline_s
+        while True:
+            try:
+                return q.get(timeout=1.0)
+            except Exception:
+                if any(p.exitcode not in (None, 0) for p in procs) or time.time() > t_end:
+                    for p in procs:
+                        if p.is_alive():
+                            p.terminate()
+                    raise RuntimeError("an oracle worker exited early")
+
+    for _ in procs:
+        take(ready)
+    go.set()
+    res = [take(out) for _ in procs]
+    for p in procs:
+        p.join(timeout=60)
+    t0, t1 = min(r[1] for r in res), max(r[2] for r in res)    # perf_counter is system-wide on Linux
+    moved = sum(r[3] for r in res)
+    return {"value": moved / (t1 - t0) / 1e9, "unit": UNIT, "cores": n, "kind": "oracle",
+            "sample": _sample_text(cfg, min(n_sample_req, cfg.n_req), list(range(n))) + "; one process per layer, concurrently",
+            "seconds": t1 - t0}
+
+
+def cpu_baseline(cfg, n_sample_req, pool_bytes, per_core=True):
+    """the oracle timed once single-threaded and once with one process per host
+    core over layers; `cores` = what the reported leg actually used, `host_cores` = sched_getaffinity."""
+    host_cores = len(os.sched_getaffinity(0))
+    one = time_oracle(cfg, n_sample_req, 1, 0, pool_bytes)
+    out = {"value": one["value"], "unit": UNIT, "cores": 1, "kind": "oracle", "sample": one["sample"],
+           "host_cores": host_cores, "single_thread": {"value": one["value"], "cores": 1, "seconds": one["seconds"]}}
+    if per_core and host_cores > 1:
+        try:
+            many = time_oracle_per_core(cfg, n_sample_req, pool_bytes, host_cores)
+            out.update({"value": many["value"], "cores": many["cores"], "sample": many["sample"],
+                        "per_core": {"value": many["value"], "cores": many["cores"], "seconds": many["seconds"]}})
+        except Exception as e:      # a reported baseline must not take the bench line down
+            out["per_core"] = {"error": repr(e)[:200]}
+    return out
 
 
 def run_reference(args):
@@ -203,7 +303,7 @@ def run_reference(args):
             "scaling": "weak", "vs_baseline": None, "dtype": "u8", "data": "synthetic",
             "config": {"workload": cfg.name, "sample": r["sample"]},
             "cpu_baseline": {"value": r["value"], "unit": UNIT, "cores": r["cores"], "kind": "oracle",
-                             "sample": r["sample"]},
+                             "sample": r["sample"], "host_cores": len(os.sched_getaffinity(0))},
             "e2e": {"value": r["value"], "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0}
     print(json.dumps(line))
@@ -230,12 +330,9 @@ def fill_device(sess, cfg, mb, torch):
                 sess.view(mb.MOEBIUS_TP, r, l, t).view(torch.bfloat16).normal_(0.0, 1.0, generator=g)
 
 
-def run_moebius(args):
+def init_device():
     import torch
     import torch.distributed as dist
-
-    import paper_2606_26607_b200 as mb   # fails loudly if libmoebius.so is missing: no CPU fallback
-
     world = int(os.environ.get("WORLD_SIZE", "1"))
     rank = int(os.environ.get("RANK", "0"))
     local = int(os.environ.get("LOCAL_RANK", "0"))
@@ -245,14 +342,25 @@ def run_moebius(args):
     dev = "cuda:%d" % local
     if world > 1:
         dist.init_process_group("nccl", device_id=torch.device(dev))
+    return world, rank, local, dev
 
-    cfg = wl.get_config(args.config)
+
+def run_moebius(args, env, config_name, pool_policy, cap_frac, steps, warmup, full=True):
+    """Times one workload.  full=False (the other_configs entries): kernel times only -- no D2D
+    comparison copy, no e2e loop."""
+    import torch
+    import torch.distributed as dist
+
+    import paper_2606_26607_b200 as mb   # fails loudly if libmoebius.so is missing: no CPU fallback
+
+    world, rank, local, dev = env
+    cfg = wl.get_config(config_name)
     if args.layers:
         cfg = cfg.with_(L=args.layers, name="%s[L=%d]" % (cfg.name, args.layers))
     if args.w_orient:
         cfg = cfg.with_(w_orient=1, name="%s[w_orient=1]" % cfg.name)
     lens = wl.draw_seq_lens(cfg)
-    pool = wl.kv_pool_bytes(cfg, lens, args.pool)
+    pool = wl.kv_pool_bytes(cfg, lens, pool_policy)
     if args.n_req >= 0:
         lens = lens[:args.n_req]
         cfg = cfg.with_(n_req=args.n_req, name="%s[n_req=%d]" % (cfg.name, args.n_req))
@@ -264,7 +372,7 @@ def run_moebius(args):
     probe = mb.Session(c)
     resident = probe.layout.resident_bytes
     probe.close()
-    c.staging_cap_bytes = int(args.staging_cap_frac * resident)   # BASELINE.json: cap at ~2.4% of resident bytes
+    c.staging_cap_bytes = int(cap_frac * resident)   # BASELINE.json: cap at ~2.4% of resident bytes
     sess = mb.Session(c, device=dev)
     lay = sess.layout
     if args.launch:
@@ -298,7 +406,7 @@ def run_moebius(args):
     # warm-up: W round trips (the first one starts from the random tables)
     owner, bt, mode = None, bt0, TP
     first_ms = {}
-    for w in range(max(args.warmup, 1)):
+    for w in range(max(warmup, 1)):
         for to in (EP, TP):
             plan, owner, bt, _ = switch(to, owner, bt, mode)
             if w == 0:
@@ -324,7 +432,7 @@ def run_moebius(args):
     sampler.start()
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     e0.record(stream)
-    for _ in range(args.steps):
+    for _ in range(steps):
         sess.reshard(plan_t2e)
         sess.reshard(plan_e2t)
     e1.record(stream)
@@ -334,11 +442,11 @@ def run_moebius(args):
     dev_ms = e0.elapsed_time(e1)
     if args.profile_region:
         torch.cuda.cudart().cudaProfilerStop()
-    hist = mb.moebius_kernel_ms_history(sess.ctx, 64)[-2 * args.steps:]
+    hist = mb.moebius_kernel_ms_history(sess.ctx, 64)[-2 * steps:]
     k_t2e, k_e2t = hist[0::2], hist[1::2]
     # context: a plain device-to-device copy of a weight slot on this box, now (read + write bytes)
     d2d = None
-    if cfg.R > 1:
+    if cfg.R > 1 and full:
         n_copy = int(min(lay.weight_slot_bytes * (3 * cfg.L), 8 << 30)) // 256 * 256
         t0_id = mb.T_GATE if cfg.w_orient == 0 else mb.T_W13
         a0 = sess.view_desc(TP, 0, 0, t0_id).offset
@@ -361,6 +469,10 @@ def run_moebius(args):
 
     sess.free_plan(plan_t2e)     # their pinned upload images go back to the context's pool
     sess.free_plan(plan_e2t)
+    if not full:
+        clocks = sampler.summary()
+        sess.close()
+        return {k: v for k, v in locals().items() if not isinstance(v, (torch.Tensor, mb.Session))}
     # e2e: host inputs -> plan -> reshard (uploads) -> device->host read-back of the published tables
     host_tables = torch.empty(lay.table_bytes // 4, dtype=torch.int32, pin_memory=True)
     tbl_n = lay.tbl_bt_off + n * mp
@@ -369,7 +481,7 @@ def run_moebius(args):
     owner, bt_cur, mode = None, bt, TP
     h2d = d2h = 0
     plan_ms = []
-    for _ in range(args.steps):
+    for _ in range(steps):
         # moebius_reshard only enqueues: the second switch of the step is planned on the host while the
         # first one runs on the device (its inputs are the first plan's tables, known on the host)
         live = []
@@ -388,7 +500,10 @@ def run_moebius(args):
             sess.free_plan(plan)
     e2e_s = time.perf_counter() - t0
     clocks = sampler.summary()
-    return locals()
+    sess.close()
+    # no tensor and no session leaves this function: the device buffers go back to torch before the next
+    # workload is built
+    return {k: v for k, v in locals().items() if not isinstance(v, (torch.Tensor, mb.Session))}
 
 
 def reduce_over_ranks(times_ms, amounts, world, device):
@@ -405,13 +520,58 @@ def reduce_over_ranks(times_ms, amounts, world, device):
     return [float(x) for x in t], [float(x) for x in b]
 
 
+def direction_summary(st, ms_list, peak):
+    avg = float(sum(ms_list) / max(len(ms_list), 1))
+    med = float(sorted(ms_list)[len(ms_list) // 2]) if ms_list else None
+    traffic = st["w_read"] + st["w_relocated"] + st["kv_read"] + st["kv_relocated"]
+    moved = st["w_moved"] + st["kv_moved"]
+    return {"kernel_ms_avg": avg, "kernel_ms_min": min(ms_list) if ms_list else None, "kernel_ms_median": med,
+            "moved_bytes": moved, "algorithmic_traffic_bytes": traffic,
+            "effective_GBps": moved / avg / 1e6 if avg else None,
+            "traffic_GBps": traffic / avg / 1e6 if avg else None,
+            "frac_strict_vs_8TBps": 2 * moved / (avg * 1e-3) / 8e12 if avg else None,
+            "frac_traffic_vs_measured": traffic / avg / 1e6 / peak if avg else None,
+            "units": st["n_units"], "segments": st["n_segments"], "kv_moves": st["n_kv_moves"],
+            "kv_rounds": st["n_kv_rounds"], "kv_staged": st["n_kv_staged"]}
+
+
+def split_history(hist):
+    m = len(hist) // 2 * 2
+    hist = hist[len(hist) - m:]
+    return hist[0::2], hist[1::2]
+
+
+# The parity-test configs of BASELINE.json and the cache-nearly-full variant of config 4, timed after the
+# headline workload in the default run so that the driver's record carries them too.
+OTHER_CONFIGS = (("qwen3_30b", "qwen3_30b", "roomy", 0.024), ("fp8_graph", "fp8_graph", "roomy", 0.024),
+                 ("small", "small", "roomy", 0.024), ("qwen3_235b_tight_pool", "qwen3_235b", "tight", 0.05))
+
+
+def other_config_entry(r, peak):
+    k_t2e, k_e2t = split_history(r["hist"])
+    a, b = direction_summary(r["st_t2e"], k_t2e, peak), direction_summary(r["st_e2t"], k_e2t, peak)
+    lay = r["lay"]
+    return {"workload": r["cfg"].name, "kv_pool": r["pool_policy"], "steps": r["steps"],
+            "tp2ep_ms": a["kernel_ms_avg"], "ep2tp_ms": b["kernel_ms_avg"],
+            "traffic_GBps": [a["traffic_GBps"], b["traffic_GBps"]],
+            "effective_GBps": [a["effective_GBps"], b["effective_GBps"]],
+            "frac_strict": [a["frac_strict_vs_8TBps"], b["frac_strict_vs_8TBps"]],
+            "frac_traffic_vs_measured": [a["frac_traffic_vs_measured"], b["frac_traffic_vs_measured"]],
+            "kv_rounds": [a["kv_rounds"], b["kv_rounds"]], "kv_staged": [a["kv_staged"], b["kv_staged"]],
+            "first_switch_from_random_tables": r["first_ms"],
+            "resident_GB": lay.resident_bytes / 1e9,
+            "spare_plus_staging_frac": (lay.weight_spare_bytes + lay.staging_bytes) / lay.resident_bytes,
+            "staging_cap_frac": r["cap_frac"], "ms_per_step": r["dev_ms"] / r["steps"], "clocks": r["clocks"]}
+
+
 def main():
     args = parse()
     if args.impl == "reference":
         return run_reference(args)
-    r = run_moebius(args)
     import torch
     import torch.distributed as dist
+    env = init_device()
+    r = run_moebius(args, env, args.config, args.pool, args.staging_cap_frac, args.steps, max(args.warmup, 1))
     world, rank, cfg, steps = r["world"], r["rank"], r["cfg"], args.steps
     st_t2e, st_e2t = r["st_t2e"], r["st_e2t"]
     moved_step = st_t2e["w_moved"] + st_t2e["kv_moved"] + st_e2t["w_moved"] + st_e2t["kv_moved"]
@@ -420,33 +580,16 @@ def main():
         if world > 1:
             dist.destroy_process_group()
         return
-    hist = r["hist"]
-    m = len(hist) // 2 * 2
-    hist = hist[len(hist) - m:]
-    k_t2e, k_e2t = hist[0::2], hist[1::2]
+    k_t2e, k_e2t = split_history(r["hist"])
     avg = lambda x: float(sum(x) / max(len(x), 1))  # noqa: E731
-    med = lambda x: float(sorted(x)[len(x) // 2]) if x else None  # noqa: E731
     peak, peak_src = measured_peak()
-
-    def direction(st, ms_list):
-        ms = avg(ms_list)
-        traffic = st["w_read"] + st["w_relocated"] + st["kv_read"] + st["kv_relocated"]
-        moved = st["w_moved"] + st["kv_moved"]
-        return {"kernel_ms_avg": ms, "kernel_ms_min": min(ms_list) if ms_list else None, "kernel_ms_median": med(ms_list),
-                "moved_bytes": moved, "algorithmic_traffic_bytes": traffic,
-                "effective_GBps": moved / ms / 1e6 if ms else None,
-                "traffic_GBps": traffic / ms / 1e6 if ms else None,
-                "frac_strict_vs_8TBps": 2 * moved / (ms * 1e-3) / 8e12 if ms else None,
-                "frac_traffic_vs_measured": traffic / ms / 1e6 / peak if ms else None,
-                "units": st["n_units"], "segments": st["n_segments"], "kv_moves": st["n_kv_moves"],
-                "kv_rounds": st["n_kv_rounds"], "kv_staged": st["n_kv_staged"]}
-
-    d_t2e, d_e2t = direction(st_t2e, k_t2e), direction(st_e2t, k_e2t)
+    d_t2e, d_e2t = direction_summary(st_t2e, k_t2e, peak), direction_summary(st_e2t, k_e2t, peak)
     # roofline of the dominant (only) kernel: algorithmic bytes per launch / average launch duration
     alg = (d_t2e["algorithmic_traffic_bytes"] + d_e2t["algorithmic_traffic_bytes"]) / 2
     k_ms = avg(k_t2e + k_e2t)
     achieved = alg / k_ms / 1e6
     lay = r["lay"]
+    traffic, traffic_src = committed_traffic(cfg.name) if args.pool == "roomy" else (None, "no capture for this pool policy")
     line = {
         "metric": METRIC, "value": moved_all * steps / dev_ms / 1e6, "unit": UNIT, "n_gpus": world, "steps": steps,
         "warmup": max(args.warmup, 1), "ms_per_step": dev_ms / steps, "higher_is_better": True, "scaling": "weak",
@@ -463,16 +606,35 @@ def main():
         "d2d_copy_same_box": r["d2d"],
         "plan_ms": {"tp2ep": r["plan_ms_t2e"], "ep2tp": r["plan_ms_e2t"], "e2e_avg": avg(r["plan_ms"])},
         "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                     "traffic": committed_traffic(cfg.name), "peak_source": peak_src,
+                     "frac_note": "vs the measured D2D copy rate of this pool (a copy, not a physical peak); "
+                                  "the strict fraction 2*moved/(t*8 TB/s) is in tp2ep/ep2tp.frac_strict_vs_8TBps",
+                     "traffic": traffic, "traffic_source": traffic_src, "kernel_sha16": kernel_sha16(),
+                     "peak_source": peak_src,
                      "kernel": "moebius_reshard_kernel", "algorithmic_bytes_per_launch": alg, "kernel_ms_avg": k_ms},
         "e2e": {"value": moved_all * steps / e2e_ms / 1e6, "unit": UNIT, "ms_per_step": e2e_ms / steps,
                 "h2d_bytes_per_step": r["h2d"] / steps, "d2h_bytes_per_step": r["d2h"] / steps},
         "gpu_launches": 2 * steps * world,
         "clocks": r["clocks"],
     }
+    pool_bytes = r["pool"]
+    del r
+    # the other BASELINE.json configs, driver-timed in the same run (1 GPU, default workload only)
+    if world == 1 and not args.no_other_configs and args.config == "qwen3_235b" and args.pool == "roomy" \
+            and not args.layers and args.n_req < 0 and not args.w_orient:
+        torch.cuda.empty_cache()
+        others = {}
+        for key, name, pool_policy, cap in OTHER_CONFIGS:
+            try:
+                ro = run_moebius(args, env, name, pool_policy, cap, min(steps, 10), 3, full=False)
+                others[key] = other_config_entry(ro, peak)
+                line["gpu_launches"] += 2 * ro["steps"]
+                del ro
+            except Exception as e:      # one failing side workload must not cost the headline line
+                others[key] = {"error": repr(e)[:300]}
+            torch.cuda.empty_cache()
+        line["other_configs"] = others
     if not args.no_cpu_baseline:
-        cb = time_oracle(cfg, args.cpu_sample_requests, 1, 0, r["pool"])
-        line["cpu_baseline"] = {k: cb[k] for k in ("value", "unit", "cores", "kind", "sample")}
+        line["cpu_baseline"] = cpu_baseline(cfg, args.cpu_sample_requests, pool_bytes)
     print(json.dumps(line))
     if world > 1:
         dist.destroy_process_group()

@@ -452,7 +452,7 @@ def test_reshard_checks_come_before_the_first_enqueue():
     st, sess = gpu_session(SMALLISH.with_(L=1))
     owner, bt, _ = start(st, sess, TP, "random")
     plan = sess.plan(EP, st.lens, owner, bt, from_mode=TP)
-    mb.moebius_set_tma(sess.ctx, 1, 2, 32)
+    mb.moebius_set_tma(sess.ctx, 1, 1, 64)      # the default stage here is one 32-KB EP page
     torch.cuda.synchronize()
     before = sess.arena.clone()
     with pytest.raises(mb.MoebiusError) as e:
