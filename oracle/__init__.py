@@ -21,4 +21,8 @@ from .kv import (  # noqa: F401
 from .accounting import kv_bytes, scale_bytes, weight_bytes  # noqa: F401
 from .ffn import moe_ffn_dense, moe_ffn_ep, moe_ffn_tp, route_top2  # noqa: F401
 from .ffn import moe_ffn_dense_w13, moe_ffn_ep_w13, moe_ffn_tp_w13  # noqa: F401
+from .attention import (  # noqa: F401
+    ATTN_KINDS, attn_bytes, attn_ep_view, attn_forward_dense, attn_forward_ep, attn_forward_tp, attn_shape, attn_tp_view,
+    q_heads_of_rank,
+)
 from .image import OracleLayout, State, np_view, target_request_state  # noqa: F401,E402
