@@ -53,8 +53,23 @@ typedef enum {
   MOEBIUS_T_GATE_SCALE = 5, MOEBIUS_T_UP_SCALE = 6, MOEBIUS_T_DOWN_SCALE = 7, /* fp8 only */
   /* w_orient = 1 (the paper's own shapes): ids 0..2 and 5..7 are invalid, these are valid */
   MOEBIUS_T_W13 = 8, MOEBIUS_T_W2 = 9,
-  MOEBIUS_T_W13_SCALE = 10, MOEBIUS_T_W2_SCALE = 11 /* fp8 only */
+  MOEBIUS_T_W13_SCALE = 10, MOEBIUS_T_W2_SCALE = 11, /* fp8 only */
+  /* attention projections (attn_mode != 0): wq [Hq,D,H], wk/wv [Hkv,D,H], wo [H,Hq,D] */
+  MOEBIUS_T_WQ = 12, MOEBIUS_T_WK = 13, MOEBIUS_T_WV = 14, MOEBIUS_T_WO = 15
 } moebius_tensor_t;
+
+/* How the attention projections follow a switch. */
+typedef enum {
+  MOEBIUS_ATTN_NONE = 0,   /* no attention tensors in the unified buffer                              */
+  MOEBIUS_ATTN_DUAL = 1,   /* the paper's default: the full copy (EP) and the head shard (TP) are both
+                              resident at fixed views; a switch moves nothing ("pointer swap": the
+                              caller reads the views of the published active mode), at the price of
+                              one duplicated head shard per rank                                      */
+  MOEBIUS_ATTN_GATHER = 2  /* the memory-saving variant: one full-size tensor per rank; the TP view of
+                              a rank is its head shard IN PLACE inside it (a strided view for wo), so
+                              EP->TP keeps the local slice (nothing moves) and TP->EP rebuilds the
+                              rest from the other ranks' shards (the paper's All-Gather)              */
+} moebius_attn_mode_t;
 
 typedef enum {
   MOEBIUS_OK = 0,
@@ -83,8 +98,11 @@ typedef struct {
   int64_t kv_pool_bytes_per_rank_layer; /* capacity of ONE K (or V) pool of one rank and layer; a
                                  multiple of the EP page size page_tokens*kv_heads*head_dim*b    */
   int32_t max_requests, max_pages_per_request;
-  int64_t staging_cap_bytes;  /* upper bound for spare weight slot (all ranks) + KV staging, e.g.
-                                 0.024 * resident (reading A12).  0 = no bound.     */
+  int64_t staging_cap_bytes;  /* upper bound for spare weight slot (all ranks) + KV staging (+ the
+                                 duplicated attention shards of MOEBIUS_ATTN_DUAL), e.g.
+                                 0.024 * resident (reading A12).  0 = no bound. */
+  int32_t n_q_heads;          /* query heads Hq (attn_mode != 0): Hq % R == 0, Hq % kv_heads == 0   */
+  int32_t attn_mode;          /* moebius_attn_mode_t; attention weights are bf16                    */
 } moebius_config_t;
 
 /* Sizes the caller must allocate, and where things are.  All byte counts. */
@@ -104,9 +122,14 @@ typedef struct {
      max_requests, max_pages_per_request, 0...}, then owner[max_requests] (-1 = all
      ranks, TP), seq_lens[max_requests], block_tables[max_requests][max_pages_per_request] (-1 pad) */
   int32_t tbl_owner_off, tbl_lens_off, tbl_bt_off, tbl_reserved;
+  int64_t attn_full_bytes;              /* full q/k/v/o copies, all ranks and layers (0 without attention) */
+  int64_t attn_dup_bytes;               /* MOEBIUS_ATTN_DUAL: the head shards held beside them, all ranks
+                                           (1.7 GB per GPU for Qwen3-235B)              */
 } moebius_layout_t;
 
-/* One dense row-major view; offset in bytes from dev_base; shape/stride in elements. */
+/* One view; offset in bytes from dev_base; shape/stride in elements.  Every view is dense row-major
+ * except the TP view of wo under MOEBIUS_ATTN_GATHER, whose head-shard columns sit in place inside
+ * the full [H, Hq, D] tensor (stride[0] = Hq*D). */
 typedef struct {
   uint32_t struct_size;
   int32_t ndim, elem_bytes;
@@ -124,6 +147,7 @@ typedef struct {
   int64_t kv_moved, kv_relocated, kv_read;
   int64_t staging_used_bytes;            /* KV staging this plan uses                             */
   int64_t desc_upload_bytes, table_upload_bytes;
+  int64_t attn_moved, attn_relocated, attn_read;   /* attention projections (MOEBIUS_ATTN_GATHER, TP->EP) */
 } moebius_stats_t;
 
 /* ---- context (host only) ------------------------------------------------------------------ */
@@ -179,8 +203,8 @@ MOEBIUS_API int moebius_plan_stats(const moebius_plan_t* plan, moebius_stats_t* 
 
 /* Diagnostic dump of the work list for host-side hazard checking (tests).  what: 0 = segments
  * (moebius_segment_t-sized records), 1 = KV move descriptors (16 B each), 2 = 2-D
- * copy descriptors (32 B each), 3 = the dependency wave of every segment (int32 each).  buf: HOST, cap
- * bytes; *needed receives the full size. */
+ * copy descriptors (32 B each), 3 = the dependency wave of every segment (int32 each), 4 = bulk copy
+ * descriptors (16 B each).  buf: HOST, cap bytes; *needed receives the full size. */
 MOEBIUS_API int moebius_plan_export(const moebius_plan_t* plan, int what, void* buf, int64_t cap,
                                     int64_t* needed);
 

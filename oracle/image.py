@@ -4,7 +4,9 @@ The oracle does not know the address map: the caller passes `view_fn(mode, rank,
 -> (byte_offset, shape, elem_bytes)` (the fixed views the library reports) and the
 pool page counts.  Nothing here imports the CUDA path.  mode: 0 = TP, 1 = EP; tensor ids: 0 gate,
 1 up, 2 down, 3 K pool, 4 V pool, 5/6/7 fp8 scales of gate/up/down; paper orientation (w_orient = 1,
-PAPER.md:100): 8 W13, 9 W2, 10/11 their fp8 scales.
+PAPER.md:100): 8 W13, 9 W2, 10/11 their fp8 scales; attention projections: 12 wq, 13 wk,
+14 wv, 15 wo.  A view description may carry a 4th item, its strides in elements (the TP view of wo in
+the memory-saving variant sits in place inside the full tensor).
 """
 from __future__ import annotations
 
@@ -12,10 +14,12 @@ import numpy as np
 
 import workloads as wl
 
+from . import attention as oat
 from . import kv as okv
 from . import weights as ow
 
 KINDS = ("gate", "up", "down")
+ATTN_IDS = {"wq": 12, "wk": 13, "wv": 14, "wo": 15}
 TP, EP = 0, 1
 
 
@@ -45,6 +49,9 @@ class State:
     def scale(self, layer, kind):
         return wl.gen_logical_scale(self.cfg, layer, kind)
 
+    def attn(self, layer, kind):
+        return wl.gen_attn_weight(self.cfg, layer, kind, fill=self.fill)
+
     def kv(self, layer, kvi):
         key = (layer, kvi)
         if key not in self._kv:
@@ -58,9 +65,19 @@ class State:
 
 
 def np_view(image: np.ndarray, desc):
-    off, shape, eb = desc
+    off, shape, eb = desc[:3]
     dt = {1: np.uint8, 2: np.uint16, 4: np.float32}[eb]
     n = int(np.prod(shape)) * eb
+    if len(desc) > 3 and desc[3] is not None:
+        strides = tuple(desc[3])
+        dense, st = [], 1
+        for d in reversed(shape):
+            dense.insert(0, st)
+            st *= d
+        if tuple(dense) != strides:        # a strided window onto the image (writable)
+            span = (sum((d - 1) * s for d, s in zip(shape, strides)) + 1) * eb
+            flat = image[off:off + span].view(dt)
+            return np.lib.stride_tricks.as_strided(flat, shape=shape, strides=tuple(s * eb for s in strides))
     return image[off:off + n].view(dt).reshape(shape)
 
 
@@ -81,6 +98,19 @@ class OracleLayout:
         c = self.st.cfg
         return ow.tp_scale_view(S, kind, r, c.R, c.I) if self.mode == TP else ow.ep_scale_view(S, r, c.R)
 
+    def attn_view(self, r, layer, kind, mode=None):
+        c = self.st.cfg
+        X = self.st.attn(layer, kind)
+        if (self.mode if mode is None else mode) == TP:
+            return oat.attn_tp_view(X, kind, r, c.R, c.n_q_heads, c.kv_heads)
+        return oat.attn_ep_view(X, r, c.R)
+
+    def attn_modes(self):
+        """Which modes' attention views hold valid bytes while the buffer is in self.mode: both when both
+        layouts are kept resident (attn_mode 1, PAPER.md:112 'pointer swap'), else the active one only."""
+        m = getattr(self.st.cfg, "attn_mode", 0)
+        return () if not m else ((TP, EP) if m == 1 else (self.mode,))
+
     def pool(self, r, layer, kvi):
         c = self.st.cfg
         KV = self.st.kv(layer, kvi)
@@ -98,6 +128,9 @@ class OracleLayout:
                     np_view(image, self.view_fn(self.mode, r, l, tid))[...] = self.weight_view(r, l, kind)
                     if fp8:
                         np_view(image, self.view_fn(self.mode, r, l, sid))[...] = self.scale_view(r, l, kind)
+                for m in self.attn_modes():
+                    for kind, tid in ATTN_IDS.items():
+                        np_view(image, self.view_fn(m, r, l, tid))[...] = self.attn_view(r, l, kind, m)
                 for kvi in range(2):
                     pool, mask = self.pool(r, l, kvi)
                     np_view(image, self.view_fn(self.mode, r, l, 3 + kvi))[mask] = pool[mask]
@@ -120,6 +153,12 @@ class OracleLayout:
                         want = self.scale_view(r, l, kind)
                         if not np.array_equal(got.view(np.uint32), want.view(np.uint32)):
                             bad.append("scale r%d l%d %s" % (r, l, kind))
+                for m in self.attn_modes():
+                    for kind, tid in ATTN_IDS.items():
+                        got = np_view(image, self.view_fn(m, r, l, tid))
+                        want = self.attn_view(r, l, kind, m)
+                        if got.shape != want.shape or not np.array_equal(got, want):
+                            bad.append("attn r%d l%d %s (%s view)" % (r, l, kind, "TP" if m == TP else "EP"))
                 for kvi in range(2):
                     pool, mask = self.pool(r, l, kvi)
                     got = np_view(image, self.view_fn(self.mode, r, l, 3 + kvi))

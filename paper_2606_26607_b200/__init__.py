@@ -8,7 +8,7 @@ Importing this package fails loudly if the library has not been built
 from ._binding import (  # noqa: F401
     MOEBIUS_TP, MOEBIUS_EP, MOEBIUS_BF16, MOEBIUS_FP32, MOEBIUS_FP8_E4M3_B128,
     T_GATE, T_UP, T_DOWN, T_KPOOL, T_VPOOL, T_GATE_SCALE, T_UP_SCALE, T_DOWN_SCALE,
-    T_W13, T_W2, T_W13_SCALE, T_W2_SCALE,
+    T_W13, T_W2, T_W13_SCALE, T_W2_SCALE, T_WQ, T_WK, T_WV, T_WO, ATTN_NONE, ATTN_DUAL, ATTN_GATHER,
     MoebiusError, moebius_config_t, moebius_layout_t, moebius_view_t, moebius_stats_t,
     moebius_create, moebius_destroy, moebius_layout, moebius_view, moebius_bind, moebius_active_mode,
     moebius_plan, moebius_plan_destroy, moebius_block_tables, moebius_plan_stats, moebius_plan_export,
@@ -19,6 +19,6 @@ from ._binding import (  # noqa: F401
     moebius_share_stats, moebius_plan_waves, moebius_reshard_share, moebius_reshard_publish,
     moebius_arena_create, moebius_arena_destroy, moebius_arena_base, moebius_arena_ready, moebius_arena_export,
     moebius_arena_import,
-    moebius_status_str, moebius_version, lib_path, EXPORTED_SYMBOLS, SEG_DTYPE, KV_DTYPE, C2D_DTYPE,
+    moebius_status_str, moebius_version, lib_path, EXPORTED_SYMBOLS, SEG_DTYPE, KV_DTYPE, C2D_DTYPE, BULK_DTYPE,
 )
 from .session import Session, make_config  # noqa: F401

@@ -13,6 +13,8 @@ MOEBIUS_TP, MOEBIUS_EP = 0, 1
 MOEBIUS_BF16, MOEBIUS_FP32, MOEBIUS_FP8_E4M3_B128 = 0, 1, 2
 T_GATE, T_UP, T_DOWN, T_KPOOL, T_VPOOL, T_GATE_SCALE, T_UP_SCALE, T_DOWN_SCALE = range(8)
 T_W13, T_W2, T_W13_SCALE, T_W2_SCALE = range(8, 12)   # w_orient = 1
+T_WQ, T_WK, T_WV, T_WO = range(12, 16)                 # attention projections
+ATTN_NONE, ATTN_DUAL, ATTN_GATHER = 0, 1, 2
 
 EXPORTED_SYMBOLS = [
     "moebius_create", "moebius_destroy", "moebius_layout", "moebius_view", "moebius_bind",
@@ -39,7 +41,7 @@ class moebius_config_t(C.Structure):
                 ("kv_heads", C.c_int32), ("head_dim", C.c_int32), ("page_tokens", C.c_int32),
                 ("kv_dtype", C.c_int32), ("kv_pool_bytes_per_rank_layer", C.c_int64),
                 ("max_requests", C.c_int32), ("max_pages_per_request", C.c_int32),
-                ("staging_cap_bytes", C.c_int64)]
+                ("staging_cap_bytes", C.c_int64), ("n_q_heads", C.c_int32), ("attn_mode", C.c_int32)]
 
 
 class moebius_policy_config_t(C.Structure):
@@ -57,7 +59,8 @@ class moebius_layout_t(C.Structure):
                 ("rank_stride_bytes", C.c_int64), ("weight_slot_bytes", C.c_int64),
                 ("weight_spare_bytes", C.c_int64), ("staging_bytes", C.c_int64), ("desc_bytes", C.c_int64),
                 ("table_bytes", C.c_int64), ("resident_bytes", C.c_int64), ("tbl_owner_off", C.c_int32),
-                ("tbl_lens_off", C.c_int32), ("tbl_bt_off", C.c_int32), ("tbl_reserved", C.c_int32)]
+                ("tbl_lens_off", C.c_int32), ("tbl_bt_off", C.c_int32), ("tbl_reserved", C.c_int32),
+                ("attn_full_bytes", C.c_int64), ("attn_dup_bytes", C.c_int64)]
 
 
 class moebius_view_t(C.Structure):
@@ -71,7 +74,8 @@ class moebius_stats_t(C.Structure):
                 ("n_units", C.c_int64), ("w_moved", C.c_int64), ("w_relocated", C.c_int64),
                 ("w_read", C.c_int64), ("kv_moved", C.c_int64), ("kv_relocated", C.c_int64),
                 ("kv_read", C.c_int64), ("staging_used_bytes", C.c_int64),
-                ("desc_upload_bytes", C.c_int64), ("table_upload_bytes", C.c_int64)]
+                ("desc_upload_bytes", C.c_int64), ("table_upload_bytes", C.c_int64),
+                ("attn_moved", C.c_int64), ("attn_relocated", C.c_int64), ("attn_read", C.c_int64)]
 
     def as_dict(self):
         return {k: getattr(self, k) for k, _ in self._fields_ if k != "struct_size"}
@@ -89,7 +93,8 @@ SEG_DTYPE = np.dtype([
 KV_DTYPE = np.dtype([("ep_rank", "<i4"), ("ep_page", "<i4"), ("tp_page", "<i4"), ("ntok_slot", "<u4")])
 C2D_DTYPE = np.dtype([("src_off", "<i8"), ("dst_off", "<i8"), ("rows", "<u4"), ("run_bytes", "<u4"),
                       ("src_stride", "<u4"), ("dst_stride", "<u4")])
-assert SEG_DTYPE.itemsize == 128 and KV_DTYPE.itemsize == 16 and C2D_DTYPE.itemsize == 32
+BULK_DTYPE = np.dtype([("src_off", "<i8"), ("dst_off", "<i8")])
+assert SEG_DTYPE.itemsize == 128 and KV_DTYPE.itemsize == 16 and C2D_DTYPE.itemsize == 32 and BULK_DTYPE.itemsize == 16
 
 
 def lib_path() -> str:
@@ -240,7 +245,7 @@ def moebius_plan_stats(plan) -> moebius_stats_t:
 
 
 def moebius_plan_export(plan, what: int) -> np.ndarray:
-    dt = (SEG_DTYPE, KV_DTYPE, C2D_DTYPE, np.dtype("<i4"))[what]
+    dt = (SEG_DTYPE, KV_DTYPE, C2D_DTYPE, np.dtype("<i4"), BULK_DTYPE)[what]
     need = C.c_int64(0)
     _chk(_lib.moebius_plan_export(plan, what, None, 0, C.byref(need)), "moebius_plan_export")
     buf = np.zeros(need.value // dt.itemsize, dtype=dt)

@@ -206,6 +206,18 @@ __device__ __forceinline__ KvDesc tma_prefetch_desc(const DevParams& p, const Se
 __device__ __forceinline__ void tma_issue_load(const TmaCtx& c, const Seg& s, uint32_t ul, const KvDesc& d, char* stage,
                                                uint64_t* bar, uint32_t lane) {
   const DevParams& p = *c.p;
+  if (seg_kind(s) == SEG_BULK) {                      // strided rows -> dense stage [row][piece]
+    BulkUnit b;
+    decode_bulk(s, p, ul, b);
+    if (lane == 0) mbar_expect_tx(bar, b.nrows * b.piece);
+    __syncwarp();
+    if (b.src_stride == (int64_t)b.piece) {
+      if (lane == 0) bulk_g2s(stage, b.src, b.nrows * b.piece, bar);
+    } else {
+      for (uint32_t t = lane; t < b.nrows; t += 32) bulk_g2s(stage + (size_t)t * b.piece, b.src + (int64_t)t * b.src_stride, b.piece, bar);
+    }
+    return;
+  }
   if (seg_kind(s) == SEG_XPOSE) {
     Box b;
     decode_box(s, p, ul, 0, b);
@@ -269,6 +281,17 @@ __device__ __forceinline__ void tma_issue_load(const TmaCtx& c, const Seg& s, ui
 __device__ __forceinline__ void tma_issue_store(const TmaCtx& c, const Seg& s, uint32_t ul, const KvDesc& d, char* stage,
                                                 uint32_t lane) {
   const DevParams& p = *c.p;
+  if (seg_kind(s) == SEG_BULK) {
+    BulkUnit b;
+    decode_bulk(s, p, ul, b);
+    if (b.dst_stride == (int64_t)b.piece) {
+      if (lane == 0) bulk_s2g(b.dst, stage, b.nrows * b.piece);
+    } else {
+      for (uint32_t t = lane; t < b.nrows; t += 32) bulk_s2g(b.dst + (int64_t)t * b.dst_stride, stage + (size_t)t * b.piece, b.piece);
+    }
+    bulk_commit();
+    return;
+  }
   if (seg_kind(s) == SEG_XPOSE) {
     Box b;
     decode_box(s, p, ul, 0, b);
@@ -324,6 +347,12 @@ __device__ __forceinline__ void lsu_unit(const Seg& s, const DevParams& p, uint3
     c2d_copy(p.c2d[s.desc_begin + ul], p.base, lane);
     return;
   }
+  if (seg_kind(s) == SEG_BULK) {
+    BulkUnit b;
+    decode_bulk(s, p, ul, b);
+    for (uint32_t t = 0; t < b.nrows; ++t) lin_copy(b.src + (int64_t)t * b.src_stride, b.dst + (int64_t)t * b.dst_stride, b.piece, lane);
+    return;
+  }
   const uint32_t nb = seg_boxes(s, ul);
   for (uint32_t k = 0; k < nb; ++k) {
     Box b;
@@ -354,6 +383,7 @@ moebius_reshard_kernel(const __grid_constant__ DevParams p_in, const __grid_cons
     p.segs = (const Seg*)((const char*)p_in.hdr + sizeof(PlanHdr));
     p.kv = (const KvDesc*)((const char*)p_in.hdr + (int64_t)(int32_t)h.z);     // signed: a wave header sits
     p.c2d = (const C2dDesc*)((const char*)p_in.hdr + (int64_t)(int32_t)h.w);   // behind the arrays it uses
+    p.bulk = (const BulkDesc*)((const char*)p_in.hdr + (int64_t)(int32_t)__ldg(&p_in.hdr->bulk_off));
   }
   const uint32_t lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   uint64_t* bar = (uint64_t*)smem + 2 * warp;                       // 2 barriers per pipe

@@ -73,6 +73,11 @@ struct moebius_ctx {
   int64_t w_off, scale_tp_off, scale_ep_off, kv_off, rank_stride;
   moebius::ScaleGeom sg[3];
   int64_t scale_tp_layer, scale_ep_layer;  // bytes per layer per rank
+  // attention projections (attn_mode != 0): per rank and layer the four full tensors,
+  // then (MOEBIUS_ATTN_DUAL) the four head shards; offsets within one layer's block
+  int64_t attn_off, attn_layer_bytes, attn_full_off[4], attn_shard_off[4], attn_full_sz[4], attn_shard_sz[4];
+  int64_t attn_full_bytes, attn_dup_bytes;   // all ranks and layers
+  int64_t max_bulk;
   int G, rep, hpr;
   int64_t run_kv, ep_page_bytes, tp_page_bytes, pool_bytes;
   int32_t pages_ep, pages_tp;
@@ -123,6 +128,7 @@ struct moebius_plan {
   int from, to, n_req;
   std::vector<moebius::Seg> segs;
   std::vector<moebius::C2dDesc> c2d;
+  std::vector<moebius::BulkDesc> bulk;
   const moebius::KvDesc* kv;      // n_kv descriptors, inside `image`
   int64_t n_kv;
   std::vector<int32_t> lens, owner;   // target-mode request state
@@ -133,7 +139,7 @@ struct moebius_plan {
   int64_t stage_bytes; int xt_rows;   // geometry the plan was built for
   // one contiguous upload image: [segs][kv][c2d], and the table image; pinned when CUDA allows
   char* image;
-  int64_t image_bytes, kv_img_off, c2d_img_off;
+  int64_t image_bytes, kv_img_off, c2d_img_off, bulk_img_off;
   // rank-share execution (multi-GPU): per dependency wave a header + segment list inside the image
   int32_t n_waves;
   int64_t wave_img_off;

@@ -73,6 +73,12 @@ int moebius_create(const moebius_config_t* c, moebius_ctx_t** out) {
   if (!(Hkv % R == 0 || R % Hkv == 0)) return MOEBIUS_E_INVAL;
   if (c->max_requests < 0 || c->max_pages_per_request < 0) return MOEBIUS_E_INVAL;
   if (c->staging_cap_bytes < 0 || c->kv_pool_bytes_per_rank_layer < 0) return MOEBIUS_E_INVAL;
+  if (c->attn_mode < MOEBIUS_ATTN_NONE || c->attn_mode > MOEBIUS_ATTN_GATHER) return MOEBIUS_E_INVAL;
+  if (c->attn_mode != MOEBIUS_ATTN_NONE) {
+    const int Hq = c->n_q_heads;
+    if (Hq < 1 || Hq % R || Hq % Hkv) return MOEBIUS_E_INVAL;
+    if (((int64_t)D * H * 2) % 16 || ((int64_t)(Hq / R) * D * 2) % 16) return MOEBIUS_E_INVAL;
+  }
 
   moebius_ctx* x = new (std::nothrow) moebius_ctx();
   if (!x) return MOEBIUS_E_INVAL;
@@ -125,18 +131,45 @@ int moebius_create(const moebius_config_t* c, moebius_ctx_t** out) {
   }
   x->scale_tp_off = off;  off += x->scale_tp_layer * L;
   x->scale_ep_off = off;  off += x->scale_ep_layer * L;
+  // attention projections, bf16: wq [Hq,D,H], wk/wv [Hkv,D,H], wo [H,Hq,D] (reading A19)
+  x->attn_off = align_up(off, 256);
+  x->attn_layer_bytes = x->attn_full_bytes = x->attn_dup_bytes = 0;
+  memset(x->attn_full_off, 0, sizeof(x->attn_full_off)); memset(x->attn_shard_off, 0, sizeof(x->attn_shard_off));
+  memset(x->attn_full_sz, 0, sizeof(x->attn_full_sz));   memset(x->attn_shard_sz, 0, sizeof(x->attn_shard_sz));
+  if (c->attn_mode != MOEBIUS_ATTN_NONE) {
+    const int64_t head = (int64_t)D * H * 2;
+    const int Hq = c->n_q_heads;
+    const int64_t full[4] = {Hq * head, Hkv * head, Hkv * head, Hq * head};
+    const int64_t shard[4] = {(Hq / R) * head, x->hpr * head, x->hpr * head, (Hq / R) * head};
+    int64_t at = 0, sum_full = 0, sum_shard = 0;
+    for (int t = 0; t < 4; ++t) { x->attn_full_off[t] = at; x->attn_full_sz[t] = full[t]; at += align_up(full[t], 256); sum_full += full[t]; }
+    for (int t = 0; t < 4; ++t) {
+      x->attn_shard_sz[t] = shard[t];
+      sum_shard += shard[t];
+      if (c->attn_mode == MOEBIUS_ATTN_DUAL) { x->attn_shard_off[t] = at; at += align_up(shard[t], 256); }
+    }
+    x->attn_layer_bytes = at;
+    x->attn_full_bytes = sum_full * L * R;
+    x->attn_dup_bytes = c->attn_mode == MOEBIUS_ATTN_DUAL ? sum_shard * L * R : 0;
+    off = x->attn_off + x->attn_layer_bytes * L;
+  }
   off = align_up(off, 4096);
   x->kv_off = off;        off += 2 * (int64_t)L * x->pool_bytes;
   x->rank_stride = align_up(off, 2 << 20);   // 2 MiB: a rank region can be its own physical allocation (moebius_arena_*)
 
   x->spare_bytes = (int64_t)x->ep_shift * x->S * R;
-  x->resident_bytes = (int64_t)3 * L * x->S * R + 2 * (int64_t)L * x->pool_bytes * R;
+  x->resident_bytes = (int64_t)3 * L * x->S * R + 2 * (int64_t)L * x->pool_bytes * R + x->attn_full_bytes;
   const int64_t kv_total = 2 * (int64_t)L * x->pool_bytes * R;
+  // what dual residency costs beyond the single resident copy: the spare weight slot(s) and, with
+  // MOEBIUS_ATTN_DUAL, the duplicated head shards (1.1 GB + 1.7 GB = 2.4 % per GPU)
+  const int64_t overhead = x->spare_bytes + x->attn_dup_bytes;
   if (c->staging_cap_bytes == 0) {
-    x->staging_bytes = kv_total / 50;   // no bound given: 2% of the KV capacity
+    // no bound given: 2% of the KV capacity, and never less than 64 EP pages of every pool (a tiny
+    // pool would otherwise get a staging buffer smaller than one page)
+    x->staging_bytes = std::max(kv_total / 50, std::min(kv_total, 64 * x->ep_page_bytes * 2 * (int64_t)L));
   } else {
-    if (c->staging_cap_bytes < x->spare_bytes) { delete x; return MOEBIUS_E_STAGING; }
-    x->staging_bytes = std::min(c->staging_cap_bytes - x->spare_bytes, kv_total);
+    if (c->staging_cap_bytes < overhead) { delete x; return MOEBIUS_E_STAGING; }
+    x->staging_bytes = std::min(c->staging_cap_bytes - overhead, kv_total);
   }
   x->staging_bytes = x->staging_bytes / x->ep_page_bytes * x->ep_page_bytes;
 
@@ -145,8 +178,9 @@ int moebius_create(const moebius_config_t* c, moebius_ctx_t** out) {
   live_max = std::min<int64_t>(live_max, (int64_t)c->max_requests * c->max_pages_per_request);
   x->max_kv_desc = live_max;
   x->max_c2d = c->w_dtype == MOEBIUS_FP8_E4M3_B128 ? (int64_t)x->n_obj * L * R * R : 0;
+  x->max_bulk = c->attn_mode == MOEBIUS_ATTN_GATHER ? (int64_t)L * R * (2 * (int64_t)R + 2 * (int64_t)std::max(R, Hkv)) : 0;
   x->desc_bytes = align_up(kSegOff + (int64_t)(1 + kMaxCounters) * sizeof(PlanHdr) + 2 * (int64_t)kMaxSegs * sizeof(Seg) + x->max_kv_desc * sizeof(KvDesc) +
-                               x->max_c2d * sizeof(C2dDesc) + 1024, 4096);
+                               x->max_c2d * sizeof(C2dDesc) + x->max_bulk * sizeof(BulkDesc) + 1024, 4096);
   x->table_bytes = align_up(4 * ((int64_t)kTblHdrInts + 2 * (int64_t)c->max_requests +
                                  (int64_t)c->max_requests * c->max_pages_per_request), 256);
   x->bound = false;
@@ -213,6 +247,8 @@ int moebius_layout(const moebius_ctx_t* x, moebius_layout_t* o) {
   o->tbl_lens_off = kTblHdrInts + x->cfg.max_requests;
   o->tbl_bt_off = kTblHdrInts + 2 * x->cfg.max_requests;
   o->tbl_reserved = 0;
+  o->attn_full_bytes = x->attn_full_bytes;
+  o->attn_dup_bytes = x->attn_dup_bytes;
   return MOEBIUS_OK;
 }
 
@@ -248,6 +284,29 @@ int moebius_view(const moebius_ctx_t* x, moebius_mode_t mode, int rank, int laye
     o->shape[1] = c.page_tokens;
     o->shape[2] = tp ? x->hpr : c.kv_heads;
     o->shape[3] = c.head_dim;
+  } else if (t >= MOEBIUS_T_WQ && t <= MOEBIUS_T_WO) {
+    // PAPER.md:112.  EP: the full projection on every rank.  TP: the rank's head shard -- a dense tensor
+    // of its own (MOEBIUS_ATTN_DUAL) or in place inside the full one (MOEBIUS_ATTN_GATHER).
+    if (c.attn_mode == MOEBIUS_ATTN_NONE) return MOEBIUS_E_INVAL;
+    const int a = t - MOEBIUS_T_WQ, Hq = c.n_q_heads, D = c.head_dim;
+    const bool kv = a == 1 || a == 2;
+    const int64_t n_full = kv ? c.kv_heads : Hq, n_sh = kv ? x->hpr : Hq / R;
+    const int64_t first = kv ? (c.kv_heads >= R ? (int64_t)rank * x->hpr : rank / x->rep) : (int64_t)rank * (Hq / R);
+    const int64_t lbase = rbase + x->attn_off + (int64_t)layer * x->attn_layer_bytes;
+    o->elem_bytes = 2;
+    o->ndim = 3;
+    const int64_t heads = tp ? n_sh : n_full;
+    if (a != 3) { o->shape[0] = heads; o->shape[1] = D; o->shape[2] = H; }
+    else        { o->shape[0] = H; o->shape[1] = heads; o->shape[2] = D; }
+    if (!tp) o->offset = lbase + x->attn_full_off[a];
+    else if (c.attn_mode == MOEBIUS_ATTN_DUAL) o->offset = lbase + x->attn_shard_off[a];
+    else {   // in place: heads [first, first + n_sh) of the full tensor
+      o->offset = lbase + x->attn_full_off[a] + first * (a != 3 ? (int64_t)D * H * 2 : (int64_t)D * 2);
+      if (a == 3) {
+        o->stride[0] = (int64_t)Hq * D; o->stride[1] = D; o->stride[2] = 1; o->stride[3] = 0;
+        return MOEBIUS_OK;
+      }
+    }
   } else if (so >= 0) {
     if (c.w_dtype != MOEBIUS_FP8_E4M3_B128) return MOEBIUS_E_INVAL;
     const WObj& ob = x->obj[so];
@@ -394,7 +453,7 @@ struct PlanBuilder {
   moebius_plan_t* P = nullptr;
   uint32_t next_ctr = 0;
   uint64_t ub = 0;                       // units of the merged list
-  Chain cw, ck, cs;                      // weight chain, KV rounds, scale copies
+  Chain cw, ck, cs, ca;                  // weight chain, KV rounds, scale copies, attention gathers
 
   PlanBuilder(moebius_ctx* x_, moebius_mode_t from_, moebius_mode_t to_, int32_t n, const int32_t* lens,
               const int32_t* so, const int32_t* sbt)
@@ -786,6 +845,59 @@ struct PlanBuilder {
     return MOEBIUS_OK;
   }
 
+  // attention projections
+  int attention_copies() {
+    // MOEBIUS_ATTN_DUAL: both layouts are resident, the switch is a pointer swap -- nothing to do.
+    // MOEBIUS_ATTN_GATHER: a rank's head shard sits in place inside its full-size tensor, so EP->TP
+    // keeps the local slice (nothing moves) and TP->EP rebuilds the full projections from the other
+    // ranks' shards: the paper's All-Gather, here one pulled copy per (layer, tensor, receiver, head
+    // block).  Sources (a rank's own shard) are never written by this switch: no hazard, no ordering.
+    if (c.attn_mode != MOEBIUS_ATTN_GATHER || e2t || R == 1) return MOEBIUS_OK;
+    const int Hq = c.n_q_heads, D = c.head_dim, Hkv = c.kv_heads;
+    const int64_t head = (int64_t)D * c.H * 2, stage = x->stage_bytes;
+    for (int a = 0; a < 4; ++a) {
+      const bool kv = a == 1 || a == 2;
+      Seg s = blank_seg();
+      s.kind = SEG_BULK | ((x->use_tma ? PATH_TMA : PATH_LSU) << 8);
+      s.ep_is_src = 0;
+      s.desc_begin = (uint32_t)P->bulk.size();
+      int64_t run, rows, stride;
+      if (a == 3) { rows = c.H; run = (int64_t)(Hq / R) * D * 2; stride = (int64_t)Hq * D * 2; }   // wo: column block per row
+      else        { rows = 1; run = (kv ? (int64_t)x->hpr : (int64_t)(Hq / R)) * head; stride = run; }
+      s.rows_total = (uint32_t)rows;
+      s.run_bytes = (uint32_t)std::min<int64_t>(run, UINT32_MAX);
+      s.chunk_bytes = pick_chunk(run, x->use_tma ? stage : unit_bytes);
+      s.chunks_per_run = (uint32_t)(run / s.chunk_bytes);
+      s.rows_per_unit = s.chunks_per_run == 1 ? (uint32_t)std::max<int64_t>(1, std::min<int64_t>(rows, (x->use_tma ? stage : unit_bytes) / run)) : 1;
+      s.row_blocks = (uint32_t)((rows + s.rows_per_unit - 1) / s.rows_per_unit);
+      s.ep_off = stride; s.tp_off = stride;     // BULK: source / destination row strides
+      for (int l = 0; l < L; ++l) {
+        const int64_t lbase = x->attn_off + (int64_t)l * x->attn_layer_bytes + x->attn_full_off[a];
+        for (int q = 0; q < R; ++q) {
+          // blocks of the head axis, one per TP holder: block b is read from its lowest-rank holder
+          const int n_blocks = kv ? (Hkv >= R ? R : Hkv) : R;
+          for (int b = 0; b < n_blocks; ++b) {
+            const int src = kv && Hkv < R ? b * x->rep : b;            // lowest holder (the rule of reading A5)
+            const bool held = kv && Hkv < R ? (q / x->rep == b) : (q == b);
+            if (held) continue;                                         // already in place on rank q
+            const int64_t within = a == 3 ? (int64_t)b * run : (int64_t)b * run;
+            BulkDesc d;
+            d.src_off = (int64_t)src * x->rank_stride + lbase + within;
+            d.dst_off = (int64_t)q * x->rank_stride + lbase + within;
+            P->bulk.push_back(d);
+            P->stats.attn_moved += rows * run; P->stats.attn_relocated += rows * run; P->stats.attn_read += rows * run;
+          }
+        }
+      }
+      s.n_desc = (uint32_t)P->bulk.size() - s.desc_begin;
+      const int64_t nu = (int64_t)s.n_desc * s.row_blocks * s.chunks_per_run;
+      if (nu > (1ll << 30)) return fail(MOEBIUS_E_INVAL);
+      s.n_units = (uint32_t)nu;
+      push_seg(ca, s);
+    }
+    return MOEBIUS_OK;
+  }
+
   // KV rounds as segments + byte accounting
   int kv_segments() {
     // KV: descriptors ordered [level 0][level 1]...[level K][staged]
@@ -889,20 +1001,20 @@ struct PlanBuilder {
         acc += ch.segs[i].n_units;
       }
     };
-    add_chain(cs, 0); add_chain(cw, 1); add_chain(ck, 2);
+    add_chain(cs, 0); add_chain(cw, 1); add_chain(ck, 2); add_chain(ca, 3);
     std::stable_sort(items.begin(), items.end(), [](const Item& a, const Item& b) {
       if (a.chain == 0 || b.chain == 0) return a.chain == 0 && b.chain != 0;
       return a.pos < b.pos;
     });
     ub = 0;
     for (auto& it : items) {
-      Seg s = (it.chain == 0 ? cs : it.chain == 1 ? cw : ck).segs[it.idx];
+      Seg s = (it.chain == 0 ? cs : it.chain == 1 ? cw : it.chain == 2 ? ck : ca).segs[it.idx];
       s.unit_begin = (uint32_t)ub;
       ub += s.n_units;
       P->segs.push_back(s);
     }
     if (ub >= (1ull << 32) || P->segs.size() > (size_t)kMaxSegs || (int64_t)nm > x->max_kv_desc ||
-        P->c2d.size() > (size_t)x->max_c2d)
+        P->c2d.size() > (size_t)x->max_c2d || P->bulk.size() > (size_t)x->max_bulk)
       return fail(MOEBIUS_E_INVAL);
     P->total_units = (uint32_t)ub;
     P->n_counters = next_ctr;
@@ -941,9 +1053,11 @@ struct PlanBuilder {
     int64_t kv_b = align_up((int64_t)nm * sizeof(KvDesc), 256);
     int64_t c2d_b = align_up((int64_t)P->c2d.size() * sizeof(C2dDesc), 256);
     const int64_t hdr_b = sizeof(PlanHdr);
+    int64_t bulk_b = align_up((int64_t)P->bulk.size() * sizeof(BulkDesc), 256);
     P->kv_img_off = hdr_b + seg_b;
     P->c2d_img_off = hdr_b + seg_b + kv_b;
-    P->wave_img_off = hdr_b + seg_b + kv_b + c2d_b;
+    P->bulk_img_off = hdr_b + seg_b + kv_b + c2d_b;
+    P->wave_img_off = hdr_b + seg_b + kv_b + c2d_b + bulk_b;
     const int64_t wave_b = (int64_t)P->n_waves * hdr_b + (int64_t)P->segs.size() * (int64_t)sizeof(Seg);
     P->image_bytes = P->wave_img_off + wave_b;
     if (kSegOff + P->image_bytes > x->desc_bytes) return fail(MOEBIUS_E_INVAL);
@@ -957,6 +1071,7 @@ struct PlanBuilder {
       h->total_units = P->total_units;
       h->kv_off = (uint32_t)P->kv_img_off;
       h->c2d_off = (uint32_t)P->c2d_img_off;
+      h->bulk_off = (uint32_t)P->bulk_img_off;
     }
     if (!P->segs.empty()) {
       memcpy(P->image + hdr_b, P->segs.data(), P->segs.size() * sizeof(Seg));
@@ -983,6 +1098,10 @@ struct PlanBuilder {
       memcpy(P->image + P->c2d_img_off, P->c2d.data(), P->c2d.size() * sizeof(C2dDesc));
       memset(P->image + P->c2d_img_off + P->c2d.size() * sizeof(C2dDesc), 0, (size_t)(c2d_b - (int64_t)(P->c2d.size() * sizeof(C2dDesc))));
     }
+    if (bulk_b) {
+      memcpy(P->image + P->bulk_img_off, P->bulk.data(), P->bulk.size() * sizeof(BulkDesc));
+      memset(P->image + P->bulk_img_off + P->bulk.size() * sizeof(BulkDesc), 0, (size_t)(bulk_b - (int64_t)(P->bulk.size() * sizeof(BulkDesc))));
+    }
     {  // per wave: a header + that wave's segments with their own unit numbering and no dependencies;
        // descriptor offsets are relative to the wave's header (negative: the arrays sit before it)
       P->wave_hdr_off.assign((size_t)P->n_waves, 0);
@@ -1008,6 +1127,7 @@ struct PlanBuilder {
         h->total_units = units;
         h->kv_off = (uint32_t)(int32_t)(P->kv_img_off - at);
         h->c2d_off = (uint32_t)(int32_t)(P->c2d_img_off - at);
+        h->bulk_off = (uint32_t)(int32_t)(P->bulk_img_off - at);
         P->wave_units[(size_t)w] = units;
         at += hdr_b + (int64_t)n * (int64_t)sizeof(Seg);
       }
@@ -1061,7 +1181,7 @@ extern "C" int moebius_plan(moebius_ctx_t* x, moebius_mode_t from, moebius_mode_
   int rc;
   if ((rc = b.request_state()) || (rc = b.kv_moves()) || (rc = b.kv_schedule())) return rc;   // nothing allocated yet
   if ((rc = b.new_plan())) return rc;
-  if ((rc = b.weight_chain()) || (rc = b.scale_copies()) || (rc = b.kv_segments()) || (rc = b.merge_and_waves()) ||
+  if ((rc = b.weight_chain()) || (rc = b.scale_copies()) || (rc = b.attention_copies()) || (rc = b.kv_segments()) || (rc = b.merge_and_waves()) ||
       (rc = b.build_images()) || (rc = b.finish_stats()))
     return rc;                                          // the failing stage has destroyed the plan
   *out = b.P;
@@ -1090,6 +1210,7 @@ extern "C" int moebius_plan_export(const moebius_plan_t* p, int what, void* buf,
     case 1: src = p->kv;          n = p->n_kv * (int64_t)sizeof(KvDesc); break;
     case 2: src = p->c2d.data();  n = (int64_t)p->c2d.size() * sizeof(C2dDesc); break;
     case 3: src = p->seg_wave.data(); n = (int64_t)p->seg_wave.size() * 4; break;
+    case 4: src = p->bulk.data(); n = (int64_t)p->bulk.size() * sizeof(BulkDesc); break;
     default: return MOEBIUS_E_INVAL;
   }
   *needed = n;
@@ -1108,6 +1229,7 @@ extern "C" int moebius_share_stats(const moebius_plan_t* P, int rank_lo, int ran
   memset(&p, 0, sizeof(p));
   p.kv = P->kv;
   p.c2d = P->c2d.data();
+  p.bulk = P->bulk.data();
   p.rank_stride = x->rank_stride;
   int64_t units = 0, rd = 0, wr = 0, cross = 0;
   for (size_t si = 0; si < P->segs.size(); ++si) {
@@ -1122,6 +1244,13 @@ extern "C" int moebius_share_stats(const moebius_plan_t* P, int rank_lo, int ran
         const int64_t b = (int64_t)d.rows * d.run_bytes;
         rd += b; wr += b;
         if (d.src_off / x->rank_stride != d.dst_off / x->rank_stride) cross += b;
+        continue;
+      }
+      if (seg_kind(s) == SEG_BULK) {
+        BulkUnit bu;
+        decode_bulk(s, p, u, bu);
+        const int64_t b = (int64_t)bu.nrows * bu.piece;
+        rd += b; wr += b; cross += b;     // always from another rank's shard
         continue;
       }
       if (seg_kind(s) == SEG_XPOSE) {

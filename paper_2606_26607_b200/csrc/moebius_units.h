@@ -15,6 +15,9 @@
 //         = one token's G head groups side by side; a TP page row = one group).
 //   LIN   contiguous copy (KV page <-> staging slot).
 //   C2D   small 2-D strided copy in 4-byte elements (fp8 block scales).
+//   BULK  large 2-D strided copy in 16-byte elements: n_desc descriptors of one shape (rows x run with a
+//         source and a destination row stride), split into units of whole rows or of run chunks
+//         (attention head shards gathered TP->EP).
 #ifndef MOEBIUS_UNITS_H_
 #define MOEBIUS_UNITS_H_
 
@@ -28,7 +31,7 @@
 
 namespace moebius {
 
-enum : uint32_t { SEG_XPOSE = 0, SEG_KV = 1, SEG_COPY2D = 2 };
+enum : uint32_t { SEG_XPOSE = 0, SEG_KV = 1, SEG_COPY2D = 2, SEG_BULK = 3 };
 enum : uint32_t { KV_MOVE = 0, KV_MOVE_STG = 1, KV_STG_COPY = 2 };
 // How the kernel executes a segment's units (bits 8..15 of Seg::kind).  The unit geometry is the
 // same for both paths (decode_box below is the single definition); only the data path differs:
@@ -58,8 +61,8 @@ struct Seg {              // 128 bytes, uploaded verbatim
   uint32_t chunks_per_run;
   uint32_t rows_total;       // XPOSE: rows per EP rank (E/R*H for gate/up, E/R for down)
   uint32_t row_blocks;       // XPOSE: ceil(rows_total / rows_per_unit)
-  int64_t  ep_off;           // XPOSE: EP view offset in the rank region; KV: pool 0 offset
-  int64_t  tp_off;           // XPOSE: TP view offset in the rank region; KV: == ep_off
+  int64_t  ep_off;           // XPOSE: EP view offset in the rank region; KV: pool 0 offset; BULK: source row stride
+  int64_t  tp_off;           // XPOSE: TP view offset in the rank region; KV: == ep_off;   BULK: destination row stride
   uint32_t kv_mode;
   uint32_t desc_begin;       // first descriptor (KV move or C2D) of this segment; XPOSE: EP slot index
   uint32_t n_desc;
@@ -89,6 +92,11 @@ struct C2dDesc {          // 32 bytes: rows x run_bytes, 4-byte elements, offset
 };
 static_assert(sizeof(C2dDesc) == 32, "C2dDesc must be 32 bytes");
 
+struct BulkDesc {         // 16 bytes: one strided copy of the segment's shape, offsets from dev_base
+  int64_t  src_off, dst_off;
+};
+static_assert(sizeof(BulkDesc) == 16, "BulkDesc must be 16 bytes");
+
 // First 256 bytes of the uploaded work-list image.  Everything that differs from plan to plan is
 // read by the kernel from here, so the kernel's ARGUMENTS are the same for every switch of a
 // context and the launch can sit in a captured CUDA graph (moebius_reshard_staged).
@@ -97,7 +105,8 @@ struct PlanHdr {
   uint32_t total_units;
   uint32_t kv_off;        // byte offsets from the start of the image
   uint32_t c2d_off;
-  uint32_t pad_[60];
+  uint32_t bulk_off;
+  uint32_t pad_[59];
 };
 static_assert(sizeof(PlanHdr) == 256, "PlanHdr must be 256 bytes");
 
@@ -108,6 +117,7 @@ struct DevParams {        // decoded launch state (the kernel fills the plan-dep
   const Seg*       segs;
   const KvDesc* kv;
   const C2dDesc*   c2d;
+  const BulkDesc*  bulk;
   uint32_t*        ticket;
   uint32_t*        counters;
   int64_t          rank_stride;
@@ -176,8 +186,35 @@ MB_HD uint32_t unit_ep_rank(const Seg& s, const DevParams& p, uint32_t u) {
     kv_unit(s, u, pb, di);
     return (uint32_t)p.kv[s.desc_begin + di].ep_rank;
   }
+  if (seg_kind(s) == SEG_BULK) {    // pulled by the rank that receives it
+    const uint32_t per_desc = s.row_blocks * s.chunks_per_run;
+    return (uint32_t)(p.bulk[s.desc_begin + u / per_desc].dst_off / p.rank_stride);
+  }
   const C2dDesc& d = p.c2d[s.desc_begin + u];
   return (uint32_t)((s.ep_is_src ? d.src_off : d.dst_off) / p.rank_stride);
+}
+
+// BULK unit u (local to the segment): descriptor u / (row_blocks*chunks_per_run); within it row block rb
+// and run chunk ch.  The unit copies `nrows` pieces of chunk_bytes; piece t is at src + t*src_stride.
+struct BulkUnit {
+  char *src, *dst;
+  int64_t src_stride, dst_stride;
+  uint32_t nrows, piece;     // piece = bytes per row handled by this unit
+};
+MB_HD void decode_bulk(const Seg& s, const DevParams& p, uint32_t u, BulkUnit& b) {
+  const uint32_t per_desc = s.row_blocks * s.chunks_per_run;
+  const uint32_t di = u / per_desc, w = u - di * per_desc;
+  const uint32_t rb = w / s.chunks_per_run, ch = w - rb * s.chunks_per_run;
+  const BulkDesc d = p.bulk[s.desc_begin + di];
+  const uint32_t row0 = rb * s.rows_per_unit;
+  uint32_t nrows = s.rows_total - row0;
+  if (nrows > s.rows_per_unit) nrows = s.rows_per_unit;
+  b.nrows = nrows;
+  b.piece = s.chunk_bytes;
+  b.src_stride = s.ep_off;
+  b.dst_stride = s.tp_off;
+  b.src = p.base + d.src_off + (int64_t)row0 * s.ep_off + (int64_t)ch * s.chunk_bytes;
+  b.dst = p.base + d.dst_off + (int64_t)row0 * s.tp_off + (int64_t)ch * s.chunk_bytes;
 }
 
 // Decode box k of unit u (u is LOCAL to the segment).

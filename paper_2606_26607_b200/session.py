@@ -15,7 +15,7 @@ _W_DT = {"bf16": B.MOEBIUS_BF16, "fp32": B.MOEBIUS_FP32, "fp8_e4m3_b128": B.MOEB
 
 def make_config(*, R, L, E, H, I, w_dtype="bf16", kv_heads, head_dim, page_tokens,
                 kv_pool_bytes_per_rank_layer, max_requests, max_pages_per_request,
-                staging_cap_bytes=0, kv_dtype="bf16", w_orient=0) -> B.moebius_config_t:
+                staging_cap_bytes=0, kv_dtype="bf16", w_orient=0, n_q_heads=0, attn_mode=0) -> B.moebius_config_t:
     c = B.moebius_config_t()
     c.R, c.L, c.E, c.H, c.I = R, L, E, H, I
     c.w_dtype = _W_DT[w_dtype]
@@ -25,6 +25,7 @@ def make_config(*, R, L, E, H, I, w_dtype="bf16", kv_heads, head_dim, page_token
     c.kv_pool_bytes_per_rank_layer = int(kv_pool_bytes_per_rank_layer)
     c.max_requests, c.max_pages_per_request = max_requests, max_pages_per_request
     c.staging_cap_bytes = int(staging_cap_bytes)
+    c.n_q_heads, c.attn_mode = n_q_heads, attn_mode
     return c
 
 
@@ -88,9 +89,11 @@ class Session:
         """torch tensor aliasing the fixed view (raw storage dtype: int16 / uint8 / float32)."""
         import torch
         v = self.view_desc(mode, rank, layer, tensor_id)
-        n = int(np.prod([v.shape[i] for i in range(v.ndim)])) * v.elem_bytes
+        shape = [v.shape[i] for i in range(v.ndim)]
+        stride = [v.stride[i] for i in range(v.ndim)]
         dt = {1: torch.uint8, 2: torch.int16, 4: torch.float32}[v.elem_bytes]
-        return self.base[v.offset:v.offset + n].view(dt).view(*[v.shape[i] for i in range(v.ndim)])
+        span = (sum((n - 1) * st for n, st in zip(shape, stride)) + 1) * v.elem_bytes   # a strided view spans more than its elements
+        return self.base[v.offset:v.offset + span].view(dt).as_strided(shape, stride)
 
     def guards(self):
         """The guard strips between / around the buffers (for canary checks)."""

@@ -55,7 +55,7 @@ struct Checker {
 
 extern "C" __attribute__((visibility("default")))
 int emul_run(char* base, int64_t base_bytes, char* stg, int64_t stg_bytes, const Seg* segs, int n_segs,
-             const KvDesc* kv, const C2dDesc* c2d, int64_t rank_stride, int64_t* out /*[8]*/) {
+             const KvDesc* kv, const C2dDesc* c2d, int64_t rank_stride, int64_t* out /*[8]*/, const BulkDesc* bulk) {
   Checker ck;
   ck.base = base; ck.base_bytes = base_bytes; ck.stg = stg; ck.stg_bytes = stg_bytes;
   ck.n = n_segs; ck.violations = ck.oob = ck.bytes_read = ck.bytes_written = 0;
@@ -79,7 +79,7 @@ int emul_run(char* base, int64_t base_bytes, char* stg, int64_t stg_bytes, const
   }
   DevParams p;
   memset(&p, 0, sizeof(p));
-  p.base = base; p.stg = stg; p.segs = segs; p.kv = kv; p.c2d = c2d;
+  p.base = base; p.stg = stg; p.segs = segs; p.kv = kv; p.c2d = c2d; p.bulk = bulk;
   p.rank_stride = rank_stride; p.n_segs = (uint32_t)n_segs;
   uint64_t expect_begin = 0;
   int64_t bad_begin = 0;
@@ -97,6 +97,19 @@ int emul_run(char* base, int64_t base_bytes, char* stg, int64_t stg_bytes, const
           if (d.src_off < 0 || d.dst_off < 0 || src + d.run_bytes > base + base_bytes || dst + d.run_bytes > base + base_bytes) { ++ck.oob; continue; }
           memmove(dst, src, d.run_bytes);
           ck.bytes_read += d.run_bytes; ck.bytes_written += d.run_bytes;
+        }
+        continue;
+      }
+      if (seg_kind(s) == SEG_BULK) {
+        BulkUnit bu;
+        decode_bulk(s, p, u, bu);
+        for (uint32_t t = 0; t < bu.nrows; ++t) {
+          const char* src = bu.src + (int64_t)t * bu.src_stride;
+          char* dst = bu.dst + (int64_t)t * bu.dst_stride;
+          ck.on_read(src, si, (int)bu.piece);
+          ck.on_write(dst, si, (int)bu.piece);
+          if (ck.chunk_of(src) >= 0 && ck.chunk_of(dst) >= 0 && ck.chunk_of(src + bu.piece - 16) >= 0 && ck.chunk_of(dst + bu.piece - 16) >= 0)
+            memmove(dst, src, bu.piece);
         }
         continue;
       }

@@ -28,7 +28,8 @@ def mb_config(cfg: wl.Config, seq_lens, pool_policy=None, staging_cap_frac=0.0, 
     c = mb.make_config(R=cfg.R, L=cfg.L, E=cfg.E, H=cfg.H, I=cfg.I, w_dtype=cfg.w_dtype,
                        kv_heads=cfg.kv_heads, head_dim=cfg.head_dim, page_tokens=cfg.page,
                        kv_pool_bytes_per_rank_layer=pool, max_requests=max_requests or max(n, 1),
-                       max_pages_per_request=mp, staging_cap_bytes=0, w_orient=cfg.w_orient)
+                       max_pages_per_request=mp, staging_cap_bytes=0, w_orient=cfg.w_orient,
+                       n_q_heads=cfg.n_q_heads, attn_mode=cfg.attn_mode)
     if staging_cap_frac:
         s = mb.Session(c)
         c.staging_cap_bytes = int(staging_cap_frac * s.layout.resident_bytes)
@@ -42,7 +43,8 @@ State = oracle.State
 def view_fn_of(sess: mb.Session):
     def fn(mode, rank, layer, tensor_id):
         v = sess.view_desc(mode, rank, layer, tensor_id)
-        return v.offset, tuple(v.shape[i] for i in range(v.ndim)), v.elem_bytes
+        return (v.offset, tuple(v.shape[i] for i in range(v.ndim)), v.elem_bytes,
+                tuple(v.stride[i] for i in range(v.ndim)))
     return fn
 
 
@@ -83,6 +85,16 @@ def expected_bytes(st: State, from_mode: int, ep_owner):
     return w, k
 
 
+def expected_attn_bytes(st: State, from_mode: int):
+    """(moved, relocated, read) of the attention projections (oracle/attention.py)."""
+    c = st.cfg
+    if not c.attn_mode:
+        return (0, 0, 0)
+    a = oracle.attn_bytes(c.R, c.L, c.n_q_heads, c.kv_heads, c.head_dim, c.H, 2,
+                          "ep2tp" if from_mode == EP else "tp2ep", "dual" if c.attn_mode == 1 else "gather")
+    return (a["moved"], a["relocated"], a["read"])
+
+
 # ---- host emulator (CPU tests only) ---------------------------------------------------------------
 
 _EMUL = None
@@ -98,7 +110,7 @@ def emul_lib():
             subprocess.check_call(["g++", "-O2", "-std=c++17", "-shared", "-fPIC", "-o", so, src])
         _EMUL = C.CDLL(so)
         _EMUL.emul_run.argtypes = [C.c_void_p, C.c_int64, C.c_void_p, C.c_int64, C.c_void_p, C.c_int,
-                                   C.c_void_p, C.c_void_p, C.c_int64, C.c_void_p]
+                                   C.c_void_p, C.c_void_p, C.c_int64, C.c_void_p, C.c_void_p]
     return _EMUL
 
 
@@ -108,9 +120,10 @@ def emulate(sess: mb.Session, plan, image: np.ndarray, staging: np.ndarray):
     segs = mb.moebius_plan_export(plan, 0)
     kv = mb.moebius_plan_export(plan, 1)
     c2d = mb.moebius_plan_export(plan, 2)
+    bulk = mb.moebius_plan_export(plan, 4)
     out = np.zeros(8, np.int64)
     vp = lambda a: a.ctypes.data_as(C.c_void_p) if a.size else None  # noqa: E731
     emul_lib().emul_run(vp(image), image.size, vp(staging), staging.size, vp(segs), len(segs), vp(kv), vp(c2d),
-                        sess.layout.rank_stride_bytes, vp(out))
+                        sess.layout.rank_stride_bytes, vp(out), vp(bulk))
     return {"violations": int(out[0]), "oob": int(out[1]), "bad_wait": int(out[2]), "bad_begin": int(out[3]),
             "bytes_read": int(out[4]), "bytes_written": int(out[5]), "units": int(out[6])}

@@ -10,7 +10,7 @@ import numpy as np
 import pytest
 
 import workloads as wl
-from harness import (EP, TP, OracleLayout, State, expected_bytes, expected_target, mb, mb_config,
+from harness import (EP, TP, OracleLayout, State, expected_attn_bytes, expected_bytes, expected_target, mb, mb_config,
                      source_tables)
 
 torch = pytest.importorskip("torch")
@@ -91,6 +91,7 @@ def gpu_switch(st, sess, from_mode, src_owner, src_bt, execute=None):
     w, k = expected_bytes(st, from_mode, ep_owner)
     assert (stats["w_moved"], stats["w_relocated"], stats["w_read"]) == (w["moved"], w["relocated"], w["read"])
     assert (stats["kv_moved"], stats["kv_relocated"], stats["kv_read"]) == (k["moved"], k["relocated"], k["read"])
+    assert (stats["attn_moved"], stats["attn_relocated"], stats["attn_read"]) == expected_attn_bytes(st, from_mode)
     sess.free_plan(plan)
     return to_mode, (want_owner if to_mode == EP else None), want_bt, stats
 
@@ -465,3 +466,34 @@ def test_reshard_checks_come_before_the_first_enqueue():
     sess.free_plan(plan)
     gpu_switch(st, sess, TP, owner, bt)
     sess.close()
+
+
+@pytest.mark.parametrize("attn_mode", [mb.ATTN_DUAL, mb.ATTN_GATHER])
+@pytest.mark.parametrize("R,Hq,Hkv,D,H", [(8, 16, 4, 64, 256), (4, 8, 8, 32, 128), (2, 4, 1, 16, 64), (3, 6, 3, 8, 40)])
+def test_attention_projections(attn_mode, R, Hq, Hkv, D, H):
+    """SURVEY.md section 8(f) NEXT-4.  MOEBIUS_ATTN_DUAL: both layouts resident, a switch
+    moves nothing and both sets of views stay bit-exact with the oracle.  MOEBIUS_ATTN_GATHER: the head
+    shard sits in place inside the full tensor (wo as a strided view); TP->EP gathers the other ranks'
+    shards on the device (bulk 2-D copies in the fused launch), EP->TP keeps the local slice."""
+    cfg = wl.get_config("tiny").with_(R=R, E=2 * R, H=H, I=32 * R, kv_heads=Hkv, head_dim=D, n_q_heads=Hq,
+                                       attn_mode=attn_mode, L=3, n_req=9, len_dist=("uniform", 1, 80), seed=60 + R)
+    st, sess = gpu_session(cfg)
+    owner, bt, _ = start(st, sess, TP, "random")
+    mode = TP
+    for _ in range(3):
+        mode, owner, bt, stats = gpu_switch(st, sess, mode, owner, bt)
+    if attn_mode == mb.ATTN_GATHER:
+        # the strided TP view of wo, read through torch, equals the oracle's dense head shard
+        sess2_mode = mode
+        for r in range(R):
+            got = sess.view(TP, r, 1, mb.T_WO).cpu().numpy().view(np.uint16)
+            want = oracle_attn_tp(st, 1, "wo", r)
+            if sess2_mode == TP:
+                assert np.array_equal(got, want)
+    sess.close()
+
+
+def oracle_attn_tp(st, layer, kind, r):
+    import oracle
+    c = st.cfg
+    return oracle.attn_tp_view(st.attn(layer, kind), kind, r, c.R, c.n_q_heads, c.kv_heads)

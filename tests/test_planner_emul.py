@@ -5,9 +5,10 @@ the oracle bytewise.  (Device execution itself is covered by the -m gpu tests.)"
 import numpy as np
 import pytest
 
+import oracle
 import workloads as wl
-from harness import (EP, TP, OracleLayout, State, emulate, expected_bytes, expected_target, mb, mb_config,
-                     source_tables)
+from harness import (EP, TP, OracleLayout, State, emulate, expected_attn_bytes, expected_bytes, expected_target, mb,
+                     mb_config, source_tables)
 
 
 def run_switch(st, sess, image, staging, from_mode, src_owner, src_bt):
@@ -29,13 +30,14 @@ def run_switch(st, sess, image, staging, from_mode, src_owner, src_bt):
     w, k = expected_bytes(st, from_mode, ep_owner)
     assert (stats["w_moved"], stats["w_relocated"], stats["w_read"]) == (w["moved"], w["relocated"], w["read"])
     assert (stats["kv_moved"], stats["kv_relocated"], stats["kv_read"]) == (k["moved"], k["relocated"], k["read"])
-    direct_bytes = stats["w_relocated"] + stats["kv_relocated"]
+    assert (stats["attn_moved"], stats["attn_relocated"], stats["attn_read"]) == expected_attn_bytes(st, from_mode)
+    direct_bytes = stats["w_relocated"] + stats["kv_relocated"] + stats["attn_relocated"]
     staged_extra = res["bytes_written"] - direct_bytes
     assert staged_extra >= 0
     if stats["n_kv_staged"] == 0:
         # EP->TP reads a straddled scale block once per holder: `read` counts unique source bytes (A15)
         rereads = stats["w_relocated"] - stats["w_read"]
-        assert res["bytes_written"] == direct_bytes and res["bytes_read"] == stats["w_read"] + stats["kv_read"] + rereads
+        assert res["bytes_written"] == direct_bytes and res["bytes_read"] == stats["w_read"] + stats["kv_read"] + stats["attn_read"] + rereads
     tgt = OracleLayout(st, sess, to_mode, want_owner, want_bt)
     bad = tgt.compare(image)
     assert not bad, bad[:5]
@@ -349,10 +351,11 @@ def test_waves_with_barriers_are_hazard_free(first, policy, orient):
             assert all(waves[j] < waves[i] for j in range(len(orig)) if orig[j]["signal_ctr"] == s["wait_ctr"])
     kv = mb.moebius_plan_export(plan, 1)
     c2d = mb.moebius_plan_export(plan, 2)
+    bulk = mb.moebius_plan_export(plan, 4)
     out = np.zeros(8, np.int64)
     vp = lambda a: a.ctypes.data_as(C.c_void_p) if a.size else None  # noqa: E731
     emul_lib().emul_run(vp(image), image.size, vp(staging), staging.size, vp(segs), len(segs), vp(kv), vp(c2d),
-                        sess.layout.rank_stride_bytes, vp(out))
+                        sess.layout.rank_stride_bytes, vp(out), vp(bulk))
     assert out[0] == 0 and out[1] == 0 and out[2] == 0 and out[3] == 0, out
     want_owner, want_bt = expected_target(st, sess, to)
     assert not OracleLayout(st, sess, to, want_owner, want_bt).compare(image)
@@ -386,3 +389,27 @@ def test_share_stats_partition_the_plan(first, R, Hkv):
     # weights are balanced across ranks by construction; every rank has work in every weight wave
     assert all(mb.moebius_share_stats(plan, r, r + 1, 0)["units"] > 0 for r in range(R))
     sess.free_plan(plan)
+
+
+@pytest.mark.parametrize("attn_mode", [1, 2])
+@pytest.mark.parametrize("R,Hq,Hkv", [(2, 4, 2), (4, 8, 2), (4, 8, 8), (8, 16, 4), (1, 4, 2), (3, 6, 3)])
+def test_attention_projections_follow_the_switch(attn_mode, R, Hq, Hkv):
+    """default variant (both layouts resident: the switch moves nothing, both sets of
+    views hold the oracle's layouts at all times) and the memory-saving variant (TP shard in place
+    inside the full tensor; TP->EP gathers the other ranks' shards, EP->TP keeps the local slice)."""
+    cfg = wl.get_config("tiny").with_(R=R, E=R * 2, I=16 * R, kv_heads=Hkv, n_q_heads=Hq, attn_mode=attn_mode, L=2,
+                                       n_req=5, len_dist=("uniform", 1, 40), seed=40 + R)
+    st, sess, image, staging = make(cfg)
+    lay = sess.layout
+    a = oracle.attn_bytes(R, cfg.L, Hq, Hkv, cfg.head_dim, cfg.H, 2, "tp2ep", "dual" if attn_mode == 1 else "gather")
+    assert lay.attn_full_bytes == a["full_per_rank"] * R
+    assert lay.attn_dup_bytes == a["duplicated_per_rank"] * R
+    owner, bt = source_tables(st, sess, TP, "random")
+    src = OracleLayout(st, sess, TP, owner, bt)
+    src.place(image)
+    mode = TP
+    for _ in range(3):
+        mode, owner, bt, stats = run_switch(st, sess, image, staging, mode, owner, bt)
+        if attn_mode == 1:   # pointer swap: compare() has checked BOTH modes' views; nothing moved
+            assert stats["attn_moved"] == 0
+    sess.close()

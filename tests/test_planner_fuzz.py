@@ -7,7 +7,8 @@ import numpy as np
 import pytest
 
 import workloads as wl
-from harness import EP, TP, OracleLayout, State, emulate, expected_bytes, expected_target, mb, mb_config, source_tables
+from harness import (EP, TP, OracleLayout, State, emulate, expected_attn_bytes, expected_bytes, expected_target, mb, mb_config,
+                     source_tables)
 
 
 def draw_case(seed):
@@ -30,6 +31,11 @@ def draw_case(seed):
         kv_heads=Hkv, head_dim=8 * int(rng.integers(1, 5)), page=int(rng.choice([4, 16])),
         n_req=int(rng.integers(0, 14)), len_dist=("uniform", 1, int(rng.integers(2, 120))), seed=500 + seed,
         w_orient=int(rng.integers(0, 2)))
+    # attention projections: none / both layouts resident / memory-saving All-Gather
+    mult = [m for m in (1, 2, 4, 8) if (Hkv * m) % R == 0]
+    attn_mode = int(rng.choice([0, 1, 2])) if mult else 0
+    if attn_mode:
+        cfg = cfg.with_(attn_mode=attn_mode, n_q_heads=Hkv * int(rng.choice(mult)))
     policy = str(rng.choice(["roomy", "tight"]))
     first = int(rng.choice([TP, EP]))
     src = str(rng.choice(["canonical", "random"]))
@@ -69,12 +75,12 @@ def test_fuzz_round_trip(seed):
         assert np.array_equal(new_bt, want_bt)
         assert np.array_equal(new_owner, want_owner if to == EP else np.full(len(st.lens), -1, np.int32))
         w, k = expected_bytes(st, mode, owner if mode == EP else new_owner)
-        if cfg.w_dtype != "fp8_e4m3_b128":
-            assert (stats["w_moved"], stats["w_relocated"]) == (w["moved"], w["relocated"])
+        assert (stats["w_moved"], stats["w_relocated"], stats["w_read"]) == (w["moved"], w["relocated"], w["read"])
         assert (stats["kv_moved"], stats["kv_relocated"], stats["kv_read"]) == (k["moved"], k["relocated"], k["read"])
+        assert (stats["attn_moved"], stats["attn_relocated"], stats["attn_read"]) == expected_attn_bytes(st, mode)
         shares = [mb.moebius_share_stats(plan, r, r + 1) for r in range(cfg.R)]
         assert sum(s["units"] for s in shares) == stats["n_units"]
-        assert sum(s["cross"] for s in shares) == stats["w_moved"] + stats["kv_moved"]
+        assert sum(s["cross"] for s in shares) == stats["w_moved"] + stats["kv_moved"] + stats["attn_moved"]
         bad = OracleLayout(st, sess, to, want_owner, want_bt).compare(image)
         assert not bad, (seed, bad[:3])
         sess.free_plan(plan)

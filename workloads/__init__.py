@@ -20,4 +20,7 @@ from .gen import (  # noqa: F401
     weight_tag_salt,
     weight_shape,
     kv_tag_salt,
+    attn_weight_shape,
+    attn_tag_salt,
+    gen_attn_weight,
 )

@@ -108,6 +108,28 @@ def gen_logical_scale(cfg: Config, layer: int, kind: str) -> np.ndarray:
     return rng.uniform(0.5, 2.0, size=shape).astype(np.float32)
 
 
+_ATTN_ID = {"wq": 0, "wk": 1, "wv": 2, "wo": 3}
+
+
+def attn_weight_shape(cfg: Config, kind: str) -> tuple:
+    """Logical attention projections of one layer: wq [Hq,D,H], wk/wv [Hkv,D,H], wo [H,Hq,D]."""
+    Hq, Hkv, D, H = cfg.n_q_heads, cfg.kv_heads, cfg.head_dim, cfg.H
+    return {"wq": (Hq, D, H), "wk": (Hkv, D, H), "wv": (Hkv, D, H), "wo": (H, Hq, D)}[kind]
+
+
+def attn_tag_salt(cfg: Config, layer: int, kind: str) -> int:
+    return cfg.seed * 1000 + 700 + layer * 4 + _ATTN_ID[kind]
+
+
+def gen_attn_weight(cfg: Config, layer: int, kind: str, fill: str = "tag") -> np.ndarray:
+    """bf16 bit patterns (uint16) of one attention projection: coordinate tags, or N(0, 0.02)."""
+    shape = attn_weight_shape(cfg, kind)
+    if fill == "tag":
+        return tag_fill_u16(shape, salt=attn_tag_salt(cfg, layer, kind))
+    rng = np.random.default_rng((cfg.seed, 2700 + layer, _ATTN_ID[kind]))
+    return bf16_bits_from_f32(rng.normal(0.0, 0.02, size=shape).astype(np.float32))
+
+
 def draw_seq_lens(cfg: Config, n_req: int | None = None) -> np.ndarray:
     """Request lengths in tokens (int32), numpy.random.default_rng(cfg.seed)."""
     n = cfg.n_req if n_req is None else n_req
