@@ -55,6 +55,7 @@ def parse():
     ap.add_argument("--w-orient", type=int, default=0, choices=[0, 1],
                     help="0: gate,up [E,H,I], down [E,I,H] (BASELINE.json, the headline); 1: the paper's W13 [E,2I,H], W2 [E,H,I] (named in config.workload)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-naive", action="store_true", help="skip timing the staged comparison path (PAPER.md Table 1)")
     ap.add_argument("--no-other-configs", action="store_true",
                     help="default run only: skip timing configs 3, 5, 2 and the tight-pool variant after config 4")
     ap.add_argument("--profile-region", action="store_true",
@@ -440,7 +441,7 @@ def run_moebius(args, env, config_name, pool_policy, cap_frac, steps, warmup, fu
     if world > 1:
         dist.barrier()
     dev_ms = e0.elapsed_time(e1)
-    if args.profile_region:
+    if args.profile_region and (not full or args.no_naive):
         torch.cuda.cudart().cudaProfilerStop()
     hist = mb.moebius_kernel_ms_history(sess.ctx, 64)[-2 * steps:]
     k_t2e, k_e2t = hist[0::2], hist[1::2]
@@ -500,6 +501,35 @@ def run_moebius(args, env, config_name, pool_policy, cap_frac, steps, warmup, fu
             sess.free_plan(plan)
     e2e_s = time.perf_counter() - t0
     clocks = sampler.summary()
+    # the staged comparison path of PAPER.md Table 1 (permute -> exchange -> scatter through a staging
+    # buffer), timed on the same resident state right after the fused kernel: context, not the metric
+    naive = None
+    if not args.no_naive:
+        try:
+            naive = {"tp2ep_ms": [], "ep2tp_ms": []}
+            scratch = None
+            for _ in range(2):
+                for to in (EP, TP):
+                    plan = sess.plan(to, lens, owner, bt_cur, from_mode=mode)
+                    need = mb.moebius_naive_scratch_bytes(sess.ctx, plan)
+                    if scratch is None or scratch.numel() < need + 256:
+                        scratch = None
+                        scratch = torch.empty(int(need * 1.05) + 4096, dtype=torch.uint8, device=dev)
+                    off = (-scratch.data_ptr()) % 256
+                    ns = mb.moebius_reshard_naive(sess.ctx, plan, scratch.data_ptr() + off, scratch.numel() - off, stream.cuda_stream)
+                    torch.cuda.synchronize()
+                    naive["tp2ep_ms" if to == EP else "ep2tp_ms"].append(mb.moebius_last_kernel_ms(sess.ctx))
+                    naive["tp2ep" if to == EP else "ep2tp"] = ns
+                    new_owner, bt_cur = sess.block_tables(plan, n)
+                    owner = new_owner if to == EP else None
+                    sess.free_plan(plan)
+                    mode = to
+            del scratch
+        except Exception as e:      # context only: never take the bench line down
+            naive = {"error": repr(e)[:300]}
+        if args.profile_region:
+            torch.cuda.synchronize()
+            torch.cuda.cudart().cudaProfilerStop()
     sess.close()
     # no tensor and no session leaves this function: the device buffers go back to torch before the next
     # workload is built
@@ -616,6 +646,21 @@ def main():
         "gpu_launches": 2 * steps * world,
         "clocks": r["clocks"],
     }
+    nv = r.get("naive")
+    if nv and "error" not in nv:
+        def nd(key, fused, ms_key):
+            ms = min(nv[ms_key])
+            b = nv[key]["bytes_read"] + nv[key]["bytes_written"]
+            return {"ms": ms, "launches": nv[key]["launches"], "hbm_bytes_by_construction": b,
+                    "passes_vs_direct": b / fused["algorithmic_traffic_bytes"], "GBps": b / ms / 1e6,
+                    "fused_speedup": ms / fused["kernel_ms_avg"]}
+        line["naive_3stage"] = {"what": "PAPER.md Table 1 'Naive' on one device: permute -> exchange (-> scatter) through a staging "
+                                        "buffer, plain ld/st kernels, same plan and bit-identical result; context, not the metric",
+                                "tp2ep": nd("tp2ep", d_t2e, "tp2ep_ms"), "ep2tp": nd("ep2tp", d_e2t, "ep2tp_ms"),
+                                "scratch_GB": nv["tp2ep"]["scratch_bytes"] / 1e9}
+        line["gpu_launches"] += 2 * (nv["tp2ep"]["launches"] + nv["ep2tp"]["launches"])
+    elif nv:
+        line["naive_3stage"] = nv
     pool_bytes = r["pool"]
     del r
     # the other BASELINE.json configs, driver-timed in the same run (1 GPU, default workload only)

@@ -253,6 +253,26 @@ MOEBIUS_API int moebius_reshard_share(moebius_ctx_t* ctx, const moebius_plan_t* 
 MOEBIUS_API int moebius_share_stats(const moebius_plan_t* plan, int rank_lo, int rank_hi, int wave, int64_t* out4);
 MOEBIUS_API int moebius_reshard_publish(moebius_ctx_t* ctx, const moebius_plan_t* plan, void* cuda_stream);
 
+/* ---- the staged comparison path (needs a CUDA device) --------------- */
+
+/* PAPER.md:162-170 and Table 1 (:176-189): the "Naive" implementation of a switch -- per object, gather
+ * the source bytes into per-peer chunks in a staging buffer (local permute), exchange the chunks
+ * (All-to-All), and for the paged KV cache scatter the received chunks into the target pages.  On one
+ * device the exchange is a device copy, so every element makes 2 (weights: permute, exchange) or 3 (KV:
+ * gather, exchange, scatter) read+write passes through HBM where moebius_reshard makes one.  Same plan,
+ * same result bit for bit (target views, published tables, active mode); it exists to MEASURE the pass
+ * counts of Table 1 and the fused kernel's gain on the same box, and is not part of the product path.
+ *   dev_scratch   DEVICE, 256-byte aligned, at least moebius_naive_scratch_bytes(ctx, plan) bytes,
+ *                 caller-owned (the paper's staging slots S / 2S: here one weight object over all ranks,
+ *                 or a pool's gathered + received KV), outside the unified buffer and its 2.4 % budget
+ *   stats6        HOST int64[6] or NULL: {kernel launches, bytes read, bytes written, bytes of the weight
+ *                 passes, bytes of the KV passes, scratch bytes needed}
+ * Synchronises the stream once before its launches (descriptor upload from pageable host memory).
+ * With moebius_set_timing the span of its launches is recorded like a moebius_reshard kernel. */
+MOEBIUS_API int moebius_naive_scratch_bytes(const moebius_ctx_t* ctx, const moebius_plan_t* plan, int64_t* out);
+MOEBIUS_API int moebius_reshard_naive(moebius_ctx_t* ctx, const moebius_plan_t* plan, void* dev_scratch,
+                                      int64_t scratch_bytes, void* cuda_stream, int64_t* stats6);
+
 /* Kernel-only device time of the last moebius_reshard, in ms (CUDA events on its stream; the call
  * synchronises on the end event).  Enabled with moebius_set_timing(ctx, 1). */
 MOEBIUS_API int moebius_set_timing(moebius_ctx_t* ctx, int enable);

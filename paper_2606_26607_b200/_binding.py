@@ -20,6 +20,7 @@ EXPORTED_SYMBOLS = [
     "moebius_create", "moebius_destroy", "moebius_layout", "moebius_view", "moebius_bind",
     "moebius_active_mode", "moebius_plan", "moebius_plan_destroy", "moebius_block_tables",
     "moebius_plan_stats", "moebius_plan_export", "moebius_reshard", "moebius_stage_plan", "moebius_reshard_staged",
+    "moebius_naive_scratch_bytes", "moebius_reshard_naive",
     "moebius_share_stats", "moebius_plan_waves", "moebius_reshard_share", "moebius_reshard_publish",
     "moebius_arena_create", "moebius_arena_destroy", "moebius_arena_base", "moebius_arena_ready",
     "moebius_arena_export", "moebius_arena_import",
@@ -257,6 +258,24 @@ def moebius_plan_export(plan, what: int) -> np.ndarray:
 
 def moebius_reshard(ctx, plan, cuda_stream: int = 0):
     _chk(_lib.moebius_reshard(ctx, plan, _vp(cuda_stream or None)), "moebius_reshard")
+
+
+_lib.moebius_naive_scratch_bytes.argtypes = [_vp, _vp, C.POINTER(C.c_int64)]
+_lib.moebius_reshard_naive.argtypes = [_vp, _vp, _vp, C.c_int64, _vp, C.POINTER(C.c_int64)]
+
+
+def moebius_naive_scratch_bytes(ctx, plan) -> int:
+    out = C.c_int64(0)
+    _chk(_lib.moebius_naive_scratch_bytes(ctx, plan, C.byref(out)), "moebius_naive_scratch_bytes")
+    return out.value
+
+
+def moebius_reshard_naive(ctx, plan, dev_scratch: int, scratch_bytes: int, cuda_stream: int = 0) -> dict:
+    """The staged comparison path (Table 1); returns its launch / byte counts."""
+    st = (C.c_int64 * 6)()
+    _chk(_lib.moebius_reshard_naive(ctx, plan, _vp(dev_scratch), scratch_bytes, _vp(cuda_stream or None), st),
+         "moebius_reshard_naive")
+    return dict(zip(("launches", "bytes_read", "bytes_written", "w_pass_bytes", "kv_pass_bytes", "scratch_bytes"), list(st)))
 
 
 def moebius_policy_preset(kind: int, T_h: float = 256.0, cooldown_s: float = 5.0) -> moebius_policy_config_t:

@@ -497,3 +497,65 @@ def oracle_attn_tp(st, layer, kind, r):
     import oracle
     c = st.cfg
     return oracle.attn_tp_view(st.attn(layer, kind), kind, r, c.R, c.n_q_heads, c.kv_heads)
+
+
+def naive_execute(sess, plan):
+    """The staged comparison path (Table 1) instead of the fused kernel, same plan."""
+    n = mb.moebius_naive_scratch_bytes(sess.ctx, plan)
+    scratch = torch.empty(n + 512, dtype=torch.uint8, device="cuda:0")
+    off = (-scratch.data_ptr()) % 256
+    scratch[:off].fill_(CANARY)
+    scratch[off + n:].fill_(CANARY)
+    st = mb.moebius_reshard_naive(sess.ctx, plan, scratch.data_ptr() + off, n, torch.cuda.current_stream().cuda_stream)
+    torch.cuda.synchronize()
+    assert bool((scratch[:off] == CANARY).all()) and bool((scratch[off + n:] == CANARY).all()), "naive path wrote outside its scratch"
+    ps = mb.moebius_plan_stats(plan).as_dict()
+    # Table 1 on one device: every weight byte makes 2 read+write passes, every KV byte 3
+    assert st["w_pass_bytes"] == 2 * (ps["w_relocated"] - scale_relocated(sess, plan))
+    assert st["kv_pass_bytes"] == 2 * ps["kv_read"] + (ps["kv_read"] + ps["kv_relocated"]) + 2 * ps["kv_relocated"]
+    return st
+
+
+def scale_relocated(sess, plan):
+    c2d = mb.moebius_plan_export(plan, 2)
+    return int((c2d["rows"].astype(np.int64) * c2d["run_bytes"]).sum())
+
+
+NAIVE_CASES = {
+    "tiny": wl.get_config("tiny"),
+    "smallish": SMALLISH,
+    "replicated_heads": wl.get_config("tiny").with_(R=8, E=8, I=64, kv_heads=4, n_req=7, len_dist=("uniform", 1, 70), seed=13),
+    "one_head": wl.get_config("tiny").with_(R=4, E=8, I=64, kv_heads=1, n_req=7, len_dist=("uniform", 1, 70), seed=9),
+    "fp8": wl.get_config("fp8_graph").with_(L=1, E=8, H=256, I=1536, n_req=6, len_dist=("uniform", 1, 60), seed=3),
+    "paper_orient": SMALLISH.with_(w_orient=1, seed=78),
+    "odd": wl.get_config("tiny").with_(R=3, E=6, H=40, I=72, kv_heads=3, head_dim=8, n_req=9, len_dist=("uniform", 1, 90), seed=21),
+    "attn_gather": wl.get_config("tiny").with_(R=4, E=8, H=128, I=128, kv_heads=2, head_dim=32, n_q_heads=8, attn_mode=2, L=2,
+                                               n_req=9, len_dist=("uniform", 1, 80), seed=64),
+}
+
+
+@pytest.mark.parametrize("name", sorted(NAIVE_CASES))
+@pytest.mark.parametrize("first", [TP, EP])
+def test_naive_three_stage_path_is_bit_exact(name, first):
+    """SURVEY.md section 8(f) NEXT-4 (ii), Table 1: permute -> exchange (-> scatter)
+    through a staging buffer gives the same target layout, tables and accounting as the fused kernel --
+    compared with the same oracle -- and a fused switch can follow a staged one on the same buffer."""
+    cfg = NAIVE_CASES[name]
+    st, sess = gpu_session(cfg, fill="normal" if cfg.w_dtype == "fp8_e4m3_b128" else "tag", initial_mode=first)
+    owner, bt, _ = start(st, sess, first, "random")
+    mode = first
+    for k in range(4):
+        mode, owner, bt, _ = gpu_switch(st, sess, mode, owner, bt, execute=naive_execute if k != 2 else None)
+    sess.close()
+
+
+def test_naive_path_with_tight_pools_needs_no_rounds():
+    """Gathering a pool's live pages into the staging buffer first reads every source page before any
+    target page is written: the staged path is hazard-free for any tables, at the price of its passes."""
+    cfg = SMALLISH.with_(L=1, n_req=40, seed=99)
+    st, sess = gpu_session(cfg, wl.draw_seq_lens(cfg), "tight", cap_frac=0.5)
+    owner, bt, _ = start(st, sess, TP, "random", seed=1)
+    mode = TP
+    for _ in range(3):
+        mode, owner, bt, stats = gpu_switch(st, sess, mode, owner, bt, execute=naive_execute)
+    sess.close()
