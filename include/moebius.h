@@ -31,6 +31,9 @@
  *   w_orient = 1 (the paper's own shapes): two objects per layer, W13 (2 slots) at slot 3*layer and
  *   W2 (1 slot) at slot 3*layer+2; every EP view starts 2 slots (the largest object) after its TP
  *   view, so the chain has 3L+2 slots.
+ *   When staging_cap_bytes does not allow that many spare slots, the shift shrinks (down to 0: the two
+ *   views alias the same bytes) and the objects that then overlap themselves take the in-place path
+ *   (moebius_config_t::w_inplace).
  */
 #ifndef MOEBIUS_H_
 #define MOEBIUS_H_
@@ -103,6 +106,13 @@ typedef struct {
                                  0.024 * resident (reading A12).  0 = no bound. */
   int32_t n_q_heads;          /* query heads Hq (attn_mode != 0): Hq % R == 0, Hq % kv_heads == 0   */
   int32_t attn_mode;          /* moebius_attn_mode_t; attention weights are bf16                    */
+  int32_t w_inplace;          /* 0: automatic -- the EP view of an object starts as many slots after its
+                                 TP view as the cap allows: the largest object's size (every move out of
+                                 place, S1) or fewer, down to none (S2: objects that overlap themselves
+                                 are moved block by block in dependency waves, blocks on permutation
+                                 cycles parked in the bounded staging buffer).
+                                 1: force shift 0 (both views alias the same bytes: fully in place)   */
+  int32_t reserved0;
 } moebius_config_t;
 
 /* Sizes the caller must allocate, and where things are.  All byte counts. */
@@ -125,6 +135,10 @@ typedef struct {
   int64_t attn_full_bytes;              /* full q/k/v/o copies, all ranks and layers (0 without attention) */
   int64_t attn_dup_bytes;               /* MOEBIUS_ATTN_DUAL: the head shards held beside them, all ranks
                                            (1.7 GB per GPU for Qwen3-235B)              */
+  int64_t w_staging_bytes;              /* the tail of the staging buffer that parks weight blocks (S2);
+                                           0 when every object moves out of place                     */
+  int32_t w_shift_slots;                /* slots between an object's TP view and its EP view          */
+  int32_t reserved1;
 } moebius_layout_t;
 
 /* One view; offset in bytes from dev_base; shape/stride in elements.  Every view is dense row-major
@@ -148,6 +162,8 @@ typedef struct {
   int64_t staging_used_bytes;            /* KV staging this plan uses                             */
   int64_t desc_upload_bytes, table_upload_bytes;
   int64_t attn_moved, attn_relocated, attn_read;   /* attention projections (MOEBIUS_ATTN_GATHER, TP->EP) */
+  int64_t w_staged_bytes;                /* S2: expert bytes parked in (and later taken from) the staging buffer */
+  int32_t n_w_waves, n_w_parked;         /* S2: dependency waves over all in-place objects, parked blocks  */
 } moebius_stats_t;
 
 /* ---- context (host only) ------------------------------------------------------------------ */
@@ -204,7 +220,7 @@ MOEBIUS_API int moebius_plan_stats(const moebius_plan_t* plan, moebius_stats_t* 
 /* Diagnostic dump of the work list for host-side hazard checking (tests).  what: 0 = segments
  * (moebius_segment_t-sized records), 1 = KV move descriptors (16 B each), 2 = 2-D
  * copy descriptors (32 B each), 3 = the dependency wave of every segment (int32 each), 4 = bulk copy
- * descriptors (16 B each).  buf: HOST, cap bytes; *needed receives the full size. */
+ * descriptors (16 B each), 5 = weight blocks of the in-place path (16 B each).  buf: HOST, cap bytes; *needed receives the full size. */
 MOEBIUS_API int moebius_plan_export(const moebius_plan_t* plan, int what, void* buf, int64_t cap,
                                     int64_t* needed);
 

@@ -42,7 +42,8 @@ class moebius_config_t(C.Structure):
                 ("kv_heads", C.c_int32), ("head_dim", C.c_int32), ("page_tokens", C.c_int32),
                 ("kv_dtype", C.c_int32), ("kv_pool_bytes_per_rank_layer", C.c_int64),
                 ("max_requests", C.c_int32), ("max_pages_per_request", C.c_int32),
-                ("staging_cap_bytes", C.c_int64), ("n_q_heads", C.c_int32), ("attn_mode", C.c_int32)]
+                ("staging_cap_bytes", C.c_int64), ("n_q_heads", C.c_int32), ("attn_mode", C.c_int32),
+                ("w_inplace", C.c_int32), ("reserved0", C.c_int32)]
 
 
 class moebius_policy_config_t(C.Structure):
@@ -61,7 +62,8 @@ class moebius_layout_t(C.Structure):
                 ("weight_spare_bytes", C.c_int64), ("staging_bytes", C.c_int64), ("desc_bytes", C.c_int64),
                 ("table_bytes", C.c_int64), ("resident_bytes", C.c_int64), ("tbl_owner_off", C.c_int32),
                 ("tbl_lens_off", C.c_int32), ("tbl_bt_off", C.c_int32), ("tbl_reserved", C.c_int32),
-                ("attn_full_bytes", C.c_int64), ("attn_dup_bytes", C.c_int64)]
+                ("attn_full_bytes", C.c_int64), ("attn_dup_bytes", C.c_int64), ("w_staging_bytes", C.c_int64),
+                ("w_shift_slots", C.c_int32), ("reserved1", C.c_int32)]
 
 
 class moebius_view_t(C.Structure):
@@ -76,7 +78,8 @@ class moebius_stats_t(C.Structure):
                 ("w_read", C.c_int64), ("kv_moved", C.c_int64), ("kv_relocated", C.c_int64),
                 ("kv_read", C.c_int64), ("staging_used_bytes", C.c_int64),
                 ("desc_upload_bytes", C.c_int64), ("table_upload_bytes", C.c_int64),
-                ("attn_moved", C.c_int64), ("attn_relocated", C.c_int64), ("attn_read", C.c_int64)]
+                ("attn_moved", C.c_int64), ("attn_relocated", C.c_int64), ("attn_read", C.c_int64),
+                ("w_staged_bytes", C.c_int64), ("n_w_waves", C.c_int32), ("n_w_parked", C.c_int32)]
 
     def as_dict(self):
         return {k: getattr(self, k) for k, _ in self._fields_ if k != "struct_size"}
@@ -95,6 +98,7 @@ KV_DTYPE = np.dtype([("ep_rank", "<i4"), ("ep_page", "<i4"), ("tp_page", "<i4"),
 C2D_DTYPE = np.dtype([("src_off", "<i8"), ("dst_off", "<i8"), ("rows", "<u4"), ("run_bytes", "<u4"),
                       ("src_stride", "<u4"), ("dst_stride", "<u4")])
 BULK_DTYPE = np.dtype([("src_off", "<i8"), ("dst_off", "<i8")])
+WBLK_DTYPE = np.dtype([("q", "<u4"), ("row0", "<u4"), ("nrows", "<u4"), ("slot", "<u4")])
 assert SEG_DTYPE.itemsize == 128 and KV_DTYPE.itemsize == 16 and C2D_DTYPE.itemsize == 32 and BULK_DTYPE.itemsize == 16
 
 
@@ -246,7 +250,7 @@ def moebius_plan_stats(plan) -> moebius_stats_t:
 
 
 def moebius_plan_export(plan, what: int) -> np.ndarray:
-    dt = (SEG_DTYPE, KV_DTYPE, C2D_DTYPE, np.dtype("<i4"), BULK_DTYPE)[what]
+    dt = (SEG_DTYPE, KV_DTYPE, C2D_DTYPE, np.dtype("<i4"), BULK_DTYPE, WBLK_DTYPE)[what]
     need = C.c_int64(0)
     _chk(_lib.moebius_plan_export(plan, what, None, 0, C.byref(need)), "moebius_plan_export")
     buf = np.zeros(need.value // dt.itemsize, dtype=dt)

@@ -222,7 +222,7 @@ __device__ __forceinline__ void tma_issue_load(const TmaCtx& c, const Seg& s, ui
     Box b;
     decode_box(s, p, ul, 0, b);
     if (s.groups_per_unit == s.n_groups) {          // XT
-      const uint32_t q = ul / s.row_blocks, row0 = (ul % s.row_blocks) * s.rows_per_unit;
+      const uint32_t q = b.q, row0 = b.row0;
       const uint32_t piece = p.xt_rows * s.run_bytes;
       if (s.ep_is_src) {
         if (lane == 0) {
@@ -296,7 +296,7 @@ __device__ __forceinline__ void tma_issue_store(const TmaCtx& c, const Seg& s, u
     Box b;
     decode_box(s, p, ul, 0, b);
     if (s.groups_per_unit == s.n_groups) {          // XT
-      const uint32_t q = ul / s.row_blocks, row0 = (ul % s.row_blocks) * s.rows_per_unit;
+      const uint32_t q = b.q, row0 = b.row0;
       const uint32_t piece = p.xt_rows * s.run_bytes;
       if (s.ep_is_src) {
         const uint32_t bytes = b.nrows * s.run_bytes;
@@ -384,6 +384,7 @@ moebius_reshard_kernel(const __grid_constant__ DevParams p_in, const __grid_cons
     p.kv = (const KvDesc*)((const char*)p_in.hdr + (int64_t)(int32_t)h.z);     // signed: a wave header sits
     p.c2d = (const C2dDesc*)((const char*)p_in.hdr + (int64_t)(int32_t)h.w);   // behind the arrays it uses
     p.bulk = (const BulkDesc*)((const char*)p_in.hdr + (int64_t)(int32_t)__ldg(&p_in.hdr->bulk_off));
+    p.wblk = (const WBlk*)((const char*)p_in.hdr + (int64_t)(int32_t)__ldg(&p_in.hdr->wblk_off));
   }
   const uint32_t lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   uint64_t* bar = (uint64_t*)smem + 2 * warp;                       // 2 barriers per pipe
@@ -771,6 +772,7 @@ int launch_reshard_kernel(moebius_ctx* x, bool tma, int64_t unit_hint, cudaStrea
   p.ticket = (uint32_t*)x->desc;
   p.counters = (uint32_t*)(x->desc + kCtrOff);
   p.rank_stride = x->rank_stride;
+  p.wstg_off = x->staging_bytes - x->w_stg_bytes;
   p.page_tokens = (uint32_t)x->cfg.page_tokens;
   int threads, per_sm;
   size_t smem = 0;

@@ -10,8 +10,8 @@
 
 namespace moebius {
 
-constexpr int kMaxCounters = 4096;
-constexpr int kMaxSegs = 8192;
+constexpr int kMaxCounters = 16384;
+constexpr int kMaxSegs = 32768;
 constexpr int64_t kHdrBytes = 256;                         // ticket lives at byte 0
 constexpr int64_t kCtrOff = kHdrBytes;                     // uint32 counters[kMaxCounters]
 constexpr int64_t kSegOff = kCtrOff + 4 * kMaxCounters;    // Seg[...]
@@ -82,6 +82,9 @@ struct moebius_ctx {
   int64_t run_kv, ep_page_bytes, tp_page_bytes, pool_bytes;
   int32_t pages_ep, pages_tp;
   int64_t staging_bytes, desc_bytes, table_bytes, resident_bytes, spare_bytes;
+  int64_t w_stg_bytes;            // tail of the staging buffer reserved for parked weight blocks (S2); 0 when every
+                                  // object moves out of place
+  int64_t max_wblk;
   int64_t max_kv_desc, max_c2d;
   // bound buffers
   bool bound;
@@ -129,6 +132,7 @@ struct moebius_plan {
   std::vector<moebius::Seg> segs;
   std::vector<moebius::C2dDesc> c2d;
   std::vector<moebius::BulkDesc> bulk;
+  std::vector<moebius::WBlk> wblk;
   const moebius::KvDesc* kv;      // n_kv descriptors, inside `image`
   int64_t n_kv;
   std::vector<int32_t> lens, owner;   // target-mode request state
@@ -139,7 +143,7 @@ struct moebius_plan {
   int64_t stage_bytes; int xt_rows;   // geometry the plan was built for
   // one contiguous upload image: [segs][kv][c2d], and the table image; pinned when CUDA allows
   char* image;
-  int64_t image_bytes, kv_img_off, c2d_img_off, bulk_img_off;
+  int64_t image_bytes, kv_img_off, c2d_img_off, bulk_img_off, wblk_img_off;
   // rank-share execution (multi-GPU): per dependency wave a header + segment list inside the image
   int32_t n_waves;
   int64_t wave_img_off;

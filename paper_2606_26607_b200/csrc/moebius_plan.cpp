@@ -25,6 +25,7 @@ void scale_blocks(int r, int R, int I, int* lo, int* hi) {
 }
 
 constexpr int kMaxLevelCap = 1024;   // hard bound on dependency rounds (counters: kMaxCounters)
+constexpr int kS2BlocksPerRank = 64;  // S2: an in-place object is cut into about this many blocks per rank
 
 }  // namespace
 
@@ -115,6 +116,22 @@ int moebius_create(const moebius_config_t* c, moebius_ctx_t** out) {
   // rank region: [weight chain: 3L+ep_shift slots][TP scales][EP scales][2L KV pools]
   x->S = align_up((int64_t)(E / R) * H * I * wb, 256);
   x->w_off = 0;
+  // How far the EP view of an object sits behind its TP view.  The largest object's size makes every
+  // move out of place (S1; PAPER.md:150-156 at object grain).  When the cap does not allow that many
+  // spare slots the shift shrinks -- to 0 if need be, where both views alias the same bytes -- and the
+  // objects that overlap themselves take the in-place path (S2, s2_object below), with at least a fifth of
+  // the cap kept for staging.
+  if (R > 1) {
+    const int max_obj = x->ep_shift;
+    int64_t dup = 0;
+    if (c->attn_mode == MOEBIUS_ATTN_DUAL)
+      dup = (2 * (int64_t)(c->n_q_heads / R) + 2 * (int64_t)x->hpr) * D * H * 2 * L * R;
+    int sft = max_obj;
+    if (c->w_inplace) sft = 0;
+    else if (c->staging_cap_bytes > 0)
+      while (sft > 0 && (int64_t)sft * x->S * R + dup > (sft == max_obj ? c->staging_cap_bytes : c->staging_cap_bytes / 5 * 4)) --sft;
+    x->ep_shift = sft;
+  }
   int64_t off = (int64_t)(3 * L + x->ep_shift) * x->S;
   x->scale_tp_layer = x->scale_ep_layer = 0;
   memset(x->sg, 0, sizeof(x->sg));
@@ -172,6 +189,21 @@ int moebius_create(const moebius_config_t* c, moebius_ctx_t** out) {
     x->staging_bytes = std::min(c->staging_cap_bytes - overhead, kv_total);
   }
   x->staging_bytes = x->staging_bytes / x->ep_page_bytes * x->ep_page_bytes;
+  // S2: the tail half of the staging buffer parks weight blocks, the head stays with the KV schedule
+  x->w_stg_bytes = 0;
+  x->max_wblk = 0;
+  if (R > 1) {
+    bool s2 = false;
+    for (int o = 0; o < x->n_obj; ++o) s2 |= x->obj[o].n_slots > x->ep_shift;
+    if (s2) {
+      if (c->staging_cap_bytes == 0) {   // no bound given: room to park 2R+2 of the largest EP rows (one expert matrix)
+        const int64_t need = (2 * (int64_t)R + 2) * I * H * wb * 2;
+        x->staging_bytes = std::max(x->staging_bytes, align_up(2 * need, x->ep_page_bytes));
+      }
+      x->w_stg_bytes = x->staging_bytes / 2 / 256 * 256;
+      x->max_wblk = (int64_t)L * x->n_obj * R * 4 * kS2BlocksPerRank;
+    }
+  }
 
   // descriptor buffer: header, counters, segments, KV moves (each live page at most twice), scale copies
   int64_t live_max = std::max<int64_t>((int64_t)x->pages_tp, (int64_t)x->pages_ep * R);
@@ -180,7 +212,7 @@ int moebius_create(const moebius_config_t* c, moebius_ctx_t** out) {
   x->max_c2d = c->w_dtype == MOEBIUS_FP8_E4M3_B128 ? (int64_t)x->n_obj * L * R * R : 0;
   x->max_bulk = c->attn_mode == MOEBIUS_ATTN_GATHER ? (int64_t)L * R * (2 * (int64_t)R + 2 * (int64_t)std::max(R, Hkv)) : 0;
   x->desc_bytes = align_up(kSegOff + (int64_t)(1 + kMaxCounters) * sizeof(PlanHdr) + 2 * (int64_t)kMaxSegs * sizeof(Seg) + x->max_kv_desc * sizeof(KvDesc) +
-                               x->max_c2d * sizeof(C2dDesc) + x->max_bulk * sizeof(BulkDesc) + 1024, 4096);
+                               x->max_c2d * sizeof(C2dDesc) + (x->max_bulk + x->max_wblk) * sizeof(BulkDesc) + x->max_wblk * sizeof(WBlk) + 1024, 4096);
   x->table_bytes = align_up(4 * ((int64_t)kTblHdrInts + 2 * (int64_t)c->max_requests +
                                  (int64_t)c->max_requests * c->max_pages_per_request), 256);
   x->bound = false;
@@ -249,6 +281,9 @@ int moebius_layout(const moebius_ctx_t* x, moebius_layout_t* o) {
   o->tbl_reserved = 0;
   o->attn_full_bytes = x->attn_full_bytes;
   o->attn_dup_bytes = x->attn_dup_bytes;
+  o->w_staging_bytes = x->w_stg_bytes;
+  o->w_shift_slots = x->ep_shift;
+  o->reserved1 = 0;
   return MOEBIUS_OK;
 }
 
@@ -679,7 +714,7 @@ struct PlanBuilder {
           K = 0;
           int64_t ns = 0;
           for (int m = 0; m < nm; ++m) { if (!mv[m].staged) K = std::max(K, (int)mv[m].level); else ++ns; }
-          if (ns * x->ep_page_bytes <= x->staging_bytes || max_level >= kMaxLevelCap) break;
+          if (ns * x->ep_page_bytes <= x->staging_bytes - x->w_stg_bytes || max_level >= kMaxLevelCap) break;
         }
       } else if (any_self) {
         // self-overlapping moves only: they are staged; nobody else depends on anything
@@ -690,7 +725,7 @@ struct PlanBuilder {
     pools_per_group = n_pools_all;
     if (n_staged > 0) {
       int64_t per_pool = (int64_t)n_staged * x->ep_page_bytes;
-      int64_t fit = x->staging_bytes / per_pool;
+      int64_t fit = (x->staging_bytes - x->w_stg_bytes) / per_pool;
       if (fit < 1) return MOEBIUS_E_STAGING;
       pools_per_group = (int)std::min<int64_t>(fit, n_pools_all);
       if (n_staged >= (1 << 24)) return MOEBIUS_E_STAGING;
@@ -710,6 +745,185 @@ struct PlanBuilder {
     memset(&P->stats, 0, sizeof(P->stats));
     P->stats.struct_size = sizeof(moebius_stats_t);
     next_ctr = 0;
+    return MOEBIUS_OK;
+  }
+
+  // ---- S2 (BASELINE.json north_star: "in-place permutation cycles through a bounded
+  // staging buffer") -- one object whose EP view starts fewer slots behind its TP view than the object is
+  // long, so that part of what it writes lands on its own unread source.
+  // The object is cut into BLOCKS (rows [i*T, (i+1)*T) of EP rank q: contiguous on the EP side, R pieces
+  // on the TP side).  Block b BLOCKS on block a when b's destination overlaps a's source and a has not
+  // been read yet.  The blocks are executed in dependency WAVES: a wave holds every block all of whose
+  // blockers were read in earlier waves.  When no block is ready (the permutation's cycles) the cheapest
+  // blocked block is chosen and its blockers are PARKED: their source is saved into a staging slot
+  // (EP->TP: the EP rows are copied there; TP->EP: the block is transposed INTO the slot) and finished
+  // from the slot once their own destination is free; a slot is reused as soon as its block is finished.
+  // `tmpl` carries the object's shape and unit geometry as weight_chain chose them.
+  int s2_object(const Seg& tmpl_in, int& prev_ctr, uint32_t& prev_units) {
+    Seg tmpl = tmpl_in;
+    const int64_t run = tmpl.run_bytes, rt = tmpl.rows_total, Rr = (int64_t)R * run;
+    const int64_t sS = (int64_t)x->ep_shift * x->S;            // EP view offset minus TP view offset
+    const bool xt = seg_path(tmpl) == PATH_TMA && tmpl.groups_per_unit == tmpl.n_groups;
+    // a tensor-map box cannot address the staging buffer: staged EP sides of short-run objects use ld/st
+    Seg lsu = tmpl;
+    if (xt) {
+      lsu.kind = SEG_XPOSE;
+      lsu.groups_per_unit = R; lsu.chunk_bytes = (uint32_t)run; lsu.chunks_per_run = 1;
+      lsu.rows_per_unit = (uint32_t)std::max<int64_t>(1, unit_bytes / Rr);
+    }
+    // 2R+2 slots let the simulation below always make progress; with less staging it is tried with what
+    // fits (it reports E_STAGING itself when a cycle needs more parked blocks than there are slots)
+    int64_t unit_rows = xt ? tmpl.rows_per_unit : 1;
+    int64_t t_max = x->w_stg_bytes / (2 * (int64_t)R + 2) / Rr;
+    if (t_max < 1) t_max = std::min<int64_t>(1, x->w_stg_bytes / Rr);
+    if (t_max < 1) return MOEBIUS_E_STAGING;
+    if (xt && t_max < unit_rows) {       // blocks smaller than one box: the whole object goes through ld/st
+      tmpl = lsu;
+      unit_rows = 1;
+    }
+    int64_t T = (rt + kS2BlocksPerRank - 1) / kS2BlocksPerRank;
+    T = (T + unit_rows - 1) / unit_rows * unit_rows;
+    T = std::min(T, t_max / unit_rows * unit_rows);
+    T = std::max<int64_t>(T, unit_rows);
+    const int nb = (int)((rt + T - 1) / T), NB = nb * R;
+    const int64_t slot_bytes = T * Rr;
+    const int n_slots = (int)std::min<int64_t>(x->w_stg_bytes / slot_bytes, 1 << 20);
+    auto rows_of = [&](int i) { return std::min<int64_t>(T, rt - (int64_t)i * T); };
+    // blockers of every block (CSR): the blocks whose SOURCE this block's DESTINATION overlaps
+    std::vector<int32_t> bo((size_t)NB + 1, 0), bl;
+    std::vector<uint8_t> self((size_t)NB, 0);
+    for (int q = 0; q < R; ++q) for (int i = 0; i < nb; ++i) {
+      const int b = q * nb + i;
+      int32_t tmp[160]; int nt = 0;
+      auto note = [&](int a) { if (a == b) self[(size_t)b] = 1; else if (nt < 160) tmp[nt++] = a; };
+      if (e2t) {     // writes TP rows [q*rt + i*T, +rows) on EVERY rank; sources: EP rows of rank j at sS + row*Rr
+        const int64_t y0 = ((int64_t)q * rt + (int64_t)i * T) * run, y1 = y0 + rows_of(i) * run;
+        if (y1 > sS && y0 < sS + rt * Rr) {
+          const int64_t lo = std::max<int64_t>(0, (y0 - sS) / (T * Rr)), hi = std::min<int64_t>(nb - 1, (y1 - 1 - sS) / (T * Rr));
+          for (int j = 0; j < R; ++j) for (int64_t a = (y0 < sS ? 0 : lo); a <= hi; ++a) note(j * nb + (int)a);
+        }
+      } else {       // writes EP rows [i*T, +rows) of rank q; sources: TP rows (global index q2*rt + row) read on every rank
+        const int64_t w0 = sS + (int64_t)i * T * Rr, w1 = w0 + rows_of(i) * Rr;
+        const int64_t g0 = w0 / run, g1 = std::min<int64_t>((w1 - 1) / run, (int64_t)R * rt - 1);
+        for (int64_t g = g0; g <= g1;) {
+          const int64_t q2 = g / rt, i2 = (g % rt) / T;
+          note((int)(q2 * nb + i2));
+          g = q2 * rt + std::min<int64_t>(rt, (i2 + 1) * T);     // first row of the next block
+        }
+      }
+      std::sort(tmp, tmp + nt);
+      nt = (int)(std::unique(tmp, tmp + nt) - tmp);
+      for (int k = 0; k < nt; ++k) bl.push_back(tmp[k]);
+      bo[(size_t)b + 1] = (int32_t)bl.size();
+    }
+    // greedy wave simulation
+    enum { OP_MOVE = 0, OP_FINISH = 1, OP_PARK = 2 };
+    struct Op { int32_t blk, op, slot; };
+    std::vector<std::vector<Op>> waves;
+    std::vector<int32_t> read_wave((size_t)NB, INT32_MAX);    // wave in which the block's source was read (moved or parked)
+    std::vector<int32_t> slot_of((size_t)NB, -1);
+    std::vector<uint8_t> done((size_t)NB, 0);
+    std::vector<int32_t> free_slots;
+    for (int k = n_slots - 1; k >= 0; --k) free_slots.push_back(k);
+    int n_done = 0, n_parked = 0;
+    while (n_done < NB) {
+      const int32_t w = (int32_t)waves.size();
+      if (w > 4 * NB + 8) return MOEBIUS_E_STAGING;
+      std::vector<Op> ops;
+      std::vector<int32_t> freed;
+      for (int b = 0; b < NB; ++b) {
+        if (done[(size_t)b]) continue;
+        if (self[(size_t)b] && !(slot_of[(size_t)b] >= 0 && read_wave[(size_t)b] < w)) continue;
+        if (slot_of[(size_t)b] >= 0 && read_wave[(size_t)b] >= w) continue;     // parked in this very wave
+        bool ok = true;
+        for (int32_t e = bo[(size_t)b]; e < bo[(size_t)b + 1] && ok; ++e) ok = read_wave[(size_t)bl[(size_t)e]] < w;
+        if (!ok) continue;
+        if (slot_of[(size_t)b] >= 0) { ops.push_back({b, OP_FINISH, slot_of[(size_t)b]}); freed.push_back(slot_of[(size_t)b]); }
+        else { ops.push_back({b, OP_MOVE, 0}); read_wave[(size_t)b] = w; }
+        done[(size_t)b] = 1; ++n_done;
+      }
+      if (ops.empty()) {      // a cycle: park the blockers of the block that needs the fewest parks
+        int best = -1, best_need = INT32_MAX;
+        for (int b = 0; b < NB; ++b) {
+          if (done[(size_t)b]) continue;
+          int need = (self[(size_t)b] && slot_of[(size_t)b] < 0) ? 1 : 0;
+          for (int32_t e = bo[(size_t)b]; e < bo[(size_t)b + 1]; ++e) need += read_wave[(size_t)bl[(size_t)e]] == INT32_MAX;
+          if (need > 0 && need < best_need) { best = b; best_need = need; }
+        }
+        if (best < 0 || best_need > (int)free_slots.size()) return MOEBIUS_E_STAGING;
+        auto park = [&](int a) {
+          const int32_t sl = free_slots.back(); free_slots.pop_back();
+          slot_of[(size_t)a] = sl; read_wave[(size_t)a] = w;
+          ops.push_back({a, OP_PARK, sl});
+          ++n_parked;
+          P->stats.w_staged_bytes += rows_of(a % nb) * Rr;
+        };
+        if (self[(size_t)best] && slot_of[(size_t)best] < 0) park(best);
+        for (int32_t e = bo[(size_t)best]; e < bo[(size_t)best + 1]; ++e)
+          if (read_wave[(size_t)bl[(size_t)e]] == INT32_MAX) park(bl[(size_t)e]);
+      }
+      for (int32_t sl : freed) free_slots.push_back(sl);
+      waves.push_back(std::move(ops));
+    }
+    P->stats.n_w_waves += (int32_t)waves.size();
+    P->stats.n_w_parked += n_parked;
+    // segments: per wave up to three kinds of work, full and ragged blocks apart (a segment has one shape)
+    for (const std::vector<Op>& ops : waves) {
+      if (next_ctr >= (uint32_t)kMaxCounters) return MOEBIUS_E_STAGING;
+      const int ctr = (int)next_ctr++;
+      uint32_t wave_units = 0;
+      for (int kind = 0; kind < 3; ++kind) for (int ragged = 0; ragged < 2; ++ragged) {
+        const int64_t rows = ragged ? rows_of(nb - 1) : T;
+        if (ragged && rows == T) continue;
+        std::vector<WBlk> blks;
+        for (const Op& o : ops) {
+          const int i = o.blk % nb;
+          if (o.op != kind || (rows_of(i) != T) != (ragged != 0)) continue;
+          blks.push_back({(uint32_t)(o.blk / nb), (uint32_t)((int64_t)i * T), (uint32_t)rows_of(i), (uint32_t)o.slot});
+        }
+        if (blks.empty()) continue;
+        // which side of the work is plain copying between the EP rows and the slot
+        const bool copy = (kind == OP_PARK && e2t) || (kind == OP_FINISH && !e2t);
+        Seg t;
+        if (!copy) {
+          t = (kind == OP_MOVE) ? tmpl : (xt && seg_path(tmpl) == PATH_TMA ? lsu : tmpl);
+          t.kv_mode = kind == OP_MOVE ? 0u : 1u;             // 1: the EP side of every block is its staging slot
+          t.pool_begin = (uint32_t)P->wblk.size();
+          t.n_desc = (uint32_t)blks.size();
+          t.pool_bytes = slot_bytes;
+          const uint32_t rbpb = (uint32_t)((rows + t.rows_per_unit - 1) / t.rows_per_unit);
+          t.pools_per_unit = rbpb * (t.n_groups / t.groups_per_unit) * t.chunks_per_run;
+          t.n_units = t.n_desc * t.pools_per_unit;
+          for (const WBlk& k : blks) P->wblk.push_back(k);
+        } else {
+          t = blank_seg();
+          t.kind = SEG_BULK | ((x->use_tma ? PATH_TMA : PATH_LSU) << 8);
+          t.kv_mode = e2t ? 2u : 1u;                           // EP->TP park: destination in staging; TP->EP finish: source
+          t.ep_is_src = e2t;
+          t.rows_total = (uint32_t)(rows * R);                 // the block's EP rows as R*rows contiguous runs
+          t.run_bytes = (uint32_t)run;
+          const int64_t lim = x->use_tma ? x->stage_bytes : unit_bytes;
+          t.chunk_bytes = pick_chunk(run, lim);
+          t.chunks_per_run = (uint32_t)(run / t.chunk_bytes);
+          t.rows_per_unit = t.chunks_per_run == 1 ? (uint32_t)std::max<int64_t>(1, std::min<int64_t>(rows * R, lim / run)) : 1;
+          t.row_blocks = (t.rows_total + t.rows_per_unit - 1) / t.rows_per_unit;
+          t.ep_off = run; t.tp_off = run;
+          t.desc_begin = (uint32_t)P->bulk.size();
+          t.n_desc = (uint32_t)blks.size();
+          for (const WBlk& k : blks) {
+            const int64_t ep = (int64_t)k.q * x->rank_stride + tmpl.ep_off + (int64_t)k.row0 * Rr;
+            const int64_t sl = (int64_t)k.slot * slot_bytes;
+            P->bulk.push_back(e2t ? BulkDesc{ep, sl} : BulkDesc{sl, ep});
+          }
+          t.n_units = t.n_desc * t.row_blocks * t.chunks_per_run;
+        }
+        t.wait_ctr = prev_ctr; t.wait_target = prev_units;
+        t.signal_ctr = ctr;
+        wave_units += t.n_units;
+        push_seg(cw, t);
+      }
+      prev_ctr = ctr; prev_units = wave_units;
+    }
     return MOEBIUS_OK;
   }
 
@@ -772,6 +986,10 @@ struct PlanBuilder {
         int64_t nu = (int64_t)R * s.row_blocks * (s.n_groups / s.groups_per_unit) * s.chunks_per_run;
         if (nu > (1ll << 30)) return fail(MOEBIUS_E_INVAL);
         s.n_units = (uint32_t)nu;
+        if (ob.n_slots > x->ep_shift) {      // its EP view overlaps its own TP view: the in-place path (S2)
+          if (int rc = s2_object(s, prev_ctr, prev_units)) return fail(rc);
+          continue;
+        }
         s.wait_ctr = prev_ctr; s.wait_target = prev_units;
         if (next_ctr >= (uint32_t)kMaxCounters) return fail(MOEBIUS_E_INVAL);   // the counters sit below the uploaded image
         s.signal_ctr = (int32_t)next_ctr++;
@@ -1014,7 +1232,8 @@ struct PlanBuilder {
       P->segs.push_back(s);
     }
     if (ub >= (1ull << 32) || P->segs.size() > (size_t)kMaxSegs || (int64_t)nm > x->max_kv_desc ||
-        P->c2d.size() > (size_t)x->max_c2d || P->bulk.size() > (size_t)x->max_bulk)
+        P->c2d.size() > (size_t)x->max_c2d || P->bulk.size() > (size_t)(x->max_bulk + x->max_wblk) ||
+        P->wblk.size() > (size_t)x->max_wblk)
       return fail(MOEBIUS_E_INVAL);
     P->total_units = (uint32_t)ub;
     P->n_counters = next_ctr;
@@ -1054,10 +1273,12 @@ struct PlanBuilder {
     int64_t c2d_b = align_up((int64_t)P->c2d.size() * sizeof(C2dDesc), 256);
     const int64_t hdr_b = sizeof(PlanHdr);
     int64_t bulk_b = align_up((int64_t)P->bulk.size() * sizeof(BulkDesc), 256);
+    int64_t wblk_b = align_up((int64_t)P->wblk.size() * sizeof(WBlk), 256);
     P->kv_img_off = hdr_b + seg_b;
     P->c2d_img_off = hdr_b + seg_b + kv_b;
     P->bulk_img_off = hdr_b + seg_b + kv_b + c2d_b;
-    P->wave_img_off = hdr_b + seg_b + kv_b + c2d_b + bulk_b;
+    P->wblk_img_off = hdr_b + seg_b + kv_b + c2d_b + bulk_b;
+    P->wave_img_off = hdr_b + seg_b + kv_b + c2d_b + bulk_b + wblk_b;
     const int64_t wave_b = (int64_t)P->n_waves * hdr_b + (int64_t)P->segs.size() * (int64_t)sizeof(Seg);
     P->image_bytes = P->wave_img_off + wave_b;
     if (kSegOff + P->image_bytes > x->desc_bytes) return fail(MOEBIUS_E_INVAL);
@@ -1072,6 +1293,7 @@ struct PlanBuilder {
       h->kv_off = (uint32_t)P->kv_img_off;
       h->c2d_off = (uint32_t)P->c2d_img_off;
       h->bulk_off = (uint32_t)P->bulk_img_off;
+      h->wblk_off = (uint32_t)P->wblk_img_off;
     }
     if (!P->segs.empty()) {
       memcpy(P->image + hdr_b, P->segs.data(), P->segs.size() * sizeof(Seg));
@@ -1102,6 +1324,10 @@ struct PlanBuilder {
       memcpy(P->image + P->bulk_img_off, P->bulk.data(), P->bulk.size() * sizeof(BulkDesc));
       memset(P->image + P->bulk_img_off + P->bulk.size() * sizeof(BulkDesc), 0, (size_t)(bulk_b - (int64_t)(P->bulk.size() * sizeof(BulkDesc))));
     }
+    if (wblk_b) {
+      memcpy(P->image + P->wblk_img_off, P->wblk.data(), P->wblk.size() * sizeof(WBlk));
+      memset(P->image + P->wblk_img_off + P->wblk.size() * sizeof(WBlk), 0, (size_t)(wblk_b - (int64_t)(P->wblk.size() * sizeof(WBlk))));
+    }
     {  // per wave: a header + that wave's segments with their own unit numbering and no dependencies;
        // descriptor offsets are relative to the wave's header (negative: the arrays sit before it)
       P->wave_hdr_off.assign((size_t)P->n_waves, 0);
@@ -1128,6 +1354,7 @@ struct PlanBuilder {
         h->kv_off = (uint32_t)(int32_t)(P->kv_img_off - at);
         h->c2d_off = (uint32_t)(int32_t)(P->c2d_img_off - at);
         h->bulk_off = (uint32_t)(int32_t)(P->bulk_img_off - at);
+        h->wblk_off = (uint32_t)(int32_t)(P->wblk_img_off - at);
         P->wave_units[(size_t)w] = units;
         at += hdr_b + (int64_t)n * (int64_t)sizeof(Seg);
       }
@@ -1211,6 +1438,7 @@ extern "C" int moebius_plan_export(const moebius_plan_t* p, int what, void* buf,
     case 2: src = p->c2d.data();  n = (int64_t)p->c2d.size() * sizeof(C2dDesc); break;
     case 3: src = p->seg_wave.data(); n = (int64_t)p->seg_wave.size() * 4; break;
     case 4: src = p->bulk.data(); n = (int64_t)p->bulk.size() * sizeof(BulkDesc); break;
+    case 5: src = p->wblk.data(); n = (int64_t)p->wblk.size() * sizeof(WBlk); break;
     default: return MOEBIUS_E_INVAL;
   }
   *needed = n;
@@ -1230,6 +1458,7 @@ extern "C" int moebius_share_stats(const moebius_plan_t* P, int rank_lo, int ran
   p.kv = P->kv;
   p.c2d = P->c2d.data();
   p.bulk = P->bulk.data();
+  p.wblk = P->wblk.data();
   p.rank_stride = x->rank_stride;
   int64_t units = 0, rd = 0, wr = 0, cross = 0;
   for (size_t si = 0; si < P->segs.size(); ++si) {
@@ -1250,18 +1479,18 @@ extern "C" int moebius_share_stats(const moebius_plan_t* P, int rank_lo, int ran
         BulkUnit bu;
         decode_bulk(s, p, u, bu);
         const int64_t b = (int64_t)bu.nrows * bu.piece;
-        rd += b; wr += b; cross += b;     // always from another rank's shard
-        continue;
+        rd += b; wr += b;
+        if (!(s.kv_mode & 3u)) cross += b;     // attention gather: always from another rank's shard; a parked
+        continue;                               // block stays on its rank
       }
       if (seg_kind(s) == SEG_XPOSE) {
-        uint32_t v = u / s.chunks_per_run;
-        const uint32_t jgroups = s.n_groups / s.groups_per_unit;
-        const uint32_t jg = v % jgroups;
-        const uint32_t rb = (v / jgroups) % s.row_blocks;
-        const int64_t nrows = std::min<int64_t>(s.rows_per_unit, (int64_t)s.rows_total - (int64_t)rb * s.rows_per_unit);
-        const int64_t per_group = nrows * s.chunk_bytes;
+        Box bx;
+        decode_box(s, p, u, 0, bx);
+        const int64_t per_group = (int64_t)bx.nrows * s.chunk_bytes;
         rd += per_group * s.groups_per_unit; wr += per_group * s.groups_per_unit;
-        for (uint32_t g = jg * s.groups_per_unit; g < (jg + 1) * s.groups_per_unit; ++g)
+        // a block moving between the EP rows and its staging slot stays on its rank (kv_mode & 1: the EP
+        // side is the slot, so only the TP pieces of other ranks cross)
+        for (uint32_t g = bx.g0; g < bx.g0 + s.groups_per_unit; ++g)
           if ((int)g != q) cross += per_group;
         continue;
       }

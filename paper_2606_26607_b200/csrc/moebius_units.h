@@ -92,7 +92,20 @@ struct C2dDesc {          // 32 bytes: rows x run_bytes, 4-byte elements, offset
 };
 static_assert(sizeof(C2dDesc) == 32, "C2dDesc must be 32 bytes");
 
-struct BulkDesc {         // 16 bytes: one strided copy of the segment's shape, offsets from dev_base
+// XPOSE block-list mode (an object whose EP view overlaps its own TP view is moved
+// block by block in dependency waves, blocks on cycles parked in the bounded staging buffer).  A block is
+// rows [row0, row0 + nrows) of EP rank q; `slot` is its staging slot when the segment's EP side is the
+// staging buffer (Seg::kv_mode & 1).  Fields reused by such a segment: n_desc = number of blocks (0 = the
+// whole object, the common case), pool_begin = first WBlk, pools_per_unit = units per block, pool_bytes =
+// bytes of one staging slot.
+struct WBlk {
+  uint32_t q, row0, nrows, slot;
+};
+static_assert(sizeof(WBlk) == 16, "WBlk must be 16 bytes");
+
+struct BulkDesc {         // 16 bytes: one strided copy of the segment's shape; offsets from dev_base, or from
+                          // the weight part of the staging buffer when Seg::kv_mode has bit 0 (source) /
+                          // bit 1 (destination) set
   int64_t  src_off, dst_off;
 };
 static_assert(sizeof(BulkDesc) == 16, "BulkDesc must be 16 bytes");
@@ -106,7 +119,8 @@ struct PlanHdr {
   uint32_t kv_off;        // byte offsets from the start of the image
   uint32_t c2d_off;
   uint32_t bulk_off;
-  uint32_t pad_[59];
+  uint32_t wblk_off;
+  uint32_t pad_[58];
 };
 static_assert(sizeof(PlanHdr) == 256, "PlanHdr must be 256 bytes");
 
@@ -118,6 +132,8 @@ struct DevParams {        // decoded launch state (the kernel fills the plan-dep
   const KvDesc* kv;
   const C2dDesc*   c2d;
   const BulkDesc*  bulk;
+  const WBlk*      wblk;
+  int64_t          wstg_off;      // weight part of the staging buffer (its tail), bytes from `stg`
   uint32_t*        ticket;
   uint32_t*        counters;
   int64_t          rank_stride;
@@ -146,6 +162,7 @@ struct Box {
   uint32_t lin;
   char    *lin_src, *lin_dst;
   uint64_t lin_bytes;
+  uint32_t q, row0;       // XPOSE: EP rank and first row of this unit (tensor-map coordinates)
 };
 
 // KV unit u of a segment = (pool block pb, descriptor di), pool-block-major: consecutive units are
@@ -177,6 +194,7 @@ MB_HD uint32_t tp_src_rank(uint32_t g, uint32_t rep, int32_t owner) {
 // that owns this rank.
 MB_HD uint32_t unit_ep_rank(const Seg& s, const DevParams& p, uint32_t u) {
   if (seg_kind(s) == SEG_XPOSE) {
+    if (s.n_desc) return p.wblk[s.pool_begin + u / s.pools_per_unit].q;
     u /= s.chunks_per_run;
     u /= s.n_groups / s.groups_per_unit;
     return u / s.row_blocks;
@@ -188,7 +206,9 @@ MB_HD uint32_t unit_ep_rank(const Seg& s, const DevParams& p, uint32_t u) {
   }
   if (seg_kind(s) == SEG_BULK) {    // pulled by the rank that receives it
     const uint32_t per_desc = s.row_blocks * s.chunks_per_run;
-    return (uint32_t)(p.bulk[s.desc_begin + u / per_desc].dst_off / p.rank_stride);
+    const BulkDesc d = p.bulk[s.desc_begin + u / per_desc];
+    // a copy into / out of the staging buffer belongs to the rank whose bytes it parks
+    return (uint32_t)(((s.kv_mode & 2u) ? d.src_off : d.dst_off) / p.rank_stride);
   }
   const C2dDesc& d = p.c2d[s.desc_begin + u];
   return (uint32_t)((s.ep_is_src ? d.src_off : d.dst_off) / p.rank_stride);
@@ -213,8 +233,10 @@ MB_HD void decode_bulk(const Seg& s, const DevParams& p, uint32_t u, BulkUnit& b
   b.piece = s.chunk_bytes;
   b.src_stride = s.ep_off;
   b.dst_stride = s.tp_off;
-  b.src = p.base + d.src_off + (int64_t)row0 * s.ep_off + (int64_t)ch * s.chunk_bytes;
-  b.dst = p.base + d.dst_off + (int64_t)row0 * s.tp_off + (int64_t)ch * s.chunk_bytes;
+  char* sb = (s.kv_mode & 1u) ? p.stg + p.wstg_off : p.base;
+  char* db = (s.kv_mode & 2u) ? p.stg + p.wstg_off : p.base;
+  b.src = sb + d.src_off + (int64_t)row0 * s.ep_off + (int64_t)ch * s.chunk_bytes;
+  b.dst = db + d.dst_off + (int64_t)row0 * s.tp_off + (int64_t)ch * s.chunk_bytes;
 }
 
 // Decode box k of unit u (u is LOCAL to the segment).
@@ -224,24 +246,39 @@ MB_HD void decode_box(const Seg& s, const DevParams& p, uint32_t u, uint32_t k, 
   b.rep = s.rep;
   b.tp_row_stride = s.run_bytes;
   if (seg_kind(s) == SEG_XPOSE) {
-    uint32_t ch = u % s.chunks_per_run;  u /= s.chunks_per_run;
-    uint32_t jgroups = s.n_groups / s.groups_per_unit;
-    uint32_t jg = u % jgroups;           u /= jgroups;
-    uint32_t rb = u % s.row_blocks;      uint32_t q = u / s.row_blocks;
-    uint32_t row0 = rb * s.rows_per_unit;
-    uint32_t nrows = s.rows_total - row0;
+    const uint32_t jgroups = s.n_groups / s.groups_per_unit;
+    uint32_t q, row0, row_end, blk_row0 = 0, slot = 0;
+    if (s.n_desc) {                       // block-list mode: unit = (block, row block, group block, chunk)
+      const uint32_t di = u / s.pools_per_unit;
+      u -= di * s.pools_per_unit;
+      const WBlk k = p.wblk[s.pool_begin + di];
+      q = k.q; blk_row0 = k.row0; row_end = k.row0 + k.nrows; slot = k.slot;
+    } else {
+      q = u / (s.row_blocks * jgroups * s.chunks_per_run);
+      u -= q * (s.row_blocks * jgroups * s.chunks_per_run);
+      row_end = s.rows_total;
+    }
+    const uint32_t ch = u % s.chunks_per_run;  u /= s.chunks_per_run;
+    const uint32_t jg = u % jgroups;           const uint32_t rb = u / jgroups;
+    row0 = blk_row0 + rb * s.rows_per_unit;
+    uint32_t nrows = row_end - row0;
     if (nrows > s.rows_per_unit) nrows = s.rows_per_unit;
     b.nrows = nrows;
+    b.q = q; b.row0 = row0;
     b.J = s.groups_per_unit;
     b.g0 = jg * s.groups_per_unit;
     b.cc = s.chunk_bytes >> 4;
     b.owner = -1;
     b.ep_row_stride = s.n_groups * s.run_bytes;
-    int64_t ep = (int64_t)q * p.rank_stride + s.ep_off +
-                 ((int64_t)row0 * s.n_groups + b.g0) * s.run_bytes + (int64_t)ch * s.chunk_bytes;
     int64_t tp = s.tp_off + ((int64_t)q * s.rows_total + row0) * s.run_bytes + (int64_t)ch * s.chunk_bytes;
-    b.ep = p.base + ep;
     b.tp = p.base + tp;
+    if (s.n_desc && (s.kv_mode & 1u)) {   // the block's EP rows live in its staging slot
+      b.ep = p.stg + p.wstg_off + (int64_t)slot * s.pool_bytes +
+             ((int64_t)(row0 - blk_row0) * s.n_groups + b.g0) * s.run_bytes + (int64_t)ch * s.chunk_bytes;
+    } else {
+      b.ep = p.base + (int64_t)q * p.rank_stride + s.ep_off +
+             ((int64_t)row0 * s.n_groups + b.g0) * s.run_bytes + (int64_t)ch * s.chunk_bytes;
+    }
     return;
   }
   // SEG_KV

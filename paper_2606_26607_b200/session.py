@@ -15,7 +15,8 @@ _W_DT = {"bf16": B.MOEBIUS_BF16, "fp32": B.MOEBIUS_FP32, "fp8_e4m3_b128": B.MOEB
 
 def make_config(*, R, L, E, H, I, w_dtype="bf16", kv_heads, head_dim, page_tokens,
                 kv_pool_bytes_per_rank_layer, max_requests, max_pages_per_request,
-                staging_cap_bytes=0, kv_dtype="bf16", w_orient=0, n_q_heads=0, attn_mode=0) -> B.moebius_config_t:
+                staging_cap_bytes=0, kv_dtype="bf16", w_orient=0, n_q_heads=0, attn_mode=0,
+                w_inplace=0) -> B.moebius_config_t:
     c = B.moebius_config_t()
     c.R, c.L, c.E, c.H, c.I = R, L, E, H, I
     c.w_dtype = _W_DT[w_dtype]
@@ -26,6 +27,7 @@ def make_config(*, R, L, E, H, I, w_dtype="bf16", kv_heads, head_dim, page_token
     c.max_requests, c.max_pages_per_request = max_requests, max_pages_per_request
     c.staging_cap_bytes = int(staging_cap_bytes)
     c.n_q_heads, c.attn_mode = n_q_heads, attn_mode
+    c.w_inplace = w_inplace
     return c
 
 
@@ -80,6 +82,10 @@ class Session:
             self.tables = self.arena[offs[3]:offs[3] + sizes[3]].view(torch.int32)
             B.moebius_bind(self.ctx, self.base.data_ptr(), self.staging.data_ptr(), self.desc.data_ptr(),
                            self.tables.data_ptr(), initial_mode)
+
+    def w_staging_offset(self) -> int:
+        """Where the weight part of the staging buffer starts (its tail; S2 parks blocks there)."""
+        return int(self.layout.staging_bytes - self.layout.w_staging_bytes)
 
     # -- views ------------------------------------------------------------------------------------
     def view_desc(self, mode, rank, layer, tensor_id) -> B.moebius_view_t:

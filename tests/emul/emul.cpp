@@ -55,7 +55,8 @@ struct Checker {
 
 extern "C" __attribute__((visibility("default")))
 int emul_run(char* base, int64_t base_bytes, char* stg, int64_t stg_bytes, const Seg* segs, int n_segs,
-             const KvDesc* kv, const C2dDesc* c2d, int64_t rank_stride, int64_t* out /*[8]*/, const BulkDesc* bulk) {
+             const KvDesc* kv, const C2dDesc* c2d, int64_t rank_stride, int64_t* out /*[8]*/, const BulkDesc* bulk,
+             const WBlk* wblk, int64_t wstg_off) {
   Checker ck;
   ck.base = base; ck.base_bytes = base_bytes; ck.stg = stg; ck.stg_bytes = stg_bytes;
   ck.n = n_segs; ck.violations = ck.oob = ck.bytes_read = ck.bytes_written = 0;
@@ -79,7 +80,7 @@ int emul_run(char* base, int64_t base_bytes, char* stg, int64_t stg_bytes, const
   }
   DevParams p;
   memset(&p, 0, sizeof(p));
-  p.base = base; p.stg = stg; p.segs = segs; p.kv = kv; p.c2d = c2d; p.bulk = bulk;
+  p.base = base; p.stg = stg; p.segs = segs; p.kv = kv; p.c2d = c2d; p.bulk = bulk; p.wblk = wblk; p.wstg_off = wstg_off;
   p.rank_stride = rank_stride; p.n_segs = (uint32_t)n_segs;
   uint64_t expect_begin = 0;
   int64_t bad_begin = 0;

@@ -29,7 +29,7 @@ def mb_config(cfg: wl.Config, seq_lens, pool_policy=None, staging_cap_frac=0.0, 
                        kv_heads=cfg.kv_heads, head_dim=cfg.head_dim, page_tokens=cfg.page,
                        kv_pool_bytes_per_rank_layer=pool, max_requests=max_requests or max(n, 1),
                        max_pages_per_request=mp, staging_cap_bytes=0, w_orient=cfg.w_orient,
-                       n_q_heads=cfg.n_q_heads, attn_mode=cfg.attn_mode)
+                       n_q_heads=cfg.n_q_heads, attn_mode=cfg.attn_mode, w_inplace=cfg.w_inplace)
     if staging_cap_frac:
         s = mb.Session(c)
         c.staging_cap_bytes = int(staging_cap_frac * s.layout.resident_bytes)
@@ -110,7 +110,7 @@ def emul_lib():
             subprocess.check_call(["g++", "-O2", "-std=c++17", "-shared", "-fPIC", "-o", so, src])
         _EMUL = C.CDLL(so)
         _EMUL.emul_run.argtypes = [C.c_void_p, C.c_int64, C.c_void_p, C.c_int64, C.c_void_p, C.c_int,
-                                   C.c_void_p, C.c_void_p, C.c_int64, C.c_void_p, C.c_void_p]
+                                   C.c_void_p, C.c_void_p, C.c_int64, C.c_void_p, C.c_void_p, C.c_void_p, C.c_int64]
     return _EMUL
 
 
@@ -121,9 +121,10 @@ def emulate(sess: mb.Session, plan, image: np.ndarray, staging: np.ndarray):
     kv = mb.moebius_plan_export(plan, 1)
     c2d = mb.moebius_plan_export(plan, 2)
     bulk = mb.moebius_plan_export(plan, 4)
+    wblk = mb.moebius_plan_export(plan, 5)
     out = np.zeros(8, np.int64)
     vp = lambda a: a.ctypes.data_as(C.c_void_p) if a.size else None  # noqa: E731
     emul_lib().emul_run(vp(image), image.size, vp(staging), staging.size, vp(segs), len(segs), vp(kv), vp(c2d),
-                        sess.layout.rank_stride_bytes, vp(out), vp(bulk))
+                        sess.layout.rank_stride_bytes, vp(out), vp(bulk), vp(wblk), sess.w_staging_offset())
     return {"violations": int(out[0]), "oob": int(out[1]), "bad_wait": int(out[2]), "bad_begin": int(out[3]),
             "bytes_read": int(out[4]), "bytes_written": int(out[5]), "units": int(out[6])}

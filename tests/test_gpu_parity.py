@@ -559,3 +559,42 @@ def test_naive_path_with_tight_pools_needs_no_rounds():
     for _ in range(3):
         mode, owner, bt, stats = gpu_switch(st, sess, mode, owner, bt, execute=naive_execute)
     sess.close()
+
+
+S2_GPU_CASES = {
+    "tiny_inplace": (wl.get_config("tiny").with_(w_inplace=1), 0.0),
+    "smallish_inplace": (SMALLISH.with_(w_inplace=1, seed=81), 0.0),
+    "small_config_inplace": (wl.get_config("small").with_(w_inplace=1, L=2, n_req=16), 0.0),     # XT boxes inside blocks
+    "odd_shape_inplace": (wl.get_config("tiny").with_(R=3, E=6, H=40, I=72, kv_heads=3, head_dim=8, n_req=9,
+                                                       len_dist=("uniform", 1, 90), seed=21, w_inplace=1), 0.0),
+    "E60_R4_inplace": (wl.get_config("tiny").with_(R=4, E=60, H=24, I=32, kv_heads=4, n_req=5, seed=22, w_inplace=1), 0.0),
+    "paper_orient_shift1": (SMALLISH.with_(w_orient=1, seed=83, L=3), -1.95),
+    "paper_orient_inplace": (SMALLISH.with_(w_orient=1, w_inplace=1, seed=82), 0.0),
+    "fp8_inplace": (wl.get_config("fp8_graph").with_(L=2, E=8, H=256, I=1536, n_req=6, len_dist=("uniform", 1, 60), seed=3,
+                                                     w_inplace=1), 0.0),
+}
+
+
+@pytest.mark.parametrize("name", sorted(S2_GPU_CASES))
+@pytest.mark.parametrize("first", [TP, EP])
+def test_s2_in_place_path_on_device(name, first):
+    """SURVEY.md section 7 S2 on the device: aliased (or partly overlapping) EP / TP views, blocks in
+    dependency waves, blocks on permutation cycles parked in the bounded staging buffer -- including a
+    non-power-of-two shape (E = 60, R = 4; R = 3) -- bit-exact with the oracle in both directions."""
+    cfg, cap = S2_GPU_CASES[name]
+    lens = wl.draw_seq_lens(cfg)
+    if cap < 0:
+        probe = mb.Session(mb_config(cfg, lens))
+        cap = -cap * probe.layout.weight_slot_bytes * cfg.R / probe.layout.resident_bytes
+        probe.close()
+    st, sess = gpu_session(cfg, lens, cap_frac=cap, fill="normal" if cfg.w_dtype == "fp8_e4m3_b128" else "tag",
+                           initial_mode=first)
+    assert sess.layout.w_shift_slots < (2 if cfg.w_orient else 1) and sess.layout.w_staging_bytes > 0
+    owner, bt, _ = start(st, sess, first, "random")
+    mode = first
+    waves = 0
+    for _ in range(3):
+        mode, owner, bt, stats = gpu_switch(st, sess, mode, owner, bt)
+        waves = max(waves, stats["n_w_waves"])
+    assert waves > 0
+    sess.close()

@@ -37,7 +37,9 @@ def run_switch(st, sess, image, staging, from_mode, src_owner, src_bt):
     if stats["n_kv_staged"] == 0:
         # EP->TP reads a straddled scale block once per holder: `read` counts unique source bytes (A15)
         rereads = stats["w_relocated"] - stats["w_read"]
-        assert res["bytes_written"] == direct_bytes and res["bytes_read"] == stats["w_read"] + stats["kv_read"] + stats["attn_read"] + rereads
+        parked = stats["w_staged_bytes"]      # S2: a parked block is written to its slot and read back once more
+        assert res["bytes_written"] == direct_bytes + parked
+        assert res["bytes_read"] == stats["w_read"] + stats["kv_read"] + stats["attn_read"] + rereads + parked
     tgt = OracleLayout(st, sess, to_mode, want_owner, want_bt)
     bad = tgt.compare(image)
     assert not bad, bad[:5]
@@ -168,11 +170,20 @@ def test_staging_reused_across_pool_groups_and_too_small():
     with pytest.raises(mb.MoebiusError) as e:
         sess4.plan(EP, st.lens, owner, bt, from_mode=TP)
     assert e.value.status == -3
-    # cap below the spare weight slot itself
+    # cap below the spare weight slot itself: no longer a refusal -- the views alias (shift 0) and the
+    # weights take the in-place path, the cap going to staging
     c.staging_cap_bytes = spare - 1
-    with pytest.raises(mb.MoebiusError) as e:
-        mb.Session(c)
-    assert e.value.status == -3
+    sess5 = mb.Session(c)
+    assert sess5.layout.w_shift_slots == 0 and sess5.layout.weight_spare_bytes == 0
+    assert 0 < sess5.layout.staging_bytes <= spare - 1
+    st0 = State(cfg, [])                      # weight-only switches: all of it goes to the weights
+    empty = np.zeros((0, 1), np.int32)
+    image = np.full(sess5.layout.base_bytes, 0xA5, np.uint8)
+    staging = np.full(sess5.layout.staging_bytes, 0x5A, np.uint8)
+    OracleLayout(st0, sess5, TP, None, empty).place(image)
+    _, o5, bt5, stats5 = run_switch(st0, sess5, image, staging, TP, None, empty)
+    assert stats5["n_w_waves"] > 0 and stats5["n_w_parked"] > 0
+    run_switch(st0, sess5, image, staging, EP, np.zeros(0, np.int32), empty)
 
 
 def test_capacity_error_cancels_switch():
@@ -352,10 +363,11 @@ def test_waves_with_barriers_are_hazard_free(first, policy, orient):
     kv = mb.moebius_plan_export(plan, 1)
     c2d = mb.moebius_plan_export(plan, 2)
     bulk = mb.moebius_plan_export(plan, 4)
+    wblk = mb.moebius_plan_export(plan, 5)
     out = np.zeros(8, np.int64)
     vp = lambda a: a.ctypes.data_as(C.c_void_p) if a.size else None  # noqa: E731
     emul_lib().emul_run(vp(image), image.size, vp(staging), staging.size, vp(segs), len(segs), vp(kv), vp(c2d),
-                        sess.layout.rank_stride_bytes, vp(out), vp(bulk))
+                        sess.layout.rank_stride_bytes, vp(out), vp(bulk), vp(wblk), sess.w_staging_offset())
     assert out[0] == 0 and out[1] == 0 and out[2] == 0 and out[3] == 0, out
     want_owner, want_bt = expected_target(st, sess, to)
     assert not OracleLayout(st, sess, to, want_owner, want_bt).compare(image)
@@ -413,3 +425,83 @@ def test_attention_projections_follow_the_switch(attn_mode, R, Hq, Hkv):
         if attn_mode == 1:   # pointer swap: compare() has checked BOTH modes' views; nothing moved
             assert stats["attn_moved"] == 0
     sess.close()
+
+
+S2_CASES = {
+    # name: (config, staging cap as a fraction of resident bytes or 0)
+    "tiny_inplace": (wl.get_config("tiny").with_(w_inplace=1), 0.0),
+    "small_inplace": (SMALLISH.with_(w_inplace=1, seed=81), 0.0),
+    "odd_shape_inplace": (wl.get_config("tiny").with_(R=3, E=6, H=40, I=72, kv_heads=3, head_dim=8, n_req=9,
+                                                       len_dist=("uniform", 1, 90), seed=21, w_inplace=1), 0.0),
+    "E60_R4_inplace": (wl.get_config("tiny").with_(R=4, E=60, H=24, I=32, kv_heads=4, n_req=5, seed=22, w_inplace=1), 0.0),
+    "paper_orient_inplace": (SMALLISH.with_(w_orient=1, w_inplace=1, seed=82), 0.0),
+    "paper_orient_shift1": (SMALLISH.with_(w_orient=1, seed=83, L=3), -1.95),     # cap = 1.95 objects: one spare slot, not two
+    "fp8_inplace": (wl.get_config("fp8_graph").with_(L=2, E=8, H=256, I=1536, n_req=6, len_dist=("uniform", 1, 60), seed=3,
+                                                     w_inplace=1), 0.0),
+    "R5_inplace": (wl.get_config("tiny").with_(R=5, E=10, H=16, I=40, kv_heads=5, n_req=4, seed=23, w_inplace=1), 0.0),
+}
+
+
+@pytest.mark.parametrize("name", sorted(S2_CASES))
+@pytest.mark.parametrize("first", [TP, EP])
+def test_s2_in_place_path(name, first):
+    """SURVEY.md section 7 S2 / BASELINE.json north_star: when the cap leaves no room for a spare slot as
+    large as the largest object, the EP and TP views overlap (down to aliasing the same bytes) and the
+    move becomes an in-place permutation: blocks in dependency waves, blocks on cycles parked in the
+    bounded staging buffer.  Hazard-free under the emulator and bit-exact with the oracle, both ways."""
+    cfg, cap = S2_CASES[name]
+    st = State(cfg, fill="normal" if cfg.w_dtype == "fp8_e4m3_b128" else "tag")
+    if cap < 0:        # given in units of one object over all ranks
+        probe = mb.Session(mb_config(cfg, st.lens))
+        cap = -cap * probe.layout.weight_slot_bytes * cfg.R / probe.layout.resident_bytes
+        probe.close()
+    sess = mb.Session(mb_config(cfg, st.lens, None, cap))
+    lay = sess.layout
+    max_obj = 2 if cfg.w_orient else 1
+    assert lay.w_shift_slots < max_obj and lay.w_staging_bytes > 0
+    assert lay.weight_spare_bytes == lay.w_shift_slots * lay.weight_slot_bytes * cfg.R
+    if cap:
+        assert lay.weight_spare_bytes + lay.staging_bytes <= cap * lay.resident_bytes
+    image = np.full(lay.base_bytes, 0xA5, np.uint8)
+    staging = np.full(max(lay.staging_bytes, 16), 0x5A, np.uint8)
+    owner, bt = source_tables(st, sess, first, "random")
+    OracleLayout(st, sess, first, owner, bt).place(image)
+    mode = first
+    waves = parked = 0
+    for _ in range(3):
+        mode, owner, bt, stats = run_switch(st, sess, image, staging, mode, owner, bt)
+        waves, parked = max(waves, stats["n_w_waves"]), max(parked, stats["n_w_parked"])
+        assert stats["w_staged_bytes"] <= stats["w_relocated"]
+    assert waves > 0
+    if lay.w_shift_slots == 0:
+        assert parked > 0          # aliased views: nothing can start before something is parked
+    sess.close()
+
+
+def test_s2_is_chosen_by_the_cap_and_refuses_only_what_cannot_fit():
+    """The planner picks the shift from staging_cap_bytes: S1 (every move out of place) when a spare of
+    the largest object fits, else fewer slots plus the in-place path; E_STAGING only when not even the
+    duplicated attention shards fit."""
+    cfg = SMALLISH.with_(w_orient=1, L=3, seed=83)
+    lens = wl.draw_seq_lens(cfg)
+    probe = mb.Session(mb_config(cfg, lens))
+    res, S = probe.layout.resident_bytes, probe.layout.weight_slot_bytes * cfg.R
+    assert probe.layout.w_shift_slots == 2          # no cap: S1
+    probe.close()
+    seen = set()
+    for cap in (2.2 * S, 2 * S, 1.99 * S, 1.3 * S, S, 0.5 * S, 1):
+        c = mb_config(cfg, lens)
+        c.staging_cap_bytes = int(cap)
+        s = mb.Session(c)
+        lay = s.layout
+        seen.add(lay.w_shift_slots)
+        assert lay.weight_spare_bytes + lay.staging_bytes <= max(int(cap), lay.weight_spare_bytes)
+        assert lay.w_staging_bytes == 0 if lay.w_shift_slots == 2 else (lay.w_staging_bytes > 0 or cap < S)
+        if cap == 1:     # a cap that leaves no staging at all: the in-place path cannot park anything -> cancelled
+            bt = wl.random_page_tables(lens, None, cfg.R, lay.pages_tp, cfg.page, c.max_pages_per_request, seed=1)
+            with pytest.raises(mb.MoebiusError) as e:
+                s.plan(EP, lens, None, bt, from_mode=TP)
+            assert e.value.status == -3
+        s.close()
+    assert seen == {0, 1, 2}
+    assert res > 0

@@ -27,6 +27,7 @@ class Config:
     pool_policy: str = "roomy"   # roomy = 1.1 x (TP need + max EP live)
     w_orient: int = 0            # 0: gate,up [E,H,I], down [E,I,H] (BASELINE.json); 1: W13 [E,2I,H], W2 [E,H,I]
     n_q_heads: int = 0           # query heads (attention projections); 0 = no attention tensors
+    w_inplace: int = 0           # 1: force the fully in-place weight path (EP and TP views alias the same bytes)
     attn_mode: int = 0           # 0 none, 1 both layouts resident (pointer swap), 2 memory-saving (All-Gather rebuild)
     extra: dict = field(default_factory=dict)
 
