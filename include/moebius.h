@@ -269,6 +269,25 @@ MOEBIUS_API int moebius_reshard_share(moebius_ctx_t* ctx, const moebius_plan_t* 
 MOEBIUS_API int moebius_share_stats(const moebius_plan_t* plan, int rank_lo, int rank_hi, int wave, int64_t* out4);
 MOEBIUS_API int moebius_reshard_publish(moebius_ctx_t* ctx, const moebius_plan_t* plan, void* cuda_stream);
 
+/* The same split with the round barrier ON THE DEVICE: one launch per GPU for the whole switch instead of
+ * one launch and one host barrier per wave ("one cross-GPU barrier per dependency
+ * round").  The ranks are cut into n_shares shares, share s owning ranks
+ * [rank_bounds[s], rank_bounds[s+1]) (HOST int32[n_shares + 1], from 0 to R).  The launch executes shares
+ * [share_first, share_first + share_count): its CTAs are divided among them, every CTA walks the plan's
+ * waves taking only its share's units, and after each wave the last CTA of a share raises the share's flag
+ * (st.release.sys) in the flag page inside that share's first rank region; every CTA then waits for the
+ * flags of ALL n_shares shares (ld.acquire.sys) -- addresses inside the unified buffer, i.e. peer memory
+ * when the share runs on another GPU.
+ *   share_count == n_shares: the whole switch on this device in ONE cooperative launch whose CTA groups
+ *     play the GPUs (this is how the barrier is verified on one GPU: separate launches that wait for one
+ *     another must not be run on one device).
+ *   share_count == 1: the launch of one GPU of n_shares; the other GPUs launch theirs concurrently, after a
+ *     host barrier that follows everybody's flag clearing.  (Not exercisable on a one-GPU pool.)
+ * Uploads the work list like moebius_reshard; end the switch with moebius_reshard_publish.  Needs
+ * cooperative-launch support and 2 * n_shares * waves <= 16384. */
+MOEBIUS_API int moebius_reshard_shares(moebius_ctx_t* ctx, const moebius_plan_t* plan, int n_shares,
+                                       const int32_t* rank_bounds, int share_first, int share_count, void* cuda_stream);
+
 /* ---- the staged comparison path (needs a CUDA device) --------------- */
 
 /* PAPER.md:162-170 and Table 1 (:176-189): the "Naive" implementation of a switch -- per object, gather

@@ -20,7 +20,7 @@ EXPORTED_SYMBOLS = [
     "moebius_create", "moebius_destroy", "moebius_layout", "moebius_view", "moebius_bind",
     "moebius_active_mode", "moebius_plan", "moebius_plan_destroy", "moebius_block_tables",
     "moebius_plan_stats", "moebius_plan_export", "moebius_reshard", "moebius_stage_plan", "moebius_reshard_staged",
-    "moebius_naive_scratch_bytes", "moebius_reshard_naive",
+    "moebius_naive_scratch_bytes", "moebius_reshard_naive", "moebius_reshard_shares",
     "moebius_share_stats", "moebius_plan_waves", "moebius_reshard_share", "moebius_reshard_publish",
     "moebius_arena_create", "moebius_arena_destroy", "moebius_arena_base", "moebius_arena_ready",
     "moebius_arena_export", "moebius_arena_import",
@@ -262,6 +262,17 @@ def moebius_plan_export(plan, what: int) -> np.ndarray:
 
 def moebius_reshard(ctx, plan, cuda_stream: int = 0):
     _chk(_lib.moebius_reshard(ctx, plan, _vp(cuda_stream or None)), "moebius_reshard")
+
+
+_lib.moebius_reshard_shares.argtypes = [_vp, _vp, C.c_int, _vp, C.c_int, C.c_int, _vp]
+
+
+def moebius_reshard_shares(ctx, plan, rank_bounds, share_first: int, share_count: int, cuda_stream: int = 0):
+    """One launch executing shares [share_first, share_first + share_count) of len(rank_bounds) - 1, all
+    waves, with the device-side round barrier."""
+    b = _i32(rank_bounds)
+    _chk(_lib.moebius_reshard_shares(ctx, plan, len(b) - 1, b.ctypes.data_as(_vp), share_first, share_count,
+                                     _vp(cuda_stream or None)), "moebius_reshard_shares")
 
 
 _lib.moebius_naive_scratch_bytes.argtypes = [_vp, _vp, C.POINTER(C.c_int64)]

@@ -376,15 +376,33 @@ moebius_reshard_kernel(const __grid_constant__ DevParams p_in, const __grid_cons
   // The arguments are the same for every switch of a context (so that the launch can be replayed
   // from a captured graph); what differs per plan is read from the uploaded image's header.
   DevParams p = p_in;
-  {
-    const uint4 h = __ldg((const uint4*)p_in.hdr);
+  auto load_hdr = [&](const PlanHdr* hp) {
+    const uint4 h = __ldg((const uint4*)hp);
     p.n_segs = h.x;
     p.total_units = h.y;
-    p.segs = (const Seg*)((const char*)p_in.hdr + sizeof(PlanHdr));
-    p.kv = (const KvDesc*)((const char*)p_in.hdr + (int64_t)(int32_t)h.z);     // signed: a wave header sits
-    p.c2d = (const C2dDesc*)((const char*)p_in.hdr + (int64_t)(int32_t)h.w);   // behind the arrays it uses
-    p.bulk = (const BulkDesc*)((const char*)p_in.hdr + (int64_t)(int32_t)__ldg(&p_in.hdr->bulk_off));
-    p.wblk = (const WBlk*)((const char*)p_in.hdr + (int64_t)(int32_t)__ldg(&p_in.hdr->wblk_off));
+    p.segs = (const Seg*)((const char*)hp + sizeof(PlanHdr));
+    p.kv = (const KvDesc*)((const char*)hp + (int64_t)(int32_t)h.z);     // signed: a wave header sits
+    p.c2d = (const C2dDesc*)((const char*)hp + (int64_t)(int32_t)h.w);   // behind the arrays it uses
+    p.bulk = (const BulkDesc*)((const char*)hp + (int64_t)(int32_t)__ldg(&hp->bulk_off));
+    p.wblk = (const WBlk*)((const char*)hp + (int64_t)(int32_t)__ldg(&hp->wblk_off));
+  };
+  load_hdr(p_in.hdr);
+  // Round-barrier mode: this CTA belongs to one share and walks the plan's dependency waves, each from
+  // its own dependency-free segment list and with the share's own ticket; a barrier across ALL shares
+  // (this launch's and, on several GPUs, the peers') separates the waves.
+  const bool bar_mode = p_in.n_shares > 0;
+  uint32_t my_share = 0, share_ctas = 0, n_waves = 1;
+  const uint32_t* wave_tab = nullptr;
+  if (bar_mode) {
+    my_share = p_in.share_first + (uint32_t)(((uint64_t)blockIdx.x * p_in.share_count) / gridDim.x);
+    const uint32_t k = my_share - p_in.share_first;     // CTAs [ceil(k*G/n), ceil((k+1)*G/n)) map to share k
+    const uint32_t lo = (uint32_t)(((uint64_t)k * gridDim.x + p_in.share_count - 1) / p_in.share_count);
+    const uint32_t hi = (uint32_t)(((uint64_t)(k + 1) * gridDim.x + p_in.share_count - 1) / p_in.share_count);
+    share_ctas = hi - lo;
+    n_waves = __ldg(&p_in.hdr->n_waves);
+    wave_tab = (const uint32_t*)((const char*)p_in.hdr + __ldg(&p_in.hdr->wave_tab_off));
+    p.rank_lo = p_in.share_bounds[my_share];
+    p.rank_hi = p_in.share_bounds[my_share + 1];
   }
   const uint32_t lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   uint64_t* bar = (uint64_t*)smem + 2 * warp;                       // 2 barriers per pipe
@@ -456,6 +474,12 @@ moebius_reshard_kernel(const __grid_constant__ DevParams p_in, const __grid_cons
   auto fetch = [&]() -> uint32_t { return lane == 0 ? atomicAdd(p.ticket, 1u) : 0u; };
 
   const bool share = p.rank_hi - p.rank_lo < p.n_ranks;
+  for (uint32_t wv = 0; wv < n_waves; ++wv) {
+  if (bar_mode) {
+    load_hdr((const PlanHdr*)((const char*)p_in.hdr + __ldg(wave_tab + wv)));
+    p.ticket = p_in.counters + (size_t)my_share * n_waves + wv;      // wave lists carry no dependency: the counters are free
+    ok_si = 0xffffffffu;
+  }
   uint32_t si = 0;
   uint32_t t_next = fetch();
   for (;;) {
@@ -497,6 +521,32 @@ moebius_reshard_kernel(const __grid_constant__ DevParams p_in, const __grid_cons
     }
   }
   drain();
+  if (bar_mode) {
+    // every pipe of this CTA has drained: its writes of this wave are complete.  The last CTA of the share
+    // raises the share's flag; then everybody waits for the flags of all shares.
+    __syncthreads();
+    if (threadIdx.x == 0) {
+      __threadfence_system();
+      uint32_t* arrive = p_in.counters + (size_t)(p_in.n_shares + my_share) * n_waves + wv;
+      if (atomicAdd(arrive, 1u) + 1 == share_ctas) {
+        uint32_t* mine = (uint32_t*)(p_in.base + (int64_t)p_in.share_bounds[my_share] * p_in.rank_stride + p_in.flag_off) + wv;
+        asm volatile("st.release.sys.global.u32 [%0], %1;" :: "l"(mine), "r"(1u) : "memory");
+      }
+      for (uint32_t sh = 0; sh < p_in.n_shares; ++sh) {
+        const uint32_t* f = (const uint32_t*)(p_in.base + (int64_t)p_in.share_bounds[sh] * p_in.rank_stride + p_in.flag_off) + wv;
+        uint32_t v = 0;
+        for (uint32_t spins = 0;; ++spins) {
+          asm volatile("ld.acquire.sys.global.u32 %0, [%1];" : "=r"(v) : "l"(f) : "memory");
+          if (v) break;
+          __nanosleep(100);
+          if (spins > (1u << 26)) __trap();     // a share that never arrives must not hang the box
+        }
+      }
+    }
+    __syncthreads();
+    fence_proxy_async();     // the next wave's TMA reads see what the other shares wrote
+  }
+  }
 }
 
 // Upload images.  A plan's image is read by the async H2D copies of moebius_reshard, so a buffer that
@@ -759,10 +809,20 @@ int ready_to_launch(const moebius_ctx* x, const moebius_plan_t* P) {
 // Launches the reshard kernel over the image that sits at dev_desc + kSegOff.  `tma`: the variant with
 // the pipes' shared-memory rings (it also executes PATH_LSU segments).  `unit_hint` > 0 caps the grid
 // for small plans; 0 = the full persistent grid (plan-independent: what a captured graph needs).
+struct ShareLaunch {       // round-barrier mode of the kernel (DevParams::n_shares)
+  int n_shares, first, count;
+  const int32_t* bounds;   // [n_shares + 1]
+};
+
 int launch_reshard_kernel(moebius_ctx* x, bool tma, int64_t unit_hint, cudaStream_t st, int64_t hdr_off = 0,
-                          int rank_lo = 0, int rank_hi = -1) {
+                          int rank_lo = 0, int rank_hi = -1, const ShareLaunch* sl = nullptr) {
   DevParams p;
   memset(&p, 0, sizeof(p));
+  if (sl) {
+    p.n_shares = (uint32_t)sl->n_shares; p.share_first = (uint32_t)sl->first; p.share_count = (uint32_t)sl->count;
+    p.flag_off = x->flag_off;
+    for (int i = 0; i <= sl->n_shares; ++i) p.share_bounds[i] = (uint8_t)sl->bounds[i];
+  }
   p.base = x->base;
   p.stg = x->stg;
   p.hdr = (const PlanHdr*)(x->desc + kSegOff + hdr_off);
@@ -793,6 +853,15 @@ int launch_reshard_kernel(moebius_ctx* x, bool tma, int64_t unit_hint, cudaStrea
   if (unit_hint > 0) {
     int64_t grid_cap = (unit_hint + threads / 32 - 1) / (threads / 32);
     if (grid > grid_cap) grid = grid_cap;
+  }
+  if (sl) {
+    // CTAs of different shares wait for one another: all of them must be resident at once, which only
+    // a cooperative launch guarantees (one CTA per SM with the pipes' rings, two without)
+    void* args[4] = {(void*)&p, (void*)x->tmap_w, (void*)x->tmap_kv, (void*)x->tmap_stg};
+    const void* fn = tma ? (const void*)moebius_reshard_kernel<1> : (const void*)moebius_reshard_kernel<2>;
+    if (grid < sl->count) return MOEBIUS_E_INVAL;
+    return cudaLaunchCooperativeKernel(fn, dim3((unsigned)grid), dim3((unsigned)threads), args, smem, st) == cudaSuccess
+               ? MOEBIUS_OK : MOEBIUS_E_CUDA;
   }
   if (tma)
     moebius_reshard_kernel<1><<<(unsigned)grid, threads, smem, st>>>(p, *(const CUtensorMap*)x->tmap_w, *(const CUtensorMap*)x->tmap_kv,
@@ -913,4 +982,40 @@ extern "C" int moebius_reshard_publish(moebius_ctx_t* x, const moebius_plan_t* P
   x->active_mode = P->to;
   x->switch_count++;
   return MOEBIUS_OK;
+}
+
+// ---- the switch as ONE launch per GPU with a device-side round barrier --------------------------------
+extern "C" int moebius_reshard_shares(moebius_ctx_t* x, const moebius_plan_t* P, int n_shares, const int32_t* rank_bounds,
+                                      int share_first, int share_count, void* cuda_stream) {
+  if (!x || !P || P->ctx != x || !rank_bounds) return MOEBIUS_E_INVAL;
+  const int R = x->cfg.R;
+  if (n_shares < 1 || n_shares > R || share_first < 0 || share_count < 1 || share_first + share_count > n_shares) return MOEBIUS_E_INVAL;
+  if (rank_bounds[0] != 0 || rank_bounds[n_shares] != R) return MOEBIUS_E_INVAL;
+  for (int i = 0; i < n_shares; ++i) if (rank_bounds[i + 1] <= rank_bounds[i]) return MOEBIUS_E_INVAL;
+  if (!x->bound || x->active_mode != P->from) return MOEBIUS_E_STATE;
+  if (int rc = ready_to_launch(x, P)) return rc;
+  if (2 * (int64_t)n_shares * P->n_waves > kMaxCounters || P->n_waves > kMaxCounters) return MOEBIUS_E_INVAL;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  // tickets (one per share and wave) and arrival counters live in the counter area; the flag pages of
+  // the shares THIS launch executes are cleared here -- on several GPUs every process clears its own and
+  // a host barrier precedes the launches (one per switch, not one per wave)
+  if (cudaMemsetAsync(x->desc, 0, (size_t)kSegOff, st) != cudaSuccess) return MOEBIUS_E_CUDA;
+  for (int sh = share_first; sh < share_first + share_count; ++sh)
+    if (P->n_waves && cudaMemsetAsync(x->base + (int64_t)rank_bounds[sh] * x->rank_stride + x->flag_off, 0, (size_t)P->n_waves * 4, st) != cudaSuccess)
+      return MOEBIUS_E_CUDA;
+  if (cudaMemcpyAsync(x->desc + kSegOff, P->image, (size_t)P->image_bytes, cudaMemcpyHostToDevice, st) != cudaSuccess)
+    return MOEBIUS_E_CUDA;
+  if (P->buf.ev && cudaEventRecord((cudaEvent_t)P->buf.ev, st) != cudaSuccess) return MOEBIUS_E_CUDA;
+  cudaEvent_t ev_a = nullptr, ev_b = nullptr;
+  if (x->timing) {
+    int64_t k = x->ev_count % kTimingRing;
+    ev_a = (cudaEvent_t)x->ev[2 * k]; ev_b = (cudaEvent_t)x->ev[2 * k + 1];
+    cudaEventRecord(ev_a, st);
+  }
+  if (P->total_units) {
+    ShareLaunch sl{n_shares, share_first, share_count, rank_bounds};
+    if (int rc = launch_reshard_kernel(x, P->uses_tma, 0, st, 0, 0, -1, &sl)) return rc;
+  }
+  if (x->timing) { cudaEventRecord(ev_b, st); x->ev_count++; }
+  return MOEBIUS_OK;   // the caller ends the switch with moebius_reshard_publish, as on the wave-by-wave path
 }

@@ -71,6 +71,7 @@ struct moebius_ctx {
   moebius::WObj obj[3];
   int64_t S;                      // weight slot bytes per rank
   int64_t w_off, scale_tp_off, scale_ep_off, kv_off, rank_stride;
+  int64_t flag_off;               // per rank region: the round-barrier flag page, uint32 flag[kMaxCounters]
   moebius::ScaleGeom sg[3];
   int64_t scale_tp_layer, scale_ep_layer;  // bytes per layer per rank
   // attention projections (attn_mode != 0): per rank and layer the four full tensors,
@@ -143,7 +144,7 @@ struct moebius_plan {
   int64_t stage_bytes; int xt_rows;   // geometry the plan was built for
   // one contiguous upload image: [segs][kv][c2d], and the table image; pinned when CUDA allows
   char* image;
-  int64_t image_bytes, kv_img_off, c2d_img_off, bulk_img_off, wblk_img_off;
+  int64_t image_bytes, kv_img_off, c2d_img_off, bulk_img_off, wblk_img_off, wave_tab_img_off;
   // rank-share execution (multi-GPU): per dependency wave a header + segment list inside the image
   int32_t n_waves;
   int64_t wave_img_off;

@@ -172,6 +172,10 @@ int moebius_create(const moebius_config_t* c, moebius_ctx_t** out) {
   }
   off = align_up(off, 4096);
   x->kv_off = off;        off += 2 * (int64_t)L * x->pool_bytes;
+  // the rank's flag page for the device-side round barrier (moebius_reshard_shares): inside the unified
+  // buffer, so that a peer GPU reaches it through the same mapping as the data
+  off = align_up(off, 4096);
+  x->flag_off = off;      off += 4 * (int64_t)kMaxCounters;
   x->rank_stride = align_up(off, 2 << 20);   // 2 MiB: a rank region can be its own physical allocation (moebius_arena_*)
 
   x->spare_bytes = (int64_t)x->ep_shift * x->S * R;
@@ -1280,7 +1284,8 @@ struct PlanBuilder {
     P->wblk_img_off = hdr_b + seg_b + kv_b + c2d_b + bulk_b;
     P->wave_img_off = hdr_b + seg_b + kv_b + c2d_b + bulk_b + wblk_b;
     const int64_t wave_b = (int64_t)P->n_waves * hdr_b + (int64_t)P->segs.size() * (int64_t)sizeof(Seg);
-    P->image_bytes = P->wave_img_off + wave_b;
+    P->wave_tab_img_off = P->wave_img_off + wave_b;
+    P->image_bytes = P->wave_tab_img_off + align_up((int64_t)P->n_waves * 4, 256);
     if (kSegOff + P->image_bytes > x->desc_bytes) return fail(MOEBIUS_E_INVAL);
     P->tbl_bytes = 4 * ((int64_t)kTblHdrInts + 2 * (int64_t)c.max_requests + (int64_t)n_req * MP);
     if (!image_acquire(x, P->image_bytes + P->tbl_bytes + 256, &P->buf)) return fail(MOEBIUS_E_INVAL);
@@ -1294,6 +1299,8 @@ struct PlanBuilder {
       h->c2d_off = (uint32_t)P->c2d_img_off;
       h->bulk_off = (uint32_t)P->bulk_img_off;
       h->wblk_off = (uint32_t)P->wblk_img_off;
+      h->n_waves = (uint32_t)P->n_waves;
+      h->wave_tab_off = (uint32_t)P->wave_tab_img_off;
     }
     if (!P->segs.empty()) {
       memcpy(P->image + hdr_b, P->segs.data(), P->segs.size() * sizeof(Seg));
@@ -1358,6 +1365,9 @@ struct PlanBuilder {
         P->wave_units[(size_t)w] = units;
         at += hdr_b + (int64_t)n * (int64_t)sizeof(Seg);
       }
+      uint32_t* tab = (uint32_t*)(P->image + P->wave_tab_img_off);
+      memset(tab, 0, (size_t)align_up((int64_t)P->n_waves * 4, 256));
+      for (int32_t w = 0; w < P->n_waves; ++w) tab[w] = (uint32_t)P->wave_hdr_off[(size_t)w];
     }
     P->tbl_image = (int32_t*)(P->image + align_up(P->image_bytes, 256));
     int32_t* T = P->tbl_image;

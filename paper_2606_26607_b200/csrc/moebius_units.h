@@ -120,7 +120,9 @@ struct PlanHdr {
   uint32_t c2d_off;
   uint32_t bulk_off;
   uint32_t wblk_off;
-  uint32_t pad_[58];
+  uint32_t n_waves;       // main header only: dependency waves, and where their headers are (wave_tab_off:
+  uint32_t wave_tab_off;  // uint32[n_waves], byte offsets of the per-wave headers from the start of the image)
+  uint32_t pad_[56];
 };
 static_assert(sizeof(PlanHdr) == 256, "PlanHdr must be 256 bytes");
 
@@ -145,6 +147,15 @@ struct DevParams {        // decoded launch state (the kernel fills the plan-dep
   uint32_t         n_ranks;       // R
   uint32_t         rank_lo, rank_hi;   // rank share: only units whose EP-side rank is in [lo, hi) are
                                        // executed (multi-GPU: the ranks this GPU owns); [0, R) = all
+  // Device-side round barrier (one cross-GPU barrier per dependency round).
+  // n_shares > 0: this launch executes shares [share_first, share_first + share_count) of n_shares --
+  // its CTAs are split evenly among them -- wave by wave; share s owns ranks [share_bounds[s],
+  // share_bounds[s+1]).  After a wave the last CTA of a share raises that share's flag for the wave
+  // (st.release.sys) in the flag page of the share's first rank; every CTA then waits for the flags of
+  // ALL n_shares shares (ld.acquire.sys) -- on several GPUs those are peer addresses.
+  uint32_t         n_shares, share_first, share_count;
+  int64_t          flag_off;           // flag page offset inside a rank region: uint32 flag[wave]
+  uint8_t          share_bounds[72];
 };
 
 MB_HD uint32_t seg_kind(const Seg& s) { return s.kind & 0xFFu; }

@@ -598,3 +598,57 @@ def test_s2_in_place_path_on_device(name, first):
         waves = max(waves, stats["n_w_waves"])
     assert waves > 0
     sess.close()
+
+
+def shares_execute(bounds):
+    def run(sess, plan):
+        stream = torch.cuda.current_stream().cuda_stream
+        mb.moebius_reshard_shares(sess.ctx, plan, bounds, 0, len(bounds) - 1, stream)
+        mb.moebius_reshard_publish(sess.ctx, plan, stream)
+    return run
+
+
+BARRIER_CASES = {
+    "smallish_2": (SMALLISH, [0, 2, 4], None, 0.0),
+    "smallish_4": (SMALLISH, [0, 1, 2, 3, 4], None, 0.0),
+    "uneven_3": (SMALLISH, [0, 1, 3, 4], None, 0.0),
+    "tight_rounds_2": (SMALLISH.with_(L=1, n_req=40, seed=99), [0, 2, 4], "tight", 0.5),
+    "replicated_heads_8": (wl.get_config("tiny").with_(R=8, E=8, I=64, kv_heads=4, n_req=7, len_dist=("uniform", 1, 70), seed=13),
+                           list(range(9)), None, 0.0),
+    "fp8_2": (wl.get_config("fp8_graph").with_(L=1, E=8, H=256, I=1536, n_req=6, len_dist=("uniform", 1, 60), seed=3),
+              [0, 4, 8], None, 0.0),
+    "inplace_waves_2": (SMALLISH.with_(w_inplace=1, seed=81), [0, 2, 4], None, 0.0),
+    "attn_gather_2": (wl.get_config("tiny").with_(R=4, E=8, H=128, I=128, kv_heads=2, head_dim=32, n_q_heads=8, attn_mode=2, L=2,
+                                                  n_req=9, len_dist=("uniform", 1, 80), seed=64), [0, 2, 4], None, 0.0),
+    "small_config_4": (wl.get_config("small"), [0, 1, 2, 3, 4], None, 0.0),
+}
+
+
+@pytest.mark.parametrize("name", sorted(BARRIER_CASES))
+def test_device_side_round_barrier(name):
+    """the whole switch as ONE launch with the cross-share barrier on the
+    device -- per-share tickets, per-wave flags in the flag page inside each share's first rank region
+    (st.release.sys / ld.acquire.sys), here verified as one cooperative launch whose CTA groups play the
+    GPUs.  Same waves as the host-barrier path; bit-exact with the oracle, both directions, and a plain
+    fused switch can follow on the same buffers."""
+    cfg, bounds, policy, cap = BARRIER_CASES[name]
+    lens = wl.draw_seq_lens(cfg)
+    st, sess = gpu_session(cfg, lens, policy, cap, fill="normal" if cfg.w_dtype == "fp8_e4m3_b128" else "tag")
+    owner, bt, _ = start(st, sess, TP, "random", seed=2)
+    mode = TP
+    for k in range(4):
+        mode, owner, bt, stats = gpu_switch(st, sess, mode, owner, bt, execute=shares_execute(bounds) if k != 2 else None)
+    sess.close()
+
+
+def test_device_side_round_barrier_argument_checks():
+    st, sess = gpu_session(SMALLISH.with_(L=1))
+    owner, bt, _ = start(st, sess, TP, "random")
+    plan = sess.plan(EP, st.lens, owner, bt, from_mode=TP)
+    for bad in ([0, 2], [1, 4], [0, 2, 2, 4], [0, 3, 2, 4]):
+        with pytest.raises(mb.MoebiusError):
+            mb.moebius_reshard_shares(sess.ctx, plan, bad, 0, len(bad) - 1, 0)
+    with pytest.raises(mb.MoebiusError):
+        mb.moebius_reshard_shares(sess.ctx, plan, [0, 2, 4], 1, 2, 0)     # shares 1..2 of 2
+    assert mb.moebius_active_mode(sess.ctx) == TP
+    sess.close()
