@@ -331,6 +331,10 @@ MOEBIUS_API int moebius_set_tma(moebius_ctx_t* ctx, int enable, int pipes, int s
  * ~10 us on B200, a staged page an extra copy of it in all 2L pools); at most 1024.  Results are
  * identical for every value. */
 MOEBIUS_API int moebius_set_kv_rounds(moebius_ctx_t* ctx, int max_level);
+/* KV work is cut into slices that the merged work list interleaves with the weight chain, one per chain
+ * link where there is enough of it, so that the drain of a link hides behind independent KV units.
+ * min_units: the smallest slice (tuning; 0 = the default, 1024 units).  Results are identical. */
+MOEBIUS_API int moebius_set_kv_slice(moebius_ctx_t* ctx, int min_units);
 
 /* Launch shape override for the ld/st path (tuning): values <= 0 restore the defaults; threads is a
  * multiple of 32, at most 256. */

@@ -228,6 +228,7 @@ int moebius_create(const moebius_config_t* c, moebius_ctx_t** out) {
   x->threads = 0;
   x->unit_kb = 0;
   x->kv_max_level = 64;
+  x->kv_slice_floor = 0;
   x->use_tma = 1;
   x->n_pipes = 2;
   x->stage_bytes = 48 * 1024;
@@ -392,6 +393,12 @@ int moebius_set_tma(moebius_ctx_t* x, int enable, int pipes, int stage_kb) {
 int moebius_set_kv_rounds(moebius_ctx_t* x, int max_level) {
   if (!x || max_level < 0 || max_level > kMaxLevelCap) return MOEBIUS_E_INVAL;
   x->kv_max_level = max_level > 0 ? max_level : 64;
+  return MOEBIUS_OK;
+}
+
+int moebius_set_kv_slice(moebius_ctx_t* x, int min_units) {
+  if (!x || min_units < 0) return MOEBIUS_E_INVAL;
+  x->kv_slice_floor = min_units;
   return MOEBIUS_OK;
 }
 
@@ -1158,7 +1165,11 @@ struct PlanBuilder {
       };
       // a round = every segment that signals the same counter; the next round waits for all of them
       const int64_t kv_units_est = (int64_t)nm * ((n_pools_all + ppu - 1) / ppu);
-      const int64_t slice_units = std::max<int64_t>(8192, kv_units_est / std::max(1, 3 * L));
+      // one KV slice per chain link (and one to spare), so that every link is followed by independent
+      // work: the pipes that finish link k take KV units while its last units drain, and link k+1 finds
+      // its dependency satisfied.  Not below a few times the units in flight on the device.
+      const int64_t slice_floor = x->kv_slice_floor > 0 ? x->kv_slice_floor : 1024;
+      const int64_t slice_units = std::max<int64_t>(slice_floor, kv_units_est / std::max(1, L * x->n_obj + 1));
       int prev_ctr = -1; uint32_t prev_total = 0;
       for (int g = 0; g < n_pool_groups; ++g) {
         int pool0 = g * pools_per_group;
