@@ -97,6 +97,7 @@ struct moebius_ctx {
   int64_t switch_count;
   // launch shape (PATH_LSU tuning) and the TMA path's geometry (fixed before the first plan)
   int ctas_per_sm, threads, unit_kb;
+  int chain_bands;                // 1 (default): equal-sized objects are chained half by half (no drain between links)
   int kv_slice_floor;             // smallest KV slice the merge interleaves with the weight chain, in units (0: default)
   int kv_max_level;               // longest chain of dependent KV rounds before chains are cut by staging
   int use_tma;                    // planner emits PATH_TMA segments where the shapes allow

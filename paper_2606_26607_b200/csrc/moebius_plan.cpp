@@ -195,7 +195,7 @@ int moebius_create(const moebius_config_t* c, moebius_ctx_t** out) {
   x->staging_bytes = x->staging_bytes / x->ep_page_bytes * x->ep_page_bytes;
   // S2: the tail half of the staging buffer parks weight blocks, the head stays with the KV schedule
   x->w_stg_bytes = 0;
-  x->max_wblk = 0;
+  x->max_wblk = R > 1 ? (int64_t)L * x->n_obj * 2 * R : 0;     // banded chain: 4 segments of R/2 blocks per link
   if (R > 1) {
     bool s2 = false;
     for (int o = 0; o < x->n_obj; ++o) s2 |= x->obj[o].n_slots > x->ep_shift;
@@ -205,7 +205,7 @@ int moebius_create(const moebius_config_t* c, moebius_ctx_t** out) {
         x->staging_bytes = std::max(x->staging_bytes, align_up(2 * need, x->ep_page_bytes));
       }
       x->w_stg_bytes = x->staging_bytes / 2 / 256 * 256;
-      x->max_wblk = (int64_t)L * x->n_obj * R * 4 * kS2BlocksPerRank;
+      x->max_wblk += (int64_t)L * x->n_obj * R * 4 * kS2BlocksPerRank;
     }
   }
 
@@ -229,6 +229,7 @@ int moebius_create(const moebius_config_t* c, moebius_ctx_t** out) {
   x->unit_kb = 0;
   x->kv_max_level = 64;
   x->kv_slice_floor = 0;
+  x->chain_bands = 1;
   x->use_tma = 1;
   x->n_pipes = 2;
   x->stage_bytes = 48 * 1024;
@@ -393,6 +394,12 @@ int moebius_set_tma(moebius_ctx_t* x, int enable, int pipes, int stage_kb) {
 int moebius_set_kv_rounds(moebius_ctx_t* x, int max_level) {
   if (!x || max_level < 0 || max_level > kMaxLevelCap) return MOEBIUS_E_INVAL;
   x->kv_max_level = max_level > 0 ? max_level : 64;
+  return MOEBIUS_OK;
+}
+
+int moebius_set_chain_bands(moebius_ctx_t* x, int enable) {
+  if (!x) return MOEBIUS_E_INVAL;
+  x->chain_bands = enable ? 1 : 0;
   return MOEBIUS_OK;
 }
 
@@ -947,21 +954,17 @@ struct PlanBuilder {
     // regions it does overwrite belong to objects earlier in the chain, which have completed
     // (each link waits for the previous one, transitively for all of them).
     if (R > 1) {
-      int prev_ctr = -1; uint32_t prev_units = 0;
       const int n_links = L * x->n_obj;
-      for (int step = 0; step < n_links; ++step) {
-        const int k = e2t ? step : n_links - 1 - step;
-        const int layer = k / x->n_obj;
-        const WObj& ob = x->obj[k % x->n_obj];
-        const int tp_slot = 3 * layer + ob.slot;
-        Seg s = blank_seg();
+      // shape, data path and unit geometry of one chain link
+      auto link_seg = [&](const WObj& ob, int tp_slot, Seg& s) -> int {
+        s = blank_seg();
         s.kind = SEG_XPOSE;
         s.ep_is_src = e2t;
         s.n_groups = R;
         s.rep = 1;
         int64_t run = !ob.long_run ? (int64_t)(c.I / R) * x->wb : (int64_t)(c.I / R) * c.H * x->wb;
         s.rows_total = !ob.long_run ? (uint32_t)(c.E / R) * c.H : (uint32_t)(c.E / R) * ob.row_mult;
-        if (run > (1ll << 31)) return fail(MOEBIUS_E_INVAL);
+        if (run > (1ll << 31)) return MOEBIUS_E_INVAL;
         s.run_bytes = (uint32_t)run;
         s.desc_begin = (uint32_t)(tp_slot + x->ep_shift);   // EP slot index (tensor-map coordinate)
         const int64_t stage = x->stage_bytes;
@@ -995,8 +998,58 @@ struct PlanBuilder {
         s.tp_off = x->w_off + (int64_t)tp_slot * x->S;
         s.ep_off = x->w_off + (int64_t)(tp_slot + x->ep_shift) * x->S;
         int64_t nu = (int64_t)R * s.row_blocks * (s.n_groups / s.groups_per_unit) * s.chunks_per_run;
-        if (nu > (1ll << 30)) return fail(MOEBIUS_E_INVAL);
+        if (nu > (1ll << 30)) return MOEBIUS_E_INVAL;
         s.n_units = (uint32_t)nu;
+        return MOEBIUS_OK;
+      };
+      // Banded chain (equal-sized objects, every move out of place): a link conflicts only with its
+      // predecessor, whose source slot it overwrites, and only half by half -- the bytes a unit writes
+      // in the first half of the slot were read by the predecessor's units of the first half of the
+      // rows (EP->TP; TP->EP mirrored).  Each link is therefore cut into 2 x 2 segments (half of the EP
+      // ranks x half of the rows, as block lists) with one counter per half: a segment waits for ONE
+      // half of the predecessor and the links overlap by a quarter, so no device-wide drain separates
+      // them (12 drains cost config 2 a tenth of its time).
+      bool band = x->chain_bands && x->n_obj == 3 && x->ep_shift == 1 && R % 2 == 0;
+      for (int o = 0; o < x->n_obj && band; ++o) {
+        Seg t;
+        if (int rc = link_seg(x->obj[o], x->obj[o].slot, t)) return fail(rc);
+        band = t.rows_total % 2 == 0 && (t.rows_total / 2) % t.rows_per_unit == 0;
+      }
+      int prev_ctr = -1; uint32_t prev_units = 0;
+      int band_ctr[2] = {-1, -1}; uint32_t band_units[2] = {0, 0};
+      for (int step = 0; step < n_links; ++step) {
+        const int k = e2t ? step : n_links - 1 - step;
+        const int layer = k / x->n_obj;
+        const WObj& ob = x->obj[k % x->n_obj];
+        const int tp_slot = 3 * layer + ob.slot;
+        Seg s;
+        if (int rc = link_seg(ob, tp_slot, s)) return fail(rc);
+        if (band) {
+          if (next_ctr + 2 > (uint32_t)kMaxCounters) return fail(MOEBIUS_E_INVAL);
+          const int ctr[2] = {(int)next_ctr, (int)next_ctr + 1};
+          next_ctr += 2;
+          uint32_t sig_units[2] = {0, 0};
+          const uint32_t half = s.rows_total / 2;
+          for (int i = 0; i < 4; ++i) {
+            const int wi = i / 2, oi = i % 2;          // ordered by the half they wait for
+            const int qh = e2t ? wi : oi, rh = e2t ? oi : wi;   // half of the EP ranks, half of the rows
+            const int sig = e2t ? rh : qh;              // as a SOURCE: EP->TP read by rows, TP->EP by TP offset (= rank half)
+            Seg t = s;
+            t.pool_begin = (uint32_t)P->wblk.size();
+            t.n_desc = (uint32_t)(R / 2);
+            for (int q = qh * (R / 2); q < (qh + 1) * (R / 2); ++q) P->wblk.push_back({(uint32_t)q, (uint32_t)rh * half, half, 0u});
+            t.pools_per_unit = ((half + t.rows_per_unit - 1) / t.rows_per_unit) * (t.n_groups / t.groups_per_unit) * t.chunks_per_run;
+            t.n_units = t.n_desc * t.pools_per_unit;
+            t.kv_mode = 0; t.pool_bytes = 0;
+            t.wait_ctr = band_ctr[wi]; t.wait_target = band_units[wi];
+            t.signal_ctr = ctr[sig];
+            sig_units[sig] += t.n_units;
+            push_seg(cw, t);
+          }
+          band_ctr[0] = ctr[0]; band_ctr[1] = ctr[1];
+          band_units[0] = sig_units[0]; band_units[1] = sig_units[1];
+          continue;
+        }
         if (ob.n_slots > x->ep_shift) {      // its EP view overlaps its own TP view: the in-place path (S2)
           if (int rc = s2_object(s, prev_ctr, prev_units)) return fail(rc);
           continue;

@@ -505,3 +505,66 @@ def test_s2_is_chosen_by_the_cap_and_refuses_only_what_cannot_fit():
         s.close()
     assert seen == {0, 1, 2}
     assert res > 0
+
+
+@pytest.mark.parametrize("first", [TP, EP])
+def test_banded_chain_overlaps_links_and_the_checker_sees_a_wrong_band(first):
+    """Equal-sized objects, every move out of place: each chain link is cut into 2 x 2 segments that wait
+    for ONE half of the predecessor (moebius_set_chain_bands).  The emulator finds the schedule hazard-free
+    -- and finds violations when the two halves a link waits for are swapped (negative control: the
+    checker does see a wrong band), or when the waits are dropped."""
+    import ctypes as C
+    from harness import emul_lib
+    cfg = SMALLISH.with_(L=3, seed=55)
+    st, sess, image, staging = make(cfg)
+    owner, bt = source_tables(st, sess, first, "random")
+    src = OracleLayout(st, sess, first, owner, bt)
+    src.place(image)
+    to = EP if first == TP else TP
+    plan = sess.plan(to, st.lens, owner, bt, from_mode=first)
+    segs = mb.moebius_plan_export(plan, 0)
+    w = segs[(segs["kind"] & 0xFF) == 0]
+    n_links = cfg.L * 3
+    assert len(w) == 4 * n_links and np.all(w["n_desc"] == cfg.R // 2)          # block lists of R/2 blocks
+    assert len(set(w["signal_ctr"].tolist())) == 2 * n_links                     # two counters per link
+    first_link, later = w[:4], w[4:]
+    assert np.all(first_link["wait_ctr"] == -1) and np.all(later["wait_ctr"] >= 0)
+    # every later segment waits for exactly one of its predecessor's two counters
+    for i in range(1, n_links):
+        prev_ctrs = set(w[4 * (i - 1):4 * i]["signal_ctr"].tolist())
+        assert set(w[4 * i:4 * i + 4]["wait_ctr"].tolist()) == prev_ctrs
+    # unbanded for comparison: one segment per link
+    sess_u = mb.Session(sess.cfg)
+    mb.moebius_set_chain_bands(sess_u.ctx, False)
+    plan_u = sess_u.plan(to, st.lens, owner, bt, from_mode=first)
+    wu = mb.moebius_plan_export(plan_u, 0)
+    assert int(((wu["kind"] & 0xFF) == 0).sum()) == n_links
+    sess_u.close()
+
+    def run(tampered):
+        img = image.copy()
+        stg = staging.copy()
+        out = np.zeros(8, np.int64)
+        vp = lambda a: a.ctypes.data_as(C.c_void_p) if a.size else None  # noqa: E731
+        kv, c2d, bulk, wblk = (mb.moebius_plan_export(plan, k) for k in (1, 2, 4, 5))
+        emul_lib().emul_run(vp(img), img.size, vp(stg), stg.size, vp(tampered), len(tampered), vp(kv), vp(c2d),
+                            sess.layout.rank_stride_bytes, vp(out), vp(bulk), vp(wblk), sess.w_staging_offset())
+        return out
+
+    assert run(segs)[0] == 0 and run(segs)[2] == 0
+    swapped = segs.copy()
+    idx = np.flatnonzero((segs["kind"] & 0xFF) == 0)
+    for i in range(1, n_links):                      # make each segment wait for the OTHER half
+        blk = idx[4 * i:4 * i + 4]
+        a, b = sorted(set(segs["wait_ctr"][blk].tolist()))
+        units = {int(c): int(t) for c, t in zip(segs["wait_ctr"][blk], segs["wait_target"][blk])}
+        for j in blk:
+            other = b if segs["wait_ctr"][j] == a else a
+            swapped["wait_ctr"][j] = other
+            swapped["wait_target"][j] = units[other]
+    assert run(swapped)[0] > 0
+    dropped = segs.copy()
+    dropped["wait_ctr"][idx] = -1
+    assert run(dropped)[0] > 0
+    sess.free_plan(plan)
+    sess.close()
