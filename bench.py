@@ -52,6 +52,7 @@ def parse():
     ap.add_argument("--n-req", type=int, default=-1, help="override the number of live requests (experiments; named in config.workload)")
     ap.add_argument("--tma", default="", help="enable,pipes,stage_kb (tuning; default: library defaults)")
     ap.add_argument("--kv-rounds", type=int, default=0, help="max dependent KV rounds before chains are cut by staging (tuning)")
+    ap.add_argument("--xt-mode", type=int, default=-1, help="weight tensor-map box side: 0 EP views, 1 TP views (tuning / A-B)")
     ap.add_argument("--no-chain-bands", action="store_true", help="a chain link waits for its whole predecessor (tuning / A-B)")
     ap.add_argument("--kv-slice", type=int, default=0, help="smallest KV slice interleaved with the weight chain, in units (tuning)")
     ap.add_argument("--w-orient", type=int, default=0, choices=[0, 1],
@@ -390,6 +391,8 @@ def run_moebius(args, env, config_name, pool_policy, cap_frac, steps, warmup, fu
         mb.moebius_set_kv_slice(sess.ctx, args.kv_slice)
     if args.no_chain_bands:
         mb.moebius_set_chain_bands(sess.ctx, False)
+    if args.xt_mode >= 0:
+        mb.moebius_set_xt_mode(sess.ctx, args.xt_mode)
     fill_device(sess, cfg, mb, torch)
     TP, EP = mb.MOEBIUS_TP, mb.MOEBIUS_EP
     n = len(lens)

@@ -26,7 +26,7 @@ EXPORTED_SYMBOLS = [
     "moebius_arena_export", "moebius_arena_import",
     "moebius_set_timing", "moebius_policy_preset", "moebius_policy_create", "moebius_policy_destroy",
     "moebius_policy_mode", "moebius_policy_step", "moebius_capacity_check", "moebius_policy_calibrate",
-    "moebius_last_kernel_ms", "moebius_kernel_ms_history", "moebius_set_launch", "moebius_set_tma", "moebius_set_kv_rounds", "moebius_set_kv_slice", "moebius_set_chain_bands", "moebius_status_str", "moebius_version",
+    "moebius_last_kernel_ms", "moebius_kernel_ms_history", "moebius_set_launch", "moebius_set_tma", "moebius_set_kv_rounds", "moebius_set_kv_slice", "moebius_set_chain_bands", "moebius_set_xt_mode", "moebius_status_str", "moebius_version",
 ]
 
 
@@ -266,7 +266,12 @@ def moebius_reshard(ctx, plan, cuda_stream: int = 0):
 
 _lib.moebius_set_kv_slice.argtypes = [_vp, C.c_int]
 _lib.moebius_set_chain_bands.argtypes = [_vp, C.c_int]
+_lib.moebius_set_xt_mode.argtypes = [_vp, C.c_int]
 _lib.moebius_reshard_shares.argtypes = [_vp, _vp, C.c_int, _vp, C.c_int, C.c_int, _vp]
+
+
+def moebius_set_xt_mode(ctx, mode: int):
+    _chk(_lib.moebius_set_xt_mode(ctx, mode), "moebius_set_xt_mode")
 
 
 def moebius_set_chain_bands(ctx, enable: bool):

@@ -161,6 +161,14 @@ __device__ __forceinline__ void tma_store_5d(const CUtensorMap* tm, int c0, int 
   asm volatile("cp.async.bulk.tensor.5d.global.shared::cta.tile.bulk_group [%0, {%1,%2,%3,%4,%5}], [%6];"
                :: "l"(tm), "r"(c0), "r"(c1), "r"(c2), "r"(c3), "r"(c4), "r"(smem_u32(src)) : "memory");
 }
+__device__ __forceinline__ void tma_load_4d(void* dst, const CUtensorMap* tm, int c0, int c1, int c2, int c3, uint64_t* bar) {
+  asm volatile("cp.async.bulk.tensor.4d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2,%3,%4,%5}], [%6];"
+               :: "r"(smem_u32(dst)), "l"(tm), "r"(c0), "r"(c1), "r"(c2), "r"(c3), "r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void tma_store_4d(const CUtensorMap* tm, int c0, int c1, int c2, int c3, const void* src) {
+  asm volatile("cp.async.bulk.tensor.4d.global.shared::cta.tile.bulk_group [%0, {%1,%2,%3,%4}], [%5];"
+               :: "l"(tm), "r"(c0), "r"(c1), "r"(c2), "r"(c3), "r"(smem_u32(src)) : "memory");
+}
 __device__ __forceinline__ void tma_load_3d(void* dst, const CUtensorMap* tm, int c0, int c1, int c2, uint64_t* bar) {
   asm volatile("cp.async.bulk.tensor.3d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2,%3,%4}], [%5];"
                :: "r"(smem_u32(dst)), "l"(tm), "r"(c0), "r"(c1), "r"(c2), "r"(smem_u32(bar)) : "memory");
@@ -184,6 +192,7 @@ struct TmaCtx {
   const CUtensorMap* tm_w;
   const CUtensorMap* tm_kv;
   const CUtensorMap* tm_stg;
+  const CUtensorMap* tm_wtp;
 };
 
 // Row coordinate (in the staging tensor map) of pool z's copy of staging slot `slot`: the staging
@@ -224,6 +233,17 @@ __device__ __forceinline__ void tma_issue_load(const TmaCtx& c, const Seg& s, ui
     if (s.groups_per_unit == s.n_groups) {          // XT
       const uint32_t q = b.q, row0 = b.row0;
       const uint32_t piece = p.xt_rows * s.run_bytes;
+      if (p.xt_mode == 1 && b.nrows == p.xt_rows) {
+        // TP-side box: the stage holds the unit in EP order [row][group][run], so the EP side is ONE
+        // contiguous bulk copy and the run transposition happens in the box over the TP views
+        // [run/4][rank][row][slot] (full units only: a ragged box would spill into the next rank's rows)
+        if (lane == 0) {
+          mbar_expect_tx(bar, piece * s.n_groups);
+          if (s.ep_is_src) bulk_g2s(stage, b.ep, piece * s.n_groups, bar);
+          else tma_load_4d(stage, c.tm_wtp, 0, 0, (int)(q * s.rows_total + row0), (int)(s.desc_begin - p.ep_shift), bar);
+        }
+        return;
+      }
       if (s.ep_is_src) {
         if (lane == 0) {
           mbar_expect_tx(bar, piece * s.n_groups);   // the box is always delivered whole (rows past the end are zero-filled)
@@ -298,6 +318,14 @@ __device__ __forceinline__ void tma_issue_store(const TmaCtx& c, const Seg& s, u
     if (s.groups_per_unit == s.n_groups) {          // XT
       const uint32_t q = b.q, row0 = b.row0;
       const uint32_t piece = p.xt_rows * s.run_bytes;
+      if (p.xt_mode == 1 && b.nrows == p.xt_rows) {
+        if (lane == 0) {
+          if (s.ep_is_src) tma_store_4d(c.tm_wtp, 0, 0, (int)(q * s.rows_total + row0), (int)(s.desc_begin - p.ep_shift), stage);
+          else bulk_s2g(b.ep, stage, piece * s.n_groups);
+        }
+        bulk_commit();
+        return;
+      }
       if (s.ep_is_src) {
         const uint32_t bytes = b.nrows * s.run_bytes;
         for (uint32_t g = lane; g < s.n_groups; g += 32)
@@ -371,7 +399,8 @@ __device__ __forceinline__ void lsu_unit(const Seg& s, const DevParams& p, uint3
 template <int kMinCtasPerSm>   // 1: plans with PATH_TMA segments (shared-memory bound); 2: ld/st-only plans
 __global__ void __launch_bounds__(256, kMinCtasPerSm)
 moebius_reshard_kernel(const __grid_constant__ DevParams p_in, const __grid_constant__ CUtensorMap tm_w,
-                       const __grid_constant__ CUtensorMap tm_kv, const __grid_constant__ CUtensorMap tm_stg) {
+                       const __grid_constant__ CUtensorMap tm_kv, const __grid_constant__ CUtensorMap tm_stg,
+                       const __grid_constant__ CUtensorMap tm_wtp) {
   extern __shared__ __align__(1024) char smem[];
   // The arguments are the same for every switch of a context (so that the launch can be replayed
   // from a captured graph); what differs per plan is read from the uploaded image's header.
@@ -413,7 +442,7 @@ moebius_reshard_kernel(const __grid_constant__ DevParams p_in, const __grid_cons
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   __syncwarp();
-  TmaCtx tc{&p, &tm_w, &tm_kv, &tm_stg};
+  TmaCtx tc{&p, &tm_w, &tm_kv, &tm_stg, &tm_wtp};
 
   // pipe state; identical in every lane (it depends on uniform values only)
   bool loading = false;           // a unit's loads are in flight
@@ -631,6 +660,7 @@ static int encode_tmaps(moebius_ctx* x) {
   memset(x->tmap_w, 0, sizeof(x->tmap_w));
   memset(x->tmap_kv, 0, sizeof(x->tmap_kv));
   memset(x->tmap_stg, 0, sizeof(x->tmap_stg));
+  memset(x->tmap_wtp, 0, sizeof(x->tmap_wtp));
   x->tmaps_valid = true;
   if (!x->use_tma || (!x->xt_ok && !x->kt_ok)) return MOEBIUS_OK;
   void* fn = nullptr;
@@ -650,6 +680,15 @@ static int encode_tmaps(moebius_ctx* x) {
     cuuint64_t strides[4] = {run * c.R, run, (cuuint64_t)x->rank_stride, (cuuint64_t)x->S};
     cuuint32_t box[5] = {(cuuint32_t)(run / 4), (cuuint32_t)x->xt_rows, (cuuint32_t)c.R, 1, 1};
     if (enc((CUtensorMap*)x->tmap_w, CU_TENSOR_MAP_DATA_TYPE_UINT32, 5, x->base + x->w_off, dims, strides, box, ones,
+            CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_NONE,
+            CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS) { x->tmaps_valid = false; return MOEBIUS_E_CUDA; }
+  }
+  if (x->xt_ok) {   // the TP views of the same slots: [run/4][rank R][row R*rows][slot], box [run/4][R][xt_rows][1]
+    const cuuint64_t run = (cuuint64_t)(c.I / c.R) * x->wb;
+    cuuint64_t dims[4] = {run / 4, (cuuint64_t)c.R, (cuuint64_t)c.E * c.H, (cuuint64_t)(3 * c.L + x->ep_shift)};
+    cuuint64_t strides[3] = {(cuuint64_t)x->rank_stride, run, (cuuint64_t)x->S};
+    cuuint32_t box[4] = {(cuuint32_t)(run / 4), (cuuint32_t)c.R, (cuuint32_t)x->xt_rows, 1};
+    if (enc((CUtensorMap*)x->tmap_wtp, CU_TENSOR_MAP_DATA_TYPE_UINT32, 4, x->base + x->w_off, dims, strides, box, ones,
             CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_NONE,
             CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS) { x->tmaps_valid = false; return MOEBIUS_E_CUDA; }
   }
@@ -833,6 +872,8 @@ int launch_reshard_kernel(moebius_ctx* x, bool tma, int64_t unit_hint, cudaStrea
   p.counters = (uint32_t*)(x->desc + kCtrOff);
   p.rank_stride = x->rank_stride;
   p.wstg_off = x->staging_bytes - x->w_stg_bytes;
+  p.xt_mode = (uint32_t)x->xt_mode;
+  p.ep_shift = (uint32_t)x->ep_shift;
   p.page_tokens = (uint32_t)x->cfg.page_tokens;
   int threads, per_sm;
   size_t smem = 0;
@@ -857,7 +898,7 @@ int launch_reshard_kernel(moebius_ctx* x, bool tma, int64_t unit_hint, cudaStrea
   if (sl) {
     // CTAs of different shares wait for one another: all of them must be resident at once, which only
     // a cooperative launch guarantees (one CTA per SM with the pipes' rings, two without)
-    void* args[4] = {(void*)&p, (void*)x->tmap_w, (void*)x->tmap_kv, (void*)x->tmap_stg};
+    void* args[5] = {(void*)&p, (void*)x->tmap_w, (void*)x->tmap_kv, (void*)x->tmap_stg, (void*)x->tmap_wtp};
     const void* fn = tma ? (const void*)moebius_reshard_kernel<1> : (const void*)moebius_reshard_kernel<2>;
     if (grid < sl->count) return MOEBIUS_E_INVAL;
     return cudaLaunchCooperativeKernel(fn, dim3((unsigned)grid), dim3((unsigned)threads), args, smem, st) == cudaSuccess
@@ -865,10 +906,10 @@ int launch_reshard_kernel(moebius_ctx* x, bool tma, int64_t unit_hint, cudaStrea
   }
   if (tma)
     moebius_reshard_kernel<1><<<(unsigned)grid, threads, smem, st>>>(p, *(const CUtensorMap*)x->tmap_w, *(const CUtensorMap*)x->tmap_kv,
-                                                                     *(const CUtensorMap*)x->tmap_stg);
+                                                                     *(const CUtensorMap*)x->tmap_stg, *(const CUtensorMap*)x->tmap_wtp);
   else
     moebius_reshard_kernel<2><<<(unsigned)grid, threads, 0, st>>>(p, *(const CUtensorMap*)x->tmap_w, *(const CUtensorMap*)x->tmap_kv,
-                                                                  *(const CUtensorMap*)x->tmap_stg);
+                                                                  *(const CUtensorMap*)x->tmap_stg, *(const CUtensorMap*)x->tmap_wtp);
   return cudaGetLastError() == cudaSuccess ? MOEBIUS_OK : MOEBIUS_E_CUDA;
 }
 

@@ -110,6 +110,8 @@ struct moebius_ctx {
   int kt_pools;                   // pools per KV unit
   alignas(64) unsigned char tmap_w[128];   // CUtensorMap storage (encoded at bind time)
   alignas(64) unsigned char tmap_kv[128];
+  alignas(64) unsigned char tmap_wtp[128];  // the TP views of the weight slots (xt_mode 1)
+  int xt_mode;
   alignas(64) unsigned char tmap_stg[128];  // the staging buffer as an array of EP-page images
   bool tmaps_valid;
   bool prepared;                  // device_prepare has run for the current buffers and stage geometry

@@ -230,6 +230,7 @@ int moebius_create(const moebius_config_t* c, moebius_ctx_t** out) {
   x->kv_max_level = 64;
   x->kv_slice_floor = 0;
   x->chain_bands = 1;
+  x->xt_mode = 0;
   x->use_tma = 1;
   x->n_pipes = 2;
   x->stage_bytes = 48 * 1024;
@@ -394,6 +395,12 @@ int moebius_set_tma(moebius_ctx_t* x, int enable, int pipes, int stage_kb) {
 int moebius_set_kv_rounds(moebius_ctx_t* x, int max_level) {
   if (!x || max_level < 0 || max_level > kMaxLevelCap) return MOEBIUS_E_INVAL;
   x->kv_max_level = max_level > 0 ? max_level : 64;
+  return MOEBIUS_OK;
+}
+
+int moebius_set_xt_mode(moebius_ctx_t* x, int mode) {
+  if (!x || mode < 0 || mode > 1) return MOEBIUS_E_INVAL;
+  x->xt_mode = mode;
   return MOEBIUS_OK;
 }
 

@@ -153,6 +153,8 @@ struct DevParams {        // decoded launch state (the kernel fills the plan-dep
   // share_bounds[s+1]).  After a wave the last CTA of a share raises that share's flag for the wave
   // (st.release.sys) in the flag page of the share's first rank; every CTA then waits for the flags of
   // ALL n_shares shares (ld.acquire.sys) -- on several GPUs those are peer addresses.
+  uint32_t         xt_mode;       // PATH_TMA weight boxes: 0 = tensor map over the EP views, 1 = over the TP views
+  uint32_t         ep_shift;      // slots between a TP view and its EP view
   uint32_t         n_shares, share_first, share_count;
   int64_t          flag_off;           // flag page offset inside a rank region: uint32 flag[wave]
   uint8_t          share_bounds[72];

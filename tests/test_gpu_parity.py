@@ -220,6 +220,27 @@ def test_tma_shapes(first, pipes, stage_kb):
     sess.close()
 
 
+@pytest.mark.parametrize("pipes,stage_kb", [(2, 48), (4, 24), (2, 16)])
+@pytest.mark.parametrize("first", [TP, EP])
+@pytest.mark.parametrize("which", ["smallish", "small", "ragged", "inplace"])
+def test_tp_side_box(which, first, pipes, stage_kb):
+    """moebius_set_xt_mode(ctx, 1): the EP side of a short-run weight unit is one contiguous bulk copy and
+    the tensor-map box covers the TP views.  Identical results; ragged last row blocks (rows per rank not a
+    multiple of the box) fall back to the EP-side box unit by unit; block lists (banded chain, in-place
+    path) use it too."""
+    cfg = {"smallish": SMALLISH, "small": wl.get_config("small").with_(L=2, n_req=20),
+           "ragged": wl.get_config("tiny").with_(R=4, E=12, H=50, I=128, kv_heads=4, n_req=6, seed=31),
+           "inplace": wl.get_config("small").with_(w_inplace=1, L=2, n_req=16)}[which]
+    st, sess = gpu_session(cfg, initial_mode=first, tma=(1, pipes, stage_kb))
+    mb.moebius_set_xt_mode(sess.ctx, 1)
+    owner, bt, _ = start(st, sess, first, "random")
+    mode, owner, bt, _ = gpu_switch(st, sess, first, owner, bt)
+    mode, owner, bt, _ = gpu_switch(st, sess, mode, owner, bt)
+    mb.moebius_set_xt_mode(sess.ctx, 0)
+    gpu_switch(st, sess, mode, owner, bt)
+    sess.close()
+
+
 @pytest.mark.parametrize("tma", [0, 1])
 def test_small_config_both_paths(tma):
     """BASELINE.json config 2 on the ld/st path and on the TMA path: identical results."""
