@@ -53,7 +53,7 @@ def parse():
     ap.add_argument("--tma", default="", help="enable,pipes,stage_kb (tuning; default: library defaults)")
     ap.add_argument("--kv-rounds", type=int, default=0, help="max dependent KV rounds before chains are cut by staging (tuning)")
     ap.add_argument("--xt-mode", type=int, default=-1, help="weight tensor-map box side: 0 EP views, 1 TP views (tuning / A-B)")
-    ap.add_argument("--no-chain-bands", action="store_true", help="a chain link waits for its whole predecessor (tuning / A-B)")
+    ap.add_argument("--chain-bands", action="store_true", help="banded weight chain: links overlap half by half (tuning / A-B; off by default)")
     ap.add_argument("--kv-slice", type=int, default=0, help="smallest KV slice interleaved with the weight chain, in units (tuning)")
     ap.add_argument("--w-orient", type=int, default=0, choices=[0, 1],
                     help="0: gate,up [E,H,I], down [E,I,H] (BASELINE.json, the headline); 1: the paper's W13 [E,2I,H], W2 [E,H,I] (named in config.workload)")
@@ -389,8 +389,8 @@ def run_moebius(args, env, config_name, pool_policy, cap_frac, steps, warmup, fu
         mb.moebius_set_kv_rounds(sess.ctx, args.kv_rounds)
     if args.kv_slice:
         mb.moebius_set_kv_slice(sess.ctx, args.kv_slice)
-    if args.no_chain_bands:
-        mb.moebius_set_chain_bands(sess.ctx, False)
+    if args.chain_bands:
+        mb.moebius_set_chain_bands(sess.ctx, True)
     if args.xt_mode >= 0:
         mb.moebius_set_xt_mode(sess.ctx, args.xt_mode)
     fill_device(sess, cfg, mb, torch)

@@ -333,13 +333,14 @@ MOEBIUS_API int moebius_set_tma(moebius_ctx_t* ctx, int enable, int pipes, int s
 MOEBIUS_API int moebius_set_kv_rounds(moebius_ctx_t* ctx, int max_level);
 /* KV work is cut into slices that the merged work list interleaves with the weight chain, one per chain
  * link where there is enough of it, so that the drain of a link hides behind independent KV units.
- * min_units: the smallest slice (tuning; 0 = the default, 1024 units).  Results are identical. */
+ * min_units: the smallest slice (tuning; 0 = the default, 8192 units).  Results are identical. */
 MOEBIUS_API int moebius_set_kv_slice(moebius_ctx_t* ctx, int min_units);
-/* Weight chain (tuning; before moebius_plan).  enable != 0 (the default): when all objects have the same
- * size and every move is out of place, a link is cut into 2 x 2 segments (half of the EP ranks x half of
- * the rows) that wait for ONE half of the predecessor, so consecutive links overlap instead of being
- * separated by a device-wide drain (PAPER.md:156 fixes the order, not the grain).  enable == 0: a link
- * waits for the whole predecessor.  Results are identical. */
+/* Weight chain (tuning; before moebius_plan).  enable != 0: when all objects have the same size and every
+ * move is out of place, a link is cut into 2 x 2 segments (half of the EP ranks x half of the rows) that
+ * wait for ONE half of the predecessor, so consecutive links overlap instead of being separated by a
+ * device-wide drain (PAPER.md:156 fixes the order, not the grain).  enable == 0 (the default: the banded
+ * order measured slower on B200 than the drains it removes): a link waits for the whole predecessor.
+ * Results are identical. */
 MOEBIUS_API int moebius_set_chain_bands(moebius_ctx_t* ctx, int enable);
 /* Which side of a short-run weight unit (gate, up, W2) goes through the tensor-map box (tuning; any time).
  * 0: the box covers the EP rows [run][row][group] and lands group-major, the TP side is R contiguous

@@ -450,16 +450,19 @@ moebius_reshard_kernel(const __grid_constant__ DevParams p_in, const __grid_cons
   KvDesc ld_d = {0, 0, 0, 0};
   uint32_t phase0 = 0, phase1 = 0;
   uint32_t next_stage = 0;
-  // completion signals are batched: units whose store groups are committed but not yet signalled all
-  // belong to counter pend_ctr; one fence + one atomicAdd publishes them when the counter changes or
-  // the pipe drains (a per-unit fence + atomic costs a third of the pipe's time)
-  int32_t pend_ctr = -1;
-  uint32_t pend_n = 0;
+  // Completion signals are batched: units whose store groups are committed but not yet signalled all
+  // belong to counter pend_ctr; one fence + one atomicAdd publishes them (a per-unit fence + atomic costs
+  // a third of the pipe's time).  When the counter changes -- every segment boundary of a banded chain --
+  // the batch is not published at once, which would mean waiting for its last store group: it is put
+  // aside (old_*) and published two units later, when a wait for "all but the two youngest groups"
+  // returns at once.  A drain publishes everything.
+  int32_t pend_ctr = -1, old_ctr = -1;
+  uint32_t pend_n = 0, old_n = 0, old_age = 0;
 
-  auto publish = [&]() {                // after every lane's pending writes have completed
+  auto publish = [&](int32_t ctr, uint32_t n) {   // after every lane's writes of those units have completed
     fence_proxy_async();
     __syncwarp();
-    if (lane == 0 && pend_ctr >= 0 && pend_n) { __threadfence(); atomicAdd(p.counters + pend_ctr, pend_n); }
+    if (lane == 0 && ctr >= 0 && n) { __threadfence(); atomicAdd(p.counters + ctr, n); }
   };
   auto retire = [&]() {                  // loads landed -> issue the stores of the loading unit
     if (!loading) return;
@@ -468,16 +471,28 @@ moebius_reshard_kernel(const __grid_constant__ DevParams p_in, const __grid_cons
     if (lane == 0) mbar_wait(bar + ld_stage, ld_stage ? phase1 : phase0);
     __syncwarp();
     tma_issue_store(tc, s, ld_ul, ld_d, ring + (size_t)ld_stage * p.stage_bytes, lane);
-    if (ctr != pend_ctr && pend_ctr >= 0 && pend_n) { bulk_wait<1>(); publish(); }   // all but the group just committed
     if (ld_stage) phase1 ^= 1; else phase0 ^= 1;
-    if (ctr != pend_ctr) { pend_ctr = ctr; pend_n = 0; }
+    if (old_n && ++old_age >= 2) {       // the batch put aside is two groups old: complete, or nearly
+      bulk_wait<2>();
+      publish(old_ctr, old_n);
+      old_n = 0;
+    }
+    if (ctr != pend_ctr) {
+      if (pend_ctr >= 0 && pend_n) {
+        if (old_n) { bulk_wait<1>(); publish(old_ctr, old_n); }   // all but the group just committed
+        old_ctr = pend_ctr; old_n = pend_n; old_age = 0;
+      }
+      pend_ctr = ctr; pend_n = 0;
+    }
     ++pend_n;
     loading = false;
   };
   auto drain = [&]() {                   // everything this pipe has in flight completes and is signalled
     retire();
     bulk_wait<0>();
-    publish();
+    publish(old_ctr, old_n);
+    publish(pend_ctr, pend_n);
+    old_n = 0;
     pend_n = 0;
     __syncwarp();
   };

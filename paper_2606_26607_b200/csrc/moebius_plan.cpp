@@ -229,7 +229,7 @@ int moebius_create(const moebius_config_t* c, moebius_ctx_t** out) {
   x->unit_kb = 0;
   x->kv_max_level = 64;
   x->kv_slice_floor = 0;
-  x->chain_bands = 1;
+  x->chain_bands = 0;
   x->xt_mode = 0;
   x->use_tma = 1;
   x->n_pipes = 2;
@@ -913,6 +913,7 @@ struct PlanBuilder {
         if (!copy) {
           t = (kind == OP_MOVE) ? tmpl : (xt && seg_path(tmpl) == PATH_TMA ? lsu : tmpl);
           t.kv_mode = kind == OP_MOVE ? 0u : 1u;             // 1: the EP side of every block is its staging slot
+          t.stg_pools = 0;                                    // an irregular list: WBlk descriptors
           t.pool_begin = (uint32_t)P->wblk.size();
           t.n_desc = (uint32_t)blks.size();
           t.pool_bytes = slot_bytes;
@@ -1015,7 +1016,10 @@ struct PlanBuilder {
       // rows (EP->TP; TP->EP mirrored).  Each link is therefore cut into 2 x 2 segments (half of the EP
       // ranks x half of the rows, as block lists) with one counter per half: a segment waits for ONE
       // half of the predecessor and the links overlap by a quarter, so no device-wide drain separates
-      // them (12 drains cost config 2 a tenth of its time).
+      // them.  OFF by default (moebius_set_chain_bands): measured on B200 it removes every stall (0 pipes
+      // ever wait, against 296 per link) and is still 9-13 % SLOWER at the 30B shape (weight-only switch
+      // 2.57 ms vs 2.30 ms at L = 6) -- the quarter-object order itself costs more than the drains it
+      // saves, even with the waits switched off (2.50 ms); DESIGN.md section 3.
       bool band = x->chain_bands && x->n_obj == 3 && x->ep_shift == 1 && R % 2 == 0;
       for (int o = 0; o < x->n_obj && band; ++o) {
         Seg t;
@@ -1042,9 +1046,9 @@ struct PlanBuilder {
             const int qh = e2t ? wi : oi, rh = e2t ? oi : wi;   // half of the EP ranks, half of the rows
             const int sig = e2t ? rh : qh;              // as a SOURCE: EP->TP read by rows, TP->EP by TP offset (= rank half)
             Seg t = s;
-            t.pool_begin = (uint32_t)P->wblk.size();
-            t.n_desc = (uint32_t)(R / 2);
-            for (int q = qh * (R / 2); q < (qh + 1) * (R / 2); ++q) P->wblk.push_back({(uint32_t)q, (uint32_t)rh * half, half, 0u});
+            t.n_desc = (uint32_t)(R / 2);                 // a regular block list: rows [rh*half, +half) of ranks qh*R/2 ...
+            t.stg_pools = 1; t.stg_pool_begin = (uint32_t)(qh * (R / 2));
+            t.pool_begin = (uint32_t)rh * half; t.n_pools = half;
             t.pools_per_unit = ((half + t.rows_per_unit - 1) / t.rows_per_unit) * (t.n_groups / t.groups_per_unit) * t.chunks_per_run;
             t.n_units = t.n_desc * t.pools_per_unit;
             t.kv_mode = 0; t.pool_bytes = 0;
@@ -1225,11 +1229,11 @@ struct PlanBuilder {
       };
       // a round = every segment that signals the same counter; the next round waits for all of them
       const int64_t kv_units_est = (int64_t)nm * ((n_pools_all + ppu - 1) / ppu);
-      // one KV slice per chain link (and one to spare), so that every link is followed by independent
-      // work: the pipes that finish link k take KV units while its last units drain, and link k+1 finds
-      // its dependency satisfied.  Not below a few times the units in flight on the device.
-      const int64_t slice_floor = x->kv_slice_floor > 0 ? x->kv_slice_floor : 1024;
-      const int64_t slice_units = std::max<int64_t>(slice_floor, kv_units_est / std::max(1, L * x->n_obj + 1));
+      // KV work is cut into slices that the merge interleaves with the weight chain, so that a link's
+      // drain hides behind independent KV units.  (One slice per link, floor 1024, was measured: no gain
+      // at the 235B shape, -1 % at the 30B shape; moebius_set_kv_slice sets the floor.)
+      const int64_t slice_floor = x->kv_slice_floor > 0 ? x->kv_slice_floor : 8192;
+      const int64_t slice_units = std::max<int64_t>(slice_floor, kv_units_est / std::max(1, 3 * L));
       int prev_ctr = -1; uint32_t prev_total = 0;
       for (int g = 0; g < n_pool_groups; ++g) {
         int pool0 = g * pools_per_group;

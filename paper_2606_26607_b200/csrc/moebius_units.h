@@ -97,7 +97,9 @@ static_assert(sizeof(C2dDesc) == 32, "C2dDesc must be 32 bytes");
 // rows [row0, row0 + nrows) of EP rank q; `slot` is its staging slot when the segment's EP side is the
 // staging buffer (Seg::kv_mode & 1).  Fields reused by such a segment: n_desc = number of blocks (0 = the
 // whole object, the common case), pool_begin = first WBlk, pools_per_unit = units per block, pool_bytes =
-// bytes of one staging slot.
+// bytes of one staging slot.  REGULAR block lists (the banded chain: the same rows of consecutive ranks)
+// carry no descriptors at all -- a dependent global load per unit costs the issuing pipe a tenth of its
+// rate: stg_pools = 1 marks them, block i is rows [pool_begin, pool_begin + n_pools) of rank stg_pool_begin + i.
 struct WBlk {
   uint32_t q, row0, nrows, slot;
 };
@@ -207,7 +209,7 @@ MB_HD uint32_t tp_src_rank(uint32_t g, uint32_t rep, int32_t owner) {
 // that owns this rank.
 MB_HD uint32_t unit_ep_rank(const Seg& s, const DevParams& p, uint32_t u) {
   if (seg_kind(s) == SEG_XPOSE) {
-    if (s.n_desc) return p.wblk[s.pool_begin + u / s.pools_per_unit].q;
+    if (s.n_desc) return s.stg_pools ? s.stg_pool_begin + u / s.pools_per_unit : p.wblk[s.pool_begin + u / s.pools_per_unit].q;
     u /= s.chunks_per_run;
     u /= s.n_groups / s.groups_per_unit;
     return u / s.row_blocks;
@@ -264,8 +266,12 @@ MB_HD void decode_box(const Seg& s, const DevParams& p, uint32_t u, uint32_t k, 
     if (s.n_desc) {                       // block-list mode: unit = (block, row block, group block, chunk)
       const uint32_t di = u / s.pools_per_unit;
       u -= di * s.pools_per_unit;
-      const WBlk k = p.wblk[s.pool_begin + di];
-      q = k.q; blk_row0 = k.row0; row_end = k.row0 + k.nrows; slot = k.slot;
+      if (s.stg_pools) {                  // regular: computed, no descriptor
+        q = s.stg_pool_begin + di; blk_row0 = s.pool_begin; row_end = s.pool_begin + s.n_pools;
+      } else {
+        const WBlk k = p.wblk[s.pool_begin + di];
+        q = k.q; blk_row0 = k.row0; row_end = k.row0 + k.nrows; slot = k.slot;
+      }
     } else {
       q = u / (s.row_blocks * jgroups * s.chunks_per_run);
       u -= q * (s.row_blocks * jgroups * s.chunks_per_run);

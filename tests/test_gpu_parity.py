@@ -673,3 +673,21 @@ def test_device_side_round_barrier_argument_checks():
         mb.moebius_reshard_shares(sess.ctx, plan, [0, 2, 4], 1, 2, 0)     # shares 1..2 of 2
     assert mb.moebius_active_mode(sess.ctx) == TP
     sess.close()
+
+
+@pytest.mark.parametrize("which", ["smallish", "small", "fp8"])
+@pytest.mark.parametrize("first", [TP, EP])
+def test_banded_chain_on_device(which, first):
+    """moebius_set_chain_bands(ctx, 1): links cut into 2 x 2 segments that wait for one half of their
+    predecessor (no device-wide drain between links).  Off by default -- measured slower -- but kept
+    correct: bit-exact with the oracle, both directions."""
+    cfg = {"smallish": SMALLISH, "small": wl.get_config("small"),
+           "fp8": wl.get_config("fp8_graph").with_(L=2, E=16, H=256, I=1536, n_req=6, len_dist=("uniform", 1, 60), seed=3)}[which]
+    st, sess = gpu_session(cfg, fill="normal" if cfg.w_dtype == "fp8_e4m3_b128" else "tag", initial_mode=first)
+    mb.moebius_set_chain_bands(sess.ctx, True)
+    owner, bt, _ = start(st, sess, first, "random")
+    mode = first
+    for _ in range(3):
+        mode, owner, bt, stats = gpu_switch(st, sess, mode, owner, bt)
+    assert stats["n_segments"] >= 4 * 3 * cfg.L
+    sess.close()

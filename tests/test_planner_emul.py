@@ -517,6 +517,7 @@ def test_banded_chain_overlaps_links_and_the_checker_sees_a_wrong_band(first):
     from harness import emul_lib
     cfg = SMALLISH.with_(L=3, seed=55)
     st, sess, image, staging = make(cfg)
+    mb.moebius_set_chain_bands(sess.ctx, True)
     owner, bt = source_tables(st, sess, first, "random")
     src = OracleLayout(st, sess, first, owner, bt)
     src.place(image)
@@ -525,7 +526,8 @@ def test_banded_chain_overlaps_links_and_the_checker_sees_a_wrong_band(first):
     segs = mb.moebius_plan_export(plan, 0)
     w = segs[(segs["kind"] & 0xFF) == 0]
     n_links = cfg.L * 3
-    assert len(w) == 4 * n_links and np.all(w["n_desc"] == cfg.R // 2)          # block lists of R/2 blocks
+    assert len(w) == 4 * n_links and np.all(w["n_desc"] == cfg.R // 2)          # (regular) block lists of R/2 blocks
+    assert np.all(w["stg_pools"] == 1) and len(mb.moebius_plan_export(plan, 5)) == 0   # no descriptors
     assert len(set(w["signal_ctr"].tolist())) == 2 * n_links                     # two counters per link
     first_link, later = w[:4], w[4:]
     assert np.all(first_link["wait_ctr"] == -1) and np.all(later["wait_ctr"] >= 0)
@@ -534,8 +536,7 @@ def test_banded_chain_overlaps_links_and_the_checker_sees_a_wrong_band(first):
         prev_ctrs = set(w[4 * (i - 1):4 * i]["signal_ctr"].tolist())
         assert set(w[4 * i:4 * i + 4]["wait_ctr"].tolist()) == prev_ctrs
     # unbanded for comparison: one segment per link
-    sess_u = mb.Session(sess.cfg)
-    mb.moebius_set_chain_bands(sess_u.ctx, False)
+    sess_u = mb.Session(sess.cfg)          # the default: unbanded
     plan_u = sess_u.plan(to, st.lens, owner, bt, from_mode=first)
     wu = mb.moebius_plan_export(plan_u, 0)
     assert int(((wu["kind"] & 0xFF) == 0).sum()) == n_links

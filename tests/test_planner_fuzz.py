@@ -56,6 +56,8 @@ def test_fuzz_round_trip(seed):
         return
     if rounds:
         mb.moebius_set_kv_rounds(sess.ctx, rounds)
+    if seed % 3 == 0:
+        mb.moebius_set_chain_bands(sess.ctx, True)      # the banded weight chain (off by default)
     image = np.full(sess.layout.base_bytes, 0xA5, np.uint8)
     staging = np.full(max(sess.layout.staging_bytes, 16), 0x5A, np.uint8)
     mode = first
