@@ -343,9 +343,11 @@ MOEBIUS_API int moebius_set_kv_slice(moebius_ctx_t* ctx, int min_units);
  * Results are identical. */
 MOEBIUS_API int moebius_set_chain_bands(moebius_ctx_t* ctx, int enable);
 /* Which side of a short-run weight unit (gate, up, W2) goes through the tensor-map box (tuning; any time).
- * 0: the box covers the EP rows [run][row][group] and lands group-major, the TP side is R contiguous
- * bulk copies.  1: the EP side is ONE contiguous bulk copy and the box covers the TP views
- * [run][rank][row], landing in EP order (full units only; ragged ones use mode 0).  Results are identical. */
+ * 1 (the default; measured 2-4 % faster EP->TP, 0.3 % TP->EP on B200): the EP side is ONE contiguous bulk
+ * copy and the box covers the TP views [run][rank][row], landing in EP order (full units only; ragged
+ * ones use mode 0).  0: the box covers the EP rows [run][row][group] and lands group-major, the TP side is
+ * R contiguous bulk copies.  Bits 4-5 (tuning): L2 promotion of the TP-side map, 0 none / 1, 2, 3 = 64,
+ * 128, 256 bytes.  Results are identical. */
 MOEBIUS_API int moebius_set_xt_mode(moebius_ctx_t* ctx, int mode);
 
 /* Launch shape override for the ld/st path (tuning): values <= 0 restore the defaults; threads is a

@@ -703,8 +703,10 @@ static int encode_tmaps(moebius_ctx* x) {
     cuuint64_t dims[4] = {run / 4, (cuuint64_t)c.R, (cuuint64_t)c.E * c.H, (cuuint64_t)(3 * c.L + x->ep_shift)};
     cuuint64_t strides[3] = {(cuuint64_t)x->rank_stride, run, (cuuint64_t)x->S};
     cuuint32_t box[4] = {(cuuint32_t)(run / 4), (cuuint32_t)c.R, (cuuint32_t)x->xt_rows, 1};
+    const CUtensorMapL2promotion promo = x->xt_promo == 1 ? CU_TENSOR_MAP_L2_PROMOTION_L2_64B : x->xt_promo == 2 ? CU_TENSOR_MAP_L2_PROMOTION_L2_128B
+                                        : x->xt_promo == 3 ? CU_TENSOR_MAP_L2_PROMOTION_L2_256B : CU_TENSOR_MAP_L2_PROMOTION_NONE;
     if (enc((CUtensorMap*)x->tmap_wtp, CU_TENSOR_MAP_DATA_TYPE_UINT32, 4, x->base + x->w_off, dims, strides, box, ones,
-            CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_NONE,
+            CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, promo,
             CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS) { x->tmaps_valid = false; return MOEBIUS_E_CUDA; }
   }
   if (x->kt_ok) {

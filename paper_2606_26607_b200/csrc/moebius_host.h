@@ -111,7 +111,8 @@ struct moebius_ctx {
   alignas(64) unsigned char tmap_w[128];   // CUtensorMap storage (encoded at bind time)
   alignas(64) unsigned char tmap_kv[128];
   alignas(64) unsigned char tmap_wtp[128];  // the TP views of the weight slots (xt_mode 1)
-  int xt_mode;
+  int xt_mode;                    // 1 (default): weight boxes over the TP views; 0: over the EP views
+  int xt_promo;                   // L2 promotion of that tensor map (0 none, 1/2/3 = 64/128/256 B; tuning)
   alignas(64) unsigned char tmap_stg[128];  // the staging buffer as an array of EP-page images
   bool tmaps_valid;
   bool prepared;                  // device_prepare has run for the current buffers and stage geometry

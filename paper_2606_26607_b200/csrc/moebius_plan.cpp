@@ -230,7 +230,8 @@ int moebius_create(const moebius_config_t* c, moebius_ctx_t** out) {
   x->kv_max_level = 64;
   x->kv_slice_floor = 0;
   x->chain_bands = 0;
-  x->xt_mode = 0;
+  x->xt_mode = 1;
+  x->xt_promo = 0;
   x->use_tma = 1;
   x->n_pipes = 2;
   x->stage_bytes = 48 * 1024;
@@ -399,8 +400,11 @@ int moebius_set_kv_rounds(moebius_ctx_t* x, int max_level) {
 }
 
 int moebius_set_xt_mode(moebius_ctx_t* x, int mode) {
-  if (!x || mode < 0 || mode > 1) return MOEBIUS_E_INVAL;
-  x->xt_mode = mode;
+  if (!x || mode < 0 || (mode & 15) > 1 || (mode >> 4) > 3) return MOEBIUS_E_INVAL;
+  const bool re_encode = (mode >> 4) != x->xt_promo;
+  x->xt_mode = mode & 15;
+  x->xt_promo = mode >> 4;
+  if (re_encode) { x->tmaps_valid = false; return device_prepare(x); }
   return MOEBIUS_OK;
 }
 
