@@ -349,7 +349,7 @@ def init_device():
     return world, rank, local, dev
 
 
-def run_moebius(args, env, config_name, pool_policy, cap_frac, steps, warmup, full=True):
+def run_moebius(args, env, config_name, pool_policy, cap_frac, steps, warmup, full=True, overrides=None):
     """Times one workload.  full=False (the other_configs entries): kernel times only -- no D2D
     comparison copy, no e2e loop."""
     import torch
@@ -359,9 +359,11 @@ def run_moebius(args, env, config_name, pool_policy, cap_frac, steps, warmup, fu
 
     world, rank, local, dev = env
     cfg = wl.get_config(config_name)
+    if overrides:
+        cfg = cfg.with_(name="%s[%s]" % (cfg.name, ",".join("%s=%s" % kv for kv in sorted(overrides.items()))), **overrides)
     if args.layers:
         cfg = cfg.with_(L=args.layers, name="%s[L=%d]" % (cfg.name, args.layers))
-    if args.w_orient:
+    if args.w_orient and not overrides:
         cfg = cfg.with_(w_orient=1, name="%s[w_orient=1]" % cfg.name)
     lens = wl.draw_seq_lens(cfg)
     pool = wl.kv_pool_bytes(cfg, lens, pool_policy)
@@ -582,8 +584,12 @@ def split_history(hist):
 
 # The parity-test configs of BASELINE.json and the cache-nearly-full variant of config 4, timed after the
 # headline workload in the default run so that the driver's record carries them too.
-OTHER_CONFIGS = (("qwen3_30b", "qwen3_30b", "roomy", 0.024), ("fp8_graph", "fp8_graph", "roomy", 0.024),
-                 ("small", "small", "roomy", 0.024), ("qwen3_235b_tight_pool", "qwen3_235b", "tight", 0.05))
+OTHER_CONFIGS = (("qwen3_30b", "qwen3_30b", "roomy", 0.024, None), ("fp8_graph", "fp8_graph", "roomy", 0.024, None),
+                 ("small", "small", "roomy", 0.024, None), ("qwen3_235b_tight_pool", "qwen3_235b", "tight", 0.024, None),
+                 # the paper's own orientation: config 4 inside the cap with two spare slots; config 5
+                 # only with one, so its W13 objects take the in-place path (S2: dependency waves, parked blocks)
+                 ("qwen3_235b_paper_orient", "qwen3_235b", "roomy", 0.024, {"w_orient": 1}),
+                 ("fp8_graph_paper_orient_in_place", "fp8_graph", "roomy", 0.024, {"w_orient": 1}))
 
 
 def other_config_entry(r, peak):
@@ -598,6 +604,8 @@ def other_config_entry(r, peak):
             "frac_traffic_vs_measured": [a["frac_traffic_vs_measured"], b["frac_traffic_vs_measured"]],
             "kv_rounds": [a["kv_rounds"], b["kv_rounds"]], "kv_staged": [a["kv_staged"], b["kv_staged"]],
             "first_switch_from_random_tables": r["first_ms"],
+            "w_shift_slots": lay.w_shift_slots, "w_waves": [r["st_t2e"]["n_w_waves"], r["st_e2t"]["n_w_waves"]],
+            "w_parked_blocks": [r["st_t2e"]["n_w_parked"], r["st_e2t"]["n_w_parked"]],
             "resident_GB": lay.resident_bytes / 1e9,
             "spare_plus_staging_frac": (lay.weight_spare_bytes + lay.staging_bytes) / lay.resident_bytes,
             "staging_cap_frac": r["cap_frac"], "ms_per_step": r["dev_ms"] / r["steps"], "clocks": r["clocks"]}
@@ -677,9 +685,9 @@ def main():
             and not args.layers and args.n_req < 0 and not args.w_orient:
         torch.cuda.empty_cache()
         others = {}
-        for key, name, pool_policy, cap in OTHER_CONFIGS:
+        for key, name, pool_policy, cap, over in OTHER_CONFIGS:
             try:
-                ro = run_moebius(args, env, name, pool_policy, cap, min(steps, 10), 3, full=False)
+                ro = run_moebius(args, env, name, pool_policy, cap, min(steps, 10), 3, full=False, overrides=over)
                 others[key] = other_config_entry(ro, peak)
                 line["gpu_launches"] += 2 * ro["steps"]
                 del ro

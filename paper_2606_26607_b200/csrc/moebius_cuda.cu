@@ -782,7 +782,7 @@ int device_prepare(moebius_ctx* x) {
     x->ev_valid = true;
   }
   if (int rc = encode_tmaps(x)) return rc;
-  const bool tma = x->use_tma && (x->xt_ok || x->kt_ok);
+  const bool tma = x->use_tma != 0;   // bulk copies (long runs, attention shards, parked blocks) need the pipes' rings too
   if (tma) {
     const size_t smem = 1024 + (size_t)x->n_pipes * 2 * (size_t)x->stage_bytes;
     if (cudaFuncSetAttribute(moebius_reshard_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) {
@@ -997,7 +997,7 @@ extern "C" int moebius_reshard_staged(moebius_ctx_t* x, void* cuda_stream) {
   if (cudaMemsetAsync(x->desc, 0, (size_t)kSegOff, st) != cudaSuccess) return MOEBIUS_E_CUDA;
   if (cudaMemcpyAsync(x->desc + kSegOff, x->mailbox, (size_t)img_cap, cudaMemcpyHostToDevice, st) != cudaSuccess)
     return MOEBIUS_E_CUDA;
-  const bool tma = x->use_tma && (x->xt_ok || x->kt_ok);
+  const bool tma = x->use_tma != 0;   // bulk copies (long runs, attention shards, parked blocks) need the pipes' rings too
   if (int rc = launch_reshard_kernel(x, tma, 0, st)) return rc;
   if (cudaMemcpyAsync(x->tables, x->mailbox + img_cap, (size_t)x->table_bytes, cudaMemcpyHostToDevice, st) != cudaSuccess)
     return MOEBIUS_E_CUDA;

@@ -168,3 +168,46 @@ def test_switch_itself_inside_a_captured_graph():
     assert first_stats["n_kv_rounds"] > 1         # the first plan really needed rounds
     assert len(seen) >= 2                          # the replays executed plans of different size
     sess.close()
+
+
+def test_graph_replay_with_aliased_views():
+    """The fixed-address proof with the in-place weight path (w_inplace = 1: the EP and the TP view of an
+    object alias the same bytes): the reader graphs captured once replay correctly
+    after every switch."""
+    cfg = wl.get_config("small").with_(L=2, H=128, I=256, n_req=12, len_dist=("uniform", 1, 150), seed=25, w_inplace=1)
+    run_graph_stress(cfg, 4)
+
+
+def test_captured_switch_with_in_place_waves():
+    """moebius_reshard_staged inside a captured graph, replayed for plans of the in-place path (dozens of
+    dependency waves, parked blocks): everything plan-dependent is read from the uploaded image."""
+    cfg = wl.get_config("small").with_(L=2, H=128, I=256, n_req=20, len_dist=("uniform", 1, 200), seed=27, w_inplace=1)
+    st = State(cfg, fill="tag")
+    sess = mb.Session(mb_config(cfg, st.lens), device="cuda:0", initial_mode=TP)
+    n = len(st.lens)
+    readers = {m: ModeGraph(sess, cfg, m, n, False) for m in (TP, EP)}
+    owner, bt = source_tables(st, sess, TP, "random")
+    image = np.full(sess.layout.base_bytes, 0xA5, np.uint8)
+    OracleLayout(st, sess, TP, owner, bt).place(image)
+    sess.base[:image.size].copy_(torch.from_numpy(image))
+    mode = TP
+    plan = sess.plan(EP, st.lens, owner, bt, from_mode=mode)
+    assert mb.moebius_plan_stats(plan).as_dict()["n_w_waves"] > 0
+    sess.stage(plan)
+    switch_graph = torch.cuda.CUDAGraph()
+    torch.cuda.synchronize()
+    with torch.cuda.graph(switch_graph):
+        sess.reshard_staged(torch.cuda.current_stream())
+    for k in range(4):
+        to = EP if mode == TP else TP
+        if k > 0:
+            plan = sess.plan(to, st.lens, owner, bt, from_mode=mode)
+            sess.stage(plan)
+        switch_graph.replay()
+        readers[to].replay()
+        want_owner, want_bt = expected_target(st, sess, to)
+        readers[to].check(st, want_owner, want_bt)
+        torch.cuda.synchronize()
+        sess.free_plan(plan)
+        owner, bt, mode = (want_owner if to == EP else None), want_bt, to
+    sess.close()
