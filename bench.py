@@ -51,6 +51,7 @@ def parse():
                     help="cap on spare slot + staging as a fraction of resident bytes (0 = library default)")
     ap.add_argument("--n-req", type=int, default=-1, help="override the number of live requests (experiments; named in config.workload)")
     ap.add_argument("--tma", default="", help="enable,pipes,stage_kb (tuning; default: library defaults)")
+    ap.add_argument("--ring", default="", help="ring_kb,max_loads of the pipes' rings (tuning; after --tma)")
     ap.add_argument("--kv-rounds", type=int, default=0, help="max dependent KV rounds before chains are cut by staging (tuning)")
     ap.add_argument("--xt-mode", type=int, default=-1, help="weight tensor-map box side: 0 EP views, 1 TP views (tuning / A-B)")
     ap.add_argument("--chain-bands", action="store_true", help="banded weight chain: links overlap half by half (tuning / A-B; off by default)")
@@ -387,6 +388,9 @@ def run_moebius(args, env, config_name, pool_policy, cap_frac, steps, warmup, fu
     if args.tma:
         a, b, u = (int(x) for x in args.tma.split(","))
         mb.moebius_set_tma(sess.ctx, a, b, u)
+    if args.ring:
+        a, b = (int(x) for x in args.ring.split(","))
+        mb.moebius_set_ring(sess.ctx, a, b)
     if args.kv_rounds:
         mb.moebius_set_kv_rounds(sess.ctx, args.kv_rounds)
     if args.kv_slice:

@@ -318,11 +318,20 @@ MOEBIUS_API int moebius_kernel_ms_history(moebius_ctx_t* ctx, float* out_ms, int
 
 /* Data-path selection, before the first moebius_plan of a context.  enable != 0 (the default):
  * segments whose shapes allow it run on the TMA path (tensor-map loads/stores through shared memory,
- * `pipes` warps per SM with two `stage_kb` KB stages each; 0 = the context's defaults: the stage is a whole
- * number of EP pages near 48 KB and the pipes fill 208 KB -- 2 and 48 at 16-KB pages).  enable == 0:
+ * `pipes` warps per SM, each with a ring of two `stage_kb` KB stages; 0 = the context's defaults: the stage
+ * is a whole number of EP pages near 48 KB and the pipes fill 208 KB -- 2 and 48 at 16-KB pages).  enable == 0:
  * everything runs on the ld.global/st.global path.  Results are identical either way.  A plan built
  * before the call cannot be executed after it (MOEBIUS_E_STATE).  2*pipes*stage_kb <= 208. */
 MOEBIUS_API int moebius_set_tma(moebius_ctx_t* ctx, int enable, int pipes, int stage_kb);
+/* The pipes' shared-memory rings (tuning; after moebius_set_tma, which resets the ring to two stages).
+ * A TMA unit takes exactly the bytes it needs from its pipe's ring, first in first out, so units smaller
+ * than a stage pack the ring deeper.  ring_kb: bytes of one pipe's ring in KB, >= stage_kb,
+ * pipes * ring_kb <= 208; 0 = two stages.  max_loads: units of one pipe whose loads may be in flight at
+ * once (1..7; 0 = the default 2: a store's shared-memory read completes long before a load lands, so two
+ * loads in flight per pipe and a store that is waited for at once keep more bytes in flight than one load
+ * behind two draining stores -- measured 1.4-2.3 % faster on B200 at the BASELINE shapes).
+ * Results are identical.  PAPER.md:172 fixes what a slice move reads and writes, not how it is staged. */
+MOEBIUS_API int moebius_set_ring(moebius_ctx_t* ctx, int ring_kb, int max_loads);
 
 /* KV schedule (tuning; before moebius_plan).  When target pages overlap live source pages the page
  * moves form dependency chains; the planner runs them in at most `max_level` + 2 device-wide rounds

@@ -26,7 +26,7 @@ EXPORTED_SYMBOLS = [
     "moebius_arena_export", "moebius_arena_import",
     "moebius_set_timing", "moebius_policy_preset", "moebius_policy_create", "moebius_policy_destroy",
     "moebius_policy_mode", "moebius_policy_step", "moebius_capacity_check", "moebius_policy_calibrate",
-    "moebius_last_kernel_ms", "moebius_kernel_ms_history", "moebius_set_launch", "moebius_set_tma", "moebius_set_kv_rounds", "moebius_set_kv_slice", "moebius_set_chain_bands", "moebius_set_xt_mode", "moebius_status_str", "moebius_version",
+    "moebius_last_kernel_ms", "moebius_kernel_ms_history", "moebius_set_launch", "moebius_set_tma", "moebius_set_ring", "moebius_set_kv_rounds", "moebius_set_kv_slice", "moebius_set_chain_bands", "moebius_set_xt_mode", "moebius_status_str", "moebius_version",
 ]
 
 
@@ -155,6 +155,7 @@ _lib.moebius_last_kernel_ms.argtypes = [_vp, C.POINTER(C.c_float)]
 _lib.moebius_kernel_ms_history.argtypes = [_vp, C.POINTER(C.c_float), C.c_int, C.POINTER(C.c_int)]
 _lib.moebius_set_launch.argtypes = [_vp, C.c_int, C.c_int, C.c_int]
 _lib.moebius_set_tma.argtypes = [_vp, C.c_int, C.c_int, C.c_int]
+_lib.moebius_set_ring.argtypes = [_vp, C.c_int, C.c_int]
 _lib.moebius_set_kv_rounds.argtypes = [_vp, C.c_int]
 _lib.moebius_status_str.argtypes = [C.c_int]
 _lib.moebius_status_str.restype = C.c_char_p
@@ -444,6 +445,10 @@ def moebius_set_launch(ctx, ctas_per_sm: int = 0, threads: int = 0, unit_kb: int
 
 def moebius_set_tma(ctx, enable: bool = True, pipes: int = 0, stage_kb: int = 0):
     _chk(_lib.moebius_set_tma(ctx, int(enable), pipes, stage_kb), "moebius_set_tma")
+
+
+def moebius_set_ring(ctx, ring_kb: int = 0, max_loads: int = 0):
+    _chk(_lib.moebius_set_ring(ctx, ring_kb, max_loads), "moebius_set_ring")
 
 
 def moebius_set_kv_rounds(ctx, max_level: int = 0):

@@ -391,11 +391,47 @@ __device__ __forceinline__ void lsu_unit(const Seg& s, const DevParams& p, uint3
   }
 }
 
-// Every warp is a PIPE: it takes unit tickets in list order and, for PATH_TMA units, keeps a
-// two-stage software pipeline in its private slice of shared memory -- the loads of unit i+1 fly
-// while the stores of unit i drain (lane 0 issues everything; measured best among 1-6 pipes x 2-4
-// stages).  PATH_LSU units are copied by the whole warp.  Before a pipe blocks on a
-// dependency counter it drains its own pipeline, so waits can never be circular.
+// Every warp is a PIPE: it takes unit tickets in list order and, for PATH_TMA units, runs a software
+// pipeline through its private RING in shared memory (ring_bytes per pipe).  A unit takes exactly the
+// bytes it needs from the ring, in FIFO order -- 24-KB weight units and 16-KB KV pages pack the same
+// 48-KB ring two resp. three deep -- its loads land there (mbarrier), its stores drain from there (bulk
+// async-group), and the space returns when the store has read it.  Up to ld_max units of a pipe have
+// their loads in flight while the stores of the units before them drain.  Measured on B200: finer units on
+// more pipes smooth the read/write mix the DRAM sees (4 pipes x 48-KB ring against 2 pipes x 2 x 48-KB
+// stages: weights + 2 %, KV + 1.5-2.5 %), as long as no ring byte stays empty.
+// PATH_LSU units are copied by the whole warp.  Before a pipe blocks on a dependency counter it drains its
+// own pipeline, so waits can never be circular.
+constexpr uint32_t kPipeQ = 8;            // units in flight per pipe (ring entries, mbarriers)
+constexpr uint32_t kPipeHdrBytes = 384;   // per pipe: kPipeQ mbarriers + kPipeQ entries
+struct PipeEnt {          // 32 bytes: one unit in flight
+  uint32_t si, ul, off, size;
+  KvDesc   d;
+};
+static_assert(kPipeQ * 8 + kPipeQ * sizeof(PipeEnt) <= kPipeHdrBytes, "pipe header");
+
+__device__ __forceinline__ void bulk_wait_read_n(uint32_t n) {   // the immediate operand, for n < kPipeQ
+  switch (n) {
+    case 0: bulk_wait_read<0>(); break;
+    case 1: bulk_wait_read<1>(); break;
+    case 2: bulk_wait_read<2>(); break;
+    case 3: bulk_wait_read<3>(); break;
+    case 4: bulk_wait_read<4>(); break;
+    case 5: bulk_wait_read<5>(); break;
+    case 6: bulk_wait_read<6>(); break;
+    default: bulk_wait_read<7>(); break;
+  }
+}
+
+// Ring bytes a PATH_TMA unit occupies (what its loads deliver), rounded to the 128-byte alignment a
+// tensor-map box needs in shared memory.
+__device__ __forceinline__ uint32_t tma_unit_bytes(const Seg& s, const DevParams& p, uint32_t ul) {
+  uint32_t b;
+  if (seg_kind(s) == SEG_KV) b = seg_boxes(s, ul) * s.ep_page_bytes;
+  else if (seg_kind(s) == SEG_XPOSE && s.groups_per_unit == s.n_groups) b = p.xt_rows * s.run_bytes * s.n_groups;   // a box is delivered whole
+  else b = s.rows_per_unit * s.chunk_bytes;          // LT and BULK: rows x piece
+  return (b + 127u) & ~127u;
+}
+
 template <int kMinCtasPerSm>   // 1: plans with PATH_TMA segments (shared-memory bound); 2: ld/st-only plans
 __global__ void __launch_bounds__(256, kMinCtasPerSm)
 moebius_reshard_kernel(const __grid_constant__ DevParams p_in, const __grid_constant__ CUtensorMap tm_w,
@@ -434,22 +470,25 @@ moebius_reshard_kernel(const __grid_constant__ DevParams p_in, const __grid_cons
     p.rank_hi = p_in.share_bounds[my_share + 1];
   }
   const uint32_t lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-  uint64_t* bar = (uint64_t*)smem + 2 * warp;                       // 2 barriers per pipe
-  char* ring = smem + 1024 + (size_t)warp * 2 * p.stage_bytes;     // 2 stages per pipe
-  if (lane == 0 && p.stage_bytes) {
-    mbar_init(bar, 1);
-    mbar_init(bar + 1, 1);
+  const uint32_t n_pipes = blockDim.x >> 5;
+  uint64_t* bar = (uint64_t*)(smem + (size_t)warp * kPipeHdrBytes);           // kPipeQ barriers per pipe
+  PipeEnt* ent = (PipeEnt*)(smem + (size_t)warp * kPipeHdrBytes + kPipeQ * 8);
+  const uint32_t hdr_bytes = (n_pipes * kPipeHdrBytes + 1023u) & ~1023u;
+  char* ring = smem + hdr_bytes + (size_t)warp * p.ring_bytes;
+  if (lane == 0 && p.ring_bytes) {
+    for (uint32_t i = 0; i < kPipeQ; ++i) mbar_init(bar + i, 1);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   __syncwarp();
   TmaCtx tc{&p, &tm_w, &tm_kv, &tm_stg, &tm_wtp};
 
-  // pipe state; identical in every lane (it depends on uniform values only)
-  bool loading = false;           // a unit's loads are in flight
-  uint32_t ld_si = 0, ld_ul = 0, ld_stage = 0;
-  KvDesc ld_d = {0, 0, 0, 0};
-  uint32_t phase0 = 0, phase1 = 0;
-  uint32_t next_stage = 0;
+  // pipe state; identical in every lane (it depends on uniform values only).  Units in flight are
+  // entries [q_tail, q_head) of the FIFO: [q_tail, q_load) have their stores committed (one bulk group
+  // each, in this order), [q_load, q_head) their loads in flight.  Entry i uses barrier i % kPipeQ, whose
+  // phase parity is (i / kPipeQ) & 1.
+  uint32_t q_head = 0, q_load = 0, q_tail = 0;
+  uint32_t ring_wr = 0, ring_free = p.ring_bytes;
+  const uint32_t ld_max = p.ld_max ? p.ld_max : 2u;
   // Completion signals are batched: units whose store groups are committed but not yet signalled all
   // belong to counter pend_ctr; one fence + one atomicAdd publishes them (a per-unit fence + atomic costs
   // a third of the pipe's time).  When the counter changes -- every segment boundary of a banded chain --
@@ -464,14 +503,15 @@ moebius_reshard_kernel(const __grid_constant__ DevParams p_in, const __grid_cons
     __syncwarp();
     if (lane == 0 && ctr >= 0 && n) { __threadfence(); atomicAdd(p.counters + ctr, n); }
   };
-  auto retire = [&]() {                  // loads landed -> issue the stores of the loading unit
-    if (!loading) return;
-    const Seg& s = p.segs[ld_si];
+  auto retire = [&]() {                  // oldest loading unit: its loads landed -> issue its stores
+    const uint32_t e = q_load % kPipeQ;
+    const PipeEnt en = ent[e];
+    const Seg& s = p.segs[en.si];
     const int32_t ctr = s.signal_ctr;
-    if (lane == 0) mbar_wait(bar + ld_stage, ld_stage ? phase1 : phase0);
+    if (lane == 0) mbar_wait(bar + e, (q_load / kPipeQ) & 1u);
     __syncwarp();
-    tma_issue_store(tc, s, ld_ul, ld_d, ring + (size_t)ld_stage * p.stage_bytes, lane);
-    if (ld_stage) phase1 ^= 1; else phase0 ^= 1;
+    tma_issue_store(tc, s, en.ul, en.d, ring + en.off, lane);
+    ++q_load;
     if (old_n && ++old_age >= 2) {       // the batch put aside is two groups old: complete, or nearly
       bulk_wait<2>();
       publish(old_ctr, old_n);
@@ -485,15 +525,23 @@ moebius_reshard_kernel(const __grid_constant__ DevParams p_in, const __grid_cons
       pend_ctr = ctr; pend_n = 0;
     }
     ++pend_n;
-    loading = false;
+  };
+  auto release = [&]() {                 // oldest storing unit: its stores have read the ring -> space returns
+    bulk_wait_read_n(q_load - q_tail - 1);   // wait_group is per thread: every lane waits for its own stores,
+    __syncwarp();                            // and all of them have before any lane refills the space
+    ring_free += ent[q_tail % kPipeQ].size;
+    ++q_tail;
   };
   auto drain = [&]() {                   // everything this pipe has in flight completes and is signalled
-    retire();
+    while (q_load != q_head) retire();
     bulk_wait<0>();
     publish(old_ctr, old_n);
     publish(pend_ctr, pend_n);
     old_n = 0;
     pend_n = 0;
+    q_tail = q_load;
+    ring_wr = 0;
+    ring_free = p.ring_bytes;
     __syncwarp();
   };
   uint32_t ok_si = 0xffffffffu;          // segment whose dependency this pipe has already seen satisfied
@@ -546,13 +594,32 @@ moebius_reshard_kernel(const __grid_constant__ DevParams p_in, const __grid_cons
     }
     if (seg_path(s) == PATH_TMA) {
       const KvDesc d = tma_prefetch_desc(p, s, ul);   // its latency hides behind the wait in retire()
-      retire();
+      const uint32_t need = tma_unit_bytes(s, p, ul);
+      while (q_head - q_load >= ld_max) retire();     // at most ld_max units of this pipe are loading
       wait_for(s, si);
-      bulk_wait_read<1>();     // the stage about to be refilled was read by the store group before the last one
-      __syncwarp();            // wait_group is per thread: every lane's stores have read the stage before lane 0 refills it
-      tma_issue_load(tc, s, ul, d, ring + (size_t)next_stage * p.stage_bytes, bar + next_stage, lane);
-      loading = true; ld_si = si; ld_ul = ul; ld_stage = next_stage; ld_d = d;
-      next_stage ^= 1;
+      // space: contiguous in the ring; a unit that does not fit before the end takes the tail as padding
+      bool wrap;
+      uint32_t pad;
+      for (;;) {
+        if (q_head == q_tail) { ring_wr = 0; ring_free = p.ring_bytes; }   // nothing in flight: start over
+        wrap = ring_wr + need > p.ring_bytes;
+        pad = wrap ? p.ring_bytes - ring_wr : 0u;
+        if (ring_free >= need + pad && q_head - q_tail < kPipeQ) break;
+        if (q_load == q_tail) retire();
+        release();
+      }
+      const uint32_t off = wrap ? 0u : ring_wr;
+      ring_wr = off + need;
+      ring_free -= need + pad;
+      const uint32_t e = q_head % kPipeQ;
+      if (lane == 0) {
+        PipeEnt en;
+        en.si = si; en.ul = ul; en.off = off; en.size = need + pad; en.d = d;
+        ent[e] = en;
+      }
+      __syncwarp();
+      tma_issue_load(tc, s, ul, d, ring + off, bar + e, lane);
+      ++q_head;
       t_next = fetch();        // its latency hides behind the loads just issued
     } else {
       t_next = fetch();
@@ -755,6 +822,10 @@ namespace moebius {
 // moebius_bind and again by moebius_set_tma (the stage geometry changes the maps and the attribute), so
 // that moebius_reshard / _staged / _share find everything in place: they create no event, resolve no
 // symbol, encode no descriptor and set no attribute.
+static size_t pipe_smem_bytes(const moebius_ctx* x) {   // per-pipe headers (barriers + FIFO entries), then the rings
+  return (((size_t)x->n_pipes * kPipeHdrBytes + 1023) & ~(size_t)1023) + (size_t)x->n_pipes * (size_t)x->ring_bytes;
+}
+
 int device_prepare(moebius_ctx* x) {
   x->prepared = false;
   if (!x->bound) return MOEBIUS_OK;
@@ -784,7 +855,7 @@ int device_prepare(moebius_ctx* x) {
   if (int rc = encode_tmaps(x)) return rc;
   const bool tma = x->use_tma != 0;   // bulk copies (long runs, attention shards, parked blocks) need the pipes' rings too
   if (tma) {
-    const size_t smem = 1024 + (size_t)x->n_pipes * 2 * (size_t)x->stage_bytes;
+    const size_t smem = pipe_smem_bytes(x);
     if (cudaFuncSetAttribute(moebius_reshard_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) {
       cudaGetLastError();
       return MOEBIUS_E_CUDA;
@@ -898,10 +969,12 @@ int launch_reshard_kernel(moebius_ctx* x, bool tma, int64_t unit_hint, cudaStrea
     // one CTA per SM, n_pipes warps, each with two private stages (tensor maps and the shared-memory
     // attribute were set up by device_prepare)
     p.stage_bytes = (uint32_t)x->stage_bytes;
+    p.ring_bytes = (uint32_t)x->ring_bytes;
+    p.ld_max = (uint32_t)x->ld_max;
     p.xt_rows = (uint32_t)x->xt_rows;
     threads = 32 * x->n_pipes;
     per_sm = 1;
-    smem = 1024 + (size_t)x->n_pipes * 2 * (size_t)x->stage_bytes;
+    smem = pipe_smem_bytes(x);
     if (smem != x->smem_set || !x->tmaps_valid) return MOEBIUS_E_STATE;
   } else {
     threads = x->threads > 0 ? x->threads : 256;

@@ -102,7 +102,9 @@ struct moebius_ctx {
   int kv_max_level;               // longest chain of dependent KV rounds before chains are cut by staging
   int use_tma;                    // planner emits PATH_TMA segments where the shapes allow
   int n_pipes;                    // TMA pipes (warps) per CTA, one CTA per SM
-  int64_t stage_bytes;            // bytes of one shared-memory stage; 2 stages per pipe
+  int64_t stage_bytes;            // largest PATH_TMA unit (what the planner sizes units to)
+  int64_t ring_bytes;             // shared-memory ring of one pipe (units take what they need, FIFO)
+  int ld_max;                     // units of one pipe whose loads may be in flight at once
   int def_pipes;                  // the defaults moebius_create derived from the EP page size
   int64_t def_stage_bytes;
   int xt_ok, kt_ok;               // weight / KV tensor maps exist for this config

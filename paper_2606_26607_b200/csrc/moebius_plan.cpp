@@ -246,6 +246,8 @@ int moebius_create(const moebius_config_t* c, moebius_ctx_t** out) {
       x->n_pipes = (int)std::max<int64_t>(1, std::min<int64_t>(4, (208 * 1024) / (2 * sb)));
     }
   }
+  x->ring_bytes = 2 * x->stage_bytes;
+  x->ld_max = 2;
   x->def_pipes = x->n_pipes;
   x->def_stage_bytes = x->stage_bytes;
   x->tmaps_valid = false;
@@ -388,9 +390,19 @@ int moebius_set_tma(moebius_ctx_t* x, int enable, int pipes, int stage_kb) {
   x->use_tma = enable ? 1 : 0;
   x->n_pipes = np;
   x->stage_bytes = sb;
+  x->ring_bytes = 2 * sb;
   x->tmaps_valid = false;
   tma_geometry(x);
   return device_prepare(x);   // a bound context re-encodes its tensor maps and shared-memory size here
+}
+
+int moebius_set_ring(moebius_ctx_t* x, int ring_kb, int max_loads) {
+  if (!x || ring_kb < 0 || max_loads < 0 || max_loads > 7) return MOEBIUS_E_INVAL;
+  const int64_t rb = ring_kb > 0 ? (int64_t)ring_kb * 1024 : 2 * x->stage_bytes;
+  if (rb < x->stage_bytes || (int64_t)x->n_pipes * rb > 208 * 1024) return MOEBIUS_E_INVAL;
+  x->ring_bytes = rb;
+  x->ld_max = max_loads > 0 ? max_loads : 2;
+  return device_prepare(x);   // the kernel's shared-memory size follows the ring
 }
 
 int moebius_set_kv_rounds(moebius_ctx_t* x, int max_level) {

@@ -220,6 +220,36 @@ def test_tma_shapes(first, pipes, stage_kb):
     sess.close()
 
 
+@pytest.mark.parametrize("pipes,stage_kb,ring_kb,max_loads", [
+    (2, 48, 96, 1), (2, 48, 96, 2), (2, 48, 48, 1), (4, 24, 52, 3), (2, 16, 100, 6), (3, 32, 68, 7), (1, 24, 200, 7),
+    (8, 8, 26, 2), (2, 40, 41, 1)])
+@pytest.mark.parametrize("which", ["smallish", "small_tight", "inplace"])
+def test_ring_shapes(which, pipes, stage_kb, ring_kb, max_loads):
+    """The pipes' rings (moebius_set_ring): a unit takes the bytes it needs, first in first out, so rings
+    that are no multiple of a unit (wrap padding), rings of exactly one unit, mixed unit sizes (weight
+    boxes, bulk chunks, 1-3 KV pages, staged pages, parked blocks) and up to 7 loads in flight per pipe
+    must all give the same bytes."""
+    cfg = {"smallish": SMALLISH, "small_tight": wl.get_config("small").with_(L=2, n_req=24),
+           "inplace": wl.get_config("small").with_(w_inplace=1, L=2, n_req=16)}[which]
+    kw = dict(policy="tight", cap_frac=0.5) if which == "small_tight" else {}
+    st, sess = gpu_session(cfg, initial_mode=TP, tma=(1, pipes, stage_kb), **kw)
+    mb.moebius_set_ring(sess.ctx, ring_kb, max_loads)
+    owner, bt, _ = start(st, sess, TP, "random")
+    mode, owner, bt, _ = gpu_switch(st, sess, TP, owner, bt)
+    mode, owner, bt, _ = gpu_switch(st, sess, mode, owner, bt)
+    gpu_switch(st, sess, mode, owner, bt)
+    sess.close()
+
+
+def test_ring_arguments():
+    st, sess = gpu_session(SMALLISH, tma=(1, 2, 48))
+    for bad in ((47, 1), (105, 1), (96, 8), (-1, 0)):      # below a stage, over 208 KB in all, too deep
+        with pytest.raises(mb.MoebiusError):
+            mb.moebius_set_ring(sess.ctx, *bad)
+    mb.moebius_set_ring(sess.ctx, 0, 0)
+    sess.close()
+
+
 @pytest.mark.parametrize("pipes,stage_kb", [(2, 48), (4, 24), (2, 16)])
 @pytest.mark.parametrize("first", [TP, EP])
 @pytest.mark.parametrize("which", ["smallish", "small", "ragged", "inplace"])
