@@ -52,6 +52,7 @@ def parse():
     ap.add_argument("--n-req", type=int, default=-1, help="override the number of live requests (experiments; named in config.workload)")
     ap.add_argument("--tma", default="", help="enable,pipes,stage_kb (tuning; default: library defaults)")
     ap.add_argument("--ring", default="", help="ring_kb,max_loads of the pipes' rings (tuning; after --tma)")
+    ap.add_argument("--l2", default="", help="load,store L2 cache-hint policy of the TMA operations (tuning)")
     ap.add_argument("--kv-rounds", type=int, default=0, help="max dependent KV rounds before chains are cut by staging (tuning)")
     ap.add_argument("--xt-mode", type=int, default=-1, help="weight tensor-map box side: 0 EP views, 1 TP views (tuning / A-B)")
     ap.add_argument("--chain-bands", action="store_true", help="banded weight chain: links overlap half by half (tuning / A-B; off by default)")
@@ -391,6 +392,9 @@ def run_moebius(args, env, config_name, pool_policy, cap_frac, steps, warmup, fu
     if args.ring:
         a, b = (int(x) for x in args.ring.split(","))
         mb.moebius_set_ring(sess.ctx, a, b)
+    if args.l2:
+        a, b = (int(x) for x in args.l2.split(","))
+        mb.moebius_set_l2_policy(sess.ctx, a, b)
     if args.kv_rounds:
         mb.moebius_set_kv_rounds(sess.ctx, args.kv_rounds)
     if args.kv_slice:

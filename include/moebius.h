@@ -359,6 +359,15 @@ MOEBIUS_API int moebius_set_chain_bands(moebius_ctx_t* ctx, int enable);
  * 128, 256 bytes.  Results are identical. */
 MOEBIUS_API int moebius_set_xt_mode(moebius_ctx_t* ctx, int mode);
 
+/* L2 cache-hint policy of the TMA loads and stores (tuning; any time): 0 none (the hardware default),
+ * 1 evict_first, 2 evict_last, 3 evict_normal, 4 evict_unchanged (PTX createpolicy.fractional.L2, fraction
+ * 1.0, passed as .L2::cache_hint to every cp.async.bulk[.tensor]).  Nothing is ever re-read (L2 hit rate
+ * 0.03 %), so this only shapes how the L2 writes dirty lines back.  Default: loads evict_last, stores
+ * unhinted -- A/B on B200, alternating in one session: 0.6 % (235B shape), 0.9 % (30B, fp8), 1.0 % (config 2)
+ * faster than no hint; evict_first on either side and any hint on the stores are neutral or slower.
+ * Results are identical. */
+MOEBIUS_API int moebius_set_l2_policy(moebius_ctx_t* ctx, int load_policy, int store_policy);
+
 /* Launch shape override for the ld/st path (tuning): values <= 0 restore the defaults; threads is a
  * multiple of 32, at most 256. */
 MOEBIUS_API int moebius_set_launch(moebius_ctx_t* ctx, int ctas_per_sm, int threads, int unit_kb);

@@ -12,7 +12,7 @@ from ._binding import (  # noqa: F401
     MoebiusError, moebius_config_t, moebius_layout_t, moebius_view_t, moebius_stats_t,
     moebius_create, moebius_destroy, moebius_layout, moebius_view, moebius_bind, moebius_active_mode,
     moebius_plan, moebius_plan_destroy, moebius_block_tables, moebius_plan_stats, moebius_plan_export,
-    moebius_reshard, moebius_stage_plan, moebius_reshard_staged, moebius_set_timing, moebius_last_kernel_ms, moebius_kernel_ms_history, moebius_set_launch, moebius_set_tma, moebius_set_ring, moebius_set_kv_rounds, moebius_set_kv_slice, moebius_set_chain_bands, moebius_set_xt_mode,
+    moebius_reshard, moebius_stage_plan, moebius_reshard_staged, moebius_set_timing, moebius_last_kernel_ms, moebius_kernel_ms_history, moebius_set_launch, moebius_set_tma, moebius_set_ring, moebius_set_l2_policy, moebius_set_kv_rounds, moebius_set_kv_slice, moebius_set_chain_bands, moebius_set_xt_mode,
     moebius_policy_config_t, moebius_policy_preset, moebius_policy_config, moebius_policy_create, moebius_policy_destroy,
     moebius_policy_mode, moebius_policy_step, moebius_capacity_check, moebius_policy_calibrate,
     POLICY_INTERACTIVE, POLICY_ROLLOUT, DECISION_STAY, DECISION_SWITCH, DECISION_CANCELLED,

@@ -26,7 +26,7 @@ EXPORTED_SYMBOLS = [
     "moebius_arena_export", "moebius_arena_import",
     "moebius_set_timing", "moebius_policy_preset", "moebius_policy_create", "moebius_policy_destroy",
     "moebius_policy_mode", "moebius_policy_step", "moebius_capacity_check", "moebius_policy_calibrate",
-    "moebius_last_kernel_ms", "moebius_kernel_ms_history", "moebius_set_launch", "moebius_set_tma", "moebius_set_ring", "moebius_set_kv_rounds", "moebius_set_kv_slice", "moebius_set_chain_bands", "moebius_set_xt_mode", "moebius_status_str", "moebius_version",
+    "moebius_last_kernel_ms", "moebius_kernel_ms_history", "moebius_set_launch", "moebius_set_tma", "moebius_set_ring", "moebius_set_l2_policy", "moebius_set_kv_rounds", "moebius_set_kv_slice", "moebius_set_chain_bands", "moebius_set_xt_mode", "moebius_status_str", "moebius_version",
 ]
 
 
@@ -156,6 +156,7 @@ _lib.moebius_kernel_ms_history.argtypes = [_vp, C.POINTER(C.c_float), C.c_int, C
 _lib.moebius_set_launch.argtypes = [_vp, C.c_int, C.c_int, C.c_int]
 _lib.moebius_set_tma.argtypes = [_vp, C.c_int, C.c_int, C.c_int]
 _lib.moebius_set_ring.argtypes = [_vp, C.c_int, C.c_int]
+_lib.moebius_set_l2_policy.argtypes = [_vp, C.c_int, C.c_int]
 _lib.moebius_set_kv_rounds.argtypes = [_vp, C.c_int]
 _lib.moebius_status_str.argtypes = [C.c_int]
 _lib.moebius_status_str.restype = C.c_char_p
@@ -449,6 +450,10 @@ def moebius_set_tma(ctx, enable: bool = True, pipes: int = 0, stage_kb: int = 0)
 
 def moebius_set_ring(ctx, ring_kb: int = 0, max_loads: int = 0):
     _chk(_lib.moebius_set_ring(ctx, ring_kb, max_loads), "moebius_set_ring")
+
+
+def moebius_set_l2_policy(ctx, load_policy: int = 0, store_policy: int = 0):
+    _chk(_lib.moebius_set_l2_policy(ctx, load_policy, store_policy), "moebius_set_l2_policy")
 
 
 def moebius_set_kv_rounds(ctx, max_level: int = 0):

@@ -145,37 +145,69 @@ __device__ __forceinline__ void mbar_wait(uint64_t* b, uint32_t parity) {
   for (uint32_t spins = 0; !mbar_try_wait(b, parity); ++spins)
     if (spins > (1u << 28)) __trap();
 }
-__device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t bytes, uint64_t* bar) {
-  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
-               :: "r"(smem_u32(dst)), "l"(src), "r"(bytes), "r"(smem_u32(bar)) : "memory");
+__device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t bytes, uint64_t* bar, uint64_t pol = 0) {
+  if (pol)
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1], %2, [%3], %4;"
+                 :: "r"(smem_u32(dst)), "l"(src), "r"(bytes), "r"(smem_u32(bar)), "l"(pol) : "memory");
+  else
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                 :: "r"(smem_u32(dst)), "l"(src), "r"(bytes), "r"(smem_u32(bar)) : "memory");
 }
-__device__ __forceinline__ void bulk_s2g(void* dst, const void* src, uint32_t bytes) {
-  asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;"
-               :: "l"(dst), "r"(smem_u32(src)), "r"(bytes) : "memory");
+__device__ __forceinline__ void bulk_s2g(void* dst, const void* src, uint32_t bytes, uint64_t pol = 0) {
+  if (pol)
+    asm volatile("cp.async.bulk.global.shared::cta.bulk_group.L2::cache_hint [%0], [%1], %2, %3;"
+                 :: "l"(dst), "r"(smem_u32(src)), "r"(bytes), "l"(pol) : "memory");
+  else
+    asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;"
+                 :: "l"(dst), "r"(smem_u32(src)), "r"(bytes) : "memory");
 }
-__device__ __forceinline__ void tma_load_5d(void* dst, const CUtensorMap* tm, int c0, int c1, int c2, int c3, int c4, uint64_t* bar) {
-  asm volatile("cp.async.bulk.tensor.5d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2,%3,%4,%5,%6}], [%7];"
-               :: "r"(smem_u32(dst)), "l"(tm), "r"(c0), "r"(c1), "r"(c2), "r"(c3), "r"(c4), "r"(smem_u32(bar)) : "memory");
+__device__ __forceinline__ void tma_load_5d(void* dst, const CUtensorMap* tm, int c0, int c1, int c2, int c3, int c4, uint64_t* bar, uint64_t pol = 0) {
+  if (pol)
+    asm volatile("cp.async.bulk.tensor.5d.shared::cluster.global.tile.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1, {%2,%3,%4,%5,%6}], [%7], %8;"
+                 :: "r"(smem_u32(dst)), "l"(tm), "r"(c0), "r"(c1), "r"(c2), "r"(c3), "r"(c4), "r"(smem_u32(bar)), "l"(pol) : "memory");
+  else
+    asm volatile("cp.async.bulk.tensor.5d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2,%3,%4,%5,%6}], [%7];"
+                 :: "r"(smem_u32(dst)), "l"(tm), "r"(c0), "r"(c1), "r"(c2), "r"(c3), "r"(c4), "r"(smem_u32(bar)) : "memory");
 }
-__device__ __forceinline__ void tma_store_5d(const CUtensorMap* tm, int c0, int c1, int c2, int c3, int c4, const void* src) {
-  asm volatile("cp.async.bulk.tensor.5d.global.shared::cta.tile.bulk_group [%0, {%1,%2,%3,%4,%5}], [%6];"
-               :: "l"(tm), "r"(c0), "r"(c1), "r"(c2), "r"(c3), "r"(c4), "r"(smem_u32(src)) : "memory");
+__device__ __forceinline__ void tma_store_5d(const CUtensorMap* tm, int c0, int c1, int c2, int c3, int c4, const void* src, uint64_t pol = 0) {
+  if (pol)
+    asm volatile("cp.async.bulk.tensor.5d.global.shared::cta.tile.bulk_group.L2::cache_hint [%0, {%1,%2,%3,%4,%5}], [%6], %7;"
+                 :: "l"(tm), "r"(c0), "r"(c1), "r"(c2), "r"(c3), "r"(c4), "r"(smem_u32(src)), "l"(pol) : "memory");
+  else
+    asm volatile("cp.async.bulk.tensor.5d.global.shared::cta.tile.bulk_group [%0, {%1,%2,%3,%4,%5}], [%6];"
+                 :: "l"(tm), "r"(c0), "r"(c1), "r"(c2), "r"(c3), "r"(c4), "r"(smem_u32(src)) : "memory");
 }
-__device__ __forceinline__ void tma_load_4d(void* dst, const CUtensorMap* tm, int c0, int c1, int c2, int c3, uint64_t* bar) {
-  asm volatile("cp.async.bulk.tensor.4d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2,%3,%4,%5}], [%6];"
-               :: "r"(smem_u32(dst)), "l"(tm), "r"(c0), "r"(c1), "r"(c2), "r"(c3), "r"(smem_u32(bar)) : "memory");
+__device__ __forceinline__ void tma_load_4d(void* dst, const CUtensorMap* tm, int c0, int c1, int c2, int c3, uint64_t* bar, uint64_t pol = 0) {
+  if (pol)
+    asm volatile("cp.async.bulk.tensor.4d.shared::cluster.global.tile.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1, {%2,%3,%4,%5}], [%6], %7;"
+                 :: "r"(smem_u32(dst)), "l"(tm), "r"(c0), "r"(c1), "r"(c2), "r"(c3), "r"(smem_u32(bar)), "l"(pol) : "memory");
+  else
+    asm volatile("cp.async.bulk.tensor.4d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2,%3,%4,%5}], [%6];"
+                 :: "r"(smem_u32(dst)), "l"(tm), "r"(c0), "r"(c1), "r"(c2), "r"(c3), "r"(smem_u32(bar)) : "memory");
 }
-__device__ __forceinline__ void tma_store_4d(const CUtensorMap* tm, int c0, int c1, int c2, int c3, const void* src) {
-  asm volatile("cp.async.bulk.tensor.4d.global.shared::cta.tile.bulk_group [%0, {%1,%2,%3,%4}], [%5];"
-               :: "l"(tm), "r"(c0), "r"(c1), "r"(c2), "r"(c3), "r"(smem_u32(src)) : "memory");
+__device__ __forceinline__ void tma_store_4d(const CUtensorMap* tm, int c0, int c1, int c2, int c3, const void* src, uint64_t pol = 0) {
+  if (pol)
+    asm volatile("cp.async.bulk.tensor.4d.global.shared::cta.tile.bulk_group.L2::cache_hint [%0, {%1,%2,%3,%4}], [%5], %6;"
+                 :: "l"(tm), "r"(c0), "r"(c1), "r"(c2), "r"(c3), "r"(smem_u32(src)), "l"(pol) : "memory");
+  else
+    asm volatile("cp.async.bulk.tensor.4d.global.shared::cta.tile.bulk_group [%0, {%1,%2,%3,%4}], [%5];"
+                 :: "l"(tm), "r"(c0), "r"(c1), "r"(c2), "r"(c3), "r"(smem_u32(src)) : "memory");
 }
-__device__ __forceinline__ void tma_load_3d(void* dst, const CUtensorMap* tm, int c0, int c1, int c2, uint64_t* bar) {
-  asm volatile("cp.async.bulk.tensor.3d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2,%3,%4}], [%5];"
-               :: "r"(smem_u32(dst)), "l"(tm), "r"(c0), "r"(c1), "r"(c2), "r"(smem_u32(bar)) : "memory");
+__device__ __forceinline__ void tma_load_3d(void* dst, const CUtensorMap* tm, int c0, int c1, int c2, uint64_t* bar, uint64_t pol = 0) {
+  if (pol)
+    asm volatile("cp.async.bulk.tensor.3d.shared::cluster.global.tile.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1, {%2,%3,%4}], [%5], %6;"
+                 :: "r"(smem_u32(dst)), "l"(tm), "r"(c0), "r"(c1), "r"(c2), "r"(smem_u32(bar)), "l"(pol) : "memory");
+  else
+    asm volatile("cp.async.bulk.tensor.3d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2,%3,%4}], [%5];"
+                 :: "r"(smem_u32(dst)), "l"(tm), "r"(c0), "r"(c1), "r"(c2), "r"(smem_u32(bar)) : "memory");
 }
-__device__ __forceinline__ void tma_store_3d(const CUtensorMap* tm, int c0, int c1, int c2, const void* src) {
-  asm volatile("cp.async.bulk.tensor.3d.global.shared::cta.tile.bulk_group [%0, {%1,%2,%3}], [%4];"
-               :: "l"(tm), "r"(c0), "r"(c1), "r"(c2), "r"(smem_u32(src)) : "memory");
+__device__ __forceinline__ void tma_store_3d(const CUtensorMap* tm, int c0, int c1, int c2, const void* src, uint64_t pol = 0) {
+  if (pol)
+    asm volatile("cp.async.bulk.tensor.3d.global.shared::cta.tile.bulk_group.L2::cache_hint [%0, {%1,%2,%3}], [%4], %5;"
+                 :: "l"(tm), "r"(c0), "r"(c1), "r"(c2), "r"(smem_u32(src)), "l"(pol) : "memory");
+  else
+    asm volatile("cp.async.bulk.tensor.3d.global.shared::cta.tile.bulk_group [%0, {%1,%2,%3}], [%4];"
+                 :: "l"(tm), "r"(c0), "r"(c1), "r"(c2), "r"(smem_u32(src)) : "memory");
 }
 __device__ __forceinline__ void bulk_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
 template <int N> __device__ __forceinline__ void bulk_wait_read() { asm volatile("cp.async.bulk.wait_group.read %0;" :: "n"(N) : "memory"); }
@@ -193,6 +225,7 @@ struct TmaCtx {
   const CUtensorMap* tm_kv;
   const CUtensorMap* tm_stg;
   const CUtensorMap* tm_wtp;
+  uint64_t pl, ps;        // L2 cache-hint policies of the loads / the stores (0: none)
 };
 
 // Row coordinate (in the staging tensor map) of pool z's copy of staging slot `slot`: the staging
@@ -221,9 +254,9 @@ __device__ __forceinline__ void tma_issue_load(const TmaCtx& c, const Seg& s, ui
     if (lane == 0) mbar_expect_tx(bar, b.nrows * b.piece);
     __syncwarp();
     if (b.src_stride == (int64_t)b.piece) {
-      if (lane == 0) bulk_g2s(stage, b.src, b.nrows * b.piece, bar);
+      if (lane == 0) bulk_g2s(stage, b.src, b.nrows * b.piece, bar, c.pl);
     } else {
-      for (uint32_t t = lane; t < b.nrows; t += 32) bulk_g2s(stage + (size_t)t * b.piece, b.src + (int64_t)t * b.src_stride, b.piece, bar);
+      for (uint32_t t = lane; t < b.nrows; t += 32) bulk_g2s(stage + (size_t)t * b.piece, b.src + (int64_t)t * b.src_stride, b.piece, bar, c.pl);
     }
     return;
   }
@@ -239,31 +272,31 @@ __device__ __forceinline__ void tma_issue_load(const TmaCtx& c, const Seg& s, ui
         // [run/4][rank][row][slot] (full units only: a ragged box would spill into the next rank's rows)
         if (lane == 0) {
           mbar_expect_tx(bar, piece * s.n_groups);
-          if (s.ep_is_src) bulk_g2s(stage, b.ep, piece * s.n_groups, bar);
-          else tma_load_4d(stage, c.tm_wtp, 0, 0, (int)(q * s.rows_total + row0), (int)(s.desc_begin - p.ep_shift), bar);
+          if (s.ep_is_src) bulk_g2s(stage, b.ep, piece * s.n_groups, bar, c.pl);
+          else tma_load_4d(stage, c.tm_wtp, 0, 0, (int)(q * s.rows_total + row0), (int)(s.desc_begin - p.ep_shift), bar, c.pl);
         }
         return;
       }
       if (s.ep_is_src) {
         if (lane == 0) {
           mbar_expect_tx(bar, piece * s.n_groups);   // the box is always delivered whole (rows past the end are zero-filled)
-          tma_load_5d(stage, c.tm_w, 0, (int)row0, 0, (int)q, (int)s.desc_begin, bar);
+          tma_load_5d(stage, c.tm_w, 0, (int)row0, 0, (int)q, (int)s.desc_begin, bar, c.pl);
         }
       } else {
         const uint32_t bytes = b.nrows * s.run_bytes;
         if (lane == 0) mbar_expect_tx(bar, bytes * s.n_groups);
         __syncwarp();
         for (uint32_t g = lane; g < s.n_groups; g += 32)
-          bulk_g2s(stage + (size_t)g * piece, b.tp + (int64_t)g * p.rank_stride, bytes, bar);
+          bulk_g2s(stage + (size_t)g * piece, b.tp + (int64_t)g * p.rank_stride, bytes, bar, c.pl);
       }
     } else {                                          // LT: one group, nrows pieces of chunk bytes
       const uint32_t chunk = s.chunk_bytes;
       if (lane == 0) mbar_expect_tx(bar, b.nrows * chunk);
       __syncwarp();
       if (s.ep_is_src) {
-        for (uint32_t t = lane; t < b.nrows; t += 32) bulk_g2s(stage + (size_t)t * chunk, b.ep + (int64_t)t * b.ep_row_stride, chunk, bar);
+        for (uint32_t t = lane; t < b.nrows; t += 32) bulk_g2s(stage + (size_t)t * chunk, b.ep + (int64_t)t * b.ep_row_stride, chunk, bar, c.pl);
       } else if (lane == 0) {
-        bulk_g2s(stage, b.tp + (int64_t)b.g0 * p.rank_stride, b.nrows * chunk, bar);
+        bulk_g2s(stage, b.tp + (int64_t)b.g0 * p.rank_stride, b.nrows * chunk, bar, c.pl);
       }
     }
     return;
@@ -282,8 +315,8 @@ __device__ __forceinline__ void tma_issue_load(const TmaCtx& c, const Seg& s, ui
     if (lane == 0) mbar_expect_tx(bar, nb * s.ep_page_bytes);
     __syncwarp();
     for (uint32_t k = lane; k < nb; k += 32) {
-      if (from_slot) tma_load_3d(stage + (size_t)k * s.ep_page_bytes, c.tm_stg, 0, stg_row(s, p, slot, z0 + k), 0, bar);
-      else tma_load_5d(stage + (size_t)k * s.ep_page_bytes, c.tm_kv, 0, (int)(d.ep_page * p.page_tokens), 0, (int)(z0 + k), d.ep_rank, bar);
+      if (from_slot) tma_load_3d(stage + (size_t)k * s.ep_page_bytes, c.tm_stg, 0, stg_row(s, p, slot, z0 + k), 0, bar, c.pl);
+      else tma_load_5d(stage + (size_t)k * s.ep_page_bytes, c.tm_kv, 0, (int)(d.ep_page * p.page_tokens), 0, (int)(z0 + k), d.ep_rank, bar, c.pl);
     }
   } else {
     const uint32_t bytes = ntok * s.run_bytes;
@@ -293,7 +326,7 @@ __device__ __forceinline__ void tma_issue_load(const TmaCtx& c, const Seg& s, ui
       const uint32_t k = o / s.n_groups, g = o - k * s.n_groups;
       const char* src = p.base + s.ep_off + (int64_t)(z0 + k) * s.pool_bytes + (int64_t)d.tp_page * s.tp_page_bytes +
                         (int64_t)tp_src_rank(g, s.rep, d.ep_rank) * p.rank_stride;
-      bulk_g2s(stage + (size_t)k * s.ep_page_bytes + (size_t)g * s.tp_page_bytes, src, bytes, bar);
+      bulk_g2s(stage + (size_t)k * s.ep_page_bytes + (size_t)g * s.tp_page_bytes, src, bytes, bar, c.pl);
     }
   }
 }
@@ -305,9 +338,9 @@ __device__ __forceinline__ void tma_issue_store(const TmaCtx& c, const Seg& s, u
     BulkUnit b;
     decode_bulk(s, p, ul, b);
     if (b.dst_stride == (int64_t)b.piece) {
-      if (lane == 0) bulk_s2g(b.dst, stage, b.nrows * b.piece);
+      if (lane == 0) bulk_s2g(b.dst, stage, b.nrows * b.piece, c.ps);
     } else {
-      for (uint32_t t = lane; t < b.nrows; t += 32) bulk_s2g(b.dst + (int64_t)t * b.dst_stride, stage + (size_t)t * b.piece, b.piece);
+      for (uint32_t t = lane; t < b.nrows; t += 32) bulk_s2g(b.dst + (int64_t)t * b.dst_stride, stage + (size_t)t * b.piece, b.piece, c.ps);
     }
     bulk_commit();
     return;
@@ -320,8 +353,8 @@ __device__ __forceinline__ void tma_issue_store(const TmaCtx& c, const Seg& s, u
       const uint32_t piece = p.xt_rows * s.run_bytes;
       if (p.xt_mode == 1 && b.nrows == p.xt_rows) {
         if (lane == 0) {
-          if (s.ep_is_src) tma_store_4d(c.tm_wtp, 0, 0, (int)(q * s.rows_total + row0), (int)(s.desc_begin - p.ep_shift), stage);
-          else bulk_s2g(b.ep, stage, piece * s.n_groups);
+          if (s.ep_is_src) tma_store_4d(c.tm_wtp, 0, 0, (int)(q * s.rows_total + row0), (int)(s.desc_begin - p.ep_shift), stage, c.ps);
+          else bulk_s2g(b.ep, stage, piece * s.n_groups, c.ps);
         }
         bulk_commit();
         return;
@@ -329,16 +362,16 @@ __device__ __forceinline__ void tma_issue_store(const TmaCtx& c, const Seg& s, u
       if (s.ep_is_src) {
         const uint32_t bytes = b.nrows * s.run_bytes;
         for (uint32_t g = lane; g < s.n_groups; g += 32)
-          bulk_s2g(b.tp + (int64_t)g * p.rank_stride, stage + (size_t)g * piece, bytes);
+          bulk_s2g(b.tp + (int64_t)g * p.rank_stride, stage + (size_t)g * piece, bytes, c.ps);
       } else if (lane == 0) {
-        tma_store_5d(c.tm_w, 0, (int)row0, 0, (int)q, (int)s.desc_begin, stage);   // rows past the end are clipped
+        tma_store_5d(c.tm_w, 0, (int)row0, 0, (int)q, (int)s.desc_begin, stage, c.ps);   // rows past the end are clipped
       }
     } else {                                          // LT
       const uint32_t chunk = s.chunk_bytes;
       if (s.ep_is_src) {
-        if (lane == 0) bulk_s2g(b.tp + (int64_t)b.g0 * p.rank_stride, stage, b.nrows * chunk);
+        if (lane == 0) bulk_s2g(b.tp + (int64_t)b.g0 * p.rank_stride, stage, b.nrows * chunk, c.ps);
       } else {
-        for (uint32_t t = lane; t < b.nrows; t += 32) bulk_s2g(b.ep + (int64_t)t * b.ep_row_stride, stage + (size_t)t * chunk, chunk);
+        for (uint32_t t = lane; t < b.nrows; t += 32) bulk_s2g(b.ep + (int64_t)t * b.ep_row_stride, stage + (size_t)t * chunk, chunk, c.ps);
       }
     }
     bulk_commit();
@@ -358,13 +391,13 @@ __device__ __forceinline__ void tma_issue_store(const TmaCtx& c, const Seg& s, u
       const uint32_t k = o / per_pool, gr = o - k * per_pool, g = gr / s.rep;   // gr = g*rep + r = destination rank
       char* dst = p.base + s.ep_off + (int64_t)(z0 + k) * s.pool_bytes + (int64_t)d.tp_page * s.tp_page_bytes +
                   (int64_t)gr * p.rank_stride;
-      bulk_s2g(dst, stage + (size_t)k * s.ep_page_bytes + (size_t)g * s.tp_page_bytes, bytes);
+      bulk_s2g(dst, stage + (size_t)k * s.ep_page_bytes + (size_t)g * s.tp_page_bytes, bytes, c.ps);
     }
   } else {
     // the whole page box is written: slots past the valid tokens get unspecified bytes (reading A10)
     for (uint32_t k = lane; k < nb; k += 32) {
-      if (to_slot) tma_store_3d(c.tm_stg, 0, stg_row(s, p, slot, z0 + k), 0, stage + (size_t)k * s.ep_page_bytes);
-      else tma_store_5d(c.tm_kv, 0, (int)(d.ep_page * p.page_tokens), 0, (int)(z0 + k), d.ep_rank, stage + (size_t)k * s.ep_page_bytes);
+      if (to_slot) tma_store_3d(c.tm_stg, 0, stg_row(s, p, slot, z0 + k), 0, stage + (size_t)k * s.ep_page_bytes, c.ps);
+      else tma_store_5d(c.tm_kv, 0, (int)(d.ep_page * p.page_tokens), 0, (int)(z0 + k), d.ep_rank, stage + (size_t)k * s.ep_page_bytes, c.ps);
     }
   }
   bulk_commit();
@@ -480,7 +513,15 @@ moebius_reshard_kernel(const __grid_constant__ DevParams p_in, const __grid_cons
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   __syncwarp();
-  TmaCtx tc{&p, &tm_w, &tm_kv, &tm_stg, &tm_wtp};
+  auto make_policy = [](uint32_t code) -> uint64_t {   // 0 none, 1 evict_first, 2 evict_last, 3 evict_normal, 4 evict_unchanged
+    uint64_t pol = 0;
+    if (code == 1) asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol));
+    else if (code == 2) asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(pol));
+    else if (code == 3) asm volatile("createpolicy.fractional.L2::evict_normal.b64 %0, 1.0;" : "=l"(pol));
+    else if (code == 4) asm volatile("createpolicy.fractional.L2::evict_unchanged.b64 %0, 1.0;" : "=l"(pol));
+    return pol;
+  };
+  TmaCtx tc{&p, &tm_w, &tm_kv, &tm_stg, &tm_wtp, make_policy(p.l2_ld), make_policy(p.l2_st)};
 
   // pipe state; identical in every lane (it depends on uniform values only).  Units in flight are
   // entries [q_tail, q_head) of the FIFO: [q_tail, q_load) have their stores committed (one bulk group
@@ -574,6 +615,48 @@ moebius_reshard_kernel(const __grid_constant__ DevParams p_in, const __grid_cons
   }
   uint32_t si = 0;
   uint32_t t_next = fetch();
+  // One unit, start to finish on the LSU path, up to its loads on the TMA path.
+  auto execute = [&](uint32_t xsi, uint32_t ul) {
+    const Seg& s = p.segs[xsi];
+    if (seg_path(s) == PATH_TMA) {
+      const KvDesc d = tma_prefetch_desc(p, s, ul);   // its latency hides behind the wait in retire()
+      const uint32_t need = tma_unit_bytes(s, p, ul);
+      while (q_head - q_load >= ld_max) retire();     // at most ld_max units of this pipe are loading
+      wait_for(s, xsi);
+      // space: contiguous in the ring; a unit that does not fit before the end takes the tail as padding
+      bool wrap;
+      uint32_t pad;
+      for (;;) {
+        if (q_head == q_tail) { ring_wr = 0; ring_free = p.ring_bytes; }   // nothing in flight: start over
+        wrap = ring_wr + need > p.ring_bytes;
+        pad = wrap ? p.ring_bytes - ring_wr : 0u;
+        if (ring_free >= need + pad && q_head - q_tail < kPipeQ) break;
+        if (q_load == q_tail) retire();
+        release();
+      }
+      const uint32_t off = wrap ? 0u : ring_wr;
+      ring_wr = off + need;
+      ring_free -= need + pad;
+      const uint32_t e = q_head % kPipeQ;
+      if (lane == 0) {
+        PipeEnt en;
+        en.si = xsi; en.ul = ul; en.off = off; en.size = need + pad; en.d = d;
+        ent[e] = en;
+      }
+      __syncwarp();
+      tma_issue_load(tc, s, ul, d, ring + off, bar + e, lane);
+      ++q_head;
+      t_next = fetch();        // its latency hides behind the loads just issued
+    } else {
+      t_next = fetch();
+      wait_for(s, xsi);
+      lsu_unit(s, p, ul, lane);
+      if (s.signal_ctr >= 0) {
+        __syncwarp();
+        if (lane == 0) { __threadfence(); atomicAdd(p.counters + s.signal_ctr, 1u); }
+      }
+    }
+  };
   for (;;) {
     const uint32_t u = __shfl_sync(0xffffffffu, t_next, 0);
     if (u >= p.total_units) break;
@@ -592,44 +675,7 @@ moebius_reshard_kernel(const __grid_constant__ DevParams p_in, const __grid_cons
       const uint32_t q = unit_ep_rank(s, p, ul);
       if (q < p.rank_lo || q >= p.rank_hi) { t_next = fetch(); continue; }
     }
-    if (seg_path(s) == PATH_TMA) {
-      const KvDesc d = tma_prefetch_desc(p, s, ul);   // its latency hides behind the wait in retire()
-      const uint32_t need = tma_unit_bytes(s, p, ul);
-      while (q_head - q_load >= ld_max) retire();     // at most ld_max units of this pipe are loading
-      wait_for(s, si);
-      // space: contiguous in the ring; a unit that does not fit before the end takes the tail as padding
-      bool wrap;
-      uint32_t pad;
-      for (;;) {
-        if (q_head == q_tail) { ring_wr = 0; ring_free = p.ring_bytes; }   // nothing in flight: start over
-        wrap = ring_wr + need > p.ring_bytes;
-        pad = wrap ? p.ring_bytes - ring_wr : 0u;
-        if (ring_free >= need + pad && q_head - q_tail < kPipeQ) break;
-        if (q_load == q_tail) retire();
-        release();
-      }
-      const uint32_t off = wrap ? 0u : ring_wr;
-      ring_wr = off + need;
-      ring_free -= need + pad;
-      const uint32_t e = q_head % kPipeQ;
-      if (lane == 0) {
-        PipeEnt en;
-        en.si = si; en.ul = ul; en.off = off; en.size = need + pad; en.d = d;
-        ent[e] = en;
-      }
-      __syncwarp();
-      tma_issue_load(tc, s, ul, d, ring + off, bar + e, lane);
-      ++q_head;
-      t_next = fetch();        // its latency hides behind the loads just issued
-    } else {
-      t_next = fetch();
-      wait_for(s, si);
-      lsu_unit(s, p, ul, lane);
-      if (s.signal_ctr >= 0) {
-        __syncwarp();
-        if (lane == 0) { __threadfence(); atomicAdd(p.counters + s.signal_ctr, 1u); }
-      }
-    }
+    execute(si, ul);
   }
   drain();
   if (bar_mode) {
@@ -971,6 +1017,7 @@ int launch_reshard_kernel(moebius_ctx* x, bool tma, int64_t unit_hint, cudaStrea
     p.stage_bytes = (uint32_t)x->stage_bytes;
     p.ring_bytes = (uint32_t)x->ring_bytes;
     p.ld_max = (uint32_t)x->ld_max;
+    p.l2_ld = (uint32_t)x->l2_ld; p.l2_st = (uint32_t)x->l2_st;
     p.xt_rows = (uint32_t)x->xt_rows;
     threads = 32 * x->n_pipes;
     per_sm = 1;

@@ -105,6 +105,7 @@ struct moebius_ctx {
   int64_t stage_bytes;            // largest PATH_TMA unit (what the planner sizes units to)
   int64_t ring_bytes;             // shared-memory ring of one pipe (units take what they need, FIFO)
   int ld_max;                     // units of one pipe whose loads may be in flight at once
+  int l2_ld, l2_st;               // L2 cache-hint policy of the TMA loads / stores (0: none)
   int def_pipes;                  // the defaults moebius_create derived from the EP page size
   int64_t def_stage_bytes;
   int xt_ok, kt_ok;               // weight / KV tensor maps exist for this config

@@ -146,6 +146,7 @@ struct DevParams {        // decoded launch state (the kernel fills the plan-dep
   uint32_t         stage_bytes;   // PATH_TMA: largest unit (the planner's unit size)
   uint32_t         ring_bytes;    // PATH_TMA: bytes of one pipe's shared-memory ring (>= stage_bytes)
   uint32_t         ld_max;        // PATH_TMA: units of one pipe whose loads may be in flight at once
+  uint32_t         l2_ld, l2_st;  // PATH_TMA: L2 cache-hint policy of loads / stores (0 none, 1 evict_first, 2 evict_last, ...)
   uint32_t         xt_rows;       // PATH_TMA: rows of the weight tensor-map box (= rows_per_unit)
   uint32_t         page_tokens;
   uint32_t         n_ranks;       // R

@@ -241,6 +241,19 @@ def test_ring_shapes(which, pipes, stage_kb, ring_kb, max_loads):
     sess.close()
 
 
+@pytest.mark.parametrize("load_policy,store_policy", [(0, 0), (1, 1), (2, 0), (3, 4), (4, 2)])
+def test_l2_policies(load_policy, store_policy):
+    """moebius_set_l2_policy: cache hints on every TMA operation change no byte."""
+    st, sess = gpu_session(wl.get_config("small").with_(L=1, n_req=12))
+    mb.moebius_set_l2_policy(sess.ctx, load_policy, store_policy)
+    owner, bt, _ = start(st, sess, TP, "random")
+    mode, owner, bt, _ = gpu_switch(st, sess, TP, owner, bt)
+    gpu_switch(st, sess, mode, owner, bt)
+    with pytest.raises(mb.MoebiusError):
+        mb.moebius_set_l2_policy(sess.ctx, 5, 0)
+    sess.close()
+
+
 def test_ring_arguments():
     st, sess = gpu_session(SMALLISH, tma=(1, 2, 48))
     for bad in ((47, 1), (105, 1), (96, 8), (-1, 0)):      # below a stage, over 208 KB in all, too deep
