@@ -59,6 +59,8 @@ def parse():
     ap.add_argument("--kv-slice", type=int, default=0, help="smallest KV slice interleaved with the weight chain, in units (tuning)")
     ap.add_argument("--w-orient", type=int, default=0, choices=[0, 1],
                     help="0: gate,up [E,H,I], down [E,I,H] (BASELINE.json, the headline); 1: the paper's W13 [E,2I,H], W2 [E,H,I] (named in config.workload)")
+    ap.add_argument("--w-inplace", action="store_true",
+                    help="force shift 0: EP and TP views alias the same bytes, every object takes the in-place path (named in config.workload)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-naive", action="store_true", help="skip timing the staged comparison path (PAPER.md Table 1)")
     ap.add_argument("--no-other-configs", action="store_true",
@@ -367,6 +369,8 @@ def run_moebius(args, env, config_name, pool_policy, cap_frac, steps, warmup, fu
         cfg = cfg.with_(L=args.layers, name="%s[L=%d]" % (cfg.name, args.layers))
     if args.w_orient and not overrides:
         cfg = cfg.with_(w_orient=1, name="%s[w_orient=1]" % cfg.name)
+    if args.w_inplace and not overrides:
+        cfg = cfg.with_(w_inplace=1, name="%s[w_inplace=1]" % cfg.name)
     lens = wl.draw_seq_lens(cfg)
     pool = wl.kv_pool_bytes(cfg, lens, pool_policy)
     if args.n_req >= 0:
@@ -376,7 +380,7 @@ def run_moebius(args, env, config_name, pool_policy, cap_frac, steps, warmup, fu
     c = mb.make_config(R=cfg.R, L=cfg.L, E=cfg.E, H=cfg.H, I=cfg.I, w_dtype=cfg.w_dtype, kv_heads=cfg.kv_heads,
                        head_dim=cfg.head_dim, page_tokens=cfg.page, kv_pool_bytes_per_rank_layer=pool,
                        max_requests=max(len(lens), 1), max_pages_per_request=mp, staging_cap_bytes=0,
-                       w_orient=cfg.w_orient)
+                       w_orient=cfg.w_orient, w_inplace=cfg.w_inplace)
     probe = mb.Session(c)
     resident = probe.layout.resident_bytes
     probe.close()
@@ -690,7 +694,7 @@ def main():
     del r
     # the other BASELINE.json configs, driver-timed in the same run (1 GPU, default workload only)
     if world == 1 and not args.no_other_configs and args.config == "qwen3_235b" and args.pool == "roomy" \
-            and not args.layers and args.n_req < 0 and not args.w_orient:
+            and not args.layers and args.n_req < 0 and not args.w_orient and not args.w_inplace:
         torch.cuda.empty_cache()
         others = {}
         for key, name, pool_policy, cap, over in OTHER_CONFIGS:

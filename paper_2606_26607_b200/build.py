@@ -26,6 +26,8 @@ def build(force: bool = False, verbose: bool = False) -> str:
     cmd = [nvcc, "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
            "-shared", "-Xcompiler", "-fPIC,-fvisibility=hidden,-Wall", "-cudart", "static",
            "-o", LIB] + [os.path.join(CSRC, f) for f in SOURCES]
+    extra = os.environ.get("MOEBIUS_NVCC_FLAGS", "").split()   # e.g. -DMOEBIUS_PIPE_STATS (profiling aid)
+    cmd[1:1] = extra
     if verbose:
         cmd.insert(1, "-Xptxas=-v")
         print(" ".join(cmd))

@@ -434,6 +434,19 @@ __device__ __forceinline__ void lsu_unit(const Seg& s, const DevParams& p, uint3
 // stages: weights + 2 %, KV + 1.5-2.5 %), as long as no ring byte stays empty.
 // PATH_LSU units are copied by the whole warp.  Before a pipe blocks on a dependency counter it drains its
 // own pipeline, so waits can never be circular.
+// -DMOEBIUS_PIPE_STATS: every pipe adds up where its time goes (globaltimer ns, lane 0) and the sums land
+// in the descriptor buffer's header at bytes 64.. (uint64 each: retire wait, release wait, dependency
+// stall, stalls, units, active time, publish wait, ticket wait); the header is zeroed by every moebius_reshard.
+#ifdef MOEBIUS_PIPE_STATS
+__device__ __forceinline__ uint64_t gtime() { uint64_t t; asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t)); return t; }
+#define MB_STAT_T0 const uint64_t stat_t0_ = gtime()
+#define MB_STAT_ADD(i) stat_[i] += gtime() - stat_t0_
+#define MB_STAT_INC(i) stat_[i] += 1
+#else
+#define MB_STAT_T0
+#define MB_STAT_ADD(i)
+#define MB_STAT_INC(i)
+#endif
 constexpr uint32_t kPipeQ = 8;            // units in flight per pipe (ring entries, mbarriers)
 constexpr uint32_t kPipeHdrBytes = 384;   // per pipe: kPipeQ mbarriers + kPipeQ entries
 struct PipeEnt {          // 32 bytes: one unit in flight
@@ -523,6 +536,10 @@ moebius_reshard_kernel(const __grid_constant__ DevParams p_in, const __grid_cons
   };
   TmaCtx tc{&p, &tm_w, &tm_kv, &tm_stg, &tm_wtp, make_policy(p.l2_ld), make_policy(p.l2_st)};
 
+#ifdef MOEBIUS_PIPE_STATS
+  uint64_t stat_[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+  const uint64_t stat_begin_ = gtime();
+#endif
   // pipe state; identical in every lane (it depends on uniform values only).  Units in flight are
   // entries [q_tail, q_head) of the FIFO: [q_tail, q_load) have their stores committed (one bulk group
   // each, in this order), [q_load, q_head) their loads in flight.  Entry i uses barrier i % kPipeQ, whose
@@ -549,12 +566,12 @@ moebius_reshard_kernel(const __grid_constant__ DevParams p_in, const __grid_cons
     const PipeEnt en = ent[e];
     const Seg& s = p.segs[en.si];
     const int32_t ctr = s.signal_ctr;
-    if (lane == 0) mbar_wait(bar + e, (q_load / kPipeQ) & 1u);
+    { MB_STAT_T0; if (lane == 0) mbar_wait(bar + e, (q_load / kPipeQ) & 1u); MB_STAT_ADD(0); }
     __syncwarp();
     tma_issue_store(tc, s, en.ul, en.d, ring + en.off, lane);
     ++q_load;
     if (old_n && ++old_age >= 2) {       // the batch put aside is two groups old: complete, or nearly
-      bulk_wait<2>();
+      { MB_STAT_T0; bulk_wait<2>(); MB_STAT_ADD(6); }
       publish(old_ctr, old_n);
       old_n = 0;
     }
@@ -568,7 +585,7 @@ moebius_reshard_kernel(const __grid_constant__ DevParams p_in, const __grid_cons
     ++pend_n;
   };
   auto release = [&]() {                 // oldest storing unit: its stores have read the ring -> space returns
-    bulk_wait_read_n(q_load - q_tail - 1);   // wait_group is per thread: every lane waits for its own stores,
+    { MB_STAT_T0; bulk_wait_read_n(q_load - q_tail - 1); MB_STAT_ADD(1); }   // wait_group is per thread: every lane waits for its own stores,
     __syncwarp();                            // and all of them have before any lane refills the space
     ring_free += ent[q_tail % kPipeQ].size;
     ++q_tail;
@@ -593,6 +610,8 @@ moebius_reshard_kernel(const __grid_constant__ DevParams p_in, const __grid_cons
     if (lane == 0) ok = ld_acquire(p.counters + s.wait_ctr) >= s.wait_target;
     ok = __shfl_sync(0xffffffffu, ok, 0);
     if (!ok) {
+      MB_STAT_T0;
+      MB_STAT_INC(3);
       drain();
       if (lane == 0) {
         for (uint32_t spins = 0; ld_acquire(p.counters + s.wait_ctr) < s.wait_target; ++spins) {
@@ -600,11 +619,13 @@ moebius_reshard_kernel(const __grid_constant__ DevParams p_in, const __grid_cons
           if (spins > (1u << 26)) __trap();
         }
       }
+      MB_STAT_ADD(2);
     }
     __syncwarp();
     fence_proxy_async();     // every lane issues TMA reads of what the signalling units wrote
   };
-  auto fetch = [&]() -> uint32_t { return lane == 0 ? atomicAdd(p.ticket, 1u) : 0u; };
+  uint32_t t_next = 0;
+  auto fetch = [&]() { if (lane == 0) t_next = atomicAdd(p.ticket, 1u); };
 
   const bool share = p.rank_hi - p.rank_lo < p.n_ranks;
   for (uint32_t wv = 0; wv < n_waves; ++wv) {
@@ -614,10 +635,11 @@ moebius_reshard_kernel(const __grid_constant__ DevParams p_in, const __grid_cons
     ok_si = 0xffffffffu;
   }
   uint32_t si = 0;
-  uint32_t t_next = fetch();
+  fetch();
   // One unit, start to finish on the LSU path, up to its loads on the TMA path.
   auto execute = [&](uint32_t xsi, uint32_t ul) {
     const Seg& s = p.segs[xsi];
+    MB_STAT_INC(4);
     if (seg_path(s) == PATH_TMA) {
       const KvDesc d = tma_prefetch_desc(p, s, ul);   // its latency hides behind the wait in retire()
       const uint32_t need = tma_unit_bytes(s, p, ul);
@@ -646,9 +668,9 @@ moebius_reshard_kernel(const __grid_constant__ DevParams p_in, const __grid_cons
       __syncwarp();
       tma_issue_load(tc, s, ul, d, ring + off, bar + e, lane);
       ++q_head;
-      t_next = fetch();        // its latency hides behind the loads just issued
+      fetch();                 // its latency hides behind the loads just issued
     } else {
-      t_next = fetch();
+      fetch();
       wait_for(s, xsi);
       lsu_unit(s, p, ul, lane);
       if (s.signal_ctr >= 0) {
@@ -658,7 +680,8 @@ moebius_reshard_kernel(const __grid_constant__ DevParams p_in, const __grid_cons
     }
   };
   for (;;) {
-    const uint32_t u = __shfl_sync(0xffffffffu, t_next, 0);
+    uint32_t u;
+    { MB_STAT_T0; u = __shfl_sync(0xffffffffu, t_next, 0); MB_STAT_ADD(7); }
     if (u >= p.total_units) break;
     // units are handed out in increasing order: search forward from the last segment
     while (si + 1 < p.n_segs && u >= __ldg(&p.segs[si + 1].unit_begin)) {
@@ -673,7 +696,7 @@ moebius_reshard_kernel(const __grid_constant__ DevParams p_in, const __grid_cons
     const uint32_t ul = u - s.unit_begin;
     if (share) {   // rank share: this launch executes only the units of the ranks it owns
       const uint32_t q = unit_ep_rank(s, p, ul);
-      if (q < p.rank_lo || q >= p.rank_hi) { t_next = fetch(); continue; }
+      if (q < p.rank_lo || q >= p.rank_hi) { fetch(); continue; }
     }
     execute(si, ul);
   }
@@ -704,6 +727,13 @@ moebius_reshard_kernel(const __grid_constant__ DevParams p_in, const __grid_cons
     fence_proxy_async();     // the next wave's TMA reads see what the other shares wrote
   }
   }
+#ifdef MOEBIUS_PIPE_STATS
+  if (lane == 0) {
+    stat_[5] = gtime() - stat_begin_;
+    unsigned long long* out = (unsigned long long*)((char*)p_in.ticket + 64);
+    for (int i = 0; i < 8; ++i) atomicAdd(out + i, (unsigned long long)stat_[i]);
+  }
+#endif
 }
 
 // Upload images.  A plan's image is read by the async H2D copies of moebius_reshard, so a buffer that
