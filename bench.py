@@ -601,7 +601,10 @@ OTHER_CONFIGS = (("qwen3_30b", "qwen3_30b", "roomy", 0.024, None), ("fp8_graph",
                  # the paper's own orientation: config 4 inside the cap with two spare slots; config 5
                  # only with one, so its W13 objects take the in-place path (S2: dependency waves, parked blocks)
                  ("qwen3_235b_paper_orient", "qwen3_235b", "roomy", 0.024, {"w_orient": 1}),
-                 ("fp8_graph_paper_orient_in_place", "fp8_graph", "roomy", 0.024, {"w_orient": 1}))
+                 ("fp8_graph_paper_orient_in_place", "fp8_graph", "roomy", 0.024, {"w_orient": 1}),
+                 # config 4 with NO spare slot at all: EP and TP views alias the same bytes (shift 0), every object
+                 # is permuted in place through the staging buffer, under a cap of 1.2 % of resident
+                 ("qwen3_235b_aliased_in_place", "qwen3_235b", "roomy", 0.012, {"w_inplace": 1}))
 
 
 def other_config_entry(r, peak):

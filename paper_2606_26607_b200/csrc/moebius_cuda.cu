@@ -234,6 +234,11 @@ __device__ __forceinline__ int stg_row(const Seg& s, const DevParams& p, uint32_
   return (int)((slot * s.stg_pools + (z - s.stg_pool_begin)) * p.page_tokens);
 }
 
+// A block-list segment whose EP side is the block's staging slot (in-place path: parked blocks).  Only the
+// TP-side box can serve it -- the EP-side tensor map covers the views, not the staging buffer -- so the planner
+// puts such a segment on the TMA path only when every unit of it is a whole box.
+__device__ __forceinline__ bool staged_ep(const Seg& s) { return s.n_desc != 0 && (s.kv_mode & 1u) != 0; }
+
 __device__ __forceinline__ KvDesc tma_prefetch_desc(const DevParams& p, const Seg& s, uint32_t ul) {
   KvDesc d = {0, 0, 0, 0};
   if (seg_kind(s) == SEG_KV) {
@@ -266,7 +271,7 @@ __device__ __forceinline__ void tma_issue_load(const TmaCtx& c, const Seg& s, ui
     if (s.groups_per_unit == s.n_groups) {          // XT
       const uint32_t q = b.q, row0 = b.row0;
       const uint32_t piece = p.xt_rows * s.run_bytes;
-      if (p.xt_mode == 1 && b.nrows == p.xt_rows) {
+      if ((p.xt_mode == 1 || staged_ep(s)) && b.nrows == p.xt_rows) {
         // TP-side box: the stage holds the unit in EP order [row][group][run], so the EP side is ONE
         // contiguous bulk copy and the run transposition happens in the box over the TP views
         // [run/4][rank][row][slot] (full units only: a ragged box would spill into the next rank's rows)
@@ -351,7 +356,7 @@ __device__ __forceinline__ void tma_issue_store(const TmaCtx& c, const Seg& s, u
     if (s.groups_per_unit == s.n_groups) {          // XT
       const uint32_t q = b.q, row0 = b.row0;
       const uint32_t piece = p.xt_rows * s.run_bytes;
-      if (p.xt_mode == 1 && b.nrows == p.xt_rows) {
+      if ((p.xt_mode == 1 || staged_ep(s)) && b.nrows == p.xt_rows) {
         if (lane == 0) {
           if (s.ep_is_src) tma_store_4d(c.tm_wtp, 0, 0, (int)(q * s.rows_total + row0), (int)(s.desc_begin - p.ep_shift), stage, c.ps);
           else bulk_s2g(b.ep, stage, piece * s.n_groups, c.ps);

@@ -3,6 +3,7 @@
 // page-move list with its dependency rounds and bounded staging, and the byte accounting.
 // Product code: it shares nothing with oracle/.
 #include <algorithm>
+#include <functional>
 #include <cstdlib>
 #include <cstring>
 #include <new>
@@ -809,7 +810,22 @@ struct PlanBuilder {
   // (EP->TP: the EP rows are copied there; TP->EP: the block is transposed INTO the slot) and finished
   // from the slot once their own destination is free; a slot is reused as soon as its block is finished.
   // `tmpl` carries the object's shape and unit geometry as weight_chain chose them.
-  int s2_object(const Seg& tmpl_in, int& prev_ctr, uint32_t& prev_units) {
+  // The schedule of one in-place object: its blocks, the waves of the greedy simulation, and the shapes
+  // its segments take.  stg_base / stg_bytes: the part of the weight staging area this object may use
+  // (objects whose schedules run concurrently get disjoint parts).
+  enum { OP_MOVE = 0, OP_FINISH = 1, OP_PARK = 2 };
+  struct S2Op { int32_t blk, op, slot; };
+  struct S2Sched {
+    Seg tmpl, lsu;
+    bool xt;
+    int64_t T, rt, Rr, run, slot_bytes;
+    int nb;
+    int64_t first_slot;                    // where the object's slots start in the weight staging area (set by the caller)
+    int peak_slots;                        // slots the schedule ever uses (they are handed out lowest first)
+    std::vector<std::vector<S2Op>> waves;
+  };
+
+  int s2_schedule(const Seg& tmpl_in, int64_t stg_bytes, S2Sched& sc) {
     Seg tmpl = tmpl_in;
     const int64_t run = tmpl.run_bytes, rt = tmpl.rows_total, Rr = (int64_t)R * run;
     const int64_t sS = (int64_t)x->ep_shift * x->S;            // EP view offset minus TP view offset
@@ -824,8 +840,8 @@ struct PlanBuilder {
     // 2R+2 slots let the simulation below always make progress; with less staging it is tried with what
     // fits (it reports E_STAGING itself when a cycle needs more parked blocks than there are slots)
     int64_t unit_rows = xt ? tmpl.rows_per_unit : 1;
-    int64_t t_max = x->w_stg_bytes / (2 * (int64_t)R + 2) / Rr;
-    if (t_max < 1) t_max = std::min<int64_t>(1, x->w_stg_bytes / Rr);
+    int64_t t_max = stg_bytes / (2 * (int64_t)R + 2) / Rr;
+    if (t_max < 1) t_max = std::min<int64_t>(1, stg_bytes / Rr);
     if (t_max < 1) return MOEBIUS_E_STAGING;
     if (xt && t_max < unit_rows) {       // blocks smaller than one box: the whole object goes through ld/st
       tmpl = lsu;
@@ -837,7 +853,7 @@ struct PlanBuilder {
     T = std::max<int64_t>(T, unit_rows);
     const int nb = (int)((rt + T - 1) / T), NB = nb * R;
     const int64_t slot_bytes = T * Rr;
-    const int n_slots = (int)std::min<int64_t>(x->w_stg_bytes / slot_bytes, 1 << 20);
+    const int n_slots = (int)std::min<int64_t>(stg_bytes / slot_bytes, 1 << 20);
     auto rows_of = [&](int i) { return std::min<int64_t>(T, rt - (int64_t)i * T); };
     // blockers of every block (CSR): the blocks whose SOURCE this block's DESTINATION overlaps
     std::vector<int32_t> bo((size_t)NB + 1, 0), bl;
@@ -867,15 +883,18 @@ struct PlanBuilder {
       bo[(size_t)b + 1] = (int32_t)bl.size();
     }
     // greedy wave simulation
-    enum { OP_MOVE = 0, OP_FINISH = 1, OP_PARK = 2 };
-    struct Op { int32_t blk, op, slot; };
-    std::vector<std::vector<Op>> waves;
+    typedef S2Op Op;
+    std::vector<std::vector<Op>>& waves = sc.waves;
+    waves.clear();
     std::vector<int32_t> read_wave((size_t)NB, INT32_MAX);    // wave in which the block's source was read (moved or parked)
     std::vector<int32_t> slot_of((size_t)NB, -1);
     std::vector<uint8_t> done((size_t)NB, 0);
     std::vector<int32_t> free_slots;
     for (int k = n_slots - 1; k >= 0; --k) free_slots.push_back(k);
-    int n_done = 0, n_parked = 0;
+    int n_done = 0, n_parked = 0, peak = 0;
+    // parks per stall: an eighth of the blocks -- against one block at a time that is 10 x fewer waves for the
+    // same number of parked blocks (config 4's shapes: 128 -> 10-13 waves per object, 260-295 -> 271-324 parked)
+    const int s2_batch = std::max(1, NB / 8);
     while (n_done < NB) {
       const int32_t w = (int32_t)waves.size();
       if (w > 4 * NB + 8) return MOEBIUS_E_STAGING;
@@ -892,36 +911,59 @@ struct PlanBuilder {
         else { ops.push_back({b, OP_MOVE, 0}); read_wave[(size_t)b] = w; }
         done[(size_t)b] = 1; ++n_done;
       }
-      if (ops.empty()) {      // a cycle: park the blockers of the block that needs the fewest parks
-        int best = -1, best_need = INT32_MAX;
-        for (int b = 0; b < NB; ++b) {
-          if (done[(size_t)b]) continue;
-          int need = (self[(size_t)b] && slot_of[(size_t)b] < 0) ? 1 : 0;
-          for (int32_t e = bo[(size_t)b]; e < bo[(size_t)b + 1]; ++e) need += read_wave[(size_t)bl[(size_t)e]] == INT32_MAX;
-          if (need > 0 && need < best_need) { best = b; best_need = need; }
-        }
-        if (best < 0 || best_need > (int)free_slots.size()) return MOEBIUS_E_STAGING;
+      if (ops.empty()) {      // cycles: park the blockers of the blocks that need the fewest parks
         auto park = [&](int a) {
           const int32_t sl = free_slots.back(); free_slots.pop_back();
+          peak = std::max(peak, sl + 1);
           slot_of[(size_t)a] = sl; read_wave[(size_t)a] = w;
           ops.push_back({a, OP_PARK, sl});
           ++n_parked;
           P->stats.w_staged_bytes += rows_of(a % nb) * Rr;
         };
-        if (self[(size_t)best] && slot_of[(size_t)best] < 0) park(best);
-        for (int32_t e = bo[(size_t)best]; e < bo[(size_t)best + 1]; ++e)
-          if (read_wave[(size_t)bl[(size_t)e]] == INT32_MAX) park(bl[(size_t)e]);
+        // One stall opens several blocks at once (s2_batch parks per wave at most): fewer, fatter waves.
+        int parks = 0;
+        do {
+          int best = -1, best_need = INT32_MAX;
+          for (int b = 0; b < NB; ++b) {
+            if (done[(size_t)b]) continue;
+            int need = (self[(size_t)b] && slot_of[(size_t)b] < 0) ? 1 : 0;
+            for (int32_t e = bo[(size_t)b]; e < bo[(size_t)b + 1]; ++e) need += read_wave[(size_t)bl[(size_t)e]] == INT32_MAX;
+            if (need > 0 && need < best_need) { best = b; best_need = need; }
+          }
+          if (best < 0) break;
+          if (best_need > (int)free_slots.size()) {
+            if (parks == 0) return MOEBIUS_E_STAGING;
+            break;
+          }
+          if (self[(size_t)best] && slot_of[(size_t)best] < 0) park(best);
+          for (int32_t e = bo[(size_t)best]; e < bo[(size_t)best + 1]; ++e)
+            if (read_wave[(size_t)bl[(size_t)e]] == INT32_MAX) park(bl[(size_t)e]);
+          parks += best_need;
+        } while (parks < s2_batch);
       }
+      // freed slots go back so that the lowest index is handed out next (peak_slots stays the true peak)
       for (int32_t sl : freed) free_slots.push_back(sl);
+      std::sort(free_slots.begin(), free_slots.end(), std::greater<int32_t>());
       waves.push_back(std::move(ops));
     }
-    P->stats.n_w_waves += (int32_t)waves.size();
     P->stats.n_w_parked += n_parked;
-    // segments: per wave up to three kinds of work, full and ragged blocks apart (a segment has one shape)
-    for (const std::vector<Op>& ops : waves) {
-      if (next_ctr >= (uint32_t)kMaxCounters) return MOEBIUS_E_STAGING;
-      const int ctr = (int)next_ctr++;
-      uint32_t wave_units = 0;
+    sc.tmpl = tmpl; sc.lsu = lsu; sc.xt = xt;
+    sc.T = T; sc.rt = rt; sc.Rr = Rr; sc.run = run; sc.slot_bytes = slot_bytes; sc.nb = nb; sc.first_slot = 0; sc.peak_slots = peak;
+    return MOEBIUS_OK;
+  }
+
+  // Segments of ONE wave of a schedule: up to three kinds of work, full and ragged blocks apart (a segment
+  // has one shape); every segment waits for (wait_ctr, wait_target) and signals ctr.  Returns the units added.
+  uint32_t s2_emit_wave(const S2Sched& sc, size_t w, int wait_ctr, uint32_t wait_target, int ctr) {
+    const Seg& tmpl = sc.tmpl; const Seg& lsu = sc.lsu;
+    const bool xt = sc.xt;
+    const int64_t T = sc.T, rt = sc.rt, Rr = sc.Rr, run = sc.run, slot_bytes = sc.slot_bytes;
+    const int nb = sc.nb;
+    auto rows_of = [&](int i) { return std::min<int64_t>(T, rt - (int64_t)i * T); };
+    typedef S2Op Op;
+    const std::vector<Op>& ops = sc.waves[w];
+    uint32_t wave_units = 0;
+    {
       for (int kind = 0; kind < 3; ++kind) for (int ragged = 0; ragged < 2; ++ragged) {
         const int64_t rows = ragged ? rows_of(nb - 1) : T;
         if (ragged && rows == T) continue;
@@ -929,14 +971,17 @@ struct PlanBuilder {
         for (const Op& o : ops) {
           const int i = o.blk % nb;
           if (o.op != kind || (rows_of(i) != T) != (ragged != 0)) continue;
-          blks.push_back({(uint32_t)(o.blk / nb), (uint32_t)((int64_t)i * T), (uint32_t)rows_of(i), (uint32_t)o.slot});
+          blks.push_back({(uint32_t)(o.blk / nb), (uint32_t)((int64_t)i * T), (uint32_t)rows_of(i), (uint32_t)(sc.first_slot + o.slot)});
         }
         if (blks.empty()) continue;
         // which side of the work is plain copying between the EP rows and the slot
         const bool copy = (kind == OP_PARK && e2t) || (kind == OP_FINISH && !e2t);
         Seg t;
         if (!copy) {
-          t = (kind == OP_MOVE) ? tmpl : (xt && seg_path(tmpl) == PATH_TMA ? lsu : tmpl);
+          // a parked block's EP side is its staging slot: on the TMA path the TP-side box serves it (the EP side
+          // is then one bulk copy from / into the slot), which needs whole boxes; ragged rows go through ld/st
+          const bool box_ok = xt && seg_path(tmpl) == PATH_TMA && rows % (int64_t)tmpl.rows_per_unit == 0;
+          t = (kind == OP_MOVE || !xt || box_ok) ? tmpl : lsu;
           t.kv_mode = kind == OP_MOVE ? 0u : 1u;             // 1: the EP side of every block is its staging slot
           t.stg_pools = 0;                                    // an irregular list: WBlk descriptors
           t.pool_begin = (uint32_t)P->wblk.size();
@@ -968,12 +1013,64 @@ struct PlanBuilder {
           }
           t.n_units = t.n_desc * t.row_blocks * t.chunks_per_run;
         }
-        t.wait_ctr = prev_ctr; t.wait_target = prev_units;
+        t.wait_ctr = wait_ctr; t.wait_target = wait_target;
         t.signal_ctr = ctr;
         wave_units += t.n_units;
         push_seg(cw, t);
       }
-      prev_ctr = ctr; prev_units = wave_units;
+    }
+    return wave_units;
+  }
+
+  // One in-place object on its own: its waves one after the other, behind (prev_ctr, prev_units).
+  int s2_object(const Seg& tmpl_in, int& prev_ctr, uint32_t& prev_units) {
+    S2Sched sc;
+    if (int rc = s2_schedule(tmpl_in, x->w_stg_bytes, sc)) return rc;
+    P->stats.n_w_waves += (int32_t)sc.waves.size();
+    for (size_t w = 0; w < sc.waves.size(); ++w) {
+      if (next_ctr >= (uint32_t)kMaxCounters) return MOEBIUS_E_STAGING;
+      const int ctr = (int)next_ctr++;
+      const uint32_t units = s2_emit_wave(sc, w, prev_ctr, prev_units, ctr);
+      prev_ctr = ctr; prev_units = units;
+    }
+    return MOEBIUS_OK;
+  }
+
+  // Aliased views (shift 0): an object's move stays inside its own slot, so the objects do not depend on one
+  // another and their schedules run side by side -- wave w of every object of a group is ONE dependency
+  // level of the launch -- each object parking into its own part of the staging area.  A group is as many
+  // consecutive objects as the staging area holds at the peak of their schedules.
+  int s2_objects_concurrent(const std::vector<Seg>& tmpls) {
+    // every object is scheduled as if it were alone (same blocks, same waves as on its own); what it needs
+    // of the staging area is the peak of slots its schedule ever holds
+    std::vector<S2Sched> sc(tmpls.size());
+    for (size_t o = 0; o < tmpls.size(); ++o)
+      if (int rc = s2_schedule(tmpls[o], x->w_stg_bytes, sc[o])) return rc;
+    int prev_ctr = -1; uint32_t prev_units = 0;
+    for (size_t o0 = 0; o0 < sc.size();) {
+      size_t n = 0;
+      int64_t end = 0;
+      while (o0 + n < sc.size()) {
+        S2Sched& c = sc[o0 + n];
+        const int64_t first = (end + c.slot_bytes - 1) / c.slot_bytes;
+        const int64_t e = (first + std::max(1, c.peak_slots)) * c.slot_bytes;
+        if (n > 0 && e > x->w_stg_bytes) break;
+        c.first_slot = first;
+        end = e;
+        ++n;
+      }
+      size_t n_waves = 0;
+      for (size_t k = 0; k < n; ++k) n_waves = std::max(n_waves, sc[o0 + k].waves.size());
+      P->stats.n_w_waves += (int32_t)n_waves;
+      for (size_t w = 0; w < n_waves; ++w) {
+        if (next_ctr >= (uint32_t)kMaxCounters) return MOEBIUS_E_STAGING;
+        const int ctr = (int)next_ctr++;
+        uint32_t units = 0;
+        for (size_t k = 0; k < n; ++k)
+          if (w < sc[o0 + k].waves.size()) units += s2_emit_wave(sc[o0 + k], w, prev_ctr, prev_units, ctr);
+        prev_ctr = ctr; prev_units = units;
+      }
+      o0 += n;
     }
     return MOEBIUS_OK;
   }
@@ -1053,7 +1150,16 @@ struct PlanBuilder {
       }
       int prev_ctr = -1; uint32_t prev_units = 0;
       int band_ctr[2] = {-1, -1}; uint32_t band_units[2] = {0, 0};
-      for (int step = 0; step < n_links; ++step) {
+      if (x->ep_shift == 0) {       // aliased views: independent objects, their in-place schedules side by side
+        std::vector<Seg> tmpls((size_t)n_links);
+        for (int step = 0; step < n_links; ++step) {
+          const int k = e2t ? step : n_links - 1 - step;
+          const WObj& ob = x->obj[k % x->n_obj];
+          if (int rc = link_seg(ob, 3 * (k / x->n_obj) + ob.slot, tmpls[(size_t)step])) return fail(rc);
+        }
+        if (int rc = s2_objects_concurrent(tmpls)) return fail(rc);
+      }
+      for (int step = 0; step < n_links && x->ep_shift > 0; ++step) {
         const int k = e2t ? step : n_links - 1 - step;
         const int layer = k / x->n_obj;
         const WObj& ob = x->obj[k % x->n_obj];
