@@ -246,8 +246,26 @@ __device__ __forceinline__ KvDesc tma_prefetch_desc(const DevParams& p, const Se
     kv_unit(s, ul, pb, di);
     const int4 v = __ldg((const int4*)(p.kv + s.desc_begin + di));
     d.ep_rank = v.x; d.ep_page = v.y; d.tp_page = v.z; d.ntok_slot = (uint32_t)v.w;
+  } else if (seg_kind(s) == SEG_BULK) {                                   // the unit's BulkDesc (two int64 offsets)
+    const int4 v = __ldg((const int4*)(p.bulk + s.desc_begin + ul / (s.row_blocks * s.chunks_per_run)));
+    d.ep_rank = v.x; d.ep_page = v.y; d.tp_page = v.z; d.ntok_slot = (uint32_t)v.w;
+  } else if (seg_kind(s) == SEG_XPOSE && s.n_desc && !s.stg_pools) {    // an irregular block list: the unit's WBlk
+    const int4 v = __ldg((const int4*)(p.wblk + s.pool_begin + ul / s.pools_per_unit));
+    d.ep_rank = v.x; d.ep_page = v.y; d.tp_page = v.z; d.ntok_slot = (uint32_t)v.w;   // q, row0, nrows, slot
   }
   return d;
+}
+
+// The prefetched descriptor of a block-list unit (tma_prefetch_desc stores a WBlk in the KvDesc's 16 bytes).
+__device__ __forceinline__ BulkDesc bulk_of(const KvDesc& d) {
+  BulkDesc b;
+  b.src_off = (int64_t)(((uint64_t)(uint32_t)d.ep_page << 32) | (uint32_t)d.ep_rank);
+  b.dst_off = (int64_t)(((uint64_t)d.ntok_slot << 32) | (uint32_t)d.tp_page);
+  return b;
+}
+__device__ __forceinline__ bool has_wblk(const Seg& s) { return s.n_desc != 0 && s.stg_pools == 0; }
+__device__ __forceinline__ WBlk wblk_of(const KvDesc& d) {
+  return WBlk{(uint32_t)d.ep_rank, (uint32_t)d.ep_page, (uint32_t)d.tp_page, d.ntok_slot};
 }
 
 __device__ __forceinline__ void tma_issue_load(const TmaCtx& c, const Seg& s, uint32_t ul, const KvDesc& d, char* stage,
@@ -255,7 +273,7 @@ __device__ __forceinline__ void tma_issue_load(const TmaCtx& c, const Seg& s, ui
   const DevParams& p = *c.p;
   if (seg_kind(s) == SEG_BULK) {                      // strided rows -> dense stage [row][piece]
     BulkUnit b;
-    decode_bulk(s, p, ul, b);
+    decode_bulk(s, p, ul, b, true, bulk_of(d));
     if (lane == 0) mbar_expect_tx(bar, b.nrows * b.piece);
     __syncwarp();
     if (b.src_stride == (int64_t)b.piece) {
@@ -267,7 +285,7 @@ __device__ __forceinline__ void tma_issue_load(const TmaCtx& c, const Seg& s, ui
   }
   if (seg_kind(s) == SEG_XPOSE) {
     Box b;
-    decode_box(s, p, ul, 0, b);
+    decode_box(s, p, ul, 0, b, has_wblk(s), wblk_of(d));
     if (s.groups_per_unit == s.n_groups) {          // XT
       const uint32_t q = b.q, row0 = b.row0;
       const uint32_t piece = p.xt_rows * s.run_bytes;
@@ -341,7 +359,7 @@ __device__ __forceinline__ void tma_issue_store(const TmaCtx& c, const Seg& s, u
   const DevParams& p = *c.p;
   if (seg_kind(s) == SEG_BULK) {
     BulkUnit b;
-    decode_bulk(s, p, ul, b);
+    decode_bulk(s, p, ul, b, true, bulk_of(d));
     if (b.dst_stride == (int64_t)b.piece) {
       if (lane == 0) bulk_s2g(b.dst, stage, b.nrows * b.piece, c.ps);
     } else {
@@ -352,7 +370,7 @@ __device__ __forceinline__ void tma_issue_store(const TmaCtx& c, const Seg& s, u
   }
   if (seg_kind(s) == SEG_XPOSE) {
     Box b;
-    decode_box(s, p, ul, 0, b);
+    decode_box(s, p, ul, 0, b, has_wblk(s), wblk_of(d));
     if (s.groups_per_unit == s.n_groups) {          // XT
       const uint32_t q = b.q, row0 = b.row0;
       const uint32_t piece = p.xt_rows * s.run_bytes;
@@ -554,12 +572,15 @@ moebius_reshard_kernel(const __grid_constant__ DevParams p_in, const __grid_cons
   const uint32_t ld_max = p.ld_max ? p.ld_max : 2u;
   // Completion signals are batched: units whose store groups are committed but not yet signalled all
   // belong to counter pend_ctr; one fence + one atomicAdd publishes them (a per-unit fence + atomic costs
-  // a third of the pipe's time).  When the counter changes -- every segment boundary of a banded chain --
-  // the batch is not published at once, which would mean waiting for its last store group: it is put
-  // aside (old_*) and published two units later, when a wait for "all but the two youngest groups"
-  // returns at once.  A drain publishes everything.
-  int32_t pend_ctr = -1, old_ctr = -1;
-  uint32_t pend_n = 0, old_n = 0, old_age = 0;
+  // a third of the pipe's time).  When the counter changes the batch is CLOSED but not published at once,
+  // which would mean waiting for its last store group: it waits in a short queue (cq_*, oldest first) and
+  // is published two units later, when a wait for "all but the two youngest groups" returns at once.
+  // Three entries are enough for a counter that changes with every unit (block lists of the in-place
+  // path, where a wave of an object is a handful of units per pipe).  A drain publishes everything.
+  int32_t pend_ctr = -1;
+  uint32_t pend_n = 0;
+  int32_t cq_c0 = -1, cq_c1 = -1, cq_c2 = -1;       // scalars, not arrays: they stay in registers
+  uint32_t cq_n0 = 0, cq_n1 = 0, cq_n2 = 0, cq_a0 = 0, cq_a1 = 0, cq_len = 0;   // ages of entries 0 and 1 (entry 2 is always the newest)
 
   auto publish = [&](int32_t ctr, uint32_t n) {   // after every lane's writes of those units have completed
     fence_proxy_async();
@@ -575,15 +596,27 @@ moebius_reshard_kernel(const __grid_constant__ DevParams p_in, const __grid_cons
     __syncwarp();
     tma_issue_store(tc, s, en.ul, en.d, ring + en.off, lane);
     ++q_load;
-    if (old_n && ++old_age >= 2) {       // the batch put aside is two groups old: complete, or nearly
+    ++cq_a0; ++cq_a1;
+    if (cq_len && cq_a0 >= 2) {          // the oldest closed batch is two groups old: complete, or nearly
       { MB_STAT_T0; bulk_wait<2>(); MB_STAT_ADD(6); }
-      publish(old_ctr, old_n);
-      old_n = 0;
+      while (cq_len && cq_a0 >= 2) {
+        publish(cq_c0, cq_n0);
+        cq_c0 = cq_c1; cq_n0 = cq_n1; cq_a0 = cq_a1;
+        cq_c1 = cq_c2; cq_n1 = cq_n2; cq_a1 = 0;
+        --cq_len;
+      }
     }
     if (ctr != pend_ctr) {
       if (pend_ctr >= 0 && pend_n) {
-        if (old_n) { bulk_wait<1>(); publish(old_ctr, old_n); }   // all but the group just committed
-        old_ctr = pend_ctr; old_n = pend_n; old_age = 0;
+        if (cq_len == 3) {               // cannot happen while batches leave at age 2: kept for safety
+          bulk_wait<1>();
+          publish(cq_c0, cq_n0); publish(cq_c1, cq_n1); publish(cq_c2, cq_n2);
+          cq_len = 0;
+        }
+        if (cq_len == 0) { cq_c0 = pend_ctr; cq_n0 = pend_n; cq_a0 = 0; }
+        else if (cq_len == 1) { cq_c1 = pend_ctr; cq_n1 = pend_n; cq_a1 = 0; }
+        else { cq_c2 = pend_ctr; cq_n2 = pend_n; }
+        ++cq_len;
       }
       pend_ctr = ctr; pend_n = 0;
     }
@@ -598,19 +631,26 @@ moebius_reshard_kernel(const __grid_constant__ DevParams p_in, const __grid_cons
   auto drain = [&]() {                   // everything this pipe has in flight completes and is signalled
     while (q_load != q_head) retire();
     bulk_wait<0>();
-    publish(old_ctr, old_n);
+    if (cq_len > 0) publish(cq_c0, cq_n0);
+    if (cq_len > 1) publish(cq_c1, cq_n1);
+    if (cq_len > 2) publish(cq_c2, cq_n2);
+    cq_len = 0;
     publish(pend_ctr, pend_n);
-    old_n = 0;
     pend_n = 0;
     q_tail = q_load;
     ring_wr = 0;
     ring_free = p.ring_bytes;
     __syncwarp();
   };
-  uint32_t ok_si = 0xffffffffu;          // segment whose dependency this pipe has already seen satisfied
+  // The dependency this pipe has already seen satisfied: counter ok_ctr had reached ok_target.  Counters only
+  // grow, so every segment that waits for the same counter and no higher a target -- all segments of one
+  // wave of an in-place object, all slices of one KV round -- passes without another acquire-load.
+  int32_t ok_ctr = -1;
+  uint32_t ok_target = 0;
   auto wait_for = [&](const Seg& s, uint32_t si) {   // dependency of a segment (chain links, KV rounds)
-    if (s.wait_ctr < 0 || si == ok_si) return;       // one acquire-load per segment, not per unit
-    ok_si = si;
+    (void)si;
+    if (s.wait_ctr < 0 || (s.wait_ctr == ok_ctr && s.wait_target <= ok_target)) return;
+    ok_ctr = s.wait_ctr; ok_target = s.wait_target;
     uint32_t ok = 0;
     if (lane == 0) ok = ld_acquire(p.counters + s.wait_ctr) >= s.wait_target;
     ok = __shfl_sync(0xffffffffu, ok, 0);
@@ -637,7 +677,7 @@ moebius_reshard_kernel(const __grid_constant__ DevParams p_in, const __grid_cons
   if (bar_mode) {
     load_hdr((const PlanHdr*)((const char*)p_in.hdr + __ldg(wave_tab + wv)));
     p.ticket = p_in.counters + (size_t)my_share * n_waves + wv;      // wave lists carry no dependency: the counters are free
-    ok_si = 0xffffffffu;
+    ok_ctr = -1;
   }
   uint32_t si = 0;
   fetch();
@@ -688,14 +728,24 @@ moebius_reshard_kernel(const __grid_constant__ DevParams p_in, const __grid_cons
     uint32_t u;
     { MB_STAT_T0; u = __shfl_sync(0xffffffffu, t_next, 0); MB_STAT_ADD(7); }
     if (u >= p.total_units) break;
-    // units are handed out in increasing order: search forward from the last segment
-    while (si + 1 < p.n_segs && u >= __ldg(&p.segs[si + 1].unit_begin)) {
-      uint32_t lo = si + 1, hi = p.n_segs - 1;  // last segment whose unit_begin <= u
-      while (lo < hi) {
-        uint32_t mid = (lo + hi + 1) >> 1;
-        if (__ldg(&p.segs[mid].unit_begin) <= u) lo = mid; else hi = mid - 1;
+    // units are handed out in increasing order: search forward from the last segment.  The warp looks at the
+    // next 32 segments at once (one round trip; plans of many small segments -- block lists of the in-place
+    // path, tight-pool rounds -- change segment every few units, and a binary search is a dozen dependent
+    // loads each time); only a jump beyond them falls back to the binary search.
+    if (si + 1 < p.n_segs) {
+      const uint32_t cand = si + 1 + lane;
+      const bool le = cand < p.n_segs && __ldg(&p.segs[cand].unit_begin) <= u;
+      const uint32_t m = __ballot_sync(0xffffffffu, le);      // unit_begin is non-decreasing: a prefix of ones
+      if (m == 0xffffffffu) {
+        uint32_t lo = si + 32, hi = p.n_segs - 1;              // last segment whose unit_begin <= u
+        while (lo < hi) {
+          uint32_t mid = (lo + hi + 1) >> 1;
+          if (__ldg(&p.segs[mid].unit_begin) <= u) lo = mid; else hi = mid - 1;
+        }
+        si = lo;
+      } else {
+        si += (uint32_t)__popc(m);
       }
-      si = lo;
     }
     const Seg& s = p.segs[si];
     const uint32_t ul = u - s.unit_begin;

@@ -825,6 +825,12 @@ struct PlanBuilder {
     std::vector<std::vector<S2Op>> waves;
   };
 
+  struct S2Cached {
+    int64_t run, rt, T, sS; int nb, n_slots, peak, n_parked; int64_t staged_bytes;
+    std::vector<std::vector<S2Op>> waves;
+  };
+  std::vector<S2Cached> s2_cache;
+
   int s2_schedule(const Seg& tmpl_in, int64_t stg_bytes, S2Sched& sc) {
     Seg tmpl = tmpl_in;
     const int64_t run = tmpl.run_bytes, rt = tmpl.rows_total, Rr = (int64_t)R * run;
@@ -855,6 +861,18 @@ struct PlanBuilder {
     const int64_t slot_bytes = T * Rr;
     const int n_slots = (int)std::min<int64_t>(stg_bytes / slot_bytes, 1 << 20);
     auto rows_of = [&](int i) { return std::min<int64_t>(T, rt - (int64_t)i * T); };
+    // objects of one shape have one schedule (every layer's gate and up, every layer's down): simulate once
+    struct { int64_t run, rt, T, sS; int nb, n_slots; } key = {run, rt, T, sS, nb, n_slots};
+    for (const S2Cached& c : s2_cache)
+      if (c.run == key.run && c.rt == key.rt && c.T == key.T && c.sS == key.sS && c.nb == key.nb && c.n_slots == key.n_slots) {
+        sc.waves = c.waves;
+        P->stats.n_w_parked += c.n_parked;
+        P->stats.w_staged_bytes += c.staged_bytes;
+        sc.tmpl = tmpl; sc.lsu = lsu; sc.xt = xt;
+        sc.T = T; sc.rt = rt; sc.Rr = Rr; sc.run = run; sc.slot_bytes = slot_bytes; sc.nb = nb; sc.first_slot = 0; sc.peak_slots = c.peak;
+        return MOEBIUS_OK;
+      }
+    const int64_t staged_before = P->stats.w_staged_bytes;
     // blockers of every block (CSR): the blocks whose SOURCE this block's DESTINATION overlaps
     std::vector<int32_t> bo((size_t)NB + 1, 0), bl;
     std::vector<uint8_t> self((size_t)NB, 0);
@@ -881,6 +899,51 @@ struct PlanBuilder {
       nt = (int)(std::unique(tmp, tmp + nt) - tmp);
       for (int k = 0; k < nt; ++k) bl.push_back(tmp[k]);
       bo[(size_t)b + 1] = (int32_t)bl.size();
+    }
+    // Which blocks to park: a feedback vertex set F of the blocker graph (without F the graph has no cycle, so
+    // parking only blocks of F always suffices).  Greedy: blocks that block themselves; then, as long as
+    // pruning the blocks with no blocker or nothing blocked left among the rest does not empty it, the block
+    // with the most (blockers x blocked).  For aliased views of a power-of-two shape the graph is the de
+    // Bruijn graph on R-ary words of length 3 (block (q, a, b) is blocked by (j, q, a) for every j) and this
+    // finds its minimum, the 176 necklaces of 512 words; taking the blockers of whichever block needs the
+    // fewest parks, as round 2's first version did, parks 260-324.
+    std::vector<uint8_t> inF((size_t)NB, 0);
+    {
+      std::vector<int32_t> so((size_t)NB + 1, 0), sl_;
+      for (int b = 0; b < NB; ++b) for (int32_t e = bo[(size_t)b]; e < bo[(size_t)b + 1]; ++e) so[(size_t)bl[(size_t)e] + 1]++;
+      for (int b = 0; b < NB; ++b) so[(size_t)b + 1] += so[(size_t)b];
+      sl_.resize((size_t)so[(size_t)NB]);
+      { std::vector<int32_t> pos(so.begin(), so.end() - 1);
+        for (int b = 0; b < NB; ++b) for (int32_t e = bo[(size_t)b]; e < bo[(size_t)b + 1]; ++e) sl_[(size_t)pos[(size_t)bl[(size_t)e]]++] = b; }
+      std::vector<uint8_t> alive((size_t)NB, 1);
+      std::vector<int32_t> nin((size_t)NB, 0), nout((size_t)NB, 0);
+      for (int b = 0; b < NB; ++b) if (self[(size_t)b]) { inF[(size_t)b] = 1; alive[(size_t)b] = 0; }
+      for (int b = 0; b < NB; ++b) if (alive[(size_t)b]) {
+        for (int32_t e = bo[(size_t)b]; e < bo[(size_t)b + 1]; ++e) nin[(size_t)b] += alive[(size_t)bl[(size_t)e]];
+        for (int32_t e = so[(size_t)b]; e < so[(size_t)b + 1]; ++e) nout[(size_t)b] += alive[(size_t)sl_[(size_t)e]];
+      }
+      std::vector<int32_t> stack;
+      auto kill = [&](int b) {           // b leaves the graph; neighbours that lose their last edge follow
+        alive[(size_t)b] = 0;
+        for (int32_t e = bo[(size_t)b]; e < bo[(size_t)b + 1]; ++e) { const int a = bl[(size_t)e]; if (alive[(size_t)a] && --nout[(size_t)a] == 0) stack.push_back(a); }
+        for (int32_t e = so[(size_t)b]; e < so[(size_t)b + 1]; ++e) { const int a = sl_[(size_t)e]; if (alive[(size_t)a] && --nin[(size_t)a] == 0) stack.push_back(a); }
+      };
+      auto prune = [&]() {
+        while (!stack.empty()) { const int b = stack.back(); stack.pop_back(); if (alive[(size_t)b]) kill(b); }
+      };
+      for (int b = 0; b < NB; ++b) if (alive[(size_t)b] && (nin[(size_t)b] == 0 || nout[(size_t)b] == 0)) stack.push_back(b);
+      prune();
+      for (;;) {
+        int best = -1; int64_t best_w = -1;
+        for (int b = 0; b < NB; ++b) if (alive[(size_t)b]) {
+          const int64_t wgt = (int64_t)nin[(size_t)b] * nout[(size_t)b];
+          if (wgt > best_w) { best_w = wgt; best = b; }
+        }
+        if (best < 0) break;
+        inF[(size_t)best] = 1;
+        kill(best);
+        prune();
+      }
     }
     // greedy wave simulation
     typedef S2Op Op;
@@ -923,13 +986,22 @@ struct PlanBuilder {
         // One stall opens several blocks at once (s2_batch parks per wave at most): fewer, fatter waves.
         int parks = 0;
         do {
-          int best = -1, best_need = INT32_MAX;
+          // the block that needs the fewest parks among those whose unread blockers all belong to F (there is
+          // always one while something is left: without F the graph is acyclic); any block as a last resort
+          int best = -1, best_need = INT32_MAX, any = -1, any_need = INT32_MAX;
           for (int b = 0; b < NB; ++b) {
             if (done[(size_t)b]) continue;
             int need = (self[(size_t)b] && slot_of[(size_t)b] < 0) ? 1 : 0;
-            for (int32_t e = bo[(size_t)b]; e < bo[(size_t)b + 1]; ++e) need += read_wave[(size_t)bl[(size_t)e]] == INT32_MAX;
-            if (need > 0 && need < best_need) { best = b; best_need = need; }
+            bool in_f = true;
+            for (int32_t e = bo[(size_t)b]; e < bo[(size_t)b + 1]; ++e) {
+              const int a = bl[(size_t)e];
+              if (read_wave[(size_t)a] == INT32_MAX) { ++need; in_f = in_f && inF[(size_t)a]; }
+            }
+            if (need <= 0) continue;
+            if (in_f && need < best_need) { best = b; best_need = need; }
+            if (need < any_need) { any = b; any_need = need; }
           }
+          if (best < 0 && parks == 0) { best = any; best_need = any_need; }
           if (best < 0) break;
           if (best_need > (int)free_slots.size()) {
             if (parks == 0) return MOEBIUS_E_STAGING;
@@ -947,6 +1019,7 @@ struct PlanBuilder {
       waves.push_back(std::move(ops));
     }
     P->stats.n_w_parked += n_parked;
+    s2_cache.push_back({run, rt, T, sS, nb, n_slots, peak, n_parked, P->stats.w_staged_bytes - staged_before, waves});
     sc.tmpl = tmpl; sc.lsu = lsu; sc.xt = xt;
     sc.T = T; sc.rt = rt; sc.Rr = Rr; sc.run = run; sc.slot_bytes = slot_bytes; sc.nb = nb; sc.first_slot = 0; sc.peak_slots = peak;
     return MOEBIUS_OK;
@@ -1059,17 +1132,34 @@ struct PlanBuilder {
         end = e;
         ++n;
       }
+      // Inside a group every object runs its own chain of waves (its own counters): the segments are laid
+      // out wave by wave across the objects, so by the time a pipe reaches wave w+1 of an object the other
+      // objects' wave-w units have been handed out in between and its wave w is long complete -- no
+      // device-wide drain per wave.  Only the groups are separated: the last wave of every object signals
+      // the group's counter, and the next group, which reuses the staging area, waits for all of it.
       size_t n_waves = 0;
       for (size_t k = 0; k < n; ++k) n_waves = std::max(n_waves, sc[o0 + k].waves.size());
       P->stats.n_w_waves += (int32_t)n_waves;
-      for (size_t w = 0; w < n_waves; ++w) {
-        if (next_ctr >= (uint32_t)kMaxCounters) return MOEBIUS_E_STAGING;
-        const int ctr = (int)next_ctr++;
-        uint32_t units = 0;
-        for (size_t k = 0; k < n; ++k)
-          if (w < sc[o0 + k].waves.size()) units += s2_emit_wave(sc[o0 + k], w, prev_ctr, prev_units, ctr);
-        prev_ctr = ctr; prev_units = units;
-      }
+      if (next_ctr >= (uint32_t)kMaxCounters) return MOEBIUS_E_STAGING;
+      const int group_ctr = (int)next_ctr++;
+      uint32_t group_units = 0;
+      std::vector<int> o_ctr(n, prev_ctr);
+      std::vector<uint32_t> o_units(n, prev_units);
+      for (size_t w = 0; w < n_waves; ++w)
+        for (size_t k = 0; k < n; ++k) {
+          const S2Sched& c = sc[o0 + k];
+          if (w >= c.waves.size()) continue;
+          const bool last = w + 1 == c.waves.size();
+          int ctr = group_ctr;
+          if (!last) {
+            if (next_ctr >= (uint32_t)kMaxCounters) return MOEBIUS_E_STAGING;
+            ctr = (int)next_ctr++;
+          }
+          const uint32_t units = s2_emit_wave(c, w, o_ctr[k], o_units[k], ctr);
+          if (last) group_units += units;
+          o_ctr[k] = ctr; o_units[k] = units;
+        }
+      prev_ctr = group_ctr; prev_units = group_units;
       o0 += n;
     }
     return MOEBIUS_OK;

@@ -239,11 +239,11 @@ struct BulkUnit {
   int64_t src_stride, dst_stride;
   uint32_t nrows, piece;     // piece = bytes per row handled by this unit
 };
-MB_HD void decode_bulk(const Seg& s, const DevParams& p, uint32_t u, BulkUnit& b) {
+MB_HD void decode_bulk(const Seg& s, const DevParams& p, uint32_t u, BulkUnit& b, bool has_pre = false, BulkDesc pre = BulkDesc{0, 0}) {
   const uint32_t per_desc = s.row_blocks * s.chunks_per_run;
   const uint32_t di = u / per_desc, w = u - di * per_desc;
   const uint32_t rb = w / s.chunks_per_run, ch = w - rb * s.chunks_per_run;
-  const BulkDesc d = p.bulk[s.desc_begin + di];
+  const BulkDesc d = has_pre ? pre : p.bulk[s.desc_begin + di];
   const uint32_t row0 = rb * s.rows_per_unit;
   uint32_t nrows = s.rows_total - row0;
   if (nrows > s.rows_per_unit) nrows = s.rows_per_unit;
@@ -258,7 +258,9 @@ MB_HD void decode_bulk(const Seg& s, const DevParams& p, uint32_t u, BulkUnit& b
 }
 
 // Decode box k of unit u (u is LOCAL to the segment).
-MB_HD void decode_box(const Seg& s, const DevParams& p, uint32_t u, uint32_t k, Box& b) {
+// `pre`: the unit's WBlk descriptor if the caller has fetched it already (block lists: the TMA pipes prefetch
+// it with the ticket, so that no dependent global load sits between a ticket and its first TMA operation).
+MB_HD void decode_box(const Seg& s, const DevParams& p, uint32_t u, uint32_t k, Box& b, bool has_pre = false, WBlk pre = WBlk{0, 0, 0, 0}) {
   b.lin = 0;
   b.run_bytes = s.run_bytes;
   b.rep = s.rep;
@@ -272,7 +274,7 @@ MB_HD void decode_box(const Seg& s, const DevParams& p, uint32_t u, uint32_t k, 
       if (s.stg_pools) {                  // regular: computed, no descriptor
         q = s.stg_pool_begin + di; blk_row0 = s.pool_begin; row_end = s.pool_begin + s.n_pools;
       } else {
-        const WBlk k = p.wblk[s.pool_begin + di];
+        const WBlk k = has_pre ? pre : p.wblk[s.pool_begin + di];
         q = k.q; blk_row0 = k.row0; row_end = k.row0 + k.nrows; slot = k.slot;
       }
     } else {
