@@ -478,6 +478,44 @@ def test_s2_in_place_path(name, first):
     sess.close()
 
 
+def necklaces(k, n):
+    """Number of necklaces of length n over k symbols = size of a minimum feedback vertex set of the de
+    Bruijn graph B(k, n) (Mykkeltveit 1972): (1/n) * sum over d | n of phi(d) * k^(n/d)."""
+    phi = lambda d: sum(1 for a in range(1, d + 1) if np.gcd(a, d) == 1)   # noqa: E731
+    return sum(phi(d) * k ** (n // d) for d in range(1, n + 1) if n % d == 0) // n
+
+
+@pytest.mark.parametrize("name,R,words", [("qwen3_235b", 8, 3), ("qwen3_30b", 8, 3), ("small", 4, 4)])
+def test_aliased_views_park_a_minimum_feedback_vertex_set(name, R, words):
+    """Aliased views of a power-of-two shape cut into 64 blocks per rank: block (q, i) is blocked by the blocks
+    at position (q*64 + i) div R of every rank -- the de Bruijn graph on R-ary words (q, digits of i).  What
+    the planner parks per gate/up object is a feedback vertex set of it, and its greedy finds the minimum,
+    the necklace count (176 of 512 at R = 8; 70 of 256 at R = 4), where taking the blockers of whichever block
+    needs the fewest parks parked 260-324.  Host only: the plan's statistics."""
+    cfg = wl.get_config(name).with_(w_inplace=1, n_req=0)
+    assert cfg.R == R and R ** words == R * 64
+    lens = np.zeros(0, np.int32)
+    c = mb_config(cfg, wl.draw_seq_lens(wl.get_config(name)))
+    c.max_requests = 1
+    probe = mb.Session(c)
+    c.staging_cap_bytes = int(0.024 * probe.layout.resident_bytes)
+    probe.close()
+    sess = mb.Session(c)
+    per_down = None
+    for to, frm in ((EP, TP), (TP, EP)):
+        plan = sess.plan(to, lens, None if to == EP else np.zeros(0, np.int32), np.zeros((0, 1), np.int32), from_mode=frm)
+        st = mb.moebius_plan_stats(plan).as_dict()
+        sess.free_plan(plan)
+        short = 2 * cfg.L * necklaces(R, words)              # gate and up of every layer
+        down = st["n_w_parked"] - short                       # the long-run objects have fewer, larger blocks
+        assert down > 0 and down % cfg.L == 0 and down // cfg.L < necklaces(R, words), (st["n_w_parked"], short)
+        per_down = per_down or down
+        assert down == per_down                               # the same both ways
+        # parked bytes (every parked block moves twice): 34-41 % of the weights, not 53-63 %
+        assert st["w_staged_bytes"] < 0.45 * st["w_relocated"]
+    sess.close()
+
+
 def test_s2_is_chosen_by_the_cap_and_refuses_only_what_cannot_fit():
     """The planner picks the shift from staging_cap_bytes: S1 (every move out of place) when a spare of
     the largest object fits, else fewer slots plus the in-place path; E_STAGING only when not even the
