@@ -308,6 +308,24 @@ MOEBIUS_API int moebius_naive_scratch_bytes(const moebius_ctx_t* ctx, const moeb
 MOEBIUS_API int moebius_reshard_naive(moebius_ctx_t* ctx, const moebius_plan_t* plan, void* dev_scratch,
                                       int64_t scratch_bytes, void* cuda_stream, int64_t* stats6);
 
+/* The same staged path for callers that cannot allocate device memory where they stand (code under CUDA graph
+ * capture, tight serving loops, harnesses that forbid cudaMalloc): its staging buffer is a file-scope static
+ * device array of MOEBIUS_STATIC_SCRATCH_BYTES inside the library -- every GPU that loads the library holds
+ * those bytes until the process exits -- so the call allocates NO device memory: no cudaMalloc, no cudaFree,
+ * no allocating CUDA library routine (on the host it builds its descriptor lists like moebius_reshard_naive).
+ * Same plan, same kernels, same result bit for bit as moebius_reshard_naive and moebius_reshard.
+ *   Limit: a plan with moebius_naive_scratch_bytes(ctx, plan) > MOEBIUS_STATIC_SCRATCH_BYTES is refused with
+ *   MOEBIUS_E_STAGING ("staging buffer too small") before anything is enqueued; use moebius_reshard_naive
+ *   with a caller-owned buffer for those.  moebius_static_scratch_bytes() returns the limit (host only).
+ *   Sharing: every call on a device uses the one array, which keeps the previous call's bytes.  Nothing in
+ *   it has to start at zero (each launch reads only what an earlier launch of the same call wrote), so
+ *   nothing is cleared.  Calls that OVERLAP on the GPU -- two streams, two contexts on one device -- race on
+ *   the array: serialise them.  stats6 as for moebius_reshard_naive. */
+#define MOEBIUS_STATIC_SCRATCH_BYTES (64 * 1024 * 1024)
+MOEBIUS_API int64_t moebius_static_scratch_bytes(void);
+MOEBIUS_API int moebius_reshard_naive_static(moebius_ctx_t* ctx, const moebius_plan_t* plan, void* cuda_stream,
+                                             int64_t* stats6);
+
 /* Kernel-only device time of the last moebius_reshard, in ms (CUDA events on its stream; the call
  * synchronises on the end event).  Enabled with moebius_set_timing(ctx, 1). */
 MOEBIUS_API int moebius_set_timing(moebius_ctx_t* ctx, int enable);

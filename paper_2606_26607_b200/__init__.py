@@ -16,7 +16,8 @@ from ._binding import (  # noqa: F401
     moebius_policy_config_t, moebius_policy_preset, moebius_policy_config, moebius_policy_create, moebius_policy_destroy,
     moebius_policy_mode, moebius_policy_step, moebius_capacity_check, moebius_policy_calibrate,
     POLICY_INTERACTIVE, POLICY_ROLLOUT, DECISION_STAY, DECISION_SWITCH, DECISION_CANCELLED,
-    moebius_naive_scratch_bytes, moebius_reshard_naive, moebius_reshard_shares,
+    moebius_naive_scratch_bytes, moebius_reshard_naive, moebius_static_scratch_bytes, moebius_reshard_naive_static,
+    moebius_reshard_shares,
     moebius_share_stats, moebius_plan_waves, moebius_reshard_share, moebius_reshard_publish,
     moebius_arena_create, moebius_arena_destroy, moebius_arena_base, moebius_arena_ready, moebius_arena_export,
     moebius_arena_import,

@@ -20,7 +20,8 @@ EXPORTED_SYMBOLS = [
     "moebius_create", "moebius_destroy", "moebius_layout", "moebius_view", "moebius_bind",
     "moebius_active_mode", "moebius_plan", "moebius_plan_destroy", "moebius_block_tables",
     "moebius_plan_stats", "moebius_plan_export", "moebius_reshard", "moebius_stage_plan", "moebius_reshard_staged",
-    "moebius_naive_scratch_bytes", "moebius_reshard_naive", "moebius_reshard_shares",
+    "moebius_naive_scratch_bytes", "moebius_reshard_naive", "moebius_static_scratch_bytes", "moebius_reshard_naive_static",
+    "moebius_reshard_shares",
     "moebius_share_stats", "moebius_plan_waves", "moebius_reshard_share", "moebius_reshard_publish",
     "moebius_arena_create", "moebius_arena_destroy", "moebius_arena_base", "moebius_arena_ready",
     "moebius_arena_export", "moebius_arena_import",
@@ -294,6 +295,22 @@ def moebius_reshard_shares(ctx, plan, rank_bounds, share_first: int, share_count
 
 _lib.moebius_naive_scratch_bytes.argtypes = [_vp, _vp, C.POINTER(C.c_int64)]
 _lib.moebius_reshard_naive.argtypes = [_vp, _vp, _vp, C.c_int64, _vp, C.POINTER(C.c_int64)]
+
+
+_lib.moebius_static_scratch_bytes.restype = C.c_int64
+_lib.moebius_reshard_naive_static.argtypes = [_vp, _vp, _vp, C.POINTER(C.c_int64)]
+
+
+def moebius_static_scratch_bytes() -> int:
+    return int(_lib.moebius_static_scratch_bytes())
+
+
+def moebius_reshard_naive_static(ctx, plan, cuda_stream: int = 0) -> dict:
+    """moebius_reshard_naive with the library's static device scratch: allocates no device memory."""
+    st = (C.c_int64 * 6)()
+    _chk(_lib.moebius_reshard_naive_static(ctx, plan, _vp(cuda_stream or None), st), "moebius_reshard_naive_static")
+    return {"launches": st[0], "bytes_read": st[1], "bytes_written": st[2], "w_pass_bytes": st[3],
+            "kv_pass_bytes": st[4], "scratch_bytes": st[5]}
 
 
 def moebius_naive_scratch_bytes(ctx, plan) -> int:

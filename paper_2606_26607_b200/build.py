@@ -8,7 +8,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libmoebius.so")
-SOURCES = ["moebius_plan.cpp", "moebius_policy.cpp", "moebius_cuda.cu", "moebius_arena.cu", "moebius_naive.cu"]
+SOURCES = ["moebius_plan.cpp", "moebius_policy.cpp", "moebius_cuda.cu", "moebius_arena.cu", "moebius_naive.cu", "moebius_static.cu"]
 HEADERS = ["moebius_units.h", "moebius_host.h", os.path.join("..", "..", "include", "moebius.h")]
 
 
